@@ -1,0 +1,161 @@
+/*
+ * wcsim.h -- C ABI of libwcsim: the data-parallel hot path of the Wire-Cell LArTPC signal
+ * simulation on one wire plane, hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ *     M(t,x) = sum_{t',x'} R(t-t', x-x') S(t',x') + N(t,x)          PAPER.md:38-40, Section 2.1, Eq. (1)
+ *
+ * S is built from "ionization electron groups" (depos) by the Raster and Scatter-add tasks of
+ * PAPER.md:54-58 (Section 2.2); the convolution follows the FFT route of PAPER.md:46-52 (Eq. 2);
+ * N is the optional electronics-noise term of Eq. (1), model from BASELINE.json configs[3].
+ * Where the paper is silent the readings A1..A20 of DESIGN.md apply; each call names the ones it uses.
+ *
+ * Conventions
+ *   - Grids are wire-major, tick fastest: S[wire * n_ticks + tick], fp32.  Bin k covers [k, k+1) on both axes (A1).
+ *   - Every pointer says HOST or DEVICE.  Device pointers must belong to the device that was current at
+ *     wcsim_plan_create.  The library never takes ownership of a caller's buffer.
+ *   - All work is enqueued on the plan's CUDA stream (the `cuda_stream` given at creation; 0/NULL = the legacy
+ *     default stream) and returns without waiting, except wcsim_plan_create (synchronises once), wcsim_sync,
+ *     wcsim_plan_destroy and the *_host convenience calls (they synchronise before returning).
+ *   - Return value: WCSIM_OK (0) or a negative wcsim_status.  Nothing throws or aborts across this boundary.
+ *     Asynchronous CUDA faults surface at the next synchronising call as WCSIM_ECUDA.
+ *   - There is no CPU fallback: without a CUDA device every call that needs one returns WCSIM_ECUDA.
+ */
+#ifndef WCSIM_H
+#define WCSIM_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum wcsim_status {
+    WCSIM_OK = 0,
+    WCSIM_EINVAL = -1, /* NULL pointer, non-positive size, even n_rwires, bad padding, nsigma <= 0, unknown mode */
+    WCSIM_ENOMEM = -2, /* host or device allocation failed */
+    WCSIM_ECUDA = -3,  /* a CUDA runtime call or kernel failed; wcsim_last_cuda_error() gives the cudaError_t */
+    WCSIM_ESTATE = -4  /* call not valid in the plan's current state */
+} wcsim_status;
+
+/* scatter_mode of wcsim_plan_create */
+#define WCSIM_SCATTER_ATOMIC 0 /* fp32 red.global adds straight into S; order of equal-address adds is not fixed */
+#define WCSIM_SCATTER_TILED 1  /* depos are binned by grid tile, each tile is accumulated in shared memory in
+                                  integer / fixed-point arithmetic (order independent => bitwise reproducible)
+                                  and stored once; "deterministic sort-by-tile mode" of BASELINE.json north_star */
+
+typedef struct wcsim_plan wcsim_plan; /* opaque; owns S, M, the spectra, the response spectrum, twiddles, tile lists */
+
+/* FFT padding.  0 on an axis = automatic: the next power of two >= n_ticks + n_rticks - 1 (ticks) and
+ * >= n_wires + (n_rwires-1)/2 (wires) (A13).  Explicit values must be powers of two that satisfy those bounds,
+ * with ticks >= 32 and wires >= 16. */
+typedef struct wcsim_pad {
+    int wires;
+    int ticks;
+} wcsim_pad;
+
+/* Depositions as a structure of arrays ("structures/objects of arrays").  DEVICE pointers,
+ * n elements each, caller-owned, must stay valid until the enqueued work has run. */
+typedef struct wcsim_depos {
+    const float *t0;      /* centre on the drift-time axis, in ticks */
+    const float *x0;      /* centre on the wire-pitch axis, in pitches */
+    const float *sigma_t; /* Gaussian width in ticks, >= 0 */
+    const float *sigma_x; /* Gaussian width in pitches, >= 0 */
+    const float *q;       /* charge in electrons (sign is carried) */
+} wcsim_depos;
+
+/* Counters kept on the device, copied out by wcsim_get_stats (which synchronises). */
+typedef struct wcsim_stats {
+    unsigned long long depos_skipped; /* depos with a non-finite field or a negative sigma: skipped, not rastered */
+    unsigned long long bins_drawn;    /* patch bins inside the grid that were deposited (or drawn) */
+} wcsim_stats;
+
+/*
+ * p0 Plan ("the similarly transformed 2D detector response array R(omega_t, omega_x)").
+ *   response : HOST, n_rwires x n_rticks floats, tick fastest.  Row (n_rwires-1)/2 is wire offset dx = 0 (A11),
+ *              column dt = 0..n_rticks-1 is causal in time.  Copied; the caller may free it on return.
+ *   n_rwires : odd.
+ *   nsigma   : patch half-width in sigmas (A2), > 0; all BASELINE.json configs use 3.
+ * Embeds R in the padded grid (wrap-around on the wire axis), transforms it in fp64 by the definition of the DFT,
+ * folds the 1/(pad.wires*pad.ticks) of the inverse transform in (A14) and keeps it as fp32.  S and M start at zero.
+ * On failure *out is NULL.
+ */
+int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *response, int n_rwires, int n_rticks,
+                      wcsim_pad pad, float nsigma, int scatter_mode, void *cuda_stream);
+
+/*
+ * a1-a3 Raster + fluctuation + scatter-add (PAPER.md:82 for the binomial fluctuation).
+ * For every depo d (id = depo_id_base + d): extent floor(c - nsigma s) .. floor(c + nsigma s) on each axis (A2),
+ * per-axis bin weights 1/2 [erf((i+1-c)/(sqrt2 s)) - erf((i-c)/(sqrt2 s))] (sigma < 1e-6: all weight in bin
+ * floor(c), A4), patch p_ij = wt_i wx_j with no renormalisation (A3).
+ *   fluctuate = 0 : S[j][i] += q p_ij                         (weights in fp32)
+ *   fluctuate = 1 : S[j][i] += sign(q) B(floor(|q|+1/2), p_ij; w)   (weights, p and the sampler in fp64; A6, A7)
+ *                   with w the Philox4x32-10 word keyed (seed, id, absolute grid bin j*n_ticks+i) (A8).
+ * Bins outside the grid are dropped and not drawn (A5).  S accumulates across calls; wcsim_clear zeroes it.
+ *   depos           : struct of DEVICE pointers (the struct itself is read on the host during the call).
+ *   dev_depo_totals : DEVICE, n int32, or NULL.  With fluctuate = 1 receives the signed sum of each depo's draws.
+ * n = 0 is valid and does nothing.
+ */
+int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n, unsigned long long depo_id_base,
+                         unsigned long long seed, int fluctuate, int *dev_depo_totals);
+
+/*
+ * a4-a6 Convolution by Eq. (2): M = crop(irfft2(Rhat * rfft2(zero_pad(S)))).  S is preserved.
+ * Equals the linear convolution of Eq. (1) on the n_wires x n_ticks window exactly, up to fp32 rounding (A10-A13).
+ * If noise was armed with wcsim_arm_noise, it is added inside the last transform and the arm is cleared.
+ */
+int wcsim_convolve(wcsim_plan *plan);
+
+/*
+ * a7 Noise (Eq. (1)'s N(t,x); model of BASELINE.json configs[3]; A15-A17): per wire x, on the padded
+ * tick length P, k = 0..P/2: Z_k = amp[k] exp(2 pi i u(seed, x, k)), u from Philox4x32-10;
+ * N[x][t] = P^-1/2 [Re Z_0 + 2 sum_{0<k<P/2} Re(Z_k e^{2 pi i k t / P}) + Re Z_{P/2} (-1)^t];  M += N for t < n_ticks.
+ *   amp : HOST, P/2+1 floats, or NULL for the built-in A(f) = 3 (f/f0) exp(-f/f0), f0 = 0.1 f_Nyquist.
+ * wcsim_add_noise runs now, as its own pass over M.  wcsim_arm_noise defers it into the next wcsim_convolve,
+ * where it costs no extra pass over M; both give the same M up to fp32 rounding.
+ */
+int wcsim_add_noise(wcsim_plan *plan, const float *amp, unsigned long long seed);
+int wcsim_arm_noise(wcsim_plan *plan, const float *amp, unsigned long long seed);
+
+/* Waits for the plan's stream, frees everything the plan owns.  NULL is accepted. */
+int wcsim_plan_destroy(wcsim_plan *plan);
+
+/* ---- accessories ---- */
+int wcsim_clear(wcsim_plan *plan);       /* S = 0 (enqueued) */
+int wcsim_clear_output(wcsim_plan *plan); /* M = 0 (enqueued) */
+int wcsim_sync(wcsim_plan *plan);        /* waits for the plan's stream; returns the first deferred CUDA fault */
+int wcsim_set_scatter_mode(wcsim_plan *plan, int scatter_mode);
+/* borrowed DEVICE pointers to n_wires*n_ticks floats, valid until wcsim_plan_destroy */
+int wcsim_charge_ptr(wcsim_plan *plan, float **dev);
+int wcsim_output_ptr(wcsim_plan *plan, float **dev);
+int wcsim_get_dims(const wcsim_plan *plan, int *n_wires, int *n_ticks, int *pad_wires, int *pad_ticks);
+int wcsim_get_stats(wcsim_plan *plan, wcsim_stats *out); /* synchronises */
+int wcsim_reset_stats(wcsim_plan *plan);
+
+/*
+ * End-to-end convenience with HOST buffers (what bench.py's `e2e` times): copies the five depo arrays
+ * host->device, clears S, rasters+scatters, convolves (with noise if noise_seed_or_0 != 0 ... see `noise`),
+ * copies M device->host, synchronises.
+ *   host_* : HOST, n floats each (pinned memory makes the copies asynchronous)
+ *   host_M : HOST, n_wires*n_ticks floats, written
+ *   noise  : 0 = none, 1 = built-in amplitude spectrum with `noise_seed`
+ */
+int wcsim_simulate_host(wcsim_plan *plan, const float *host_t0, const float *host_x0, const float *host_sigma_t,
+                        const float *host_sigma_x, const float *host_q, long long n, unsigned long long seed,
+                        int fluctuate, int noise, unsigned long long noise_seed, float *host_M);
+
+/* Test/diagnostic hooks: exact pieces of the path, exposed so that parity can be checked piecewise. */
+/* out[4] (DEVICE, 4*n uint32) = Philox4x32-10(ctr = dev_ctr[4*i..], key = dev_key[2*i..]) for i < n */
+int wcsim_debug_philox(const unsigned int *dev_ctr, const unsigned int *dev_key, unsigned int *dev_out, long long n,
+                       void *cuda_stream);
+/* dev_k[i] = B(dev_N[i], dev_p[i]; dev_w[i]) -- the device binomial sampler (fp64 in, fp64 integer-valued out) */
+int wcsim_debug_binomial(const double *dev_N, const double *dev_p, const unsigned int *dev_w, double *dev_k,
+                         long long n, void *cuda_stream);
+/* copy the response spectrum Rhat[kx][kt] (kx < pad_wires, kt <= pad_ticks/2) to HOST as interleaved re,im floats */
+int wcsim_debug_response_spectrum(wcsim_plan *plan, float *host_out);
+
+const char *wcsim_strerror(int status);
+int wcsim_last_cuda_error(void); /* cudaError_t of the most recent WCSIM_ECUDA on this thread, else 0 */
+const char *wcsim_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WCSIM_H */
