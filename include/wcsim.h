@@ -130,6 +130,22 @@ int wcsim_get_stats(wcsim_plan *plan, wcsim_stats *out); /* synchronises */
 int wcsim_reset_stats(wcsim_plan *plan);
 
 /*
+ * Stage timing (what bench.py's per-stage numbers and `roofline` come from).  While enabled, every call records a
+ * CUDA event pair on the plan's stream around each stage it enqueues; wcsim_get_stage_times synchronises, adds the
+ * finished spans up and returns, per stage, the total milliseconds and the number of spans (arrays of WCSIM_N_STAGES).
+ */
+#define WCSIM_STAGE_RASTER 0       /* a1-a3: the whole wcsim_raster_scatter call */
+#define WCSIM_STAGE_ROWS_FORWARD 1 /* a4, tick axis */
+#define WCSIM_STAGE_COLS 2         /* a4 wire axis + a5 multiply + a6 wire axis */
+#define WCSIM_STAGE_ROWS_INVERSE 3 /* a6 tick axis (+ armed noise) */
+#define WCSIM_STAGE_NOISE 4        /* a7 as its own pass (wcsim_add_noise) */
+#define WCSIM_N_STAGES 5
+int wcsim_set_profiling(wcsim_plan *plan, int enable);
+int wcsim_get_stage_times(wcsim_plan *plan, double *ms, unsigned long long *calls, int reset);
+/* number of kernels of this library enqueued through `plan` so far (memsets and copies are not counted) */
+int wcsim_get_launch_count(const wcsim_plan *plan, unsigned long long *out);
+
+/*
  * End-to-end convenience with HOST buffers (what bench.py's `e2e` times): copies the five depo arrays
  * host->device, clears S, rasters+scatters, convolves (with noise if noise_seed_or_0 != 0 ... see `noise`),
  * copies M device->host, synchronises.

@@ -1,0 +1,368 @@
+"""Thin ctypes binding of libwcsim.so (include/wcsim.h): argument marshalling only.
+
+Every function has the name and the argument order of the C call it wraps; device arrays are torch CUDA tensors
+(torch supplies device memory and the stream, nothing else) and are passed down as raw pointers.  There is no CPU
+fallback: if the library cannot be loaded the import of this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+WCSIM_OK, WCSIM_EINVAL, WCSIM_ENOMEM, WCSIM_ECUDA, WCSIM_ESTATE = 0, -1, -2, -3, -4
+WCSIM_SCATTER_ATOMIC, WCSIM_SCATTER_TILED = 0, 1
+
+# every symbol include/wcsim.h declares (tests check that the library exports all of them)
+SYMBOLS = [
+    "wcsim_plan_create", "wcsim_raster_scatter", "wcsim_convolve", "wcsim_add_noise", "wcsim_arm_noise",
+    "wcsim_plan_destroy", "wcsim_clear", "wcsim_clear_output", "wcsim_sync", "wcsim_set_scatter_mode",
+    "wcsim_charge_ptr", "wcsim_output_ptr", "wcsim_get_dims", "wcsim_get_stats", "wcsim_reset_stats",
+    "wcsim_simulate_host", "wcsim_set_profiling", "wcsim_get_stage_times", "wcsim_get_launch_count",
+    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum",
+    "wcsim_strerror", "wcsim_last_cuda_error", "wcsim_version",
+]
+
+
+class wcsim_pad(C.Structure):
+    _fields_ = [("wires", C.c_int), ("ticks", C.c_int)]
+
+
+class wcsim_depos(C.Structure):
+    _fields_ = [(k, C.c_void_p) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")]
+
+
+class wcsim_stats(C.Structure):
+    _fields_ = [("depos_skipped", C.c_ulonglong), ("bins_drawn", C.c_ulonglong)]
+
+
+class WcsimError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        msg = lib().wcsim_strerror(status).decode()
+        if status == WCSIM_ECUDA:
+            msg += " [cudaError_t %d]" % lib().wcsim_last_cuda_error()
+        super().__init__("%s: %s (%d)" % (where, msg, status))
+
+
+_lib = None
+
+
+def lib():
+    """The loaded libwcsim.so (built in-tree with nvcc on first use).  Raises if it cannot be had."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        vp, ll, ull, i = C.c_void_p, C.c_longlong, C.c_ulonglong, C.c_int
+        L.wcsim_plan_create.argtypes = [C.POINTER(vp), i, i, vp, i, i, wcsim_pad, C.c_float, i, vp]
+        L.wcsim_raster_scatter.argtypes = [vp, C.POINTER(wcsim_depos), ll, ull, ull, i, vp]
+        L.wcsim_convolve.argtypes = [vp]
+        L.wcsim_add_noise.argtypes = [vp, vp, ull]
+        L.wcsim_arm_noise.argtypes = [vp, vp, ull]
+        L.wcsim_plan_destroy.argtypes = [vp]
+        L.wcsim_clear.argtypes = [vp]
+        L.wcsim_clear_output.argtypes = [vp]
+        L.wcsim_sync.argtypes = [vp]
+        L.wcsim_set_scatter_mode.argtypes = [vp, i]
+        L.wcsim_charge_ptr.argtypes = [vp, C.POINTER(vp)]
+        L.wcsim_output_ptr.argtypes = [vp, C.POINTER(vp)]
+        L.wcsim_get_dims.argtypes = [vp] + [C.POINTER(i)] * 4
+        L.wcsim_get_stats.argtypes = [vp, C.POINTER(wcsim_stats)]
+        L.wcsim_reset_stats.argtypes = [vp]
+        L.wcsim_simulate_host.argtypes = [vp, vp, vp, vp, vp, vp, ll, ull, i, i, ull, vp]
+        L.wcsim_set_profiling.argtypes = [vp, i]
+        L.wcsim_get_stage_times.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(ull), i]
+        L.wcsim_get_launch_count.argtypes = [vp, C.POINTER(ull)]
+        L.wcsim_debug_philox.argtypes = [vp, vp, vp, ll, vp]
+        L.wcsim_debug_binomial.argtypes = [vp, vp, vp, vp, ll, vp]
+        L.wcsim_debug_response_spectrum.argtypes = [vp, vp]
+        L.wcsim_strerror.argtypes = [i]
+        L.wcsim_strerror.restype = C.c_char_p
+        L.wcsim_last_cuda_error.argtypes = []
+        L.wcsim_version.argtypes = []
+        L.wcsim_version.restype = C.c_char_p
+        for name in SYMBOLS:
+            fn = getattr(L, name)
+            if fn.restype is not C.c_char_p:
+                fn.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(status, where):
+    if status != WCSIM_OK:
+        raise WcsimError(status, where)
+
+
+def _dev_ptr(t, dtype=None):
+    """Raw device pointer of a contiguous torch CUDA tensor (None -> NULL)."""
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError("expected dtype %s, got %s" % (dtype, t.dtype))
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+class _Borrowed:
+    """A device buffer owned by a plan, exposed through __cuda_array_interface__ so torch can view it without a copy."""
+
+    def __init__(self, ptr, shape, owner):
+        self._owner = owner
+        self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": "<f4", "data": (int(ptr), False),
+                                         "version": 2, "strides": None}
+
+
+# ---- the C calls, one to one ------------------------------------------------------------------------------------
+def wcsim_plan_create(n_wires, n_ticks, response, pad=(0, 0), nsigma=3.0, scatter_mode=WCSIM_SCATTER_ATOMIC,
+                      stream=None):
+    """response: host numpy array [n_rwires][n_rticks] float32.  Returns the opaque plan handle."""
+    r = np.ascontiguousarray(response, dtype=np.float32)
+    if r.ndim != 2:
+        raise ValueError("response must be 2-D [n_rwires][n_rticks]")
+    h = C.c_void_p()
+    st = lib().wcsim_plan_create(C.byref(h), int(n_wires), int(n_ticks), r.ctypes.data_as(C.c_void_p), r.shape[0],
+                                 r.shape[1], wcsim_pad(int(pad[0]), int(pad[1])), float(nsigma), int(scatter_mode),
+                                 _stream_ptr(stream))
+    _check(st, "wcsim_plan_create")
+    return h
+
+
+def wcsim_raster_scatter(plan, depos, n=None, depo_id_base=0, seed=0, fluctuate=False, dev_depo_totals=None):
+    """depos: dict (or object) of torch CUDA float32 tensors t0, x0, sigma_t, sigma_x, q."""
+    import torch
+    get = (lambda k: depos[k]) if isinstance(depos, dict) else (lambda k: getattr(depos, k))
+    arrs = [get(k) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")]
+    if n is None:
+        n = arrs[0].numel()
+    for a in arrs:
+        if a.numel() < n:
+            raise ValueError("depo array shorter than n")
+    d = wcsim_depos(*[_dev_ptr(a, torch.float32) for a in arrs])
+    st = lib().wcsim_raster_scatter(plan, C.byref(d), int(n), int(depo_id_base), int(seed), int(bool(fluctuate)),
+                                    _dev_ptr(dev_depo_totals, torch.int32))
+    _check(st, "wcsim_raster_scatter")
+
+
+def wcsim_convolve(plan):
+    _check(lib().wcsim_convolve(plan), "wcsim_convolve")
+
+
+def _amp_ptr(amp):
+    if amp is None:
+        return None, None
+    a = np.ascontiguousarray(amp, dtype=np.float32)
+    return a, a.ctypes.data_as(C.c_void_p)
+
+
+def wcsim_add_noise(plan, amp=None, seed=0):
+    keep, p = _amp_ptr(amp)
+    _check(lib().wcsim_add_noise(plan, p, int(seed)), "wcsim_add_noise")
+
+
+def wcsim_arm_noise(plan, amp=None, seed=0):
+    keep, p = _amp_ptr(amp)
+    _check(lib().wcsim_arm_noise(plan, p, int(seed)), "wcsim_arm_noise")
+
+
+def wcsim_plan_destroy(plan):
+    _check(lib().wcsim_plan_destroy(plan), "wcsim_plan_destroy")
+
+
+def wcsim_clear(plan):
+    _check(lib().wcsim_clear(plan), "wcsim_clear")
+
+
+def wcsim_clear_output(plan):
+    _check(lib().wcsim_clear_output(plan), "wcsim_clear_output")
+
+
+def wcsim_sync(plan):
+    _check(lib().wcsim_sync(plan), "wcsim_sync")
+
+
+def wcsim_set_scatter_mode(plan, scatter_mode):
+    _check(lib().wcsim_set_scatter_mode(plan, int(scatter_mode)), "wcsim_set_scatter_mode")
+
+
+def wcsim_get_dims(plan):
+    v = [C.c_int() for _ in range(4)]
+    _check(lib().wcsim_get_dims(plan, *[C.byref(x) for x in v]), "wcsim_get_dims")
+    return tuple(x.value for x in v)
+
+
+def _borrow(plan, fn, name):
+    import torch
+    p = C.c_void_p()
+    _check(fn(plan, C.byref(p)), name)
+    n_wires, n_ticks, _, _ = wcsim_get_dims(plan)
+    return torch.as_tensor(_Borrowed(p.value, (n_wires, n_ticks), plan), device="cuda")
+
+
+def wcsim_charge_ptr(plan):
+    """S as a torch view [n_wires][n_ticks] of the plan's buffer (borrowed: valid until wcsim_plan_destroy)."""
+    return _borrow(plan, lib().wcsim_charge_ptr, "wcsim_charge_ptr")
+
+
+def wcsim_output_ptr(plan):
+    """M as a torch view [n_wires][n_ticks] of the plan's buffer (borrowed)."""
+    return _borrow(plan, lib().wcsim_output_ptr, "wcsim_output_ptr")
+
+
+def wcsim_get_stats(plan):
+    s = wcsim_stats()
+    _check(lib().wcsim_get_stats(plan, C.byref(s)), "wcsim_get_stats")
+    return {"depos_skipped": int(s.depos_skipped), "bins_drawn": int(s.bins_drawn)}
+
+
+def wcsim_reset_stats(plan):
+    _check(lib().wcsim_reset_stats(plan), "wcsim_reset_stats")
+
+
+def wcsim_simulate_host(plan, host_depos, host_M, n=None, seed=0, fluctuate=False, noise=False, noise_seed=0):
+    """host_depos: dict of HOST float32 arrays (numpy, or torch CPU tensors -- pinned makes the copies asynchronous);
+    host_M: HOST float32 [n_wires][n_ticks], written."""
+    def hp(a):
+        if hasattr(a, "data_ptr"):
+            assert (not a.is_cuda) and a.is_contiguous() and a.element_size() == 4
+            return C.c_void_p(a.data_ptr()), a.numel()
+        assert a.dtype == np.float32 and a.flags.c_contiguous
+        return a.ctypes.data_as(C.c_void_p), a.size
+    ptrs = [hp(host_depos[k]) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")]
+    if n is None:
+        n = ptrs[0][1]
+    pm, _ = hp(host_M)
+    st = lib().wcsim_simulate_host(plan, *[p for p, _ in ptrs], int(n), int(seed), int(bool(fluctuate)),
+                                   int(bool(noise)), int(noise_seed), pm)
+    _check(st, "wcsim_simulate_host")
+
+
+STAGES = ("raster", "rows_forward", "cols", "rows_inverse", "noise")
+
+
+def wcsim_set_profiling(plan, enable):
+    _check(lib().wcsim_set_profiling(plan, int(bool(enable))), "wcsim_set_profiling")
+
+
+def wcsim_get_stage_times(plan, reset=True):
+    """{stage: (total ms, spans)} accumulated since the last reset (synchronises)."""
+    ms = (C.c_double * len(STAGES))()
+    calls = (C.c_ulonglong * len(STAGES))()
+    _check(lib().wcsim_get_stage_times(plan, ms, calls, int(bool(reset))), "wcsim_get_stage_times")
+    return {s: (float(ms[k]), int(calls[k])) for k, s in enumerate(STAGES)}
+
+
+def wcsim_get_launch_count(plan):
+    v = C.c_ulonglong()
+    _check(lib().wcsim_get_launch_count(plan, C.byref(v)), "wcsim_get_launch_count")
+    return int(v.value)
+
+
+def wcsim_debug_philox(dev_ctr, dev_key, dev_out, n, stream=None):
+    _check(lib().wcsim_debug_philox(_dev_ptr(dev_ctr), _dev_ptr(dev_key), _dev_ptr(dev_out), int(n),
+                                    _stream_ptr(stream)), "wcsim_debug_philox")
+
+
+def wcsim_debug_binomial(dev_N, dev_p, dev_w, dev_k, n, stream=None):
+    _check(lib().wcsim_debug_binomial(_dev_ptr(dev_N), _dev_ptr(dev_p), _dev_ptr(dev_w), _dev_ptr(dev_k), int(n),
+                                      _stream_ptr(stream)), "wcsim_debug_binomial")
+
+
+def wcsim_debug_response_spectrum(plan):
+    _, _, pad_w, pad_t = wcsim_get_dims(plan)
+    out = np.zeros((pad_w, pad_t // 2 + 1, 2), dtype=np.float32)
+    _check(lib().wcsim_debug_response_spectrum(plan, out.ctypes.data_as(C.c_void_p)), "wcsim_debug_response_spectrum")
+    return out[..., 0] + 1j * out[..., 1]
+
+
+def wcsim_version():
+    return lib().wcsim_version().decode()
+
+
+class Plan:
+    """Context-managed plan handle: `with Plan(...) as p: p.raster_scatter(...); p.convolve(); M = p.output()`."""
+
+    def __init__(self, n_wires, n_ticks, response, pad=(0, 0), nsigma=3.0, scatter_mode=WCSIM_SCATTER_ATOMIC,
+                 stream=None):
+        self.handle = wcsim_plan_create(n_wires, n_ticks, response, pad, nsigma, scatter_mode, stream)
+        self.n_wires, self.n_ticks, self.pad_w, self.pad_t = wcsim_get_dims(self.handle)
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def destroy(self):
+        if self.handle is not None:
+            h, self.handle = self.handle, None
+            wcsim_plan_destroy(h)
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def raster_scatter(self, depos, **kw):
+        wcsim_raster_scatter(self.handle, depos, **kw)
+
+    def convolve(self):
+        wcsim_convolve(self.handle)
+
+    def add_noise(self, amp=None, seed=0):
+        wcsim_add_noise(self.handle, amp, seed)
+
+    def arm_noise(self, amp=None, seed=0):
+        wcsim_arm_noise(self.handle, amp, seed)
+
+    def clear(self):
+        wcsim_clear(self.handle)
+
+    def clear_output(self):
+        wcsim_clear_output(self.handle)
+
+    def sync(self):
+        wcsim_sync(self.handle)
+
+    def set_scatter_mode(self, mode):
+        wcsim_set_scatter_mode(self.handle, mode)
+
+    def charge(self):
+        return wcsim_charge_ptr(self.handle)
+
+    def output(self):
+        return wcsim_output_ptr(self.handle)
+
+    def stats(self):
+        return wcsim_get_stats(self.handle)
+
+    def reset_stats(self):
+        wcsim_reset_stats(self.handle)
+
+    def set_profiling(self, enable):
+        wcsim_set_profiling(self.handle, enable)
+
+    def stage_times(self, reset=True):
+        return wcsim_get_stage_times(self.handle, reset)
+
+    def launch_count(self):
+        return wcsim_get_launch_count(self.handle)
+
+    def simulate_host(self, host_depos, host_M, **kw):
+        wcsim_simulate_host(self.handle, host_depos, host_M, **kw)
+
+    def response_spectrum(self):
+        return wcsim_debug_response_spectrum(self.handle)

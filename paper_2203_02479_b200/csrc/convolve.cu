@@ -1,0 +1,299 @@
+// convolve.cu -- steps a4-a6 (and a7 fused) of the hot path: the FFT convolution of Eq. (2), PAPER.md:46-52:
+//     S(t,x) -> S(w_t, w_x),   M(w_t, w_x) = R(w_t, w_x) S(w_t, w_x),   M(w_t, w_x) -> M(t,x)
+// as three kernels over the zero-padded pad_w x pad_t grid (A13), none of which touches a padded element in HBM:
+//
+//   rows_forward : one CTA per populated wire row.  The real row of pad_t samples is packed as pad_t/2 complex
+//                  points (even + i odd), transformed in shared memory, and split into the half spectrum
+//                  k = 0 .. pad_t/2.  Samples beyond n_ticks are zeros made in registers.
+//   cols         : one CTA per tile of C adjacent tick-frequencies.  Forward transform over the wire axis (rows
+//                  beyond n_wires are zeros made in registers), multiply by the response spectrum while the data
+//                  is still in registers, inverse transform, store only the n_wires rows that are kept.
+//   rows_inverse : one CTA per kept wire row.  Half spectrum -> packed complex -> inverse transform -> the first
+//                  n_ticks real samples.  The noise spectrum of step a7 is added to the row spectrum here, so noise
+//                  costs no pass over M of its own.
+//
+// The 1/(pad_w pad_t) of the inverse transform is folded into Rhat (A14).  The FFT engine is csrc/fft.cuh.
+#include "fft.cuh"
+#include "internal.h"
+#include "rng.cuh"
+
+namespace wcsim {
+
+namespace {
+
+template <int N>
+struct RowCfg {
+    static constexpr int E = 16;
+    static constexpr int threads = N / E;
+    static constexpr int smem_bytes = SmemSize<N, 1>::float2s * (int)sizeof(float2);
+};
+template <int N>
+struct ColCfg {
+    static constexpr int C = N <= 1024 ? 8 : (N <= 4096 ? 4 : 2);
+    static constexpr int E = N <= 1024 ? 16 : 32;
+    static constexpr int threads = (N / E) * C;
+    static constexpr int smem_bytes = SmemSize<N, C>::float2s * (int)sizeof(float2);
+};
+
+// ------------------------------------------------------------------------------------------------------------------
+// a4, tick axis: real row -> half spectrum
+// ------------------------------------------------------------------------------------------------------------------
+template <int N, bool VEC>
+__global__ void __launch_bounds__(RowCfg<N>::threads) rows_forward_kernel(GridDims g, ConvBuffers b)
+{
+    constexpr int E = RowCfg<N>::E, NT = N / E;
+    extern __shared__ float2 smem[];
+    const int row = blockIdx.x, i = threadIdx.x;
+    const float *src = b.S + (size_t)row * g.n_ticks;
+    float2 v[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int pt = i + e * NT;
+        if constexpr (VEC) {
+            v[e] = (2 * pt < g.n_ticks) ? __ldg(reinterpret_cast<const float2 *>(src) + pt) : make_float2(0.f, 0.f);
+        } else {
+            v[e].x = (2 * pt < g.n_ticks) ? __ldg(src + 2 * pt) : 0.f;
+            v[e].y = (2 * pt + 1 < g.n_ticks) ? __ldg(src + 2 * pt + 1) : 0.f;
+        }
+    }
+    fft_block<N, 1, E, -1>(v, smem, i, 0, b.tw_row, false);
+    // split Z = FFT(even + i odd) into the spectrum of the real row:
+    //   A = (Z_k + conj Z_{N-k})/2, B = (Z_k - conj Z_{N-k})/(2i), X_k = A + exp(-2 pi i k / 2N) B
+    __syncthreads();
+#pragma unroll
+    for (int e = 0; e < E; ++e) smem[smem_index<1>(i + e * NT, 0)] = v[e];
+    __syncthreads();
+    float2 *dst = b.spec + (size_t)row * b.spec_stride;
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int k = i + e * NT;
+        const float2 zk = v[e];
+        const float2 zn = smem[smem_index<1>((N - k) & (N - 1), 0)];
+        const float2 A = make_float2(0.5f * (zk.x + zn.x), 0.5f * (zk.y - zn.y));
+        const float2 B = make_float2(0.5f * (zk.y + zn.y), -0.5f * (zk.x - zn.x));
+        const float2 w = load_tw(b.tw_real, k);
+        dst[k] = cadd(A, cmul(w, B));
+        if (k == 0) dst[N] = make_float2(zk.x - zk.y, 0.f);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// a4 wire axis, a5 multiply, a6 wire axis
+// ------------------------------------------------------------------------------------------------------------------
+template <int N>
+__global__ void __launch_bounds__(ColCfg<N>::threads) cols_kernel(GridDims g, ConvBuffers b)
+{
+    constexpr int C = ColCfg<N>::C, E = ColCfg<N>::E, NT = N / E;
+    extern __shared__ float2 smem[];
+    const int c = threadIdx.x % C, i = threadIdx.x / C;
+    const int col = blockIdx.x * C + c;
+    float2 *spec = b.spec + col;
+    const float2 *rh = b.Rhat + col;
+    float2 v[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int x = i + e * NT;
+        v[e] = (x < g.n_wires) ? spec[(size_t)x * b.spec_stride] : make_float2(0.f, 0.f);
+    }
+    fft_block<N, C, E, -1>(v, smem, i, c, b.tw_col, false);
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int x = i + e * NT;
+        v[e] = cmul(v[e], __ldg(rh + (size_t)x * b.spec_stride));
+    }
+    fft_block<N, C, E, +1>(v, smem, i, c, b.tw_col, true);
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int x = i + e * NT;
+        if (x < g.n_wires) spec[(size_t)x * b.spec_stride] = v[e];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// a6 tick axis (+ a7 noise): half spectrum -> real row
+// ------------------------------------------------------------------------------------------------------------------
+// noise spectrum of bin k on `wire`: amp[k] exp(2 pi i u), u = (word + 1/2) 2^-32 (A15-A17); amp is pre-scaled
+__device__ __forceinline__ float2 noise_bin(const NoiseArgs &nz, uint32_t wire, uint32_t k)
+{
+    const uint4 words = noise_words(nz.seed, wire, k >> 2);
+    const uint32_t w = pick_word(words, k & 3u);
+    float s, c;
+    sincospif((float)w * 4.656612873077393e-10f + 2.3283064365386963e-10f, &s, &c); // 2u = w 2^-31 + 2^-32
+    const float a = __ldg(nz.amp + k);
+    return make_float2(a * c, a * s);
+}
+
+template <int N, bool VEC>
+__global__ void __launch_bounds__(RowCfg<N>::threads) rows_inverse_kernel(GridDims g, ConvBuffers b, NoiseArgs nz,
+                                                                           bool use_spec, bool accumulate)
+{
+    constexpr int E = RowCfg<N>::E, NT = N / E;
+    extern __shared__ float2 smem[];
+    const int row = blockIdx.x, i = threadIdx.x;
+    const float2 *src = b.spec + (size_t)row * b.spec_stride;
+    const bool noisy = nz.amp != nullptr;
+    // stage X_k (+ noise) in shared memory so that every thread can reach the partner X_{N-k}
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int k = i + e * NT;
+        float2 x = use_spec ? __ldg(src + k) : make_float2(0.f, 0.f);
+        if (noisy) x = cadd(x, noise_bin(nz, (uint32_t)row, (uint32_t)k));
+        if (k == 0) {
+            x.y = 0.f; // the imaginary parts of the DC and Nyquist bins do not reach a real output
+            float2 xn = use_spec ? __ldg(src + N) : make_float2(0.f, 0.f);
+            if (noisy) xn = cadd(xn, noise_bin(nz, (uint32_t)row, (uint32_t)N));
+            xn.y = 0.f;
+            smem[smem_index<1>(N, 0)] = xn;
+        }
+        smem[smem_index<1>(k, 0)] = x;
+    }
+    __syncthreads();
+    // Z_k = (X_k + conj X_{N-k}) + i exp(+2 pi i k / 2N) (X_k - conj X_{N-k});  inverse FFT of Z = even + i odd
+    float2 v[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int k = i + e * NT;
+        const float2 xk = smem[smem_index<1>(k, 0)];
+        const float2 xn = smem[smem_index<1>(N - k, 0)];
+        const float2 s = make_float2(xk.x + xn.x, xk.y - xn.y);
+        const float2 d = make_float2(xk.x - xn.x, xk.y + xn.y);
+        const float2 w = load_tw(b.tw_real, k); // (cos, -sin)
+        const float2 t = make_float2(w.x * d.x + w.y * d.y, w.x * d.y - w.y * d.x);
+        v[e] = make_float2(s.x - t.y, s.y + t.x);
+    }
+    fft_block<N, 1, E, +1>(v, smem, i, 0, b.tw_row, true);
+    float *dst = b.M + (size_t)row * g.n_ticks;
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int pt = i + e * NT;
+        if constexpr (VEC) {
+            if (2 * pt < g.n_ticks) {
+                float2 *p = reinterpret_cast<float2 *>(dst) + pt;
+                float2 o = v[e];
+                if (accumulate) o = cadd(o, *p);
+                *p = o;
+            }
+        } else {
+            if (2 * pt < g.n_ticks) dst[2 * pt] = v[e].x + (accumulate ? dst[2 * pt] : 0.f);
+            if (2 * pt + 1 < g.n_ticks) dst[2 * pt + 1] = v[e].y + (accumulate ? dst[2 * pt + 1] : 0.f);
+        }
+    }
+}
+
+template <typename K>
+cudaError_t set_smem(K kernel, int bytes)
+{
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+#define WCSIM_ROW_SIZES(X) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096) X(8192) X(16384)
+#define WCSIM_COL_SIZES(X) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096) X(8192)
+
+} // namespace
+
+bool conv_sizes_supported(int pad_w, int pad_t)
+{
+    const int n = pad_t / 2;
+    bool row_ok = false, col_ok = false;
+#define X(NN) row_ok = row_ok || (n == NN);
+    WCSIM_ROW_SIZES(X)
+#undef X
+#define X(NN) col_ok = col_ok || (pad_w == NN);
+    WCSIM_COL_SIZES(X)
+#undef X
+    return row_ok && col_ok && pad_t == 2 * n;
+}
+
+cudaError_t conv_configure(int pad_w, int pad_t)
+{
+    cudaError_t err = cudaSuccess;
+    switch (pad_t / 2) {
+#define X(NN)                                                                                                          \
+    case NN:                                                                                                           \
+        if (err == cudaSuccess) err = set_smem(rows_forward_kernel<NN, true>, RowCfg<NN>::smem_bytes);                 \
+        if (err == cudaSuccess) err = set_smem(rows_forward_kernel<NN, false>, RowCfg<NN>::smem_bytes);                \
+        if (err == cudaSuccess) err = set_smem(rows_inverse_kernel<NN, true>, RowCfg<NN>::smem_bytes);                 \
+        if (err == cudaSuccess) err = set_smem(rows_inverse_kernel<NN, false>, RowCfg<NN>::smem_bytes);                \
+        break;
+        WCSIM_ROW_SIZES(X)
+#undef X
+    default:
+        return cudaErrorInvalidValue;
+    }
+    switch (pad_w) {
+#define X(NN)                                                                                                          \
+    case NN:                                                                                                           \
+        if (err == cudaSuccess) err = set_smem(cols_kernel<NN>, ColCfg<NN>::smem_bytes);                               \
+        break;
+        WCSIM_COL_SIZES(X)
+#undef X
+    default:
+        return cudaErrorInvalidValue;
+    }
+    return err;
+}
+
+static bool rows_vectorisable(GridDims g, const void *p)
+{
+    return (g.n_ticks % 2 == 0) && (reinterpret_cast<uintptr_t>(p) % 8 == 0);
+}
+
+cudaError_t launch_rows_forward(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st)
+{
+    const bool vec = rows_vectorisable(g, b.S);
+    switch (pad_t / 2) {
+#define X(NN)                                                                                                          \
+    case NN:                                                                                                           \
+        if (vec)                                                                                                       \
+            rows_forward_kernel<NN, true><<<g.n_wires, RowCfg<NN>::threads, RowCfg<NN>::smem_bytes, st>>>(g, b);       \
+        else                                                                                                           \
+            rows_forward_kernel<NN, false><<<g.n_wires, RowCfg<NN>::threads, RowCfg<NN>::smem_bytes, st>>>(g, b);      \
+        break;
+        WCSIM_ROW_SIZES(X)
+#undef X
+    default:
+        return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cols(GridDims g, int pad_w, int pad_t, ConvBuffers b, cudaStream_t st)
+{
+    (void)pad_t;
+    switch (pad_w) {
+#define X(NN)                                                                                                          \
+    case NN:                                                                                                           \
+        cols_kernel<NN><<<b.spec_stride / ColCfg<NN>::C, ColCfg<NN>::threads, ColCfg<NN>::smem_bytes, st>>>(g, b);     \
+        break;
+        WCSIM_COL_SIZES(X)
+#undef X
+    default:
+        return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rows_inverse(GridDims g, int pad_t, ConvBuffers b, NoiseArgs noise, bool use_spec, bool accumulate,
+                                cudaStream_t st)
+{
+    const bool vec = rows_vectorisable(g, b.M);
+    switch (pad_t / 2) {
+#define X(NN)                                                                                                          \
+    case NN:                                                                                                           \
+        if (vec)                                                                                                       \
+            rows_inverse_kernel<NN, true><<<g.n_wires, RowCfg<NN>::threads, RowCfg<NN>::smem_bytes, st>>>(             \
+                g, b, noise, use_spec, accumulate);                                                                    \
+        else                                                                                                           \
+            rows_inverse_kernel<NN, false><<<g.n_wires, RowCfg<NN>::threads, RowCfg<NN>::smem_bytes, st>>>(            \
+                g, b, noise, use_spec, accumulate);                                                                    \
+        break;
+        WCSIM_ROW_SIZES(X)
+#undef X
+    default:
+        return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+} // namespace wcsim

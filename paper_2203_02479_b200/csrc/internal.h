@@ -1,0 +1,81 @@
+// internal.h -- host-side declarations shared by the translation units of libwcsim (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace wcsim {
+
+struct DepoArrays {
+    const float *t0, *x0, *sigma_t, *sigma_x, *q;
+};
+
+struct GridDims {
+    int n_wires, n_ticks;
+};
+
+// device counters (wcsim_stats)
+struct Counters {
+    unsigned long long depos_skipped;
+    unsigned long long bins_drawn;
+};
+
+// ---- raster.cu ----
+// a1-a3, atomic mode: S[wire][tick] += patch of every depo (red.global.add.f32)
+cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
+                                 double nsigma, float *S, int *depo_totals, Counters *counters, int sm_count,
+                                 cudaStream_t st);
+
+// a1-a3, tiled mode (deterministic): scratch buffers are owned by the plan and grown by the caller
+struct TileScratch {
+    int tile_w, tile_t;           // tile shape in bins
+    int tiles_w, tiles_t;         // tile counts
+    unsigned int *tile_count;     // [n_tiles + 1] counts, then exclusive offsets
+    unsigned int *tile_cursor;    // [n_tiles] fill cursors
+    unsigned int *entries;        // [capacity] depo indices grouped by tile
+    unsigned long long capacity;  // entries allocated
+    unsigned int *total;          // [1] total number of (depo, tile) pairs
+};
+cudaError_t launch_tile_count(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts, cudaStream_t st);
+cudaError_t launch_tile_scan(TileScratch ts, cudaStream_t st);
+cudaError_t launch_tile_fill(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts, cudaStream_t st);
+cudaError_t launch_count_invalid(DepoArrays d, long long n, Counters *counters, cudaStream_t st);
+void tile_shape(int *tile_w, int *tile_t);
+cudaError_t launch_tile_accumulate(GridDims g, DepoArrays d, uint64_t id_base, uint64_t seed, int fluctuate,
+                                   double nsigma, TileScratch ts, float *S, int *depo_totals, Counters *counters,
+                                   cudaStream_t st);
+
+// ---- convolve.cu ----
+struct ConvBuffers {
+    const float *S;       // [n_wires][n_ticks]
+    float *M;             // [n_wires][n_ticks]
+    float2 *spec;         // [n_wires][spec_stride]  row spectra, then (in place) the product spectra
+    const float2 *Rhat;   // [pad_w][spec_stride]
+    const float2 *tw_row; // [pad_t/2]  exp(-2 pi i j / (pad_t/2))
+    const float2 *tw_real;// [pad_t/2]  exp(-2 pi i j / pad_t)
+    const float2 *tw_col; // [pad_w]    exp(-2 pi i j / pad_w)
+    int spec_stride;      // pad_t/2 + 8
+};
+struct NoiseArgs {
+    const float *amp; // DEVICE [pad_t/2 + 1], already scaled by pad_t^-1/2; NULL = no noise
+    uint64_t seed;
+};
+bool conv_sizes_supported(int pad_w, int pad_t);
+cudaError_t conv_configure(int pad_w, int pad_t); // sets the kernels' shared-memory attributes (once per plan)
+cudaError_t launch_rows_forward(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st);
+cudaError_t launch_cols(GridDims g, int pad_w, int pad_t, ConvBuffers b, cudaStream_t st);
+// M = (accumulate ? M : 0) + c2r(use_spec ? spec : 0  +  noise)
+cudaError_t launch_rows_inverse(GridDims g, int pad_t, ConvBuffers b, NoiseArgs noise, bool use_spec, bool accumulate,
+                                cudaStream_t st);
+
+// ---- response.cu ---- (plan time)
+// Rhat[kx][kt] = 1/(pad_w pad_t) sum_dx sum_dt R[dx+c][dt] exp(-2 pi i (kx dx / pad_w + kt dt / pad_t)), fp64 -> fp32
+cudaError_t build_response_spectrum(const float *dev_R, int n_rw, int n_rt, int pad_w, int pad_t, int spec_stride,
+                                    double2 *dev_tmp /* [n_rw][pad_t/2+1] */, float2 *dev_Rhat, cudaStream_t st);
+
+// ---- debug.cu ----
+cudaError_t launch_debug_philox(const unsigned int *ctr, const unsigned int *key, unsigned int *out, long long n,
+                                cudaStream_t st);
+cudaError_t launch_debug_binomial(const double *N, const double *p, const unsigned int *w, double *k, long long n,
+                                  cudaStream_t st);
+
+} // namespace wcsim

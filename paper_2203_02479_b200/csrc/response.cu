@@ -1,0 +1,113 @@
+// response.cu -- step p0: the "similarly transformed 2D detector response array R(w_t, w_x)" of PAPER.md:44, built
+// once per plan.  R (n_rw x n_rt, wire-centred, tick-causal: A11) is embedded in the pad_w x pad_t grid with
+// wrap-around on the wire axis and transformed by the definition of the DFT in fp64 -- R has only n_rw * n_rt
+// non-zero samples, so the two separable sums below are cheap -- then scaled by 1/(pad_w pad_t) (A14) and rounded
+// to fp32 once.  Also holds the small diagnostic kernels behind wcsim_debug_*.
+#include "internal.h"
+#include "rng.cuh"
+
+namespace wcsim {
+
+namespace {
+
+// exp(-2 pi i m / n) for integers 0 <= m < n, n a power of two: sincospi of an exactly representable argument
+__device__ __forceinline__ double2 unit_root(long long m, int n)
+{
+    double s, c;
+    sincospi(-2.0 * (double)m / (double)n, &s, &c);
+    return make_double2(c, s);
+}
+
+// tmp[r][kt] = sum_dt R[r][dt] exp(-2 pi i kt dt / pad_t),  kt = 0 .. pad_t/2
+__global__ void response_ticks_kernel(const float *__restrict__ R, int n_rw, int n_rt, int pad_t,
+                                      double2 *__restrict__ tmp)
+{
+    const int kt = blockIdx.x * blockDim.x + threadIdx.x;
+    const int r = blockIdx.y;
+    if (kt > pad_t / 2) return;
+    double re = 0.0, im = 0.0;
+    for (int dt = 0; dt < n_rt; ++dt) {
+        const double v = (double)R[(size_t)r * n_rt + dt];
+        const double2 w = unit_root(((long long)kt * dt) & (pad_t - 1), pad_t);
+        re += v * w.x;
+        im += v * w.y;
+    }
+    tmp[(size_t)r * (pad_t / 2 + 1) + kt] = make_double2(re, im);
+}
+
+// Rhat[kx][kt] = scale * sum_dx tmp[dx + c][kt] exp(-2 pi i kx dx / pad_w),  dx = -c .. c
+__global__ void response_wires_kernel(const double2 *__restrict__ tmp, int n_rw, int pad_w, int pad_t, int spec_stride,
+                                      float2 *__restrict__ Rhat)
+{
+    const int kt = blockIdx.x * blockDim.x + threadIdx.x;
+    const int kx = blockIdx.y;
+    if (kt >= spec_stride) return;
+    float2 out = make_float2(0.f, 0.f);
+    if (kt <= pad_t / 2) {
+        const int c = (n_rw - 1) / 2;
+        double re = 0.0, im = 0.0;
+        for (int r = 0; r < n_rw; ++r) {
+            const long long dx = r - c;
+            const long long m = ((long long)kx * dx) & (long long)(pad_w - 1); // two's complement: mod pad_w
+            const double2 w = unit_root(m, pad_w);
+            const double2 v = tmp[(size_t)r * (pad_t / 2 + 1) + kt];
+            re += v.x * w.x - v.y * w.y;
+            im += v.x * w.y + v.y * w.x;
+        }
+        const double scale = 1.0 / ((double)pad_w * (double)pad_t);
+        out = make_float2((float)(re * scale), (float)(im * scale));
+    }
+    Rhat[(size_t)kx * spec_stride + kt] = out;
+}
+
+__global__ void debug_philox_kernel(const unsigned int *ctr, const unsigned int *key, unsigned int *out, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint4 r = philox4x32_10(make_uint4(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3]),
+                                  make_uint2(key[2 * i], key[2 * i + 1]));
+    out[4 * i] = r.x;
+    out[4 * i + 1] = r.y;
+    out[4 * i + 2] = r.z;
+    out[4 * i + 3] = r.w;
+}
+
+__global__ void debug_binomial_kernel(const double *N, const double *p, const unsigned int *w, double *k, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    k[i] = binomial_draw(N[i], p[i], w[i]);
+}
+
+} // namespace
+
+cudaError_t build_response_spectrum(const float *dev_R, int n_rw, int n_rt, int pad_w, int pad_t, int spec_stride,
+                                    double2 *dev_tmp, float2 *dev_Rhat, cudaStream_t st)
+{
+    const int threads = 128;
+    dim3 g1((pad_t / 2 + 1 + threads - 1) / threads, n_rw);
+    response_ticks_kernel<<<g1, threads, 0, st>>>(dev_R, n_rw, n_rt, pad_t, dev_tmp);
+    cudaError_t err = cudaGetLastError();
+    if (err != cudaSuccess) return err;
+    dim3 g2((spec_stride + threads - 1) / threads, pad_w);
+    response_wires_kernel<<<g2, threads, 0, st>>>(dev_tmp, n_rw, pad_w, pad_t, spec_stride, dev_Rhat);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_debug_philox(const unsigned int *ctr, const unsigned int *key, unsigned int *out, long long n,
+                                cudaStream_t st)
+{
+    if (n <= 0) return cudaSuccess;
+    debug_philox_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(ctr, key, out, n);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_debug_binomial(const double *N, const double *p, const unsigned int *w, double *k, long long n,
+                                  cudaStream_t st)
+{
+    if (n <= 0) return cudaSuccess;
+    debug_binomial_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(N, p, w, k, n);
+    return cudaGetLastError();
+}
+
+} // namespace wcsim

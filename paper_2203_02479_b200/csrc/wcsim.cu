@@ -1,0 +1,621 @@
+// wcsim.cu -- the C ABI of include/wcsim.h: plan life cycle, argument checking, buffer ownership and the launch
+// sequences.  All arithmetic of the path lives in raster.cu / convolve.cu / response.cu; there is no CPU fallback.
+#include "../../include/wcsim.h"
+#include "internal.h"
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace wcsim;
+
+struct wcsim_plan {
+    int n_wires = 0, n_ticks = 0, pad_w = 0, pad_t = 0, n_rw = 0, n_rt = 0, spec_stride = 0;
+    double nsigma = 3.0;
+    int scatter_mode = WCSIM_SCATTER_ATOMIC;
+    cudaStream_t stream = nullptr;
+    int device = 0, sm_count = 148;
+    float *S = nullptr, *M = nullptr;
+    float2 *spec = nullptr, *Rhat = nullptr, *tw_row = nullptr, *tw_real = nullptr, *tw_col = nullptr;
+    Counters *counters = nullptr;
+    float *amp_builtin = nullptr, *amp_custom = nullptr; // device, pad_t/2+1, scaled by pad_t^-1/2
+    bool noise_armed = false;
+    const float *armed_amp = nullptr;
+    uint64_t armed_seed = 0;
+    TileScratch ts{};
+    unsigned int *host_total = nullptr; // pinned
+    float *stage[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    long long stage_cap = 0;
+    // profiling: CUDA events recorded around each stage on the plan's stream while enabled
+    struct Span {
+        cudaEvent_t beg, end;
+        int stage;
+    };
+    bool profiling = false;
+    std::vector<Span> pending;
+    std::vector<cudaEvent_t> free_events;
+    double stage_ms[WCSIM_N_STAGES] = {0, 0, 0, 0, 0};
+    unsigned long long stage_calls[WCSIM_N_STAGES] = {0, 0, 0, 0, 0};
+    unsigned long long launches = 0; // kernels of this library enqueued so far
+};
+
+namespace {
+
+thread_local int tls_cuda_error = 0;
+
+int fail_cuda(cudaError_t e)
+{
+    tls_cuda_error = (int)e;
+    cudaGetLastError(); // clear the sticky-less error state
+    return e == cudaErrorMemoryAllocation ? WCSIM_ENOMEM : WCSIM_ECUDA;
+}
+
+#define CU_TRY(expr)                                                                                                   \
+    do {                                                                                                               \
+        cudaError_t e__ = (expr);                                                                                      \
+        if (e__ != cudaSuccess) return fail_cuda(e__);                                                                 \
+    } while (0)
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) {
+            ok = false;
+            return;
+        }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard()
+    {
+        int cur = -1;
+        if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+    }
+};
+
+cudaEvent_t take_event(wcsim_plan *p)
+{
+    cudaEvent_t e = nullptr;
+    if (!p->free_events.empty()) {
+        e = p->free_events.back();
+        p->free_events.pop_back();
+    } else if (cudaEventCreate(&e) != cudaSuccess) {
+        e = nullptr;
+    }
+    return e;
+}
+
+// accumulate finished spans into stage_ms (synchronises the stream)
+int harvest_spans(wcsim_plan *p)
+{
+    if (p->pending.empty()) return WCSIM_OK;
+    CU_TRY(cudaStreamSynchronize(p->stream));
+    for (auto &sp : p->pending) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, sp.beg, sp.end) == cudaSuccess) {
+            p->stage_ms[sp.stage] += (double)ms;
+            p->stage_calls[sp.stage] += 1;
+        }
+        p->free_events.push_back(sp.beg);
+        p->free_events.push_back(sp.end);
+    }
+    p->pending.clear();
+    return WCSIM_OK;
+}
+
+// RAII span: records an event pair around a stage when profiling is enabled
+struct StageSpan {
+    wcsim_plan *p;
+    cudaEvent_t beg = nullptr, end = nullptr;
+    int stage;
+    StageSpan(wcsim_plan *plan, int st) : p(plan), stage(st)
+    {
+        if (!p->profiling) return;
+        if (p->pending.size() >= 8192) harvest_spans(p);
+        beg = take_event(p);
+        end = take_event(p);
+        if (beg && end) cudaEventRecord(beg, p->stream);
+    }
+    ~StageSpan()
+    {
+        if (beg && end) {
+            cudaEventRecord(end, p->stream);
+            p->pending.push_back({beg, end, stage});
+        }
+    }
+};
+
+bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+int next_pow2(long long n, int floor_)
+{
+    long long p = floor_;
+    while (p < n) p <<= 1;
+    return p > (1 << 30) ? 0 : (int)p;
+}
+
+ConvBuffers conv_buffers(const wcsim_plan *p)
+{
+    ConvBuffers b;
+    b.S = p->S;
+    b.M = p->M;
+    b.spec = p->spec;
+    b.Rhat = p->Rhat;
+    b.tw_row = p->tw_row;
+    b.tw_real = p->tw_real;
+    b.tw_col = p->tw_col;
+    b.spec_stride = p->spec_stride;
+    return b;
+}
+
+int upload_twiddles(float2 **dev, int n, int denom, cudaStream_t st)
+{
+    std::vector<float2> h((size_t)n);
+    for (int j = 0; j < n; ++j) {
+        const double a = -2.0 * M_PI * (double)j / (double)denom;
+        h[j] = make_float2((float)cos(a), (float)sin(a));
+    }
+    CU_TRY(cudaMalloc((void **)dev, sizeof(float2) * (size_t)n));
+    CU_TRY(cudaMemcpyAsync(*dev, h.data(), sizeof(float2) * (size_t)n, cudaMemcpyHostToDevice, st));
+    CU_TRY(cudaStreamSynchronize(st));
+    return WCSIM_OK;
+}
+
+// amplitude spectrum -> device, scaled by pad_t^-1/2 (orthonormal inverse transform, A15)
+int upload_amp(wcsim_plan *p, const float *host_amp, float *dev)
+{
+    const int nk = p->pad_t / 2 + 1;
+    std::vector<float> h((size_t)nk);
+    const double scale = 1.0 / sqrt((double)p->pad_t);
+    for (int k = 0; k < nk; ++k) {
+        double a;
+        if (host_amp) {
+            a = (double)host_amp[k];
+        } else { // A(f) = 3 (f/f0) exp(-f/f0), f0 = 0.1 f_Nyquist, f in cycles per tick (configs[3])
+            const double f = (double)k / (double)p->pad_t, f0 = 0.1 * 0.5;
+            a = 3.0 * (f / f0) * exp(-(f / f0));
+        }
+        h[k] = (float)(a * scale);
+    }
+    CU_TRY(cudaMemcpyAsync(dev, h.data(), sizeof(float) * (size_t)nk, cudaMemcpyHostToDevice, p->stream));
+    CU_TRY(cudaStreamSynchronize(p->stream)); // h goes out of scope
+    return WCSIM_OK;
+}
+
+int ensure_stage(wcsim_plan *p, long long n)
+{
+    if (n <= p->stage_cap) return WCSIM_OK;
+    CU_TRY(cudaStreamSynchronize(p->stream));
+    for (float *&s : p->stage) {
+        if (s) cudaFree(s);
+        s = nullptr;
+    }
+    p->stage_cap = 0;
+    const long long cap = n + n / 4 + 1024;
+    for (float *&s : p->stage) CU_TRY(cudaMalloc((void **)&s, sizeof(float) * (size_t)cap));
+    p->stage_cap = cap;
+    return WCSIM_OK;
+}
+
+int raster_tiled(wcsim_plan *p, GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
+                 int *totals)
+{
+    TileScratch &ts = p->ts;
+    const int n_tiles = ts.tiles_w * ts.tiles_t;
+    if (n > 0xFFFFFFFFll) return WCSIM_EINVAL; // entries hold 32-bit depo indices
+    CU_TRY(cudaMemsetAsync(ts.tile_count, 0, sizeof(unsigned int) * (size_t)(n_tiles + 1), p->stream));
+    CU_TRY(launch_tile_count(g, d, n, p->nsigma, ts, p->stream));
+    CU_TRY(launch_tile_scan(ts, p->stream));
+    CU_TRY(cudaMemcpyAsync(p->host_total, ts.total, sizeof(unsigned int), cudaMemcpyDeviceToHost, p->stream));
+    CU_TRY(cudaStreamSynchronize(p->stream));
+    const unsigned long long need = *p->host_total;
+    if (need > ts.capacity) {
+        if (ts.entries) cudaFree(ts.entries);
+        ts.entries = nullptr;
+        ts.capacity = 0;
+        const unsigned long long cap = need + need / 4 + 4096;
+        CU_TRY(cudaMalloc((void **)&ts.entries, sizeof(unsigned int) * cap));
+        ts.capacity = cap;
+    }
+    CU_TRY(launch_tile_fill(g, d, n, p->nsigma, ts, p->stream));
+    if (totals) CU_TRY(cudaMemsetAsync(totals, 0, sizeof(int) * (size_t)n, p->stream));
+    CU_TRY(launch_count_invalid(d, n, p->counters, p->stream));
+    CU_TRY(launch_tile_accumulate(g, d, id_base, seed, fluctuate, p->nsigma, ts, p->S, totals, p->counters, p->stream));
+    return WCSIM_OK;
+}
+
+int destroy_impl(wcsim_plan *p)
+{
+    int rc = WCSIM_OK;
+    if (cudaStreamSynchronize(p->stream) != cudaSuccess) rc = fail_cuda(cudaGetLastError());
+    void *bufs[] = {p->S,        p->M,           p->spec,        p->Rhat,           p->tw_row,        p->tw_real,
+                    p->tw_col,   p->counters,    p->amp_builtin, p->amp_custom,     p->ts.tile_count, p->ts.tile_cursor,
+                    p->ts.entries, p->ts.total,  p->stage[0],    p->stage[1],       p->stage[2],      p->stage[3],
+                    p->stage[4]};
+    for (void *b : bufs)
+        if (b) cudaFree(b);
+    if (p->host_total) cudaFreeHost(p->host_total);
+    for (auto &sp : p->pending) {
+        cudaEventDestroy(sp.beg);
+        cudaEventDestroy(sp.end);
+    }
+    for (cudaEvent_t e : p->free_events) cudaEventDestroy(e);
+    delete p;
+    return rc;
+}
+
+} // namespace
+
+extern "C" {
+
+int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *response, int n_rwires, int n_rticks,
+                      wcsim_pad pad, float nsigma, int scatter_mode, void *cuda_stream)
+{
+    if (!out) return WCSIM_EINVAL;
+    *out = nullptr;
+    if (!response || n_wires <= 0 || n_ticks <= 0 || n_rwires <= 0 || n_rticks <= 0 || (n_rwires % 2) == 0)
+        return WCSIM_EINVAL;
+    if (!(nsigma > 0.0f) || !std::isfinite(nsigma)) return WCSIM_EINVAL;
+    if (scatter_mode != WCSIM_SCATTER_ATOMIC && scatter_mode != WCSIM_SCATTER_TILED) return WCSIM_EINVAL;
+    if (pad.wires < 0 || pad.ticks < 0) return WCSIM_EINVAL;
+    const int c = (n_rwires - 1) / 2;
+    const long long need_t = (long long)n_ticks + n_rticks - 1, need_w = (long long)n_wires + c;
+    const int pad_t = pad.ticks ? pad.ticks : next_pow2(need_t, 32);
+    const int pad_w = pad.wires ? pad.wires : next_pow2(need_w, 16);
+    if (!is_pow2(pad_t) || !is_pow2(pad_w) || pad_t < need_t || pad_w < need_w || pad_t < 32 || pad_w < 16)
+        return WCSIM_EINVAL;
+    if (pad_w < n_rwires) return WCSIM_EINVAL; // the wrapped response must not overlap itself
+    if (!conv_sizes_supported(pad_w, pad_t)) return WCSIM_EINVAL;
+    if ((long long)n_wires * n_ticks > 0x7FFFFFFFll * 2) return WCSIM_EINVAL;
+
+    int dev = 0;
+    CU_TRY(cudaGetDevice(&dev));
+    wcsim_plan *p = new (std::nothrow) wcsim_plan;
+    if (!p) return WCSIM_ENOMEM;
+    p->n_wires = n_wires;
+    p->n_ticks = n_ticks;
+    p->pad_w = pad_w;
+    p->pad_t = pad_t;
+    p->n_rw = n_rwires;
+    p->n_rt = n_rticks;
+    p->spec_stride = pad_t / 2 + 8;
+    p->nsigma = (double)nsigma;
+    p->scatter_mode = scatter_mode;
+    p->stream = (cudaStream_t)cuda_stream;
+    p->device = dev;
+
+    float *dev_R = nullptr;
+    double2 *dev_tmp = nullptr;
+    int rc = [&]() -> int {
+        CU_TRY(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev));
+        const size_t grid = (size_t)n_wires * n_ticks;
+        CU_TRY(cudaMalloc((void **)&p->S, sizeof(float) * grid));
+        CU_TRY(cudaMalloc((void **)&p->M, sizeof(float) * grid));
+        CU_TRY(cudaMalloc((void **)&p->spec, sizeof(float2) * (size_t)n_wires * p->spec_stride));
+        CU_TRY(cudaMalloc((void **)&p->Rhat, sizeof(float2) * (size_t)pad_w * p->spec_stride));
+        CU_TRY(cudaMalloc((void **)&p->counters, sizeof(Counters)));
+        CU_TRY(cudaMalloc((void **)&p->amp_builtin, sizeof(float) * (size_t)(pad_t / 2 + 1)));
+        CU_TRY(cudaMalloc((void **)&p->amp_custom, sizeof(float) * (size_t)(pad_t / 2 + 1)));
+        CU_TRY(cudaMemsetAsync(p->S, 0, sizeof(float) * grid, p->stream));
+        CU_TRY(cudaMemsetAsync(p->M, 0, sizeof(float) * grid, p->stream));
+        CU_TRY(cudaMemsetAsync(p->spec, 0, sizeof(float2) * (size_t)n_wires * p->spec_stride, p->stream));
+        CU_TRY(cudaMemsetAsync(p->counters, 0, sizeof(Counters), p->stream));
+        int r = upload_twiddles(&p->tw_row, pad_t / 2, pad_t / 2, p->stream);
+        if (r) return r;
+        r = upload_twiddles(&p->tw_real, pad_t / 2, pad_t, p->stream);
+        if (r) return r;
+        r = upload_twiddles(&p->tw_col, pad_w, pad_w, p->stream);
+        if (r) return r;
+        r = upload_amp(p, nullptr, p->amp_builtin);
+        if (r) return r;
+        // tile lists of the deterministic scatter mode
+        tile_shape(&p->ts.tile_w, &p->ts.tile_t);
+        p->ts.tiles_w = (n_wires + p->ts.tile_w - 1) / p->ts.tile_w;
+        p->ts.tiles_t = (n_ticks + p->ts.tile_t - 1) / p->ts.tile_t;
+        const size_t n_tiles = (size_t)p->ts.tiles_w * p->ts.tiles_t;
+        CU_TRY(cudaMalloc((void **)&p->ts.tile_count, sizeof(unsigned int) * (n_tiles + 1)));
+        CU_TRY(cudaMalloc((void **)&p->ts.tile_cursor, sizeof(unsigned int) * n_tiles));
+        CU_TRY(cudaMalloc((void **)&p->ts.total, sizeof(unsigned int)));
+        CU_TRY(cudaMallocHost((void **)&p->host_total, sizeof(unsigned int)));
+        // response spectrum
+        const size_t nr = (size_t)n_rwires * n_rticks;
+        CU_TRY(cudaMalloc((void **)&dev_R, sizeof(float) * nr));
+        CU_TRY(cudaMalloc((void **)&dev_tmp, sizeof(double2) * (size_t)n_rwires * (pad_t / 2 + 1)));
+        CU_TRY(cudaMemcpyAsync(dev_R, response, sizeof(float) * nr, cudaMemcpyHostToDevice, p->stream));
+        CU_TRY(build_response_spectrum(dev_R, n_rwires, n_rticks, pad_w, pad_t, p->spec_stride, dev_tmp, p->Rhat,
+                                       p->stream));
+        CU_TRY(conv_configure(pad_w, pad_t));
+        CU_TRY(cudaStreamSynchronize(p->stream));
+        return WCSIM_OK;
+    }();
+    if (dev_R) cudaFree(dev_R);
+    if (dev_tmp) cudaFree(dev_tmp);
+    if (rc != WCSIM_OK) {
+        const int keep = tls_cuda_error;
+        destroy_impl(p);
+        tls_cuda_error = keep;
+        return rc;
+    }
+    *out = p;
+    return WCSIM_OK;
+}
+
+int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n, unsigned long long depo_id_base,
+                         unsigned long long seed, int fluctuate, int *dev_depo_totals)
+{
+    if (!plan || n < 0) return WCSIM_EINVAL;
+    if (n == 0) return WCSIM_OK;
+    if (!depos || !depos->t0 || !depos->x0 || !depos->sigma_t || !depos->sigma_x || !depos->q) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    if (!guard.ok) return fail_cuda(cudaGetLastError());
+    const GridDims g{plan->n_wires, plan->n_ticks};
+    const DepoArrays d{depos->t0, depos->x0, depos->sigma_t, depos->sigma_x, depos->q};
+    StageSpan span(plan, WCSIM_STAGE_RASTER);
+    if (plan->scatter_mode == WCSIM_SCATTER_TILED) {
+        plan->launches += 5;
+        return raster_tiled(plan, g, d, n, depo_id_base, seed, fluctuate != 0, dev_depo_totals);
+    }
+    plan->launches += 1;
+    CU_TRY(launch_raster_atomic(g, d, n, depo_id_base, seed, fluctuate != 0, plan->nsigma, plan->S, dev_depo_totals,
+                                plan->counters, plan->sm_count, plan->stream));
+    return WCSIM_OK;
+}
+
+int wcsim_convolve(wcsim_plan *plan)
+{
+    if (!plan) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    if (!guard.ok) return fail_cuda(cudaGetLastError());
+    const GridDims g{plan->n_wires, plan->n_ticks};
+    const ConvBuffers b = conv_buffers(plan);
+    NoiseArgs nz{nullptr, 0};
+    if (plan->noise_armed) {
+        nz.amp = plan->armed_amp;
+        nz.seed = plan->armed_seed;
+        plan->noise_armed = false;
+    }
+    {
+        StageSpan span(plan, WCSIM_STAGE_ROWS_FORWARD);
+        CU_TRY(launch_rows_forward(g, plan->pad_t, b, plan->stream));
+    }
+    {
+        StageSpan span(plan, WCSIM_STAGE_COLS);
+        CU_TRY(launch_cols(g, plan->pad_w, plan->pad_t, b, plan->stream));
+    }
+    {
+        StageSpan span(plan, WCSIM_STAGE_ROWS_INVERSE);
+        CU_TRY(launch_rows_inverse(g, plan->pad_t, b, nz, true, false, plan->stream));
+    }
+    plan->launches += 3;
+    return WCSIM_OK;
+}
+
+static int noise_amp_ptr(wcsim_plan *plan, const float *amp, const float **dev)
+{
+    if (!amp) {
+        *dev = plan->amp_builtin;
+        return WCSIM_OK;
+    }
+    const int rc = upload_amp(plan, amp, plan->amp_custom);
+    *dev = plan->amp_custom;
+    return rc;
+}
+
+int wcsim_add_noise(wcsim_plan *plan, const float *amp, unsigned long long seed)
+{
+    if (!plan) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    if (!guard.ok) return fail_cuda(cudaGetLastError());
+    NoiseArgs nz{nullptr, seed};
+    const int rc = noise_amp_ptr(plan, amp, &nz.amp);
+    if (rc) return rc;
+    const GridDims g{plan->n_wires, plan->n_ticks};
+    StageSpan span(plan, WCSIM_STAGE_NOISE);
+    CU_TRY(launch_rows_inverse(g, plan->pad_t, conv_buffers(plan), nz, false, true, plan->stream));
+    plan->launches += 1;
+    return WCSIM_OK;
+}
+
+int wcsim_arm_noise(wcsim_plan *plan, const float *amp, unsigned long long seed)
+{
+    if (!plan) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    if (!guard.ok) return fail_cuda(cudaGetLastError());
+    const float *dev = nullptr;
+    const int rc = noise_amp_ptr(plan, amp, &dev);
+    if (rc) return rc;
+    plan->armed_amp = dev;
+    plan->armed_seed = seed;
+    plan->noise_armed = true;
+    return WCSIM_OK;
+}
+
+int wcsim_plan_destroy(wcsim_plan *plan)
+{
+    if (!plan) return WCSIM_OK;
+    DeviceGuard guard(plan->device);
+    return destroy_impl(plan);
+}
+
+int wcsim_clear(wcsim_plan *plan)
+{
+    if (!plan) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    CU_TRY(cudaMemsetAsync(plan->S, 0, sizeof(float) * (size_t)plan->n_wires * plan->n_ticks, plan->stream));
+    return WCSIM_OK;
+}
+
+int wcsim_clear_output(wcsim_plan *plan)
+{
+    if (!plan) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    CU_TRY(cudaMemsetAsync(plan->M, 0, sizeof(float) * (size_t)plan->n_wires * plan->n_ticks, plan->stream));
+    return WCSIM_OK;
+}
+
+int wcsim_sync(wcsim_plan *plan)
+{
+    if (!plan) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    CU_TRY(cudaStreamSynchronize(plan->stream));
+    return WCSIM_OK;
+}
+
+int wcsim_set_scatter_mode(wcsim_plan *plan, int scatter_mode)
+{
+    if (!plan || (scatter_mode != WCSIM_SCATTER_ATOMIC && scatter_mode != WCSIM_SCATTER_TILED)) return WCSIM_EINVAL;
+    plan->scatter_mode = scatter_mode;
+    return WCSIM_OK;
+}
+
+int wcsim_charge_ptr(wcsim_plan *plan, float **dev)
+{
+    if (!plan || !dev) return WCSIM_EINVAL;
+    *dev = plan->S;
+    return WCSIM_OK;
+}
+
+int wcsim_output_ptr(wcsim_plan *plan, float **dev)
+{
+    if (!plan || !dev) return WCSIM_EINVAL;
+    *dev = plan->M;
+    return WCSIM_OK;
+}
+
+int wcsim_get_dims(const wcsim_plan *plan, int *n_wires, int *n_ticks, int *pad_wires, int *pad_ticks)
+{
+    if (!plan) return WCSIM_EINVAL;
+    if (n_wires) *n_wires = plan->n_wires;
+    if (n_ticks) *n_ticks = plan->n_ticks;
+    if (pad_wires) *pad_wires = plan->pad_w;
+    if (pad_ticks) *pad_ticks = plan->pad_t;
+    return WCSIM_OK;
+}
+
+int wcsim_get_stats(wcsim_plan *plan, wcsim_stats *out)
+{
+    if (!plan || !out) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    Counters c;
+    CU_TRY(cudaMemcpyAsync(&c, plan->counters, sizeof(c), cudaMemcpyDeviceToHost, plan->stream));
+    CU_TRY(cudaStreamSynchronize(plan->stream));
+    out->depos_skipped = c.depos_skipped;
+    out->bins_drawn = c.bins_drawn;
+    return WCSIM_OK;
+}
+
+int wcsim_reset_stats(wcsim_plan *plan)
+{
+    if (!plan) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    CU_TRY(cudaMemsetAsync(plan->counters, 0, sizeof(Counters), plan->stream));
+    return WCSIM_OK;
+}
+
+int wcsim_simulate_host(wcsim_plan *plan, const float *host_t0, const float *host_x0, const float *host_sigma_t,
+                        const float *host_sigma_x, const float *host_q, long long n, unsigned long long seed,
+                        int fluctuate, int noise, unsigned long long noise_seed, float *host_M)
+{
+    if (!plan || n < 0 || !host_M) return WCSIM_EINVAL;
+    if (n > 0 && (!host_t0 || !host_x0 || !host_sigma_t || !host_sigma_x || !host_q)) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    if (!guard.ok) return fail_cuda(cudaGetLastError());
+    int rc = ensure_stage(plan, n);
+    if (rc) return rc;
+    const float *src[5] = {host_t0, host_x0, host_sigma_t, host_sigma_x, host_q};
+    for (int a = 0; a < 5 && n > 0; ++a)
+        CU_TRY(cudaMemcpyAsync(plan->stage[a], src[a], sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, plan->stream));
+    rc = wcsim_clear(plan);
+    if (rc) return rc;
+    const wcsim_depos d{plan->stage[0], plan->stage[1], plan->stage[2], plan->stage[3], plan->stage[4]};
+    rc = wcsim_raster_scatter(plan, &d, n, 0ull, seed, fluctuate, nullptr);
+    if (rc) return rc;
+    if (noise) {
+        rc = wcsim_arm_noise(plan, nullptr, noise_seed);
+        if (rc) return rc;
+    }
+    rc = wcsim_convolve(plan);
+    if (rc) return rc;
+    CU_TRY(cudaMemcpyAsync(host_M, plan->M, sizeof(float) * (size_t)plan->n_wires * plan->n_ticks,
+                           cudaMemcpyDeviceToHost, plan->stream));
+    CU_TRY(cudaStreamSynchronize(plan->stream));
+    return WCSIM_OK;
+}
+
+int wcsim_debug_philox(const unsigned int *dev_ctr, const unsigned int *dev_key, unsigned int *dev_out, long long n,
+                       void *cuda_stream)
+{
+    if (n < 0 || (n > 0 && (!dev_ctr || !dev_key || !dev_out))) return WCSIM_EINVAL;
+    CU_TRY(launch_debug_philox(dev_ctr, dev_key, dev_out, n, (cudaStream_t)cuda_stream));
+    return WCSIM_OK;
+}
+
+int wcsim_debug_binomial(const double *dev_N, const double *dev_p, const unsigned int *dev_w, double *dev_k,
+                         long long n, void *cuda_stream)
+{
+    if (n < 0 || (n > 0 && (!dev_N || !dev_p || !dev_w || !dev_k))) return WCSIM_EINVAL;
+    CU_TRY(launch_debug_binomial(dev_N, dev_p, dev_w, dev_k, n, (cudaStream_t)cuda_stream));
+    return WCSIM_OK;
+}
+
+int wcsim_debug_response_spectrum(wcsim_plan *plan, float *host_out)
+{
+    if (!plan || !host_out) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    const int nk = plan->pad_t / 2 + 1;
+    CU_TRY(cudaMemcpy2DAsync(host_out, sizeof(float2) * (size_t)nk, plan->Rhat, sizeof(float2) * (size_t)plan->spec_stride,
+                             sizeof(float2) * (size_t)nk, (size_t)plan->pad_w, cudaMemcpyDeviceToHost, plan->stream));
+    CU_TRY(cudaStreamSynchronize(plan->stream));
+    return WCSIM_OK;
+}
+
+int wcsim_set_profiling(wcsim_plan *plan, int enable)
+{
+    if (!plan) return WCSIM_EINVAL;
+    plan->profiling = enable != 0;
+    return WCSIM_OK;
+}
+
+int wcsim_get_stage_times(wcsim_plan *plan, double *ms, unsigned long long *calls, int reset)
+{
+    if (!plan || !ms || !calls) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    const int rc = harvest_spans(plan);
+    if (rc) return rc;
+    for (int s = 0; s < WCSIM_N_STAGES; ++s) {
+        ms[s] = plan->stage_ms[s];
+        calls[s] = plan->stage_calls[s];
+        if (reset) {
+            plan->stage_ms[s] = 0.0;
+            plan->stage_calls[s] = 0;
+        }
+    }
+    return WCSIM_OK;
+}
+
+int wcsim_get_launch_count(const wcsim_plan *plan, unsigned long long *out)
+{
+    if (!plan || !out) return WCSIM_EINVAL;
+    *out = plan->launches;
+    return WCSIM_OK;
+}
+
+const char *wcsim_strerror(int status)
+{
+    switch (status) {
+    case WCSIM_OK: return "ok";
+    case WCSIM_EINVAL: return "invalid argument";
+    case WCSIM_ENOMEM: return "out of host or device memory";
+    case WCSIM_ECUDA: return "CUDA runtime or kernel failure (see wcsim_last_cuda_error)";
+    case WCSIM_ESTATE: return "call not valid in the plan's current state";
+    default: return "unknown wcsim status";
+    }
+}
+
+int wcsim_last_cuda_error(void) { return tls_cuda_error; }
+
+const char *wcsim_version(void) { return "wcsim 0.1 (sm_100a)"; }
+
+} // extern "C"

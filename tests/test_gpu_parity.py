@@ -1,0 +1,370 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the fp64 CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json north_star's:
+  fluctuation off: rel-L2 <= 1e-5 and max-abs <= 1e-4 max|.| (checked on S and on M separately)
+  fluctuation on : integer grids equal bin by bin, flipped bins <= 1e-6 of drawn bins
+Sizes here are small enough for the oracle to finish in seconds while spanning several FFT tiles, several scatter
+tiles and ragged tails; full-size configs are in test_gpu_configs.py."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+REL_L2, MAX_ABS = 1e-5, 1e-4
+
+
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.fail("these tests need a CUDA device (run with -m gpu on the B200 box)")
+
+
+@pytest.fixture(scope="module")
+def B():
+    _need_gpu()
+    from paper_2203_02479_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def O():
+    import oracle
+    oracle.lib()
+    return oracle
+
+
+def to_dev(depos):
+    return {k: torch.from_numpy(np.ascontiguousarray(v)).cuda() for k, v in depos.items()}
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+def assert_close(got, ref, what, rel=REL_L2, mabs=MAX_ABS):
+    got = np.asarray(got, dtype=np.float64)
+    r = rel_l2(got, ref)
+    m = float(np.max(np.abs(got - ref)))
+    scale = float(np.max(np.abs(ref)))
+    assert r <= rel, "%s: rel-L2 %.3e > %.1e" % (what, r, rel)
+    assert m <= mabs * scale, "%s: max-abs %.3e > %.1e * %.3e" % (what, m, mabs, scale)
+    return r, m / max(scale, 1e-300)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# pieces
+# ---------------------------------------------------------------------------------------------------------------
+def test_philox_matches_oracle(B, O):
+    rng = np.random.default_rng(5)
+    n = 4096
+    ctr = rng.integers(0, 2**32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2**32, size=(n, 2), dtype=np.uint64).astype(np.uint32)
+    ctr[0] = 0
+    key[0] = 0
+    ctr[1] = 0xFFFFFFFF
+    key[1] = 0xFFFFFFFF
+    d_ctr = torch.from_numpy(ctr.view(np.int32)).cuda()
+    d_key = torch.from_numpy(key.view(np.int32)).cuda()
+    d_out = torch.zeros((n, 4), dtype=torch.int32, device="cuda")
+    B.wcsim_debug_philox(d_ctr, d_key, d_out, n)
+    torch.cuda.synchronize()
+    got = d_out.cpu().numpy().view(np.uint32)
+    for i in list(range(64)) + [n - 1]:
+        assert np.array_equal(got[i], O.philox4x32_10(ctr[i], key[i]))
+    assert got[0].tolist() == [0x6627E8D5, 0xE169C58D, 0xBC57AC4C, 0x9B00DBD8]
+
+
+def test_binomial_sampler_matches_oracle(B, O):
+    rng = np.random.default_rng(7)
+    n = 200_000
+    N = np.floor(np.exp(rng.uniform(0, np.log(2e5), n)))
+    p = np.where(rng.random(n) < 0.5, rng.random(n), np.exp(rng.uniform(np.log(1e-9), 0, n)))
+    w = rng.integers(0, 2**32, size=n, dtype=np.uint64).astype(np.uint32)
+    # edge cases: N = 0, p = 0, p = 1, p just above and below 1/2, mu at the branch point, extreme words
+    N[:8] = [0, 10, 10, 1000, 1000, 32, 5000, 5000]
+    p[:8] = [0.3, 0.0, 1.0, 0.5, np.nextafter(0.5, 1), 0.5, 1e-300, 1 - 1e-16]
+    w[8:12] = [0, 0xFFFFFFFF, 0x80000000, 0x7FFFFFFF]
+    dN, dp = torch.from_numpy(N).cuda(), torch.from_numpy(p).cuda()
+    dw = torch.from_numpy(w.view(np.int32)).cuda()
+    dk = torch.zeros(n, dtype=torch.float64, device="cuda")
+    B.wcsim_debug_binomial(dN, dp, dw, dk, n)
+    torch.cuda.synchronize()
+    got = dk.cpu().numpy()
+    ref = np.array([O.binomial(N[i], p[i], int(w[i])) for i in range(n)])
+    bad = np.flatnonzero(got != ref)
+    assert bad.size <= max(1, int(1e-6 * n)), "sampler differs in %d of %d draws, first %s" % (
+        bad.size, n, [(N[i], p[i], w[i], got[i], ref[i]) for i in bad[:5]])
+    assert np.all(got >= 0) and np.all(got <= N)
+
+
+def test_response_spectrum(B):
+    from paper_2203_02479_b200 import synth
+    R = synth.response()
+    with B.Plan(64, 512, R, pad=(128, 1024)) as p:
+        got = p.response_spectrum()
+    emb = np.zeros((128, 1024))
+    c = (R.shape[0] - 1) // 2
+    for dx in range(-c, c + 1):
+        emb[dx % 128, : R.shape[1]] += R[dx + c].astype(np.float64)
+    ref = np.fft.rfft2(emb) / (128 * 1024)
+    assert rel_l2(got, ref) < 2e-7
+    assert np.max(np.abs(got - ref)) < 2e-7 * np.max(np.abs(ref))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# configs[0]: the whole path, fluctuation off
+# ---------------------------------------------------------------------------------------------------------------
+def test_config0_raster_and_convolve(B, O):
+    from paper_2203_02479_b200 import synth
+    cfg = synth.config(0)
+    pl = cfg["planes"][0]
+    S_ref, _, st_ref = O.raster_scatter(pl["n_wires"], pl["n_ticks"], pl["depos"], fluctuate=False)
+    M_ref = O.convolve_direct(S_ref, pl["response"])
+    for mode in (B.WCSIM_SCATTER_ATOMIC, B.WCSIM_SCATTER_TILED):
+        with B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]),
+                    scatter_mode=mode) as p:
+            p.raster_scatter(to_dev(pl["depos"]), seed=1, fluctuate=False)
+            p.convolve()
+            p.sync()
+            S = p.charge().cpu().numpy()
+            M = p.output().cpu().numpy()
+            st = p.stats()
+        assert_close(S, S_ref, "S mode %d" % mode)
+        assert_close(M, M_ref, "M mode %d" % mode)
+        assert st["bins_drawn"] == st_ref["drawn"] and st["depos_skipped"] == 0
+
+
+def test_convolve_alone_matches_definition(B, O):
+    """Random dense S written straight into the plan's buffer: isolates a4-a6 from the raster."""
+    from paper_2203_02479_b200 import synth
+    rng = np.random.default_rng(11)
+    for (nw, nt, pw, pt, rw, rt) in [(64, 512, 128, 1024, 21, 200), (50, 301, 64, 512, 5, 40), (16, 40, 32, 64, 3, 9)]:
+        R = synth.response(rw, rt)
+        S = (rng.standard_normal((nw, nt)) * (rng.random((nw, nt)) < 0.2)).astype(np.float32)
+        M_ref = O.convolve_direct(S.astype(np.float64), R)
+        with B.Plan(nw, nt, R, pad=(pw, pt)) as p:
+            p.charge().copy_(torch.from_numpy(S).cuda())
+            p.convolve()
+            p.sync()
+            M = p.output().cpu().numpy()
+            assert np.array_equal(p.charge().cpu().numpy(), S), "S must be preserved"
+        assert_close(M, M_ref, "M %dx%d" % (nw, nt))
+
+
+def test_delta_reproduces_response(B):
+    from paper_2203_02479_b200 import synth
+    R = synth.response()
+    with B.Plan(64, 512, R) as p:
+        S = torch.zeros((64, 512), device="cuda")
+        S[30, 100] = 1.0
+        p.charge().copy_(S)
+        p.convolve()
+        p.sync()
+        M = p.output().cpu().numpy().astype(np.float64)
+    ref = np.zeros((64, 512))
+    ref[20:41, 100:300] = R
+    assert np.max(np.abs(M - ref)) <= 1e-5 * np.max(np.abs(R))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# fluctuation on: integer grids
+# ---------------------------------------------------------------------------------------------------------------
+def _fluct_case(B, O, n_wires, n_ticks, R, depos, seed, id_base=0, mode=0):
+    S_ref, tot_ref, st_ref = O.raster_scatter(n_wires, n_ticks, depos, seed=seed, fluctuate=True, id_base=id_base,
+                                              want_totals=True)
+    n = depos["t0"].shape[0]
+    with B.Plan(n_wires, n_ticks, R, scatter_mode=mode) as p:
+        tot = torch.full((n,), -12345, dtype=torch.int32, device="cuda")
+        p.raster_scatter(to_dev(depos), seed=seed, fluctuate=True, depo_id_base=id_base, dev_depo_totals=tot)
+        p.sync()
+        S = p.charge().cpu().numpy().astype(np.float64)
+        st = p.stats()
+        tot = tot.cpu().numpy()
+    assert np.max(np.abs(S_ref)) < 2**24, "integer-valued fp32 adds must stay exact"
+    flips = int(np.count_nonzero(S != S_ref))
+    assert st["bins_drawn"] == st_ref["drawn"]
+    assert flips <= 1e-6 * st_ref["drawn"], "%d bins differ of %d drawn" % (flips, st_ref["drawn"])
+    assert int(np.count_nonzero(tot != tot_ref)) <= flips
+    return S, S_ref
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_fluctuation_integer_grid_exact(B, O, mode):
+    from paper_2203_02479_b200 import synth
+    cfg = synth.config(1, n_depos=20_000)
+    pl = cfg["planes"][0]
+    S, S_ref = _fluct_case(B, O, pl["n_wires"], pl["n_ticks"], synth.response(5, 16), pl["depos"], seed=1, mode=mode)
+    assert np.all(S == np.rint(S))
+    # charge mean: sum of draws against sum N p (independent binomials: var <= sum N p)
+    q = pl["depos"]["q"].astype(np.float64)
+    assert abs(S.sum() - S_ref.sum()) == 0
+    assert abs(S.sum() - np.floor(q + 0.5).sum() * 0.9946) < 0.02 * q.sum()
+
+
+def test_fluctuation_negative_charge_big_ids_and_wide_patches(B, O):
+    from paper_2203_02479_b200 import synth
+    d = synth.depos_uniform_box(300, gen_seed=3)
+    d["q"][::3] *= -1.0
+    d["sigma_t"][:20] = 14.0  # 85-tick patches: several 31-bin chunks
+    d["sigma_x"][:10] = 12.0  # 73-wire patches, clipped by the 64-wire grid
+    d["sigma_t"][20:25] = 0.0
+    d["sigma_x"][25:30] = 0.0
+    d["q"][30] = 0.2  # N = 0
+    d["q"][31] = 0.5  # N = 1 (round half up)
+    for mode in (0, 1):
+        _fluct_case(B, O, 64, 512, synth.response(3, 8), d, seed=0xDEADBEEFCAFE, id_base=(1 << 40) + 17, mode=mode)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# edge cases of the raster
+# ---------------------------------------------------------------------------------------------------------------
+def test_raster_edge_cases(B, O):
+    from paper_2203_02479_b200 import synth
+    f = np.float32
+    depos = {
+        #            inside  edge-lo  edge-hi  off-grid  sigma0  on-edge  nan     inf-q   neg-sigma  wide
+        "t0": np.array([100.3, 0.2, 510.9, -50.0, 77.5, 64.0, np.nan, 10.0, 10.0, 250.0], dtype=f),
+        "x0": np.array([30.7, 0.1, 63.8, 200.0, 12.5, 8.0, 5.0, 5.0, 5.0, 31.0], dtype=f),
+        "sigma_t": np.array([1.5, 2.0, 2.0, 1.0, 0.0, 1.0, 1.0, 1.0, -1.0, 40.0], dtype=f),
+        "sigma_x": np.array([0.8, 1.0, 1.0, 1.0, 0.0, 1.0, 1.0, 1.0, 1.0, 15.0], dtype=f),
+        "q": np.array([1000, 2000, 3000, 4000, 5000, 6000, 7000, np.inf, 9000, 1e5], dtype=f),
+    }
+    S_ref, _, st_ref = O.raster_scatter(64, 512, depos, fluctuate=False)
+    assert st_ref["skipped"] == 3
+    for mode in (0, 1):
+        with B.Plan(64, 512, synth.response(3, 8), scatter_mode=mode) as p:
+            p.raster_scatter(to_dev(depos), fluctuate=False)
+            p.sync()
+            S = p.charge().cpu().numpy()
+            st = p.stats()
+            assert st == {"depos_skipped": 3, "bins_drawn": st_ref["drawn"]}
+            assert_close(S, S_ref, "edge cases mode %d" % mode)
+            assert np.all(np.isfinite(S))
+            # accumulation across calls, n = 0, clear
+            p.raster_scatter(to_dev(depos), fluctuate=False)
+            p.raster_scatter(to_dev(depos), n=0)
+            p.sync()
+            assert_close(p.charge().cpu().numpy(), 2 * S_ref, "accumulate mode %d" % mode)
+            p.clear()
+            p.sync()
+            assert float(p.charge().abs().max()) == 0.0
+
+
+def test_odd_tick_count_uses_scalar_rows(B, O):
+    from paper_2203_02479_b200 import synth
+    rng = np.random.default_rng(3)
+    R = synth.response(5, 30)
+    d = synth.depos_uniform_box(50, gen_seed=9)
+    d["t0"] = (d["t0"] * 0.5).astype(np.float32)
+    S_ref, _, _ = O.raster_scatter(64, 255, d, fluctuate=False)
+    M_ref = O.convolve_direct(S_ref, R)
+    with B.Plan(64, 255, R) as p:
+        p.raster_scatter(to_dev(d), fluctuate=False)
+        p.convolve()
+        p.sync()
+        assert_close(p.charge().cpu().numpy(), S_ref, "S odd ticks")
+        assert_close(p.output().cpu().numpy(), M_ref, "M odd ticks")
+
+
+def test_tiled_mode_is_bitwise_reproducible(B):
+    from paper_2203_02479_b200 import synth
+    cfg = synth.config(1, n_depos=30_000)
+    pl = cfg["planes"][0]
+    d = to_dev(pl["depos"])
+    outs = []
+    with B.Plan(pl["n_wires"], pl["n_ticks"], synth.response(3, 8), scatter_mode=B.WCSIM_SCATTER_TILED) as p:
+        for _ in range(3):
+            p.clear()
+            p.raster_scatter(d, fluctuate=False)
+            p.sync()
+            outs.append(p.charge().clone())
+    assert torch.equal(outs[0], outs[1]) and torch.equal(outs[0], outs[2])
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# noise
+# ---------------------------------------------------------------------------------------------------------------
+def test_noise_alone_and_fused(B, O):
+    """S = 0 => M = N: the noise is checked on its own, against the oracle's full rows."""
+    from paper_2203_02479_b200 import synth
+    R = synth.response(5, 30)
+    nw, nt = 40, 700
+    with B.Plan(nw, nt, R) as p:
+        P = p.pad_t
+        ref = O.noise_add(np.zeros((nw, nt)), P, seed=1)
+        p.clear_output()
+        p.add_noise(seed=1)
+        p.sync()
+        N1 = p.output().cpu().numpy()
+        assert_close(N1, ref, "noise standalone", rel=2e-5)
+        # fused into the inverse transform of a convolution of S = 0
+        p.arm_noise(seed=1)
+        p.convolve()
+        p.sync()
+        N2 = p.output().cpu().numpy()
+        assert_close(N2, ref, "noise fused", rel=2e-5)
+        # a second convolve is noise free again (the arm is cleared)
+        p.convolve()
+        p.sync()
+        assert float(p.output().abs().max()) == 0.0
+        # custom amplitude spectrum and another seed
+        amp = np.linspace(1.0, 0.0, P // 2 + 1).astype(np.float32)
+        ref2 = O.noise_add(np.zeros((nw, nt)), P, seed=99, amp=amp.astype(np.float64))
+        p.clear_output()
+        p.add_noise(amp=amp, seed=99)
+        p.sync()
+        assert_close(p.output().cpu().numpy(), ref2, "noise custom amp", rel=2e-5)
+    rms = float(np.sqrt(np.mean(N1.astype(np.float64) ** 2)))
+    assert abs(rms - 0.4743) < 0.02
+
+
+def test_noise_plus_signal_both_orders_agree(B, O):
+    from paper_2203_02479_b200 import synth
+    cfg = synth.config(0)
+    pl = cfg["planes"][0]
+    with B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"])) as p:
+        d = to_dev(pl["depos"])
+        p.raster_scatter(d, fluctuate=False)
+        p.convolve()
+        p.add_noise(seed=5)
+        p.sync()
+        A = p.output().cpu().numpy().astype(np.float64)
+        p.arm_noise(seed=5)
+        p.convolve()
+        p.sync()
+        Bm = p.output().cpu().numpy().astype(np.float64)
+    assert rel_l2(A, Bm) < 1e-6
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# host-buffer entry point and error behaviour
+# ---------------------------------------------------------------------------------------------------------------
+def test_simulate_host_end_to_end(B, O):
+    from paper_2203_02479_b200 import synth
+    cfg = synth.config(0)
+    pl = cfg["planes"][0]
+    S_ref, _, _ = O.raster_scatter(pl["n_wires"], pl["n_ticks"], pl["depos"], fluctuate=False)
+    M_ref = O.convolve_direct(S_ref, pl["response"])
+    host = {k: torch.from_numpy(v).pin_memory() for k, v in pl["depos"].items()}
+    out = torch.empty((pl["n_wires"], pl["n_ticks"]), dtype=torch.float32).pin_memory()
+    with B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"]) as p:
+        p.simulate_host(host, out, fluctuate=False)
+        assert_close(out.numpy(), M_ref, "simulate_host")
+        p.simulate_host(host, out, fluctuate=False)  # S is cleared inside: same answer
+        assert_close(out.numpy(), M_ref, "simulate_host again")
+
+
+def test_error_codes(B):
+    from paper_2203_02479_b200 import synth
+    R = synth.response()
+    for kw in (dict(pad=(64, 1024)), dict(pad=(128, 512)), dict(pad=(96, 1024)), dict(nsigma=0.0),
+               dict(scatter_mode=7)):
+        with pytest.raises(B.WcsimError) as e:
+            B.Plan(64, 512, R, **kw)
+        assert e.value.status == B.WCSIM_EINVAL
+    with pytest.raises(B.WcsimError):
+        B.Plan(64, 512, R[:20])  # even response width
+    with B.Plan(64, 512, R) as p:
+        assert (p.pad_w, p.pad_t) == (128, 1024)
+        with pytest.raises(B.WcsimError):
+            p.set_scatter_mode(3)
