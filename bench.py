@@ -1,0 +1,371 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the hot path M = R (*) S + N of arXiv 2203.02479 on B200.
+
+    python bench.py --gpus N --steps K --warmup W            # this repo's CUDA path (libwcsim.so through the C ABI)
+    python bench.py --impl reference --steps K --warmup W    # the fp64 CPU oracle, as it stands, on the host cores
+
+A "step" is one plane-event of BASELINE.json configs[1] (800 wires x 6000 ticks padded to 1024 x 8192, 100k depos,
+binomial fluctuation on): clear S, raster + fluctuate + scatter-add, FFT-convolve with the response.  `value` is
+depositions per second through that whole path (so ms_per_step is the "ms per plane-event" of BASELINE.json's
+metric), inputs resident in HBM; `e2e` is the same through wcsim_simulate_host with pinned HOST buffers, the
+host<->device copies inside the timed region.  L2 (126 MB) is flushed between timed steps by writing a 256 MB
+buffer, outside the per-step CUDA-event pairs.  Multi-GPU: replicas only, one process per GPU.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC, UNIT = "depos_per_sec_plane_event", "depos/s"
+FLUSH_BYTES = 256 << 20
+
+
+def load_peaks():
+    """Measured roofline denominators (driver-written MEASURED_PEAKS.json), else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            p = json.load(f)
+        return {"hbm_gbs": float(p["hbm_gbs"]), "source": "measured (MEASURED_PEAKS.json)",
+                "sm_max_mhz": float(p.get("sm_max_mhz", 1965.0))}
+    except Exception:
+        return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)", "sm_max_mhz": 1965.0}
+
+
+def stage_bytes(pl):
+    """Algorithmic HBM bytes of each convolution kernel for one plane-event."""
+    nw, nt, pw, pt = pl["n_wires"], pl["n_ticks"], pl["pad_w"], pl["pad_t"]
+    nk = pt // 2 + 1
+    grid, spec, rhat = nw * nt * 4, nw * nk * 8, pw * nk * 8
+    return {"rows_forward": grid + spec, "cols": 2 * spec + rhat, "rows_inverse": spec + grid}
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons of one GPU while the timed region runs (NVML, in a thread)."""
+
+    BAD = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20}
+    NOTE = {"sw_power_cap": 0x4}
+
+    def __init__(self, index, period=0.005):
+        self.index, self.period = index, period
+        self.mhz, self.reasons, self.max_mhz = [], 0, None
+        self._stop = threading.Event()
+        self._thread = None
+        self._h = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._h = None
+
+    def sample(self):
+        if self._h is None:
+            return
+        try:
+            self.mhz.append(float(self._nv.nvmlDeviceGetClockInfo(self._h, self._nv.NVML_CLOCK_SM)))
+            try:
+                r = self._nv.nvmlDeviceGetCurrentClocksEventReasons(self._h)
+            except Exception:
+                r = self._nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+            self.reasons |= int(r)
+        except Exception:
+            pass
+
+    def _run(self):
+        while not self._stop.is_set():
+            self.sample()
+            self._stop.wait(self.period)
+
+    def start(self):
+        self.sample()
+        self._thread = threading.Thread(target=self._run, daemon=True)
+        self._thread.start()
+
+    def stop(self):
+        self.sample()
+        self._stop.set()
+        if self._thread:
+            self._thread.join()
+
+    def summary(self):
+        names = [n for n, bit in {**self.BAD, **self.NOTE}.items() if self.reasons & bit]
+        if not self.mhz:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unsampled"], "samples": 0}
+        return {"sm_mhz": statistics.median(self.mhz), "sm_max_mhz": self.max_mhz, "reasons": names,
+                "samples": len(self.mhz)}
+
+
+# --------------------------------------------------------------------------------------------------------------------
+# this repo's arm
+# --------------------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import numpy as np
+    import torch
+    from paper_2203_02479_b200 import binding as B, replicas, synth
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    rank, local_rank, world = replicas.env_world()
+    if world != args.gpus and world > 1:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d" % (args.gpus, world))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    replicas.init("nccl")
+    B.lib()  # fails loudly here if libwcsim.so cannot be built or loaded
+
+    cfg = synth.config(args.config)
+    pl = cfg["planes"][0]
+    n_depos = int(pl["depos"]["t0"].shape[0])
+    fluct = bool(cfg["fluctuate"]) and not args.no_fluct
+    mode = B.WCSIM_SCATTER_TILED if args.scatter == "tiled" else B.WCSIM_SCATTER_ATOMIC
+    stream = torch.cuda.current_stream()
+    plan = B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]), nsigma=cfg["nsigma"],
+                  scatter_mode=mode, stream=stream)
+    d = {k: torch.from_numpy(v).to(dev) for k, v in pl["depos"].items()}
+    flush = torch.empty(FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
+
+    def step():
+        plan.clear()
+        plan.raster_scatter(d, seed=cfg["fluct_seed"], fluctuate=fluct)
+        plan.convolve()
+
+    def timed(fn, k, sampler=None):
+        """k steps; L2 flushed before each; returns the per-step device times in ms (CUDA events on the stream)."""
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
+        replicas.barrier()
+        torch.cuda.synchronize()
+        if sampler:
+            sampler.start()
+        for a, b in ev:
+            flush.fill_(1.0)
+            a.record(stream)
+            fn()
+            b.record(stream)
+        if sampler:
+            sampler.sample()
+        torch.cuda.synchronize()
+        if sampler:
+            sampler.stop()
+        replicas.barrier()
+        return [a.elapsed_time(b) for a, b in ev]
+
+    # ---- device-resident arm -------------------------------------------------------------------------------------
+    plan.set_profiling(True)
+    for _ in range(args.warmup):
+        flush.fill_(1.0)
+        step()
+    torch.cuda.synchronize()
+    plan.stage_times(reset=True)
+    launches0 = plan.launch_count()
+    sampler = ClockSampler(local_rank if "CUDA_VISIBLE_DEVICES" not in os.environ else
+                           int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank]))
+    per_step = timed(step, args.steps, sampler)
+    launches = plan.launch_count() - launches0
+    stages = plan.stage_times(reset=True)
+    plan.set_profiling(False)
+    local_s = sum(per_step) * 1e-3
+    value, slowest_s = replicas.whole_job_throughput(n_depos * args.steps, local_s, dev)
+    ms_per_step = slowest_s * 1e3 / args.steps
+
+    # the same loop without the per-stage event pairs (they sit between the kernels): reported for information
+    per_step_plain = timed(step, args.steps)
+
+    # ---- end to end through the C ABI with host buffers -------------------------------------------------------------
+    host = {k: torch.from_numpy(v).pin_memory() for k, v in pl["depos"].items()}
+    host_M = torch.empty((pl["n_wires"], pl["n_ticks"]), dtype=torch.float32).pin_memory()
+
+    def step_e2e():
+        plan.simulate_host(host, host_M, seed=cfg["fluct_seed"], fluctuate=fluct)
+
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    for _ in range(min(args.warmup, 3)):
+        step_e2e()
+    replicas.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        step_e2e()  # synchronises before returning: host_M holds this step's M
+    torch.cuda.synchronize()
+    e2e_local = time.perf_counter() - t0
+    replicas.barrier()
+    e2e_value, e2e_slowest = replicas.whole_job_throughput(n_depos * e2e_steps, e2e_local, dev)
+    h2d, d2h = 5 * 4 * n_depos, 4 * pl["n_wires"] * pl["n_ticks"]
+
+    # ---- roofline of the dominant kernel --------------------------------------------------------------------------
+    peaks = load_peaks()
+    sb = stage_bytes(pl)
+    stage_rows = []
+    for name in ("raster", "rows_forward", "cols", "rows_inverse"):
+        ms, calls = stages[name]
+        if calls == 0:
+            continue
+        avg = ms / calls
+        row = {"stage": name, "ms": avg}
+        if name in sb:
+            gbs = sb[name] / (avg * 1e-3) / 1e9
+            row.update({"bound": "hbm", "bytes": sb[name], "achieved_gbs": gbs, "frac": gbs / peaks["hbm_gbs"]})
+        else:
+            row.update({"bound": "alu", "depos_per_s": n_depos / (avg * 1e-3)})
+        stage_rows.append(row)
+    conv_ms = sum(r["ms"] for r in stage_rows if r["stage"] in sb)
+    conv_bytes = sum(sb.values())
+    conv_gbs = conv_bytes / (conv_ms * 1e-3) / 1e9
+    dom = max((r for r in stage_rows if r["stage"] in sb), key=lambda r: r["ms"])
+    roofline = {"kernel": dom["stage"], "bound": "hbm", "achieved": dom["achieved_gbs"], "peak": peaks["hbm_gbs"],
+                "unit": "GB/s", "frac": dom["frac"], "traffic": TRAFFIC.get(dom["stage"]),
+                "peak_source": peaks["source"],
+                "convolve": {"ms": conv_ms, "bytes": conv_bytes, "achieved": conv_gbs,
+                             "frac": conv_gbs / peaks["hbm_gbs"], "frac_of_8TBs_nominal": conv_gbs / 8000.0},
+                "stages": stage_rows}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if not fluct else "f32 (f64 fluctuation weights and sampler)", "data": "synthetic",
+        "config": {"workload": cfg["name"] + (", fluctuation on" if fluct else ", fluctuation off"),
+                   "grid": [pl["n_wires"], pl["n_ticks"]], "pad": [pl["pad_w"], pl["pad_t"]],
+                   "response": list(pl["response"].shape), "depos": n_depos, "scatter": args.scatter,
+                   "parallelism": "replicas x%d" % world, "l2": "flushed between timed steps (256 MB write)"},
+        "clocks": sampler.summary(),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": e2e_slowest * 1e3 / e2e_steps, "steps": e2e_steps},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "ms_per_step_median": statistics.median(per_step),
+        "ms_per_step_min": min(per_step),
+        "ms_per_step_without_stage_events": sum(per_step_plain) / len(per_step_plain),
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(cfg, budget_s=args.cpu_budget)
+    if rank == 0 and world == 1 and args.cufft:
+        out["cufft_comparator"] = cufft_comparator(pl, dev, flush)
+    plan.destroy()
+    replicas.shutdown()
+    if rank == 0:
+        print(json.dumps(out))
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+# (profiles/r01_ncu_full.md); None until a capture of the current kernels exists
+TRAFFIC = {"rows_forward": None, "cols": None, "rows_inverse": None}
+
+
+def cufft_comparator(pl, dev, flush):
+    """cuFFT (through torch.fft) R2C -> pointwise multiply -> C2R on the same padded sizes: comparator only."""
+    import torch
+    nw, nt, pw, pt = pl["n_wires"], pl["n_ticks"], pl["pad_w"], pl["pad_t"]
+    S = torch.rand((nw, nt), device=dev)
+    Rh = torch.fft.rfft2(torch.rand((pw, pt), device=dev))
+    ms = []
+    for it in range(8):
+        flush.fill_(1.0)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        M = torch.fft.irfft2(torch.fft.rfft2(S, s=(pw, pt)) * Rh, s=(pw, pt))[:nw, :nt]
+        b.record()
+        torch.cuda.synchronize()
+        if it >= 3:
+            ms.append(a.elapsed_time(b))
+    return {"ms": statistics.median(ms), "what": "torch.fft.rfft2 (cuFFT) * Rhat -> irfft2, crop; comparator only"}
+
+
+# --------------------------------------------------------------------------------------------------------------------
+# the oracle on the host cores (cpu_baseline leg and --impl reference)
+# --------------------------------------------------------------------------------------------------------------------
+def oracle_step(cfg, O):
+    """One plane-event of the workload through oracle/ as it stands: raster+fluctuate+scatter, FFT-route convolve."""
+    pl = cfg["planes"][0]
+    S, _, _ = O.raster_scatter(pl["n_wires"], pl["n_ticks"], pl["depos"], seed=cfg["fluct_seed"],
+                               fluctuate=cfg["fluctuate"], nsigma=cfg["nsigma"])
+    return O.convolve_fft(S, pl["response"], pl["pad_w"], pl["pad_t"])
+
+
+def cpu_baseline(cfg, budget_s=15.0):
+    import oracle as O
+    O.lib()
+    n_depos = int(cfg["planes"][0]["depos"]["t0"].shape[0])
+    oracle_step(cfg, O)  # page in
+    t0 = time.perf_counter()
+    reps = 0
+    while reps < 1 or (time.perf_counter() - t0 < budget_s and reps < 50):
+        oracle_step(cfg, O)
+        reps += 1
+    dt = time.perf_counter() - t0
+    return {"value": n_depos * reps / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+            "ms_per_step": dt * 1e3 / reps,
+            "sample": "%d whole plane-events of the same workload (all %d depos, full grid), fp64, "
+                      "FFT-route convolution" % (reps, n_depos)}
+
+
+def run_reference(args):
+    """The reference arm of this tier is the oracle (there is no reference code): timed on the host, rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2203_02479_b200 import synth
+    import oracle as O
+    O.lib()
+    cfg = synth.config(args.config)
+    pl = cfg["planes"][0]
+    n_depos = int(pl["depos"]["t0"].shape[0])
+    steps = max(1, min(args.steps, args.ref_max_steps))
+    for _ in range(max(1, min(args.warmup, 2))):
+        oracle_step(cfg, O)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle_step(cfg, O)
+    dt = time.perf_counter() - t0
+    value = n_depos * steps / dt
+    sample = ("each step = one whole plane-event of the workload (all %d depos, full grid); %d of the %d requested "
+              "steps run to stay within minutes" % (n_depos, steps, args.steps))
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3 / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"] + ", fluctuation on", "grid": [pl["n_wires"], pl["n_ticks"]],
+                   "pad": [pl["pad_w"], pl["pad_t"]], "response": list(pl["response"].shape), "depos": n_depos,
+                   "parallelism": "host cores (OpenMP)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index of the timed workload")
+    ap.add_argument("--scatter", default="atomic", choices=["atomic", "tiled"])
+    ap.add_argument("--no-fluct", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=200)
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cufft", action="store_true", help="also time the cuFFT comparator")
+    ap.add_argument("--ref-max-steps", type=int, default=20)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3  # timing rule: at least 3 warm-up steps
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
