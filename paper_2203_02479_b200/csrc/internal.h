@@ -17,9 +17,12 @@ struct GridDims {
 struct Counters {
     unsigned long long depos_skipped;
     unsigned long long bins_drawn;
+    unsigned long long next_batch; // work counter of the atomic-mode raster kernel; the kernel leaves it at 0
+    unsigned long long warps_done;
 };
 
 // ---- raster.cu ----
+cudaError_t raster_configure(); // shared-memory attributes of the raster kernels (once per plan)
 // a1-a3, atomic mode: S[wire][tick] += patch of every depo (red.global.add.f32)
 cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
                                  double nsigma, float *S, int *depo_totals, Counters *counters, int sm_count,

@@ -1,11 +1,20 @@
 // raster.cu -- steps a1-a3 of the hot path: Raster, charge fluctuation, Scatter-add
 // (Section 2.2; Section 3.1 for the binomial fluctuation).
 //
-// One warp owns one depo at a time (the SoA layout of PAPER.md:72 makes the depo the unit of parallelism).  The
-// lanes evaluate erf at consecutive bin edges of one axis, a shuffle turns neighbouring edges into bin weights
-// ("erf bin edges once per axis"), and the patch p_ij = wt_i wx_j is formed in registers: lanes run along the tick
-// axis (contiguous in S), the wire index is broadcast by shuffle.  Nothing of the patch is ever written to HBM
-// except the final adds into S.
+// Atomic mode (raster_batch_kernel): a warp takes 32 depos at a time, one per lane (the SoA layout of PAPER.md:72
+// makes the depo the unit of parallelism and the loads coalesce).  Each lane works out its depo's patch extent; a warp
+// scan lays all bin EDGES of the 32 patches end to end and the lanes evaluate erf over that flat list ("erf bin edges
+// once per axis"), leaving the values in the warp's shared-memory scratch; then the lanes walk the flat list of all
+// BINS of the 32 patches, 32 at a time, each forming p_ij = wt_i wx_j from four edge values.  All lanes are busy
+// whatever the patch shapes are (patches are 1-5 wires x 1-16 ticks in BASELINE.json's configs).  With fluctuation on,
+// bins are first sorted by the routine that will draw them (inversion / AS 241 central / AS 241 tail) into three
+// per-warp queues and drawn 32 at a time from one queue, so the fp64 sampler runs without divergence.  A patch with
+// more edges than the scratch holds falls back to the one-warp-per-depo walk (raster_depo), which chunks it.
+// Nothing of a patch is ever written to HBM except the final adds into S.
+//
+// raster_depo (big patches, tiled mode): one warp owns one depo.  The lanes evaluate erf at consecutive bin edges of
+// one axis, a shuffle turns neighbouring edges into bin weights, lanes run along the tick axis (contiguous in S),
+// the wire index is broadcast by shuffle.
 //
 //   fluctuate = 0: fp32 weights (erff), value q * (wt * wx)
 //   fluctuate = 1: fp64 weights (erf), p = wt * wx, integer draw B(N, p; Philox word of the absolute bin)
@@ -158,38 +167,252 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v)
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// atomic mode: persistent grid, warp w takes depos w, w + n_warps, ...
+// atomic mode: warps fetch batches of 32 depos from a device-side counter until none is left
 // ------------------------------------------------------------------------------------------------------------------
+constexpr int kBatchWarps = 8;          // warps per CTA
+constexpr int kEdgeCap = 768;           // edge values per warp scratch (32 patches of 16 x 5 bins need 736)
+constexpr int kQueueCap = 64;           // entries per draw queue (at most 31 left over + 32 pushed)
+
 template <bool FLUCT>
-__global__ void __launch_bounds__(256) raster_atomic_kernel(GridDims g, DepoArrays d, long long n, uint64_t id_base,
-                                                            uint64_t seed, double nsigma, float *__restrict__ S,
-                                                            int *__restrict__ totals, Counters *counters)
+struct BatchScratch {
+    using T = typename std::conditional<FLUCT, double, float>::type;
+    T edge[kEdgeCap];
+    int eoff[33], boff[33];
+};
+struct DrawQueues {
+    double p[kNumDrawQueues][kQueueCap];
+    double N[kNumDrawQueues][kQueueCap];
+    uint32_t w[kNumDrawQueues][kQueueCap];
+    uint32_t bin[kNumDrawQueues][kQueueCap];   // wire * n_ticks + tick
+    uint32_t flags[kNumDrawQueues][kQueueCap]; // bit 0 mirror, bit 1 negative charge, bits 8.. depo index in the call
+};
+template <bool FLUCT>
+struct BatchSmem {
+    BatchScratch<FLUCT> scratch[kBatchWarps];
+};
+template <>
+struct BatchSmem<true> {
+    BatchScratch<true> scratch[kBatchWarps];
+    DrawQueues queues[kBatchWarps];
+};
+
+// largest d in [0, 32) with off[d] <= x (off is an exclusive prefix, off[32] > x)
+__device__ __forceinline__ int owner_of(const int *off, int x)
 {
-    const int lane = threadIdx.x & 31;
-    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const long long n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
+    int lo = 0;
+#pragma unroll
+    for (int step = 16; step > 0; step >>= 1)
+        if (off[lo + step] <= x) lo += step;
+    return lo;
+}
+
+__device__ __forceinline__ int warp_incl_scan(int v, int lane)
+{
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, v, o);
+        if (lane >= o) v += t;
+    }
+    return v;
+}
+
+// draws `take` entries from the top of queue `cls` (lane < take) and adds them to S
+__device__ __forceinline__ void drain_queue(DrawQueues &Q, int cls, int &count, bool everything, float *__restrict__ S,
+                                            int *__restrict__ totals, int lane)
+{
+    while (count >= 32 || (everything && count > 0)) {
+        const int take = min(32, count);
+        count -= take;
+        if (lane < take) {
+            const int e = count + lane;
+            const uint32_t fl = Q.flags[cls][e];
+            const double N = Q.N[cls][e];
+            const double k = draw_classified(cls, N, Q.p[cls][e], Q.w[cls][e], (fl & 1u) != 0);
+            if (k != 0.0) {
+                const float v = (fl & 2u) ? -(float)k : (float)k;
+                atomicAdd(S + Q.bin[cls][e], v);
+                if (totals != nullptr) atomicAdd(totals + (fl >> 8), (int)v);
+            }
+        }
+        __syncwarp();
+    }
+}
+
+template <bool FLUCT>
+__global__ void __launch_bounds__(kBatchWarps * 32) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
+                                                                        uint64_t id_base, uint64_t seed, double nsigma,
+                                                                        float *__restrict__ S, int *__restrict__ totals,
+                                                                        Counters *counters)
+{
+    using T = typename std::conditional<FLUCT, double, float>::type;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    BatchSmem<FLUCT> &sm = *reinterpret_cast<BatchSmem<FLUCT> *>(smem_raw);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    BatchScratch<FLUCT> &sc = sm.scratch[wid];
     const GlobalSink sink{S, g.n_ticks};
+    const long long n_batches = (n + 31) >> 5;
     unsigned long long drawn = 0, skipped = 0;
-    for (long long i = warp; i < n; i += n_warps) {
-        const float t0 = __ldg(d.t0 + i), x0 = __ldg(d.x0 + i), st = __ldg(d.sigma_t + i), sx = __ldg(d.sigma_x + i),
-                    q = __ldg(d.q + i);
-        int tot = 0;
-        if (depo_valid(t0, x0, st, sx, q)) {
-            drawn += raster_depo<FLUCT>(t0, x0, st, sx, q, id_base + (uint64_t)i, seed, nsigma, g.n_ticks, 0, g.n_wires,
-                                        0, g.n_ticks, sink, lane, &tot);
-        } else {
-            skipped += (lane == 0);
+    int qcount[kNumDrawQueues] = {0, 0, 0};
+
+    for (;;) {
+        long long batch = 0;
+        if (lane == 0) batch = (long long)atomicAdd(&counters->next_batch, 1ull);
+        batch = __shfl_sync(0xffffffffu, batch, 0);
+        if (batch >= n_batches) break;
+        const long long i = (batch << 5) + lane;
+        float t0 = 0.f, x0 = 0.f, st = 0.f, sx = 0.f, q = 0.f;
+        bool valid = false;
+        if (i < n) {
+            t0 = __ldg(d.t0 + i), x0 = __ldg(d.x0 + i), st = __ldg(d.sigma_t + i), sx = __ldg(d.sigma_x + i),
+            q = __ldg(d.q + i);
+            valid = depo_valid(t0, x0, st, sx, q);
+            skipped += !valid;
         }
-        if (totals != nullptr) {
-            tot = warp_sum(tot);
-            if (lane == 0) totals[i] = tot;
+        const double T0 = t0, X0 = x0, ST = st, SX = sx;
+        Extent et{0, 0}, ex{0, 0};
+        if (valid) {
+            et = axis_extent(T0, ST, nsigma, 0, g.n_ticks);
+            ex = axis_extent(X0, SX, nsigma, 0, g.n_wires);
         }
+        const bool live = et.lo < et.hi && ex.lo < ex.hi;
+        const int nt = live ? et.hi - et.lo : 0, nx = live ? ex.hi - ex.lo : 0;
+        const bool big = nt + nx + 2 > kEdgeCap || (long long)nt * nx > (1 << 24);
+        const int ne = (live && !big) ? nt + nx + 2 : 0, nb = (live && !big) ? nt * nx : 0;
+        const int eincl = warp_incl_scan(ne, lane), bincl = warp_incl_scan(nb, lane);
+        __syncwarp();
+        sc.eoff[lane] = eincl - ne;
+        sc.boff[lane] = bincl - nb;
+        if (lane == 31) {
+            sc.eoff[32] = eincl;
+            sc.boff[32] = bincl;
+        }
+        __syncwarp();
+        const double Ntr = floor(fabs((double)q) + 0.5);
+        drawn += (unsigned long long)nb;
+
+        // patches too big for the scratch: the whole warp walks them one at a time
+        unsigned int big_mask = __ballot_sync(0xffffffffu, live && big);
+        while (big_mask) {
+            const int src = __ffs(big_mask) - 1;
+            big_mask &= big_mask - 1;
+            int tot = 0;
+            drawn += raster_depo<FLUCT>(__shfl_sync(0xffffffffu, t0, src), __shfl_sync(0xffffffffu, x0, src),
+                                        __shfl_sync(0xffffffffu, st, src), __shfl_sync(0xffffffffu, sx, src),
+                                        __shfl_sync(0xffffffffu, q, src), id_base + (uint64_t)((batch << 5) + src), seed,
+                                        nsigma, g.n_ticks, 0, g.n_wires, 0, g.n_ticks, sink, lane, &tot);
+            if (totals != nullptr) {
+                tot = warp_sum(tot);
+                if (lane == 0 && tot != 0) atomicAdd(totals + (batch << 5) + src, tot);
+            }
+        }
+
+        // sub-batches of consecutive depos whose edges fit the scratch (normally all 32 at once)
+        int d0 = 0;
+        while (d0 < 32) {
+            const int ebase = sc.eoff[d0];
+            const unsigned int fits = __ballot_sync(0xffffffffu, lane >= d0 && eincl - ebase <= kEdgeCap);
+            const int d1 = d0 + __popc(fits); // eincl is monotone: the fitting lanes are d0 .. d1-1, at least one
+            const int etot = sc.eoff[d1] - ebase, bbase = sc.boff[d0], btot = sc.boff[d1] - bbase;
+            // ---- edges: erf((edge - centre) / (sqrt2 sigma)), flat over the sub-batch -------------------------------
+            for (int e0 = 0; e0 < etot; e0 += 32) {
+                const int e = e0 + lane;
+                const bool act = e < etot;
+                const int own = owner_of(sc.eoff, ebase + (act ? e : 0));
+                const int le = ebase + e - sc.eoff[own];
+                const int nto = __shfl_sync(0xffffffffu, nt, own);
+                const bool on_t = le <= nto;
+                const int lo_t = __shfl_sync(0xffffffffu, et.lo, own), lo_x = __shfl_sync(0xffffffffu, ex.lo, own);
+                const double ct = __shfl_sync(0xffffffffu, T0, own), cx = __shfl_sync(0xffffffffu, X0, own);
+                const double sgt = __shfl_sync(0xffffffffu, ST, own), sgx = __shfl_sync(0xffffffffu, SX, own);
+                const double centre = on_t ? ct : cx, sigma = on_t ? sgt : sgx;
+                const int coord = on_t ? lo_t + le : lo_x + (le - nto - 1);
+                T E;
+                if (sigma < 1e-6) { // all weight in bin floor(centre) (A4): a step from -1 to +1 after that bin's low edge
+                    E = ((double)coord <= floor(centre)) ? T(-1) : T(1);
+                } else {
+                    const double dd = __dsub_rn((double)coord, centre);
+                    if constexpr (FLUCT) {
+                        E = erf(__ddiv_rn(dd, __dmul_rn(1.4142135623730951, sigma)));
+                    } else {
+                        const float inv = 1.0f / (1.41421356f * (float)sigma);
+                        E = erff((float)dd * inv);
+                    }
+                }
+                if (act) sc.edge[e] = E;
+            }
+            __syncwarp();
+            // ---- bins: p_ij = wt_i wx_j, flat over the sub-batch ----------------------------------------------------
+            for (int b0 = 0; b0 < btot; b0 += 32) {
+                const int b = b0 + lane;
+                const bool act = b < btot;
+                const int own = owner_of(sc.boff, bbase + (act ? b : 0));
+                const int l = bbase + b - sc.boff[own];
+                const int nto = __shfl_sync(0xffffffffu, nt, own);
+                const int lo_t = __shfl_sync(0xffffffffu, et.lo, own), lo_x = __shfl_sync(0xffffffffu, ex.lo, own);
+                const int j = act ? (int)((unsigned)l / (unsigned)max(nto, 1)) : 0; // wire index in the patch
+                const int ii = act ? l - j * nto : 0;                              // tick index in the patch
+                const T *E = sc.edge + (sc.eoff[own] - ebase);
+                const T wt = T(0.5) * (E[ii + 1] - E[ii]);
+                const T wx = T(0.5) * (E[nto + 1 + j + 1] - E[nto + 1 + j]);
+                const int wire = lo_x + j, tick = lo_t + ii;
+                if constexpr (FLUCT) {
+                    const double Nn = __shfl_sync(0xffffffffu, Ntr, own);
+                    const float qq = __shfl_sync(0xffffffffu, q, own);
+                    double p = __dmul_rn(wt, wx);
+                    const uint64_t gbin = (uint64_t)wire * (uint64_t)g.n_ticks + (uint64_t)tick;
+                    const uint64_t id = id_base + (uint64_t)((batch << 5) + own);
+                    uint32_t w = pick_word(fluct_words(seed, id, gbin >> 2), (uint32_t)gbin & 3u);
+                    bool mirror = false;
+                    int cls = act ? classify_draw(Nn, p, w, mirror) : (int)kDrawZero;
+                    const uint32_t fl = (mirror ? 1u : 0u) | (qq < 0.0f ? 2u : 0u) |
+                                        ((uint32_t)((batch << 5) + own) << 8);
+                    if (cls == kDrawAll) { // p >= 1: every electron lands here
+                        const float v = (fl & 2u) ? -(float)Nn : (float)Nn;
+                        atomicAdd(S + gbin, v);
+                        if (totals != nullptr) atomicAdd(totals + (batch << 5) + own, (int)v);
+                    }
+                    DrawQueues &Q = sm.queues[wid];
+#pragma unroll
+                    for (int c = 0; c < kNumDrawQueues; ++c) {
+                        const unsigned int m = __ballot_sync(0xffffffffu, cls == c);
+                        if (cls == c) {
+                            const int pos = qcount[c] + __popc(m & ((1u << lane) - 1u));
+                            Q.p[c][pos] = p;
+                            Q.N[c][pos] = Nn;
+                            Q.w[c][pos] = w;
+                            Q.bin[c][pos] = (uint32_t)gbin;
+                            Q.flags[c][pos] = fl;
+                        }
+                        qcount[c] += __popc(m);
+                    }
+                    __syncwarp();
+#pragma unroll
+                    for (int c = 0; c < kNumDrawQueues; ++c) drain_queue(Q, c, qcount[c], false, S, totals, lane);
+                } else {
+                    const float qq = __shfl_sync(0xffffffffu, q, own);
+                    if (act) sink.add(wire, tick, qq * (wt * wx));
+                }
+            }
+            __syncwarp();
+            d0 = d1;
+        }
+    }
+    if constexpr (FLUCT) {
+#pragma unroll
+        for (int c = 0; c < kNumDrawQueues; ++c) drain_queue(sm.queues[wid], c, qcount[c], true, S, totals, lane);
     }
     drawn = warp_sum(drawn);
     skipped = warp_sum(skipped);
     if (lane == 0) {
         if (drawn) atomicAdd(&counters->bins_drawn, drawn);
         if (skipped) atomicAdd(&counters->depos_skipped, skipped);
+        // the last warp to leave re-arms the batch counter for the next launch on this stream
+        const unsigned long long n_warps = (unsigned long long)gridDim.x * kBatchWarps;
+        __threadfence();
+        if (atomicAdd(&counters->warps_done, 1ull) == n_warps - 1) {
+            counters->next_batch = 0ull;
+            counters->warps_done = 0ull;
+        }
     }
 }
 
@@ -336,21 +559,32 @@ __global__ void count_invalid_kernel(DepoArrays d, long long n, Counters *counte
 
 } // namespace
 
+cudaError_t raster_configure()
+{
+    cudaError_t err = cudaFuncSetAttribute(raster_batch_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)sizeof(BatchSmem<true>));
+    if (err != cudaSuccess) return err;
+    return cudaFuncSetAttribute(raster_batch_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)sizeof(BatchSmem<false>));
+}
+
 cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
                                  double nsigma, float *S, int *depo_totals, Counters *counters, int sm_count,
                                  cudaStream_t st)
 {
     if (n <= 0) return cudaSuccess;
-    const int threads = 256, warps_per_cta = threads / 32;
-    long long ctas = (n + warps_per_cta - 1) / warps_per_cta;
-    const long long max_ctas = (long long)sm_count * 8; // 2048 threads per SM resident
+    const long long n_batches = (n + 31) / 32;
+    const size_t smem = fluctuate ? sizeof(BatchSmem<true>) : sizeof(BatchSmem<false>);
+    const int ctas_per_sm = (int)((200u * 1024u) / smem) > 8 ? 8 : (int)((200u * 1024u) / smem);
+    long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
+    const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
     if (ctas > max_ctas) ctas = max_ctas;
     if (fluctuate)
-        raster_atomic_kernel<true><<<(unsigned)ctas, threads, 0, st>>>(g, d, n, id_base, seed, nsigma, S, depo_totals,
-                                                                      counters);
+        raster_batch_kernel<true><<<(unsigned)ctas, kBatchWarps * 32, smem, st>>>(g, d, n, id_base, seed, nsigma, S,
+                                                                                 depo_totals, counters);
     else
-        raster_atomic_kernel<false><<<(unsigned)ctas, threads, 0, st>>>(g, d, n, id_base, seed, nsigma, S, depo_totals,
-                                                                       counters);
+        raster_batch_kernel<false><<<(unsigned)ctas, kBatchWarps * 32, smem, st>>>(g, d, n, id_base, seed, nsigma, S,
+                                                                                  depo_totals, counters);
     return cudaGetLastError();
 }
 

@@ -327,6 +327,7 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
         CU_TRY(build_response_spectrum(dev_R, n_rwires, n_rticks, pad_w, pad_t, p->spec_stride, dev_tmp, p->Rhat,
                                        p->stream));
         CU_TRY(conv_configure(pad_w, pad_t));
+        CU_TRY(raster_configure());
         CU_TRY(cudaStreamSynchronize(p->stream));
         return WCSIM_OK;
     }();
@@ -358,6 +359,10 @@ int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n
         return raster_tiled(plan, g, d, n, depo_id_base, seed, fluctuate != 0, dev_depo_totals);
     }
     plan->launches += 1;
+    if (dev_depo_totals) {
+        if (n > (1ll << 24)) return WCSIM_EINVAL; // per-depo totals are indexed with 24 bits in the draw queues
+        CU_TRY(cudaMemsetAsync(dev_depo_totals, 0, sizeof(int) * (size_t)n, plan->stream));
+    }
     CU_TRY(launch_raster_atomic(g, d, n, depo_id_base, seed, fluctuate != 0, plan->nsigma, plan->S, dev_depo_totals,
                                 plan->counters, plan->sm_count, plan->stream));
     return WCSIM_OK;
