@@ -169,8 +169,10 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v)
 // ------------------------------------------------------------------------------------------------------------------
 // atomic mode: warps fetch batches of 32 depos from a device-side counter until none is left
 // ------------------------------------------------------------------------------------------------------------------
-constexpr int kBatchWarps = 8;          // warps per CTA
-constexpr int kEdgeCap = 768;           // edge values per warp scratch (32 patches of 16 x 5 bins need 736)
+constexpr int kBatchWarps = 4;          // warps per CTA
+constexpr int kBatchShift = 3;          // log2 of the depos a warp fetches at a time (lanes beyond that own no depo):
+constexpr int kBatchDepos = 1 << kBatchShift; // small batches keep the per-warp serial path short and the load balanced
+constexpr int kEdgeCap = 256;           // edge values per warp scratch (8 patches of 16 x 5 bins need 184)
 constexpr int kQueueCap = 64;           // entries per draw queue (at most 31 left over + 32 pushed)
 
 template <bool FLUCT>
@@ -181,7 +183,7 @@ struct BatchScratch {
 };
 struct DrawQueues {
     double p[kNumDrawQueues][kQueueCap];
-    double N[kNumDrawQueues][kQueueCap];
+    float N[kNumDrawQueues][kQueueCap]; // floor(|q| + 1/2) of a float q is always a float
     uint32_t w[kNumDrawQueues][kQueueCap];
     uint32_t bin[kNumDrawQueues][kQueueCap];   // wire * n_ticks + tick
     uint32_t flags[kNumDrawQueues][kQueueCap]; // bit 0 mirror, bit 1 negative charge, bits 8.. depo index in the call
@@ -226,7 +228,7 @@ __device__ __forceinline__ void drain_queue(DrawQueues &Q, int cls, int &count, 
         if (lane < take) {
             const int e = count + lane;
             const uint32_t fl = Q.flags[cls][e];
-            const double N = Q.N[cls][e];
+            const double N = (double)Q.N[cls][e];
             const double k = draw_classified(cls, N, Q.p[cls][e], Q.w[cls][e], (fl & 1u) != 0);
             if (k != 0.0) {
                 const float v = (fl & 2u) ? -(float)k : (float)k;
@@ -250,19 +252,19 @@ __global__ void __launch_bounds__(kBatchWarps * 32) raster_batch_kernel(GridDims
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     BatchScratch<FLUCT> &sc = sm.scratch[wid];
     const GlobalSink sink{S, g.n_ticks};
-    const long long n_batches = (n + 31) >> 5;
+    const long long n_batches = (n + kBatchDepos - 1) >> kBatchShift;
     unsigned long long drawn = 0, skipped = 0;
-    int qcount[kNumDrawQueues] = {0, 0, 0};
+    int qcount[kNumDrawQueues] = {};
 
     for (;;) {
         long long batch = 0;
         if (lane == 0) batch = (long long)atomicAdd(&counters->next_batch, 1ull);
         batch = __shfl_sync(0xffffffffu, batch, 0);
         if (batch >= n_batches) break;
-        const long long i = (batch << 5) + lane;
+        const long long i = (batch << kBatchShift) + lane;
         float t0 = 0.f, x0 = 0.f, st = 0.f, sx = 0.f, q = 0.f;
         bool valid = false;
-        if (i < n) {
+        if (lane < kBatchDepos && i < n) {
             t0 = __ldg(d.t0 + i), x0 = __ldg(d.x0 + i), st = __ldg(d.sigma_t + i), sx = __ldg(d.sigma_x + i),
             q = __ldg(d.q + i);
             valid = depo_valid(t0, x0, st, sx, q);
@@ -287,7 +289,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32) raster_batch_kernel(GridDims
             sc.boff[32] = bincl;
         }
         __syncwarp();
-        const double Ntr = floor(fabs((double)q) + 0.5);
+        const float Ntr = (float)floor(fabs((double)q) + 0.5); // exact: see DrawQueues::N
         drawn += (unsigned long long)nb;
 
         // patches too big for the scratch: the whole warp walks them one at a time
@@ -298,11 +300,11 @@ __global__ void __launch_bounds__(kBatchWarps * 32) raster_batch_kernel(GridDims
             int tot = 0;
             drawn += raster_depo<FLUCT>(__shfl_sync(0xffffffffu, t0, src), __shfl_sync(0xffffffffu, x0, src),
                                         __shfl_sync(0xffffffffu, st, src), __shfl_sync(0xffffffffu, sx, src),
-                                        __shfl_sync(0xffffffffu, q, src), id_base + (uint64_t)((batch << 5) + src), seed,
+                                        __shfl_sync(0xffffffffu, q, src), id_base + (uint64_t)((batch << kBatchShift) + src), seed,
                                         nsigma, g.n_ticks, 0, g.n_wires, 0, g.n_ticks, sink, lane, &tot);
             if (totals != nullptr) {
                 tot = warp_sum(tot);
-                if (lane == 0 && tot != 0) atomicAdd(totals + (batch << 5) + src, tot);
+                if (lane == 0 && tot != 0) atomicAdd(totals + (batch << kBatchShift) + src, tot);
             }
         }
 
@@ -322,9 +324,9 @@ __global__ void __launch_bounds__(kBatchWarps * 32) raster_batch_kernel(GridDims
                 const int nto = __shfl_sync(0xffffffffu, nt, own);
                 const bool on_t = le <= nto;
                 const int lo_t = __shfl_sync(0xffffffffu, et.lo, own), lo_x = __shfl_sync(0xffffffffu, ex.lo, own);
-                const double ct = __shfl_sync(0xffffffffu, T0, own), cx = __shfl_sync(0xffffffffu, X0, own);
-                const double sgt = __shfl_sync(0xffffffffu, ST, own), sgx = __shfl_sync(0xffffffffu, SX, own);
-                const double centre = on_t ? ct : cx, sigma = on_t ? sgt : sgx;
+                const float ct = __shfl_sync(0xffffffffu, t0, own), cx = __shfl_sync(0xffffffffu, x0, own);
+                const float sgt = __shfl_sync(0xffffffffu, st, own), sgx = __shfl_sync(0xffffffffu, sx, own);
+                const double centre = (double)(on_t ? ct : cx), sigma = (double)(on_t ? sgt : sgx);
                 const int coord = on_t ? lo_t + le : lo_x + (le - nto - 1);
                 T E;
                 if (sigma < 1e-6) { // all weight in bin floor(centre) (A4): a step from -1 to +1 after that bin's low edge
@@ -356,20 +358,20 @@ __global__ void __launch_bounds__(kBatchWarps * 32) raster_batch_kernel(GridDims
                 const T wx = T(0.5) * (E[nto + 1 + j + 1] - E[nto + 1 + j]);
                 const int wire = lo_x + j, tick = lo_t + ii;
                 if constexpr (FLUCT) {
-                    const double Nn = __shfl_sync(0xffffffffu, Ntr, own);
+                    const double Nn = (double)__shfl_sync(0xffffffffu, Ntr, own);
                     const float qq = __shfl_sync(0xffffffffu, q, own);
                     double p = __dmul_rn(wt, wx);
                     const uint64_t gbin = (uint64_t)wire * (uint64_t)g.n_ticks + (uint64_t)tick;
-                    const uint64_t id = id_base + (uint64_t)((batch << 5) + own);
+                    const uint64_t id = id_base + (uint64_t)((batch << kBatchShift) + own);
                     uint32_t w = pick_word(fluct_words(seed, id, gbin >> 2), (uint32_t)gbin & 3u);
                     bool mirror = false;
                     int cls = act ? classify_draw(Nn, p, w, mirror) : (int)kDrawZero;
                     const uint32_t fl = (mirror ? 1u : 0u) | (qq < 0.0f ? 2u : 0u) |
-                                        ((uint32_t)((batch << 5) + own) << 8);
+                                        ((uint32_t)((batch << kBatchShift) + own) << 8);
                     if (cls == kDrawAll) { // p >= 1: every electron lands here
                         const float v = (fl & 2u) ? -(float)Nn : (float)Nn;
                         atomicAdd(S + gbin, v);
-                        if (totals != nullptr) atomicAdd(totals + (batch << 5) + own, (int)v);
+                        if (totals != nullptr) atomicAdd(totals + (batch << kBatchShift) + own, (int)v);
                     }
                     DrawQueues &Q = sm.queues[wid];
 #pragma unroll
@@ -378,7 +380,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32) raster_batch_kernel(GridDims
                         if (cls == c) {
                             const int pos = qcount[c] + __popc(m & ((1u << lane) - 1u));
                             Q.p[c][pos] = p;
-                            Q.N[c][pos] = Nn;
+                            Q.N[c][pos] = (float)Nn;
                             Q.w[c][pos] = w;
                             Q.bin[c][pos] = (uint32_t)gbin;
                             Q.flags[c][pos] = fl;
@@ -573,7 +575,7 @@ cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t
                                  cudaStream_t st)
 {
     if (n <= 0) return cudaSuccess;
-    const long long n_batches = (n + 31) / 32;
+    const long long n_batches = (n + kBatchDepos - 1) / kBatchDepos;
     const size_t smem = fluctuate ? sizeof(BatchSmem<true>) : sizeof(BatchSmem<false>);
     const int ctas_per_sm = (int)((200u * 1024u) / smem) > 8 ? 8 : (int)((200u * 1024u) / smem);
     long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;

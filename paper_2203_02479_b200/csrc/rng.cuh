@@ -54,15 +54,46 @@ __device__ __forceinline__ uint4 noise_words(uint64_t seed, uint32_t wire, uint3
 // or a rounding boundary by ~1e-16 relative, i.e. it flips a draw with probability ~1e-13, far inside the 1e-6
 // budget of BASELINE.json north_star.
 // ------------------------------------------------------------------------------------------------------------------
-enum DrawClass : int { kDrawZero = -2, kDrawAll = -1, kDrawInversion = 0, kDrawNormalCentral = 1, kDrawNormalTail = 2 };
-constexpr int kNumDrawQueues = 3;
+enum DrawClass : int {
+    kDrawZero = -2,        // k = 0 without a draw
+    kDrawAll = -1,         // p >= 1: k = N
+    kDrawInversion0 = 0,   // inversion, mu < 2
+    kDrawInversion1 = 1,   // inversion, 2 <= mu < 6
+    kDrawInversion2 = 2,   // inversion, 6 <= mu < 16
+    kDrawNormalCentral = 3,
+    kDrawNormalTail = 4
+};
+constexpr int kNumDrawQueues = 5;
+
+// 1/k for the inversion recurrence (k is the trip count, the same in every lane that is still in the loop)
+constexpr int kInvTable = 64;
+static __constant__ double c_inv_k[kInvTable] = {0.0, 1.0 / 1.0, 1.0 / 2.0, 1.0 / 3.0, 1.0 / 4.0, 1.0 / 5.0, 1.0 / 6.0, 1.0 / 7.0, 1.0 / 8.0, 1.0 / 9.0, 1.0 / 10.0, 1.0 / 11.0, 1.0 / 12.0, 1.0 / 13.0, 1.0 / 14.0, 1.0 / 15.0, 1.0 / 16.0, 1.0 / 17.0, 1.0 / 18.0, 1.0 / 19.0, 1.0 / 20.0, 1.0 / 21.0, 1.0 / 22.0, 1.0 / 23.0, 1.0 / 24.0, 1.0 / 25.0, 1.0 / 26.0, 1.0 / 27.0, 1.0 / 28.0, 1.0 / 29.0, 1.0 / 30.0, 1.0 / 31.0, 1.0 / 32.0, 1.0 / 33.0, 1.0 / 34.0, 1.0 / 35.0, 1.0 / 36.0, 1.0 / 37.0, 1.0 / 38.0, 1.0 / 39.0, 1.0 / 40.0, 1.0 / 41.0, 1.0 / 42.0, 1.0 / 43.0, 1.0 / 44.0, 1.0 / 45.0, 1.0 / 46.0, 1.0 / 47.0, 1.0 / 48.0, 1.0 / 49.0, 1.0 / 50.0, 1.0 / 51.0, 1.0 / 52.0, 1.0 / 53.0, 1.0 / 54.0, 1.0 / 55.0, 1.0 / 56.0, 1.0 / 57.0, 1.0 / 58.0, 1.0 / 59.0, 1.0 / 60.0, 1.0 / 61.0, 1.0 / 62.0, 1.0 / 63.0};
+
+// AS 241 PPND16 coefficients: central region a0..a7 / b1..b7 and first tail region c0..c7 / d1..d7 (highest first)
+static __constant__ double c_as241_a[8] = {2.5090809287301226727e+3, 3.3430575583588128105e+4, 6.7265770927008700853e+4,
+                                           4.5921953931549871457e+4, 1.3731693765509461125e+4, 1.9715909503065514427e+3,
+                                           1.3314166789178437745e+2, 3.3871328727963666080e0};
+static __constant__ double c_as241_b[8] = {5.2264952788528545610e+3, 2.8729085735721942674e+4, 3.9307895800092710610e+4,
+                                           2.1213794301586595867e+4, 5.3941960214247511077e+3, 6.8718700749205790830e+2,
+                                           4.2313330701600911252e+1, 1.0};
+static __constant__ double c_as241_c[8] = {7.74545014278341407640e-4, 2.27238449892691845833e-2, 2.41780725177450611770e-1,
+                                           1.27045825245236838258e0,  3.64784832476320460504e0,  5.76949722146069140550e0,
+                                           4.63033784615654529590e0,  1.42343711074968357734e0};
+static __constant__ double c_as241_d[8] = {1.05075007164441684324e-9, 5.47593808499534494600e-4, 1.51986665636164571966e-2,
+                                           1.48103976427480074590e-1, 6.89767334985100004550e-1, 1.67638483018380384940e0,
+                                           2.05319162663775882187e0,  1.0};
 
 __device__ __forceinline__ double word_to_u01(uint32_t w)
 {
     return __dmul_rn(__dadd_rn((double)w, 0.5), 1.0 / 4294967296.0); // exact
 }
 
+// |u - 1/2| <= 0.425 (the double nearest 0.425) for u = (w + 1/2) 2^-32, decided on the integer word:
+// 0.075 2^32 = 322122547.2 and 0.925 2^32 = 3972844748.8, so the central region is 322122547 <= w <= 3972844748.
+__device__ __forceinline__ bool word_is_central(uint32_t w) { return w - 322122547u <= 3972844748u - 322122547u; }
+
 // Folds the p > 1/2 mirror into (p, w) and says which routine draws k.  On return p <= 1/2.
+// Shortcut: (1-p)^N >= 1 - N p (Bernoulli), so u <= 1 - mu already implies u <= F(0), i.e. k = 0, without exp/log.
 __device__ __forceinline__ int classify_draw(double N, double &p, uint32_t &w, bool &mirror)
 {
     mirror = false;
@@ -73,22 +104,29 @@ __device__ __forceinline__ int classify_draw(double N, double &p, uint32_t &w, b
         p = __dsub_rn(1.0, p);
         w = ~w;
     }
-    if (__dmul_rn(N, p) < 16.0) return kDrawInversion;
-    return fabs(__dsub_rn(word_to_u01(w), 0.5)) <= 0.425 ? kDrawNormalCentral : kDrawNormalTail;
+    const double mu = __dmul_rn(N, p);
+    if (mu < 16.0) {
+        if (mu < 1.0 && word_to_u01(w) <= 1.0 - mu) return mirror ? kDrawAll : kDrawZero;
+        return mu < 2.0 ? kDrawInversion0 : mu < 6.0 ? kDrawInversion1 : kDrawInversion2;
+    }
+    return word_is_central(w) ? kDrawNormalCentral : kDrawNormalTail;
 }
 
 __device__ __forceinline__ double draw_inversion(double N, double p, uint32_t w)
 {
     const double u = word_to_u01(w);
     double f = exp(N * log1p(-p));
-    double c = f, k = 0.0;
-    const double r = p / (1.0 - p);
-    while (u > c && k < N) {
-        k += 1.0;
-        f *= (r * (N - k + 1.0)) * __drcp_rn(k);
+    double c = f;
+    const double r = p / (1.0 - p), N1 = N + 1.0;
+    int k = 0;
+    while (u > c && (double)k < N) {
+        ++k;
+        const double kd = (double)k;
+        const double rk = k < kInvTable ? c_inv_k[k] : 1.0 / kd;
+        f *= (r * (N1 - kd)) * rk;
         c += f;
     }
-    return k;
+    return (double)k;
 }
 
 __device__ __forceinline__ double finish_normal(double N, double p, double z)
@@ -105,45 +143,27 @@ __device__ __forceinline__ double draw_normal_central(double N, double p, uint32
 {
     const double q = word_to_u01(w) - 0.5;
     const double r = 0.180625 - q * q;
-    double num = 2.5090809287301226727e+3, den = 5.2264952788528545610e+3;
-    num = fma(num, r, 3.3430575583588128105e+4); den = fma(den, r, 2.8729085735721942674e+4);
-    num = fma(num, r, 6.7265770927008700853e+4); den = fma(den, r, 3.9307895800092710610e+4);
-    num = fma(num, r, 4.5921953931549871457e+4); den = fma(den, r, 2.1213794301586595867e+4);
-    num = fma(num, r, 1.3731693765509461125e+4); den = fma(den, r, 5.3941960214247511077e+3);
-    num = fma(num, r, 1.9715909503065514427e+3); den = fma(den, r, 6.8718700749205790830e+2);
-    num = fma(num, r, 1.3314166789178437745e+2); den = fma(den, r, 4.2313330701600911252e+1);
-    num = fma(num, r, 3.3871328727963666080e0);  den = fma(den, r, 1.0);
+    double num = c_as241_a[0], den = c_as241_b[0];
+#pragma unroll
+    for (int j = 1; j < 8; ++j) {
+        num = fma(num, r, c_as241_a[j]);
+        den = fma(den, r, c_as241_b[j]);
+    }
     return finish_normal(N, p, q * num / den);
 }
 
 // AS 241 PPND16, |u - 1/2| > 0.425.  r = sqrt(-log(min(u, 1-u))) <= sqrt(33 log 2) = 4.79 for a 32-bit word, so the
-// r > 5 branch of the routine is unreachable here; it is kept (one predicated select) for the debug hook's sake.
+// routine's third region (r > 5) cannot be reached from a 32-bit word and is not coded.
 __device__ __forceinline__ double draw_normal_tail(double N, double p, uint32_t w)
 {
     const double u = word_to_u01(w);
     const double q = u - 0.5;
-    double r = sqrt(-log(q < 0.0 ? u : 1.0 - u));
-    double num, den;
-    if (r <= 5.0) {
-        r -= 1.6;
-        num = 7.74545014278341407640e-4; den = 1.05075007164441684324e-9;
-        num = fma(num, r, 2.27238449892691845833e-2); den = fma(den, r, 5.47593808499534494600e-4);
-        num = fma(num, r, 2.41780725177450611770e-1); den = fma(den, r, 1.51986665636164571966e-2);
-        num = fma(num, r, 1.27045825245236838258e0);  den = fma(den, r, 1.48103976427480074590e-1);
-        num = fma(num, r, 3.64784832476320460504e0);  den = fma(den, r, 6.89767334985100004550e-1);
-        num = fma(num, r, 5.76949722146069140550e0);  den = fma(den, r, 1.67638483018380384940e0);
-        num = fma(num, r, 4.63033784615654529590e0);  den = fma(den, r, 2.05319162663775882187e0);
-        num = fma(num, r, 1.42343711074968357734e0);  den = fma(den, r, 1.0);
-    } else {
-        r -= 5.0;
-        num = 2.01033439929228813265e-7; den = 2.04426310338993978564e-15;
-        num = fma(num, r, 2.71155556874348757815e-5); den = fma(den, r, 1.42151175831644588870e-7);
-        num = fma(num, r, 1.24266094738807843860e-3); den = fma(den, r, 1.84631831751005468180e-5);
-        num = fma(num, r, 2.65321895265761230930e-2); den = fma(den, r, 7.86869131145613259100e-4);
-        num = fma(num, r, 2.96560571828504891230e-1); den = fma(den, r, 1.48753612908506148525e-2);
-        num = fma(num, r, 1.78482653991729133580e0);  den = fma(den, r, 1.36929880922735805310e-1);
-        num = fma(num, r, 5.46378491116411436990e0);  den = fma(den, r, 5.99832206555887937690e-1);
-        num = fma(num, r, 6.65790464350110377720e0);  den = fma(den, r, 1.0);
+    const double r = sqrt(-log(q < 0.0 ? u : 1.0 - u)) - 1.6;
+    double num = c_as241_c[0], den = c_as241_d[0];
+#pragma unroll
+    for (int j = 1; j < 8; ++j) {
+        num = fma(num, r, c_as241_c[j]);
+        den = fma(den, r, c_as241_d[j]);
     }
     const double val = num / den;
     return finish_normal(N, p, q < 0.0 ? -val : val);
@@ -152,7 +172,7 @@ __device__ __forceinline__ double draw_normal_tail(double N, double p, uint32_t 
 // the draw of an already classified bin (cls >= 0), mirror undone
 __device__ __forceinline__ double draw_classified(int cls, double N, double p, uint32_t w, bool mirror)
 {
-    const double k = cls == kDrawInversion       ? draw_inversion(N, p, w)
+    const double k = cls <= kDrawInversion2       ? draw_inversion(N, p, w)
                      : cls == kDrawNormalCentral ? draw_normal_central(N, p, w)
                                                  : draw_normal_tail(N, p, w);
     return mirror ? N - k : k;
