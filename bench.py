@@ -41,12 +41,13 @@ def load_peaks():
         return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)", "sm_max_mhz": 1965.0}
 
 
-def stage_bytes(pl):
+def stage_bytes(pl, direct):
     """Algorithmic HBM bytes of each convolution kernel for one plane-event."""
     nw, nt, pw, pt = pl["n_wires"], pl["n_ticks"], pl["pad_w"], pl["pad_t"]
     nk = pt // 2 + 1
-    grid, spec, rhat = nw * nt * 4, nw * nk * 8, pw * nk * 8
-    return {"rows_forward": grid + spec, "cols": 2 * spec + rhat, "rows_inverse": spec + grid}
+    grid, spec = nw * nt * 4, nw * nk * 8
+    resp = pl["response"].shape[0] * nk * 8 if direct else pw * nk * 8  # Rt rows (direct) or Rhat (FFT wire mode)
+    return {"rows_forward": grid + spec, "cols": 2 * spec + resp, "rows_inverse": spec + grid}
 
 
 class ClockSampler:
@@ -133,6 +134,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     plan = B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]), nsigma=cfg["nsigma"],
                   scatter_mode=mode, stream=stream)
+    plan.set_wire_mode({"auto": B.WCSIM_WIRES_AUTO, "fft": B.WCSIM_WIRES_FFT, "direct": B.WCSIM_WIRES_DIRECT}[args.wires])
     d = {k: torch.from_numpy(v).to(dev) for k, v in pl["depos"].items()}
     flush = torch.empty(FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
 
@@ -205,7 +207,8 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel --------------------------------------------------------------------------
     peaks = load_peaks()
-    sb = stage_bytes(pl)
+    direct = args.wires == "direct" or (args.wires == "auto" and pl["response"].shape[0] <= 64)
+    sb = stage_bytes(pl, direct)
     stage_rows = []
     for name in ("raster", "rows_forward", "cols", "rows_inverse"):
         ms, calls = stages[name]
@@ -237,6 +240,7 @@ def run_ours(args):
         "config": {"workload": cfg["name"] + (", fluctuation on" if fluct else ", fluctuation off"),
                    "grid": [pl["n_wires"], pl["n_ticks"]], "pad": [pl["pad_w"], pl["pad_t"]],
                    "response": list(pl["response"].shape), "depos": n_depos, "scatter": args.scatter,
+                   "wire_axis": "direct" if direct else "fft",
                    "parallelism": "replicas x%d" % world, "l2": "flushed between timed steps (256 MB write)"},
         "clocks": sampler.summary(),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -352,6 +356,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index of the timed workload")
     ap.add_argument("--scatter", default="atomic", choices=["atomic", "tiled"])
+    ap.add_argument("--wires", default="auto", choices=["auto", "fft", "direct"], help="wire axis of the convolution")
     ap.add_argument("--no-fluct", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=200)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")

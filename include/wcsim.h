@@ -41,6 +41,13 @@ typedef enum wcsim_status {
                                   integer / fixed-point arithmetic (order independent => bitwise reproducible)
                                   and stored once; "deterministic sort-by-tile mode" of BASELINE.json north_star */
 
+/* wire_mode of wcsim_set_wire_mode: how wcsim_convolve treats the wire axis of Eq. (2).  Both give the same M up to
+ * fp32 rounding (the cropped result is the linear convolution either way). */
+#define WCSIM_WIRES_AUTO 0   /* direct for responses up to 64 wires wide, FFT beyond (default) */
+#define WCSIM_WIRES_FFT 1    /* pad_w-point FFT, multiply by Rhat(w_t, w_x), inverse FFT: Eq. (2) literally */
+#define WCSIM_WIRES_DIRECT 2 /* tick axis by FFT, wire axis by direct summation over the n_rwires response offsets:
+                                Mhat(w_t, x) = sum_dx Rt(w_t, dx) Shat(w_t, x - dx) */
+
 typedef struct wcsim_plan wcsim_plan; /* opaque; owns S, M, the spectra, the response spectrum, twiddles, tile lists */
 
 /* FFT padding.  0 on an axis = automatic: the next power of two >= n_ticks + n_rticks - 1 (ticks) and
@@ -122,6 +129,7 @@ int wcsim_clear(wcsim_plan *plan);       /* S = 0 (enqueued) */
 int wcsim_clear_output(wcsim_plan *plan); /* M = 0 (enqueued) */
 int wcsim_sync(wcsim_plan *plan);        /* waits for the plan's stream; returns the first deferred CUDA fault */
 int wcsim_set_scatter_mode(wcsim_plan *plan, int scatter_mode);
+int wcsim_set_wire_mode(wcsim_plan *plan, int wire_mode);
 /* borrowed DEVICE pointers to n_wires*n_ticks floats, valid until wcsim_plan_destroy */
 int wcsim_charge_ptr(wcsim_plan *plan, float **dev);
 int wcsim_output_ptr(wcsim_plan *plan, float **dev);

@@ -15,11 +15,12 @@ from . import build as _build
 
 WCSIM_OK, WCSIM_EINVAL, WCSIM_ENOMEM, WCSIM_ECUDA, WCSIM_ESTATE = 0, -1, -2, -3, -4
 WCSIM_SCATTER_ATOMIC, WCSIM_SCATTER_TILED = 0, 1
+WCSIM_WIRES_AUTO, WCSIM_WIRES_FFT, WCSIM_WIRES_DIRECT = 0, 1, 2
 
 # every symbol include/wcsim.h declares (tests check that the library exports all of them)
 SYMBOLS = [
     "wcsim_plan_create", "wcsim_raster_scatter", "wcsim_convolve", "wcsim_add_noise", "wcsim_arm_noise",
-    "wcsim_plan_destroy", "wcsim_clear", "wcsim_clear_output", "wcsim_sync", "wcsim_set_scatter_mode",
+    "wcsim_plan_destroy", "wcsim_clear", "wcsim_clear_output", "wcsim_sync", "wcsim_set_scatter_mode", "wcsim_set_wire_mode",
     "wcsim_charge_ptr", "wcsim_output_ptr", "wcsim_get_dims", "wcsim_get_stats", "wcsim_reset_stats",
     "wcsim_simulate_host", "wcsim_set_profiling", "wcsim_get_stage_times", "wcsim_get_launch_count",
     "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum",
@@ -68,6 +69,7 @@ def lib():
         L.wcsim_clear_output.argtypes = [vp]
         L.wcsim_sync.argtypes = [vp]
         L.wcsim_set_scatter_mode.argtypes = [vp, i]
+        L.wcsim_set_wire_mode.argtypes = [vp, i]
         L.wcsim_charge_ptr.argtypes = [vp, C.POINTER(vp)]
         L.wcsim_output_ptr.argtypes = [vp, C.POINTER(vp)]
         L.wcsim_get_dims.argtypes = [vp] + [C.POINTER(i)] * 4
@@ -195,6 +197,10 @@ def wcsim_sync(plan):
 
 def wcsim_set_scatter_mode(plan, scatter_mode):
     _check(lib().wcsim_set_scatter_mode(plan, int(scatter_mode)), "wcsim_set_scatter_mode")
+
+
+def wcsim_set_wire_mode(plan, wire_mode):
+    _check(lib().wcsim_set_wire_mode(plan, int(wire_mode)), "wcsim_set_wire_mode")
 
 
 def wcsim_get_dims(plan):
@@ -339,6 +345,9 @@ class Plan:
 
     def set_scatter_mode(self, mode):
         wcsim_set_scatter_mode(self.handle, mode)
+
+    def set_wire_mode(self, mode):
+        wcsim_set_wire_mode(self.handle, mode)
 
     def charge(self):
         return wcsim_charge_ptr(self.handle)

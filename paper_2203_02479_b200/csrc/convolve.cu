@@ -110,6 +110,60 @@ __global__ void __launch_bounds__(ColCfg<N>::threads) cols_kernel(GridDims g, Co
 }
 
 // ------------------------------------------------------------------------------------------------------------------
+// a4 wire axis, a5 multiply, a6 wire axis, direct form.  With the tick axis transformed, Eq. (2)'s wire-axis
+// transform / multiply / inverse transform is, for every tick frequency k, the linear convolution
+//     Mhat[x][k] = sum_{d=0}^{n_rw-1} Rt[d][k] Shat[x + c - d][k],      Rt[d][.] = rfft_t(R[d][.]) / pad_t,
+// over the n_rw wire offsets of the response (Shat = 0 outside [0, n_wires)).  For the 21- and 41-wire responses of
+// BASELINE.json's configs that is 4 n_rw FMAs per output against the ~2 x 4.3 log2(pad_w) adds and multiplies of the
+// FFT route, needs no zero-padded wire rows, no shared memory, and reads n_rw rows of Rt (0.7 MB for configs[1])
+// instead of the pad_w rows of Rhat (33.6 MB).  One thread owns one k and O consecutive output wires; lanes run
+// along k (coalesced 256-byte rows); the response is walked in chunks of D offsets held in registers, so every
+// index below is static.  Neighbouring row groups of a CTA share their halo rows through L1.
+// ------------------------------------------------------------------------------------------------------------------
+constexpr int kWiresD = 7, kWiresRG = 8;
+
+template <int O, int D>
+__global__ void __launch_bounds__(32 * kWiresRG) wires_kernel(GridDims g, ConvBuffers b, int nk)
+{
+    const int k = blockIdx.x * 32 + threadIdx.x;
+    const int x0 = (blockIdx.y * kWiresRG + threadIdx.y) * O;
+    if (k >= nk || x0 >= g.n_wires) return;
+    const size_t stride = (size_t)b.spec_stride;
+    const float2 *__restrict__ in_k = b.spec + k;
+    const float2 *__restrict__ rt_k = b.Rt + k;
+    const int c = (b.n_rw - 1) / 2;
+    float2 acc[O];
+#pragma unroll
+    for (int o = 0; o < O; ++o) acc[o] = make_float2(0.f, 0.f);
+    for (int d0 = 0; d0 < b.rt_rows; d0 += D) {
+        float2 coef[D];
+#pragma unroll
+        for (int j = 0; j < D; ++j) coef[j] = __ldg(rt_k + (size_t)(d0 + j) * stride);
+        const int rbase = x0 + c - d0 - (D - 1); // wire row of in[0]
+        float2 in[O + D - 1];
+#pragma unroll
+        for (int q = 0; q < O + D - 1; ++q) {
+            const int row = rbase + q;
+            in[q] = (row >= 0 && row < g.n_wires) ? __ldg(in_k + (size_t)row * stride) : make_float2(0.f, 0.f);
+        }
+#pragma unroll
+        for (int o = 0; o < O; ++o)
+#pragma unroll
+            for (int j = 0; j < D; ++j) {
+                const float2 s = in[o - j + D - 1], w = coef[j];
+                acc[o].x = fmaf(w.x, s.x, acc[o].x);
+                acc[o].x = fmaf(-w.y, s.y, acc[o].x);
+                acc[o].y = fmaf(w.x, s.y, acc[o].y);
+                acc[o].y = fmaf(w.y, s.x, acc[o].y);
+            }
+    }
+    float2 *__restrict__ out_k = b.spec2 + k;
+#pragma unroll
+    for (int o = 0; o < O; ++o)
+        if (x0 + o < g.n_wires) out_k[(size_t)(x0 + o) * stride] = acc[o];
+}
+
+// ------------------------------------------------------------------------------------------------------------------
 // a6 tick axis (+ a7 noise): half spectrum -> real row
 // ------------------------------------------------------------------------------------------------------------------
 // noise spectrum of bin k on `wire`: amp[k] exp(2 pi i u), u = (word + 1/2) 2^-32 (A15-A17); amp is pre-scaled
@@ -130,7 +184,7 @@ __global__ void __launch_bounds__(RowCfg<N>::threads) rows_inverse_kernel(GridDi
     constexpr int E = RowCfg<N>::E, NT = N / E;
     extern __shared__ float2 smem[];
     const int row = blockIdx.x, i = threadIdx.x;
-    const float2 *src = b.spec + (size_t)row * b.spec_stride;
+    const float2 *src = b.spec_inv + (size_t)row * b.spec_stride;
     const bool noisy = nz.amp != nullptr;
     // stage X_k (+ noise) in shared memory so that every thread can reach the partner X_{N-k}
 #pragma unroll
@@ -271,6 +325,17 @@ cudaError_t launch_cols(GridDims g, int pad_w, int pad_t, ConvBuffers b, cudaStr
     default:
         return cudaErrorInvalidValue;
     }
+    return cudaGetLastError();
+}
+
+int wires_chunk() { return kWiresD; }
+
+cudaError_t launch_wires(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st)
+{
+    constexpr int O = 8;
+    const int nk = pad_t / 2 + 1;
+    const dim3 block(32, kWiresRG), grid((nk + 31) / 32, (g.n_wires + O * kWiresRG - 1) / (O * kWiresRG));
+    wires_kernel<O, kWiresD><<<grid, block, 0, st>>>(g, b, nk);
     return cudaGetLastError();
 }
 

@@ -12,6 +12,7 @@
 // CPU (threads emulated by loops) against numpy.fft.
 #pragma once
 #include <cuda_runtime.h>
+#include <math.h>
 
 #ifndef WCSIM_HD
 #define WCSIM_HD __host__ __device__ __forceinline__
@@ -159,7 +160,35 @@ WCSIM_HD float2 load_tw(const float2 *__restrict__ tw, int idx)
 #endif
 }
 
-// One pass: twiddle + butterflies on the registers.  tw[j] = exp(-2 pi i j / N), j < N.
+// Twiddle tables, one per pass, laid out so that a warp's loads coalesce: for the pass that starts with P points
+// already combined (P > 1; its radix is 16) the factor of input r of the butterfly with k = b mod P sits at
+//   tw[tw_offset(N, P) + (r-1) P + k] = exp(-2 pi i r k / (16 P)),   r = 1..15, k < P.
+// Lanes of a warp hold consecutive k, so each of the 15 loads touches P-contiguous entries (a flat table indexed
+// r*k*step would cost up to 16 L1 wavefronts per load instead of 1-2).
+constexpr int first_radix(int n) { return (ilog2(n) % 4) ? (1 << (ilog2(n) % 4)) : 16; }
+constexpr int tw_offset(int n, int P)
+{
+    int off = 0;
+    for (int p = first_radix(n); p < P; p *= 16) off += 15 * p;
+    return off;
+}
+constexpr int tw_size(int n) { return tw_offset(n, n) > 0 ? tw_offset(n, n) : 1; }
+
+// host-side builder of the table above (fp64 angles, rounded once)
+inline void build_pass_twiddles(int n, float2 *out)
+{
+    int off = 0;
+    for (int p = first_radix(n); p < n; p *= 16) {
+        for (int r = 1; r < 16; ++r)
+            for (int k = 0; k < p; ++k) {
+                const double a = -2.0 * 3.14159265358979323846 * (double)r * (double)k / (16.0 * (double)p);
+                out[off + (r - 1) * p + k] = make_float2((float)cos(a), (float)sin(a));
+            }
+        off += 15 * p;
+    }
+}
+
+// One pass: twiddle + butterflies on the registers.
 template <int N, int E, int R, int P, int DIR>
 WCSIM_HD void fft_pass(float2 (&v)[E], int i, const float2 *__restrict__ tw)
 {
@@ -171,12 +200,13 @@ WCSIM_HD void fft_pass(float2 (&v)[E], int i, const float2 *__restrict__ tw)
 #pragma unroll
         for (int r = 0; r < R; ++r) x[r] = v[u + r * NB];
         if constexpr (P > 1) {
+            static_assert(R == 16, "passes after the first are radix 16");
             const int b = i + u * (N / E);
             const int k = b & (P - 1);
-            constexpr int step = N / (P * R);
+            constexpr int off = tw_offset(N, P);
 #pragma unroll
             for (int r = 1; r < R; ++r) {
-                float2 w = load_tw(tw, r * k * step);
+                float2 w = load_tw(tw, off + (r - 1) * P + k);
                 if (DIR > 0) w.y = -w.y;
                 x[r] = cmul(x[r], w);
             }

@@ -51,11 +51,15 @@ cudaError_t launch_tile_accumulate(GridDims g, DepoArrays d, uint64_t id_base, u
 struct ConvBuffers {
     const float *S;       // [n_wires][n_ticks]
     float *M;             // [n_wires][n_ticks]
-    float2 *spec;         // [n_wires][spec_stride]  row spectra, then (in place) the product spectra
+    float2 *spec;         // [n_wires][spec_stride]  row spectra (FFT wire mode: then, in place, the product spectra)
+    float2 *spec2;        // [n_wires][spec_stride]  product spectra of the direct wire mode
+    const float2 *spec_inv; // what rows_inverse reads: spec (FFT wire mode) or spec2 (direct wire mode)
+    const float2 *Rt;     // [rt_rows][spec_stride]  rfft_t(R[d]) / pad_t, rows d >= n_rw are zero (direct wire mode)
+    int rt_rows, n_rw;    // rt_rows = n_rw rounded up to a multiple of wires_chunk()
     const float2 *Rhat;   // [pad_w][spec_stride]
-    const float2 *tw_row; // [pad_t/2]  exp(-2 pi i j / (pad_t/2))
+    const float2 *tw_row; // per-pass twiddle tables of a pad_t/2-point FFT (fft.cuh)
     const float2 *tw_real;// [pad_t/2]  exp(-2 pi i j / pad_t)
-    const float2 *tw_col; // [pad_w]    exp(-2 pi i j / pad_w)
+    const float2 *tw_col; // per-pass twiddle tables of a pad_w-point FFT
     int spec_stride;      // pad_t/2 + 8
 };
 struct NoiseArgs {
@@ -66,6 +70,8 @@ bool conv_sizes_supported(int pad_w, int pad_t);
 cudaError_t conv_configure(int pad_w, int pad_t); // sets the kernels' shared-memory attributes (once per plan)
 cudaError_t launch_rows_forward(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st);
 cudaError_t launch_cols(GridDims g, int pad_w, int pad_t, ConvBuffers b, cudaStream_t st);
+int wires_chunk(); // response offsets per register chunk of the direct wire-axis kernel
+cudaError_t launch_wires(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st);
 // M = (accumulate ? M : 0) + c2r(use_spec ? spec : 0  +  noise)
 cudaError_t launch_rows_inverse(GridDims g, int pad_t, ConvBuffers b, NoiseArgs noise, bool use_spec, bool accumulate,
                                 cudaStream_t st);
@@ -74,6 +80,9 @@ cudaError_t launch_rows_inverse(GridDims g, int pad_t, ConvBuffers b, NoiseArgs 
 // Rhat[kx][kt] = 1/(pad_w pad_t) sum_dx sum_dt R[dx+c][dt] exp(-2 pi i (kx dx / pad_w + kt dt / pad_t)), fp64 -> fp32
 cudaError_t build_response_spectrum(const float *dev_R, int n_rw, int n_rt, int pad_w, int pad_t, int spec_stride,
                                     double2 *dev_tmp /* [n_rw][pad_t/2+1] */, float2 *dev_Rhat, cudaStream_t st);
+// Rt[d][kt] = tmp[d][kt] / pad_t for d < n_rw, 0 for n_rw <= d < rt_rows (and in the padding columns); after the above
+cudaError_t build_response_rows(const double2 *dev_tmp, int n_rw, int rt_rows, int pad_t, int spec_stride,
+                                float2 *dev_Rt, cudaStream_t st);
 
 // ---- debug.cu ----
 cudaError_t launch_debug_philox(const unsigned int *ctr, const unsigned int *key, unsigned int *out, long long n,

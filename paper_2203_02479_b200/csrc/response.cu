@@ -60,6 +60,22 @@ __global__ void response_wires_kernel(const double2 *__restrict__ tmp, int n_rw,
     Rhat[(size_t)kx * spec_stride + kt] = out;
 }
 
+// Rt[d][kt] = tmp[d][kt] / pad_t: the tick-axis spectrum of each wire offset of the response (direct wire mode)
+__global__ void response_rows_kernel(const double2 *__restrict__ tmp, int n_rw, int pad_t, int spec_stride,
+                                     float2 *__restrict__ Rt)
+{
+    const int kt = blockIdx.x * blockDim.x + threadIdx.x;
+    const int d = blockIdx.y;
+    if (kt >= spec_stride) return;
+    float2 out = make_float2(0.f, 0.f);
+    if (d < n_rw && kt <= pad_t / 2) {
+        const double2 v = tmp[(size_t)d * (pad_t / 2 + 1) + kt];
+        const double scale = 1.0 / (double)pad_t;
+        out = make_float2((float)(v.x * scale), (float)(v.y * scale));
+    }
+    Rt[(size_t)d * spec_stride + kt] = out;
+}
+
 __global__ void debug_philox_kernel(const unsigned int *ctr, const unsigned int *key, unsigned int *out, long long n)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -91,6 +107,15 @@ cudaError_t build_response_spectrum(const float *dev_R, int n_rw, int n_rt, int 
     if (err != cudaSuccess) return err;
     dim3 g2((spec_stride + threads - 1) / threads, pad_w);
     response_wires_kernel<<<g2, threads, 0, st>>>(dev_tmp, n_rw, pad_w, pad_t, spec_stride, dev_Rhat);
+    return cudaGetLastError();
+}
+
+cudaError_t build_response_rows(const double2 *dev_tmp, int n_rw, int rt_rows, int pad_t, int spec_stride,
+                                float2 *dev_Rt, cudaStream_t st)
+{
+    const int threads = 128;
+    dim3 grid((spec_stride + threads - 1) / threads, rt_rows);
+    response_rows_kernel<<<grid, threads, 0, st>>>(dev_tmp, n_rw, pad_t, spec_stride, dev_Rt);
     return cudaGetLastError();
 }
 

@@ -1,6 +1,7 @@
 // wcsim.cu -- the C ABI of include/wcsim.h: plan life cycle, argument checking, buffer ownership and the launch
 // sequences.  All arithmetic of the path lives in raster.cu / convolve.cu / response.cu; there is no CPU fallback.
 #include "../../include/wcsim.h"
+#include "fft.cuh"
 #include "internal.h"
 
 #include <cmath>
@@ -18,7 +19,10 @@ struct wcsim_plan {
     cudaStream_t stream = nullptr;
     int device = 0, sm_count = 148;
     float *S = nullptr, *M = nullptr;
-    float2 *spec = nullptr, *Rhat = nullptr, *tw_row = nullptr, *tw_real = nullptr, *tw_col = nullptr;
+    float2 *spec = nullptr, *spec2 = nullptr, *Rhat = nullptr, *Rt = nullptr;
+    float2 *tw_row = nullptr, *tw_real = nullptr, *tw_col = nullptr;
+    int rt_rows = 0;
+    int wire_mode = WCSIM_WIRES_AUTO;
     Counters *counters = nullptr;
     float *amp_builtin = nullptr, *amp_custom = nullptr; // device, pad_t/2+1, scaled by pad_t^-1/2
     bool noise_armed = false;
@@ -136,13 +140,27 @@ int next_pow2(long long n, int floor_)
     return p > (1 << 30) ? 0 : (int)p;
 }
 
+// Wire axis of the convolution: direct summation over the response's wire offsets, or FFT / multiply / inverse FFT.
+// Per output the direct form costs 4 n_rw FMAs, the FFT form ~2 x 4.3 log2(pad_w) adds and multiplies at half the
+// FMA rate plus the read of Rhat; AUTO takes the direct form up to 64 response wires (measured crossover: DESIGN.md).
+bool wires_direct(const wcsim_plan *p)
+{
+    if (p->wire_mode == WCSIM_WIRES_AUTO) return p->n_rw <= 64;
+    return p->wire_mode == WCSIM_WIRES_DIRECT;
+}
+
 ConvBuffers conv_buffers(const wcsim_plan *p)
 {
     ConvBuffers b;
     b.S = p->S;
     b.M = p->M;
     b.spec = p->spec;
+    b.spec2 = p->spec2;
+    b.spec_inv = wires_direct(p) ? p->spec2 : p->spec;
     b.Rhat = p->Rhat;
+    b.Rt = p->Rt;
+    b.rt_rows = p->rt_rows;
+    b.n_rw = p->n_rw;
     b.tw_row = p->tw_row;
     b.tw_real = p->tw_real;
     b.tw_col = p->tw_col;
@@ -150,13 +168,19 @@ ConvBuffers conv_buffers(const wcsim_plan *p)
     return b;
 }
 
+// denom > 0: flat table exp(-2 pi i j / denom), j < n.  denom = 0: the per-pass tables of fft.cuh for an n-point FFT.
 int upload_twiddles(float2 **dev, int n, int denom, cudaStream_t st)
 {
-    std::vector<float2> h((size_t)n);
-    for (int j = 0; j < n; ++j) {
-        const double a = -2.0 * M_PI * (double)j / (double)denom;
-        h[j] = make_float2((float)cos(a), (float)sin(a));
+    std::vector<float2> h((size_t)(denom > 0 ? n : tw_size(n)));
+    if (denom > 0) {
+        for (int j = 0; j < n; ++j) {
+            const double a = -2.0 * M_PI * (double)j / (double)denom;
+            h[j] = make_float2((float)cos(a), (float)sin(a));
+        }
+    } else {
+        build_pass_twiddles(n, h.data());
     }
+    n = (int)h.size();
     CU_TRY(cudaMalloc((void **)dev, sizeof(float2) * (size_t)n));
     CU_TRY(cudaMemcpyAsync(*dev, h.data(), sizeof(float2) * (size_t)n, cudaMemcpyHostToDevice, st));
     CU_TRY(cudaStreamSynchronize(st));
@@ -230,7 +254,8 @@ int destroy_impl(wcsim_plan *p)
 {
     int rc = WCSIM_OK;
     if (cudaStreamSynchronize(p->stream) != cudaSuccess) rc = fail_cuda(cudaGetLastError());
-    void *bufs[] = {p->S,        p->M,           p->spec,        p->Rhat,           p->tw_row,        p->tw_real,
+    void *bufs[] = {p->spec2,    p->Rt,
+                    p->S,        p->M,           p->spec,        p->Rhat,           p->tw_row,        p->tw_real,
                     p->tw_col,   p->counters,    p->amp_builtin, p->amp_custom,     p->ts.tile_count, p->ts.tile_cursor,
                     p->ts.entries, p->ts.total,  p->stage[0],    p->stage[1],       p->stage[2],      p->stage[3],
                     p->stage[4]};
@@ -294,19 +319,23 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
         CU_TRY(cudaMalloc((void **)&p->S, sizeof(float) * grid));
         CU_TRY(cudaMalloc((void **)&p->M, sizeof(float) * grid));
         CU_TRY(cudaMalloc((void **)&p->spec, sizeof(float2) * (size_t)n_wires * p->spec_stride));
+        CU_TRY(cudaMalloc((void **)&p->spec2, sizeof(float2) * (size_t)n_wires * p->spec_stride));
         CU_TRY(cudaMalloc((void **)&p->Rhat, sizeof(float2) * (size_t)pad_w * p->spec_stride));
+        p->rt_rows = (n_rwires + wires_chunk() - 1) / wires_chunk() * wires_chunk();
+        CU_TRY(cudaMalloc((void **)&p->Rt, sizeof(float2) * (size_t)p->rt_rows * p->spec_stride));
         CU_TRY(cudaMalloc((void **)&p->counters, sizeof(Counters)));
         CU_TRY(cudaMalloc((void **)&p->amp_builtin, sizeof(float) * (size_t)(pad_t / 2 + 1)));
         CU_TRY(cudaMalloc((void **)&p->amp_custom, sizeof(float) * (size_t)(pad_t / 2 + 1)));
         CU_TRY(cudaMemsetAsync(p->S, 0, sizeof(float) * grid, p->stream));
         CU_TRY(cudaMemsetAsync(p->M, 0, sizeof(float) * grid, p->stream));
         CU_TRY(cudaMemsetAsync(p->spec, 0, sizeof(float2) * (size_t)n_wires * p->spec_stride, p->stream));
+        CU_TRY(cudaMemsetAsync(p->spec2, 0, sizeof(float2) * (size_t)n_wires * p->spec_stride, p->stream));
         CU_TRY(cudaMemsetAsync(p->counters, 0, sizeof(Counters), p->stream));
-        int r = upload_twiddles(&p->tw_row, pad_t / 2, pad_t / 2, p->stream);
+        int r = upload_twiddles(&p->tw_row, pad_t / 2, 0, p->stream);
         if (r) return r;
         r = upload_twiddles(&p->tw_real, pad_t / 2, pad_t, p->stream);
         if (r) return r;
-        r = upload_twiddles(&p->tw_col, pad_w, pad_w, p->stream);
+        r = upload_twiddles(&p->tw_col, pad_w, 0, p->stream);
         if (r) return r;
         r = upload_amp(p, nullptr, p->amp_builtin);
         if (r) return r;
@@ -326,6 +355,7 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
         CU_TRY(cudaMemcpyAsync(dev_R, response, sizeof(float) * nr, cudaMemcpyHostToDevice, p->stream));
         CU_TRY(build_response_spectrum(dev_R, n_rwires, n_rticks, pad_w, pad_t, p->spec_stride, dev_tmp, p->Rhat,
                                        p->stream));
+        CU_TRY(build_response_rows(dev_tmp, n_rwires, p->rt_rows, pad_t, p->spec_stride, p->Rt, p->stream));
         CU_TRY(conv_configure(pad_w, pad_t));
         CU_TRY(raster_configure());
         CU_TRY(cudaStreamSynchronize(p->stream));
@@ -387,7 +417,10 @@ int wcsim_convolve(wcsim_plan *plan)
     }
     {
         StageSpan span(plan, WCSIM_STAGE_COLS);
-        CU_TRY(launch_cols(g, plan->pad_w, plan->pad_t, b, plan->stream));
+        if (wires_direct(plan))
+            CU_TRY(launch_wires(g, plan->pad_t, b, plan->stream));
+        else
+            CU_TRY(launch_cols(g, plan->pad_w, plan->pad_t, b, plan->stream));
     }
     {
         StageSpan span(plan, WCSIM_STAGE_ROWS_INVERSE);
@@ -472,6 +505,13 @@ int wcsim_set_scatter_mode(wcsim_plan *plan, int scatter_mode)
 {
     if (!plan || (scatter_mode != WCSIM_SCATTER_ATOMIC && scatter_mode != WCSIM_SCATTER_TILED)) return WCSIM_EINVAL;
     plan->scatter_mode = scatter_mode;
+    return WCSIM_OK;
+}
+
+int wcsim_set_wire_mode(wcsim_plan *plan, int wire_mode)
+{
+    if (!plan || wire_mode < WCSIM_WIRES_AUTO || wire_mode > WCSIM_WIRES_DIRECT) return WCSIM_EINVAL;
+    plan->wire_mode = wire_mode;
     return WCSIM_OK;
 }
 

@@ -37,8 +37,8 @@ template <int N, int C, int E, int DIR>
 static double check()
 {
     constexpr int NT = (N / E) * C;
-    std::vector<float2> tw(N);
-    for (int j = 0; j < N; ++j) tw[j] = make_float2((float)cos(2.0 * M_PI * j / N), (float)-sin(2.0 * M_PI * j / N));
+    std::vector<float2> tw(tw_size(N));
+    build_pass_twiddles(N, tw.data());
     std::vector<double> xr((size_t)N * C), xi((size_t)N * C);
     srand(N * 31 + C * 7 + E + DIR);
     for (auto &x : xr) x = rand() / (double)RAND_MAX - 0.5;

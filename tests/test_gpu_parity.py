@@ -138,17 +138,21 @@ def test_convolve_alone_matches_definition(B, O):
     """Random dense S written straight into the plan's buffer: isolates a4-a6 from the raster."""
     from paper_2203_02479_b200 import synth
     rng = np.random.default_rng(11)
-    for (nw, nt, pw, pt, rw, rt) in [(64, 512, 128, 1024, 21, 200), (50, 301, 64, 512, 5, 40), (16, 40, 32, 64, 3, 9)]:
+    for (nw, nt, pw, pt, rw, rt) in [(64, 512, 128, 1024, 21, 200), (50, 301, 64, 512, 5, 40), (16, 40, 32, 64, 3, 9),
+                                     (100, 90, 128, 128, 41, 30), (70, 60, 128, 64, 1, 5), (37, 500, 64, 1024, 15, 7)]:
         R = synth.response(rw, rt)
         S = (rng.standard_normal((nw, nt)) * (rng.random((nw, nt)) < 0.2)).astype(np.float32)
         M_ref = O.convolve_direct(S.astype(np.float64), R)
         with B.Plan(nw, nt, R, pad=(pw, pt)) as p:
             p.charge().copy_(torch.from_numpy(S).cuda())
-            p.convolve()
-            p.sync()
-            M = p.output().cpu().numpy()
-            assert np.array_equal(p.charge().cpu().numpy(), S), "S must be preserved"
-        assert_close(M, M_ref, "M %dx%d" % (nw, nt))
+            for mode in (B.WCSIM_WIRES_FFT, B.WCSIM_WIRES_DIRECT, B.WCSIM_WIRES_AUTO):
+                p.set_wire_mode(mode)
+                p.clear_output()
+                p.convolve()
+                p.sync()
+                M = p.output().cpu().numpy()
+                assert np.array_equal(p.charge().cpu().numpy(), S), "S must be preserved"
+                assert_close(M, M_ref, "M %dx%d wire mode %d" % (nw, nt, mode))
 
 
 def test_delta_reproduces_response(B):
