@@ -172,7 +172,7 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v)
 constexpr int kBatchWarps = 4;          // warps per CTA
 constexpr int kBatchShift = 3;          // log2 of the depos a warp fetches at a time (lanes beyond that own no depo):
 constexpr int kBatchDepos = 1 << kBatchShift; // small batches keep the per-warp serial path short and the load balanced
-constexpr int kEdgeCap = 256;           // edge values per warp scratch (8 patches of 16 x 5 bins need 184)
+constexpr int kEdgeCap = 128;           // edge values per warp scratch (8 patches of 16 x 5 bins need 184)
 constexpr int kQueueCap = 64;           // entries per draw queue (at most 31 left over + 32 pushed)
 
 template <bool FLUCT>
@@ -241,7 +241,7 @@ __device__ __forceinline__ void drain_queue(DrawQueues &Q, int cls, int &count, 
 }
 
 template <bool FLUCT>
-__global__ void __launch_bounds__(kBatchWarps * 32) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
+__global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
                                                                         uint64_t id_base, uint64_t seed, double nsigma,
                                                                         float *__restrict__ S, int *__restrict__ totals,
                                                                         Counters *counters)
@@ -577,7 +577,8 @@ cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t
     if (n <= 0) return cudaSuccess;
     const long long n_batches = (n + kBatchDepos - 1) / kBatchDepos;
     const size_t smem = fluctuate ? sizeof(BatchSmem<true>) : sizeof(BatchSmem<false>);
-    const int ctas_per_sm = (int)((200u * 1024u) / smem) > 8 ? 8 : (int)((200u * 1024u) / smem);
+    const int fit = (int)((227u * 1024u) / (smem + 1024u)); // 227 KB per SM, 1 KB reserved per CTA
+    const int ctas_per_sm = fit > 8 ? 8 : fit;
     long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
     const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
     if (ctas > max_ctas) ctas = max_ctas;
