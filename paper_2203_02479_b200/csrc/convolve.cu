@@ -26,6 +26,8 @@ struct RowCfg {
     static constexpr int E = 16;
     static constexpr int threads = N / E;
     static constexpr int smem_bytes = SmemSize<N, 1>::float2s * (int)sizeof(float2);
+    // 64 registers per thread: 1024 threads of row transforms resident per SM whatever the row length
+    static constexpr int min_ctas = threads >= 1024 ? 1 : (1024 / threads > 8 ? 8 : 1024 / threads);
 };
 template <int N>
 struct ColCfg {
@@ -39,7 +41,7 @@ struct ColCfg {
 // a4, tick axis: real row -> half spectrum
 // ------------------------------------------------------------------------------------------------------------------
 template <int N, bool VEC>
-__global__ void __launch_bounds__(RowCfg<N>::threads) rows_forward_kernel(GridDims g, ConvBuffers b)
+__global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_forward_kernel(GridDims g, ConvBuffers b)
 {
     constexpr int E = RowCfg<N>::E, NT = N / E;
     extern __shared__ float2 smem[];
@@ -118,49 +120,54 @@ __global__ void __launch_bounds__(ColCfg<N>::threads) cols_kernel(GridDims g, Co
 // FFT route, needs no zero-padded wire rows, no shared memory, and reads n_rw rows of Rt (0.7 MB for configs[1])
 // instead of the pad_w rows of Rhat (33.6 MB).  One thread owns one k and O consecutive output wires; lanes run
 // along k (coalesced 256-byte rows); the response is walked in chunks of D offsets held in registers, so every
-// index below is static.  Neighbouring row groups of a CTA share their halo rows through L1.
+// register index below is static.  The spectrum buffer carries zero halo rows below wire 0 and above wire
+// n_wires-1 (wires_halo(), written once at plan time), so no load is predicated, and with the row stride a template
+// argument every load of a chunk is one instruction off a single pointer (immediate offsets): the inner loop is
+// 4 O D FFMAs against O + 2 D - 1 loads.  Neighbouring row groups of a CTA share their halo rows through L1.
 // ------------------------------------------------------------------------------------------------------------------
-constexpr int kWiresD = 7, kWiresRG = 8;
+constexpr int kWiresD = 7, kWiresRG = 8, kWiresO = 8;
 
-template <int O, int D>
-__global__ void __launch_bounds__(32 * kWiresRG) wires_kernel(GridDims g, ConvBuffers b, int nk)
+// STRIDE = 0: row stride read from the buffers (any pad_t); NCH = 0: chunk count read from the buffers (any n_rw),
+// else the chunk loop is unrolled so that the loads of the next chunk are in flight under the FFMAs of this one
+template <int O, int D, int NCH, int STRIDE>
+__global__ void __launch_bounds__(32 * kWiresRG, 3) wires_kernel(GridDims g, ConvBuffers b, int nk)
 {
     const int k = blockIdx.x * 32 + threadIdx.x;
     const int x0 = (blockIdx.y * kWiresRG + threadIdx.y) * O;
     if (k >= nk || x0 >= g.n_wires) return;
-    const size_t stride = (size_t)b.spec_stride;
-    const float2 *__restrict__ in_k = b.spec + k;
-    const float2 *__restrict__ rt_k = b.Rt + k;
+    const ptrdiff_t stride = STRIDE ? (ptrdiff_t)STRIDE : (ptrdiff_t)b.spec_stride;
     const int c = (b.n_rw - 1) / 2;
     float2 acc[O];
 #pragma unroll
     for (int o = 0; o < O; ++o) acc[o] = make_float2(0.f, 0.f);
-    for (int d0 = 0; d0 < b.rt_rows; d0 += D) {
-        float2 coef[D];
+    // chunk d0 uses wire rows x0 + c - d0 - (D-1) .. x0 + c - d0 + O - 1 (halo rows included) and Rt rows d0 .. d0+D-1
+    const float2 *__restrict__ in = b.spec + k + ((ptrdiff_t)x0 + c - (D - 1)) * stride;
+    const float2 *__restrict__ rt = b.Rt + k;
+    const int n_chunks = NCH ? NCH : b.rt_rows / D;
 #pragma unroll
-        for (int j = 0; j < D; ++j) coef[j] = __ldg(rt_k + (size_t)(d0 + j) * stride);
-        const int rbase = x0 + c - d0 - (D - 1); // wire row of in[0]
-        float2 in[O + D - 1];
+    for (int ch = 0; ch < n_chunks; ++ch) {
+        float2 coef[D], s[O + D - 1];
 #pragma unroll
-        for (int q = 0; q < O + D - 1; ++q) {
-            const int row = rbase + q;
-            in[q] = (row >= 0 && row < g.n_wires) ? __ldg(in_k + (size_t)row * stride) : make_float2(0.f, 0.f);
-        }
+        for (int j = 0; j < D; ++j) coef[j] = __ldg(rt + j * stride);
+#pragma unroll
+        for (int q = 0; q < O + D - 1; ++q) s[q] = __ldg(in + q * stride);
 #pragma unroll
         for (int o = 0; o < O; ++o)
 #pragma unroll
             for (int j = 0; j < D; ++j) {
-                const float2 s = in[o - j + D - 1], w = coef[j];
-                acc[o].x = fmaf(w.x, s.x, acc[o].x);
-                acc[o].x = fmaf(-w.y, s.y, acc[o].x);
-                acc[o].y = fmaf(w.x, s.y, acc[o].y);
-                acc[o].y = fmaf(w.y, s.x, acc[o].y);
+                const float2 v = s[o - j + D - 1], w = coef[j];
+                acc[o].x = fmaf(w.x, v.x, acc[o].x);
+                acc[o].x = fmaf(-w.y, v.y, acc[o].x);
+                acc[o].y = fmaf(w.x, v.y, acc[o].y);
+                acc[o].y = fmaf(w.y, v.x, acc[o].y);
             }
+        in -= D * stride;
+        rt += D * stride;
     }
-    float2 *__restrict__ out_k = b.spec2 + k;
+    float2 *__restrict__ out = b.spec2 + k + (ptrdiff_t)x0 * stride;
 #pragma unroll
     for (int o = 0; o < O; ++o)
-        if (x0 + o < g.n_wires) out_k[(size_t)(x0 + o) * stride] = acc[o];
+        if (x0 + o < g.n_wires) out[o * stride] = acc[o];
 }
 
 // ------------------------------------------------------------------------------------------------------------------
@@ -178,7 +185,7 @@ __device__ __forceinline__ float2 noise_bin(const NoiseArgs &nz, uint32_t wire, 
 }
 
 template <int N, bool VEC>
-__global__ void __launch_bounds__(RowCfg<N>::threads) rows_inverse_kernel(GridDims g, ConvBuffers b, NoiseArgs nz,
+__global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_inverse_kernel(GridDims g, ConvBuffers b, NoiseArgs nz,
                                                                            bool use_spec, bool accumulate)
 {
     constexpr int E = RowCfg<N>::E, NT = N / E;
@@ -330,12 +337,29 @@ cudaError_t launch_cols(GridDims g, int pad_w, int pad_t, ConvBuffers b, cudaStr
 
 int wires_chunk() { return kWiresD; }
 
+// zero rows the direct wire kernel may read below wire 0 / above wire n_wires-1 of the row spectra
+void wires_halo(int n_rw, int *below, int *above)
+{
+    const int c = (n_rw - 1) / 2;
+    const int rt_rows = (n_rw + kWiresD - 1) / kWiresD * kWiresD;
+    *below = rt_rows - 1 - c; // lowest row read: 0 + c - (rt_rows - D) - (D - 1)
+    *above = kWiresO - 1 + c; // highest: (n_wires - 1) + (O - 1) + c, from the last, ragged row group
+}
+
 cudaError_t launch_wires(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st)
 {
-    constexpr int O = 8;
+    constexpr int O = kWiresO;
     const int nk = pad_t / 2 + 1;
     const dim3 block(32, kWiresRG), grid((nk + 31) / 32, (g.n_wires + O * kWiresRG - 1) / (O * kWiresRG));
-    wires_kernel<O, kWiresD><<<grid, block, 0, st>>>(g, b, nk);
+    // BASELINE.json's paddings and response widths (21 wires -> 3 chunks, 41 -> 6) get immediate-offset loads and an
+    // unrolled chunk loop; anything else takes the generic instance
+    const int key = b.rt_rows / kWiresD * 100000 + b.spec_stride;
+    switch (key) {
+    case 3 * 100000 + 1024 / 2 + 8: wires_kernel<O, kWiresD, 3, 1024 / 2 + 8><<<grid, block, 0, st>>>(g, b, nk); break;
+    case 3 * 100000 + 8192 / 2 + 8: wires_kernel<O, kWiresD, 3, 8192 / 2 + 8><<<grid, block, 0, st>>>(g, b, nk); break;
+    case 6 * 100000 + 16384 / 2 + 8: wires_kernel<O, kWiresD, 6, 16384 / 2 + 8><<<grid, block, 0, st>>>(g, b, nk); break;
+    default: wires_kernel<O, kWiresD, 0, 0><<<grid, block, 0, st>>>(g, b, nk); break;
+    }
     return cudaGetLastError();
 }
 

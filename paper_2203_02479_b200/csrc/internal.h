@@ -51,7 +51,8 @@ cudaError_t launch_tile_accumulate(GridDims g, DepoArrays d, uint64_t id_base, u
 struct ConvBuffers {
     const float *S;       // [n_wires][n_ticks]
     float *M;             // [n_wires][n_ticks]
-    float2 *spec;         // [n_wires][spec_stride]  row spectra (FFT wire mode: then, in place, the product spectra)
+    float2 *spec;         // [n_wires][spec_stride]  row spectra (FFT wire mode: then, in place, the product spectra);
+                          // wires_halo() zero rows sit below row 0 and above row n_wires-1 of the allocation
     float2 *spec2;        // [n_wires][spec_stride]  product spectra of the direct wire mode
     const float2 *spec_inv; // what rows_inverse reads: spec (FFT wire mode) or spec2 (direct wire mode)
     const float2 *Rt;     // [rt_rows][spec_stride]  rfft_t(R[d]) / pad_t, rows d >= n_rw are zero (direct wire mode)
@@ -71,6 +72,7 @@ cudaError_t conv_configure(int pad_w, int pad_t); // sets the kernels' shared-me
 cudaError_t launch_rows_forward(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st);
 cudaError_t launch_cols(GridDims g, int pad_w, int pad_t, ConvBuffers b, cudaStream_t st);
 int wires_chunk(); // response offsets per register chunk of the direct wire-axis kernel
+void wires_halo(int n_rw, int *below, int *above); // zero rows of `spec` that kernel reads outside [0, n_wires)
 cudaError_t launch_wires(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st);
 // M = (accumulate ? M : 0) + c2r(use_spec ? spec : 0  +  noise)
 cudaError_t launch_rows_inverse(GridDims g, int pad_t, ConvBuffers b, NoiseArgs noise, bool use_spec, bool accumulate,

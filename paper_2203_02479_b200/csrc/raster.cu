@@ -334,7 +334,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
                 } else {
                     const double dd = __dsub_rn((double)coord, centre);
                     if constexpr (FLUCT) {
-                        E = erf(__ddiv_rn(dd, __dmul_rn(1.4142135623730951, sigma)));
+                        E = erf(fast_div(dd, 1.4142135623730951 * sigma));
                     } else {
                         const float inv = 1.0f / (1.41421356f * (float)sigma);
                         E = erff((float)dd * inv);
@@ -374,18 +374,24 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
                         if (totals != nullptr) atomicAdd(totals + (batch << kBatchShift) + own, (int)v);
                     }
                     DrawQueues &Q = sm.queues[wid];
+                    // one slot per bin in the queue of its class: position = queue fill + rank among the lanes of the
+                    // same class (ballots), then a single block of stores for all classes
+                    unsigned int mine = 0;
+                    int base = 0;
 #pragma unroll
                     for (int c = 0; c < kNumDrawQueues; ++c) {
                         const unsigned int m = __ballot_sync(0xffffffffu, cls == c);
-                        if (cls == c) {
-                            const int pos = qcount[c] + __popc(m & ((1u << lane) - 1u));
-                            Q.p[c][pos] = p;
-                            Q.N[c][pos] = (float)Nn;
-                            Q.w[c][pos] = w;
-                            Q.bin[c][pos] = (uint32_t)gbin;
-                            Q.flags[c][pos] = fl;
-                        }
+                        mine = (cls == c) ? m : mine;
+                        base = (cls == c) ? qcount[c] : base;
                         qcount[c] += __popc(m);
+                    }
+                    if (cls >= 0) {
+                        const int pos = base + __popc(mine & ((1u << lane) - 1u));
+                        Q.p[cls][pos] = p;
+                        Q.N[cls][pos] = (float)Nn;
+                        Q.w[cls][pos] = w;
+                        Q.bin[cls][pos] = (uint32_t)gbin;
+                        Q.flags[cls][pos] = fl;
                     }
                     __syncwarp();
 #pragma unroll

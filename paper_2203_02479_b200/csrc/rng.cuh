@@ -49,9 +49,9 @@ __device__ __forceinline__ uint4 noise_words(uint64_t seed, uint32_t wire, uint3
 //   mu = N p < 16: inversion of the CDF from k = 0;  else clamp(rint(mu + sqrt(mu (1-p)) Phi^-1(u)), 0, N).
 // The sampler is split into a classification and three straight-line draw routines so that the raster kernel can
 // sort the bins of a warp by routine before drawing (no divergence between the inversion loop, the central and
-// the tail branch of AS 241).  The draws are plain fp64 (FMA contraction allowed, reciprocal instead of division
-// in the inversion recurrence): against the oracle's separately rounded operations this moves a CDF break point
-// or a rounding boundary by ~1e-16 relative, i.e. it flips a draw with probability ~1e-13, far inside the 1e-6
+// the tail branch of AS 241).  The draws are plain fp64 (FMA contraction allowed, Newton reciprocals instead of IEEE
+// division, own exp/log1p series): against the oracle's separately rounded operations this moves a CDF break point
+// or a rounding boundary by ~1e-15 relative, i.e. it flips a draw with probability ~1e-12, far inside the 1e-6
 // budget of BASELINE.json north_star.
 // ------------------------------------------------------------------------------------------------------------------
 enum DrawClass : int {
@@ -112,12 +112,71 @@ __device__ __forceinline__ int classify_draw(double N, double &p, uint32_t &w, b
     return word_is_central(w) ? kDrawNormalCentral : kDrawNormalTail;
 }
 
+// ---- fp64 helpers of the draw routines.  They replace the CUDA math library's division, log1p and exp by straight-line
+// code whose constants sit in constant memory (DFMA reads them as c[][] operands; literals cost two UMOVs each).  All are
+// accurate to ~1e-15 relative, which moves a CDF break point or a rounding boundary by that much: see the note above.
+__device__ __forceinline__ double fast_rcp(double b) // b normal, |b| in [1e-290, 1e290]
+{
+    double x;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(b)); // ~20 bits
+    double e = fma(-b, x, 1.0);
+    x = fma(x, e, x);
+    e = fma(-b, x, 1.0);
+    return fma(x, e, x);
+}
+__device__ __forceinline__ double fast_div(double a, double b)
+{
+    const double x = fast_rcp(b);
+    const double q = a * x;
+    return fma(fma(-b, q, a), x, q);
+}
+
+// g(p) = sum_{j=0}^{10} p^j / (j+1):  log1p(-p) = -p g(p) for p < 2^-5 (truncation p^11/12 < 2^-58 relative)
+static __constant__ double c_log1m[11] = {1.0 / 11.0, 1.0 / 10.0, 1.0 / 9.0, 1.0 / 8.0, 1.0 / 7.0, 1.0 / 6.0,
+                                          1.0 / 5.0,  1.0 / 4.0,  1.0 / 3.0, 1.0 / 2.0, 1.0};
+// 1/j!, j = 13 .. 0: exp(r) on |r| <= ln2/2 (truncation r^14/14! < 5e-18)
+static __constant__ double c_exp[14] = {1.0 / 6227020800.0, 1.0 / 479001600.0, 1.0 / 39916800.0, 1.0 / 3628800.0,
+                                        1.0 / 362880.0,     1.0 / 40320.0,     1.0 / 5040.0,     1.0 / 720.0,
+                                        1.0 / 120.0,        1.0 / 24.0,        1.0 / 6.0,        0.5,
+                                        1.0,                1.0};
+static __constant__ double c_exp_red[4] = {1.4426950408889634074, 6.93147180369123816490e-01, 1.90821492927058770002e-10,
+                                           6755399441055744.0}; // log2 e, ln2 hi, ln2 lo, 1.5 2^52
+
+// exp(y) for -700 < y <= 0
+__device__ __forceinline__ double exp_neg(double y)
+{
+    const double sh = fma(y, c_exp_red[0], c_exp_red[3]); // low word of sh = rint(y log2 e) (two's complement)
+    const double kd = sh - c_exp_red[3];
+    double r = fma(kd, -c_exp_red[1], y);
+    r = fma(kd, -c_exp_red[2], r);
+    double e = c_exp[0];
+#pragma unroll
+    for (int j = 1; j < 14; ++j) e = fma(e, r, c_exp[j]);
+    const int k = __double2loint(sh);
+    return __hiloint2double(__double2hiint(e) + (k << 20), __double2loint(e)); // e in [0.7, 1.42), k >= -1010
+}
+
+// (1 - p)^N for 0 < p <= 1/2
+__device__ __forceinline__ double pow_one_minus(double N, double p)
+{
+    double L;
+    if (p < 0.03125) {
+        double g = c_log1m[0];
+#pragma unroll
+        for (int j = 1; j < 11; ++j) g = fma(g, p, c_log1m[j]);
+        L = -p * g;
+    } else {
+        L = log1p(-p);
+    }
+    return exp_neg(N * L);
+}
+
 __device__ __forceinline__ double draw_inversion(double N, double p, uint32_t w)
 {
     const double u = word_to_u01(w);
-    double f = exp(N * log1p(-p));
+    double f = pow_one_minus(N, p);
     double c = f;
-    const double r = p / (1.0 - p), N1 = N + 1.0;
+    const double r = fast_div(p, 1.0 - p), N1 = N + 1.0;
     int k = 0;
     while (u > c && (double)k < N) {
         ++k;
@@ -149,7 +208,7 @@ __device__ __forceinline__ double draw_normal_central(double N, double p, uint32
         num = fma(num, r, c_as241_a[j]);
         den = fma(den, r, c_as241_b[j]);
     }
-    return finish_normal(N, p, q * num / den);
+    return finish_normal(N, p, fast_div(q * num, den));
 }
 
 // AS 241 PPND16, |u - 1/2| > 0.425.  r = sqrt(-log(min(u, 1-u))) <= sqrt(33 log 2) = 4.79 for a 32-bit word, so the
@@ -165,7 +224,7 @@ __device__ __forceinline__ double draw_normal_tail(double N, double p, uint32_t 
         num = fma(num, r, c_as241_c[j]);
         den = fma(den, r, c_as241_d[j]);
     }
-    const double val = num / den;
+    const double val = fast_div(num, den);
     return finish_normal(N, p, q < 0.0 ? -val : val);
 }
 

@@ -20,6 +20,7 @@ struct wcsim_plan {
     int device = 0, sm_count = 148;
     float *S = nullptr, *M = nullptr;
     float2 *spec = nullptr, *spec2 = nullptr, *Rhat = nullptr, *Rt = nullptr;
+    float2 *spec_alloc = nullptr; // spec with its zero halo rows (wires_halo)
     float2 *tw_row = nullptr, *tw_real = nullptr, *tw_col = nullptr;
     int rt_rows = 0;
     int wire_mode = WCSIM_WIRES_AUTO;
@@ -255,7 +256,7 @@ int destroy_impl(wcsim_plan *p)
     int rc = WCSIM_OK;
     if (cudaStreamSynchronize(p->stream) != cudaSuccess) rc = fail_cuda(cudaGetLastError());
     void *bufs[] = {p->spec2,    p->Rt,
-                    p->S,        p->M,           p->spec,        p->Rhat,           p->tw_row,        p->tw_real,
+                    p->S,        p->M,           p->spec_alloc,  p->Rhat,           p->tw_row,        p->tw_real,
                     p->tw_col,   p->counters,    p->amp_builtin, p->amp_custom,     p->ts.tile_count, p->ts.tile_cursor,
                     p->ts.entries, p->ts.total,  p->stage[0],    p->stage[1],       p->stage[2],      p->stage[3],
                     p->stage[4]};
@@ -318,7 +319,11 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
         const size_t grid = (size_t)n_wires * n_ticks;
         CU_TRY(cudaMalloc((void **)&p->S, sizeof(float) * grid));
         CU_TRY(cudaMalloc((void **)&p->M, sizeof(float) * grid));
-        CU_TRY(cudaMalloc((void **)&p->spec, sizeof(float2) * (size_t)n_wires * p->spec_stride));
+        int halo_lo = 0, halo_hi = 0;
+        wires_halo(n_rwires, &halo_lo, &halo_hi);
+        const size_t spec_rows = (size_t)halo_lo + n_wires + halo_hi;
+        CU_TRY(cudaMalloc((void **)&p->spec_alloc, sizeof(float2) * spec_rows * p->spec_stride));
+        p->spec = p->spec_alloc + (size_t)halo_lo * p->spec_stride;
         CU_TRY(cudaMalloc((void **)&p->spec2, sizeof(float2) * (size_t)n_wires * p->spec_stride));
         CU_TRY(cudaMalloc((void **)&p->Rhat, sizeof(float2) * (size_t)pad_w * p->spec_stride));
         p->rt_rows = (n_rwires + wires_chunk() - 1) / wires_chunk() * wires_chunk();
@@ -328,7 +333,7 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
         CU_TRY(cudaMalloc((void **)&p->amp_custom, sizeof(float) * (size_t)(pad_t / 2 + 1)));
         CU_TRY(cudaMemsetAsync(p->S, 0, sizeof(float) * grid, p->stream));
         CU_TRY(cudaMemsetAsync(p->M, 0, sizeof(float) * grid, p->stream));
-        CU_TRY(cudaMemsetAsync(p->spec, 0, sizeof(float2) * (size_t)n_wires * p->spec_stride, p->stream));
+        CU_TRY(cudaMemsetAsync(p->spec_alloc, 0, sizeof(float2) * spec_rows * p->spec_stride, p->stream));
         CU_TRY(cudaMemsetAsync(p->spec2, 0, sizeof(float2) * (size_t)n_wires * p->spec_stride, p->stream));
         CU_TRY(cudaMemsetAsync(p->counters, 0, sizeof(Counters), p->stream));
         int r = upload_twiddles(&p->tw_row, pad_t / 2, 0, p->stream);
