@@ -198,12 +198,13 @@ struct BatchSmem<true> {
     DrawQueues queues[kBatchWarps];
 };
 
-// largest d in [0, 32) with off[d] <= x (off is an exclusive prefix, off[32] > x)
+// largest d in [0, kBatchDepos) with off[d] <= x (off is an exclusive prefix over the depos of a batch; entries from
+// kBatchDepos on all hold the total, which is > x)
 __device__ __forceinline__ int owner_of(const int *off, int x)
 {
     int lo = 0;
 #pragma unroll
-    for (int step = 16; step > 0; step >>= 1)
+    for (int step = kBatchDepos / 2; step > 0; step >>= 1)
         if (off[lo + step] <= x) lo += step;
     return lo;
 }
@@ -351,7 +352,9 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
                 const int l = bbase + b - sc.boff[own];
                 const int nto = __shfl_sync(0xffffffffu, nt, own);
                 const int lo_t = __shfl_sync(0xffffffffu, et.lo, own), lo_x = __shfl_sync(0xffffffffu, ex.lo, own);
-                const int j = act ? (int)((unsigned)l / (unsigned)max(nto, 1)) : 0; // wire index in the patch
+                // wire index in the patch, l / nto: (l + 1/2) / nto is at least 1/(2 nto) away from an integer, far more
+                // than the rounding of the product below for l < 2^22 (a flat-path patch has < 2^14 bins)
+                const int j = act ? __float2int_rz(((float)l + 0.5f) * __frcp_rn((float)max(nto, 1))) : 0;
                 const int ii = act ? l - j * nto : 0;                              // tick index in the patch
                 const T *E = sc.edge + (sc.eoff[own] - ebase);
                 const T wt = T(0.5) * (E[ii + 1] - E[ii]);

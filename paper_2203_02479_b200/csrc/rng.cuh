@@ -176,16 +176,21 @@ __device__ __forceinline__ double draw_inversion(double N, double p, uint32_t w)
     const double u = word_to_u01(w);
     double f = pow_one_minus(N, p);
     double c = f;
-    const double r = fast_div(p, 1.0 - p), N1 = N + 1.0;
-    int k = 0;
-    while (u > c && (double)k < N) {
-        ++k;
-        const double kd = (double)k;
-        const double rk = k < kInvTable ? c_inv_k[k] : 1.0 / kd;
-        f *= (r * (N1 - kd)) * rk;
-        c += f;
+    // f_k = f_{k-1} r (N - k + 1) / k with r = p / (1 - p), written as f_{k-1} (r (N+1) / k - r).  The trip count is kept
+    // uniform over the warp (lanes that are done stop updating), so 1/k is a uniform constant-bank operand.
+    const double r = fast_div(p, 1.0 - p), rN1 = r * (N + 1.0);
+    double kd = 0.0;
+    bool go = u > c && kd < N;
+    for (int k = 1; __any_sync(__activemask(), go); ++k) {
+        const double rk = k < kInvTable ? c_inv_k[k] : 1.0 / (double)k;
+        if (go) {
+            kd += 1.0;
+            f *= fma(rN1, rk, -r);
+            c += f;
+            go = u > c && kd < N;
+        }
     }
-    return (double)k;
+    return kd;
 }
 
 __device__ __forceinline__ double finish_normal(double N, double p, double z)
