@@ -170,6 +170,7 @@ def run_ours(args):
         step()
     torch.cuda.synchronize()
     plan.stage_times(reset=True)
+    plan.reset_stats()
     launches0 = plan.launch_count()
     sampler = ClockSampler(local_rank if "CUDA_VISIBLE_DEVICES" not in os.environ else
                            int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank]))
@@ -183,6 +184,7 @@ def run_ours(args):
 
     # the same loop without the per-stage event pairs (they sit between the kernels): reported for information
     per_step_plain = timed(step, args.steps)
+    stats = plan.stats()
 
     # ---- end to end through the C ABI with host buffers -------------------------------------------------------------
     host = {k: torch.from_numpy(v).pin_memory() for k, v in pl["depos"].items()}
@@ -225,13 +227,35 @@ def run_ours(args):
     conv_ms = sum(r["ms"] for r in stage_rows if r["stage"] in sb)
     conv_bytes = sum(sb.values())
     conv_gbs = conv_bytes / (conv_ms * 1e-3) / 1e9
-    dom = max((r for r in stage_rows if r["stage"] in sb), key=lambda r: r["ms"])
-    roofline = {"kernel": dom["stage"], "bound": "hbm", "achieved": dom["achieved_gbs"], "peak": peaks["hbm_gbs"],
-                "unit": "GB/s", "frac": dom["frac"], "traffic": TRAFFIC.get(dom["stage"]),
-                "peak_source": peaks["source"],
-                "convolve": {"ms": conv_ms, "bytes": conv_bytes, "achieved": conv_gbs,
-                             "frac": conv_gbs / peaks["hbm_gbs"], "frac_of_8TBs_nominal": conv_gbs / 8000.0},
-                "stages": stage_rows}
+    pass_model = survey_pass_model_bytes(pl)
+    convolve = {"ms": conv_ms, "bytes": conv_bytes, "achieved": conv_gbs, "frac": conv_gbs / peaks["hbm_gbs"],
+                "frac_of_8TBs_nominal": conv_gbs / 8000.0,
+                # SURVEY.md 8(d)'s pass model of the stage (all three passes by FFT, Rhat read in full): the bytes an
+                # FFT convolution moves; the direct wire-axis pass avoids 33 MB of them on configs[1]
+                "survey_pass_model_bytes": pass_model,
+                "frac_of_survey_pass_model": pass_model / (conv_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    dom = max(stage_rows, key=lambda r: r["ms"])
+    if dom["stage"] == "raster" and fluct:
+        # ALU bound: algorithmic fp64 work of the oracle's arithmetic, ~70 flop per drawn bin,
+        # against 148 SMs x 64 fp64 FMA lanes x 2 flop x the SM clock
+        bins = stats["bins_drawn"] / max(1, args.steps + args.steps)  # two timed loops ran since the reset
+        tflops = bins * FP64_FLOP_PER_BIN / (dom["ms"] * 1e-3) / 1e12
+        peak = 148 * 64 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+        roofline = {"kernel": "raster_batch_kernel<fluct>", "bound": "alu", "achieved": tflops, "peak": peak,
+                    "unit": "TFLOP/s", "frac": tflops / peak, "traffic": TRAFFIC.get("raster") if args.config == 1 else None,
+                    "peak_source": "derived: 148 SMs x 64 fp64 FMA/clk x 2 x %.0f MHz (DESIGN.md); DFMA microbenchmark "
+                                   "reached 56.4 of 64 per clk per SM" % peaks["sm_max_mhz"],
+                    "algorithmic": {"bins_per_launch": bins, "fp64_flop_per_bin": FP64_FLOP_PER_BIN,
+                                    "bins_per_s": bins / (dom["ms"] * 1e-3)}}
+    else:
+        if dom["stage"] not in sb:
+            dom = max((r for r in stage_rows if r["stage"] in sb), key=lambda r: r["ms"])
+        roofline = {"kernel": dom["stage"], "bound": "hbm", "achieved": dom["achieved_gbs"], "peak": peaks["hbm_gbs"],
+                    "unit": "GB/s", "frac": dom["frac"], "traffic": TRAFFIC.get(dom["stage"]) if args.config == 1 else None,
+                    "peak_source": peaks["source"]}
+    roofline["hbm_peak"] = {"gbs": peaks["hbm_gbs"], "source": peaks["source"]}
+    roofline["convolve"] = convolve
+    roofline["stages"] = stage_rows
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -261,9 +285,18 @@ def run_ours(args):
         print(json.dumps(out))
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r01_ncu_full.md); None until a capture of the current kernels exists
-TRAFFIC = {"rows_forward": None, "cols": None, "rows_inverse": None}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1], from the committed `ncu --set full` capture
+# (profiles/r01_ncu_full.md; cold-cache replays, so reads are compulsory misses and writes mostly stay in L2)
+TRAFFIC = {"raster": 6.03e6, "rows_forward": 19.29e6, "cols": 27.2e6, "rows_inverse": 26.39e6}
+# algorithmic fp64 work per drawn bin of the fluctuated raster (DESIGN.md section 6 derives it from the oracle's steps)
+FP64_FLOP_PER_BIN = 70.0
+
+
+def survey_pass_model_bytes(pl):
+    """read S, write+read the populated row spectra twice, read Rhat, write M."""
+    nw, nt, pw, pt = pl["n_wires"], pl["n_ticks"], pl["pad_w"], pl["pad_t"]
+    nk = pt // 2 + 1
+    return 2 * nw * nt * 4 + 4 * nw * nk * 8 + pw * nk * 8
 
 
 def cufft_comparator(pl, dev, flush):

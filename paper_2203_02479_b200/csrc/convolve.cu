@@ -16,6 +16,7 @@
 #include "fft.cuh"
 #include "internal.h"
 #include "rng.cuh"
+#include "tma.cuh"
 
 namespace wcsim {
 
@@ -78,6 +79,31 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
         if (k == 0) dst[N] = make_float2(zk.x - zk.y, 0.f);
     }
 }
+
+// Persistent, TMA-staged variant of the inverse row kernel (512 <= pad_t/2 <= 4096: configs[0..3]).  A CTA walks rows
+// blockIdx.x, blockIdx.x + gridDim.x, ...; one thread issues a single bulk copy (cp.async.bulk, mbarrier-tracked) of
+// the NEXT row into the staging buffer as soon as every thread has lifted the current row into registers, so the copy
+// runs under the butterflies and the rows are no longer load -> wait -> compute one after the other.
+// Shared memory per CTA: FFT exchange buffer + one staged row + the mbarrier, three CTAs per SM.
+// (The same staging was tried for the forward rows and lost 1.5 us on configs[1]: there the plain kernel already reads
+// its row straight into registers, and four 64-register CTAs per SM beat three 80-register ones.)
+template <int N>
+struct RowTma {
+    static constexpr int threads = RowCfg<N>::threads;
+    static constexpr int min_ctas = threads <= 256 ? 3 : (threads <= 512 ? 2 : 1);
+    static constexpr int work_bytes = (RowCfg<N>::smem_bytes + 127) / 128 * 128;
+    static constexpr bool enabled = N <= 4096 && N >= 512;
+    static int smem_bytes(int stage_bytes) { return work_bytes + (stage_bytes + 127) / 128 * 128 + 16; }
+    static int grid(int rows, int stage_bytes, int sm_count)
+    {
+        int per_sm = (227 * 1024) / (smem_bytes(stage_bytes) + 1024);
+        per_sm = per_sm > min_ctas ? min_ctas : per_sm;
+        const int slots = sm_count * (per_sm > 0 ? per_sm : 1);
+        // equal rows per CTA where the count allows it: ceil(rows / ceil(rows / slots))
+        const int rounds = (rows + slots - 1) / slots;
+        return (rows + rounds - 1) / rounds;
+    }
+};
 
 // ------------------------------------------------------------------------------------------------------------------
 // a4 wire axis, a5 multiply, a6 wire axis
@@ -241,11 +267,104 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
     }
 }
 
+// a6 tick axis (+ a7 noise), TMA-staged: the row spectrum lands in shared memory by one bulk copy, so the partner bin
+// X_{N-k} is read where the copy put it (no staging stores); the noise spectrum is added to the staged row in place.
+template <int N>
+__global__ void __launch_bounds__(RowTma<N>::threads, RowTma<N>::min_ctas) rows_inverse_tma_kernel(GridDims g, ConvBuffers b,
+                                                                                                   NoiseArgs nz)
+{
+    constexpr int E = RowCfg<N>::E, NT = N / E;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float2 *smem = reinterpret_cast<float2 *>(smem_raw);
+    const uint32_t row_bytes = (uint32_t)b.spec_stride * 8u; // whole stride: a multiple of 64
+    float2 *stage = reinterpret_cast<float2 *>(smem_raw + RowTma<N>::work_bytes);
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + RowTma<N>::work_bytes + (row_bytes + 127) / 128 * 128);
+    const int i = threadIdx.x;
+    const bool noisy = nz.amp != nullptr;
+    int row = blockIdx.x;
+    if (i == 0) {
+        mbar_init(bar, 1);
+        mbar_arrive_expect_tx(bar, row_bytes);
+        bulk_copy_g2s(stage, b.spec_inv + (size_t)row * b.spec_stride, row_bytes, bar);
+    }
+    __syncthreads();
+    uint32_t parity = 0;
+    for (; row < g.n_wires; row += gridDim.x) {
+        mbar_wait(bar, parity);
+        parity ^= 1u;
+        if (noisy) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const int k = i + e * NT;
+                stage[k] = cadd(stage[k], noise_bin(nz, (uint32_t)row, (uint32_t)k));
+                if (k == 0) stage[N] = cadd(stage[N], noise_bin(nz, (uint32_t)row, (uint32_t)N));
+            }
+            __syncthreads();
+        }
+        // Z_k = (X_k + conj X_{N-k}) + i exp(+2 pi i k / 2N) (X_k - conj X_{N-k});  inverse FFT of Z = even + i odd
+        float2 v[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int k = i + e * NT;
+            float2 xk = stage[k], xn = stage[N - k];
+            if (k == 0) xk.y = 0.f, xn.y = 0.f; // imaginary parts of the DC and Nyquist bins do not reach a real output
+            const float2 s = make_float2(xk.x + xn.x, xk.y - xn.y);
+            const float2 d = make_float2(xk.x - xn.x, xk.y + xn.y);
+            const float2 w = load_tw(b.tw_real, k); // (cos, -sin)
+            const float2 t = make_float2(w.x * d.x + w.y * d.y, w.x * d.y - w.y * d.x);
+            v[e] = make_float2(s.x - t.y, s.y + t.x);
+        }
+        __syncthreads(); // every thread is done with the staged row and with last row's exchange buffer
+        const int next = row + gridDim.x;
+        if (i == 0 && next < g.n_wires) {
+            fence_proxy_async(); // the generic-proxy accesses to the stage above precede the async-proxy refill
+            mbar_arrive_expect_tx(bar, row_bytes);
+            bulk_copy_g2s(stage, b.spec_inv + (size_t)next * b.spec_stride, row_bytes, bar);
+        }
+        fft_block<N, 1, E, +1>(v, smem, i, 0, b.tw_row, false);
+        float2 *dst = reinterpret_cast<float2 *>(b.M + (size_t)row * g.n_ticks);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int pt = i + e * NT;
+            if (2 * pt < g.n_ticks) dst[pt] = v[e];
+        }
+    }
+}
+
 template <typename K>
 cudaError_t set_smem(K kernel, int bytes)
 {
     if (bytes <= 48 * 1024) return cudaSuccess;
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+constexpr int kTmaSmemCap = 200 * 1024;
+template <int NN>
+cudaError_t configure_tma()
+{
+    if constexpr (RowTma<NN>::enabled) {
+        return cudaFuncSetAttribute(rows_inverse_tma_kernel<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    kTmaSmemCap);
+    }
+    return cudaSuccess;
+}
+
+// the TMA-staged kernel wants 16-byte aligned rows (bulk copies) and float2 stores into M
+template <int NN>
+bool inverse_tma_ok(GridDims g, const ConvBuffers &b)
+{
+    if constexpr (!RowTma<NN>::enabled) return false;
+    return g.n_ticks % 2 == 0 && reinterpret_cast<uintptr_t>(b.M) % 8 == 0 &&
+           reinterpret_cast<uintptr_t>(b.spec_inv) % 16 == 0 && RowTma<NN>::smem_bytes(b.spec_stride * 8) <= kTmaSmemCap;
+}
+template <int NN>
+void launch_inverse_tma(GridDims g, ConvBuffers b, NoiseArgs nz, cudaStream_t st)
+{
+    if constexpr (RowTma<NN>::enabled) {
+        const int stage = b.spec_stride * 8;
+        rows_inverse_tma_kernel<NN><<<RowTma<NN>::grid(g.n_wires, stage, b.sm_count), RowTma<NN>::threads,
+                                      RowTma<NN>::smem_bytes(stage), st>>>(g, b, nz);
+    }
 }
 
 #define WCSIM_ROW_SIZES(X) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096) X(8192) X(16384)
@@ -276,6 +395,7 @@ cudaError_t conv_configure(int pad_w, int pad_t)
         if (err == cudaSuccess) err = set_smem(rows_forward_kernel<NN, false>, RowCfg<NN>::smem_bytes);                \
         if (err == cudaSuccess) err = set_smem(rows_inverse_kernel<NN, true>, RowCfg<NN>::smem_bytes);                 \
         if (err == cudaSuccess) err = set_smem(rows_inverse_kernel<NN, false>, RowCfg<NN>::smem_bytes);                \
+        if (err == cudaSuccess) err = configure_tma<NN>();                                                             \
         break;
         WCSIM_ROW_SIZES(X)
 #undef X
@@ -370,7 +490,9 @@ cudaError_t launch_rows_inverse(GridDims g, int pad_t, ConvBuffers b, NoiseArgs 
     switch (pad_t / 2) {
 #define X(NN)                                                                                                          \
     case NN:                                                                                                           \
-        if (vec)                                                                                                       \
+        if (use_spec && !accumulate && inverse_tma_ok<NN>(g, b))                                                       \
+            launch_inverse_tma<NN>(g, b, noise, st);                                                                   \
+        else if (vec)                                                                                                  \
             rows_inverse_kernel<NN, true><<<g.n_wires, RowCfg<NN>::threads, RowCfg<NN>::smem_bytes, st>>>(             \
                 g, b, noise, use_spec, accumulate);                                                                    \
         else                                                                                                           \

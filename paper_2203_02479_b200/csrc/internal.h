@@ -62,6 +62,7 @@ struct ConvBuffers {
     const float2 *tw_real;// [pad_t/2]  exp(-2 pi i j / pad_t)
     const float2 *tw_col; // per-pass twiddle tables of a pad_w-point FFT
     int spec_stride;      // pad_t/2 + 8
+    int sm_count;         // SMs of the plan's device (grid size of the persistent row kernels)
 };
 struct NoiseArgs {
     const float *amp; // DEVICE [pad_t/2 + 1], already scaled by pad_t^-1/2; NULL = no noise

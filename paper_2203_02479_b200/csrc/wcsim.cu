@@ -166,6 +166,7 @@ ConvBuffers conv_buffers(const wcsim_plan *p)
     b.tw_real = p->tw_real;
     b.tw_col = p->tw_col;
     b.spec_stride = p->spec_stride;
+    b.sm_count = p->sm_count;
     return b;
 }
 
