@@ -9,7 +9,9 @@ binomial fluctuation on): clear S, raster + fluctuate + scatter-add, FFT-convolv
 depositions per second through that whole path (so ms_per_step is the "ms per plane-event" of BASELINE.json's
 metric), inputs resident in HBM; `e2e` is the same through wcsim_simulate_host with pinned HOST buffers, the
 host<->device copies inside the timed region.  L2 (126 MB) is flushed between timed steps by writing a 256 MB
-buffer, outside the per-step CUDA-event pairs.  Multi-GPU: replicas only, one process per GPU.
+buffer, outside the per-step CUDA-event pairs.  `roofline` is the dominant kernel's (the fluctuated raster: ALU bound),
+with the FFT-convolve stage's HBM fractions under roofline.convolve; per-kernel durations come from a second pass of
+the same K steps with CUDA-event pairs around every stage.  Multi-GPU: replicas only, one process per GPU.
 """
 from __future__ import annotations
 
@@ -164,26 +166,33 @@ def run_ours(args):
         return [a.elapsed_time(b) for a, b in ev]
 
     # ---- device-resident arm -------------------------------------------------------------------------------------
-    plan.set_profiling(True)
+    # The headline is timed with one CUDA-event pair per plane-event and nothing between the kernels.  The per-kernel
+    # durations of the roofline come from a second pass of the same K steps with the library's own event pairs around
+    # every stage (wcsim_set_profiling): those records sit between the kernels and cost ~20 us per step on
+    # configs[1], so they are kept out of the headline and reported as ms_per_step_with_stage_events.
     for _ in range(args.warmup):
         flush.fill_(1.0)
         step()
     torch.cuda.synchronize()
-    plan.stage_times(reset=True)
     plan.reset_stats()
     launches0 = plan.launch_count()
     sampler = ClockSampler(local_rank if "CUDA_VISIBLE_DEVICES" not in os.environ else
                            int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank]))
     per_step = timed(step, args.steps, sampler)
     launches = plan.launch_count() - launches0
-    stages = plan.stage_times(reset=True)
-    plan.set_profiling(False)
     local_s = sum(per_step) * 1e-3
     value, slowest_s = replicas.whole_job_throughput(n_depos * args.steps, local_s, dev)
     ms_per_step = slowest_s * 1e3 / args.steps
 
-    # the same loop without the per-stage event pairs (they sit between the kernels): reported for information
-    per_step_plain = timed(step, args.steps)
+    plan.set_profiling(True)
+    for _ in range(min(args.warmup, 3)):
+        flush.fill_(1.0)
+        step()
+    torch.cuda.synchronize()
+    plan.stage_times(reset=True)
+    per_step_staged = timed(step, args.steps)
+    stages = plan.stage_times(reset=True)
+    plan.set_profiling(False)
     stats = plan.stats()
 
     # ---- end to end through the C ABI with host buffers -------------------------------------------------------------
@@ -238,7 +247,7 @@ def run_ours(args):
     if dom["stage"] == "raster" and fluct:
         # ALU bound: algorithmic fp64 work of the oracle's arithmetic, ~70 flop per drawn bin,
         # against 148 SMs x 64 fp64 FMA lanes x 2 flop x the SM clock
-        bins = stats["bins_drawn"] / max(1, args.steps + args.steps)  # two timed loops ran since the reset
+        bins = stats["bins_drawn"] / max(1, 2 * args.steps + min(args.warmup, 3))  # plane-events since the reset
         tflops = bins * FP64_FLOP_PER_BIN / (dom["ms"] * 1e-3) / 1e12
         peak = 148 * 64 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
         roofline = {"kernel": "raster_batch_kernel<fluct>", "bound": "alu", "achieved": tflops, "peak": peak,
@@ -273,7 +282,7 @@ def run_ours(args):
         "roofline": roofline,
         "ms_per_step_median": statistics.median(per_step),
         "ms_per_step_min": min(per_step),
-        "ms_per_step_without_stage_events": sum(per_step_plain) / len(per_step_plain),
+        "ms_per_step_with_stage_events": sum(per_step_staged) / len(per_step_staged),
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(cfg, budget_s=args.cpu_budget)
