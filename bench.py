@@ -216,6 +216,12 @@ def run_ours(args):
     e2e_value, e2e_slowest = replicas.whole_job_throughput(n_depos * e2e_steps, e2e_local, dev)
     h2d, d2h = 5 * 4 * n_depos, 4 * pl["n_wires"] * pl["n_ticks"]
 
+    # ---- several independent plane-events in flight (the paper's section 3.3 runs several processes
+    # per GPU for the same reason: one event does not fill the device).  Extra figure, not the headline.
+    concurrent = None
+    if args.streams > 1 and world == 1:
+        concurrent = concurrent_planes(args, B, cfg, pl, d, fluct, mode, dev, n_depos)
+
     # ---- roofline of the dominant kernel --------------------------------------------------------------------------
     peaks = load_peaks()
     direct = args.wires == "direct" or (args.wires == "auto" and pl["response"].shape[0] <= 64)
@@ -284,6 +290,8 @@ def run_ours(args):
         "ms_per_step_min": min(per_step),
         "ms_per_step_with_stage_events": sum(per_step_staged) / len(per_step_staged),
     }
+    if concurrent:
+        out["concurrent"] = concurrent
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(cfg, budget_s=args.cpu_budget)
     if rank == 0 and world == 1 and args.cufft:
@@ -306,6 +314,41 @@ def survey_pass_model_bytes(pl):
     nw, nt, pw, pt = pl["n_wires"], pl["n_ticks"], pl["pad_w"], pl["pad_t"]
     nk = pt // 2 + 1
     return 2 * nw * nt * 4 + 4 * nw * nk * 8 + pw * nk * 8
+
+
+def concurrent_planes(args, B, cfg, pl, d, fluct, mode, dev, n_depos):
+    """K plane-events of the same workload issued round-robin to `--streams` plans, each with its own stream and
+    buffers (working set n x 90 MB > L2 for n >= 2, so no flush); one CUDA-event pair around all K."""
+    import torch
+    n = args.streams
+    streams = [torch.cuda.Stream(device=dev) for _ in range(n)]
+    plans = [B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]), nsigma=cfg["nsigma"],
+                    scatter_mode=mode, stream=st) for st in streams]
+    main = torch.cuda.current_stream()
+
+    def run(k):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record(main)
+        for st in streams:
+            st.wait_event(a)
+        for i in range(k):
+            p = plans[i % n]
+            p.clear()
+            p.raster_scatter(d, seed=cfg["fluct_seed"], fluctuate=fluct)
+            p.convolve()
+        for st in streams:
+            main.wait_stream(st)
+        b.record(main)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b)
+
+    run(max(n, min(args.warmup, 3) * n))
+    ms = run(args.steps)
+    for p in plans:
+        p.destroy()
+    return {"streams": n, "steps": args.steps, "ms_per_step": ms / args.steps, "value": n_depos * args.steps / (ms * 1e-3),
+            "unit": UNIT, "what": "independent plane-events in flight on %d streams (throughput, not latency)" % n}
 
 
 def cufft_comparator(pl, dev, flush):
@@ -400,6 +443,7 @@ def main():
     ap.add_argument("--scatter", default="atomic", choices=["atomic", "tiled"])
     ap.add_argument("--wires", default="auto", choices=["auto", "fft", "direct"], help="wire axis of the convolution")
     ap.add_argument("--no-fluct", action="store_true")
+    ap.add_argument("--streams", type=int, default=3, help="plane-events in flight for the extra `concurrent` figure")
     ap.add_argument("--e2e-steps", type=int, default=200)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
