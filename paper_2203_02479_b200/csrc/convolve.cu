@@ -16,6 +16,7 @@
 #include "fft.cuh"
 #include "internal.h"
 #include "rng.cuh"
+#include "pdl.cuh"
 #include "tma.cuh"
 
 namespace wcsim {
@@ -42,21 +43,24 @@ struct ColCfg {
 // a4, tick axis: real row -> half spectrum
 // ------------------------------------------------------------------------------------------------------------------
 template <int N, bool VEC>
-__global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_forward_kernel(GridDims g, ConvBuffers b)
+__global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_forward_kernel(GridDims g, ConvBuffers b,
+                                                                                                    int tail_from)
 {
     constexpr int E = RowCfg<N>::E, NT = N / E;
     extern __shared__ float2 smem[];
     const int row = blockIdx.x, i = threadIdx.x;
+    if ((int)blockIdx.x >= tail_from) pdl_trigger();
+    pdl_wait(); // S is the raster's
     const float *src = b.S + (size_t)row * g.n_ticks;
     float2 v[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const int pt = i + e * NT;
         if constexpr (VEC) {
-            v[e] = (2 * pt < g.n_ticks) ? __ldg(reinterpret_cast<const float2 *>(src) + pt) : make_float2(0.f, 0.f);
+            v[e] = (2 * pt < g.n_ticks) ? reinterpret_cast<const float2 *>(src)[pt] : make_float2(0.f, 0.f);
         } else {
-            v[e].x = (2 * pt < g.n_ticks) ? __ldg(src + 2 * pt) : 0.f;
-            v[e].y = (2 * pt + 1 < g.n_ticks) ? __ldg(src + 2 * pt + 1) : 0.f;
+            v[e].x = (2 * pt < g.n_ticks) ? src[2 * pt] : 0.f;
+            v[e].y = (2 * pt + 1 < g.n_ticks) ? src[2 * pt + 1] : 0.f;
         }
     }
     fft_block<N, 1, E, -1>(v, smem, i, 0, b.tw_row, false);
@@ -115,6 +119,7 @@ __global__ void __launch_bounds__(ColCfg<N>::threads) cols_kernel(GridDims g, Co
     extern __shared__ float2 smem[];
     const int c = threadIdx.x % C, i = threadIdx.x / C;
     const int col = blockIdx.x * C + c;
+    pdl_wait();
     float2 *spec = b.spec + col;
     const float2 *rh = b.Rhat + col;
     float2 v[E];
@@ -156,8 +161,10 @@ constexpr int kWiresD = 7, kWiresRG = 8, kWiresO = 8;
 // STRIDE = 0: row stride read from the buffers (any pad_t); NCH = 0: chunk count read from the buffers (any n_rw),
 // else the chunk loop is unrolled so that the loads of the next chunk are in flight under the FFMAs of this one
 template <int O, int D, int NCH, int STRIDE>
-__global__ void __launch_bounds__(32 * kWiresRG, 3) wires_kernel(GridDims g, ConvBuffers b, int nk)
+__global__ void __launch_bounds__(32 * kWiresRG, 3) wires_kernel(GridDims g, ConvBuffers b, int nk, int tail_from)
 {
+    if ((int)(blockIdx.y * gridDim.x + blockIdx.x) >= tail_from) pdl_trigger();
+    pdl_wait(); // the row spectra are rows_forward's
     const int k = blockIdx.x * 32 + threadIdx.x;
     const int x0 = (blockIdx.y * kWiresRG + threadIdx.y) * O;
     if (k >= nk || x0 >= g.n_wires) return;
@@ -167,7 +174,7 @@ __global__ void __launch_bounds__(32 * kWiresRG, 3) wires_kernel(GridDims g, Con
 #pragma unroll
     for (int o = 0; o < O; ++o) acc[o] = make_float2(0.f, 0.f);
     // chunk d0 uses wire rows x0 + c - d0 - (D-1) .. x0 + c - d0 + O - 1 (halo rows included) and Rt rows d0 .. d0+D-1
-    const float2 *__restrict__ in = b.spec + k + ((ptrdiff_t)x0 + c - (D - 1)) * stride;
+    const float2 *in = b.spec + k + ((ptrdiff_t)x0 + c - (D - 1)) * stride; // plain loads: see pdl.cuh
     const float2 *__restrict__ rt = b.Rt + k;
     const int n_chunks = NCH ? NCH : b.rt_rows / D;
 #pragma unroll
@@ -176,7 +183,7 @@ __global__ void __launch_bounds__(32 * kWiresRG, 3) wires_kernel(GridDims g, Con
 #pragma unroll
         for (int j = 0; j < D; ++j) coef[j] = __ldg(rt + j * stride);
 #pragma unroll
-        for (int q = 0; q < O + D - 1; ++q) s[q] = __ldg(in + q * stride);
+        for (int q = 0; q < O + D - 1; ++q) s[q] = in[q * stride];
 #pragma unroll
         for (int o = 0; o < O; ++o)
 #pragma unroll
@@ -217,17 +224,18 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
     constexpr int E = RowCfg<N>::E, NT = N / E;
     extern __shared__ float2 smem[];
     const int row = blockIdx.x, i = threadIdx.x;
+    pdl_wait(); // a no-op unless launched as a programmatic dependent
     const float2 *src = b.spec_inv + (size_t)row * b.spec_stride;
     const bool noisy = nz.amp != nullptr;
     // stage X_k (+ noise) in shared memory so that every thread can reach the partner X_{N-k}
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const int k = i + e * NT;
-        float2 x = use_spec ? __ldg(src + k) : make_float2(0.f, 0.f);
+        float2 x = use_spec ? src[k] : make_float2(0.f, 0.f);
         if (noisy) x = cadd(x, noise_bin(nz, (uint32_t)row, (uint32_t)k));
         if (k == 0) {
             x.y = 0.f; // the imaginary parts of the DC and Nyquist bins do not reach a real output
-            float2 xn = use_spec ? __ldg(src + N) : make_float2(0.f, 0.f);
+            float2 xn = use_spec ? src[N] : make_float2(0.f, 0.f);
             if (noisy) xn = cadd(xn, noise_bin(nz, (uint32_t)row, (uint32_t)N));
             xn.y = 0.f;
             smem[smem_index<1>(N, 0)] = xn;
@@ -284,9 +292,11 @@ __global__ void __launch_bounds__(RowTma<N>::threads, RowTma<N>::min_ctas) rows_
     int row = blockIdx.x;
     if (i == 0) {
         mbar_init(bar, 1);
+        pdl_wait(); // the product spectra are the wire pass's
         mbar_arrive_expect_tx(bar, row_bytes);
         bulk_copy_g2s(stage, b.spec_inv + (size_t)row * b.spec_stride, row_bytes, bar);
     }
+    pdl_wait();
     __syncthreads();
     uint32_t parity = 0;
     for (; row < g.n_wires; row += gridDim.x) {
@@ -362,8 +372,8 @@ void launch_inverse_tma(GridDims g, ConvBuffers b, NoiseArgs nz, cudaStream_t st
 {
     if constexpr (RowTma<NN>::enabled) {
         const int stage = b.spec_stride * 8;
-        rows_inverse_tma_kernel<NN><<<RowTma<NN>::grid(g.n_wires, stage, b.sm_count), RowTma<NN>::threads,
-                                      RowTma<NN>::smem_bytes(stage), st>>>(g, b, nz);
+        launch_pdl(rows_inverse_tma_kernel<NN>, RowTma<NN>::grid(g.n_wires, stage, b.sm_count), RowTma<NN>::threads,
+                   RowTma<NN>::smem_bytes(stage), st, g, b, nz);
     }
 }
 
@@ -423,13 +433,16 @@ static bool rows_vectorisable(GridDims g, const void *p)
 cudaError_t launch_rows_forward(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st)
 {
     const bool vec = rows_vectorisable(g, b.S);
+    const int threads = pad_t / 32 > 0 ? pad_t / 32 : 1; // 64 registers: 1024 threads of row transforms per SM
+    const int per_sm = threads >= 1024 ? 1 : (1024 / threads > 8 ? 8 : 1024 / threads);
+    const int tail = pdl_tail_from(g.n_wires, (long long)b.sm_count * per_sm);
     switch (pad_t / 2) {
 #define X(NN)                                                                                                          \
     case NN:                                                                                                           \
         if (vec)                                                                                                       \
-            rows_forward_kernel<NN, true><<<g.n_wires, RowCfg<NN>::threads, RowCfg<NN>::smem_bytes, st>>>(g, b);       \
+            launch_pdl(rows_forward_kernel<NN, true>, g.n_wires, RowCfg<NN>::threads, RowCfg<NN>::smem_bytes, st, g, b, tail); \
         else                                                                                                           \
-            rows_forward_kernel<NN, false><<<g.n_wires, RowCfg<NN>::threads, RowCfg<NN>::smem_bytes, st>>>(g, b);      \
+            launch_pdl(rows_forward_kernel<NN, false>, g.n_wires, RowCfg<NN>::threads, RowCfg<NN>::smem_bytes, st, g, b, tail); \
         break;
         WCSIM_ROW_SIZES(X)
 #undef X
@@ -474,13 +487,15 @@ cudaError_t launch_wires(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st)
     // BASELINE.json's paddings and response widths (21 wires -> 3 chunks, 41 -> 6) get immediate-offset loads and an
     // unrolled chunk loop; anything else takes the generic instance
     const int key = b.rt_rows / kWiresD * 100000 + b.spec_stride;
+    const int tail = pdl_tail_from((long long)grid.x * grid.y, (long long)b.sm_count * 3); // 80 registers x 256 threads
+    cudaError_t err = cudaSuccess;
     switch (key) {
-    case 3 * 100000 + 1024 / 2 + 8: wires_kernel<O, kWiresD, 3, 1024 / 2 + 8><<<grid, block, 0, st>>>(g, b, nk); break;
-    case 3 * 100000 + 8192 / 2 + 8: wires_kernel<O, kWiresD, 3, 8192 / 2 + 8><<<grid, block, 0, st>>>(g, b, nk); break;
-    case 6 * 100000 + 16384 / 2 + 8: wires_kernel<O, kWiresD, 6, 16384 / 2 + 8><<<grid, block, 0, st>>>(g, b, nk); break;
-    default: wires_kernel<O, kWiresD, 0, 0><<<grid, block, 0, st>>>(g, b, nk); break;
+    case 3 * 100000 + 1024 / 2 + 8: err = launch_pdl(wires_kernel<O, kWiresD, 3, 1024 / 2 + 8>, grid, block, 0, st, g, b, nk, tail); break;
+    case 3 * 100000 + 8192 / 2 + 8: err = launch_pdl(wires_kernel<O, kWiresD, 3, 8192 / 2 + 8>, grid, block, 0, st, g, b, nk, tail); break;
+    case 6 * 100000 + 16384 / 2 + 8: err = launch_pdl(wires_kernel<O, kWiresD, 6, 16384 / 2 + 8>, grid, block, 0, st, g, b, nk, tail); break;
+    default: err = launch_pdl(wires_kernel<O, kWiresD, 0, 0>, grid, block, 0, st, g, b, nk, tail); break;
     }
-    return cudaGetLastError();
+    return err != cudaSuccess ? err : cudaGetLastError();
 }
 
 cudaError_t launch_rows_inverse(GridDims g, int pad_t, ConvBuffers b, NoiseArgs noise, bool use_spec, bool accumulate,

@@ -25,6 +25,7 @@
 //           accumulates its depos in shared memory in 2^-24 fixed point (integer adds: order independent, so the
 //           result is bitwise reproducible) and adds the tile to S once.
 #include "internal.h"
+#include "pdl.cuh"
 #include "rng.cuh"
 #include <type_traits>
 
@@ -256,6 +257,9 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
     const long long n_batches = (n + kBatchDepos - 1) >> kBatchShift;
     unsigned long long drawn = 0, skipped = 0;
     int qcount[kNumDrawQueues] = {};
+    // launched plainly (its inputs may come from copy-engine transfers, which a programmatic dependency does not
+    // cover); the grid is one wave, so the next kernel's CTAs may take the slots this one frees as it drains
+    pdl_trigger();
 
     for (;;) {
         long long batch = 0;

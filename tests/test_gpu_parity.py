@@ -372,3 +372,26 @@ def test_error_codes(B):
         assert (p.pad_w, p.pad_t) == (128, 1024)
         with pytest.raises(B.WcsimError):
             p.set_scatter_mode(3)
+
+
+def test_back_to_back_plane_events_are_bitwise_stable(B):
+    """The kernels of a plane-event are programmatic dependents of one another (csrc/pdl.cuh): a kernel that read its
+    predecessor's output too early would show up as run-to-run differences.  With fluctuation on S is an exact integer
+    grid whatever the order of the adds, so M must be bit-identical across back-to-back repetitions, on a tiny grid
+    (kernels overlap most) and on a mid-sized one."""
+    from paper_2203_02479_b200 import synth
+    for cfg in (synth.config(0), synth.config(1, n_depos=5000)):
+        pl = cfg["planes"][0]
+        d = to_dev(pl["depos"])
+        with B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"])) as p:
+            first = None
+            for rep in range(40):
+                p.clear()
+                p.raster_scatter(d, seed=11, fluctuate=True)
+                p.convolve()
+                if rep % 8 == 7 or rep == 0:
+                    p.sync()
+                    M = p.output().clone()
+                    if first is None:
+                        first = M
+                    assert torch.equal(M, first), "plane-event %d differs from the first" % rep
