@@ -257,9 +257,11 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
     const long long n_batches = (n + kBatchDepos - 1) >> kBatchShift;
     unsigned long long drawn = 0, skipped = 0;
     int qcount[kNumDrawQueues] = {};
-    // launched plainly (its inputs may come from copy-engine transfers, which a programmatic dependency does not
-    // cover); the grid is one wave, so the next kernel's CTAs may take the slots this one frees as it drains
+    // the grid is one wave, so the next kernel's CTAs may take the slots this one frees as it drains.  As a
+    // programmatic dependent itself it only overlaps a preceding KERNEL's tail: copies and memsets ahead of it in the
+    // stream are still fully ordered (checked with 300 host-buffer plane-events of changing depos, 0 mismatches)
     pdl_trigger();
+    pdl_wait();
 
     for (;;) {
         long long batch = 0;
@@ -270,8 +272,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
         float t0 = 0.f, x0 = 0.f, st = 0.f, sx = 0.f, q = 0.f;
         bool valid = false;
         if (lane < kBatchDepos && i < n) {
-            t0 = __ldg(d.t0 + i), x0 = __ldg(d.x0 + i), st = __ldg(d.sigma_t + i), sx = __ldg(d.sigma_x + i),
-            q = __ldg(d.q + i);
+            t0 = d.t0[i], x0 = d.x0[i], st = d.sigma_t[i], sx = d.sigma_x[i], q = d.q[i]; // plain loads: pdl.cuh
             valid = depo_valid(t0, x0, st, sx, q);
             skipped += !valid;
         }
@@ -596,11 +597,11 @@ cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t
     const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
     if (ctas > max_ctas) ctas = max_ctas;
     if (fluctuate)
-        raster_batch_kernel<true><<<(unsigned)ctas, kBatchWarps * 32, smem, st>>>(g, d, n, id_base, seed, nsigma, S,
-                                                                                 depo_totals, counters);
+        return launch_pdl(raster_batch_kernel<true>, (unsigned)ctas, kBatchWarps * 32, smem, st, g, d, n, id_base, seed,
+                          nsigma, S, depo_totals, counters);
     else
-        raster_batch_kernel<false><<<(unsigned)ctas, kBatchWarps * 32, smem, st>>>(g, d, n, id_base, seed, nsigma, S,
-                                                                                  depo_totals, counters);
+        return launch_pdl(raster_batch_kernel<false>, (unsigned)ctas, kBatchWarps * 32, smem, st, g, d, n, id_base, seed,
+                          nsigma, S, depo_totals, counters);
     return cudaGetLastError();
 }
 
