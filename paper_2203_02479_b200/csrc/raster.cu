@@ -173,6 +173,7 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v)
 constexpr int kBatchWarps = 4;          // warps per CTA
 constexpr int kBatchShift = 3;          // log2 of the depos a warp fetches at a time (lanes beyond that own no depo):
 constexpr int kBatchDepos = 1 << kBatchShift; // small batches keep the per-warp serial path short and the load balanced
+constexpr int kTailDepos = 2, kTailPerWarp = 4; // guided scheduling of the last batches (raster_batch_kernel)
 constexpr int kEdgeCap = 128;           // edge values per warp scratch (8 patches of 16 x 5 bins need 184)
 constexpr int kQueueCap = 64;           // entries per draw queue (at most 31 left over + 32 pushed)
 
@@ -254,7 +255,14 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     BatchScratch<FLUCT> &sc = sm.scratch[wid];
     const GlobalSink sink{S, g.n_ticks};
-    const long long n_batches = (n + kBatchDepos - 1) >> kBatchShift;
+    // guided batches: kBatchDepos depos at a time, then kTailDepos at a time for the last kTailPerWarp depos per warp of the
+    // grid, so that the warps run out of work within a short batch of one another (a batch of 8 lasts ~20 us on
+    // configs[1], where a warp gets only 3-4 of them)
+    const long long n_warps_grid = (long long)gridDim.x * kBatchWarps;
+    const long long tail_depos = n_warps_grid * kTailPerWarp < n ? n_warps_grid * kTailPerWarp : n;
+    const long long big_batches = (n - tail_depos) >> kBatchShift;
+    const long long big_depos = big_batches << kBatchShift;
+    const long long n_batches = big_batches + (n - big_depos + kTailDepos - 1) / kTailDepos;
     unsigned long long drawn = 0, skipped = 0;
     int qcount[kNumDrawQueues] = {};
     // the grid is one wave, so the next kernel's CTAs may take the slots this one frees as it drains.  As a
@@ -268,10 +276,12 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
         if (lane == 0) batch = (long long)atomicAdd(&counters->next_batch, 1ull);
         batch = __shfl_sync(0xffffffffu, batch, 0);
         if (batch >= n_batches) break;
-        const long long i = (batch << kBatchShift) + lane;
+        const long long first = batch < big_batches ? batch << kBatchShift : big_depos + (batch - big_batches) * kTailDepos;
+        const int count = batch < big_batches ? kBatchDepos : kTailDepos;
+        const long long i = first + lane;
         float t0 = 0.f, x0 = 0.f, st = 0.f, sx = 0.f, q = 0.f;
         bool valid = false;
-        if (lane < kBatchDepos && i < n) {
+        if (lane < count && i < n) {
             t0 = d.t0[i], x0 = d.x0[i], st = d.sigma_t[i], sx = d.sigma_x[i], q = d.q[i]; // plain loads: pdl.cuh
             valid = depo_valid(t0, x0, st, sx, q);
             skipped += !valid;
@@ -306,11 +316,11 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
             int tot = 0;
             drawn += raster_depo<FLUCT>(__shfl_sync(0xffffffffu, t0, src), __shfl_sync(0xffffffffu, x0, src),
                                         __shfl_sync(0xffffffffu, st, src), __shfl_sync(0xffffffffu, sx, src),
-                                        __shfl_sync(0xffffffffu, q, src), id_base + (uint64_t)((batch << kBatchShift) + src), seed,
+                                        __shfl_sync(0xffffffffu, q, src), id_base + (uint64_t)(first + src), seed,
                                         nsigma, g.n_ticks, 0, g.n_wires, 0, g.n_ticks, sink, lane, &tot);
             if (totals != nullptr) {
                 tot = warp_sum(tot);
-                if (lane == 0 && tot != 0) atomicAdd(totals + (batch << kBatchShift) + src, tot);
+                if (lane == 0 && tot != 0) atomicAdd(totals + first + src, tot);
             }
         }
 
@@ -370,16 +380,16 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
                     const float qq = __shfl_sync(0xffffffffu, q, own);
                     double p = __dmul_rn(wt, wx);
                     const uint64_t gbin = (uint64_t)wire * (uint64_t)g.n_ticks + (uint64_t)tick;
-                    const uint64_t id = id_base + (uint64_t)((batch << kBatchShift) + own);
+                    const uint64_t id = id_base + (uint64_t)(first + own);
                     uint32_t w = pick_word(fluct_words(seed, id, gbin >> 2), (uint32_t)gbin & 3u);
                     bool mirror = false;
                     int cls = act ? classify_draw(Nn, p, w, mirror) : (int)kDrawZero;
                     const uint32_t fl = (mirror ? 1u : 0u) | (qq < 0.0f ? 2u : 0u) |
-                                        ((uint32_t)((batch << kBatchShift) + own) << 8);
+                                        ((uint32_t)(first + own) << 8);
                     if (cls == kDrawAll) { // p >= 1: every electron lands here
                         const float v = (fl & 2u) ? -(float)Nn : (float)Nn;
                         atomicAdd(S + gbin, v);
-                        if (totals != nullptr) atomicAdd(totals + (batch << kBatchShift) + own, (int)v);
+                        if (totals != nullptr) atomicAdd(totals + first + own, (int)v);
                     }
                     DrawQueues &Q = sm.queues[wid];
                     // one slot per bin in the queue of its class: position = queue fill + rank among the lanes of the
