@@ -170,6 +170,10 @@ int wcsim_simulate_host(wcsim_plan *plan, const float *host_t0, const float *hos
 int wcsim_debug_philox(const unsigned int *dev_ctr, const unsigned int *dev_key, unsigned int *dev_out, long long n,
                        void *cuda_stream);
 /* dev_k[i] = B(dev_N[i], dev_p[i]; dev_w[i]) -- the device binomial sampler (fp64 in, fp64 integer-valued out) */
+/* The raster's own fp64 erf (a 48-interval degree-12 Taylor table, csrc/erf_table.cuh) evaluated on the HOST with the
+ * same code the kernels run: out[i] = erf(z[i]).  HOST pointers, n elements each; no device is touched.  Used by the
+ * CPU tests to pin the table against a library erf (bin weights of reading A2). */
+int wcsim_debug_erf(const double *host_z, double *host_out, long long n);
 int wcsim_debug_binomial(const double *dev_N, const double *dev_p, const unsigned int *dev_w, double *dev_k,
                          long long n, void *cuda_stream);
 /* copy the response spectrum Rhat[kx][kt] (kx < pad_wires, kt <= pad_ticks/2) to HOST as interleaved re,im floats */

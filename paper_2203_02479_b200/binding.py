@@ -23,7 +23,7 @@ SYMBOLS = [
     "wcsim_plan_destroy", "wcsim_clear", "wcsim_clear_output", "wcsim_sync", "wcsim_set_scatter_mode", "wcsim_set_wire_mode",
     "wcsim_charge_ptr", "wcsim_output_ptr", "wcsim_get_dims", "wcsim_get_stats", "wcsim_reset_stats",
     "wcsim_simulate_host", "wcsim_set_profiling", "wcsim_get_stage_times", "wcsim_get_launch_count",
-    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum",
+    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf",
     "wcsim_strerror", "wcsim_last_cuda_error", "wcsim_version",
 ]
 
@@ -82,6 +82,7 @@ def lib():
         L.wcsim_debug_philox.argtypes = [vp, vp, vp, ll, vp]
         L.wcsim_debug_binomial.argtypes = [vp, vp, vp, vp, ll, vp]
         L.wcsim_debug_response_spectrum.argtypes = [vp, vp]
+        L.wcsim_debug_erf.argtypes = [vp, vp, ll]
         L.wcsim_strerror.argtypes = [i]
         L.wcsim_strerror.restype = C.c_char_p
         L.wcsim_last_cuda_error.argtypes = []
@@ -284,6 +285,16 @@ def wcsim_debug_philox(dev_ctr, dev_key, dev_out, n, stream=None):
 def wcsim_debug_binomial(dev_N, dev_p, dev_w, dev_k, n, stream=None):
     _check(lib().wcsim_debug_binomial(_dev_ptr(dev_N), _dev_ptr(dev_p), _dev_ptr(dev_w), _dev_ptr(dev_k), int(n),
                                       _stream_ptr(stream)), "wcsim_debug_binomial")
+
+
+def wcsim_debug_erf(z):
+    """The raster's table erf evaluated on the host (no device needed)."""
+    import numpy as np
+    z = np.ascontiguousarray(z, dtype=np.float64)
+    out = np.empty_like(z)
+    _check(lib().wcsim_debug_erf(z.ctypes.data_as(C.c_void_p), out.ctypes.data_as(C.c_void_p), int(z.size)),
+           "wcsim_debug_erf")
+    return out
 
 
 def wcsim_debug_response_spectrum(plan):

@@ -22,7 +22,8 @@ struct Counters {
 };
 
 // ---- raster.cu ----
-cudaError_t raster_configure(); // shared-memory attributes of the raster kernels (once per plan)
+cudaError_t raster_configure(cudaStream_t st); // erf table and shared-memory attributes of the raster kernels (per plan)
+void erf_table_host(const double *z, double *out, long long n); // the table erf of erf_table.cuh, evaluated on the host
 // a1-a3, atomic mode: S[wire][tick] += patch of every depo (red.global.add.f32)
 cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
                                  double nsigma, float *S, int *depo_totals, Counters *counters, int sm_count,

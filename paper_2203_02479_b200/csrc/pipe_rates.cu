@@ -25,6 +25,16 @@ __global__ void __launch_bounds__(256) k(float *out, float a, float b, double da
         u[c] = threadIdx.x + c;
     }
     const float2 a2 = make_float2(a, a * 0.5f), b2 = make_float2(b, b * 0.5f);
+    // per-thread register operands (read from memory so they are not constant-bank or uniform operands)
+    float y[CHAINS], z[CHAINS];
+    float2 y2[CHAINS], z2[CHAINS];
+#pragma unroll
+    for (int c = 0; c < CHAINS; ++c) {
+        y[c] = out[(threadIdx.x + c) & 3] + 1.0f;
+        z[c] = out[(threadIdx.x + 2 * c) & 3] + 0.5f;
+        y2[c] = make_float2(y[c], z[c]);
+        z2[c] = make_float2(z[c], y[c]);
+    }
     for (int it = 0; it < ITERS; ++it) {
 #pragma unroll
         for (int c = 0; c < CHAINS; ++c) {
@@ -49,6 +59,11 @@ __global__ void __launch_bounds__(256) k(float *out, float a, float b, double da
                 x[c] = x[c] + a;
             }
             if (KIND == 11) d[c] = d[c] * da;
+            if (KIND == 12) x[c] = fmaf(y[c], z[c], x[c]);
+            if (KIND == 13) x[c] = x[c] + y[c];
+            if (KIND == 14) x2[c] = __ffma2_rn(y2[c], z2[c], x2[c]);
+            if (KIND == 15) x[c] = x[c] * y[c];
+            if (KIND == 16) x2[c] = __fadd2_rn(x2[c], y2[c]);
         }
     }
     float s = 0;
@@ -74,7 +89,8 @@ template <int KIND>
 void run(const char *name, double ops_per_inner)
 {
     float *out;
-    cudaMalloc(&out, 4);
+    cudaMalloc(&out, 16);
+    cudaMemset(out, 0, 16);
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
@@ -97,7 +113,12 @@ void run(const char *name, double ops_per_inner)
 int main()
 {
     run<0>("FFMA 3-reg", 1);
+    run<12>("FFMA 3 distinct regs", 1);
     run<1>("FFMA2", 1);
+    run<14>("FFMA2 3 distinct regs", 1);
+    run<13>("FADD reg+reg", 1);
+    run<15>("FMUL reg*reg", 1);
+    run<16>("FADD2 reg+reg", 1);
     run<2>("FADD", 1);
     run<3>("FADD2", 1);
     run<4>("FMUL2", 1);

@@ -25,6 +25,7 @@
 //           accumulates its depos in shared memory in 2^-24 fixed point (integer adds: order independent, so the
 //           result is bitwise reproducible) and adds the tile to S once.
 #include "internal.h"
+#include "erf_table.cuh"
 #include "pdl.cuh"
 #include "rng.cuh"
 #include <type_traits>
@@ -32,6 +33,8 @@
 namespace wcsim {
 
 namespace {
+
+__device__ double g_erf_tab[(kErfDegree + 1) * kErfIntervals]; // erf_table.cuh; filled by raster_configure()
 
 constexpr int kChunk = 31;             // bins per warp pass on one axis (32 edges)
 constexpr int kTileW = 16, kTileT = 256;
@@ -77,7 +80,7 @@ __device__ __forceinline__ T axis_weights(int base, double centre, double sigma,
         const double d = __dsub_rn((double)(base + lane), centre);
         if constexpr (sizeof(T) == 8) {
             const double s = __dmul_rn(1.4142135623730951, sigma);
-            E = erf(__ddiv_rn(d, s));
+            E = erf_from_table(g_erf_tab, __ddiv_rn(d, s));
         } else {
             const float inv = 1.0f / (1.41421356f * (float)sigma);
             E = erff((float)d * inv);
@@ -350,7 +353,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
                 } else {
                     const double dd = __dsub_rn((double)coord, centre);
                     if constexpr (FLUCT) {
-                        E = erf(fast_div(dd, 1.4142135623730951 * sigma));
+                        E = erf_from_table(g_erf_tab, fast_div(dd, 1.4142135623730951 * sigma));
                     } else {
                         const float inv = 1.0f / (1.41421356f * (float)sigma);
                         E = erff((float)dd * inv);
@@ -585,9 +588,26 @@ __global__ void count_invalid_kernel(DepoArrays d, long long n, Counters *counte
 
 } // namespace
 
-cudaError_t raster_configure()
+void erf_table_host(const double *z, double *out, long long n)
 {
-    cudaError_t err = cudaFuncSetAttribute(raster_batch_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    static double tab[(kErfDegree + 1) * kErfIntervals];
+    static bool built = false;
+    if (!built) {
+        build_erf_table(tab);
+        built = true;
+    }
+    for (long long i = 0; i < n; ++i) out[i] = erf_from_table(tab, z[i]);
+}
+
+cudaError_t raster_configure(cudaStream_t st)
+{
+    double tab[(kErfDegree + 1) * kErfIntervals];
+    build_erf_table(tab);
+    cudaError_t err = cudaMemcpyToSymbolAsync(g_erf_tab, tab, sizeof(tab), 0, cudaMemcpyHostToDevice, st);
+    if (err != cudaSuccess) return err;
+    err = cudaStreamSynchronize(st); // `tab` is on this stack
+    if (err != cudaSuccess) return err;
+    err = cudaFuncSetAttribute(raster_batch_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            (int)sizeof(BatchSmem<true>));
     if (err != cudaSuccess) return err;
     return cudaFuncSetAttribute(raster_batch_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,

@@ -363,7 +363,7 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
                                        p->stream));
         CU_TRY(build_response_rows(dev_tmp, n_rwires, p->rt_rows, pad_t, p->spec_stride, p->Rt, p->stream));
         CU_TRY(conv_configure(pad_w, pad_t));
-        CU_TRY(raster_configure());
+        CU_TRY(raster_configure(p->stream));
         CU_TRY(cudaStreamSynchronize(p->stream));
         return WCSIM_OK;
     }();
@@ -394,13 +394,17 @@ int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n
         plan->launches += 5;
         return raster_tiled(plan, g, d, n, depo_id_base, seed, fluctuate != 0, dev_depo_totals);
     }
-    plan->launches += 1;
-    if (dev_depo_totals) {
-        if (n > (1ll << 24)) return WCSIM_EINVAL; // per-depo totals are indexed with 24 bits in the draw queues
-        CU_TRY(cudaMemsetAsync(dev_depo_totals, 0, sizeof(int) * (size_t)n, plan->stream));
+    if (dev_depo_totals) CU_TRY(cudaMemsetAsync(dev_depo_totals, 0, sizeof(int) * (size_t)n, plan->stream));
+    // the draw queues index per-depo totals with 24 bits: with totals requested, launch 2^24 depos at a time
+    const long long chunk = dev_depo_totals ? (1ll << 24) : n;
+    for (long long first = 0; first < n; first += chunk) {
+        const long long m = n - first < chunk ? n - first : chunk;
+        const DepoArrays dc{d.t0 + first, d.x0 + first, d.sigma_t + first, d.sigma_x + first, d.q + first};
+        plan->launches += 1;
+        CU_TRY(launch_raster_atomic(g, dc, m, depo_id_base + (unsigned long long)first, seed, fluctuate != 0, plan->nsigma,
+                                    plan->S, dev_depo_totals ? dev_depo_totals + first : nullptr, plan->counters,
+                                    plan->sm_count, plan->stream));
     }
-    CU_TRY(launch_raster_atomic(g, d, n, depo_id_base, seed, fluctuate != 0, plan->nsigma, plan->S, dev_depo_totals,
-                                plan->counters, plan->sm_count, plan->stream));
     return WCSIM_OK;
 }
 
@@ -600,6 +604,13 @@ int wcsim_debug_philox(const unsigned int *dev_ctr, const unsigned int *dev_key,
 {
     if (n < 0 || (n > 0 && (!dev_ctr || !dev_key || !dev_out))) return WCSIM_EINVAL;
     CU_TRY(launch_debug_philox(dev_ctr, dev_key, dev_out, n, (cudaStream_t)cuda_stream));
+    return WCSIM_OK;
+}
+
+int wcsim_debug_erf(const double *host_z, double *host_out, long long n)
+{
+    if (n < 0 || (n > 0 && (!host_z || !host_out))) return WCSIM_EINVAL;
+    erf_table_host(host_z, host_out, n);
     return WCSIM_OK;
 }
 
