@@ -164,6 +164,17 @@ int wcsim_get_launch_count(const wcsim_plan *plan, unsigned long long *out);
 int wcsim_simulate_host(wcsim_plan *plan, const float *host_t0, const float *host_x0, const float *host_sigma_t,
                         const float *host_sigma_x, const float *host_q, long long n, unsigned long long seed,
                         int fluctuate, int noise, unsigned long long noise_seed, float *host_M);
+/*
+ * The same, without the final synchronisation: everything (the host->device copies of the depos, the kernels and the
+ * device->host copy of M) is enqueued on the plan's stream and the call returns.  host_M holds this plane-event's
+ * M(t,x) (Eq. 1) once wcsim_sync(plan) has returned; the host depo arrays must stay valid and unchanged
+ * until then, and must be pinned for the copies to be asynchronous.  Two plans on two streams, used alternately,
+ * overlap one event's device->host copy with the next event's copies and kernels (what bench.py's `e2e` does).
+ * Errors: as wcsim_simulate_host; asynchronous CUDA errors surface at wcsim_sync.
+ */
+int wcsim_simulate_host_async(wcsim_plan *plan, const float *host_t0, const float *host_x0, const float *host_sigma_t,
+                        const float *host_sigma_x, const float *host_q, long long n, unsigned long long seed,
+                        int fluctuate, int noise, unsigned long long noise_seed, float *host_M);
 
 /* Test/diagnostic hooks: exact pieces of the path, exposed so that parity can be checked piecewise. */
 /* out[4] (DEVICE, 4*n uint32) = Philox4x32-10(ctr = dev_ctr[4*i..], key = dev_key[2*i..]) for i < n */

@@ -23,7 +23,7 @@ SYMBOLS = [
     "wcsim_plan_destroy", "wcsim_clear", "wcsim_clear_output", "wcsim_sync", "wcsim_set_scatter_mode", "wcsim_set_wire_mode",
     "wcsim_charge_ptr", "wcsim_output_ptr", "wcsim_get_dims", "wcsim_get_stats", "wcsim_reset_stats",
     "wcsim_simulate_host", "wcsim_set_profiling", "wcsim_get_stage_times", "wcsim_get_launch_count",
-    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf",
+    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf", "wcsim_simulate_host_async",
     "wcsim_strerror", "wcsim_last_cuda_error", "wcsim_version",
 ]
 
@@ -76,6 +76,7 @@ def lib():
         L.wcsim_get_stats.argtypes = [vp, C.POINTER(wcsim_stats)]
         L.wcsim_reset_stats.argtypes = [vp]
         L.wcsim_simulate_host.argtypes = [vp, vp, vp, vp, vp, vp, ll, ull, i, i, ull, vp]
+        L.wcsim_simulate_host_async.argtypes = [vp, vp, vp, vp, vp, vp, ll, ull, i, i, ull, vp]
         L.wcsim_set_profiling.argtypes = [vp, i]
         L.wcsim_get_stage_times.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(ull), i]
         L.wcsim_get_launch_count.argtypes = [vp, C.POINTER(ull)]
@@ -238,7 +239,8 @@ def wcsim_reset_stats(plan):
     _check(lib().wcsim_reset_stats(plan), "wcsim_reset_stats")
 
 
-def wcsim_simulate_host(plan, host_depos, host_M, n=None, seed=0, fluctuate=False, noise=False, noise_seed=0):
+def wcsim_simulate_host(plan, host_depos, host_M, n=None, seed=0, fluctuate=False, noise=False, noise_seed=0,
+                        _fn="wcsim_simulate_host"):
     """host_depos: dict of HOST float32 arrays (numpy, or torch CPU tensors -- pinned makes the copies asynchronous);
     host_M: HOST float32 [n_wires][n_ticks], written."""
     def hp(a):
@@ -251,9 +253,14 @@ def wcsim_simulate_host(plan, host_depos, host_M, n=None, seed=0, fluctuate=Fals
     if n is None:
         n = ptrs[0][1]
     pm, _ = hp(host_M)
-    st = lib().wcsim_simulate_host(plan, *[p for p, _ in ptrs], int(n), int(seed), int(bool(fluctuate)),
-                                   int(bool(noise)), int(noise_seed), pm)
-    _check(st, "wcsim_simulate_host")
+    st = getattr(lib(), _fn)(plan, *[p for p, _ in ptrs], int(n), int(seed), int(bool(fluctuate)),
+                             int(bool(noise)), int(noise_seed), pm)
+    _check(st, _fn)
+
+
+def wcsim_simulate_host_async(plan, host_depos, host_M, **kw):
+    """As wcsim_simulate_host without the final synchronisation: host_M is valid after wcsim_sync(plan)."""
+    wcsim_simulate_host(plan, host_depos, host_M, _fn="wcsim_simulate_host_async", **kw)
 
 
 STAGES = ("raster", "rows_forward", "cols", "rows_inverse", "noise")
@@ -383,6 +390,9 @@ class Plan:
 
     def simulate_host(self, host_depos, host_M, **kw):
         wcsim_simulate_host(self.handle, host_depos, host_M, **kw)
+
+    def simulate_host_async(self, host_depos, host_M, **kw):
+        wcsim_simulate_host_async(self.handle, host_depos, host_M, **kw)
 
     def response_spectrum(self):
         return wcsim_debug_response_spectrum(self.handle)

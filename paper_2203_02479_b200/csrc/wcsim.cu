@@ -569,7 +569,7 @@ int wcsim_reset_stats(wcsim_plan *plan)
     return WCSIM_OK;
 }
 
-int wcsim_simulate_host(wcsim_plan *plan, const float *host_t0, const float *host_x0, const float *host_sigma_t,
+int wcsim_simulate_host_async(wcsim_plan *plan, const float *host_t0, const float *host_x0, const float *host_sigma_t,
                         const float *host_sigma_x, const float *host_q, long long n, unsigned long long seed,
                         int fluctuate, int noise, unsigned long long noise_seed, float *host_M)
 {
@@ -595,6 +595,18 @@ int wcsim_simulate_host(wcsim_plan *plan, const float *host_t0, const float *hos
     if (rc) return rc;
     CU_TRY(cudaMemcpyAsync(host_M, plan->M, sizeof(float) * (size_t)plan->n_wires * plan->n_ticks,
                            cudaMemcpyDeviceToHost, plan->stream));
+    return WCSIM_OK;
+}
+
+int wcsim_simulate_host(wcsim_plan *plan, const float *host_t0, const float *host_x0, const float *host_sigma_t,
+                        const float *host_sigma_x, const float *host_q, long long n, unsigned long long seed,
+                        int fluctuate, int noise, unsigned long long noise_seed, float *host_M)
+{
+    const int rc = wcsim_simulate_host_async(plan, host_t0, host_x0, host_sigma_t, host_sigma_x, host_q, n, seed,
+                                             fluctuate, noise, noise_seed, host_M);
+    if (rc) return rc;
+    DeviceGuard guard(plan->device);
+    if (!guard.ok) return fail_cuda(cudaGetLastError());
     CU_TRY(cudaStreamSynchronize(plan->stream));
     return WCSIM_OK;
 }

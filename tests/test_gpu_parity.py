@@ -395,3 +395,38 @@ def test_back_to_back_plane_events_are_bitwise_stable(B):
                     if first is None:
                         first = M
                     assert torch.equal(M, first), "plane-event %d differs from the first" % rep
+
+
+def test_simulate_host_async_two_plans_alternating(B, O):
+    """wcsim_simulate_host_async on two plans/streams used alternately (bench.py's e2e loop): every plane-event's M,
+    read from its pinned host buffer after wcsim_sync, equals the synchronous call's and the oracle's."""
+    from paper_2203_02479_b200 import synth
+    cfg = synth.config(0)
+    pl = cfg["planes"][0]
+    nw, nt, R = pl["n_wires"], pl["n_ticks"], pl["response"]
+    sets, refs = [], []
+    for k in range(3):
+        d = {kk: v.copy() for kk, v in pl["depos"].items()}
+        d["q"] = (d["q"] * (1.0 + 0.25 * k)).astype(np.float32)
+        d["t0"] = (d["t0"] + 3.0 * k).astype(np.float32)
+        S_ref, _, _ = O.raster_scatter(nw, nt, d, fluctuate=False)
+        refs.append(O.convolve_direct(S_ref, R))
+        sets.append({kk: torch.from_numpy(v).pin_memory() for kk, v in d.items()})
+    streams = [torch.cuda.Stream() for _ in range(2)]
+    plans = [B.Plan(nw, nt, R, stream=st) for st in streams]
+    outs = [torch.empty((nw, nt), dtype=torch.float32).pin_memory() for _ in range(2)]
+    pending = [None, None]
+    try:
+        for i in range(12):
+            j, k = i % 2, i % 3
+            plans[j].sync()
+            if pending[j] is not None:
+                assert_close(outs[j].numpy(), refs[pending[j]], "async plane-event %d" % (i - 2))
+            plans[j].simulate_host_async(sets[k], outs[j], fluctuate=False)
+            pending[j] = k
+        for j in range(2):
+            plans[j].sync()
+            assert_close(outs[j].numpy(), refs[pending[j]], "last async plane-events")
+    finally:
+        for p in plans:
+            p.destroy()
