@@ -29,7 +29,8 @@ extern "C" {
 
 typedef enum wcsim_status {
     WCSIM_OK = 0,
-    WCSIM_EINVAL = -1, /* NULL pointer, non-positive size, even n_rwires, bad padding, nsigma <= 0, unknown mode */
+    WCSIM_EINVAL = -1, /* NULL pointer, non-positive size, even n_rwires, bad padding, nsigma <= 0, unknown mode,
+                          n_wires * n_ticks >= 2^30 */
     WCSIM_ENOMEM = -2, /* host or device allocation failed */
     WCSIM_ECUDA = -3,  /* a CUDA runtime call or kernel failed; wcsim_last_cuda_error() gives the cudaError_t */
     WCSIM_ESTATE = -4  /* call not valid in the plan's current state */

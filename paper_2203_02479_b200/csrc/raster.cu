@@ -186,21 +186,24 @@ struct BatchScratch {
     T edge[kEdgeCap];
     int eoff[33], boff[33];
 };
+// 20 bytes per queued bin (24 with per-depo totals): the bytes per warp decide how many warps an SM holds
+constexpr uint32_t kBinMirror = 1u << 30, kBinNegative = 1u << 31, kBinMask = kBinMirror - 1u; // grid < 2^30 bins
+template <bool TOT>
 struct DrawQueues {
     double p[kNumDrawQueues][kQueueCap];
     float N[kNumDrawQueues][kQueueCap]; // floor(|q| + 1/2) of a float q is always a float
     uint32_t w[kNumDrawQueues][kQueueCap];
-    uint32_t bin[kNumDrawQueues][kQueueCap];   // wire * n_ticks + tick
-    uint32_t flags[kNumDrawQueues][kQueueCap]; // bit 0 mirror, bit 1 negative charge, bits 8.. depo index in the call
+    uint32_t bin[kNumDrawQueues][kQueueCap]; // wire * n_ticks + tick | kBinMirror | kBinNegative
+    uint32_t depo[TOT ? kNumDrawQueues : 1][TOT ? kQueueCap : 1]; // depo index in the call (per-depo totals only)
 };
-template <bool FLUCT>
+template <bool FLUCT, bool TOT>
 struct BatchSmem {
     BatchScratch<FLUCT> scratch[kBatchWarps];
 };
-template <>
-struct BatchSmem<true> {
+template <bool TOT>
+struct BatchSmem<true, TOT> {
     BatchScratch<true> scratch[kBatchWarps];
-    DrawQueues queues[kBatchWarps];
+    DrawQueues<TOT> queues[kBatchWarps];
 };
 
 // largest d in [0, kBatchDepos) with off[d] <= x (off is an exclusive prefix over the depos of a batch; entries from
@@ -225,36 +228,37 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane)
 }
 
 // draws `take` entries from the top of queue `cls` (lane < take) and adds them to S
-__device__ __forceinline__ void drain_queue(DrawQueues &Q, int cls, int &count, bool everything, float *__restrict__ S,
-                                            int *__restrict__ totals, int lane)
+template <bool TOT>
+__device__ __forceinline__ void drain_queue(DrawQueues<TOT> &Q, int cls, int &count, bool everything,
+                                            float *__restrict__ S, int *__restrict__ totals, int lane)
 {
     while (count >= 32 || (everything && count > 0)) {
         const int take = min(32, count);
         count -= take;
         if (lane < take) {
             const int e = count + lane;
-            const uint32_t fl = Q.flags[cls][e];
+            const uint32_t fb = Q.bin[cls][e];
             const double N = (double)Q.N[cls][e];
-            const double k = draw_classified(cls, N, Q.p[cls][e], Q.w[cls][e], (fl & 1u) != 0);
+            const double k = draw_classified(cls, N, Q.p[cls][e], Q.w[cls][e], (fb & kBinMirror) != 0);
             if (k != 0.0) {
-                const float v = (fl & 2u) ? -(float)k : (float)k;
-                atomicAdd(S + Q.bin[cls][e], v);
-                if (totals != nullptr) atomicAdd(totals + (fl >> 8), (int)v);
+                const float v = (fb & kBinNegative) ? -(float)k : (float)k;
+                atomicAdd(S + (fb & kBinMask), v);
+                if constexpr (TOT) atomicAdd(totals + Q.depo[cls][e], (int)v);
             }
         }
         __syncwarp();
     }
 }
 
-template <bool FLUCT>
-__global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
+template <bool FLUCT, bool TOT>
+__global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
                                                                         uint64_t id_base, uint64_t seed, double nsigma,
                                                                         float *__restrict__ S, int *__restrict__ totals,
                                                                         Counters *counters)
 {
     using T = typename std::conditional<FLUCT, double, float>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    BatchSmem<FLUCT> &sm = *reinterpret_cast<BatchSmem<FLUCT> *>(smem_raw);
+    BatchSmem<FLUCT, TOT> &sm = *reinterpret_cast<BatchSmem<FLUCT, TOT> *>(smem_raw);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     BatchScratch<FLUCT> &sc = sm.scratch[wid];
     const GlobalSink sink{S, g.n_ticks};
@@ -387,14 +391,13 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
                     uint32_t w = pick_word(fluct_words(seed, id, gbin >> 2), (uint32_t)gbin & 3u);
                     bool mirror = false;
                     int cls = act ? classify_draw(Nn, p, w, mirror) : (int)kDrawZero;
-                    const uint32_t fl = (mirror ? 1u : 0u) | (qq < 0.0f ? 2u : 0u) |
-                                        ((uint32_t)(first + own) << 8);
+                    const uint32_t fb = (uint32_t)gbin | (mirror ? kBinMirror : 0u) | (qq < 0.0f ? kBinNegative : 0u);
                     if (cls == kDrawAll) { // p >= 1: every electron lands here
-                        const float v = (fl & 2u) ? -(float)Nn : (float)Nn;
+                        const float v = (qq < 0.0f) ? -(float)Nn : (float)Nn;
                         atomicAdd(S + gbin, v);
-                        if (totals != nullptr) atomicAdd(totals + first + own, (int)v);
+                        if constexpr (TOT) atomicAdd(totals + first + own, (int)v);
                     }
-                    DrawQueues &Q = sm.queues[wid];
+                    DrawQueues<TOT> &Q = sm.queues[wid];
                     // one slot per bin in the queue of its class: position = queue fill + rank among the lanes of the
                     // same class (ballots), then a single block of stores for all classes
                     unsigned int mine = 0;
@@ -411,8 +414,8 @@ __global__ void __launch_bounds__(kBatchWarps * 32, 6) raster_batch_kernel(GridD
                         Q.p[cls][pos] = p;
                         Q.N[cls][pos] = (float)Nn;
                         Q.w[cls][pos] = w;
-                        Q.bin[cls][pos] = (uint32_t)gbin;
-                        Q.flags[cls][pos] = fl;
+                        Q.bin[cls][pos] = fb;
+                        if constexpr (TOT) Q.depo[cls][pos] = (uint32_t)(first + own);
                     }
                     __syncwarp();
 #pragma unroll
@@ -607,11 +610,30 @@ cudaError_t raster_configure(cudaStream_t st)
     if (err != cudaSuccess) return err;
     err = cudaStreamSynchronize(st); // `tab` is on this stack
     if (err != cudaSuccess) return err;
-    err = cudaFuncSetAttribute(raster_batch_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           (int)sizeof(BatchSmem<true>));
+    err = cudaFuncSetAttribute(raster_batch_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (int)sizeof(BatchSmem<true, true>));
     if (err != cudaSuccess) return err;
-    return cudaFuncSetAttribute(raster_batch_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)sizeof(BatchSmem<false>));
+    err = cudaFuncSetAttribute(raster_batch_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (int)sizeof(BatchSmem<true, false>));
+    if (err != cudaSuccess) return err;
+    return cudaFuncSetAttribute(raster_batch_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)sizeof(BatchSmem<false, false>));
+}
+
+template <bool FLUCT, bool TOT>
+static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, double nsigma,
+                                       float *S, int *depo_totals, Counters *counters, int sm_count, cudaStream_t st)
+{
+    const long long n_batches = (n + kBatchDepos - 1) / kBatchDepos;
+    const size_t smem = sizeof(BatchSmem<FLUCT, TOT>);
+    const int fit = (int)((227u * 1024u) / (smem + 1024u)); // 227 KB per SM, 1 KB reserved per CTA
+    const int cap = FLUCT ? 6 : 8; // the kernel's __launch_bounds__ (7 CTAs of 72 registers: configs[1] -2 %, [2] +1.5 %)
+    const int ctas_per_sm = fit > cap ? cap : fit;
+    long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
+    const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
+    if (ctas > max_ctas) ctas = max_ctas;
+    return launch_pdl(raster_batch_kernel<FLUCT, TOT>, (unsigned)ctas, kBatchWarps * 32, smem, st, g, d, n, id_base, seed,
+                      nsigma, S, depo_totals, counters);
 }
 
 cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
@@ -619,20 +641,11 @@ cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t
                                  cudaStream_t st)
 {
     if (n <= 0) return cudaSuccess;
-    const long long n_batches = (n + kBatchDepos - 1) / kBatchDepos;
-    const size_t smem = fluctuate ? sizeof(BatchSmem<true>) : sizeof(BatchSmem<false>);
-    const int fit = (int)((227u * 1024u) / (smem + 1024u)); // 227 KB per SM, 1 KB reserved per CTA
-    const int ctas_per_sm = fit > 8 ? 8 : fit;
-    long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
-    const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
-    if (ctas > max_ctas) ctas = max_ctas;
-    if (fluctuate)
-        return launch_pdl(raster_batch_kernel<true>, (unsigned)ctas, kBatchWarps * 32, smem, st, g, d, n, id_base, seed,
-                          nsigma, S, depo_totals, counters);
-    else
-        return launch_pdl(raster_batch_kernel<false>, (unsigned)ctas, kBatchWarps * 32, smem, st, g, d, n, id_base, seed,
-                          nsigma, S, depo_totals, counters);
-    return cudaGetLastError();
+    if (!fluctuate) // no draws, no per-depo integer totals
+        return launch_raster_batch<false, false>(g, d, n, id_base, seed, nsigma, S, nullptr, counters, sm_count, st);
+    if (depo_totals)
+        return launch_raster_batch<true, true>(g, d, n, id_base, seed, nsigma, S, depo_totals, counters, sm_count, st);
+    return launch_raster_batch<true, false>(g, d, n, id_base, seed, nsigma, S, nullptr, counters, sm_count, st);
 }
 
 cudaError_t launch_tile_count(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts, cudaStream_t st)

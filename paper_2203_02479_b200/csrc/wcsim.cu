@@ -295,7 +295,7 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
         return WCSIM_EINVAL;
     if (pad_w < n_rwires) return WCSIM_EINVAL; // the wrapped response must not overlap itself
     if (!conv_sizes_supported(pad_w, pad_t)) return WCSIM_EINVAL;
-    if ((long long)n_wires * n_ticks > 0x7FFFFFFFll * 2) return WCSIM_EINVAL;
+    if ((long long)n_wires * n_ticks >= (1ll << 30)) return WCSIM_EINVAL; // bin index + 2 flag bits in 32 (draw queues)
 
     int dev = 0;
     CU_TRY(cudaGetDevice(&dev));
