@@ -140,9 +140,13 @@ def run_ours(args):
     d = {k: torch.from_numpy(v).to(dev) for k, v in pl["depos"].items()}
     flush = torch.empty(FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
 
+    noisy = bool(cfg.get("noise"))  # configs[3]: per-wire noise rides the inverse row transform (step a7)
+
     def step():
         plan.clear()
         plan.raster_scatter(d, seed=cfg["fluct_seed"], fluctuate=fluct)
+        if noisy:
+            plan.arm_noise(None, seed=cfg["noise_seed"])
         plan.convolve()
 
     def timed(fn, k, sampler=None):
@@ -294,7 +298,8 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if not fluct else "f32 (f64 fluctuation weights and sampler)", "data": "synthetic",
-        "config": {"workload": cfg["name"] + (", fluctuation on" if fluct else ", fluctuation off"),
+        "config": {"workload": cfg["name"] + (", fluctuation on" if fluct else ", fluctuation off") +
+                               (", noise fused (plane 0 timed)" if noisy else ""),
                    "grid": [pl["n_wires"], pl["n_ticks"]], "pad": [pl["pad_w"], pl["pad_t"]],
                    "response": list(pl["response"].shape), "depos": n_depos, "scatter": args.scatter,
                    "wire_axis": "direct" if direct else "fft",

@@ -207,12 +207,16 @@ __global__ void __launch_bounds__(32 * kWiresRG, 3) wires_kernel(GridDims g, Con
 // a6 tick axis (+ a7 noise): half spectrum -> real row
 // ------------------------------------------------------------------------------------------------------------------
 // noise spectrum of bin k on `wire`: amp[k] exp(2 pi i u), u = (word + 1/2) 2^-32 (A15-A17); amp is pre-scaled
+__device__ __forceinline__ float noise_phase(uint32_t w) // 2u = w 2^-31 + 2^-32, the argument of sincospi
+{
+    return (float)w * 4.656612873077393e-10f + 2.3283064365386963e-10f;
+}
 __device__ __forceinline__ float2 noise_bin(const NoiseArgs &nz, uint32_t wire, uint32_t k)
 {
     const uint4 words = noise_words(nz.seed, wire, k >> 2);
     const uint32_t w = pick_word(words, k & 3u);
     float s, c;
-    sincospif((float)w * 4.656612873077393e-10f + 2.3283064365386963e-10f, &s, &c); // 2u = w 2^-31 + 2^-32
+    sincospif(noise_phase(w), &s, &c);
     const float a = __ldg(nz.amp + k);
     return make_float2(a * c, a * s);
 }
@@ -303,12 +307,20 @@ __global__ void __launch_bounds__(RowTma<N>::threads, RowTma<N>::min_ctas) rows_
         mbar_wait(bar, parity);
         parity ^= 1u;
         if (noisy) {
-#pragma unroll
-            for (int e = 0; e < E; ++e) {
-                const int k = i + e * NT;
-                stage[k] = cadd(stage[k], noise_bin(nz, (uint32_t)row, (uint32_t)k));
-                if (k == 0) stage[N] = cadd(stage[N], noise_bin(nz, (uint32_t)row, (uint32_t)N));
+            // one Philox call gives the phases of four consecutive frequency bins (A17): a thread takes whole calls
+            for (int q = i; q < N / 4; q += NT) {
+                const uint4 words = noise_words(nz.seed, (uint32_t)row, (uint32_t)q);
+                const float4 a = __ldg(reinterpret_cast<const float4 *>(nz.amp) + q);
+                float4 *x = reinterpret_cast<float4 *>(stage + 4 * q);
+                float4 lo = x[0], hi = x[1];
+                float sn, cs;
+                sincospif(noise_phase(words.x), &sn, &cs), lo.x = fmaf(a.x, cs, lo.x), lo.y = fmaf(a.x, sn, lo.y);
+                sincospif(noise_phase(words.y), &sn, &cs), lo.z = fmaf(a.y, cs, lo.z), lo.w = fmaf(a.y, sn, lo.w);
+                sincospif(noise_phase(words.z), &sn, &cs), hi.x = fmaf(a.z, cs, hi.x), hi.y = fmaf(a.z, sn, hi.y);
+                sincospif(noise_phase(words.w), &sn, &cs), hi.z = fmaf(a.w, cs, hi.z), hi.w = fmaf(a.w, sn, hi.w);
+                x[0] = lo, x[1] = hi;
             }
+            if (i == 0) stage[N] = cadd(stage[N], noise_bin(nz, (uint32_t)row, (uint32_t)N));
             __syncthreads();
         }
         // Z_k = (X_k + conj X_{N-k}) + i exp(+2 pi i k / 2N) (X_k - conj X_{N-k});  inverse FFT of Z = even + i odd
