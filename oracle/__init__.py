@@ -49,6 +49,8 @@ def lib():
         L.wco_norm_ppf.restype = C.c_double
         L.wco_binomial.argtypes = [C.c_double, C.c_double, C.c_uint32]
         L.wco_binomial.restype = C.c_double
+        L.wco_normal_draw.argtypes = [C.c_double, C.c_double, C.c_uint32]
+        L.wco_normal_draw.restype = C.c_double
         L.wco_axis_extent.argtypes = [C.c_double, C.c_double, C.c_double, i64p, i64p]
         L.wco_axis_extent.restype = None
         L.wco_axis_weight.argtypes = [C.c_int64, C.c_double, C.c_double]
@@ -121,6 +123,11 @@ def binomial(N: float, p: float, w: int) -> float:
     return float(lib().wco_binomial(float(N), float(p), int(w) & 0xFFFFFFFF))
 
 
+def normal_draw(N: float, p: float, w: int) -> float:
+    """The normal-approximation draw of the paper's Kokkos port (reading A21)."""
+    return float(lib().wco_normal_draw(float(N), float(p), int(w) & 0xFFFFFFFF))
+
+
 def axis_extent(centre, sigma, nsigma=3.0):
     i0, i1 = C.c_int64(), C.c_int64()
     lib().wco_axis_extent(float(centre), float(sigma), float(nsigma), C.byref(i0), C.byref(i1))
@@ -144,6 +151,18 @@ def patch_axes(t0, x0, sigma_t, sigma_x, nsigma=3.0, max_bins=4096):
     return it0.value, ix0.value, wt[: it1.value - it0.value].copy(), wx[: ix1.value - ix0.value].copy()
 
 
+def _fluct_mode(fluctuate) -> int:
+    """False/0: off, True/1: binomial (A6), 2 or "normal": normal approximation (A21)."""
+    if fluctuate == "normal":
+        return 2
+    if fluctuate == "binomial":
+        return 1
+    m = int(fluctuate)
+    if m not in (0, 1, 2):
+        raise ValueError("fluctuate must be 0, 1 or 2")
+    return m
+
+
 def raster_scatter(n_wires, n_ticks, depos, *, seed=0, fluctuate=False, nsigma=3.0, ids=None, id_base=0,
                    window=None, want_totals=False, S=None):
     """depos = dict(t0,x0,sigma_t,sigma_x,q) of float arrays.  Returns (S_window fp64, totals|None, stats)."""
@@ -161,7 +180,7 @@ def raster_scatter(n_wires, n_ticks, depos, *, seed=0, fluctuate=False, nsigma=3
         assert ids.shape[0] == n
         idp = _p(ids, C.c_uint64)
     rc = lib().wco_raster_scatter(n_wires, n_ticks, _p(t0, C.c_float), _p(x0, C.c_float), _p(st, C.c_float),
-                                  _p(sx, C.c_float), _p(q, C.c_float), n, idp, id_base, seed, int(bool(fluctuate)),
+                                  _p(sx, C.c_float), _p(q, C.c_float), n, idp, id_base, seed, _fluct_mode(fluctuate),
                                   float(nsigma), w0, w1, k0, k1, _p(S, C.c_double),
                                   _p(totals, C.c_int32) if want_totals else None, _p(stats, C.c_int64))
     if rc != 0:

@@ -24,6 +24,8 @@
  *   philox ................ published known-answer vectors (tests/golden/)
  *   norm_ppf .............. published normal quantiles (tests/golden/), scipy ndtri
  *   binomial .............. exact binomial CDF break points, mirror identity, moments
+ *   normal_draw ........... its formula restated with scipy's ndtri, moments, the paper's
+ *                           0.01 % agreement with the binomial waveforms
  *   noise ................. Parseval closed form, spectrum round trip, direct vs FFT
  * PARITY UNPINNED (conventions of this build that nothing in the paper fixes;
  * DESIGN.md readings A3, A6, A8, A15): no patch renormalisation; the mu<16
@@ -221,6 +223,28 @@ int wco_patch_axes(float t0, float x0, float sigma_t, float sigma_x, double nsig
 }
 
 /* ------------------------------------------------------------------------- */
+/* Normal-approximation draw G(N, p, w) -- the sampler of the paper's Kokkos    */
+/* port: "the Kokkos version uses normal distribution to approximate the       */
+/* binomial distribution", PAPER.md:82 (Section 3.1).  Reading A21:            */
+/*   N = 0 or p <= 0 -> 0;  p >= 1 -> N;                                       */
+/*   else clamp(rint(N p + sqrt(N p (1-p)) Phi^-1(u)), 0, N) for EVERY mu       */
+/*   (no inversion branch, no mirror), u = (w + 1/2) 2^-32, Phi^-1 = AS 241.    */
+/* ------------------------------------------------------------------------- */
+double wco_normal_draw(double N, double p, uint32_t w)
+{
+    if (!(N > 0.0) || !(p > 0.0)) return 0.0;
+    if (p >= 1.0) return N;
+    double u = u01(w);
+    double mu = N * p;
+    double sd = sqrt(mu * (1.0 - p));
+    double x = mu + sd * wco_norm_ppf(u);
+    double k = rint(x);
+    if (k < 0.0) k = 0.0;
+    if (k > N) k = N;
+    return k;
+}
+
+/* ------------------------------------------------------------------------- */
 /* Raster + Scatter-add: patches "stacked and summed over a    */
 /* larger grid"; dense grid as in PAPER.md:75.  Serial, in depo order.          */
 /*                                                                            */
@@ -233,6 +257,7 @@ int wco_patch_axes(float t0, float x0, float sigma_t, float sigma_x, double nsig
 /*                                                                            */
 /* fluctuate = 0: c = Q p.   fluctuate = 1: Ntr = floor(|Q| + 1/2),             */
 /* c = sign(Q) B(Ntr, p, word(seed, id, g)), g = wire*n_ticks + tick (A6-A9).   */
+/* fluctuate = 2: the same with the normal-approximation draw G (A21).          */
 /* ids == NULL means depo i has id id_base + i.                                */
 /* totals (optional, n entries): signed sum of the draws over all in-grid bins */
 /* of each depo (forces drawing outside the window too).                       */
@@ -272,7 +297,8 @@ int wco_raster_scatter(int n_wires, int n_ticks,
                 double c;
                 if (fluctuate) {
                     uint64_t g = (uint64_t)j * (uint64_t)n_ticks + (uint64_t)i;
-                    double k = wco_binomial(Ntr, p, wco_fluct_word(seed, id, g));
+                    uint32_t word = wco_fluct_word(seed, id, g);
+                    double k = (fluctuate == 2) ? wco_normal_draw(Ntr, p, word) : wco_binomial(Ntr, p, word);
                     tot += (int64_t)(sgn * k);
                     c = sgn * k;
                 } else {
