@@ -132,6 +132,8 @@ def run_ours(args):
     pl = cfg["planes"][0]
     n_depos = int(pl["depos"]["t0"].shape[0])
     fluct = bool(cfg["fluctuate"]) and not args.no_fluct
+    if fluct and args.fluct == "normal":
+        fluct = 2
     mode = B.WCSIM_SCATTER_TILED if args.scatter == "tiled" else B.WCSIM_SCATTER_ATOMIC
     stream = torch.cuda.current_stream()
     plan = B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]), nsigma=cfg["nsigma"],
@@ -298,7 +300,8 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if not fluct else "f32 (f64 fluctuation weights and sampler)", "data": "synthetic",
-        "config": {"workload": cfg["name"] + (", fluctuation on" if fluct else ", fluctuation off") +
+        "config": {"workload": cfg["name"] + (", fluctuation off" if not fluct else ", normal-approximation fluctuation" if fluct == 2
+                                             else ", fluctuation on") +
                                (", noise fused (plane 0 timed)" if noisy else ""),
                    "grid": [pl["n_wires"], pl["n_ticks"]], "pad": [pl["pad_w"], pl["pad_t"]],
                    "response": list(pl["response"].shape), "depos": n_depos, "scatter": args.scatter,
@@ -468,6 +471,8 @@ def main():
     ap.add_argument("--scatter", default="atomic", choices=["atomic", "tiled"])
     ap.add_argument("--wires", default="auto", choices=["auto", "fft", "direct"], help="wire axis of the convolution")
     ap.add_argument("--no-fluct", action="store_true")
+    ap.add_argument("--fluct", default="binomial", choices=["binomial", "normal"],
+                    help="sampler of the fluctuated raster: reading A6 (headline) or the Kokkos port's normal approximation (A21)")
     ap.add_argument("--streams", type=int, default=3, help="plane-events in flight for the extra `concurrent` figure")
     ap.add_argument("--e2e-steps", type=int, default=200)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")

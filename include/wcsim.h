@@ -96,9 +96,12 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
  *   fluctuate = 0 : S[j][i] += q p_ij                         (weights in fp32)
  *   fluctuate = 1 : S[j][i] += sign(q) B(floor(|q|+1/2), p_ij; w)   (weights, p and the sampler in fp64; A6, A7)
  *                   with w the Philox4x32-10 word keyed (seed, id, absolute grid bin j*n_ticks+i) (A8).
+ *   fluctuate = 2 : the same with the normal approximation the paper's Kokkos port uses (A21):
+ *                   S[j][i] += sign(q) clamp(rint(N p + sqrt(N p (1-p)) Phi^-1(u)), 0, N), N = floor(|q|+1/2), for every mu.
+ *                   Any other value: WCSIM_EINVAL.
  * Bins outside the grid are dropped and not drawn (A5).  S accumulates across calls; wcsim_clear zeroes it.
  *   depos           : struct of DEVICE pointers (the struct itself is read on the host during the call).
- *   dev_depo_totals : DEVICE, n int32, or NULL.  With fluctuate = 1 receives the signed sum of each depo's draws.
+ *   dev_depo_totals : DEVICE, n int32, or NULL.  With fluctuate = 1 or 2 receives the signed sum of each depo's draws.
  * n = 0 is valid and does nothing.
  */
 int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n, unsigned long long depo_id_base,
@@ -181,12 +184,15 @@ int wcsim_simulate_host_async(wcsim_plan *plan, const float *host_t0, const floa
 /* out[4] (DEVICE, 4*n uint32) = Philox4x32-10(ctr = dev_ctr[4*i..], key = dev_key[2*i..]) for i < n */
 int wcsim_debug_philox(const unsigned int *dev_ctr, const unsigned int *dev_key, unsigned int *dev_out, long long n,
                        void *cuda_stream);
-/* dev_k[i] = B(dev_N[i], dev_p[i]; dev_w[i]) -- the device binomial sampler (fp64 in, fp64 integer-valued out) */
 /* The raster's own fp64 erf (a 48-interval degree-12 Taylor table, csrc/erf_table.cuh) evaluated on the HOST with the
  * same code the kernels run: out[i] = erf(z[i]).  HOST pointers, n elements each; no device is touched.  Used by the
  * CPU tests to pin the table against a library erf (bin weights of reading A2). */
 int wcsim_debug_erf(const double *host_z, double *host_out, long long n);
+/* dev_k[i] = B(dev_N[i], dev_p[i]; dev_w[i]) -- the device binomial sampler (fp64 in, fp64 integer-valued out) */
 int wcsim_debug_binomial(const double *dev_N, const double *dev_p, const unsigned int *dev_w, double *dev_k,
+                         long long n, void *cuda_stream);
+/* dev_k[i] = G(dev_N[i], dev_p[i]; dev_w[i]) -- the normal-approximation draw of fluctuate = 2 (A21) */
+int wcsim_debug_normal_draw(const double *dev_N, const double *dev_p, const unsigned int *dev_w, double *dev_k,
                          long long n, void *cuda_stream);
 /* copy the response spectrum Rhat[kx][kt] (kx < pad_wires, kt <= pad_ticks/2) to HOST as interleaved re,im floats */
 int wcsim_debug_response_spectrum(wcsim_plan *plan, float *host_out);

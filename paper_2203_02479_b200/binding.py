@@ -23,7 +23,7 @@ SYMBOLS = [
     "wcsim_plan_destroy", "wcsim_clear", "wcsim_clear_output", "wcsim_sync", "wcsim_set_scatter_mode", "wcsim_set_wire_mode",
     "wcsim_charge_ptr", "wcsim_output_ptr", "wcsim_get_dims", "wcsim_get_stats", "wcsim_reset_stats",
     "wcsim_simulate_host", "wcsim_set_profiling", "wcsim_get_stage_times", "wcsim_get_launch_count",
-    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf", "wcsim_simulate_host_async",
+    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf", "wcsim_simulate_host_async", "wcsim_debug_normal_draw",
     "wcsim_strerror", "wcsim_last_cuda_error", "wcsim_version",
 ]
 
@@ -82,6 +82,7 @@ def lib():
         L.wcsim_get_launch_count.argtypes = [vp, C.POINTER(ull)]
         L.wcsim_debug_philox.argtypes = [vp, vp, vp, ll, vp]
         L.wcsim_debug_binomial.argtypes = [vp, vp, vp, vp, ll, vp]
+        L.wcsim_debug_normal_draw.argtypes = [vp, vp, vp, vp, ll, vp]
         L.wcsim_debug_response_spectrum.argtypes = [vp, vp]
         L.wcsim_debug_erf.argtypes = [vp, vp, ll]
         L.wcsim_strerror.argtypes = [i]
@@ -144,6 +145,16 @@ def wcsim_plan_create(n_wires, n_ticks, response, pad=(0, 0), nsigma=3.0, scatte
     return h
 
 
+WCSIM_FLUCT_OFF, WCSIM_FLUCT_BINOMIAL, WCSIM_FLUCT_NORMAL = 0, 1, 2
+
+
+def _fluct(fluctuate) -> int:
+    """False/0: off; True/1/"binomial": reading A6; 2/"normal": the Kokkos port's normal approximation (A21)."""
+    if isinstance(fluctuate, str):
+        return {"off": 0, "binomial": 1, "normal": 2}[fluctuate]
+    return int(fluctuate)
+
+
 def wcsim_raster_scatter(plan, depos, n=None, depo_id_base=0, seed=0, fluctuate=False, dev_depo_totals=None):
     """depos: dict (or object) of torch CUDA float32 tensors t0, x0, sigma_t, sigma_x, q."""
     import torch
@@ -155,7 +166,7 @@ def wcsim_raster_scatter(plan, depos, n=None, depo_id_base=0, seed=0, fluctuate=
         if a.numel() < n:
             raise ValueError("depo array shorter than n")
     d = wcsim_depos(*[_dev_ptr(a, torch.float32) for a in arrs])
-    st = lib().wcsim_raster_scatter(plan, C.byref(d), int(n), int(depo_id_base), int(seed), int(bool(fluctuate)),
+    st = lib().wcsim_raster_scatter(plan, C.byref(d), int(n), int(depo_id_base), int(seed), _fluct(fluctuate),
                                     _dev_ptr(dev_depo_totals, torch.int32))
     _check(st, "wcsim_raster_scatter")
 
@@ -253,7 +264,7 @@ def wcsim_simulate_host(plan, host_depos, host_M, n=None, seed=0, fluctuate=Fals
     if n is None:
         n = ptrs[0][1]
     pm, _ = hp(host_M)
-    st = getattr(lib(), _fn)(plan, *[p for p, _ in ptrs], int(n), int(seed), int(bool(fluctuate)),
+    st = getattr(lib(), _fn)(plan, *[p for p, _ in ptrs], int(n), int(seed), _fluct(fluctuate),
                              int(bool(noise)), int(noise_seed), pm)
     _check(st, _fn)
 
@@ -292,6 +303,11 @@ def wcsim_debug_philox(dev_ctr, dev_key, dev_out, n, stream=None):
 def wcsim_debug_binomial(dev_N, dev_p, dev_w, dev_k, n, stream=None):
     _check(lib().wcsim_debug_binomial(_dev_ptr(dev_N), _dev_ptr(dev_p), _dev_ptr(dev_w), _dev_ptr(dev_k), int(n),
                                       _stream_ptr(stream)), "wcsim_debug_binomial")
+
+
+def wcsim_debug_normal_draw(dev_N, dev_p, dev_w, dev_k, n, stream=None):
+    _check(lib().wcsim_debug_normal_draw(_dev_ptr(dev_N), _dev_ptr(dev_p), _dev_ptr(dev_w), _dev_ptr(dev_k), int(n),
+                                         _stream_ptr(stream)), "wcsim_debug_normal_draw")
 
 
 def wcsim_debug_erf(z):

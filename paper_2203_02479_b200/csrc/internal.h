@@ -92,6 +92,6 @@ cudaError_t build_response_rows(const double2 *dev_tmp, int n_rw, int rt_rows, i
 cudaError_t launch_debug_philox(const unsigned int *ctr, const unsigned int *key, unsigned int *out, long long n,
                                 cudaStream_t st);
 cudaError_t launch_debug_binomial(const double *N, const double *p, const unsigned int *w, double *k, long long n,
-                                  cudaStream_t st);
+                                  bool normal_only, cudaStream_t st);
 
 } // namespace wcsim

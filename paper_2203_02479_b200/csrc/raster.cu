@@ -18,6 +18,7 @@
 //
 //   fluctuate = 0: fp32 weights (erff), value q * (wt * wx)
 //   fluctuate = 1: fp64 weights (erf), p = wt * wx, integer draw B(N, p; Philox word of the absolute bin)
+//   fluctuate = 2: the same with the normal-approximation draw of the paper's Kokkos port (reading A21)
 //
 // Two scatter modes:
 //   atomic: red.global.add.f32 straight into S
@@ -115,7 +116,8 @@ struct TileSink {
 template <bool FLUCT, typename Sink>
 __device__ __forceinline__ unsigned int raster_depo(float t0f, float x0f, float stf, float sxf, float qf, uint64_t id,
                                                     uint64_t seed, double nsigma, int n_ticks, int w_lo, int w_hi,
-                                                    int k_lo, int k_hi, const Sink &sink, int lane, int *lane_total)
+                                                    int k_lo, int k_hi, const Sink &sink, int lane, int *lane_total,
+                                                    bool normal_only)
 {
     using T = typename std::conditional<FLUCT, double, float>::type;
     const double T0 = t0f, X0 = x0f, ST = stf, SX = sxf;
@@ -141,7 +143,7 @@ __device__ __forceinline__ unsigned int raster_depo(float t0f, float x0f, float 
                         const double p = __dmul_rn(wt, wxj);
                         const uint64_t g = (uint64_t)wire * (uint64_t)n_ticks + (uint64_t)tick;
                         const uint4 words = fluct_words(seed, id, g >> 2);
-                        const double k = binomial_draw(Ntr, p, pick_word(words, (uint32_t)g & 3u));
+                        const double k = binomial_draw(Ntr, p, pick_word(words, (uint32_t)g & 3u), normal_only);
                         if (k != 0.0) {
                             const double v = sgn * k;
                             *lane_total += (int)v;
@@ -254,7 +256,7 @@ template <bool FLUCT, bool TOT>
 __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
                                                                         uint64_t id_base, uint64_t seed, double nsigma,
                                                                         float *__restrict__ S, int *__restrict__ totals,
-                                                                        Counters *counters)
+                                                                        Counters *counters, bool normal_only)
 {
     using T = typename std::conditional<FLUCT, double, float>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -324,7 +326,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
             drawn += raster_depo<FLUCT>(__shfl_sync(0xffffffffu, t0, src), __shfl_sync(0xffffffffu, x0, src),
                                         __shfl_sync(0xffffffffu, st, src), __shfl_sync(0xffffffffu, sx, src),
                                         __shfl_sync(0xffffffffu, q, src), id_base + (uint64_t)(first + src), seed,
-                                        nsigma, g.n_ticks, 0, g.n_wires, 0, g.n_ticks, sink, lane, &tot);
+                                        nsigma, g.n_ticks, 0, g.n_wires, 0, g.n_ticks, sink, lane, &tot, normal_only);
             if (totals != nullptr) {
                 tot = warp_sum(tot);
                 if (lane == 0 && tot != 0) atomicAdd(totals + first + src, tot);
@@ -390,7 +392,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
                     const uint64_t id = id_base + (uint64_t)(first + own);
                     uint32_t w = pick_word(fluct_words(seed, id, gbin >> 2), (uint32_t)gbin & 3u);
                     bool mirror = false;
-                    int cls = act ? classify_draw(Nn, p, w, mirror) : (int)kDrawZero;
+                    int cls = act ? classify_draw(Nn, p, w, mirror, normal_only) : (int)kDrawZero;
                     const uint32_t fb = (uint32_t)gbin | (mirror ? kBinMirror : 0u) | (qq < 0.0f ? kBinNegative : 0u);
                     if (cls == kDrawAll) { // p >= 1: every electron lands here
                         const float v = (qq < 0.0f) ? -(float)Nn : (float)Nn;
@@ -540,7 +542,7 @@ __global__ void tile_fill_kernel(GridDims g, DepoArrays d, long long n, double n
 template <bool FLUCT>
 __global__ void __launch_bounds__(256) tile_accumulate_kernel(GridDims g, DepoArrays d, uint64_t id_base, uint64_t seed,
                                                               double nsigma, TileScratch ts, float *__restrict__ S,
-                                                              int *__restrict__ totals, Counters *counters)
+                                                              int *__restrict__ totals, Counters *counters, bool normal_only)
 {
     __shared__ unsigned long long acc[kTileW * kTileT];
     const int tile = blockIdx.x;
@@ -560,7 +562,7 @@ __global__ void __launch_bounds__(256) tile_accumulate_kernel(GridDims g, DepoAr
                     q = __ldg(d.q + i);
         int tot = 0;
         drawn += raster_depo<FLUCT>(t0, x0, st, sx, q, id_base + (uint64_t)i, seed, nsigma, g.n_ticks, w0, w1, k0, k1,
-                                    sink, lane, &tot);
+                                    sink, lane, &tot, normal_only);
         if (totals != nullptr) {
             tot = warp_sum(tot);
             if (lane == 0 && tot != 0) atomicAdd(totals + i, tot);
@@ -622,7 +624,8 @@ cudaError_t raster_configure(cudaStream_t st)
 
 template <bool FLUCT, bool TOT>
 static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, double nsigma,
-                                       float *S, int *depo_totals, Counters *counters, int sm_count, cudaStream_t st)
+                                       float *S, int *depo_totals, Counters *counters, int sm_count, cudaStream_t st,
+                                       bool normal_only)
 {
     const long long n_batches = (n + kBatchDepos - 1) / kBatchDepos;
     const size_t smem = sizeof(BatchSmem<FLUCT, TOT>);
@@ -633,7 +636,7 @@ static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, ui
     const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
     if (ctas > max_ctas) ctas = max_ctas;
     return launch_pdl(raster_batch_kernel<FLUCT, TOT>, (unsigned)ctas, kBatchWarps * 32, smem, st, g, d, n, id_base, seed,
-                      nsigma, S, depo_totals, counters);
+                      nsigma, S, depo_totals, counters, normal_only);
 }
 
 cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
@@ -642,10 +645,11 @@ cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t
 {
     if (n <= 0) return cudaSuccess;
     if (!fluctuate) // no draws, no per-depo integer totals
-        return launch_raster_batch<false, false>(g, d, n, id_base, seed, nsigma, S, nullptr, counters, sm_count, st);
+        return launch_raster_batch<false, false>(g, d, n, id_base, seed, nsigma, S, nullptr, counters, sm_count, st, false);
     if (depo_totals)
-        return launch_raster_batch<true, true>(g, d, n, id_base, seed, nsigma, S, depo_totals, counters, sm_count, st);
-    return launch_raster_batch<true, false>(g, d, n, id_base, seed, nsigma, S, nullptr, counters, sm_count, st);
+        return launch_raster_batch<true, true>(g, d, n, id_base, seed, nsigma, S, depo_totals, counters, sm_count, st,
+                                               fluctuate == 2);
+    return launch_raster_batch<true, false>(g, d, n, id_base, seed, nsigma, S, nullptr, counters, sm_count, st, fluctuate == 2);
 }
 
 cudaError_t launch_tile_count(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts, cudaStream_t st)
@@ -674,9 +678,11 @@ cudaError_t launch_tile_accumulate(GridDims g, DepoArrays d, uint64_t id_base, u
 {
     const int n_tiles = ts.tiles_w * ts.tiles_t;
     if (fluctuate)
-        tile_accumulate_kernel<true><<<n_tiles, 256, 0, st>>>(g, d, id_base, seed, nsigma, ts, S, depo_totals, counters);
+        tile_accumulate_kernel<true><<<n_tiles, 256, 0, st>>>(g, d, id_base, seed, nsigma, ts, S, depo_totals, counters,
+                                                              fluctuate == 2);
     else
-        tile_accumulate_kernel<false><<<n_tiles, 256, 0, st>>>(g, d, id_base, seed, nsigma, ts, S, depo_totals, counters);
+        tile_accumulate_kernel<false><<<n_tiles, 256, 0, st>>>(g, d, id_base, seed, nsigma, ts, S, depo_totals, counters,
+                                                               false);
     return cudaGetLastError();
 }
 

@@ -88,11 +88,12 @@ __global__ void debug_philox_kernel(const unsigned int *ctr, const unsigned int 
     out[4 * i + 3] = r.w;
 }
 
-__global__ void debug_binomial_kernel(const double *N, const double *p, const unsigned int *w, double *k, long long n)
+__global__ void debug_binomial_kernel(const double *N, const double *p, const unsigned int *w, double *k, long long n,
+                                      bool normal_only)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    k[i] = binomial_draw(N[i], p[i], w[i]);
+    k[i] = binomial_draw(N[i], p[i], w[i], normal_only);
 }
 
 } // namespace
@@ -128,10 +129,10 @@ cudaError_t launch_debug_philox(const unsigned int *ctr, const unsigned int *key
 }
 
 cudaError_t launch_debug_binomial(const double *N, const double *p, const unsigned int *w, double *k, long long n,
-                                  cudaStream_t st)
+                                  bool normal_only, cudaStream_t st)
 {
     if (n <= 0) return cudaSuccess;
-    debug_binomial_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(N, p, w, k, n);
+    debug_binomial_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(N, p, w, k, n, normal_only);
     return cudaGetLastError();
 }
 

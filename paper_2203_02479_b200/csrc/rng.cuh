@@ -94,11 +94,14 @@ __device__ __forceinline__ bool word_is_central(uint32_t w) { return w - 3221225
 
 // Folds the p > 1/2 mirror into (p, w) and says which routine draws k.  On return p <= 1/2.
 // Shortcut: (1-p)^N >= 1 - N p (Bernoulli), so u <= 1 - mu already implies u <= F(0), i.e. k = 0, without exp/log.
-__device__ __forceinline__ int classify_draw(double N, double &p, uint32_t &w, bool &mirror)
+// normal_only: the normal-approximation sampler of the paper's Kokkos port (reading A21): the rounded normal
+// for every mu, no inversion branch and no mirror -- only the two AS 241 routines are ever queued.
+__device__ __forceinline__ int classify_draw(double N, double &p, uint32_t &w, bool &mirror, bool normal_only = false)
 {
     mirror = false;
     if (!(N > 0.0) || !(p > 0.0)) return kDrawZero;
     if (p >= 1.0) return kDrawAll;
+    if (normal_only) return word_is_central(w) ? kDrawNormalCentral : kDrawNormalTail;
     mirror = p > 0.5;
     if (mirror) {
         p = __dsub_rn(1.0, p);
@@ -243,10 +246,10 @@ __device__ __forceinline__ double draw_classified(int cls, double N, double p, u
 }
 
 // the whole sampler for one bin (debug hook, big-patch and tiled paths)
-__device__ __forceinline__ double binomial_draw(double N, double p, uint32_t w)
+__device__ __forceinline__ double binomial_draw(double N, double p, uint32_t w, bool normal_only = false)
 {
     bool mirror;
-    const int cls = classify_draw(N, p, w, mirror);
+    const int cls = classify_draw(N, p, w, mirror, normal_only);
     if (cls == kDrawZero) return 0.0;
     if (cls == kDrawAll) return N;
     return draw_classified(cls, N, p, w, mirror);

@@ -382,7 +382,7 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
 int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n, unsigned long long depo_id_base,
                          unsigned long long seed, int fluctuate, int *dev_depo_totals)
 {
-    if (!plan || n < 0) return WCSIM_EINVAL;
+    if (!plan || n < 0 || fluctuate < 0 || fluctuate > 2) return WCSIM_EINVAL;
     if (n == 0) return WCSIM_OK;
     if (!depos || !depos->t0 || !depos->x0 || !depos->sigma_t || !depos->sigma_x || !depos->q) return WCSIM_EINVAL;
     DeviceGuard guard(plan->device);
@@ -392,7 +392,7 @@ int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n
     StageSpan span(plan, WCSIM_STAGE_RASTER);
     if (plan->scatter_mode == WCSIM_SCATTER_TILED) {
         plan->launches += 5;
-        return raster_tiled(plan, g, d, n, depo_id_base, seed, fluctuate != 0, dev_depo_totals);
+        return raster_tiled(plan, g, d, n, depo_id_base, seed, fluctuate, dev_depo_totals);
     }
     if (dev_depo_totals) CU_TRY(cudaMemsetAsync(dev_depo_totals, 0, sizeof(int) * (size_t)n, plan->stream));
     // the draw queues index per-depo totals with 24 bits: with totals requested, launch 2^24 depos at a time
@@ -401,7 +401,7 @@ int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n
         const long long m = n - first < chunk ? n - first : chunk;
         const DepoArrays dc{d.t0 + first, d.x0 + first, d.sigma_t + first, d.sigma_x + first, d.q + first};
         plan->launches += 1;
-        CU_TRY(launch_raster_atomic(g, dc, m, depo_id_base + (unsigned long long)first, seed, fluctuate != 0, plan->nsigma,
+        CU_TRY(launch_raster_atomic(g, dc, m, depo_id_base + (unsigned long long)first, seed, fluctuate, plan->nsigma,
                                     plan->S, dev_depo_totals ? dev_depo_totals + first : nullptr, plan->counters,
                                     plan->sm_count, plan->stream));
     }
@@ -630,7 +630,15 @@ int wcsim_debug_binomial(const double *dev_N, const double *dev_p, const unsigne
                          long long n, void *cuda_stream)
 {
     if (n < 0 || (n > 0 && (!dev_N || !dev_p || !dev_w || !dev_k))) return WCSIM_EINVAL;
-    CU_TRY(launch_debug_binomial(dev_N, dev_p, dev_w, dev_k, n, (cudaStream_t)cuda_stream));
+    CU_TRY(launch_debug_binomial(dev_N, dev_p, dev_w, dev_k, n, false, (cudaStream_t)cuda_stream));
+    return WCSIM_OK;
+}
+
+int wcsim_debug_normal_draw(const double *dev_N, const double *dev_p, const unsigned int *dev_w, double *dev_k,
+                         long long n, void *cuda_stream)
+{
+    if (n < 0 || (n > 0 && (!dev_N || !dev_p || !dev_w || !dev_k))) return WCSIM_EINVAL;
+    CU_TRY(launch_debug_binomial(dev_N, dev_p, dev_w, dev_k, n, true, (cudaStream_t)cuda_stream));
     return WCSIM_OK;
 }
 

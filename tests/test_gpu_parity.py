@@ -430,3 +430,51 @@ def test_simulate_host_async_two_plans_alternating(B, O):
     finally:
         for p in plans:
             p.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# fluctuate = 2: the normal-approximation sampler of the paper's Kokkos port (reading A21)
+# ---------------------------------------------------------------------------------------------------------------
+def test_normal_draw_sampler_matches_oracle(B, O):
+    rng = np.random.default_rng(9)
+    n = 200_000
+    N = np.floor(np.exp(rng.uniform(0, np.log(2e5), n)))
+    p = np.where(rng.random(n) < 0.5, rng.random(n), np.exp(rng.uniform(np.log(1e-9), 0, n)))
+    w = rng.integers(0, 2**32, size=n, dtype=np.uint64).astype(np.uint32)
+    N[:6] = [0, 10, 10, 1000, 32, 5000]
+    p[:6] = [0.3, 0.0, 1.0, 0.5, 0.5, 1e-300]
+    w[6:10] = [0, 0xFFFFFFFF, 0x80000000, 0x7FFFFFFF]
+    dN, dp = torch.from_numpy(N).cuda(), torch.from_numpy(p).cuda()
+    dw = torch.from_numpy(w.view(np.int32)).cuda()
+    dk = torch.zeros(n, dtype=torch.float64, device="cuda")
+    B.wcsim_debug_normal_draw(dN, dp, dw, dk, n)
+    torch.cuda.synchronize()
+    got = dk.cpu().numpy()
+    ref = np.array([O.normal_draw(N[i], p[i], int(w[i])) for i in range(n)])
+    bad = np.flatnonzero(got != ref)
+    assert bad.size <= max(1, int(1e-6 * n)), [(N[i], p[i], w[i], got[i], ref[i]) for i in bad[:5]]
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_normal_fluctuation_integer_grid_exact(B, O, mode):
+    from paper_2203_02479_b200 import synth
+    cfg = synth.config(1, n_depos=30_000)
+    pl = cfg["planes"][0]
+    nw, nt = pl["n_wires"], pl["n_ticks"]
+    S_ref, tot_ref, st = O.raster_scatter(nw, nt, pl["depos"], seed=3, fluctuate=2, want_totals=True)
+    d = to_dev(pl["depos"])
+    totals = torch.zeros(30_000, dtype=torch.int32, device="cuda")
+    with B.Plan(nw, nt, synth.response(5, 16), scatter_mode=mode) as p:
+        p.clear()
+        p.raster_scatter(d, seed=3, fluctuate=2, dev_depo_totals=totals)
+        p.sync()
+        S = p.charge().cpu().numpy().astype(np.float64)
+        with pytest.raises(B.WcsimError):
+            p.raster_scatter(d, seed=3, fluctuate=3)
+    flipped = int(np.count_nonzero(S != S_ref))
+    assert flipped <= 1e-6 * st["drawn"], (flipped, st["drawn"])
+    assert int(np.count_nonzero(totals.cpu().numpy() != tot_ref)) <= flipped
+    # and it is a different grid from the binomial one (same words, different sampler on small means)
+    S_bin, _, _ = O.raster_scatter(nw, nt, pl["depos"], seed=3, fluctuate=1)
+    assert np.count_nonzero(S != S_bin) > 1000
+    assert abs(S.sum() - S_bin.sum()) <= 3e-4 * S_bin.sum()  # agreement at the 0.01 % level
