@@ -92,23 +92,39 @@ __device__ __forceinline__ T axis_weights(int base, double centre, double sigma,
     return w;
 }
 
+// Where a bin's value goes.  index() is the code of a bin kept in the draw queues (< 2^30), add_at() the accumulation.
 struct GlobalSink {
     float *S;
     int n_ticks;
-    __device__ __forceinline__ void add(int wire, int tick, float v) const
+    __device__ __forceinline__ uint32_t index(int wire, int tick) const
     {
-        atomicAdd(S + (size_t)wire * n_ticks + tick, v); // result unused -> RED.E.ADD.F32
+        return (uint32_t)wire * (uint32_t)n_ticks + (uint32_t)tick;
     }
+    __device__ __forceinline__ void add_at(uint32_t idx, float v) const
+    {
+        atomicAdd(S + idx, v); // result unused -> RED.E.ADD.F32
+    }
+    __device__ __forceinline__ void add(int wire, int tick, float v) const { add_at(index(wire, tick), v); }
 };
 
 struct TileSink {
     unsigned long long *acc; // shared memory, [kTileW][kTileT]
     int w0, k0;
-    __device__ __forceinline__ void add(int wire, int tick, float v) const
+    __device__ __forceinline__ uint32_t index(int wire, int tick) const
+    {
+        return (uint32_t)((wire - w0) * kTileT + (tick - k0));
+    }
+    __device__ __forceinline__ void add_at(uint32_t idx, float v) const
     {
         const long long q = __double2ll_rn((double)v * kFixScale);
-        atomicAdd(acc + (wire - w0) * kTileT + (tick - k0), (unsigned long long)q);
+        atomicAdd(acc + idx, (unsigned long long)q);
     }
+    __device__ __forceinline__ void add(int wire, int tick, float v) const { add_at(index(wire, tick), v); }
+};
+
+// the clip window of a batch: the grid, or one tile of it
+struct Clip {
+    int w_lo, w_hi, k_lo, k_hi;
 };
 
 // Rasters depo (t0, x0, st, sx, q) into the clip window [w_lo, w_hi) x [k_lo, k_hi) (already inside the grid).
@@ -230,9 +246,9 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane)
 }
 
 // draws `take` entries from the top of queue `cls` (lane < take) and adds them to S
-template <bool TOT>
-__device__ __forceinline__ void drain_queue(DrawQueues<TOT> &Q, int cls, int &count, bool everything,
-                                            float *__restrict__ S, int *__restrict__ totals, int lane)
+template <bool TOT, typename Sink>
+__device__ __forceinline__ void drain_queue(DrawQueues<TOT> &Q, int cls, int &count, bool everything, const Sink &sink,
+                                            int *__restrict__ totals, int lane)
 {
     while (count >= 32 || (everything && count > 0)) {
         const int take = min(32, count);
@@ -244,11 +260,166 @@ __device__ __forceinline__ void drain_queue(DrawQueues<TOT> &Q, int cls, int &co
             const double k = draw_classified(cls, N, Q.p[cls][e], Q.w[cls][e], (fb & kBinMirror) != 0);
             if (k != 0.0) {
                 const float v = (fb & kBinNegative) ? -(float)k : (float)k;
-                atomicAdd(S + (fb & kBinMask), v);
+                sink.add_at(fb & kBinMask, v);
                 if constexpr (TOT) atomicAdd(totals + Q.depo[cls][e], (int)v);
             }
         }
         __syncwarp();
+    }
+}
+
+// One batch of up to kBatchDepos depos, one per lane (lane l < count owns a depo, the others own none): extents clipped to
+// `clip`, edges, bins, draws.  Shared by the atomic kernel (clip = the grid, sink = S) and the tiled kernel (clip = a
+// tile, sink = the tile's fixed-point accumulators).  The call-wide index of the depo of lane `own` is dbase + own, or
+// dbase + (lane own's dl) when the batch comes from an index list (INDIRECT).
+template <bool FLUCT, bool TOT, bool INDIRECT, typename Sink>
+__device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const Sink &sink, float t0, float x0, float st,
+                                                  float sx, float q, bool valid, long long dbase, uint32_t dl,
+                                                  uint64_t id_base, uint64_t seed, double nsigma, bool normal_only,
+                                                  int *__restrict__ totals, BatchScratch<FLUCT> &sc,
+                                                  DrawQueues<TOT> *queues, int (&qcount)[kNumDrawQueues],
+                                                  unsigned long long &drawn, int lane)
+{
+    using T = typename std::conditional<FLUCT, double, float>::type;
+    auto depo_of = [&](int own) -> long long {
+        if constexpr (INDIRECT) return dbase + (long long)__shfl_sync(0xffffffffu, dl, own);
+        else return dbase + own;
+    };
+    const double T0 = t0, X0 = x0, ST = st, SX = sx;
+    Extent et{0, 0}, ex{0, 0};
+    if (valid) {
+        et = axis_extent(T0, ST, nsigma, clip.k_lo, clip.k_hi);
+        ex = axis_extent(X0, SX, nsigma, clip.w_lo, clip.w_hi);
+    }
+    const bool live = et.lo < et.hi && ex.lo < ex.hi;
+    const int nt = live ? et.hi - et.lo : 0, nx = live ? ex.hi - ex.lo : 0;
+    const bool big = nt + nx + 2 > kEdgeCap || (long long)nt * nx > (1 << 24);
+    const int ne = (live && !big) ? nt + nx + 2 : 0, nb = (live && !big) ? nt * nx : 0;
+    const int eincl = warp_incl_scan(ne, lane), bincl = warp_incl_scan(nb, lane);
+    __syncwarp();
+    sc.eoff[lane] = eincl - ne;
+    sc.boff[lane] = bincl - nb;
+    if (lane == 31) {
+        sc.eoff[32] = eincl;
+        sc.boff[32] = bincl;
+    }
+    __syncwarp();
+    const float Ntr = (float)floor(fabs((double)q) + 0.5); // exact: see DrawQueues::N
+    drawn += (unsigned long long)nb;
+
+    // patches too big for the scratch: the whole warp walks them one at a time
+    unsigned int big_mask = __ballot_sync(0xffffffffu, live && big);
+    while (big_mask) {
+        const int src = __ffs(big_mask) - 1;
+        big_mask &= big_mask - 1;
+        int tot = 0;
+        drawn += raster_depo<FLUCT>(__shfl_sync(0xffffffffu, t0, src), __shfl_sync(0xffffffffu, x0, src),
+                                    __shfl_sync(0xffffffffu, st, src), __shfl_sync(0xffffffffu, sx, src),
+                                    __shfl_sync(0xffffffffu, q, src), id_base + (uint64_t)depo_of(src), seed,
+                                    nsigma, g.n_ticks, clip.w_lo, clip.w_hi, clip.k_lo, clip.k_hi, sink, lane, &tot, normal_only);
+        if (totals != nullptr) {
+            tot = warp_sum(tot);
+            if (lane == 0 && tot != 0) atomicAdd(totals + depo_of(src), tot);
+        }
+    }
+
+    // sub-batches of consecutive depos whose edges fit the scratch (normally all 32 at once)
+    int d0 = 0;
+    while (d0 < 32) {
+        const int ebase = sc.eoff[d0];
+        const unsigned int fits = __ballot_sync(0xffffffffu, lane >= d0 && eincl - ebase <= kEdgeCap);
+        const int d1 = d0 + __popc(fits); // eincl is monotone: the fitting lanes are d0 .. d1-1, at least one
+        const int etot = sc.eoff[d1] - ebase, bbase = sc.boff[d0], btot = sc.boff[d1] - bbase;
+        // ---- edges: erf((edge - centre) / (sqrt2 sigma)), flat over the sub-batch -------------------------------
+        for (int e0 = 0; e0 < etot; e0 += 32) {
+            const int e = e0 + lane;
+            const bool act = e < etot;
+            const int own = owner_of(sc.eoff, ebase + (act ? e : 0));
+            const int le = ebase + e - sc.eoff[own];
+            const int nto = __shfl_sync(0xffffffffu, nt, own);
+            const bool on_t = le <= nto;
+            const int lo_t = __shfl_sync(0xffffffffu, et.lo, own), lo_x = __shfl_sync(0xffffffffu, ex.lo, own);
+            const float ct = __shfl_sync(0xffffffffu, t0, own), cx = __shfl_sync(0xffffffffu, x0, own);
+            const float sgt = __shfl_sync(0xffffffffu, st, own), sgx = __shfl_sync(0xffffffffu, sx, own);
+            const double centre = (double)(on_t ? ct : cx), sigma = (double)(on_t ? sgt : sgx);
+            const int coord = on_t ? lo_t + le : lo_x + (le - nto - 1);
+            T E;
+            if (sigma < 1e-6) { // all weight in bin floor(centre) (A4): a step from -1 to +1 after that bin's low edge
+                E = ((double)coord <= floor(centre)) ? T(-1) : T(1);
+            } else {
+                const double dd = __dsub_rn((double)coord, centre);
+                if constexpr (FLUCT) {
+                    E = erf_from_table(g_erf_tab, fast_div(dd, 1.4142135623730951 * sigma));
+                } else {
+                    const float inv = 1.0f / (1.41421356f * (float)sigma);
+                    E = erff((float)dd * inv);
+                }
+            }
+            if (act) sc.edge[e] = E;
+        }
+        __syncwarp();
+        // ---- bins: p_ij = wt_i wx_j, flat over the sub-batch ----------------------------------------------------
+        for (int b0 = 0; b0 < btot; b0 += 32) {
+            const int b = b0 + lane;
+            const bool act = b < btot;
+            const int own = owner_of(sc.boff, bbase + (act ? b : 0));
+            const int l = bbase + b - sc.boff[own];
+            const int nto = __shfl_sync(0xffffffffu, nt, own);
+            const int lo_t = __shfl_sync(0xffffffffu, et.lo, own), lo_x = __shfl_sync(0xffffffffu, ex.lo, own);
+            // wire index in the patch, l / nto: (l + 1/2) / nto is at least 1/(2 nto) away from an integer, far more
+            // than the rounding of the product below for l < 2^22 (a flat-path patch has < 2^14 bins)
+            const int j = act ? __float2int_rz(((float)l + 0.5f) * __frcp_rn((float)max(nto, 1))) : 0;
+            const int ii = act ? l - j * nto : 0;                              // tick index in the patch
+            const T *E = sc.edge + (sc.eoff[own] - ebase);
+            const T wt = T(0.5) * (E[ii + 1] - E[ii]);
+            const T wx = T(0.5) * (E[nto + 1 + j + 1] - E[nto + 1 + j]);
+            const int wire = lo_x + j, tick = lo_t + ii;
+            if constexpr (FLUCT) {
+                const double Nn = (double)__shfl_sync(0xffffffffu, Ntr, own);
+                const float qq = __shfl_sync(0xffffffffu, q, own);
+                double p = __dmul_rn(wt, wx);
+                const uint64_t gbin = (uint64_t)wire * (uint64_t)g.n_ticks + (uint64_t)tick;
+                const long long dio = depo_of(own);
+                const uint64_t id = id_base + (uint64_t)dio;
+                uint32_t w = pick_word(fluct_words(seed, id, gbin >> 2), (uint32_t)gbin & 3u);
+                bool mirror = false;
+                int cls = act ? classify_draw(Nn, p, w, mirror, normal_only) : (int)kDrawZero;
+                const uint32_t fb = sink.index(wire, tick) | (mirror ? kBinMirror : 0u) | (qq < 0.0f ? kBinNegative : 0u);
+                if (cls == kDrawAll) { // p >= 1: every electron lands here
+                    const float v = (qq < 0.0f) ? -(float)Nn : (float)Nn;
+                    if (act) sink.add(wire, tick, v);
+                    if constexpr (TOT) atomicAdd(totals + dio, (int)v);
+                }
+                DrawQueues<TOT> &Q = *queues;
+                // one slot per bin in the queue of its class: position = queue fill + rank among the lanes of the
+                // same class (ballots), then a single block of stores for all classes
+                unsigned int mine = 0;
+                int base = 0;
+#pragma unroll
+                for (int c = 0; c < kNumDrawQueues; ++c) {
+                    const unsigned int m = __ballot_sync(0xffffffffu, cls == c);
+                    mine = (cls == c) ? m : mine;
+                    base = (cls == c) ? qcount[c] : base;
+                    qcount[c] += __popc(m);
+                }
+                if (cls >= 0) {
+                    const int pos = base + __popc(mine & ((1u << lane) - 1u));
+                    Q.p[cls][pos] = p;
+                    Q.N[cls][pos] = (float)Nn;
+                    Q.w[cls][pos] = w;
+                    Q.bin[cls][pos] = fb;
+                    if constexpr (TOT) Q.depo[cls][pos] = (uint32_t)dio;
+                }
+                __syncwarp();
+#pragma unroll
+                for (int c = 0; c < kNumDrawQueues; ++c) drain_queue(Q, c, qcount[c], false, sink, totals, lane);
+            } else {
+                const float qq = __shfl_sync(0xffffffffu, q, own);
+                if (act) sink.add(wire, tick, qq * (wt * wx));
+            }
+        }
+        __syncwarp();
+        d0 = d1;
     }
 }
 
@@ -264,6 +435,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     BatchScratch<FLUCT> &sc = sm.scratch[wid];
     const GlobalSink sink{S, g.n_ticks};
+    const Clip clip{0, g.n_wires, 0, g.n_ticks};
     // guided batches: kBatchDepos depos at a time, then kTailDepos at a time for the last kTailPerWarp depos per warp of the
     // grid, so that the warps run out of work within a short batch of one another (a batch of 8 lasts ~20 us on
     // configs[1], where a warp gets only 3-4 of them)
@@ -295,145 +467,16 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
             valid = depo_valid(t0, x0, st, sx, q);
             skipped += !valid;
         }
-        const double T0 = t0, X0 = x0, ST = st, SX = sx;
-        Extent et{0, 0}, ex{0, 0};
-        if (valid) {
-            et = axis_extent(T0, ST, nsigma, 0, g.n_ticks);
-            ex = axis_extent(X0, SX, nsigma, 0, g.n_wires);
-        }
-        const bool live = et.lo < et.hi && ex.lo < ex.hi;
-        const int nt = live ? et.hi - et.lo : 0, nx = live ? ex.hi - ex.lo : 0;
-        const bool big = nt + nx + 2 > kEdgeCap || (long long)nt * nx > (1 << 24);
-        const int ne = (live && !big) ? nt + nx + 2 : 0, nb = (live && !big) ? nt * nx : 0;
-        const int eincl = warp_incl_scan(ne, lane), bincl = warp_incl_scan(nb, lane);
-        __syncwarp();
-        sc.eoff[lane] = eincl - ne;
-        sc.boff[lane] = bincl - nb;
-        if (lane == 31) {
-            sc.eoff[32] = eincl;
-            sc.boff[32] = bincl;
-        }
-        __syncwarp();
-        const float Ntr = (float)floor(fabs((double)q) + 0.5); // exact: see DrawQueues::N
-        drawn += (unsigned long long)nb;
-
-        // patches too big for the scratch: the whole warp walks them one at a time
-        unsigned int big_mask = __ballot_sync(0xffffffffu, live && big);
-        while (big_mask) {
-            const int src = __ffs(big_mask) - 1;
-            big_mask &= big_mask - 1;
-            int tot = 0;
-            drawn += raster_depo<FLUCT>(__shfl_sync(0xffffffffu, t0, src), __shfl_sync(0xffffffffu, x0, src),
-                                        __shfl_sync(0xffffffffu, st, src), __shfl_sync(0xffffffffu, sx, src),
-                                        __shfl_sync(0xffffffffu, q, src), id_base + (uint64_t)(first + src), seed,
-                                        nsigma, g.n_ticks, 0, g.n_wires, 0, g.n_ticks, sink, lane, &tot, normal_only);
-            if (totals != nullptr) {
-                tot = warp_sum(tot);
-                if (lane == 0 && tot != 0) atomicAdd(totals + first + src, tot);
-            }
-        }
-
-        // sub-batches of consecutive depos whose edges fit the scratch (normally all 32 at once)
-        int d0 = 0;
-        while (d0 < 32) {
-            const int ebase = sc.eoff[d0];
-            const unsigned int fits = __ballot_sync(0xffffffffu, lane >= d0 && eincl - ebase <= kEdgeCap);
-            const int d1 = d0 + __popc(fits); // eincl is monotone: the fitting lanes are d0 .. d1-1, at least one
-            const int etot = sc.eoff[d1] - ebase, bbase = sc.boff[d0], btot = sc.boff[d1] - bbase;
-            // ---- edges: erf((edge - centre) / (sqrt2 sigma)), flat over the sub-batch -------------------------------
-            for (int e0 = 0; e0 < etot; e0 += 32) {
-                const int e = e0 + lane;
-                const bool act = e < etot;
-                const int own = owner_of(sc.eoff, ebase + (act ? e : 0));
-                const int le = ebase + e - sc.eoff[own];
-                const int nto = __shfl_sync(0xffffffffu, nt, own);
-                const bool on_t = le <= nto;
-                const int lo_t = __shfl_sync(0xffffffffu, et.lo, own), lo_x = __shfl_sync(0xffffffffu, ex.lo, own);
-                const float ct = __shfl_sync(0xffffffffu, t0, own), cx = __shfl_sync(0xffffffffu, x0, own);
-                const float sgt = __shfl_sync(0xffffffffu, st, own), sgx = __shfl_sync(0xffffffffu, sx, own);
-                const double centre = (double)(on_t ? ct : cx), sigma = (double)(on_t ? sgt : sgx);
-                const int coord = on_t ? lo_t + le : lo_x + (le - nto - 1);
-                T E;
-                if (sigma < 1e-6) { // all weight in bin floor(centre) (A4): a step from -1 to +1 after that bin's low edge
-                    E = ((double)coord <= floor(centre)) ? T(-1) : T(1);
-                } else {
-                    const double dd = __dsub_rn((double)coord, centre);
-                    if constexpr (FLUCT) {
-                        E = erf_from_table(g_erf_tab, fast_div(dd, 1.4142135623730951 * sigma));
-                    } else {
-                        const float inv = 1.0f / (1.41421356f * (float)sigma);
-                        E = erff((float)dd * inv);
-                    }
-                }
-                if (act) sc.edge[e] = E;
-            }
-            __syncwarp();
-            // ---- bins: p_ij = wt_i wx_j, flat over the sub-batch ----------------------------------------------------
-            for (int b0 = 0; b0 < btot; b0 += 32) {
-                const int b = b0 + lane;
-                const bool act = b < btot;
-                const int own = owner_of(sc.boff, bbase + (act ? b : 0));
-                const int l = bbase + b - sc.boff[own];
-                const int nto = __shfl_sync(0xffffffffu, nt, own);
-                const int lo_t = __shfl_sync(0xffffffffu, et.lo, own), lo_x = __shfl_sync(0xffffffffu, ex.lo, own);
-                // wire index in the patch, l / nto: (l + 1/2) / nto is at least 1/(2 nto) away from an integer, far more
-                // than the rounding of the product below for l < 2^22 (a flat-path patch has < 2^14 bins)
-                const int j = act ? __float2int_rz(((float)l + 0.5f) * __frcp_rn((float)max(nto, 1))) : 0;
-                const int ii = act ? l - j * nto : 0;                              // tick index in the patch
-                const T *E = sc.edge + (sc.eoff[own] - ebase);
-                const T wt = T(0.5) * (E[ii + 1] - E[ii]);
-                const T wx = T(0.5) * (E[nto + 1 + j + 1] - E[nto + 1 + j]);
-                const int wire = lo_x + j, tick = lo_t + ii;
-                if constexpr (FLUCT) {
-                    const double Nn = (double)__shfl_sync(0xffffffffu, Ntr, own);
-                    const float qq = __shfl_sync(0xffffffffu, q, own);
-                    double p = __dmul_rn(wt, wx);
-                    const uint64_t gbin = (uint64_t)wire * (uint64_t)g.n_ticks + (uint64_t)tick;
-                    const uint64_t id = id_base + (uint64_t)(first + own);
-                    uint32_t w = pick_word(fluct_words(seed, id, gbin >> 2), (uint32_t)gbin & 3u);
-                    bool mirror = false;
-                    int cls = act ? classify_draw(Nn, p, w, mirror, normal_only) : (int)kDrawZero;
-                    const uint32_t fb = (uint32_t)gbin | (mirror ? kBinMirror : 0u) | (qq < 0.0f ? kBinNegative : 0u);
-                    if (cls == kDrawAll) { // p >= 1: every electron lands here
-                        const float v = (qq < 0.0f) ? -(float)Nn : (float)Nn;
-                        atomicAdd(S + gbin, v);
-                        if constexpr (TOT) atomicAdd(totals + first + own, (int)v);
-                    }
-                    DrawQueues<TOT> &Q = sm.queues[wid];
-                    // one slot per bin in the queue of its class: position = queue fill + rank among the lanes of the
-                    // same class (ballots), then a single block of stores for all classes
-                    unsigned int mine = 0;
-                    int base = 0;
-#pragma unroll
-                    for (int c = 0; c < kNumDrawQueues; ++c) {
-                        const unsigned int m = __ballot_sync(0xffffffffu, cls == c);
-                        mine = (cls == c) ? m : mine;
-                        base = (cls == c) ? qcount[c] : base;
-                        qcount[c] += __popc(m);
-                    }
-                    if (cls >= 0) {
-                        const int pos = base + __popc(mine & ((1u << lane) - 1u));
-                        Q.p[cls][pos] = p;
-                        Q.N[cls][pos] = (float)Nn;
-                        Q.w[cls][pos] = w;
-                        Q.bin[cls][pos] = fb;
-                        if constexpr (TOT) Q.depo[cls][pos] = (uint32_t)(first + own);
-                    }
-                    __syncwarp();
-#pragma unroll
-                    for (int c = 0; c < kNumDrawQueues; ++c) drain_queue(Q, c, qcount[c], false, S, totals, lane);
-                } else {
-                    const float qq = __shfl_sync(0xffffffffu, q, own);
-                    if (act) sink.add(wire, tick, qq * (wt * wx));
-                }
-            }
-            __syncwarp();
-            d0 = d1;
-        }
+        if constexpr (FLUCT)
+            raster_batch_body<FLUCT, TOT, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, id_base, seed, nsigma,
+                                                 normal_only, totals, sc, &sm.queues[wid], qcount, drawn, lane);
+        else
+            raster_batch_body<FLUCT, TOT, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, id_base, seed, nsigma,
+                                                 normal_only, totals, sc, (DrawQueues<TOT> *)nullptr, qcount, drawn, lane);
     }
     if constexpr (FLUCT) {
 #pragma unroll
-        for (int c = 0; c < kNumDrawQueues; ++c) drain_queue(sm.queues[wid], c, qcount[c], true, S, totals, lane);
+        for (int c = 0; c < kNumDrawQueues; ++c) drain_queue(sm.queues[wid], c, qcount[c], true, sink, totals, lane);
     }
     drawn = warp_sum(drawn);
     skipped = warp_sum(skipped);
