@@ -582,41 +582,70 @@ __global__ void tile_fill_kernel(GridDims g, DepoArrays d, long long n, double n
         }
 }
 
-template <bool FLUCT>
-__global__ void __launch_bounds__(256) tile_accumulate_kernel(GridDims g, DepoArrays d, uint64_t id_base, uint64_t seed,
-                                                              double nsigma, TileScratch ts, float *__restrict__ S,
-                                                              int *__restrict__ totals, Counters *counters, bool normal_only)
+// One CTA per tile.  Its warps take the tile's depos (the index list built by count / scan / fill) eight at a time and
+// run the same flat-list batch body as the atomic kernel, clipped to the tile and accumulating into the tile's
+// fixed-point shared-memory accumulators; the tile is added to S once at the end.
+constexpr int kTileWarps = 8;
+template <bool FLUCT, bool TOT>
+struct TileSmem {
+    unsigned long long acc[kTileW * kTileT];
+    BatchScratch<FLUCT> scratch[kTileWarps];
+};
+template <bool TOT>
+struct TileSmem<true, TOT> {
+    unsigned long long acc[kTileW * kTileT];
+    BatchScratch<true> scratch[kTileWarps];
+    DrawQueues<TOT> queues[kTileWarps];
+};
+
+template <bool FLUCT, bool TOT>
+__global__ void __launch_bounds__(kTileWarps * 32, 2) tile_accumulate_kernel(GridDims g, DepoArrays d, uint64_t id_base,
+                                                                          uint64_t seed, double nsigma, TileScratch ts,
+                                                                          float *__restrict__ S, int *__restrict__ totals,
+                                                                          Counters *counters, bool normal_only)
 {
-    __shared__ unsigned long long acc[kTileW * kTileT];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    TileSmem<FLUCT, TOT> &sm = *reinterpret_cast<TileSmem<FLUCT, TOT> *>(smem_raw);
     const int tile = blockIdx.x;
     const unsigned int beg = ts.tile_count[tile], end = ts.tile_count[tile + 1];
     if (beg == end) return; // uniform over the CTA
     const int tw = tile / ts.tiles_t, tt = tile % ts.tiles_t;
     const int w0 = tw * kTileW, k0 = tt * kTileT;
     const int w1 = min(w0 + kTileW, g.n_wires), k1 = min(k0 + kTileT, g.n_ticks);
-    for (int i = threadIdx.x; i < kTileW * kTileT; i += blockDim.x) acc[i] = 0ull;
+    for (int i = threadIdx.x; i < kTileW * kTileT; i += blockDim.x) sm.acc[i] = 0ull;
     __syncthreads();
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
-    const TileSink sink{acc, w0, k0};
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const TileSink sink{sm.acc, w0, k0};
+    const Clip clip{w0, w1, k0, k1};
+    BatchScratch<FLUCT> &sc = sm.scratch[wid];
     unsigned long long drawn = 0;
-    for (unsigned int e = beg + wid; e < end; e += n_warps) {
-        const unsigned int i = ts.entries[e];
-        const float t0 = __ldg(d.t0 + i), x0 = __ldg(d.x0 + i), st = __ldg(d.sigma_t + i), sx = __ldg(d.sigma_x + i),
-                    q = __ldg(d.q + i);
-        int tot = 0;
-        drawn += raster_depo<FLUCT>(t0, x0, st, sx, q, id_base + (uint64_t)i, seed, nsigma, g.n_ticks, w0, w1, k0, k1,
-                                    sink, lane, &tot, normal_only);
-        if (totals != nullptr) {
-            tot = warp_sum(tot);
-            if (lane == 0 && tot != 0) atomicAdd(totals + i, tot);
+    int qcount[kNumDrawQueues] = {};
+    for (unsigned int e0 = beg + (unsigned int)wid * kBatchDepos; e0 < end; e0 += kTileWarps * kBatchDepos) {
+        float t0 = 0.f, x0 = 0.f, st = 0.f, sx = 0.f, q = 0.f;
+        unsigned int i = 0;
+        bool valid = false;
+        if (lane < kBatchDepos && e0 + lane < end) {
+            i = ts.entries[e0 + lane];
+            t0 = __ldg(d.t0 + i), x0 = __ldg(d.x0 + i), st = __ldg(d.sigma_t + i), sx = __ldg(d.sigma_x + i), q = __ldg(d.q + i);
+            valid = depo_valid(t0, x0, st, sx, q); // listed depos are valid; kept for symmetry with the atomic kernel
         }
+        if constexpr (FLUCT)
+            raster_batch_body<FLUCT, TOT, true>(g, clip, sink, t0, x0, st, sx, q, valid, 0ll, i, id_base, seed, nsigma,
+                                                normal_only, totals, sc, &sm.queues[wid], qcount, drawn, lane);
+        else
+            raster_batch_body<FLUCT, TOT, true>(g, clip, sink, t0, x0, st, sx, q, valid, 0ll, i, id_base, seed, nsigma,
+                                                normal_only, totals, sc, (DrawQueues<TOT> *)nullptr, qcount, drawn, lane);
+    }
+    if constexpr (FLUCT) {
+#pragma unroll
+        for (int c = 0; c < kNumDrawQueues; ++c) drain_queue(sm.queues[wid], c, qcount[c], true, sink, totals, lane);
     }
     drawn = warp_sum(drawn);
     if (lane == 0 && drawn) atomicAdd(&counters->bins_drawn, drawn);
     __syncthreads();
     for (int i = threadIdx.x; i < kTileW * kTileT; i += blockDim.x) {
         const int w = w0 + i / kTileT, k = k0 + i % kTileT;
-        const long long q = (long long)acc[i];
+        const long long q = (long long)sm.acc[i];
         if (q != 0 && w < w1 && k < k1) {
             float *p = S + (size_t)w * g.n_ticks + k;
             *p = *p + (float)((double)q * (1.0 / kFixScale));
@@ -661,8 +690,17 @@ cudaError_t raster_configure(cudaStream_t st)
     err = cudaFuncSetAttribute(raster_batch_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                (int)sizeof(BatchSmem<true, false>));
     if (err != cudaSuccess) return err;
-    return cudaFuncSetAttribute(raster_batch_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)sizeof(BatchSmem<false, false>));
+    err = cudaFuncSetAttribute(raster_batch_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (int)sizeof(BatchSmem<false, false>));
+    if (err != cudaSuccess) return err;
+    err = cudaFuncSetAttribute(tile_accumulate_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (int)sizeof(TileSmem<true, true>));
+    if (err != cudaSuccess) return err;
+    err = cudaFuncSetAttribute(tile_accumulate_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (int)sizeof(TileSmem<true, false>));
+    if (err != cudaSuccess) return err;
+    return cudaFuncSetAttribute(tile_accumulate_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)sizeof(TileSmem<false, false>));
 }
 
 template <bool FLUCT, bool TOT>
@@ -715,18 +753,27 @@ cudaError_t launch_tile_fill(GridDims g, DepoArrays d, long long n, double nsigm
     return cudaGetLastError();
 }
 
+template <bool FLUCT, bool TOT>
+static cudaError_t launch_tile_accumulate_t(GridDims g, DepoArrays d, uint64_t id_base, uint64_t seed, double nsigma,
+                                            TileScratch ts, float *S, int *depo_totals, Counters *counters, bool normal_only,
+                                            cudaStream_t st)
+{
+    const int n_tiles = ts.tiles_w * ts.tiles_t;
+    tile_accumulate_kernel<FLUCT, TOT><<<n_tiles, kTileWarps * 32, sizeof(TileSmem<FLUCT, TOT>), st>>>(
+        g, d, id_base, seed, nsigma, ts, S, depo_totals, counters, normal_only);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_tile_accumulate(GridDims g, DepoArrays d, uint64_t id_base, uint64_t seed, int fluctuate,
                                    double nsigma, TileScratch ts, float *S, int *depo_totals, Counters *counters,
                                    cudaStream_t st)
 {
-    const int n_tiles = ts.tiles_w * ts.tiles_t;
-    if (fluctuate)
-        tile_accumulate_kernel<true><<<n_tiles, 256, 0, st>>>(g, d, id_base, seed, nsigma, ts, S, depo_totals, counters,
-                                                              fluctuate == 2);
-    else
-        tile_accumulate_kernel<false><<<n_tiles, 256, 0, st>>>(g, d, id_base, seed, nsigma, ts, S, depo_totals, counters,
-                                                               false);
-    return cudaGetLastError();
+    if (!fluctuate)
+        return launch_tile_accumulate_t<false, false>(g, d, id_base, seed, nsigma, ts, S, nullptr, counters, false, st);
+    if (depo_totals)
+        return launch_tile_accumulate_t<true, true>(g, d, id_base, seed, nsigma, ts, S, depo_totals, counters,
+                                                    fluctuate == 2, st);
+    return launch_tile_accumulate_t<true, false>(g, d, id_base, seed, nsigma, ts, S, nullptr, counters, fluctuate == 2, st);
 }
 
 cudaError_t launch_count_invalid(DepoArrays d, long long n, Counters *counters, cudaStream_t st)
