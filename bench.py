@@ -233,6 +233,7 @@ def run_ours(args):
     e2e_value, e2e_slowest = replicas.whole_job_throughput(n_depos * e2e_steps, e2e_local, dev)
     h2d, d2h = 5 * 4 * n_depos, 4 * pl["n_wires"] * pl["n_ticks"]
     # the synchronous call, one plane-event at a time (latency of the whole host round trip)
+    plan.simulate_host(host, host_M[0], seed=cfg["fluct_seed"], fluctuate=fluct)  # allocates the plan's staging arrays
     t0 = time.perf_counter()
     for _ in range(min(e2e_steps, 20)):
         plan.simulate_host(host, host_M[0], seed=cfg["fluct_seed"], fluctuate=fluct)
