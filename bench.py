@@ -128,7 +128,7 @@ def run_ours(args):
     replicas.init("nccl")
     B.lib()  # fails loudly here if libwcsim.so cannot be built or loaded
 
-    cfg = synth.config(args.config)
+    cfg = synth.config(args.config, sigma_scale=args.sigma_scale) if args.sigma_scale != 1.0 else synth.config(args.config)
     pl = cfg["planes"][0]
     n_depos = int(pl["depos"]["t0"].shape[0])
     fluct = bool(cfg["fluctuate"]) and not args.no_fluct
@@ -303,7 +303,9 @@ def run_ours(args):
         "dtype": "f32" if not fluct else "f32 (f64 fluctuation weights and sampler)", "data": "synthetic",
         "config": {"workload": cfg["name"] + (", fluctuation off" if not fluct else ", normal-approximation fluctuation" if fluct == 2
                                              else ", fluctuation on") +
-                               (", noise fused (plane 0 timed)" if noisy else ""),
+                               (", noise fused (plane 0 timed)" if noisy else "") +
+                               (", LARGE-PATCH VARIANT sigma x %g (not one of the five configs)" % args.sigma_scale
+                                if args.sigma_scale != 1.0 else ""),
                    "grid": [pl["n_wires"], pl["n_ticks"]], "pad": [pl["pad_w"], pl["pad_t"]],
                    "response": list(pl["response"].shape), "depos": n_depos, "scatter": args.scatter,
                    "wire_axis": "direct" if direct else "fft",
@@ -474,6 +476,8 @@ def main():
     ap.add_argument("--no-fluct", action="store_true")
     ap.add_argument("--fluct", default="binomial", choices=["binomial", "normal"],
                     help="sampler of the fluctuated raster: reading A6 (headline) or the Kokkos port's normal approximation (A21)")
+    ap.add_argument("--sigma-scale", type=float, default=1.0,
+                    help="labelled large-patch variant of configs[1]/[2] (reading A19): widths multiplied by this factor")
     ap.add_argument("--streams", type=int, default=3, help="plane-events in flight for the extra `concurrent` figure")
     ap.add_argument("--e2e-steps", type=int, default=200)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
