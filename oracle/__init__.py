@@ -151,6 +151,24 @@ def patch_axes(t0, x0, sigma_t, sigma_x, nsigma=3.0, max_bins=4096):
     return it0.value, ix0.value, wt[: it1.value - it0.value].copy(), wx[: ix1.value - ix0.value].copy()
 
 
+def drift(x, y, z, t, q, *, v_drift, D_L, D_T, tick, t_origin=0.0, lifetime=0.0, x_plane=0.0, cos_theta=1.0,
+          sin_theta=0.0, pitch_origin=0.0, pitch=1.0):
+    """Reading A22: electron groups (cm, us, electrons) -> depos of one plane (ticks, pitches)."""
+    x, y, z, t, q = (_f32(a) for a in (x, y, z, t, q))
+    n = x.shape[0]
+    out = {k: np.empty(n, dtype=np.float32) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")}
+    f32p = C.POINTER(C.c_float)
+    L = lib()
+    L.wco_drift.argtypes = [f32p] * 5 + [C.c_int64] + [C.c_double] * 11 + [f32p] * 5
+    L.wco_drift.restype = C.c_int
+    rc = L.wco_drift(*[_p(a, C.c_float) for a in (x, y, z, t, q)], n, float(v_drift), float(D_L), float(D_T), float(tick),
+                     float(t_origin), float(lifetime), float(x_plane), float(cos_theta), float(sin_theta),
+                     float(pitch_origin), float(pitch), *[_p(out[k], C.c_float) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")])
+    if rc != 0:
+        raise ValueError("wco_drift rc=%d" % rc)
+    return out
+
+
 def _fluct_mode(fluctuate) -> int:
     """False/0: off, True/1: binomial (A6), 2 or "normal": normal approximation (A21)."""
     if fluctuate == "normal":

@@ -24,6 +24,7 @@
  *   philox ................ published known-answer vectors (tests/golden/)
  *   norm_ppf .............. published normal quantiles (tests/golden/), scipy ndtri
  *   binomial .............. exact binomial CDF break points, mirror identity, moments
+ *   drift ................. the widths BASELINE.json configs[1] states for td = 2.25 ms, closed forms
  *   normal_draw ........... its formula restated with scipy's ndtri, moments, the paper's
  *                           0.01 % agreement with the binomial waveforms
  *   noise ................. Parseval closed form, spectrum round trip, direct vs FFT
@@ -242,6 +243,41 @@ double wco_normal_draw(double N, double p, uint32_t w)
     if (k < 0.0) k = 0.0;
     if (k > N) k = N;
     return k;
+}
+
+/* ------------------------------------------------------------------------- */
+/* Drift (upstream of Raster).  PAPER.md:54: "After simulating   */
+/* the diffusion process along the drifting, each ionization electron group is */
+/* diffused into a 2D distribution along the drifting and wire pitch           */
+/* directions."  Reading A22, with BASELINE.json configs[1]'s width formulas:   */
+/*   td      = (x - x_plane) / v_drift                     [us]; td < 0 -> NaN  */
+/*   t0      = (t + td - t_origin) / tick                   [ticks]             */
+/*   x0      = (y cos(theta) + z sin(theta) - pitch_origin) / pitch  [pitches]  */
+/*   sigma_t = sqrt(2 D_L td) / v_drift / tick,  sigma_x = sqrt(2 D_T td)/pitch */
+/*   Q       = q exp(-td / lifetime)   (lifetime <= 0: no attenuation)          */
+/* Units: cm, us, D in cm^2/s (so 2 D td carries a factor 1e-6).  Everything    */
+/* in fp64, results rounded once to fp32.  A group behind the plane (td < 0)    */
+/* gets NaN in all five fields, which the raster skips and counts.             */
+/* ------------------------------------------------------------------------- */
+int wco_drift(const float *x, const float *y, const float *z, const float *t, const float *q, int64_t n,
+              double v_drift, double D_L, double D_T, double tick, double t_origin, double lifetime,
+              double x_plane, double cos_theta, double sin_theta, double pitch_origin, double pitch,
+              float *t0, float *x0, float *sigma_t, float *sigma_x, float *Q)
+{
+    if (n < 0 || !(v_drift > 0.0) || !(tick > 0.0) || !(pitch > 0.0) || D_L < 0.0 || D_T < 0.0) return -1;
+    for (int64_t i = 0; i < n; ++i) {
+        double td = ((double)x[i] - x_plane) / v_drift;
+        if (!(td >= 0.0)) {
+            t0[i] = x0[i] = sigma_t[i] = sigma_x[i] = Q[i] = (float)NAN;
+            continue;
+        }
+        t0[i] = (float)((((double)t[i] + td) - t_origin) / tick);
+        x0[i] = (float)((((double)y[i] * cos_theta + (double)z[i] * sin_theta) - pitch_origin) / pitch);
+        sigma_t[i] = (float)((sqrt((2.0 * D_L * 1e-6) * td) / v_drift) / tick);
+        sigma_x[i] = (float)(sqrt((2.0 * D_T * 1e-6) * td) / pitch);
+        Q[i] = (float)((lifetime > 0.0) ? (double)q[i] * exp(-td / lifetime) : (double)q[i]);
+    }
+    return 0;
 }
 
 /* ------------------------------------------------------------------------- */
