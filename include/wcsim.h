@@ -180,6 +180,32 @@ int wcsim_simulate_host_async(wcsim_plan *plan, const float *host_t0, const floa
                         const float *host_sigma_x, const float *host_q, long long n, unsigned long long seed,
                         int fluctuate, int noise, unsigned long long noise_seed, float *host_M);
 
+/*
+ * Drift: the step upstream of the Raster ("After simulating the diffusion process along the drifting, each
+ * ionization electron group is diffused into a 2D distribution along the drifting and wire pitch directions"; reading
+ * A22).  One pass over n electron groups writes the depo arrays of n_planes planes (1..4):
+ *   td = (x - x_plane)/v_drift;  t0 = (t + td - t_origin)/tick;  x0 = (y cos_theta + z sin_theta - pitch_origin)/pitch;
+ *   sigma_t = sqrt(2 D_L td)/v_drift/tick;  sigma_x = sqrt(2 D_T td)/pitch;  q_out = q exp(-td/lifetime)
+ * computed in fp64 and rounded once to fp32.  Units: cm and us, D_L and D_T in cm^2/s, q in electrons; lifetime <= 0
+ * means no attenuation.  A group behind a plane (td < 0) gets NaN in that plane's five fields; wcsim_raster_scatter
+ * skips and counts such depos.  No plan is involved.
+ *   dev_x .. dev_q : DEVICE, n floats each, read.
+ *   planes         : HOST array of n_planes geometry records (read during the call).
+ *   out            : HOST array of n_planes wcsim_depos whose five DEVICE pointers (n floats each, caller-owned) are
+ *                    written; the const in wcsim_depos is cast away for these.
+ * Errors: WCSIM_EINVAL (NULL, n < 0, n_planes outside 1..4, non-positive v_drift / tick / pitch, negative D),
+ * WCSIM_ECUDA.  Asynchronous on cuda_stream.
+ */
+typedef struct {
+    double v_drift, D_L, D_T, tick, t_origin, lifetime;
+} wcsim_drift_params;
+typedef struct {
+    double x_plane, cos_theta, sin_theta, pitch_origin, pitch;
+} wcsim_plane_geom;
+int wcsim_drift(const float *dev_x, const float *dev_y, const float *dev_z, const float *dev_t, const float *dev_q,
+                long long n, const wcsim_drift_params *params, const wcsim_plane_geom *planes, int n_planes,
+                const wcsim_depos *out, void *cuda_stream);
+
 /* Test/diagnostic hooks: exact pieces of the path, exposed so that parity can be checked piecewise. */
 /* out[4] (DEVICE, 4*n uint32) = Philox4x32-10(ctr = dev_ctr[4*i..], key = dev_key[2*i..]) for i < n */
 int wcsim_debug_philox(const unsigned int *dev_ctr, const unsigned int *dev_key, unsigned int *dev_out, long long n,

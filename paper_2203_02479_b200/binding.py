@@ -23,7 +23,7 @@ SYMBOLS = [
     "wcsim_plan_destroy", "wcsim_clear", "wcsim_clear_output", "wcsim_sync", "wcsim_set_scatter_mode", "wcsim_set_wire_mode",
     "wcsim_charge_ptr", "wcsim_output_ptr", "wcsim_get_dims", "wcsim_get_stats", "wcsim_reset_stats",
     "wcsim_simulate_host", "wcsim_set_profiling", "wcsim_get_stage_times", "wcsim_get_launch_count",
-    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf", "wcsim_simulate_host_async", "wcsim_debug_normal_draw",
+    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf", "wcsim_simulate_host_async", "wcsim_debug_normal_draw", "wcsim_drift",
     "wcsim_strerror", "wcsim_last_cuda_error", "wcsim_version",
 ]
 
@@ -34,6 +34,14 @@ class wcsim_pad(C.Structure):
 
 class wcsim_depos(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")]
+
+
+class wcsim_drift_params(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("v_drift", "D_L", "D_T", "tick", "t_origin", "lifetime")]
+
+
+class wcsim_plane_geom(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("x_plane", "cos_theta", "sin_theta", "pitch_origin", "pitch")]
 
 
 class wcsim_stats(C.Structure):
@@ -85,6 +93,8 @@ def lib():
         L.wcsim_debug_normal_draw.argtypes = [vp, vp, vp, vp, ll, vp]
         L.wcsim_debug_response_spectrum.argtypes = [vp, vp]
         L.wcsim_debug_erf.argtypes = [vp, vp, ll]
+        L.wcsim_drift.argtypes = [vp, vp, vp, vp, vp, ll, C.POINTER(wcsim_drift_params), C.POINTER(wcsim_plane_geom), i,
+                                  C.POINTER(wcsim_depos), vp]
         L.wcsim_strerror.argtypes = [i]
         L.wcsim_strerror.restype = C.c_char_p
         L.wcsim_last_cuda_error.argtypes = []
@@ -303,6 +313,21 @@ def wcsim_debug_philox(dev_ctr, dev_key, dev_out, n, stream=None):
 def wcsim_debug_binomial(dev_N, dev_p, dev_w, dev_k, n, stream=None):
     _check(lib().wcsim_debug_binomial(_dev_ptr(dev_N), _dev_ptr(dev_p), _dev_ptr(dev_w), _dev_ptr(dev_k), int(n),
                                       _stream_ptr(stream)), "wcsim_debug_binomial")
+
+
+def wcsim_drift(groups, params, planes, out, n=None, stream=None):
+    """groups: dict x, y, z, t, q of DEVICE float32 tensors; params: dict of wcsim_drift_params fields; planes: list of
+    dicts of wcsim_plane_geom fields; out: list (one per plane) of dicts t0, x0, sigma_t, sigma_x, q of DEVICE float32
+    tensors, written."""
+    ptrs = [_dev_ptr(groups[k]) for k in ("x", "y", "z", "t", "q")]
+    if n is None:
+        n = groups["x"].numel()
+    prm = wcsim_drift_params(**{k: float(params.get(k, 0.0)) for k, _ in wcsim_drift_params._fields_})
+    geo = (wcsim_plane_geom * len(planes))(*[wcsim_plane_geom(**{k: float(p[k]) for k, _ in wcsim_plane_geom._fields_})
+                                            for p in planes])
+    outs = (wcsim_depos * len(planes))(*[wcsim_depos(*[_dev_ptr(o[k]) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")])
+                                         for o in out])
+    _check(lib().wcsim_drift(*ptrs, int(n), C.byref(prm), geo, len(planes), outs, _stream_ptr(stream)), "wcsim_drift")
 
 
 def wcsim_debug_normal_draw(dev_N, dev_p, dev_w, dev_k, n, stream=None):

@@ -1,0 +1,47 @@
+// drift.cu -- the step upstream of the Raster ("After simulating the diffusion process along the drifting,
+// each ionization electron group is diffused into a 2D distribution along the drifting and wire pitch directions";
+// SURVEY 8(f)-2, reading A22).  One pass over the electron groups writes the depo arrays of ALL planes, so the groups
+// are read once per event instead of once per plane:
+//     td = (x - x_plane)/v,  t0 = (t + td - t_origin)/tick,  x0 = (y cos(theta) + z sin(theta) - origin)/pitch,
+//     sigma_t = sqrt(2 D_L td)/v/tick,  sigma_x = sqrt(2 D_T td)/pitch,  Q = q exp(-td/lifetime)
+// in fp64, rounded once to fp32 (units: cm, us, D in cm^2/s).  A group behind a plane gets NaN fields there, which the
+// raster skips and counts.  HBM bound: 20 B in, 20 B out per group and plane.
+#include "internal.h"
+
+namespace wcsim {
+
+namespace {
+
+__global__ void __launch_bounds__(256) drift_kernel(DriftInputs in, long long n, DriftParams prm, DriftPlanes planes)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double x = in.x[i], y = in.y[i], z = in.z[i], t = in.t[i], q = in.q[i];
+    const float nan = __int_as_float(0x7fc00000);
+#pragma unroll 1
+    for (int p = 0; p < planes.n; ++p) {
+        const DriftPlane pl = planes.plane[p];
+        const double td = __ddiv_rn(__dsub_rn(x, pl.x_plane), prm.v_drift);
+        float t0 = nan, x0 = nan, st = nan, sx = nan, Q = nan;
+        if (td >= 0.0) {
+            t0 = (float)__ddiv_rn(__dsub_rn(__dadd_rn(t, td), prm.t_origin), prm.tick);
+            const double u = __dadd_rn(__dmul_rn(y, pl.cos_theta), __dmul_rn(z, pl.sin_theta));
+            x0 = (float)__ddiv_rn(__dsub_rn(u, pl.pitch_origin), pl.pitch);
+            st = (float)__ddiv_rn(__ddiv_rn(__dsqrt_rn(__dmul_rn(prm.two_DL, td)), prm.v_drift), prm.tick);
+            sx = (float)__ddiv_rn(__dsqrt_rn(__dmul_rn(prm.two_DT, td)), pl.pitch);
+            Q = (float)(prm.lifetime > 0.0 ? __dmul_rn(q, exp(-td / prm.lifetime)) : q);
+        }
+        pl.out.t0[i] = t0, pl.out.x0[i] = x0, pl.out.sigma_t[i] = st, pl.out.sigma_x[i] = sx, pl.out.q[i] = Q;
+    }
+}
+
+} // namespace
+
+cudaError_t launch_drift(DriftInputs in, long long n, DriftParams prm, DriftPlanes planes, cudaStream_t st)
+{
+    if (n <= 0 || planes.n <= 0) return cudaSuccess;
+    drift_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in, n, prm, planes);
+    return cudaGetLastError();
+}
+
+} // namespace wcsim

@@ -88,6 +88,27 @@ cudaError_t build_response_spectrum(const float *dev_R, int n_rw, int n_rt, int 
 cudaError_t build_response_rows(const double2 *dev_tmp, int n_rw, int rt_rows, int pad_t, int spec_stride,
                                 float2 *dev_Rt, cudaStream_t st);
 
+// ---- drift.cu ---- (upstream of the raster: reading A22)
+struct DriftInputs {
+    const float *x, *y, *z, *t, *q;
+};
+struct DepoOutputs {
+    float *t0, *x0, *sigma_t, *sigma_x, *q;
+};
+struct DriftParams {
+    double v_drift, two_DL, two_DT, tick, t_origin, lifetime; // two_D* = 2 D 1e-6: cm^2/us
+};
+struct DriftPlane {
+    double x_plane, cos_theta, sin_theta, pitch_origin, pitch;
+    DepoOutputs out;
+};
+constexpr int kMaxDriftPlanes = 4;
+struct DriftPlanes {
+    int n;
+    DriftPlane plane[kMaxDriftPlanes];
+};
+cudaError_t launch_drift(DriftInputs in, long long n, DriftParams prm, DriftPlanes planes, cudaStream_t st);
+
 // ---- debug.cu ----
 cudaError_t launch_debug_philox(const unsigned int *ctr, const unsigned int *key, unsigned int *out, long long n,
                                 cudaStream_t st);

@@ -619,6 +619,31 @@ int wcsim_debug_philox(const unsigned int *dev_ctr, const unsigned int *dev_key,
     return WCSIM_OK;
 }
 
+int wcsim_drift(const float *dev_x, const float *dev_y, const float *dev_z, const float *dev_t, const float *dev_q,
+                long long n, const wcsim_drift_params *params, const wcsim_plane_geom *planes, int n_planes,
+                const wcsim_depos *out, void *cuda_stream)
+{
+    if (n < 0 || !params || !planes || !out || n_planes < 1 || n_planes > kMaxDriftPlanes) return WCSIM_EINVAL;
+    if (!(params->v_drift > 0.0) || !(params->tick > 0.0) || params->D_L < 0.0 || params->D_T < 0.0) return WCSIM_EINVAL;
+    if (n == 0) return WCSIM_OK;
+    if (!dev_x || !dev_y || !dev_z || !dev_t || !dev_q) return WCSIM_EINVAL;
+    DriftPlanes dp{};
+    dp.n = n_planes;
+    for (int p = 0; p < n_planes; ++p) {
+        if (!(planes[p].pitch > 0.0)) return WCSIM_EINVAL;
+        if (!out[p].t0 || !out[p].x0 || !out[p].sigma_t || !out[p].sigma_x || !out[p].q) return WCSIM_EINVAL;
+        dp.plane[p] = DriftPlane{planes[p].x_plane, planes[p].cos_theta, planes[p].sin_theta, planes[p].pitch_origin,
+                                 planes[p].pitch,
+                                 DepoOutputs{const_cast<float *>(out[p].t0), const_cast<float *>(out[p].x0),
+                                             const_cast<float *>(out[p].sigma_t), const_cast<float *>(out[p].sigma_x),
+                                             const_cast<float *>(out[p].q)}};
+    }
+    const DriftParams prm{params->v_drift, 2.0 * params->D_L * 1e-6, 2.0 * params->D_T * 1e-6, params->tick,
+                          params->t_origin, params->lifetime};
+    CU_TRY(launch_drift(DriftInputs{dev_x, dev_y, dev_z, dev_t, dev_q}, n, prm, dp, (cudaStream_t)cuda_stream));
+    return WCSIM_OK;
+}
+
 int wcsim_debug_erf(const double *host_z, double *host_out, long long n)
 {
     if (n < 0 || (n > 0 && (!host_z || !host_out))) return WCSIM_EINVAL;
