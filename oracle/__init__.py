@@ -169,6 +169,19 @@ def drift(x, y, z, t, q, *, v_drift, D_L, D_T, tick, t_origin=0.0, lifetime=0.0,
     return out
 
 
+def digitize(M, gain, baseline, bits=12):
+    """Reading A23: ideal ADC codes of an fp32 grid, int16."""
+    M = np.ascontiguousarray(M, dtype=np.float32)
+    adc = np.empty(M.shape, dtype=np.int16)
+    L = lib()
+    L.wco_digitize.argtypes = [C.POINTER(C.c_float), C.c_int64, C.c_float, C.c_float, C.c_int, C.POINTER(C.c_int16)]
+    L.wco_digitize.restype = C.c_int
+    rc = L.wco_digitize(_p(M, C.c_float), M.size, float(gain), float(baseline), int(bits), _p(adc, C.c_int16))
+    if rc != 0:
+        raise ValueError("wco_digitize rc=%d" % rc)
+    return adc
+
+
 def _fluct_mode(fluctuate) -> int:
     """False/0: off, True/1: binomial (A6), 2 or "normal": normal approximation (A21)."""
     if fluctuate == "normal":

@@ -24,6 +24,7 @@
  *   philox ................ published known-answer vectors (tests/golden/)
  *   norm_ppf .............. published normal quantiles (tests/golden/), scipy ndtri
  *   binomial .............. exact binomial CDF break points, mirror identity, moments
+ *   digitize .............. hand-worked codes (ties, clamps), monotone, numpy restatement
  *   drift ................. the widths BASELINE.json configs[1] states for td = 2.25 ms, closed forms
  *   normal_draw ........... its formula restated with scipy's ndtri, moments, the paper's
  *                           0.01 % agreement with the binomial waveforms
@@ -243,6 +244,29 @@ double wco_normal_draw(double N, double p, uint32_t w)
     if (k < 0.0) k = 0.0;
     if (k > N) k = N;
     return k;
+}
+
+/* ------------------------------------------------------------------------- */
+/* Digitisation (downstream of M).  PAPER.md:40: "M(t,x) is the  */
+/* 'measured' value such as what is input to an analog-to-digital converter    */
+/* (ADC) channel x at time t".  Reading A23: an ideal ADC of `bits` bits,       */
+/*   code = clamp(rint(M gain + baseline), 0, 2^bits - 1),  round half to even, */
+/* the product and the sum each rounded to fp32 (M is an fp32 array; this is   */
+/* integer work decided in the kernel's precision).  NaN -> 0.                 */
+/* ------------------------------------------------------------------------- */
+int wco_digitize(const float *M, int64_t n, float gain, float baseline, int bits, int16_t *adc)
+{
+    if (n < 0 || bits < 1 || bits > 15) return -1;
+    const float top = (float)((1 << bits) - 1);
+    for (int64_t i = 0; i < n; ++i) {
+        float prod = M[i] * gain;
+        float v = prod + baseline;
+        float c = rintf(v);
+        if (!(c > 0.0f)) c = 0.0f; /* also NaN */
+        if (c > top) c = top;
+        adc[i] = (int16_t)c;
+    }
+    return 0;
 }
 
 /* ------------------------------------------------------------------------- */
