@@ -238,6 +238,35 @@ def run_ours(args):
     for _ in range(min(e2e_steps, 20)):
         plan.simulate_host(host, host_M[0], seed=cfg["fluct_seed"], fluctuate=fluct)
     e2e_sync_ms = (time.perf_counter() - t0) * 1e3 / min(e2e_steps, 20)
+    # extra: the same round trip returning 12-bit ADC codes (wcsim_digitize, reading A23) instead of the fp32 M: half the
+    # device->host bytes.  Copies are torch's, on each plan's stream; every step's codes are on the host when its plan
+    # is synchronised.
+    dev_in = [{k: torch.empty_like(v, device=dev) for k, v in host.items()} for _ in range(n_e2e_plans)]
+    dev_adc = [torch.empty((pl["n_wires"], pl["n_ticks"]), dtype=torch.int16, device=dev) for _ in range(n_e2e_plans)]
+    host_adc = [torch.empty((pl["n_wires"], pl["n_ticks"]), dtype=torch.int16).pin_memory() for _ in range(n_e2e_plans)]
+
+    def run_e2e_adc(k):
+        for i in range(k):
+            j = i % n_e2e_plans
+            p = e2e_plans[j]
+            p.sync()
+            with torch.cuda.stream(e2e_streams[j]):
+                for kk in host:
+                    dev_in[j][kk].copy_(host[kk], non_blocking=True)
+                p.clear()
+                p.raster_scatter(dev_in[j], seed=cfg["fluct_seed"], fluctuate=fluct)
+                p.convolve()
+                p.digitize(ADC_GAIN, ADC_BASELINE, 12, out=dev_adc[j])
+                host_adc[j].copy_(dev_adc[j], non_blocking=True)
+        for p in e2e_plans:
+            p.sync()
+
+    run_e2e_adc(2)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    run_e2e_adc(e2e_steps)
+    torch.cuda.synchronize()
+    e2e_adc_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
     for p in e2e_plans:
         p.destroy()
 
@@ -314,7 +343,10 @@ def run_ours(args):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_slowest * 1e3 / e2e_steps, "steps": e2e_steps,
                 "how": "wcsim_simulate_host_async on 2 plans/streams alternately, pinned host buffers",
-                "ms_per_step_synchronous_call": e2e_sync_ms},
+                "ms_per_step_synchronous_call": e2e_sync_ms,
+                "adc_variant": {"ms_per_step": e2e_adc_ms, "value": n_depos / (e2e_adc_ms * 1e-3),
+                                "d2h_bytes_per_step": d2h // 2,
+                                "what": "same round trip with wcsim_digitize: 12-bit ADC codes (int16) come back instead of fp32 M"}},
         "gpu_launches": launches,
         "roofline": roofline,
         "ms_per_step_median": statistics.median(per_step),
@@ -338,6 +370,8 @@ def run_ours(args):
 TRAFFIC = {"raster": 6.03e6, "rows_forward": 19.29e6, "cols": 27.2e6, "rows_inverse": 26.39e6}
 # algorithmic fp64 work per drawn bin of the fluctuated raster (DESIGN.md section 6 derives it from the oracle's steps)
 FP64_FLOP_PER_BIN = 70.0
+# the e2e ADC variant's ideal converter (reading A23): codes per unit of M, and pedestal
+ADC_GAIN, ADC_BASELINE = 0.01, 900.0
 
 
 def survey_pass_model_bytes(pl):

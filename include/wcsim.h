@@ -206,6 +206,16 @@ int wcsim_drift(const float *dev_x, const float *dev_y, const float *dev_z, cons
                 long long n, const wcsim_drift_params *params, const wcsim_plane_geom *planes, int n_planes,
                 const wcsim_depos *out, void *cuda_stream);
 
+/*
+ * Digitisation: the step downstream of M ("M(t,x) is the 'measured' value such as what is input to an
+ * analog-to-digital converter (ADC) channel x at time t"; reading A23).  An ideal ADC of `bits` bits:
+ *   dev_adc[x][t] = clamp(rint(M[x][t] * gain + baseline), 0, 2^bits - 1),  round half to even, fp32, NaN -> 0,
+ * over the plan's output grid (after wcsim_convolve / wcsim_add_noise), enqueued on the plan's stream.
+ *   dev_adc : DEVICE, n_wires*n_ticks int16, 8-byte aligned, caller-owned, written.
+ * Errors: WCSIM_EINVAL (NULL, bits outside 1..15, misaligned dev_adc), WCSIM_ECUDA.
+ */
+int wcsim_digitize(wcsim_plan *plan, float gain, float baseline, int bits, short *dev_adc);
+
 /* Test/diagnostic hooks: exact pieces of the path, exposed so that parity can be checked piecewise. */
 /* out[4] (DEVICE, 4*n uint32) = Philox4x32-10(ctr = dev_ctr[4*i..], key = dev_key[2*i..]) for i < n */
 int wcsim_debug_philox(const unsigned int *dev_ctr, const unsigned int *dev_key, unsigned int *dev_out, long long n,

@@ -23,7 +23,7 @@ SYMBOLS = [
     "wcsim_plan_destroy", "wcsim_clear", "wcsim_clear_output", "wcsim_sync", "wcsim_set_scatter_mode", "wcsim_set_wire_mode",
     "wcsim_charge_ptr", "wcsim_output_ptr", "wcsim_get_dims", "wcsim_get_stats", "wcsim_reset_stats",
     "wcsim_simulate_host", "wcsim_set_profiling", "wcsim_get_stage_times", "wcsim_get_launch_count",
-    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf", "wcsim_simulate_host_async", "wcsim_debug_normal_draw", "wcsim_drift",
+    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf", "wcsim_simulate_host_async", "wcsim_debug_normal_draw", "wcsim_drift", "wcsim_digitize",
     "wcsim_strerror", "wcsim_last_cuda_error", "wcsim_version",
 ]
 
@@ -93,6 +93,7 @@ def lib():
         L.wcsim_debug_normal_draw.argtypes = [vp, vp, vp, vp, ll, vp]
         L.wcsim_debug_response_spectrum.argtypes = [vp, vp]
         L.wcsim_debug_erf.argtypes = [vp, vp, ll]
+        L.wcsim_digitize.argtypes = [vp, C.c_float, C.c_float, i, vp]
         L.wcsim_drift.argtypes = [vp, vp, vp, vp, vp, ll, C.POINTER(wcsim_drift_params), C.POINTER(wcsim_plane_geom), i,
                                   C.POINTER(wcsim_depos), vp]
         L.wcsim_strerror.argtypes = [i]
@@ -315,6 +316,13 @@ def wcsim_debug_binomial(dev_N, dev_p, dev_w, dev_k, n, stream=None):
                                       _stream_ptr(stream)), "wcsim_debug_binomial")
 
 
+def wcsim_digitize(plan, gain, baseline, bits, dev_adc):
+    """dev_adc: DEVICE int16 tensor of n_wires*n_ticks elements, written (ideal ADC of reading A23)."""
+    import torch
+    _check(lib().wcsim_digitize(plan, float(gain), float(baseline), int(bits), _dev_ptr(dev_adc, torch.int16)),
+           "wcsim_digitize")
+
+
 def wcsim_drift(groups, params, planes, out, n=None, stream=None):
     """groups: dict x, y, z, t, q of DEVICE float32 tensors; params: dict of wcsim_drift_params fields; planes: list of
     dicts of wcsim_plane_geom fields; out: list (one per plane) of dicts t0, x0, sigma_t, sigma_x, q of DEVICE float32
@@ -431,6 +439,13 @@ class Plan:
 
     def simulate_host(self, host_depos, host_M, **kw):
         wcsim_simulate_host(self.handle, host_depos, host_M, **kw)
+
+    def digitize(self, gain, baseline, bits=12, out=None):
+        import torch
+        if out is None:
+            out = torch.empty((self.n_wires, self.n_ticks), dtype=torch.int16, device="cuda")
+        wcsim_digitize(self.handle, gain, baseline, bits, out)
+        return out
 
     def simulate_host_async(self, host_depos, host_M, **kw):
         wcsim_simulate_host_async(self.handle, host_depos, host_M, **kw)

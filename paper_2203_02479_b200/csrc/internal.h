@@ -108,6 +108,8 @@ struct DriftPlanes {
     DriftPlane plane[kMaxDriftPlanes];
 };
 cudaError_t launch_drift(DriftInputs in, long long n, DriftParams prm, DriftPlanes planes, cudaStream_t st);
+// ideal ADC of reading A23: adc[i] = clamp(rint(M[i] gain + baseline), 0, 2^bits - 1); M 16-byte, adc 8-byte aligned
+cudaError_t launch_digitize(const float *M, long long n, float gain, float baseline, int bits, short *adc, cudaStream_t st);
 
 // ---- debug.cu ----
 cudaError_t launch_debug_philox(const unsigned int *ctr, const unsigned int *key, unsigned int *out, long long n,

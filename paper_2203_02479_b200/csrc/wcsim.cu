@@ -619,6 +619,16 @@ int wcsim_debug_philox(const unsigned int *dev_ctr, const unsigned int *dev_key,
     return WCSIM_OK;
 }
 
+int wcsim_digitize(wcsim_plan *plan, float gain, float baseline, int bits, short *dev_adc)
+{
+    if (!plan || !dev_adc || bits < 1 || bits > 15 || (reinterpret_cast<uintptr_t>(dev_adc) & 7u)) return WCSIM_EINVAL;
+    DeviceGuard guard(plan->device);
+    if (!guard.ok) return fail_cuda(cudaGetLastError());
+    plan->launches += 1;
+    CU_TRY(launch_digitize(plan->M, (long long)plan->n_wires * plan->n_ticks, gain, baseline, bits, dev_adc, plan->stream));
+    return WCSIM_OK;
+}
+
 int wcsim_drift(const float *dev_x, const float *dev_y, const float *dev_z, const float *dev_t, const float *dev_q,
                 long long n, const wcsim_drift_params *params, const wcsim_plane_geom *planes, int n_planes,
                 const wcsim_depos *out, void *cuda_stream)

@@ -524,3 +524,27 @@ def test_drift_three_planes_matches_oracle_and_feeds_the_raster(B, O):
     assert np.count_nonzero(S != S_ref) <= max(2, 1e-6 * ost["drawn"])
     with pytest.raises(B.WcsimError):
         B.wcsim_drift(dev, dict(params, v_drift=0.0), planes, out)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# digitisation downstream of M (reading A23)
+# ---------------------------------------------------------------------------------------------------------------
+def test_digitize_matches_oracle_bit_for_bit(B, O):
+    from paper_2203_02479_b200 import synth
+    cfg = synth.config(1, n_depos=20_000)
+    pl = cfg["planes"][0]
+    nw, nt = 803, 5998  # odd sizes: the 4-sample vector path and its scalar tail
+    with B.Plan(nw, nt, synth.response(5, 16)) as p:
+        p.clear()
+        p.raster_scatter(to_dev(pl["depos"]), seed=2, fluctuate=True)
+        p.arm_noise(None, seed=7)
+        p.convolve()
+        for bits, gain, base in ((12, 0.02, 900.0), (14, 0.5, 2000.0), (8, 1e-4, 0.3)):
+            adc = p.digitize(gain, base, bits)
+            p.sync()
+            M = p.output().cpu().numpy()
+            ref = O.digitize(M, gain, base, bits)  # same fp32 input: integer work, must be identical
+            assert np.array_equal(adc.cpu().numpy(), ref), (bits, gain, base)
+            assert ref.min() >= 0 and ref.max() <= 2 ** bits - 1 and len(np.unique(ref)) > 3
+        with pytest.raises(B.WcsimError):
+            p.digitize(1.0, 0.0, 16)
