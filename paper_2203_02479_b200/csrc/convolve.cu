@@ -5,14 +5,17 @@
 //   rows_forward : one CTA per populated wire row.  The real row of pad_t samples is packed as pad_t/2 complex
 //                  points (even + i odd), transformed in shared memory, and split into the half spectrum
 //                  k = 0 .. pad_t/2.  Samples beyond n_ticks are zeros made in registers.
-//   cols         : one CTA per tile of C adjacent tick-frequencies.  Forward transform over the wire axis (rows
-//                  beyond n_wires are zeros made in registers), multiply by the response spectrum while the data
-//                  is still in registers, inverse transform, store only the n_wires rows that are kept.
-//   rows_inverse : one CTA per kept wire row.  Half spectrum -> packed complex -> inverse transform -> the first
-//                  n_ticks real samples.  The noise spectrum of step a7 is added to the row spectrum here, so noise
-//                  costs no pass over M of its own.
+//   wires        : (default when the response spans <= 64 wires) the wire-axis transform / multiply / inverse done
+//                  directly as an n_rw-tap convolution over wires for every tick frequency; see wires_kernel.
+//   cols         : (otherwise, or on request) one CTA per tile of C adjacent tick-frequencies.  Forward transform over
+//                  the wire axis (rows beyond n_wires are zeros made in registers), multiply by the response spectrum
+//                  while the data is still in registers, inverse transform, store only the n_wires rows that are kept.
+//   rows_inverse : one CTA per kept wire row (rows_inverse_tma_kernel: persistent CTAs, next row staged by a TMA bulk
+//                  copy).  Half spectrum -> packed complex -> inverse transform -> the first n_ticks real samples.
+//                  The noise spectrum of step a7 is added to the row spectrum here, so noise costs no pass over M.
 //
-// The 1/(pad_w pad_t) of the inverse transform is folded into Rhat (A14).  The FFT engine is csrc/fft.cuh.
+// The 1/(pad_w pad_t) of the inverse transform is folded into Rhat / Rt (A14).  The FFT engine is csrc/fft.cuh.  The
+// kernels of one plane-event are programmatic dependents of one another (csrc/pdl.cuh).
 #include "fft.cuh"
 #include "internal.h"
 #include "rng.cuh"

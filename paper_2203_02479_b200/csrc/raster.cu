@@ -1,30 +1,32 @@
 // raster.cu -- steps a1-a3 of the hot path: Raster, charge fluctuation, Scatter-add
 // (Section 2.2; Section 3.1 for the binomial fluctuation).
 //
-// Atomic mode (raster_batch_kernel): a warp takes 32 depos at a time, one per lane (the SoA layout of PAPER.md:72
-// makes the depo the unit of parallelism and the loads coalesce).  Each lane works out its depo's patch extent; a warp
-// scan lays all bin EDGES of the 32 patches end to end and the lanes evaluate erf over that flat list ("erf bin edges
-// once per axis"), leaving the values in the warp's shared-memory scratch; then the lanes walk the flat list of all
-// BINS of the 32 patches, 32 at a time, each forming p_ij = wt_i wx_j from four edge values.  All lanes are busy
+// Both scatter modes run raster_batch_body: a warp takes a batch of 8 depos, one per lane (the SoA layout of PAPER.md:72
+// makes the depo the unit of parallelism and the loads coalesce; lanes 8..31 own none).  Each owning lane works out its
+// depo's patch extent, clipped to the batch's window (the grid, or a tile of it); a warp scan lays all bin EDGES of the
+// batch's patches end to end and all 32 lanes evaluate erf over that flat list ("erf bin edges once per axis"; own
+// table erf, erf_table.cuh), leaving the values in the warp's shared-memory scratch; then the lanes walk the flat list
+// of all BINS of the batch, 32 at a time, each forming p_ij = wt_i wx_j from four edge values.  All lanes are busy
 // whatever the patch shapes are (patches are 1-5 wires x 1-16 ticks in BASELINE.json's configs).  With fluctuation on,
-// bins are first sorted by the routine that will draw them (inversion / AS 241 central / AS 241 tail) into three
-// per-warp queues and drawn 32 at a time from one queue, so the fp64 sampler runs without divergence.  A patch with
-// more edges than the scratch holds falls back to the one-warp-per-depo walk (raster_depo), which chunks it.
-// Nothing of a patch is ever written to HBM except the final adds into S.
+// bins are first sorted by the routine that will draw them (inversion in three mu bands / AS 241 central / AS 241
+// tail) into five per-warp queues and drawn 32 at a time from one queue, so the fp64 sampler runs without divergence.
+// A patch with more edges than the scratch holds falls back to the one-warp-per-depo walk (raster_depo), which chunks
+// it.  Nothing of a patch is ever written to HBM except the final adds into S.
 //
-// raster_depo (big patches, tiled mode): one warp owns one depo.  The lanes evaluate erf at consecutive bin edges of
-// one axis, a shuffle turns neighbouring edges into bin weights, lanes run along the tick axis (contiguous in S),
-// the wire index is broadcast by shuffle.
+// raster_depo (patches too big for the scratch): one warp owns one depo.  The lanes evaluate erf at consecutive bin
+// edges of one axis, a shuffle turns neighbouring edges into bin weights, lanes run along the tick axis (contiguous in
+// S), the wire index is broadcast by shuffle.
 //
 //   fluctuate = 0: fp32 weights (erff), value q * (wt * wx)
 //   fluctuate = 1: fp64 weights (erf), p = wt * wx, integer draw B(N, p; Philox word of the absolute bin)
 //   fluctuate = 2: the same with the normal-approximation draw of the paper's Kokkos port (reading A21)
 //
 // Two scatter modes:
-//   atomic: red.global.add.f32 straight into S
-//   tiled : depos are grouped by the grid tiles their patch overlaps (count / scan / fill), one CTA per tile
-//           accumulates its depos in shared memory in 2^-24 fixed point (integer adds: order independent, so the
-//           result is bitwise reproducible) and adds the tile to S once.
+//   atomic: raster_batch_kernel, persistent warps fetching batches from a device counter (guided: 8 depos, then 2 at a
+//           time near the end), red.global.add.f32 straight into S
+//   tiled : depos are grouped by the grid tiles their patch overlaps (count / scan / fill), one CTA per tile runs the
+//           batch body over its depos, clipped to the tile, accumulating in shared memory in 2^-24 fixed point
+//           (integer adds: order independent, so the result is bitwise reproducible) and adds the tile to S once.
 #include "internal.h"
 #include "erf_table.cuh"
 #include "pdl.cuh"
@@ -189,7 +191,7 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v)
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// atomic mode: warps fetch batches of 32 depos from a device-side counter until none is left
+// atomic mode: warps fetch batches of kBatchDepos depos from a device-side counter until none is left
 // ------------------------------------------------------------------------------------------------------------------
 constexpr int kBatchWarps = 4;          // warps per CTA
 constexpr int kBatchShift = 3;          // log2 of the depos a warp fetches at a time (lanes beyond that own no depo):
