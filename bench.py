@@ -366,8 +366,8 @@ def run_ours(args):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1], from the committed `ncu --set full` capture
-# (profiles/r01_ncu_full.md; cold-cache replays, so reads are compulsory misses and writes mostly stay in L2)
-TRAFFIC = {"raster": 6.03e6, "rows_forward": 19.29e6, "cols": 27.2e6, "rows_inverse": 26.39e6}
+# (profiles/r01i_ncu_full.md; cold-cache replays, so reads are compulsory misses and writes mostly stay in L2)
+TRAFFIC = {"raster": 6.03e6, "rows_forward": 19.29e6, "cols": 27.68e6, "rows_inverse": 26.36e6}
 # algorithmic fp64 work per drawn bin of the fluctuated raster (DESIGN.md section 6 derives it from the oracle's steps)
 FP64_FLOP_PER_BIN = 70.0
 # the e2e ADC variant's ideal converter (reading A23): codes per unit of M, and pedestal
