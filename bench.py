@@ -457,10 +457,19 @@ def cpu_baseline(cfg, budget_s=15.0):
         oracle_step(cfg, O)
         reps += 1
     dt = time.perf_counter() - t0
-    return {"value": n_depos * reps / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
-            "ms_per_step": dt * 1e3 / reps,
-            "sample": "%d whole plane-events of the same workload (all %d depos, full grid), fp64, "
-                      "FFT-route convolution" % (reps, n_depos)}
+    cores = O.num_threads()
+    out = {"value": n_depos * reps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "ms_per_step": dt * 1e3 / reps,
+           "sample": "%d whole plane-events of the same workload (all %d depos, full grid), fp64, "
+                     "FFT-route convolution" % (reps, n_depos)}
+    # one thread, what the paper's CPU-ref was: one plane-event
+    O.set_num_threads(1)
+    t0 = time.perf_counter()
+    oracle_step(cfg, O)
+    dt1 = time.perf_counter() - t0
+    O.set_num_threads(cores)
+    out["single_thread"] = {"value": n_depos / dt1, "ms_per_step": dt1 * 1e3, "cores": 1, "sample": "1 whole plane-event"}
+    return out
 
 
 def run_reference(args):

@@ -99,6 +99,14 @@ def num_threads() -> int:
     return int(lib().wco_num_threads())
 
 
+def set_num_threads(n: int) -> None:
+    """Threads of the loops over independent rows (timing only)."""
+    L = lib()
+    L.wco_set_num_threads.argtypes = [C.c_int]
+    L.wco_set_num_threads.restype = None
+    L.wco_set_num_threads(int(n))
+
+
 def philox4x32_10(ctr, key):
     c = np.asarray(ctr, dtype=np.uint32).copy()
     k = np.asarray(key, dtype=np.uint32).copy()

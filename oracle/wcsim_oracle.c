@@ -605,6 +605,16 @@ int wco_fft(double *re, double *im, int n, int sign)
     return 0;
 }
 
+/* threads used by the parallel loops over independent rows (timing only; no arithmetic depends on it) */
+void wco_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 int wco_num_threads(void)
 {
     int n = 1;
