@@ -454,6 +454,9 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
     pdl_trigger();
     pdl_wait();
 
+    // (fetching the NEXT batch's index early, to hide the ~1 us round trip of this atomic -- 14 % of the stall samples on
+    // configs[1] -- was tried: a warp then sits on a batch while it works on another, and the load balance suffers more
+    // than the latency costs: 75.7 -> 82.6 us)
     for (;;) {
         long long batch = 0;
         if (lane == 0) batch = (long long)atomicAdd(&counters->next_batch, 1ull);
