@@ -38,6 +38,8 @@ struct TileScratch {
     unsigned int *entries;        // [capacity] depo indices grouped by tile
     unsigned long long capacity;  // entries allocated
     unsigned int *total;          // [1] total number of (depo, tile) pairs
+    unsigned int slice_entries;   // listed depos per slice of a hot tile (set per call from the mean tile load)
+    unsigned long long *fix;      // [n_wires * n_ticks] 2^-24 fixed-point grid the tile CTAs add into; zero between calls
 };
 cudaError_t launch_tile_count(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts, cudaStream_t st);
 cudaError_t launch_tile_scan(TileScratch ts, cudaStream_t st);
@@ -47,6 +49,8 @@ void tile_shape(int *tile_w, int *tile_t);
 cudaError_t launch_tile_accumulate(GridDims g, DepoArrays d, uint64_t id_base, uint64_t seed, int fluctuate,
                                    double nsigma, TileScratch ts, float *S, int *depo_totals, Counters *counters,
                                    cudaStream_t st);
+// S += fix 2^-24, fix = 0 (after launch_tile_accumulate)
+cudaError_t launch_tile_finalize(GridDims g, TileScratch ts, float *S, cudaStream_t st);
 
 // ---- convolve.cu ----
 struct ConvBuffers {

@@ -118,8 +118,14 @@ struct TileSink {
     }
     __device__ __forceinline__ void add_at(uint32_t idx, float v) const
     {
-        const long long q = __double2ll_rn((double)v * kFixScale);
-        atomicAdd(acc + idx, (unsigned long long)q);
+        // a 64-bit shared-memory atomic add is a compare-and-swap loop (ATOMS.CAST.SPIN.64); two native 32-bit adds with
+        // the carry of the low word do the same sum modulo 2^64, in any order
+        const unsigned long long q = (unsigned long long)__double2ll_rn((double)v * kFixScale);
+        const unsigned int lo = (unsigned int)q, hi = (unsigned int)(q >> 32);
+        unsigned int *a = reinterpret_cast<unsigned int *>(acc + idx); // little endian: a[0] low word
+        const unsigned int old = atomicAdd(a, lo);
+        const unsigned int h = hi + ((old + lo < old) ? 1u : 0u);
+        if (h) atomicAdd(a + 1, h);
     }
     __device__ __forceinline__ void add(int wire, int tick, float v) const { add_at(index(wire, tick), v); }
 };
@@ -587,10 +593,13 @@ __global__ void tile_fill_kernel(GridDims g, DepoArrays d, long long n, double n
         }
 }
 
-// One CTA per tile.  Its warps take the tile's depos (the index list built by count / scan / fill) eight at a time and
-// run the same flat-list batch body as the atomic kernel, clipped to the tile and accumulating into the tile's
-// fixed-point shared-memory accumulators; the tile is added to S once at the end.
-constexpr int kTileWarps = 8;
+// Up to kTileSlices CTAs per tile (one per kSliceEntries listed depos, so that the hot tiles along a track do not
+// serialise on one CTA).  A CTA's warps take their slice of the tile's depos (the index list built by count / scan /
+// fill) eight at a time and run the same flat-list batch body as the atomic kernel, clipped to the tile and
+// accumulating into fixed-point shared-memory accumulators; at the end the CTA adds its non-zero accumulators into the
+// global fixed-point grid `fix` (64-bit integer atomics: order independent), and tile_finalize_kernel folds `fix`
+// into S with one float add per bin.
+constexpr int kTileWarps = 8, kTileSlices = 8, kSliceEntries = 256;
 template <bool FLUCT, bool TOT>
 struct TileSmem {
     unsigned long long acc[kTileW * kTileT];
@@ -611,9 +620,17 @@ __global__ void __launch_bounds__(kTileWarps * 32, 2) tile_accumulate_kernel(Gri
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem<FLUCT, TOT> &sm = *reinterpret_cast<TileSmem<FLUCT, TOT> *>(smem_raw);
-    const int tile = blockIdx.x;
-    const unsigned int beg = ts.tile_count[tile], end = ts.tile_count[tile + 1];
-    if (beg == end) return; // uniform over the CTA
+    const int tile = blockIdx.x / kTileSlices, slice = blockIdx.x % kTileSlices;
+    const unsigned int tile_beg = ts.tile_count[tile], tile_end = ts.tile_count[tile + 1];
+    const unsigned int listed = tile_end - tile_beg;
+    // a tile is split only when it lists well over the average (ts.slice_entries = max(kSliceEntries, 2 x mean)): on an
+    // evenly busy plane (configs[4]) slicing only adds clears, flushes and partial queue drains
+    const unsigned int n_slices = min((unsigned int)kTileSlices, (listed + ts.slice_entries - 1) / ts.slice_entries);
+    if ((unsigned int)slice >= n_slices) return; // uniform over the CTA (also: nothing listed)
+    // equal slices in whole batches
+    const unsigned int per = ((listed + n_slices - 1) / n_slices + kBatchDepos - 1) / kBatchDepos * kBatchDepos;
+    const unsigned int beg = min(tile_beg + (unsigned int)slice * per, tile_end), end = min(beg + per, tile_end);
+    if (beg == end) return;
     const int tw = tile / ts.tiles_t, tt = tile % ts.tiles_t;
     const int w0 = tw * kTileW, k0 = tt * kTileT;
     const int w1 = min(w0 + kTileW, g.n_wires), k1 = min(k0 + kTileT, g.n_ticks);
@@ -650,11 +667,20 @@ __global__ void __launch_bounds__(kTileWarps * 32, 2) tile_accumulate_kernel(Gri
     __syncthreads();
     for (int i = threadIdx.x; i < kTileW * kTileT; i += blockDim.x) {
         const int w = w0 + i / kTileT, k = k0 + i % kTileT;
-        const long long q = (long long)sm.acc[i];
-        if (q != 0 && w < w1 && k < k1) {
-            float *p = S + (size_t)w * g.n_ticks + k;
-            *p = *p + (float)((double)q * (1.0 / kFixScale));
-        }
+        const unsigned long long q = sm.acc[i];
+        if (q != 0ull && w < w1 && k < k1) atomicAdd(ts.fix + (size_t)w * g.n_ticks + k, q);
+    }
+}
+
+__global__ void __launch_bounds__(256) tile_finalize_kernel(long long n_bins, unsigned long long *__restrict__ fix,
+                                                            float *__restrict__ S)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_bins) return;
+    const long long q = (long long)fix[i];
+    if (q != 0) {
+        S[i] = S[i] + (float)((double)q * (1.0 / kFixScale));
+        fix[i] = 0ull;
     }
 }
 
@@ -764,7 +790,7 @@ static cudaError_t launch_tile_accumulate_t(GridDims g, DepoArrays d, uint64_t i
                                             cudaStream_t st)
 {
     const int n_tiles = ts.tiles_w * ts.tiles_t;
-    tile_accumulate_kernel<FLUCT, TOT><<<n_tiles, kTileWarps * 32, sizeof(TileSmem<FLUCT, TOT>), st>>>(
+    tile_accumulate_kernel<FLUCT, TOT><<<n_tiles * kTileSlices, kTileWarps * 32, sizeof(TileSmem<FLUCT, TOT>), st>>>(
         g, d, id_base, seed, nsigma, ts, S, depo_totals, counters, normal_only);
     return cudaGetLastError();
 }
@@ -779,6 +805,13 @@ cudaError_t launch_tile_accumulate(GridDims g, DepoArrays d, uint64_t id_base, u
         return launch_tile_accumulate_t<true, true>(g, d, id_base, seed, nsigma, ts, S, depo_totals, counters,
                                                     fluctuate == 2, st);
     return launch_tile_accumulate_t<true, false>(g, d, id_base, seed, nsigma, ts, S, nullptr, counters, fluctuate == 2, st);
+}
+
+cudaError_t launch_tile_finalize(GridDims g, TileScratch ts, float *S, cudaStream_t st)
+{
+    const long long n_bins = (long long)g.n_wires * g.n_ticks;
+    tile_finalize_kernel<<<(unsigned)((n_bins + 255) / 256), 256, 0, st>>>(n_bins, ts.fix, S);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_count_invalid(DepoArrays d, long long n, Counters *counters, cudaStream_t st)

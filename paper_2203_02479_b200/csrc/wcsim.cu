@@ -245,10 +245,20 @@ int raster_tiled(wcsim_plan *p, GridDims g, DepoArrays d, long long n, uint64_t 
         CU_TRY(cudaMalloc((void **)&ts.entries, sizeof(unsigned int) * cap));
         ts.capacity = cap;
     }
+    {
+        const unsigned long long twice_mean = 2ull * need / (unsigned long long)(n_tiles > 0 ? n_tiles : 1);
+        ts.slice_entries = (unsigned int)(twice_mean > 256ull ? (twice_mean < 0x7fffffffull ? twice_mean : 0x7fffffffull) : 256ull);
+    }
+    if (!ts.fix) { // first use of the tiled mode on this plan
+        const size_t bytes = sizeof(unsigned long long) * (size_t)g.n_wires * g.n_ticks;
+        CU_TRY(cudaMalloc((void **)&ts.fix, bytes));
+        CU_TRY(cudaMemsetAsync(ts.fix, 0, bytes, p->stream));
+    }
     CU_TRY(launch_tile_fill(g, d, n, p->nsigma, ts, p->stream));
     if (totals) CU_TRY(cudaMemsetAsync(totals, 0, sizeof(int) * (size_t)n, p->stream));
     CU_TRY(launch_count_invalid(d, n, p->counters, p->stream));
     CU_TRY(launch_tile_accumulate(g, d, id_base, seed, fluctuate, p->nsigma, ts, p->S, totals, p->counters, p->stream));
+    CU_TRY(launch_tile_finalize(g, ts, p->S, p->stream));
     return WCSIM_OK;
 }
 
@@ -259,7 +269,7 @@ int destroy_impl(wcsim_plan *p)
     void *bufs[] = {p->spec2,    p->Rt,
                     p->S,        p->M,           p->spec_alloc,  p->Rhat,           p->tw_row,        p->tw_real,
                     p->tw_col,   p->counters,    p->amp_builtin, p->amp_custom,     p->ts.tile_count, p->ts.tile_cursor,
-                    p->ts.entries, p->ts.total,  p->stage[0],    p->stage[1],       p->stage[2],      p->stage[3],
+                    p->ts.entries, p->ts.total, p->ts.fix,  p->stage[0],    p->stage[1],       p->stage[2],      p->stage[3],
                     p->stage[4]};
     for (void *b : bufs)
         if (b) cudaFree(b);
@@ -391,7 +401,7 @@ int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n
     const DepoArrays d{depos->t0, depos->x0, depos->sigma_t, depos->sigma_x, depos->q};
     StageSpan span(plan, WCSIM_STAGE_RASTER);
     if (plan->scatter_mode == WCSIM_SCATTER_TILED) {
-        plan->launches += 5;
+        plan->launches += 6;
         return raster_tiled(plan, g, d, n, depo_id_base, seed, fluctuate, dev_depo_totals);
     }
     if (dev_depo_totals) CU_TRY(cudaMemsetAsync(dev_depo_totals, 0, sizeof(int) * (size_t)n, plan->stream));
