@@ -134,7 +134,7 @@ def run_ours(args):
     fluct = bool(cfg["fluctuate"]) and not args.no_fluct
     if fluct and args.fluct == "normal":
         fluct = 2
-    mode = B.WCSIM_SCATTER_TILED if args.scatter == "tiled" else B.WCSIM_SCATTER_ATOMIC
+    mode = {"atomic": B.WCSIM_SCATTER_ATOMIC, "tiled": B.WCSIM_SCATTER_TILED, "fixed": B.WCSIM_SCATTER_FIXED}[args.scatter]
     stream = torch.cuda.current_stream()
     plan = B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]), nsigma=cfg["nsigma"],
                   scatter_mode=mode, stream=stream)
@@ -514,7 +514,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index of the timed workload")
-    ap.add_argument("--scatter", default="atomic", choices=["atomic", "tiled"])
+    ap.add_argument("--scatter", default="atomic", choices=["atomic", "tiled", "fixed"])
     ap.add_argument("--wires", default="auto", choices=["auto", "fft", "direct"], help="wire axis of the convolution")
     ap.add_argument("--no-fluct", action="store_true")
     ap.add_argument("--fluct", default="binomial", choices=["binomial", "normal"],

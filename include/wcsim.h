@@ -41,6 +41,9 @@ typedef enum wcsim_status {
 #define WCSIM_SCATTER_TILED 1  /* depos are binned by grid tile, each tile is accumulated in shared memory in
                                   integer / fixed-point arithmetic (order independent => bitwise reproducible)
                                   and stored once; "deterministic sort-by-tile mode" of BASELINE.json north_star */
+#define WCSIM_SCATTER_FIXED 2  /* the atomic mode's kernel adding in 2^-24 fixed point into a 64-bit grid (integer
+                                  red.global adds: order independent => bitwise reproducible), folded into S by one
+                                  pass; deterministic without sorting, 8 bytes per bin of extra device memory */
 
 /* wire_mode of wcsim_set_wire_mode: how wcsim_convolve treats the wire axis of Eq. (2).  Both give the same M up to
  * fp32 rounding (the cropped result is the linear convolution either way). */

@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 WCSIM_OK, WCSIM_EINVAL, WCSIM_ENOMEM, WCSIM_ECUDA, WCSIM_ESTATE = 0, -1, -2, -3, -4
-WCSIM_SCATTER_ATOMIC, WCSIM_SCATTER_TILED = 0, 1
+WCSIM_SCATTER_ATOMIC, WCSIM_SCATTER_TILED, WCSIM_SCATTER_FIXED = 0, 1, 2
 WCSIM_WIRES_AUTO, WCSIM_WIRES_FFT, WCSIM_WIRES_DIRECT = 0, 1, 2
 
 # every symbol include/wcsim.h declares (tests check that the library exports all of them)

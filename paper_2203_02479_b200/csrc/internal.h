@@ -29,6 +29,12 @@ cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t
                                  double nsigma, float *S, int *depo_totals, Counters *counters, int sm_count,
                                  cudaStream_t st);
 
+// the same kernel adding in 2^-24 fixed point into a 64-bit grid (RED.ADD.64: order independent, so reproducible bit for
+// bit whatever the order of the adds); launch_tile_finalize folds the grid into S afterwards
+cudaError_t launch_raster_fixed(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
+                                double nsigma, unsigned long long *fix, int *depo_totals, Counters *counters, int sm_count,
+                                cudaStream_t st);
+
 // a1-a3, tiled mode (deterministic): scratch buffers are owned by the plan and grown by the caller
 struct TileScratch {
     int tile_w, tile_t;           // tile shape in bins

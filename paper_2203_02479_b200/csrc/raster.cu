@@ -109,6 +109,28 @@ struct GlobalSink {
     __device__ __forceinline__ void add(int wire, int tick, float v) const { add_at(index(wire, tick), v); }
 };
 
+// the same adds in 2^-24 fixed point into a 64-bit grid (RED.ADD.64: order independent); tile_finalize_kernel folds it into S
+struct FixSink {
+    unsigned long long *fix;
+    int n_ticks;
+    __device__ __forceinline__ uint32_t index(int wire, int tick) const
+    {
+        return (uint32_t)wire * (uint32_t)n_ticks + (uint32_t)tick;
+    }
+    __device__ __forceinline__ void add_at(uint32_t idx, float v) const
+    {
+        atomicAdd(fix + idx, (unsigned long long)__double2ll_rn((double)v * kFixScale));
+    }
+    __device__ __forceinline__ void add(int wire, int tick, float v) const { add_at(index(wire, tick), v); }
+};
+
+template <bool FIX>
+__device__ __forceinline__ auto make_grid_sink(float *grid, int n_ticks)
+{
+    if constexpr (FIX) return FixSink{reinterpret_cast<unsigned long long *>(grid), n_ticks};
+    else return GlobalSink{grid, n_ticks};
+}
+
 struct TileSink {
     unsigned long long *acc; // shared memory, [kTileW][kTileT]
     int w0, k0;
@@ -431,7 +453,7 @@ __device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const S
     }
 }
 
-template <bool FLUCT, bool TOT>
+template <bool FLUCT, bool TOT, bool FIX>
 __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
                                                                         uint64_t id_base, uint64_t seed, double nsigma,
                                                                         float *__restrict__ S, int *__restrict__ totals,
@@ -442,7 +464,9 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
     BatchSmem<FLUCT, TOT> &sm = *reinterpret_cast<BatchSmem<FLUCT, TOT> *>(smem_raw);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     BatchScratch<FLUCT> &sc = sm.scratch[wid];
-    const GlobalSink sink{S, g.n_ticks};
+    // FIX: S points at the 64-bit fixed-point grid (deterministic mode without tiles)
+    using Sink = typename std::conditional<FIX, FixSink, GlobalSink>::type;
+    const Sink sink = make_grid_sink<FIX>(S, g.n_ticks);
     const Clip clip{0, g.n_wires, 0, g.n_ticks};
     // guided batches: kBatchDepos depos at a time, then kTailDepos at a time for the last kTailPerWarp depos per warp of the
     // grid, so that the warps run out of work within a short batch of one another (a batch of 8 lasts ~20 us on
@@ -715,15 +739,17 @@ cudaError_t raster_configure(cudaStream_t st)
     if (err != cudaSuccess) return err;
     err = cudaStreamSynchronize(st); // `tab` is on this stack
     if (err != cudaSuccess) return err;
-    err = cudaFuncSetAttribute(raster_batch_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               (int)sizeof(BatchSmem<true, true>));
+#define WCSIM_RASTER_SMEM(F, T, X)                                                                                     \
+    err = cudaFuncSetAttribute(raster_batch_kernel<F, T, X>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
+                               (int)sizeof(BatchSmem<F, T>));                                                          \
     if (err != cudaSuccess) return err;
-    err = cudaFuncSetAttribute(raster_batch_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               (int)sizeof(BatchSmem<true, false>));
-    if (err != cudaSuccess) return err;
-    err = cudaFuncSetAttribute(raster_batch_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               (int)sizeof(BatchSmem<false, false>));
-    if (err != cudaSuccess) return err;
+    WCSIM_RASTER_SMEM(true, true, false)
+    WCSIM_RASTER_SMEM(true, false, false)
+    WCSIM_RASTER_SMEM(false, false, false)
+    WCSIM_RASTER_SMEM(true, true, true)
+    WCSIM_RASTER_SMEM(true, false, true)
+    WCSIM_RASTER_SMEM(false, false, true)
+#undef WCSIM_RASTER_SMEM
     err = cudaFuncSetAttribute(tile_accumulate_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                (int)sizeof(TileSmem<true, true>));
     if (err != cudaSuccess) return err;
@@ -734,7 +760,7 @@ cudaError_t raster_configure(cudaStream_t st)
                                 (int)sizeof(TileSmem<false, false>));
 }
 
-template <bool FLUCT, bool TOT>
+template <bool FLUCT, bool TOT, bool FIX>
 static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, double nsigma,
                                        float *S, int *depo_totals, Counters *counters, int sm_count, cudaStream_t st,
                                        bool normal_only)
@@ -747,21 +773,39 @@ static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, ui
     long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
     const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
     if (ctas > max_ctas) ctas = max_ctas;
-    return launch_pdl(raster_batch_kernel<FLUCT, TOT>, (unsigned)ctas, kBatchWarps * 32, smem, st, g, d, n, id_base, seed,
+    return launch_pdl(raster_batch_kernel<FLUCT, TOT, FIX>, (unsigned)ctas, kBatchWarps * 32, smem, st, g, d, n, id_base, seed,
                       nsigma, S, depo_totals, counters, normal_only);
+}
+
+template <bool FIX>
+static cudaError_t launch_raster_grid(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
+                                      double nsigma, float *grid, int *depo_totals, Counters *counters, int sm_count,
+                                      cudaStream_t st)
+{
+    if (n <= 0) return cudaSuccess;
+    if (!fluctuate) // no draws, no per-depo integer totals
+        return launch_raster_batch<false, false, FIX>(g, d, n, id_base, seed, nsigma, grid, nullptr, counters, sm_count, st,
+                                                      false);
+    if (depo_totals)
+        return launch_raster_batch<true, true, FIX>(g, d, n, id_base, seed, nsigma, grid, depo_totals, counters, sm_count,
+                                                    st, fluctuate == 2);
+    return launch_raster_batch<true, false, FIX>(g, d, n, id_base, seed, nsigma, grid, nullptr, counters, sm_count, st,
+                                                 fluctuate == 2);
 }
 
 cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
                                  double nsigma, float *S, int *depo_totals, Counters *counters, int sm_count,
                                  cudaStream_t st)
 {
-    if (n <= 0) return cudaSuccess;
-    if (!fluctuate) // no draws, no per-depo integer totals
-        return launch_raster_batch<false, false>(g, d, n, id_base, seed, nsigma, S, nullptr, counters, sm_count, st, false);
-    if (depo_totals)
-        return launch_raster_batch<true, true>(g, d, n, id_base, seed, nsigma, S, depo_totals, counters, sm_count, st,
-                                               fluctuate == 2);
-    return launch_raster_batch<true, false>(g, d, n, id_base, seed, nsigma, S, nullptr, counters, sm_count, st, fluctuate == 2);
+    return launch_raster_grid<false>(g, d, n, id_base, seed, fluctuate, nsigma, S, depo_totals, counters, sm_count, st);
+}
+
+cudaError_t launch_raster_fixed(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
+                                double nsigma, unsigned long long *fix, int *depo_totals, Counters *counters, int sm_count,
+                                cudaStream_t st)
+{
+    return launch_raster_grid<true>(g, d, n, id_base, seed, fluctuate, nsigma, reinterpret_cast<float *>(fix), depo_totals,
+                                    counters, sm_count, st);
 }
 
 cudaError_t launch_tile_count(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts, cudaStream_t st)

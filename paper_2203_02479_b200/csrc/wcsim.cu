@@ -295,7 +295,7 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
     if (!response || n_wires <= 0 || n_ticks <= 0 || n_rwires <= 0 || n_rticks <= 0 || (n_rwires % 2) == 0)
         return WCSIM_EINVAL;
     if (!(nsigma > 0.0f) || !std::isfinite(nsigma)) return WCSIM_EINVAL;
-    if (scatter_mode != WCSIM_SCATTER_ATOMIC && scatter_mode != WCSIM_SCATTER_TILED) return WCSIM_EINVAL;
+    if (scatter_mode < WCSIM_SCATTER_ATOMIC || scatter_mode > WCSIM_SCATTER_FIXED) return WCSIM_EINVAL;
     if (pad.wires < 0 || pad.ticks < 0) return WCSIM_EINVAL;
     const int c = (n_rwires - 1) / 2;
     const long long need_t = (long long)n_ticks + n_rticks - 1, need_w = (long long)n_wires + c;
@@ -405,15 +405,30 @@ int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n
         return raster_tiled(plan, g, d, n, depo_id_base, seed, fluctuate, dev_depo_totals);
     }
     if (dev_depo_totals) CU_TRY(cudaMemsetAsync(dev_depo_totals, 0, sizeof(int) * (size_t)n, plan->stream));
-    // the draw queues index per-depo totals with 24 bits: with totals requested, launch 2^24 depos at a time
-    const long long chunk = dev_depo_totals ? (1ll << 24) : n;
+    const bool fixed = plan->scatter_mode == WCSIM_SCATTER_FIXED;
+    if (fixed && !plan->ts.fix) { // first use of the fixed-point grid on this plan
+        const size_t bytes = sizeof(unsigned long long) * (size_t)g.n_wires * g.n_ticks;
+        CU_TRY(cudaMalloc((void **)&plan->ts.fix, bytes));
+        CU_TRY(cudaMemsetAsync(plan->ts.fix, 0, bytes, plan->stream));
+    }
+    // the draw queues index per-depo totals with 32 bits: with totals requested, launch 2^31 depos at a time
+    const long long chunk = dev_depo_totals ? (1ll << 31) : n;
     for (long long first = 0; first < n; first += chunk) {
         const long long m = n - first < chunk ? n - first : chunk;
         const DepoArrays dc{d.t0 + first, d.x0 + first, d.sigma_t + first, d.sigma_x + first, d.q + first};
         plan->launches += 1;
-        CU_TRY(launch_raster_atomic(g, dc, m, depo_id_base + (unsigned long long)first, seed, fluctuate, plan->nsigma,
-                                    plan->S, dev_depo_totals ? dev_depo_totals + first : nullptr, plan->counters,
-                                    plan->sm_count, plan->stream));
+        if (fixed)
+            CU_TRY(launch_raster_fixed(g, dc, m, depo_id_base + (unsigned long long)first, seed, fluctuate, plan->nsigma,
+                                       plan->ts.fix, dev_depo_totals ? dev_depo_totals + first : nullptr, plan->counters,
+                                       plan->sm_count, plan->stream));
+        else
+            CU_TRY(launch_raster_atomic(g, dc, m, depo_id_base + (unsigned long long)first, seed, fluctuate, plan->nsigma,
+                                        plan->S, dev_depo_totals ? dev_depo_totals + first : nullptr, plan->counters,
+                                        plan->sm_count, plan->stream));
+    }
+    if (fixed) {
+        plan->launches += 1;
+        CU_TRY(launch_tile_finalize(g, plan->ts, plan->S, plan->stream));
     }
     return WCSIM_OK;
 }
@@ -523,7 +538,7 @@ int wcsim_sync(wcsim_plan *plan)
 
 int wcsim_set_scatter_mode(wcsim_plan *plan, int scatter_mode)
 {
-    if (!plan || (scatter_mode != WCSIM_SCATTER_ATOMIC && scatter_mode != WCSIM_SCATTER_TILED)) return WCSIM_EINVAL;
+    if (!plan || scatter_mode < WCSIM_SCATTER_ATOMIC || scatter_mode > WCSIM_SCATTER_FIXED) return WCSIM_EINVAL;
     plan->scatter_mode = scatter_mode;
     return WCSIM_OK;
 }

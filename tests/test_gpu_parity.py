@@ -192,7 +192,7 @@ def _fluct_case(B, O, n_wires, n_ticks, R, depos, seed, id_base=0, mode=0):
     return S, S_ref
 
 
-@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("mode", [0, 1, 2])
 def test_fluctuation_integer_grid_exact(B, O, mode):
     from paper_2203_02479_b200 import synth
     cfg = synth.config(1, n_depos=20_000)
@@ -215,7 +215,7 @@ def test_fluctuation_negative_charge_big_ids_and_wide_patches(B, O):
     d["sigma_x"][25:30] = 0.0
     d["q"][30] = 0.2  # N = 0
     d["q"][31] = 0.5  # N = 1 (round half up)
-    for mode in (0, 1):
+    for mode in (0, 1, 2):
         _fluct_case(B, O, 64, 512, synth.response(3, 8), d, seed=0xDEADBEEFCAFE, id_base=(1 << 40) + 17, mode=mode)
 
 
@@ -270,19 +270,30 @@ def test_odd_tick_count_uses_scalar_rows(B, O):
         assert_close(p.output().cpu().numpy(), M_ref, "M odd ticks")
 
 
-def test_tiled_mode_is_bitwise_reproducible(B):
+@pytest.mark.parametrize("mode", [1, 2])
+def test_deterministic_modes_are_bitwise_reproducible(B, O, mode):
+    """fluctuation off (real-valued adds): the tiled and the fixed-point modes accumulate integers, so S is the same bit
+    for bit run after run, equal between the two modes, and within tolerance of the oracle"""
     from paper_2203_02479_b200 import synth
     cfg = synth.config(1, n_depos=30_000)
     pl = cfg["planes"][0]
     d = to_dev(pl["depos"])
     outs = []
-    with B.Plan(pl["n_wires"], pl["n_ticks"], synth.response(3, 8), scatter_mode=B.WCSIM_SCATTER_TILED) as p:
+    with B.Plan(pl["n_wires"], pl["n_ticks"], synth.response(3, 8), scatter_mode=mode) as p:
         for _ in range(3):
             p.clear()
             p.raster_scatter(d, fluctuate=False)
             p.sync()
             outs.append(p.charge().clone())
+        p.set_scatter_mode(3 - mode)  # the other deterministic mode
+        p.clear()
+        p.raster_scatter(d, fluctuate=False)
+        p.sync()
+        other = p.charge().clone()
     assert torch.equal(outs[0], outs[1]) and torch.equal(outs[0], outs[2])
+    assert torch.equal(outs[0], other)
+    S_ref, _, _ = O.raster_scatter(pl["n_wires"], pl["n_ticks"], pl["depos"], fluctuate=False)
+    assert_close(outs[0].cpu().numpy(), S_ref, "deterministic S")
 
 
 # ---------------------------------------------------------------------------------------------------------------
