@@ -276,6 +276,12 @@ def run_ours(args):
     if args.streams > 1 and world == 1:
         concurrent = concurrent_planes(args, B, cfg, pl, d, fluct, mode, dev, n_depos)
 
+    # configs[3] is an APA event: three planes with their own responses, noise on every one.  Extra figure: whole events,
+    # the three planes of an event on three plans/streams (planes are independent)
+    apa = None
+    if len(cfg["planes"]) > 1 and world == 1:
+        apa = apa_events(args, B, cfg, fluct, mode, dev)
+
     # ---- roofline of the dominant kernel --------------------------------------------------------------------------
     peaks = load_peaks()
     direct = args.wires == "direct" or (args.wires == "auto" and pl["response"].shape[0] <= 64)
@@ -355,6 +361,8 @@ def run_ours(args):
     }
     if concurrent:
         out["concurrent"] = concurrent
+    if apa:
+        out["apa_event"] = apa
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(cfg, budget_s=args.cpu_budget)
     if rank == 0 and world == 1 and args.cufft:
@@ -414,6 +422,45 @@ def concurrent_planes(args, B, cfg, pl, d, fluct, mode, dev, n_depos):
         p.destroy()
     return {"streams": n, "steps": args.steps, "ms_per_step": ms / args.steps, "value": n_depos * args.steps / (ms * 1e-3),
             "unit": UNIT, "what": "independent plane-events in flight on %d streams (throughput, not latency)" % n}
+
+
+def apa_events(args, B, cfg, fluct, mode, dev):
+    """K whole events of a multi-plane config: plane p of every event on plan/stream p; one CUDA-event pair around all."""
+    import torch
+    planes = cfg["planes"]
+    streams = [torch.cuda.Stream(device=dev) for _ in planes]
+    plans = [B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]), nsigma=cfg["nsigma"],
+                    scatter_mode=mode, stream=st) for pl, st in zip(planes, streams)]
+    depos = [{k: torch.from_numpy(v).to(dev) for k, v in pl["depos"].items()} for pl in planes]
+    n_depos = sum(int(pl["depos"]["t0"].shape[0]) for pl in planes)
+    main = torch.cuda.current_stream()
+
+    def run(k):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record(main)
+        for st in streams:
+            st.wait_event(a)
+        for _ in range(k):
+            for p, d in zip(plans, depos):
+                p.clear()
+                p.raster_scatter(d, seed=cfg["fluct_seed"], fluctuate=fluct)
+                if cfg.get("noise"):
+                    p.arm_noise(None, seed=cfg["noise_seed"])
+                p.convolve()
+        for st in streams:
+            main.wait_stream(st)
+        b.record(main)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b)
+
+    run(3)
+    ms = run(args.steps)
+    for p in plans:
+        p.destroy()
+    return {"planes": len(planes), "depos_per_event": n_depos, "events": args.steps, "ms_per_event": ms / args.steps,
+            "value": n_depos * args.steps / (ms * 1e-3), "unit": UNIT,
+            "what": "whole events, plane p on plan/stream p (raster + fused noise + convolve per plane)"}
 
 
 def cufft_comparator(pl, dev, flush):
