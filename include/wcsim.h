@@ -105,7 +105,8 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
  * Bins outside the grid are dropped and not drawn (A5).  S accumulates across calls; wcsim_clear zeroes it.
  *   depos           : struct of DEVICE pointers (the struct itself is read on the host during the call).
  *   dev_depo_totals : DEVICE, n int32, or NULL.  With fluctuate = 1 or 2 receives the signed sum of each depo's draws.
- * n = 0 is valid and does nothing.
+ * n = 0 is valid and does nothing.  In WCSIM_SCATTER_TILED mode the call synchronises the stream once (the size of the
+ * per-tile depo lists is read back before they are filled) and n must be < 2^32; the other modes only enqueue.
  */
 int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n, unsigned long long depo_id_base,
                          unsigned long long seed, int fluctuate, int *dev_depo_totals);
