@@ -300,7 +300,8 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
     const int c = (n_rwires - 1) / 2;
     const long long need_t = (long long)n_ticks + n_rticks - 1, need_w = (long long)n_wires + c;
     const int pad_t = pad.ticks ? pad.ticks : next_pow2(need_t, 32);
-    const int pad_w = pad.wires ? pad.wires : next_pow2(need_w, 16);
+    // automatic wire padding also keeps the wrapped response from overlapping itself (pad_w >= n_rwires)
+    const int pad_w = pad.wires ? pad.wires : next_pow2(need_w > n_rwires ? need_w : (long long)n_rwires, 16);
     if (!is_pow2(pad_t) || !is_pow2(pad_w) || pad_t < need_t || pad_w < need_w || pad_t < 32 || pad_w < 16)
         return WCSIM_EINVAL;
     if (pad_w < n_rwires) return WCSIM_EINVAL; // the wrapped response must not overlap itself

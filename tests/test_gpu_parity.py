@@ -235,7 +235,7 @@ def test_raster_edge_cases(B, O):
     }
     S_ref, _, st_ref = O.raster_scatter(64, 512, depos, fluctuate=False)
     assert st_ref["skipped"] == 3
-    for mode in (0, 1):
+    for mode in (0, 1, 2):
         with B.Plan(64, 512, synth.response(3, 8), scatter_mode=mode) as p:
             p.raster_scatter(to_dev(depos), fluctuate=False)
             p.sync()
@@ -559,3 +559,40 @@ def test_digitize_matches_oracle_bit_for_bit(B, O):
             assert ref.min() >= 0 and ref.max() <= 2 ** bits - 1 and len(np.unique(ref)) > 3
         with pytest.raises(B.WcsimError):
             p.digitize(1.0, 0.0, 16)
+
+
+def test_degenerate_grids_and_responses(B, O):
+    """one wire, two ticks, a 1 x 1 response; a response as wide as the plane; an all-invalid and an all-off-grid depo list"""
+    f = np.float32
+    one = {k: np.array([v], dtype=f) for k, v in (("t0", 0.9), ("x0", 0.5), ("sigma_t", 0.4), ("sigma_x", 0.3), ("q", 800.0))}
+    R11 = np.array([[2.5]], dtype=f)
+    with B.Plan(1, 2, R11) as p:
+        p.raster_scatter(to_dev(one), seed=3, fluctuate=True)
+        p.convolve()
+        p.sync()
+        S = p.charge().cpu().numpy().astype(np.float64)
+        S_ref, _, _ = O.raster_scatter(1, 2, one, seed=3, fluctuate=True)
+        assert np.array_equal(S, S_ref)
+        assert_close(p.output().cpu().numpy(), 2.5 * S_ref, "1 x 1 response")
+    # response spanning more wires than the plane has (c = 10 > n_wires = 4)
+    from paper_2203_02479_b200 import synth
+    R = synth.response(21, 40)
+    d = {k: np.array(v, dtype=f) for k, v in (("t0", [20.2, 33.7]), ("x0", [1.4, 3.2]), ("sigma_t", [1.0, 2.0]),
+                                              ("sigma_x", [0.5, 0.9]), ("q", [5000.0, -7000.0]))}
+    with B.Plan(4, 64, R) as p:
+        p.raster_scatter(to_dev(d), fluctuate=False)
+        p.convolve()
+        p.sync()
+        S_ref, _, _ = O.raster_scatter(4, 64, d, fluctuate=False)
+        assert_close(p.charge().cpu().numpy(), S_ref, "narrow plane S")
+        assert_close(p.output().cpu().numpy(), O.convolve_direct(S_ref, R), "response wider than the plane")
+    bad = {"t0": np.array([np.nan, -1e4, 5.0], dtype=f), "x0": np.array([1.0, 1.0, 1e6], dtype=f),
+           "sigma_t": np.array([1.0, 1.0, 1.0], dtype=f), "sigma_x": np.array([1.0, 1.0, 1.0], dtype=f),
+           "q": np.array([1.0, 1e4, 1e4], dtype=f)}
+    for mode in (0, 1, 2):
+        with B.Plan(8, 64, synth.response(3, 8), scatter_mode=mode) as p:
+            p.raster_scatter(to_dev(bad), seed=1, fluctuate=True)
+            p.convolve()
+            p.sync()
+            assert float(p.charge().abs().max()) == 0.0 and float(p.output().abs().max()) == 0.0
+            assert p.stats() == {"depos_skipped": 1, "bins_drawn": 0}
