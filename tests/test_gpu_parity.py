@@ -596,3 +596,44 @@ def test_degenerate_grids_and_responses(B, O):
             p.sync()
             assert float(p.charge().abs().max()) == 0.0 and float(p.output().abs().max()) == 0.0
             assert p.stats() == {"depos_skipped": 1, "bins_drawn": 0}
+
+
+def test_random_shapes_sweep(B, O):
+    """Seeded sweep over grid shapes, response footprints, truncation widths, scatter modes, wire modes and samplers:
+    S against the oracle (integer grids exactly), M against the definition."""
+    from paper_2203_02479_b200 import synth
+    rng = np.random.default_rng(2024)
+    for case in range(24):
+        nw = int(rng.integers(1, 90))
+        nt = int(rng.integers(2, 700))
+        n_rw = int(rng.choice([1, 3, 5, 9, 21, 41, 65, 67]))
+        n_rt = int(rng.integers(1, 60))
+        nsigma = float(rng.choice([0.5, 1.0, 3.0, 4.5]))
+        mode = int(rng.integers(0, 3))
+        fluct = int(rng.integers(0, 3))
+        wire_mode = int(rng.choice([B.WCSIM_WIRES_AUTO, B.WCSIM_WIRES_FFT, B.WCSIM_WIRES_DIRECT]))
+        n = int(rng.integers(1, 400))
+        R = (rng.normal(0, 1, (n_rw, n_rt)) * np.exp(-np.arange(n_rt) / 10.0)).astype(np.float32)
+        d = {"t0": rng.uniform(-5, nt + 5, n), "x0": rng.uniform(-2, nw + 2, n), "sigma_t": rng.uniform(0, 4, n),
+             "sigma_x": rng.uniform(0, 2.5, n), "q": rng.lognormal(np.log(3000), 1.0, n) * rng.choice([-1, 1], n)}
+        d = {k: v.astype(np.float32) for k, v in d.items()}
+        what = "case %d: %dx%d R %dx%d nsigma %g scatter %d fluct %d wires %d n %d" % (case, nw, nt, n_rw, n_rt, nsigma, mode,
+                                                                                        fluct, wire_mode, n)
+        S_ref, tot_ref, st = O.raster_scatter(nw, nt, d, seed=case, fluctuate=fluct, nsigma=nsigma, want_totals=True)
+        totals = torch.zeros(n, dtype=torch.int32, device="cuda")
+        with B.Plan(nw, nt, R, nsigma=nsigma, scatter_mode=mode) as p:
+            p.set_wire_mode(wire_mode)
+            p.raster_scatter(to_dev(d), seed=case, fluctuate=fluct, dev_depo_totals=totals)
+            p.convolve()
+            p.sync()
+            S = p.charge().cpu().numpy().astype(np.float64)
+            M = p.output().cpu().numpy()
+            assert p.stats()["bins_drawn"] == st["drawn"], what
+        if fluct:
+            assert np.array_equal(S, S_ref), what
+            assert np.array_equal(totals.cpu().numpy(), tot_ref), what
+        elif np.abs(S_ref).max() > 0:
+            assert_close(S, S_ref, what)
+        M_ref = O.convolve_direct(S_ref, R)
+        if np.abs(M_ref).max() > 0:
+            assert_close(M, M_ref, what)
