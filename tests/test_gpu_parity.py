@@ -637,3 +637,34 @@ def test_random_shapes_sweep(B, O):
         M_ref = O.convolve_direct(S_ref, R)
         if np.abs(M_ref).max() > 0:
             assert_close(M, M_ref, what)
+
+
+def test_every_fft_size_of_both_axes(B, O):
+    """Every supported transform length: pad_t = 32 .. 32768 on the tick axis (row kernels, plain and TMA-staged) and
+    pad_w = 16 .. 8192 on the wire axis (cols_kernel and the direct wire pass), on sparse S so that the oracle's plain
+    double sum stays cheap; sampled outputs where the grid is large."""
+    rng = np.random.default_rng(77)
+    cases = [(3, pt - 10, 16, pt, 3, 9) for pt in (32, 64, 128, 256, 512, 1024, 2048, 4096, 8192, 16384, 32768)]
+    cases += [(pw - 3, 20, pw, 32, 5, 4) for pw in (16, 32, 64, 128, 256, 512, 1024, 2048, 4096, 8192)]
+    for (nw, nt, pw, pt, rw, rt) in cases:
+        R = rng.normal(0, 1, (rw, rt)).astype(np.float32)
+        S = np.zeros((nw, nt), dtype=np.float32)
+        k = min(300, nw * nt)
+        S.ravel()[rng.choice(nw * nt, k, replace=False)] = rng.normal(0, 100, k).astype(np.float32)
+        n_pts = min(3000, nw * nt)
+        flat = rng.choice(nw * nt, n_pts, replace=False)
+        px, pt_ = flat // nt, flat % nt
+        ref = O.convolve_points(S.astype(np.float64), R, px, pt_)
+        with B.Plan(nw, nt, R, pad=(pw, pt)) as p:
+            p.charge().copy_(torch.from_numpy(S).cuda())
+            for mode in (B.WCSIM_WIRES_FFT, B.WCSIM_WIRES_DIRECT):
+                p.set_wire_mode(mode)
+                p.clear_output()
+                p.convolve()
+                p.sync()
+                M = p.output().cpu().numpy()
+                got = M[px, pt_].astype(np.float64)
+                scale = max(float(np.abs(ref).max()), float(np.abs(M).max()))
+                what = "pad %dx%d wire mode %d" % (pw, pt, mode)
+                assert np.max(np.abs(got - ref)) <= MAX_ABS * scale, what
+                assert np.linalg.norm(got - ref) <= REL_L2 * max(np.linalg.norm(ref), 1e-30), what
