@@ -668,3 +668,21 @@ def test_every_fft_size_of_both_axes(B, O):
                 what = "pad %dx%d wire mode %d" % (pw, pt, mode)
                 assert np.max(np.abs(got - ref)) <= MAX_ABS * scale, what
                 assert np.linalg.norm(got - ref) <= REL_L2 * max(np.linalg.norm(ref), 1e-30), what
+
+
+@pytest.mark.parametrize("nt,pad_t", [(40, 64), (200, 256), (1000, 2048), (9000, 16384), (701, 1024)])
+def test_noise_every_row_kernel(B, O, nt, pad_t):
+    """the noise of step a7 through each inverse-row kernel: plain (short, long and odd-length rows) and TMA-staged"""
+    from paper_2203_02479_b200 import synth
+    nw = 6
+    R = synth.response(3, 8)
+    ref = O.noise_add(np.zeros((nw, nt)), pad_t, seed=21)
+    with B.Plan(nw, nt, R, pad=(16, pad_t)) as p:
+        p.arm_noise(None, seed=21)
+        p.convolve()  # S = 0: M = N, fused into the inverse rows
+        p.sync()
+        assert_close(p.output().cpu().numpy(), ref, "fused noise pad_t %d" % pad_t, rel=2e-5)
+        p.clear_output()
+        p.add_noise(seed=21)  # standalone pass
+        p.sync()
+        assert_close(p.output().cpu().numpy(), ref, "standalone noise pad_t %d" % pad_t, rel=2e-5)
