@@ -441,8 +441,14 @@ __device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const S
                     if constexpr (TOT) Q.depo[cls][pos] = (uint32_t)dio;
                 }
                 __syncwarp();
+                // counts stay below 64, so some queue holds a full warp iff the OR of the counts has bit 5 set
+                int any_full = 0;
 #pragma unroll
-                for (int c = 0; c < kNumDrawQueues; ++c) drain_queue(Q, c, qcount[c], false, sink, totals, lane);
+                for (int c = 0; c < kNumDrawQueues; ++c) any_full |= qcount[c];
+                if (any_full & 32) {
+#pragma unroll
+                    for (int c = 0; c < kNumDrawQueues; ++c) drain_queue(Q, c, qcount[c], false, sink, totals, lane);
+                }
             } else {
                 const float qq = __shfl_sync(0xffffffffu, q, own);
                 if (act) sink.add(wire, tick, qq * (wt * wx));
