@@ -184,7 +184,7 @@ __device__ __forceinline__ double draw_inversion(double N, double p, uint32_t w)
     const double r = fast_div(p, 1.0 - p), rN1 = r * (N + 1.0);
     double kd = 0.0;
     bool go = u > c && kd < N;
-    for (int k = 1; __any_sync(__activemask(), go); ++k) {
+    auto step = [&](int k) {
         const double rk = k < kInvTable ? c_inv_k[k] : 1.0 / (double)k;
         if (go) {
             kd += 1.0;
@@ -192,6 +192,10 @@ __device__ __forceinline__ double draw_inversion(double N, double p, uint32_t w)
             c += f;
             go = u > c && kd < N;
         }
+    };
+    for (int k = 1; __any_sync(__activemask(), go); k += 2) { // two terms per vote (four: slower, 73.4 -> 75.7 us)
+        step(k);
+        step(k + 1);
     }
     return kd;
 }
