@@ -59,7 +59,7 @@ def lib():
         L.wco_patch_axes.restype = C.c_int
         L.wco_raster_scatter.argtypes = [C.c_int, C.c_int, f32p, f32p, f32p, f32p, f32p, C.c_int64, u64p, C.c_uint64,
                                          C.c_uint64, C.c_int, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, f64p,
-                                         i32p, i64p]
+                                         i32p, i64p, C.c_int]
         L.wco_raster_scatter.restype = C.c_int
         L.wco_convolve_direct.argtypes = [C.c_int, C.c_int, f64p, f64p, C.c_int, C.c_int, f64p]
         L.wco_convolve_direct.restype = C.c_int
@@ -203,7 +203,7 @@ def _fluct_mode(fluctuate) -> int:
 
 
 def raster_scatter(n_wires, n_ticks, depos, *, seed=0, fluctuate=False, nsigma=3.0, ids=None, id_base=0,
-                   window=None, want_totals=False, S=None):
+                   window=None, want_totals=False, S=None, normalize=False):
     """depos = dict(t0,x0,sigma_t,sigma_x,q) of float arrays.  Returns (S_window fp64, totals|None, stats)."""
     t0, x0, st, sx, q = (_f32(depos[k]) for k in ("t0", "x0", "sigma_t", "sigma_x", "q"))
     n = t0.shape[0]
@@ -221,7 +221,8 @@ def raster_scatter(n_wires, n_ticks, depos, *, seed=0, fluctuate=False, nsigma=3
     rc = lib().wco_raster_scatter(n_wires, n_ticks, _p(t0, C.c_float), _p(x0, C.c_float), _p(st, C.c_float),
                                   _p(sx, C.c_float), _p(q, C.c_float), n, idp, id_base, seed, _fluct_mode(fluctuate),
                                   float(nsigma), w0, w1, k0, k1, _p(S, C.c_double),
-                                  _p(totals, C.c_int32) if want_totals else None, _p(stats, C.c_int64))
+                                  _p(totals, C.c_int32) if want_totals else None, _p(stats, C.c_int64),
+                                  int(bool(normalize)))
     if rc != 0:
         raise ValueError("wco_raster_scatter rc=%d" % rc)
     return S, totals, {"skipped": int(stats[0]), "drawn": int(stats[1])}

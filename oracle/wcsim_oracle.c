@@ -185,6 +185,17 @@ double wco_binomial(double N, double p, uint32_t w)
 /* "as a patch").  Readings A1 (bin k covers [k,k+1)), A2 (extent snapped      */
 /* outward), A3 (no renormalisation), A4 (sigma -> 0).                         */
 /* ------------------------------------------------------------------------- */
+/* Sum of the axis weights over the whole extent [i0, i1) of reading A2, from its two outer edges (the sum of
+ * differences of erf telescopes; the pin O2 of the tests checks that identity): the norm of reading A24. */
+double wco_axis_norm(int64_t i0, int64_t i1, double centre, double sigma)
+{
+    if (sigma < 1e-6) return 1.0;
+    double s = sqrt(2.0) * sigma;
+    double hi = erf(((double)i1 - centre) / s);
+    double lo = erf(((double)i0 - centre) / s);
+    return 0.5 * (hi - lo);
+}
+
 void wco_axis_extent(double centre, double sigma, double nsigma, int64_t *i0, int64_t *i1)
 {
     *i0 = (int64_t)floor(centre - nsigma * sigma);
@@ -318,6 +329,9 @@ int wco_drift(const float *x, const float *y, const float *z, const float *t, co
 /* fluctuate = 0: c = Q p.   fluctuate = 1: Ntr = floor(|Q| + 1/2),             */
 /* c = sign(Q) B(Ntr, p, word(seed, id, g)), g = wire*n_ticks + tick (A6-A9).   */
 /* fluctuate = 2: the same with the normal-approximation draw G (A21).          */
+/* normalize != 0 (reading A24): p_ij = (wt_i wx_j) / (W_t W_x)  */
+/* with W the sum of the axis weights over the whole +-n sigma extent, so that */
+/* a patch inside the grid carries exactly Q (fluctuation off).                */
 /* ids == NULL means depo i has id id_base + i.                                */
 /* totals (optional, n entries): signed sum of the draws over all in-grid bins */
 /* of each depo (forces drawing outside the window too).                       */
@@ -326,7 +340,7 @@ int wco_drift(const float *x, const float *y, const float *z, const float *t, co
 int wco_raster_scatter(int n_wires, int n_ticks,
                        const float *t0, const float *x0, const float *sigma_t, const float *sigma_x, const float *q,
                        int64_t n, const uint64_t *ids, uint64_t id_base, uint64_t seed, int fluctuate, double nsigma,
-                       int w0, int w1, int k0, int k1, double *Swin, int32_t *totals, int64_t *stats)
+                       int w0, int w1, int k0, int k1, double *Swin, int32_t *totals, int64_t *stats, int normalize)
 {
     if (n_wires <= 0 || n_ticks <= 0 || n < 0 || !(nsigma > 0.0)) return -1;
     if (w0 < 0 || w1 > n_wires || k0 < 0 || k1 > n_ticks || w0 > w1 || k0 > k1) return -1;
@@ -342,6 +356,7 @@ int wco_raster_scatter(int n_wires, int n_ticks,
         wco_axis_extent(X0, SX, nsigma, &ix0, &ix1);
         double Ntr = floor(fabs(Q) + 0.5);
         double sgn = (Q < 0.0) ? -1.0 : 1.0;
+        double norm = normalize ? wco_axis_norm(it0, it1, T0, ST) * wco_axis_norm(ix0, ix1, X0, SX) : 1.0;
         int64_t tot = 0;
         for (int64_t j = ix0; j < ix1; ++j) {
             if (j < 0 || j >= n_wires) continue;
@@ -354,6 +369,7 @@ int wco_raster_scatter(int n_wires, int n_ticks,
                 if (!in_win && !totals) continue;
                 double wti = wco_axis_weight(i, T0, ST);
                 double p = wti * wxj;
+                if (normalize) p = p / norm;
                 double c;
                 if (fluctuate) {
                     uint64_t g = (uint64_t)j * (uint64_t)n_ticks + (uint64_t)i;

@@ -185,3 +185,48 @@ def test_invalid_depos_are_skipped_and_counted():
          "sigma_x": [1.0, 1.0, 1.0, 1.0], "q": [100.0, 100.0, 100.0, 100.0]}
     S, _, st = oracle.raster_scatter(16, 32, d)
     assert st["skipped"] == 3 and np.isfinite(S).all() and S.sum() > 90
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# reading A24: renormalised patches (second half)
+# ---------------------------------------------------------------------------------------------------------------
+def test_normalized_patch_carries_exactly_q_inside_the_grid():
+    rng = np.random.default_rng(31)
+    n = 300
+    d = {"t0": rng.uniform(40, 460, n), "x0": rng.uniform(12, 52, n), "sigma_t": rng.uniform(0.0, 3.0, n),
+         "sigma_x": rng.uniform(0.0, 2.0, n), "q": rng.lognormal(np.log(5000), 0.5, n) * rng.choice([-1, 1], n)}
+    d = {k: v.astype(np.float32) for k, v in d.items()}
+    d["sigma_t"][:5] = 0.0
+    for i in range(0, n, 37):  # one depo at a time: its bins sum to Q within fp64 rounding of ~100 adds
+        one = {k: v[i:i + 1] for k, v in d.items()}
+        S, _, _ = oracle.raster_scatter(64, 512, one, fluctuate=False, normalize=True)
+        assert abs(S.sum() - float(one["q"][0])) <= 1e-12 * abs(float(one["q"][0]))
+        S0, _, _ = oracle.raster_scatter(64, 512, one, fluctuate=False, normalize=False)
+        assert abs(S0.sum()) <= abs(S.sum()) and abs(S0.sum()) >= 0.9946 ** 1 * 0.9946 * abs(S.sum()) - 1e-9
+        # same shape, rescaled by one number
+        nz = S0 != 0
+        ratio = S[nz] / S0[nz]
+        assert np.allclose(ratio, ratio[0], rtol=1e-12)
+
+
+def test_normalization_uses_the_whole_extent_not_the_part_inside_the_grid():
+    """a depo at the grid edge loses the charge that falls outside (A5) also when normalised"""
+    one = {k: np.array([v], dtype=np.float32) for k, v in (("t0", 0.25), ("x0", 5.5), ("sigma_t", 2.0), ("sigma_x", 0.5), ("q", 1000.0))}
+    S, _, _ = oracle.raster_scatter(16, 64, one, fluctuate=False, normalize=True)
+    from scipy.special import erf
+    inside = 0.5 * (1.0 + erf(0.25 / (np.sqrt(2.0) * 2.0)))  # mass at t >= 0 of a Gaussian centred at 0.3 ... truncated at 3 sigma
+    lo, hi = np.floor(0.25 - 6.0), np.floor(0.25 + 6.0) + 1
+    W = 0.5 * (erf((hi - 0.25) / (np.sqrt(2) * 2)) - erf((lo - 0.25) / (np.sqrt(2) * 2)))
+    part = 0.5 * (erf((hi - 0.25) / (np.sqrt(2) * 2)) - erf((0 - 0.25) / (np.sqrt(2) * 2)))
+    assert abs(S.sum() - 1000.0 * part / W) < 1e-9 * 1000.0
+    assert S.sum() < 600.0 and inside > 0.5
+
+
+def test_normalized_fluctuation_mean():
+    rng = np.random.default_rng(33)
+    one = {k: np.full(400, v, dtype=np.float32) for k, v in (("t0", 100.4), ("x0", 20.6), ("sigma_t", 1.3), ("sigma_x", 0.6), ("q", 8000.0))}
+    S, tot, _ = oracle.raster_scatter(64, 256, one, seed=9, fluctuate=True, normalize=True, want_totals=True)
+    # independent binomials with sum p = 1: E[total] = N, var = sum N p (1-p) < N
+    assert abs(tot.mean() - 8000.0) < 4 * np.sqrt(8000.0 / 400)
+    S0, tot0, _ = oracle.raster_scatter(64, 256, one, seed=9, fluctuate=True, normalize=False, want_totals=True)
+    assert tot0.mean() < tot.mean() - 2  # without it the charge beyond the extent (0.06 % here) is truncated away
