@@ -111,6 +111,12 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
 int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n, unsigned long long depo_id_base,
                          unsigned long long seed, int fluctuate, int *dev_depo_totals);
 
+/* Renormalised patches (reading A24; PAPER.md:56 leaves the patch normalisation open): with `on` != 0
+ * later wcsim_raster_scatter calls use p_ij = (wt_i wx_j) / (W_t W_x), W the sum of the axis weights over the whole
+ * +-nsigma extent, so a patch that lies inside the grid carries exactly q (fluctuate = 0) or has sum p = 1.  Charge
+ * falling outside the grid is still dropped (A5).  Default: off (reading A3). */
+int wcsim_set_normalize(wcsim_plan *plan, int on);
+
 /*
  * a4-a6 Convolution by Eq. (2): M = crop(irfft2(Rhat * rfft2(zero_pad(S)))).  S is preserved.
  * Equals the linear convolution of Eq. (1) on the n_wires x n_ticks window exactly, up to fp32 rounding (A10-A13).

@@ -23,7 +23,7 @@ SYMBOLS = [
     "wcsim_plan_destroy", "wcsim_clear", "wcsim_clear_output", "wcsim_sync", "wcsim_set_scatter_mode", "wcsim_set_wire_mode",
     "wcsim_charge_ptr", "wcsim_output_ptr", "wcsim_get_dims", "wcsim_get_stats", "wcsim_reset_stats",
     "wcsim_simulate_host", "wcsim_set_profiling", "wcsim_get_stage_times", "wcsim_get_launch_count",
-    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf", "wcsim_simulate_host_async", "wcsim_debug_normal_draw", "wcsim_drift", "wcsim_digitize",
+    "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf", "wcsim_simulate_host_async", "wcsim_debug_normal_draw", "wcsim_drift", "wcsim_digitize", "wcsim_set_normalize",
     "wcsim_strerror", "wcsim_last_cuda_error", "wcsim_version",
 ]
 
@@ -78,6 +78,7 @@ def lib():
         L.wcsim_sync.argtypes = [vp]
         L.wcsim_set_scatter_mode.argtypes = [vp, i]
         L.wcsim_set_wire_mode.argtypes = [vp, i]
+        L.wcsim_set_normalize.argtypes = [vp, i]
         L.wcsim_charge_ptr.argtypes = [vp, C.POINTER(vp)]
         L.wcsim_output_ptr.argtypes = [vp, C.POINTER(vp)]
         L.wcsim_get_dims.argtypes = [vp] + [C.POINTER(i)] * 4
@@ -221,6 +222,10 @@ def wcsim_sync(plan):
 
 def wcsim_set_scatter_mode(plan, scatter_mode):
     _check(lib().wcsim_set_scatter_mode(plan, int(scatter_mode)), "wcsim_set_scatter_mode")
+
+
+def wcsim_set_normalize(plan, on):
+    _check(lib().wcsim_set_normalize(plan, int(bool(on))), "wcsim_set_normalize")
 
 
 def wcsim_set_wire_mode(plan, wire_mode):
@@ -412,6 +417,9 @@ class Plan:
 
     def set_scatter_mode(self, mode):
         wcsim_set_scatter_mode(self.handle, mode)
+
+    def set_normalize(self, on):
+        wcsim_set_normalize(self.handle, on)
 
     def set_wire_mode(self, mode):
         wcsim_set_wire_mode(self.handle, mode)

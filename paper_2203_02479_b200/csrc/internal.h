@@ -22,6 +22,9 @@ struct Counters {
 };
 
 // ---- raster.cu ----
+// `fluctuate` of the launchers below: 0 off, 1 binomial (A6), 2 normal approximation (A21), plus kRasterNormalize for
+// renormalised patches (A24)
+constexpr int kRasterNormalize = 4;
 cudaError_t raster_configure(cudaStream_t st); // erf table and shared-memory attributes of the raster kernels (per plan)
 void erf_table_host(const double *z, double *out, long long n); // the table erf of erf_table.cuh, evaluated on the host
 // a1-a3, atomic mode: S[wire][tick] += patch of every depo (red.global.add.f32)

@@ -71,6 +71,15 @@ __device__ __forceinline__ bool depo_valid(float t0, float x0, float st, float s
     return isfinite(t0) && isfinite(x0) && isfinite(st) && isfinite(sx) && isfinite(q) && st >= 0.0f && sx >= 0.0f;
 }
 
+// sum of the axis weights over the whole extent floor(c - n s) .. floor(c + n s) + 1, from its two outer edges (A24)
+__device__ __forceinline__ double axis_norm(double centre, double sigma, double nsigma)
+{
+    if (sigma < 1e-6) return 1.0;
+    const double h = __dmul_rn(nsigma, sigma), s = 1.4142135623730951 * sigma;
+    const double lo = floor(__dsub_rn(centre, h)), hi = __dadd_rn(floor(__dadd_rn(centre, h)), 1.0);
+    return 0.5 * (erf_from_table(g_erf_tab, fast_div(hi - centre, s)) - erf_from_table(g_erf_tab, fast_div(lo - centre, s)));
+}
+
 // weights of bins base .. base+30 in lanes 0 .. 30:  1/2 [erf((i+1-c)/(sqrt2 s)) - erf((i-c)/(sqrt2 s))]   (A1, A4)
 template <typename T>
 __device__ __forceinline__ T axis_weights(int base, double centre, double sigma, int lane)
@@ -163,7 +172,7 @@ template <bool FLUCT, typename Sink>
 __device__ __forceinline__ unsigned int raster_depo(float t0f, float x0f, float stf, float sxf, float qf, uint64_t id,
                                                     uint64_t seed, double nsigma, int n_ticks, int w_lo, int w_hi,
                                                     int k_lo, int k_hi, const Sink &sink, int lane, int *lane_total,
-                                                    bool normal_only)
+                                                    bool normal_only, double inv_norm)
 {
     using T = typename std::conditional<FLUCT, double, float>::type;
     const double T0 = t0f, X0 = x0f, ST = stf, SX = sxf;
@@ -186,7 +195,7 @@ __device__ __forceinline__ unsigned int raster_depo(float t0f, float x0f, float 
                     const int wire = xc + j;
                     ++drawn;
                     if constexpr (FLUCT) {
-                        const double p = __dmul_rn(wt, wxj);
+                        const double p = __dmul_rn(wt, wxj) * inv_norm; // inv_norm = 1 unless patches are renormalised (A24)
                         const uint64_t g = (uint64_t)wire * (uint64_t)n_ticks + (uint64_t)tick;
                         const uint4 words = fluct_words(seed, id, g >> 2);
                         const double k = binomial_draw(Ntr, p, pick_word(words, (uint32_t)g & 3u), normal_only);
@@ -196,7 +205,7 @@ __device__ __forceinline__ unsigned int raster_depo(float t0f, float x0f, float 
                             sink.add(wire, tick, (float)v);
                         }
                     } else {
-                        sink.add(wire, tick, qf * (wt * wxj));
+                        sink.add(wire, tick, qf * (wt * wxj) * (float)inv_norm);
                     }
                 }
             }
@@ -305,7 +314,7 @@ __device__ __forceinline__ void drain_queue(DrawQueues<TOT> &Q, int cls, int &co
 template <bool FLUCT, bool TOT, bool INDIRECT, typename Sink>
 __device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const Sink &sink, float t0, float x0, float st,
                                                   float sx, float q, bool valid, long long dbase, uint32_t dl,
-                                                  uint64_t id_base, uint64_t seed, double nsigma, bool normal_only,
+                                                  uint64_t id_base, uint64_t seed, double nsigma, bool normal_only, bool normalize,
                                                   int *__restrict__ totals, BatchScratch<FLUCT> &sc,
                                                   DrawQueues<TOT> *queues, int (&qcount)[kNumDrawQueues],
                                                   unsigned long long &drawn, int lane)
@@ -322,6 +331,9 @@ __device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const S
         ex = axis_extent(X0, SX, nsigma, clip.w_lo, clip.w_hi);
     }
     const bool live = et.lo < et.hi && ex.lo < ex.hi;
+    // renormalised patches (reading A24): 1 / (W_t W_x), W = the axis weights summed over the whole, unclipped extent
+    double inv_norm = 1.0;
+    if (normalize && live) inv_norm = __ddiv_rn(1.0, axis_norm(T0, ST, nsigma) * axis_norm(X0, SX, nsigma));
     const int nt = live ? et.hi - et.lo : 0, nx = live ? ex.hi - ex.lo : 0;
     const bool big = nt + nx + 2 > kEdgeCap || (long long)nt * nx > (1 << 24);
     const int ne = (live && !big) ? nt + nx + 2 : 0, nb = (live && !big) ? nt * nx : 0;
@@ -346,7 +358,8 @@ __device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const S
         drawn += raster_depo<FLUCT>(__shfl_sync(0xffffffffu, t0, src), __shfl_sync(0xffffffffu, x0, src),
                                     __shfl_sync(0xffffffffu, st, src), __shfl_sync(0xffffffffu, sx, src),
                                     __shfl_sync(0xffffffffu, q, src), id_base + (uint64_t)depo_of(src), seed,
-                                    nsigma, g.n_ticks, clip.w_lo, clip.w_hi, clip.k_lo, clip.k_hi, sink, lane, &tot, normal_only);
+                                    nsigma, g.n_ticks, clip.w_lo, clip.w_hi, clip.k_lo, clip.k_hi, sink, lane, &tot, normal_only,
+                                    normalize ? __shfl_sync(0xffffffffu, inv_norm, src) : 1.0);
         if (totals != nullptr) {
             tot = warp_sum(tot);
             if (lane == 0 && tot != 0) atomicAdd(totals + depo_of(src), tot);
@@ -408,6 +421,7 @@ __device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const S
                 const double Nn = (double)__shfl_sync(0xffffffffu, Ntr, own);
                 const float qq = __shfl_sync(0xffffffffu, q, own);
                 double p = __dmul_rn(wt, wx);
+                if (normalize) p *= __shfl_sync(0xffffffffu, inv_norm, own);
                 const uint64_t gbin = (uint64_t)wire * (uint64_t)g.n_ticks + (uint64_t)tick;
                 const long long dio = depo_of(own);
                 const uint64_t id = id_base + (uint64_t)dio;
@@ -451,7 +465,8 @@ __device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const S
                 }
             } else {
                 const float qq = __shfl_sync(0xffffffffu, q, own);
-                if (act) sink.add(wire, tick, qq * (wt * wx));
+                const float scale = normalize ? (float)__shfl_sync(0xffffffffu, inv_norm, own) : 1.0f;
+                if (act) sink.add(wire, tick, qq * (wt * wx) * scale);
             }
         }
         __syncwarp();
@@ -463,7 +478,7 @@ template <bool FLUCT, bool TOT, bool FIX>
 __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
                                                                         uint64_t id_base, uint64_t seed, double nsigma,
                                                                         float *__restrict__ S, int *__restrict__ totals,
-                                                                        Counters *counters, bool normal_only)
+                                                                        Counters *counters, bool normal_only, bool normalize)
 {
     using T = typename std::conditional<FLUCT, double, float>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -510,10 +525,10 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
         }
         if constexpr (FLUCT)
             raster_batch_body<FLUCT, TOT, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, id_base, seed, nsigma,
-                                                 normal_only, totals, sc, &sm.queues[wid], qcount, drawn, lane);
+                                                 normal_only, normalize, totals, sc, &sm.queues[wid], qcount, drawn, lane);
         else
             raster_batch_body<FLUCT, TOT, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, id_base, seed, nsigma,
-                                                 normal_only, totals, sc, (DrawQueues<TOT> *)nullptr, qcount, drawn, lane);
+                                                 normal_only, normalize, totals, sc, (DrawQueues<TOT> *)nullptr, qcount, drawn, lane);
     }
     if constexpr (FLUCT) {
 #pragma unroll
@@ -646,7 +661,7 @@ template <bool FLUCT, bool TOT>
 __global__ void __launch_bounds__(kTileWarps * 32, 2) tile_accumulate_kernel(GridDims g, DepoArrays d, uint64_t id_base,
                                                                           uint64_t seed, double nsigma, TileScratch ts,
                                                                           float *__restrict__ S, int *__restrict__ totals,
-                                                                          Counters *counters, bool normal_only)
+                                                                          Counters *counters, bool normal_only, bool normalize)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem<FLUCT, TOT> &sm = *reinterpret_cast<TileSmem<FLUCT, TOT> *>(smem_raw);
@@ -683,10 +698,10 @@ __global__ void __launch_bounds__(kTileWarps * 32, 2) tile_accumulate_kernel(Gri
         }
         if constexpr (FLUCT)
             raster_batch_body<FLUCT, TOT, true>(g, clip, sink, t0, x0, st, sx, q, valid, 0ll, i, id_base, seed, nsigma,
-                                                normal_only, totals, sc, &sm.queues[wid], qcount, drawn, lane);
+                                                normal_only, normalize, totals, sc, &sm.queues[wid], qcount, drawn, lane);
         else
             raster_batch_body<FLUCT, TOT, true>(g, clip, sink, t0, x0, st, sx, q, valid, 0ll, i, id_base, seed, nsigma,
-                                                normal_only, totals, sc, (DrawQueues<TOT> *)nullptr, qcount, drawn, lane);
+                                                normal_only, normalize, totals, sc, (DrawQueues<TOT> *)nullptr, qcount, drawn, lane);
     }
     if constexpr (FLUCT) {
 #pragma unroll
@@ -769,7 +784,7 @@ cudaError_t raster_configure(cudaStream_t st)
 template <bool FLUCT, bool TOT, bool FIX>
 static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, double nsigma,
                                        float *S, int *depo_totals, Counters *counters, int sm_count, cudaStream_t st,
-                                       bool normal_only)
+                                       bool normal_only, bool normalize)
 {
     const long long n_batches = (n + kBatchDepos - 1) / kBatchDepos;
     const size_t smem = sizeof(BatchSmem<FLUCT, TOT>);
@@ -780,7 +795,7 @@ static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, ui
     const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
     if (ctas > max_ctas) ctas = max_ctas;
     return launch_pdl(raster_batch_kernel<FLUCT, TOT, FIX>, (unsigned)ctas, kBatchWarps * 32, smem, st, g, d, n, id_base, seed,
-                      nsigma, S, depo_totals, counters, normal_only);
+                      nsigma, S, depo_totals, counters, normal_only, normalize);
 }
 
 template <bool FIX>
@@ -789,14 +804,16 @@ static cudaError_t launch_raster_grid(GridDims g, DepoArrays d, long long n, uin
                                       cudaStream_t st)
 {
     if (n <= 0) return cudaSuccess;
+    const bool normalize = (fluctuate & kRasterNormalize) != 0;
+    fluctuate &= ~kRasterNormalize;
     if (!fluctuate) // no draws, no per-depo integer totals
         return launch_raster_batch<false, false, FIX>(g, d, n, id_base, seed, nsigma, grid, nullptr, counters, sm_count, st,
-                                                      false);
+                                                      false, normalize);
     if (depo_totals)
         return launch_raster_batch<true, true, FIX>(g, d, n, id_base, seed, nsigma, grid, depo_totals, counters, sm_count,
-                                                    st, fluctuate == 2);
+                                                    st, fluctuate == 2, normalize);
     return launch_raster_batch<true, false, FIX>(g, d, n, id_base, seed, nsigma, grid, nullptr, counters, sm_count, st,
-                                                 fluctuate == 2);
+                                                 fluctuate == 2, normalize);
 }
 
 cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
@@ -836,12 +853,12 @@ cudaError_t launch_tile_fill(GridDims g, DepoArrays d, long long n, double nsigm
 
 template <bool FLUCT, bool TOT>
 static cudaError_t launch_tile_accumulate_t(GridDims g, DepoArrays d, uint64_t id_base, uint64_t seed, double nsigma,
-                                            TileScratch ts, float *S, int *depo_totals, Counters *counters, bool normal_only,
+                                            TileScratch ts, float *S, int *depo_totals, Counters *counters, bool normal_only, bool normalize,
                                             cudaStream_t st)
 {
     const int n_tiles = ts.tiles_w * ts.tiles_t;
     tile_accumulate_kernel<FLUCT, TOT><<<n_tiles * kTileSlices, kTileWarps * 32, sizeof(TileSmem<FLUCT, TOT>), st>>>(
-        g, d, id_base, seed, nsigma, ts, S, depo_totals, counters, normal_only);
+        g, d, id_base, seed, nsigma, ts, S, depo_totals, counters, normal_only, normalize);
     return cudaGetLastError();
 }
 
@@ -849,12 +866,16 @@ cudaError_t launch_tile_accumulate(GridDims g, DepoArrays d, uint64_t id_base, u
                                    double nsigma, TileScratch ts, float *S, int *depo_totals, Counters *counters,
                                    cudaStream_t st)
 {
+    const bool normalize = (fluctuate & kRasterNormalize) != 0;
+    fluctuate &= ~kRasterNormalize;
     if (!fluctuate)
-        return launch_tile_accumulate_t<false, false>(g, d, id_base, seed, nsigma, ts, S, nullptr, counters, false, st);
+        return launch_tile_accumulate_t<false, false>(g, d, id_base, seed, nsigma, ts, S, nullptr, counters, false, normalize,
+                                                      st);
     if (depo_totals)
         return launch_tile_accumulate_t<true, true>(g, d, id_base, seed, nsigma, ts, S, depo_totals, counters,
-                                                    fluctuate == 2, st);
-    return launch_tile_accumulate_t<true, false>(g, d, id_base, seed, nsigma, ts, S, nullptr, counters, fluctuate == 2, st);
+                                                    fluctuate == 2, normalize, st);
+    return launch_tile_accumulate_t<true, false>(g, d, id_base, seed, nsigma, ts, S, nullptr, counters, fluctuate == 2,
+                                                 normalize, st);
 }
 
 cudaError_t launch_tile_finalize(GridDims g, TileScratch ts, float *S, cudaStream_t st)

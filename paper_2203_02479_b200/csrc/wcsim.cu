@@ -24,6 +24,7 @@ struct wcsim_plan {
     float2 *tw_row = nullptr, *tw_real = nullptr, *tw_col = nullptr;
     int rt_rows = 0;
     int wire_mode = WCSIM_WIRES_AUTO;
+    bool normalize = false; // renormalised patches (reading A24)
     Counters *counters = nullptr;
     float *amp_builtin = nullptr, *amp_custom = nullptr; // device, pad_t/2+1, scaled by pad_t^-1/2
     bool noise_armed = false;
@@ -400,6 +401,7 @@ int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n
     if (!guard.ok) return fail_cuda(cudaGetLastError());
     const GridDims g{plan->n_wires, plan->n_ticks};
     const DepoArrays d{depos->t0, depos->x0, depos->sigma_t, depos->sigma_x, depos->q};
+    if (plan->normalize) fluctuate |= kRasterNormalize; // internal.h: flag bit of the launchers' `fluctuate`
     StageSpan span(plan, WCSIM_STAGE_RASTER);
     if (plan->scatter_mode == WCSIM_SCATTER_TILED) {
         plan->launches += 6;
@@ -541,6 +543,13 @@ int wcsim_set_scatter_mode(wcsim_plan *plan, int scatter_mode)
 {
     if (!plan || scatter_mode < WCSIM_SCATTER_ATOMIC || scatter_mode > WCSIM_SCATTER_FIXED) return WCSIM_EINVAL;
     plan->scatter_mode = scatter_mode;
+    return WCSIM_OK;
+}
+
+int wcsim_set_normalize(wcsim_plan *plan, int on)
+{
+    if (!plan) return WCSIM_EINVAL;
+    plan->normalize = on != 0;
     return WCSIM_OK;
 }
 

@@ -686,3 +686,39 @@ def test_noise_every_row_kernel(B, O, nt, pad_t):
         p.add_noise(seed=21)  # standalone pass
         p.sync()
         assert_close(p.output().cpu().numpy(), ref, "standalone noise pad_t %d" % pad_t, rel=2e-5)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# renormalised patches (reading A24)
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_normalized_patches_match_oracle(B, O, mode):
+    from paper_2203_02479_b200 import synth
+    cfg = synth.config(1, n_depos=20_000)
+    pl = cfg["planes"][0]
+    nw, nt = pl["n_wires"], pl["n_ticks"]
+    d = {k: v.copy() for k, v in pl["depos"].items()}
+    d["sigma_t"][:50] = 0.0
+    d["sigma_t"][50:60] = 14.0  # wide patches: the one-warp-per-depo fallback
+    dev = to_dev(d)
+    with B.Plan(nw, nt, synth.response(5, 16), scatter_mode=mode) as p:
+        p.set_normalize(True)
+        for fluct in (0, 1, 2):
+            S_ref, tot_ref, st = O.raster_scatter(nw, nt, d, seed=6, fluctuate=fluct, normalize=True, want_totals=True)
+            totals = torch.zeros(20_000, dtype=torch.int32, device="cuda")
+            p.clear()
+            p.raster_scatter(dev, seed=6, fluctuate=fluct, dev_depo_totals=totals)
+            p.sync()
+            S = p.charge().cpu().numpy().astype(np.float64)
+            if fluct:
+                flipped = int(np.count_nonzero(S != S_ref))
+                assert flipped <= max(1, 1e-6 * st["drawn"]), (mode, fluct, flipped)
+                assert int(np.count_nonzero(totals.cpu().numpy() != tot_ref)) <= flipped
+            else:
+                assert_close(S, S_ref, "normalised S, mode %d" % mode)
+        # and it differs from the default: more charge collected
+        p.set_normalize(False)
+        p.clear()
+        p.raster_scatter(dev, fluctuate=0)
+        p.sync()
+        assert float(p.charge().sum()) < float(np.abs(S).sum())  # the default (A3) leaves the truncated tails uncollected
