@@ -234,36 +234,53 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
     pdl_wait(); // a no-op unless launched as a programmatic dependent
     const float2 *src = b.spec_inv + (size_t)row * b.spec_stride;
     const bool noisy = nz.amp != nullptr;
-    // stage X_k (+ noise) in shared memory so that every thread can reach the partner X_{N-k}
-#pragma unroll
-    for (int e = 0; e < E; ++e) {
-        const int k = i + e * NT;
-        float2 x = use_spec ? src[k] : make_float2(0.f, 0.f);
-        if (noisy) x = cadd(x, noise_bin(nz, (uint32_t)row, (uint32_t)k));
-        if (k == 0) {
-            x.y = 0.f; // the imaginary parts of the DC and Nyquist bins do not reach a real output
-            float2 xn = use_spec ? src[N] : make_float2(0.f, 0.f);
-            if (noisy) xn = cadd(xn, noise_bin(nz, (uint32_t)row, (uint32_t)N));
-            xn.y = 0.f;
-            smem[smem_index<1>(N, 0)] = xn;
-        }
-        smem[smem_index<1>(k, 0)] = x;
-    }
-    __syncthreads();
-    // Z_k = (X_k + conj X_{N-k}) + i exp(+2 pi i k / 2N) (X_k - conj X_{N-k});  inverse FFT of Z = even + i odd
     float2 v[E];
+    if (use_spec && !noisy) {
+        // plain convolution: the partner bin X_{N-k} is read straight from the spectrum row (descending, still
+        // coalesced; L1 / L2 hits), which saves the staging stores and a barrier
 #pragma unroll
-    for (int e = 0; e < E; ++e) {
-        const int k = i + e * NT;
-        const float2 xk = smem[smem_index<1>(k, 0)];
-        const float2 xn = smem[smem_index<1>(N - k, 0)];
-        const float2 s = make_float2(xk.x + xn.x, xk.y - xn.y);
-        const float2 d = make_float2(xk.x - xn.x, xk.y + xn.y);
-        const float2 w = load_tw(b.tw_real, k); // (cos, -sin)
-        const float2 t = make_float2(w.x * d.x + w.y * d.y, w.x * d.y - w.y * d.x);
-        v[e] = make_float2(s.x - t.y, s.y + t.x);
+        for (int e = 0; e < E; ++e) {
+            const int k = i + e * NT;
+            float2 xk = src[k], xn = src[N - k];
+            if (k == 0) xk.y = 0.f, xn.y = 0.f; // imaginary parts of the DC and Nyquist bins do not reach a real output
+            const float2 s = make_float2(xk.x + xn.x, xk.y - xn.y);
+            const float2 d = make_float2(xk.x - xn.x, xk.y + xn.y);
+            const float2 w = load_tw(b.tw_real, k); // (cos, -sin)
+            const float2 t = make_float2(w.x * d.x + w.y * d.y, w.x * d.y - w.y * d.x);
+            v[e] = make_float2(s.x - t.y, s.y + t.x);
+        }
+        fft_block<N, 1, E, +1>(v, smem, i, 0, b.tw_row, false);
+    } else {
+        // stage X_k (+ noise) in shared memory so that every thread can reach the partner X_{N-k}
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int k = i + e * NT;
+            float2 x = use_spec ? src[k] : make_float2(0.f, 0.f);
+            if (noisy) x = cadd(x, noise_bin(nz, (uint32_t)row, (uint32_t)k));
+            if (k == 0) {
+                x.y = 0.f; // the imaginary parts of the DC and Nyquist bins do not reach a real output
+                float2 xn = use_spec ? src[N] : make_float2(0.f, 0.f);
+                if (noisy) xn = cadd(xn, noise_bin(nz, (uint32_t)row, (uint32_t)N));
+                xn.y = 0.f;
+                smem[smem_index<1>(N, 0)] = xn;
+            }
+            smem[smem_index<1>(k, 0)] = x;
+        }
+        __syncthreads();
+        // Z_k = (X_k + conj X_{N-k}) + i exp(+2 pi i k / 2N) (X_k - conj X_{N-k});  inverse FFT of Z = even + i odd
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int k = i + e * NT;
+            const float2 xk = smem[smem_index<1>(k, 0)];
+            const float2 xn = smem[smem_index<1>(N - k, 0)];
+            const float2 s = make_float2(xk.x + xn.x, xk.y - xn.y);
+            const float2 d = make_float2(xk.x - xn.x, xk.y + xn.y);
+            const float2 w = load_tw(b.tw_real, k); // (cos, -sin)
+            const float2 t = make_float2(w.x * d.x + w.y * d.y, w.x * d.y - w.y * d.x);
+            v[e] = make_float2(s.x - t.y, s.y + t.x);
+        }
+        fft_block<N, 1, E, +1>(v, smem, i, 0, b.tw_row, true);
     }
-    fft_block<N, 1, E, +1>(v, smem, i, 0, b.tw_row, true);
     float *dst = b.M + (size_t)row * g.n_ticks;
 #pragma unroll
     for (int e = 0; e < E; ++e) {
