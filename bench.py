@@ -190,6 +190,18 @@ def run_ours(args):
     value, slowest_s = replicas.whole_job_throughput(n_depos * args.steps, local_s, dev)
     ms_per_step = slowest_s * 1e3 / args.steps
 
+    # the same K steps without the convolution: what the convolve stage adds to a back-to-back plane-event (its kernels
+    # are programmatic dependents of the raster and of one another, so this is less than the sum of their stand-alone times)
+    def step_raster_only():
+        plan.clear()
+        plan.raster_scatter(d, seed=cfg["fluct_seed"], fluctuate=fluct)
+
+    for _ in range(min(args.warmup, 3)):
+        flush.fill_(1.0)
+        step_raster_only()
+    per_step_raster = timed(step_raster_only, args.steps)
+    ms_raster_only = sum(per_step_raster) / len(per_step_raster)
+
     plan.set_profiling(True)
     for _ in range(min(args.warmup, 3)):
         flush.fill_(1.0)
@@ -309,11 +321,17 @@ def run_ours(args):
                 # FFT convolution moves; the direct wire-axis pass avoids 33 MB of them on configs[1]
                 "survey_pass_model_bytes": pass_model,
                 "frac_of_survey_pass_model": pass_model / (conv_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    # in the back-to-back plane-event (no event records between the kernels): plane-event minus (clear + raster) alone
+    conv_in_situ = ms_per_step - ms_raster_only
+    if world == 1 and conv_in_situ > 0:
+        convolve["in_plane_event"] = {"ms": conv_in_situ, "ms_clear_and_raster_alone": ms_raster_only,
+                                      "frac": conv_bytes / (conv_in_situ * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                                      "frac_of_survey_pass_model": pass_model / (conv_in_situ * 1e-3) / 1e9 / peaks["hbm_gbs"]}
     dom = max(stage_rows, key=lambda r: r["ms"])
     if dom["stage"] == "raster" and fluct:
         # ALU bound: algorithmic fp64 work of the oracle's arithmetic, ~70 flop per drawn bin,
         # against 148 SMs x 64 fp64 FMA lanes x 2 flop x the SM clock
-        bins = stats["bins_drawn"] / max(1, 2 * args.steps + min(args.warmup, 3))  # plane-events since the reset
+        bins = stats["bins_drawn"] / max(1, 3 * args.steps + 2 * min(args.warmup, 3))  # plane-events since the reset
         tflops = bins * FP64_FLOP_PER_BIN / (dom["ms"] * 1e-3) / 1e12
         peak = 148 * 64 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
         roofline = {"kernel": "raster_batch_kernel<fluct>", "bound": "alu", "achieved": tflops, "peak": peak,
