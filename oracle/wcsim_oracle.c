@@ -32,7 +32,10 @@
  * PARITY UNPINNED (conventions of this build that nothing in the paper fixes;
  * DESIGN.md readings A3, A6, A8, A15): no patch renormalisation; the mu<16
  * inversion / mu>=16 rounded-normal split of the binomial sampler and its use of
- * AS 241; the Philox counter layout; the orthonormal noise scaling.
+ * AS 241; the Philox counter layout; the orthonormal noise scaling; and, of the
+ * steps around the hot path, the conventions of readings A21-A24 (clamp and
+ * rounding of the normal draw, drift coordinates and units, the ideal ADC, the
+ * patch renormalisation).
  *
  * Build: gcc -O2 -std=c11 -fopenmp -ffp-contract=off -shared -fPIC
  *        (-ffp-contract=off: every product and sum is rounded separately, so the
