@@ -214,12 +214,12 @@ def run_ours(args):
     stats = plan.stats()
 
     # ---- end to end through the C ABI with host buffers -------------------------------------------------------------
-    # Every step copies its depos host->device and its M device->host (pinned buffers) inside the timed region.  Two
-    # plans on two streams are used alternately through wcsim_simulate_host_async, so the 19 MB device->host copy of
+    # Every step copies its depos host->device and its M device->host (pinned buffers) inside the timed region.  Three
+    # plans on three streams are used in turn through wcsim_simulate_host_async, so the 19 MB device->host copy of
     # one plane-event runs under the next event's copies and kernels; a step's M is on the host when its plan is
     # synchronised, which happens before that plan is reused and, for the last steps, before the clock stops.
     host = {k: torch.from_numpy(v).pin_memory() for k, v in pl["depos"].items()}
-    n_e2e_plans = 2
+    n_e2e_plans = 3  # two leave the device->host engine idle part of the time (436 us); four gain nothing over three
     e2e_streams = [torch.cuda.Stream(device=dev) for _ in range(n_e2e_plans)]
     e2e_plans = [B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]),
                         nsigma=cfg["nsigma"], scatter_mode=mode, stream=st) for st in e2e_streams]
@@ -228,7 +228,7 @@ def run_ours(args):
     def run_e2e(k):
         for i in range(k):
             p = e2e_plans[i % n_e2e_plans]
-            p.sync()  # the plane-event this plan ran two steps ago is complete: its host_M may be overwritten
+            p.sync()  # the plane-event this plan ran n_e2e_plans steps ago is complete: its host_M may be overwritten
             p.simulate_host_async(host, host_M[i % n_e2e_plans], seed=cfg["fluct_seed"], fluctuate=fluct)
         for p in e2e_plans:
             p.sync()
@@ -366,7 +366,7 @@ def run_ours(args):
         "clocks": sampler.summary(),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_slowest * 1e3 / e2e_steps, "steps": e2e_steps,
-                "how": "wcsim_simulate_host_async on 2 plans/streams alternately, pinned host buffers",
+                "how": "wcsim_simulate_host_async on %d plans/streams in turn, pinned host buffers" % n_e2e_plans,
                 "ms_per_step_synchronous_call": e2e_sync_ms,
                 "adc_variant": {"ms_per_step": e2e_adc_ms, "value": n_depos / (e2e_adc_ms * 1e-3),
                                 "d2h_bytes_per_step": d2h // 2,

@@ -182,7 +182,7 @@ int wcsim_simulate_host(wcsim_plan *plan, const float *host_t0, const float *hos
  * The same, without the final synchronisation: everything (the host->device copies of the depos, the kernels and the
  * device->host copy of M) is enqueued on the plan's stream and the call returns.  host_M holds this plane-event's
  * M(t,x) (Eq. 1) once wcsim_sync(plan) has returned; the host depo arrays must stay valid and unchanged
- * until then, and must be pinned for the copies to be asynchronous.  Two plans on two streams, used alternately,
+ * until then, and must be pinned for the copies to be asynchronous.  Two or three plans on as many streams, used in turn,
  * overlap one event's device->host copy with the next event's copies and kernels (what bench.py's `e2e` does).
  * Errors: as wcsim_simulate_host; asynchronous CUDA errors surface at wcsim_sync.
  */
