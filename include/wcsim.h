@@ -240,6 +240,15 @@ int wcsim_debug_binomial(const double *dev_N, const double *dev_p, const unsigne
 /* dev_k[i] = G(dev_N[i], dev_p[i]; dev_w[i]) -- the normal-approximation draw of fluctuate = 2 (A21) */
 int wcsim_debug_normal_draw(const double *dev_N, const double *dev_p, const unsigned int *dev_w, double *dev_k,
                          long long n, void *cuda_stream);
+/* The guarded fp32 fast path of the rounded-normal draw (csrc/rng.cuh; the raster takes it for mu >= 16 and falls back
+ * to the fp64 routine behind wcsim_debug_binomial when the guard rejects): dev_k[i] = its k, dev_ok[i] = 1 if the guard
+ * accepted it (then k must equal the fp64 routine's), 0 if not.  dev_p in (0, 1/2]; DEVICE pointers, n elements. */
+int wcsim_debug_fast_normal(const double *dev_N, const double *dev_p, const unsigned int *dev_w, double *dev_k,
+                            int *dev_ok, long long n, void *cuda_stream);
+/* Error of the fast path's fp32 normal quantile against the fp64 AS 241 routine over the 32-bit words
+ * first_word .. first_word + n_words - 1 (first_word + n_words <= 2^32): dev_out4 (DEVICE, 4 doubles) receives
+ * max |z32 - z64| and max |z64| over the words the fast path accepts, their number, and max |z32 - z64| / max(1, |z64|). */
+int wcsim_debug_z32_scan(unsigned long long first_word, unsigned long long n_words, double *dev_out4, void *cuda_stream);
 /* copy the response spectrum Rhat[kx][kt] (kx < pad_wires, kt <= pad_ticks/2) to HOST as interleaved re,im floats */
 int wcsim_debug_response_spectrum(wcsim_plan *plan, float *host_out);
 

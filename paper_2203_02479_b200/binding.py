@@ -24,6 +24,7 @@ SYMBOLS = [
     "wcsim_charge_ptr", "wcsim_output_ptr", "wcsim_get_dims", "wcsim_get_stats", "wcsim_reset_stats",
     "wcsim_simulate_host", "wcsim_set_profiling", "wcsim_get_stage_times", "wcsim_get_launch_count",
     "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf", "wcsim_simulate_host_async", "wcsim_debug_normal_draw", "wcsim_drift", "wcsim_digitize", "wcsim_set_normalize",
+    "wcsim_debug_fast_normal", "wcsim_debug_z32_scan",
     "wcsim_strerror", "wcsim_last_cuda_error", "wcsim_version",
 ]
 
@@ -92,6 +93,8 @@ def lib():
         L.wcsim_debug_philox.argtypes = [vp, vp, vp, ll, vp]
         L.wcsim_debug_binomial.argtypes = [vp, vp, vp, vp, ll, vp]
         L.wcsim_debug_normal_draw.argtypes = [vp, vp, vp, vp, ll, vp]
+        L.wcsim_debug_fast_normal.argtypes = [vp, vp, vp, vp, vp, ll, vp]
+        L.wcsim_debug_z32_scan.argtypes = [ull, ull, vp, vp]
         L.wcsim_debug_response_spectrum.argtypes = [vp, vp]
         L.wcsim_debug_erf.argtypes = [vp, vp, ll]
         L.wcsim_digitize.argtypes = [vp, C.c_float, C.c_float, i, vp]
@@ -341,6 +344,16 @@ def wcsim_drift(groups, params, planes, out, n=None, stream=None):
     outs = (wcsim_depos * len(planes))(*[wcsim_depos(*[_dev_ptr(o[k]) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")])
                                          for o in out])
     _check(lib().wcsim_drift(*ptrs, int(n), C.byref(prm), geo, len(planes), outs, _stream_ptr(stream)), "wcsim_drift")
+
+
+def wcsim_debug_fast_normal(dev_N, dev_p, dev_w, dev_k, dev_ok, n, stream=None):
+    _check(lib().wcsim_debug_fast_normal(_dev_ptr(dev_N), _dev_ptr(dev_p), _dev_ptr(dev_w), _dev_ptr(dev_k),
+                                         _dev_ptr(dev_ok), int(n), _stream_ptr(stream)), "wcsim_debug_fast_normal")
+
+
+def wcsim_debug_z32_scan(first_word, n_words, dev_out4, stream=None):
+    _check(lib().wcsim_debug_z32_scan(int(first_word), int(n_words), _dev_ptr(dev_out4), _stream_ptr(stream)),
+           "wcsim_debug_z32_scan")
 
 
 def wcsim_debug_normal_draw(dev_N, dev_p, dev_w, dev_k, n, stream=None):

@@ -30,7 +30,7 @@ def _nvcc() -> str:
 
 
 def _deps():
-    out = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f != "pipe_rates.cu"] + [os.path.join(INCLUDE, "wcsim.h"), __file__]
+    out = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(INCLUDE, "wcsim.h"), __file__]
     return out
 
 
@@ -69,18 +69,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_pipe_rates() -> str:
-    """The stand-alone pipe-rate microbenchmark (csrc/pipe_rates.cu): evidence for DESIGN.md's ALU peaks."""
-    exe = os.path.join(HERE, "pipe_rates")
-    r = subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", exe,
-                        os.path.join(CSRC, "pipe_rates.cu")], capture_output=True, text=True)
-    if r.returncode != 0:
-        raise RuntimeError("nvcc failed for pipe_rates.cu:\n%s\n%s" % (r.stdout, r.stderr))
-    return exe
-
-
 if __name__ == "__main__":
-    if "--pipe-rates" in sys.argv:
-        print(build_pipe_rates())
-    else:
-        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

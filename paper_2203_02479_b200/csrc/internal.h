@@ -130,4 +130,9 @@ cudaError_t launch_debug_philox(const unsigned int *ctr, const unsigned int *key
 cudaError_t launch_debug_binomial(const double *N, const double *p, const unsigned int *w, double *k, long long n,
                                   bool normal_only, cudaStream_t st);
 
+cudaError_t launch_debug_fast_normal(const double *N, const double *p, const unsigned int *w, double *k, int *ok,
+                                     long long n, cudaStream_t st);
+cudaError_t launch_debug_z32_scan(unsigned long long first, unsigned long long count, unsigned long long *out4,
+                                  cudaStream_t st);
+
 } // namespace wcsim

@@ -169,7 +169,7 @@ struct Clip {
 // Rasters depo (t0, x0, st, sx, q) into the clip window [w_lo, w_hi) x [k_lo, k_hi) (already inside the grid).
 // Returns the number of bins this lane deposited; *lane_total accumulates the lane's signed draws.
 template <bool FLUCT, typename Sink>
-__device__ __forceinline__ unsigned int raster_depo(float t0f, float x0f, float stf, float sxf, float qf, uint64_t id,
+__device__ __noinline__ unsigned int raster_depo(float t0f, float x0f, float stf, float sxf, float qf, uint64_t id,
                                                     uint64_t seed, double nsigma, int n_ticks, int w_lo, int w_hi,
                                                     int k_lo, int k_hi, const Sink &sink, int lane, int *lane_total,
                                                     bool normal_only, double inv_norm)
@@ -228,40 +228,13 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v)
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// atomic mode: warps fetch batches of kBatchDepos depos from a device-side counter until none is left
+// batches: a warp takes kBatchDepos depos at a time, one per lane
 // ------------------------------------------------------------------------------------------------------------------
 constexpr int kBatchWarps = 4;          // warps per CTA
 constexpr int kBatchShift = 3;          // log2 of the depos a warp fetches at a time (lanes beyond that own no depo):
 constexpr int kBatchDepos = 1 << kBatchShift; // small batches keep the per-warp serial path short and the load balanced
 constexpr int kTailDepos = 2, kTailPerWarp = 4; // guided scheduling of the last batches (raster_batch_kernel)
-constexpr int kEdgeCap = 128;           // edge values per warp scratch (8 patches of 16 x 5 bins need 184)
-constexpr int kQueueCap = 64;           // entries per draw queue (at most 31 left over + 32 pushed)
-
-template <bool FLUCT>
-struct BatchScratch {
-    using T = typename std::conditional<FLUCT, double, float>::type;
-    T edge[kEdgeCap];
-    int eoff[33], boff[33];
-};
-// 20 bytes per queued bin (24 with per-depo totals): the bytes per warp decide how many warps an SM holds
 constexpr uint32_t kBinMirror = 1u << 30, kBinNegative = 1u << 31, kBinMask = kBinMirror - 1u; // grid < 2^30 bins
-template <bool TOT>
-struct DrawQueues {
-    double p[kNumDrawQueues][kQueueCap];
-    float N[kNumDrawQueues][kQueueCap]; // floor(|q| + 1/2) of a float q is always a float
-    uint32_t w[kNumDrawQueues][kQueueCap];
-    uint32_t bin[kNumDrawQueues][kQueueCap]; // wire * n_ticks + tick | kBinMirror | kBinNegative
-    uint32_t depo[TOT ? kNumDrawQueues : 1][TOT ? kQueueCap : 1]; // depo index in the call (per-depo totals only)
-};
-template <bool FLUCT, bool TOT>
-struct BatchSmem {
-    BatchScratch<FLUCT> scratch[kBatchWarps];
-};
-template <bool TOT>
-struct BatchSmem<true, TOT> {
-    BatchScratch<true> scratch[kBatchWarps];
-    DrawQueues<TOT> queues[kBatchWarps];
-};
 
 // largest d in [0, kBatchDepos) with off[d] <= x (off is an exclusive prefix over the depos of a batch; entries from
 // kBatchDepos on all hold the total, which is > x)
@@ -284,46 +257,22 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane)
     return v;
 }
 
-// draws `take` entries from the top of queue `cls` (lane < take) and adds them to S
-template <bool TOT, typename Sink>
-__device__ __forceinline__ void drain_queue(DrawQueues<TOT> &Q, int cls, int &count, bool everything, const Sink &sink,
-                                            int *__restrict__ totals, int lane)
-{
-    while (count >= 32 || (everything && count > 0)) {
-        const int take = min(32, count);
-        count -= take;
-        if (lane < take) {
-            const int e = count + lane;
-            const uint32_t fb = Q.bin[cls][e];
-            const double N = (double)Q.N[cls][e];
-            const double k = draw_classified(cls, N, Q.p[cls][e], Q.w[cls][e], (fb & kBinMirror) != 0);
-            if (k != 0.0) {
-                const float v = (fb & kBinNegative) ? -(float)k : (float)k;
-                sink.add_at(fb & kBinMask, v);
-                if constexpr (TOT) atomicAdd(totals + Q.depo[cls][e], (int)v);
-            }
-        }
-        __syncwarp();
-    }
-}
+// ---- fluctuation off: flat lists of edges and of bins -----------------------------------------------------------
+constexpr int kEdgeCap = 128; // edge values per warp scratch (8 patches of 16 x 5 bins need 184: two sub-batches)
+struct FlatScratch {
+    float edge[kEdgeCap];
+    int eoff[33], boff[33];
+};
 
-// One batch of up to kBatchDepos depos, one per lane (lane l < count owns a depo, the others own none): extents clipped to
-// `clip`, edges, bins, draws.  Shared by the atomic kernel (clip = the grid, sink = S) and the tiled kernel (clip = a
-// tile, sink = the tile's fixed-point accumulators).  The call-wide index of the depo of lane `own` is dbase + own, or
-// dbase + (lane own's dl) when the batch comes from an index list (INDIRECT).
-template <bool FLUCT, bool TOT, bool INDIRECT, typename Sink>
-__device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const Sink &sink, float t0, float x0, float st,
-                                                  float sx, float q, bool valid, long long dbase, uint32_t dl,
-                                                  uint64_t id_base, uint64_t seed, double nsigma, bool normal_only, bool normalize,
-                                                  int *__restrict__ totals, BatchScratch<FLUCT> &sc,
-                                                  DrawQueues<TOT> *queues, int (&qcount)[kNumDrawQueues],
-                                                  unsigned long long &drawn, int lane)
+// One batch of up to kBatchDepos depos, one per lane (lane l < count owns a depo, the others own none), fluctuation off:
+// extents clipped to `clip`, erf at the flat list of all bin edges, then q wt_i wx_j over the flat list of all bins.
+// Shared by the atomic kernel (clip = the grid, sink = S) and the tiled kernel (clip = a tile, sink = the tile's
+// fixed-point accumulators).
+template <typename Sink>
+__device__ __forceinline__ void raster_flat_body(GridDims g, Clip clip, const Sink &sink, float t0, float x0, float st,
+                                                 float sx, float q, bool valid, double nsigma, bool normalize,
+                                                 FlatScratch &sc, unsigned long long &drawn, int lane)
 {
-    using T = typename std::conditional<FLUCT, double, float>::type;
-    auto depo_of = [&](int own) -> long long {
-        if constexpr (INDIRECT) return dbase + (long long)__shfl_sync(0xffffffffu, dl, own);
-        else return dbase + own;
-    };
     const double T0 = t0, X0 = x0, ST = st, SX = sx;
     Extent et{0, 0}, ex{0, 0};
     if (valid) {
@@ -346,7 +295,6 @@ __device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const S
         sc.boff[32] = bincl;
     }
     __syncwarp();
-    const float Ntr = (float)floor(fabs((double)q) + 0.5); // exact: see DrawQueues::N
     drawn += (unsigned long long)nb;
 
     // patches too big for the scratch: the whole warp walks them one at a time
@@ -355,18 +303,14 @@ __device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const S
         const int src = __ffs(big_mask) - 1;
         big_mask &= big_mask - 1;
         int tot = 0;
-        drawn += raster_depo<FLUCT>(__shfl_sync(0xffffffffu, t0, src), __shfl_sync(0xffffffffu, x0, src),
+        drawn += raster_depo<false>(__shfl_sync(0xffffffffu, t0, src), __shfl_sync(0xffffffffu, x0, src),
                                     __shfl_sync(0xffffffffu, st, src), __shfl_sync(0xffffffffu, sx, src),
-                                    __shfl_sync(0xffffffffu, q, src), id_base + (uint64_t)depo_of(src), seed,
-                                    nsigma, g.n_ticks, clip.w_lo, clip.w_hi, clip.k_lo, clip.k_hi, sink, lane, &tot, normal_only,
+                                    __shfl_sync(0xffffffffu, q, src), 0ull, 0ull, nsigma, g.n_ticks, clip.w_lo, clip.w_hi,
+                                    clip.k_lo, clip.k_hi, sink, lane, &tot, false,
                                     normalize ? __shfl_sync(0xffffffffu, inv_norm, src) : 1.0);
-        if (totals != nullptr) {
-            tot = warp_sum(tot);
-            if (lane == 0 && tot != 0) atomicAdd(totals + depo_of(src), tot);
-        }
     }
 
-    // sub-batches of consecutive depos whose edges fit the scratch (normally all 32 at once)
+    // sub-batches of consecutive depos whose edges fit the scratch (normally all at once)
     int d0 = 0;
     while (d0 < 32) {
         const int ebase = sc.eoff[d0];
@@ -386,22 +330,18 @@ __device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const S
             const float sgt = __shfl_sync(0xffffffffu, st, own), sgx = __shfl_sync(0xffffffffu, sx, own);
             const double centre = (double)(on_t ? ct : cx), sigma = (double)(on_t ? sgt : sgx);
             const int coord = on_t ? lo_t + le : lo_x + (le - nto - 1);
-            T E;
+            float E;
             if (sigma < 1e-6) { // all weight in bin floor(centre) (A4): a step from -1 to +1 after that bin's low edge
-                E = ((double)coord <= floor(centre)) ? T(-1) : T(1);
+                E = ((double)coord <= floor(centre)) ? -1.0f : 1.0f;
             } else {
                 const double dd = __dsub_rn((double)coord, centre);
-                if constexpr (FLUCT) {
-                    E = erf_from_table(g_erf_tab, fast_div(dd, 1.4142135623730951 * sigma));
-                } else {
-                    const float inv = 1.0f / (1.41421356f * (float)sigma);
-                    E = erff((float)dd * inv);
-                }
+                const float inv = 1.0f / (1.41421356f * (float)sigma);
+                E = erff((float)dd * inv);
             }
             if (act) sc.edge[e] = E;
         }
         __syncwarp();
-        // ---- bins: p_ij = wt_i wx_j, flat over the sub-batch ----------------------------------------------------
+        // ---- bins: q wt_i wx_j, flat over the sub-batch -----------------------------------------------------------
         for (int b0 = 0; b0 < btot; b0 += 32) {
             const int b = b0 + lane;
             const bool act = b < btot;
@@ -413,60 +353,373 @@ __device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const S
             // than the rounding of the product below for l < 2^22 (a flat-path patch has < 2^14 bins)
             const int j = act ? __float2int_rz(((float)l + 0.5f) * __frcp_rn((float)max(nto, 1))) : 0;
             const int ii = act ? l - j * nto : 0;                              // tick index in the patch
-            const T *E = sc.edge + (sc.eoff[own] - ebase);
-            const T wt = T(0.5) * (E[ii + 1] - E[ii]);
-            const T wx = T(0.5) * (E[nto + 1 + j + 1] - E[nto + 1 + j]);
-            const int wire = lo_x + j, tick = lo_t + ii;
-            if constexpr (FLUCT) {
-                const double Nn = (double)__shfl_sync(0xffffffffu, Ntr, own);
-                const float qq = __shfl_sync(0xffffffffu, q, own);
-                double p = __dmul_rn(wt, wx);
-                if (normalize) p *= __shfl_sync(0xffffffffu, inv_norm, own);
-                const uint64_t gbin = (uint64_t)wire * (uint64_t)g.n_ticks + (uint64_t)tick;
-                const long long dio = depo_of(own);
-                const uint64_t id = id_base + (uint64_t)dio;
-                uint32_t w = pick_word(fluct_words(seed, id, gbin >> 2), (uint32_t)gbin & 3u);
-                bool mirror = false;
-                int cls = act ? classify_draw(Nn, p, w, mirror, normal_only) : (int)kDrawZero;
-                const uint32_t fb = sink.index(wire, tick) | (mirror ? kBinMirror : 0u) | (qq < 0.0f ? kBinNegative : 0u);
-                if (cls == kDrawAll) { // p >= 1: every electron lands here
-                    const float v = (qq < 0.0f) ? -(float)Nn : (float)Nn;
-                    if (act) sink.add(wire, tick, v);
-                    if constexpr (TOT) atomicAdd(totals + dio, (int)v);
+            const float *E = sc.edge + (sc.eoff[own] - ebase);
+            const float wt = 0.5f * (E[ii + 1] - E[ii]);
+            const float wx = 0.5f * (E[nto + 1 + j + 1] - E[nto + 1 + j]);
+            const float qq = __shfl_sync(0xffffffffu, q, own);
+            const float scale = normalize ? (float)__shfl_sync(0xffffffffu, inv_norm, own) : 1.0f;
+            if (act) sink.add(lo_x + j, lo_t + ii, qq * (wt * wx) * scale);
+        }
+        __syncwarp();
+        d0 = d1;
+    }
+}
+
+// ---- fluctuation on: quads ------------------------------------------------------------------------------------------
+// One Philox call gives the words of four consecutive absolute grid bins (reading A8), so the unit of work of a lane is
+// a QUAD: (depo, wire row of its patch, aligned group of four bins g>>2 of that row).  A lane finds its depo once, calls
+// Philox once, loads the five tick-edge values and the wire weight once and then decides its (up to) four bins:
+//   * k known without a draw (p <= 0, p >= 1, N = 0, or u <= 1 - mu, which implies u <= (1-p)^N);
+//   * mu >= 16 (or the normal-approximation sampler): the guarded fp32 estimate of rng.cuh; accepted for ~99 % of such bins;
+//   * everything else goes to one of two per-warp shared-memory queues and is drawn by the fp64 routines of rng.cuh:
+//     the inversion queue (mu < 16), worked off by a loop whose lanes pick up the next queued bin as soon as their
+//     own inversion ends (a lane's trip count is k+1; without that the warp waits for its slowest lane), and the exact
+//     queue (bins the fp32 guard did not accept), drawn 32 at a time.
+// The edges of a batch are laid out per depo as [3 pad][nt+1 tick edges][3 pad][nx+1 wire edges], so that the five
+// loads of a quad never need a bounds check (pad values only ever reach bins that are masked off).
+constexpr int kQuadEdgeCap = 256, kEdgePad = 3;
+constexpr int kInvCap = 96, kInvDrainAt = 64, kExactCap = 64;
+constexpr int kQuadInvTab = 64;
+
+struct alignas(16) DepoRec {
+    int lo_t, lo_x;  // first tick / wire of the clipped patch
+    uint32_t shape;  // nt | nx << 8 | nq << 16 | (q < 0) << 31
+    int ebase;       // index of the patch's first pad slot in QuadScratch::edge
+    float t0, x0, N; // centre; N = floor(|q| + 1/2) (a float q makes it a float)
+    uint32_t idx;    // index of the depo in the call (relative to the batch's dbase)
+    double inv_t, inv_x; // 1 / (sqrt2 sigma); 0: sigma < 1e-6 (A4)
+};
+
+struct QuadScratch {
+    double edge[kQuadEdgeCap + 8]; // + slack: a quad past the end of a row may read up to 3 slots beyond the last pad
+    DepoRec rec[kBatchDepos];
+    double inv_norm[kBatchDepos];
+    int eoff[33], qoff[33];
+};
+// queue entry: 20 bytes (24 with per-depo totals).  [0, kInvCap): inversion queue; [kInvCap, kInvCap + kExactCap): exact queue
+template <bool TOT>
+struct QuadQueues {
+    double p[kInvCap + kExactCap];   // after the mirror: 0 < p <= 1/2
+    float N[kInvCap + kExactCap];
+    uint32_t w[kInvCap + kExactCap]; // after the mirror
+    uint32_t bin[kInvCap + kExactCap]; // sink index | kBinMirror | kBinNegative
+    uint32_t depo[TOT ? kInvCap + kExactCap : 1];
+};
+// inversions in flight between two calls of drain_inversion (one per lane)
+template <bool TOT>
+struct InvState {
+    double f[32], c[32], u[32], r[32], rN1[32];
+    float N[32], kd[32];
+    uint32_t fb[32];
+    uint32_t depo[TOT ? 32 : 1];
+};
+template <bool TOT>
+struct QuadWarp {
+    QuadScratch sc;
+    QuadQueues<TOT> q;
+    InvState<TOT> st;
+};
+// per-warp registers that live across batches
+struct QuadCounts {
+    int inv = 0, exact = 0;
+    uint32_t inflight = 0; // lanes whose InvState slot holds an unfinished inversion
+};
+
+template <bool TOT, typename Sink>
+__device__ __forceinline__ void commit_draw(const Sink &sink, int *__restrict__ totals, uint32_t fb, float N, float k,
+                                            uint32_t depo)
+{
+    if (fb & kBinMirror) k = N - k;
+    if (k != 0.0f) {
+        const float v = (fb & kBinNegative) ? -k : k;
+        sink.add_at(fb & kBinMask, v);
+        if constexpr (TOT) atomicAdd(totals + depo, (int)v);
+    }
+}
+
+// the exact queue: bins whose fp32 estimate was too close to a rounding boundary; the fp64 AS 241 routines
+template <bool TOT, typename Sink>
+__device__ __noinline__ void drain_exact(QuadQueues<TOT> &Q, int &count, bool everything, const Sink &sink,
+                                            int *__restrict__ totals, int lane)
+{
+    while (count >= 32 || (everything && count > 0)) {
+        const int take = min(32, count);
+        count -= take;
+        if (lane < take) {
+            const int e = kInvCap + count + lane;
+            const double N = (double)Q.N[e], p = Q.p[e];
+            const uint32_t w = Q.w[e];
+            const double k = word_is_central(w) ? draw_normal_central(N, p, w) : draw_normal_tail(N, p, w);
+            commit_draw<TOT>(sink, totals, Q.bin[e], Q.N[e], (float)k, TOT ? Q.depo[e] : 0u);
+        }
+        __syncwarp();
+    }
+}
+
+// The inversion queue (reading A6, mu < 16): k = the number of CDF values F(0), F(1), ... below u, summed term by term
+// in fp64 exactly as draw_inversion does.  Every lane runs its own inversion; a lane whose inversion has ended commits it
+// and takes the next queued bin, so the loop's lanes stay busy whatever the individual trip counts are.  With
+// `finish` false the call returns as soon as the queue is empty and parks the unfinished inversions in `st`
+// (`inflight` says which lanes); the next call picks them up.  With `finish` true it runs until nothing is left.
+template <bool TOT, typename Sink>
+__device__ __noinline__ void drain_inversion(QuadQueues<TOT> &Q, InvState<TOT> &st, int &count, uint32_t &inflight,
+                                                bool finish, const double *__restrict__ inv_k, const Sink &sink,
+                                                int *__restrict__ totals, int lane)
+{
+    const uint32_t bit = 1u << lane;
+    bool active = (inflight & bit) != 0;
+    double f = 0.0, c = 0.0, u = 0.0, r = 0.0, rN1 = 0.0;
+    float N = 0.f, kd = 0.f;
+    uint32_t fb = 0u, depo = 0u;
+    if (active) {
+        f = st.f[lane], c = st.c[lane], u = st.u[lane], r = st.r[lane], rN1 = st.rN1[lane];
+        N = st.N[lane], kd = st.kd[lane], fb = st.fb[lane];
+        if constexpr (TOT) depo = st.depo[lane];
+    }
+    for (;;) {
+        const uint32_t idle = __ballot_sync(0xffffffffu, !active);
+        if (idle) {
+            if (count > 0) {
+                const int take = min(__popc(idle), count);
+                const int rank = __popc(idle & (bit - 1u));
+                if (!active && rank < take) {
+                    const int e = count - 1 - rank;
+                    const double p = Q.p[e];
+                    N = Q.N[e];
+                    fb = Q.bin[e];
+                    if constexpr (TOT) depo = Q.depo[e];
+                    u = word_to_u01(Q.w[e]);
+                    f = pow_one_minus((double)N, p);
+                    c = f;
+                    r = fast_div(p, 1.0 - p);
+                    rN1 = r * ((double)N + 1.0);
+                    kd = 0.f;
+                    active = true;
                 }
-                DrawQueues<TOT> &Q = *queues;
-                // one slot per bin in the queue of its class: position = queue fill + rank among the lanes of the
-                // same class (ballots), then a single block of stores for all classes
-                unsigned int mine = 0;
-                int base = 0;
+                count -= take;
+            } else if (!finish || idle == 0xffffffffu) {
+                break;
+            }
+        }
+        // f_k = f_{k-1} r (N - k + 1) / k, written as f_{k-1} (r (N+1) / k - r)
 #pragma unroll
-                for (int c = 0; c < kNumDrawQueues; ++c) {
-                    const unsigned int m = __ballot_sync(0xffffffffu, cls == c);
-                    mine = (cls == c) ? m : mine;
-                    base = (cls == c) ? qcount[c] : base;
-                    qcount[c] += __popc(m);
-                }
-                if (cls >= 0) {
-                    const int pos = base + __popc(mine & ((1u << lane) - 1u));
-                    Q.p[cls][pos] = p;
-                    Q.N[cls][pos] = (float)Nn;
-                    Q.w[cls][pos] = w;
-                    Q.bin[cls][pos] = fb;
-                    if constexpr (TOT) Q.depo[cls][pos] = (uint32_t)dio;
-                }
-                __syncwarp();
-                // counts stay below 64, so some queue holds a full warp iff the OR of the counts has bit 5 set
-                int any_full = 0;
-#pragma unroll
-                for (int c = 0; c < kNumDrawQueues; ++c) any_full |= qcount[c];
-                if (any_full & 32) {
-#pragma unroll
-                    for (int c = 0; c < kNumDrawQueues; ++c) drain_queue(Q, c, qcount[c], false, sink, totals, lane);
-                }
+        for (int s = 0; s < 4; ++s) {
+            if (active && u > c && kd < N) {
+                kd += 1.0f;
+                const double rk = kd < (float)kQuadInvTab ? inv_k[(int)kd] : fast_rcp((double)kd);
+                f *= fma(rN1, rk, -r);
+                c += f;
+            }
+        }
+        if (active && !(u > c && kd < N)) {
+            commit_draw<TOT>(sink, totals, fb, N, kd, depo);
+            active = false;
+        }
+    }
+    inflight = __ballot_sync(0xffffffffu, active);
+    if (active) {
+        st.f[lane] = f, st.c[lane] = c, st.u[lane] = u, st.r[lane] = r, st.rN1[lane] = rN1;
+        st.N[lane] = N, st.kd[lane] = kd, st.fb[lane] = fb;
+        if constexpr (TOT) st.depo[lane] = depo;
+    }
+    __syncwarp();
+}
+
+// everything still queued or in flight (end of a kernel's work)
+template <bool TOT, typename Sink>
+__device__ __forceinline__ void drain_all(QuadWarp<TOT> &ws, QuadCounts &qc, const double *__restrict__ inv_k,
+                                          const Sink &sink, int *__restrict__ totals, int lane)
+{
+    drain_inversion<TOT>(ws.q, ws.st, qc.inv, qc.inflight, true, inv_k, sink, totals, lane);
+    drain_exact<TOT>(ws.q, qc.exact, true, sink, totals, lane);
+}
+
+// One batch of up to kBatchDepos depos, one per lane (lanes >= kBatchDepos own none), fluctuation on.  The call-wide index
+// of the depo of lane l is dbase + l, or dbase + dl (of lane l) when the batch comes from an index list (INDIRECT).
+template <bool TOT, bool INDIRECT, typename Sink>
+__device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Sink &sink, float t0, float x0, float st,
+                                                 float sx, float q, bool valid, long long dbase, uint32_t dl,
+                                                 uint64_t id_base, uint64_t seed, double nsigma, bool normal_only,
+                                                 bool normalize, int *__restrict__ totals, QuadWarp<TOT> &ws,
+                                                 QuadCounts &qc, const double *__restrict__ inv_k,
+                                                 unsigned long long &drawn, int lane)
+{
+    QuadScratch &sc = ws.sc;
+    QuadQueues<TOT> &Q = ws.q;
+    const double T0 = t0, X0 = x0, ST = st, SX = sx;
+    Extent et{0, 0}, ex{0, 0};
+    if (valid) {
+        et = axis_extent(T0, ST, nsigma, clip.k_lo, clip.k_hi);
+        ex = axis_extent(X0, SX, nsigma, clip.w_lo, clip.w_hi);
+    }
+    const bool live = et.lo < et.hi && ex.lo < ex.hi;
+    const int nt = live ? et.hi - et.lo : 0, nx = live ? ex.hi - ex.lo : 0;
+    const bool big = nt + nx + 2 + 2 * kEdgePad > kQuadEdgeCap || nt > 255 || nx > 255;
+    const bool flat = live && !big;
+    // quads per wire row: with n_ticks a multiple of 4 every row of a patch starts at the same offset in its quad
+    const bool aligned = (g.n_ticks & 3) == 0;
+    const int nq = aligned ? ((((et.lo & 3) + nt - 1) >> 2) + 1) : (((nt + 2) >> 2) + 1);
+    const int ne = flat ? nt + nx + 2 : 0, nqs = flat ? nx * nq : 0;
+    const int eincl = warp_incl_scan(ne, lane), qincl = warp_incl_scan(nqs, lane);
+    const float Ntr = (float)floor(fabs((double)q) + 0.5);
+    const uint32_t didx = INDIRECT ? dl : (uint32_t)lane;
+    __syncwarp();
+    sc.eoff[lane] = eincl - ne;
+    sc.qoff[lane] = qincl - nqs;
+    if (lane == 31) {
+        sc.eoff[32] = eincl;
+        sc.qoff[32] = qincl;
+    }
+    if (lane < kBatchDepos) {
+        DepoRec rc;
+        rc.lo_t = et.lo, rc.lo_x = ex.lo;
+        rc.shape = (uint32_t)nt | ((uint32_t)nx << 8) | ((uint32_t)nq << 16) | (q < 0.0f ? 0x80000000u : 0u);
+        rc.ebase = 0;
+        rc.t0 = t0, rc.x0 = x0, rc.N = Ntr, rc.idx = didx;
+        rc.inv_t = ST < 1e-6 ? 0.0 : fast_rcp(1.4142135623730951 * ST);
+        rc.inv_x = SX < 1e-6 ? 0.0 : fast_rcp(1.4142135623730951 * SX);
+        sc.rec[lane] = rc;
+        // renormalised patches (reading A24): 1 / (W_t W_x), W = the axis weights summed over the whole, unclipped extent
+        if (normalize)
+            sc.inv_norm[lane] = flat ? __ddiv_rn(1.0, axis_norm(T0, ST, nsigma) * axis_norm(X0, SX, nsigma)) : 1.0;
+    }
+    __syncwarp();
+    if (flat) drawn += (unsigned long long)(nt * nx);
+
+    // patches too big for the scratch: the whole warp walks them one at a time (fp64 sampler per bin)
+    unsigned int big_mask = __ballot_sync(0xffffffffu, live && big);
+    while (big_mask) {
+        const int src = __ffs(big_mask) - 1;
+        big_mask &= big_mask - 1;
+        int tot = 0;
+        const long long dio = dbase + (long long)__shfl_sync(0xffffffffu, didx, src);
+        double inv_norm = 1.0;
+        if (normalize) {
+            if (lane == src) inv_norm = __ddiv_rn(1.0, axis_norm(T0, ST, nsigma) * axis_norm(X0, SX, nsigma));
+            inv_norm = __shfl_sync(0xffffffffu, inv_norm, src);
+        }
+        drawn += raster_depo<true>(__shfl_sync(0xffffffffu, t0, src), __shfl_sync(0xffffffffu, x0, src),
+                                   __shfl_sync(0xffffffffu, st, src), __shfl_sync(0xffffffffu, sx, src),
+                                   __shfl_sync(0xffffffffu, q, src), id_base + (uint64_t)dio, seed, nsigma, g.n_ticks,
+                                   clip.w_lo, clip.w_hi, clip.k_lo, clip.k_hi, sink, lane, &tot, normal_only, inv_norm);
+        if (totals != nullptr) {
+            tot = warp_sum(tot);
+            if (lane == 0 && tot != 0) atomicAdd(totals + dio, tot);
+        }
+    }
+
+    // sub-batches of consecutive depos whose padded edge lists fit the scratch (normally the whole batch)
+    int d0 = 0;
+    while (d0 < 32) {
+        const int ebase = sc.eoff[d0];
+        const unsigned int fits =
+            __ballot_sync(0xffffffffu, lane >= d0 && eincl - ebase + 2 * kEdgePad * (min(lane, kBatchDepos - 1) - d0 + 1) <= kQuadEdgeCap);
+        const int d1 = d0 + __popc(fits); // monotone: the fitting lanes are d0 .. d1-1, at least one
+        const int etot = sc.eoff[d1] - ebase, qbase = sc.qoff[d0], qtot = sc.qoff[d1] - qbase;
+        if (lane >= d0 && lane < d1 && lane < kBatchDepos) sc.rec[lane].ebase = eincl - ne - ebase + 2 * kEdgePad * (lane - d0);
+        __syncwarp();
+        // ---- edges: erf((edge - centre) / (sqrt2 sigma)) in fp64, flat over the sub-batch ---------------------------
+        for (int e0 = 0; e0 < etot; e0 += 32) {
+            const int e = e0 + lane;
+            const bool act = e < etot;
+            const int own = owner_of(sc.eoff, ebase + (act ? e : 0));
+            const int le = ebase + e - sc.eoff[own];
+            const DepoRec &rc = sc.rec[own];
+            const int4 a = *reinterpret_cast<const int4 *>(&rc.lo_t);
+            const float2 ctr = *reinterpret_cast<const float2 *>(&rc.t0);
+            const double2 inv2 = *reinterpret_cast<const double2 *>(&rc.inv_t);
+            const int nto = a.z & 255;
+            const bool on_t = le <= nto;
+            const int coord = on_t ? a.x + le : a.y + (le - nto - 1);
+            const double centre = (double)(on_t ? ctr.x : ctr.y), inv = on_t ? inv2.x : inv2.y;
+            double E;
+            if (inv == 0.0) { // all weight in bin floor(centre) (A4): a step from -1 to +1 after that bin's low edge
+                E = ((double)coord <= floor(centre)) ? -1.0 : 1.0;
             } else {
-                const float qq = __shfl_sync(0xffffffffu, q, own);
-                const float scale = normalize ? (float)__shfl_sync(0xffffffffu, inv_norm, own) : 1.0f;
-                if (act) sink.add(wire, tick, qq * (wt * wx) * scale);
+                E = erf_from_table(g_erf_tab, __dsub_rn((double)coord, centre) * inv);
+            }
+            if (act) sc.edge[a.w + kEdgePad + le + (on_t ? 0 : kEdgePad)] = E;
+        }
+        __syncwarp();
+        // ---- quads ----------------------------------------------------------------------------------------------------
+        for (int s0 = 0; s0 < qtot; s0 += 32) {
+            const int s = s0 + lane;
+            const bool act = s < qtot;
+            const int own = owner_of(sc.qoff, qbase + (act ? s : 0));
+            const int l = act ? qbase + s - sc.qoff[own] : 0;
+            const DepoRec &rc = sc.rec[own];
+            const int4 a = *reinterpret_cast<const int4 *>(&rc.lo_t);
+            const float4 bq = *reinterpret_cast<const float4 *>(&rc.t0);
+            const float Nf = bq.z;
+            const uint32_t didx_o = __float_as_uint(bq.w);
+            const int nto = a.z & 255, nqo = (a.z >> 16) & 255;
+            const bool neg = a.z < 0;
+            // wire row of the quad, l / nq: (l + 1/2) / nq is at least 1/(2 nq) away from an integer, far more than the
+            // rounding of the product for l < 2^16
+            const int j = __float2int_rz(((float)l + 0.5f) * __frcp_rn((float)max(nqo, 1)));
+            const int qi = l - j * nqo;
+            const int wire = a.y + j;
+            const uint32_t g0 = (uint32_t)wire * (uint32_t)g.n_ticks + (uint32_t)a.x; // absolute bin of the row's first tick
+            const uint32_t gq = (g0 >> 2) + (uint32_t)qi;
+            const int ii0 = (int)(4u * gq - g0); // patch tick index of the quad's first bin: -3 .. nt-1
+            const double *E = sc.edge + a.w + kEdgePad;
+            const double wxq = 0.25 * (E[nto + 1 + kEdgePad + j + 1] - E[nto + 1 + kEdgePad + j]); // wx / 2
+            const double inv_n = normalize ? sc.inv_norm[own] : 1.0;
+            const long long dio = dbase + (long long)didx_o;
+            const uint4 words = fluct_words(seed, id_base + (uint64_t)dio, (uint64_t)gq);
+            const uint32_t idx0 = sink.index(wire, a.x);
+            const double Nd = (double)Nf;
+
+            // the four bins of the quad, one after the other (a loop, not unrolled: the code of the kernel has to stay
+            // inside the instruction cache)
+#pragma unroll 1
+            for (int k = 0; k < 4; ++k) {
+                uint32_t w = k == 0 ? words.x : k == 1 ? words.y : k == 2 ? words.z : words.w;
+                const double ea = E[ii0 + k], eb = E[ii0 + k + 1];
+                const int ii = ii0 + k;
+                const bool v = act && (unsigned)ii < (unsigned)nto;
+                double p = __dmul_rn(__dsub_rn(eb, ea), wxq); // = wt wx: the two factors 1/2 are exact scalings
+                if (normalize) p *= inv_n;
+                const bool nontrivial = v && p > 0.0 && p < 1.0 && Nf > 0.0f;
+                float kv = (p >= 1.0) ? Nf : 0.0f; // p <= 0 or N = 0: k = 0; p >= 1: k = N
+                bool mirror = false;
+                if (!normal_only && p > 0.5 && p < 1.0) {
+                    mirror = true;
+                    p = __dsub_rn(1.0, p);
+                    w = ~w;
+                }
+                const double mu = __dmul_rn(Nd, p);
+                const bool small = !normal_only && mu < 16.0;
+                bool decided = !nontrivial;
+                if (nontrivial) {
+                    if (small) {
+                        // u <= 1 - mu implies u <= (1-p)^N = F(0), i.e. k = 0 (Bernoulli); in fp32 with a margin that
+                        // covers the roundings of u, mu and their sum (3 x 2^-24)
+                        const float uf = fmaf((float)w, 2.3283064365386963e-10f, 1.1641532182693481e-10f);
+                        decided = uf + (float)mu <= 0.9999996f;
+                    } else if (p <= 0.5) {
+                        decided = fast_normal_draw(Nf, p, mu, w, kv);
+                    }
+                }
+                const uint32_t fb = (idx0 + (uint32_t)ii) | (mirror ? kBinMirror : 0u) | (neg ? kBinNegative : 0u);
+                if (v && decided) commit_draw<TOT>(sink, totals, fb, Nf, kv, (uint32_t)dio);
+                const bool to_inv = nontrivial && !decided && small, to_exact = nontrivial && !decided && !small;
+                const unsigned int mi = __ballot_sync(0xffffffffu, to_inv), me = __ballot_sync(0xffffffffu, to_exact);
+                if (to_inv || to_exact) {
+                    const int pos = to_inv ? qc.inv + __popc(mi & ((1u << lane) - 1u))
+                                           : kInvCap + qc.exact + __popc(me & ((1u << lane) - 1u));
+                    Q.p[pos] = p;
+                    Q.N[pos] = Nf;
+                    Q.w[pos] = w;
+                    Q.bin[pos] = fb;
+                    if constexpr (TOT) Q.depo[pos] = (uint32_t)dio;
+                }
+                qc.inv += __popc(mi);
+                qc.exact += __popc(me);
+                __syncwarp();
+                if (qc.inv >= kInvDrainAt)
+                    drain_inversion<TOT>(Q, ws.st, qc.inv, qc.inflight, false, inv_k, sink, totals, lane);
+                if (qc.exact >= 32) drain_exact<TOT>(Q, qc.exact, false, sink, totals, lane);
             }
         }
         __syncwarp();
@@ -474,45 +727,65 @@ __device__ __forceinline__ void raster_batch_body(GridDims g, Clip clip, const S
     }
 }
 
+// shared memory of the batch kernels
+template <bool FLUCT, bool TOT>
+struct BatchSmem {
+    FlatScratch scratch[kBatchWarps];
+};
+template <bool TOT>
+struct BatchSmem<true, TOT> {
+    double inv_k[kQuadInvTab]; // 1/k of the inversion recurrence
+    QuadWarp<TOT> warp[kBatchWarps];
+};
+
+__device__ __forceinline__ void fill_inv_k(double *inv_k)
+{
+    for (int k = threadIdx.x; k < kQuadInvTab; k += blockDim.x) inv_k[k] = k ? 1.0 / (double)k : 0.0;
+    __syncthreads();
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// atomic mode: persistent warps; a warp's first batch is its own index in the grid, further ones come from a device
+// counter (guided: kBatchDepos depos at a time, kTailDepos at a time near the end)
+// ------------------------------------------------------------------------------------------------------------------
 template <bool FLUCT, bool TOT, bool FIX>
 __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
                                                                         uint64_t id_base, uint64_t seed, double nsigma,
                                                                         float *__restrict__ S, int *__restrict__ totals,
                                                                         Counters *counters, bool normal_only, bool normalize)
 {
-    using T = typename std::conditional<FLUCT, double, float>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     BatchSmem<FLUCT, TOT> &sm = *reinterpret_cast<BatchSmem<FLUCT, TOT> *>(smem_raw);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    BatchScratch<FLUCT> &sc = sm.scratch[wid];
     // FIX: S points at the 64-bit fixed-point grid (deterministic mode without tiles)
     using Sink = typename std::conditional<FIX, FixSink, GlobalSink>::type;
     const Sink sink = make_grid_sink<FIX>(S, g.n_ticks);
     const Clip clip{0, g.n_wires, 0, g.n_ticks};
     // guided batches: kBatchDepos depos at a time, then kTailDepos at a time for the last kTailPerWarp depos per warp of the
-    // grid, so that the warps run out of work within a short batch of one another (a batch of 8 lasts ~20 us on
-    // configs[1], where a warp gets only 3-4 of them)
+    // grid, so that the warps run out of work within a short batch of one another (on configs[1] a warp gets only
+    // 3-4 batches of 8)
     const long long n_warps_grid = (long long)gridDim.x * kBatchWarps;
     const long long tail_depos = n_warps_grid * kTailPerWarp < n ? n_warps_grid * kTailPerWarp : n;
     const long long big_batches = (n - tail_depos) >> kBatchShift;
     const long long big_depos = big_batches << kBatchShift;
     const long long n_batches = big_batches + (n - big_depos + kTailDepos - 1) / kTailDepos;
     unsigned long long drawn = 0, skipped = 0;
-    int qcount[kNumDrawQueues] = {};
+    QuadCounts qc;
+    if constexpr (FLUCT) fill_inv_k(sm.inv_k);
     // the grid is one wave, so the next kernel's CTAs may take the slots this one frees as it drains.  As a
     // programmatic dependent itself it only overlaps a preceding KERNEL's tail: copies and memsets ahead of it in the
     // stream are still fully ordered (checked with 300 host-buffer plane-events of changing depos, 0 mismatches)
     pdl_trigger();
     pdl_wait();
 
-    // (fetching the NEXT batch's index early, to hide the ~1 us round trip of this atomic -- 14 % of the stall samples on
-    // configs[1] -- was tried: a warp then sits on a batch while it works on another, and the load balance suffers more
-    // than the latency costs: 75.7 -> 82.6 us)
-    for (;;) {
-        long long batch = 0;
-        if (lane == 0) batch = (long long)atomicAdd(&counters->next_batch, 1ull);
-        batch = __shfl_sync(0xffffffffu, batch, 0);
-        if (batch >= n_batches) break;
+    // The first batch of a warp is its index in the grid: all warps start at once, and thousands of atomics on one
+    // counter would queue up behind one another for microseconds (same-address atomics are served one every ~2 ns; with
+    // every batch fetched from the counter the fetch was 42 % of the stall samples of the unfluctuated raster on
+    // configs[1]).  Later batches come from the counter, which keeps the load balanced.
+    // (Fetching the NEXT batch's index early to hide the round trip was tried: a warp then sits on a batch while it
+    // works on another, and the load balance suffers more than the latency costs.)
+    long long batch = (long long)blockIdx.x * kBatchWarps + wid;
+    while (batch < n_batches) {
         const long long first = batch < big_batches ? batch << kBatchShift : big_depos + (batch - big_batches) * kTailDepos;
         const int count = batch < big_batches ? kBatchDepos : kTailDepos;
         const long long i = first + lane;
@@ -524,24 +797,22 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
             skipped += !valid;
         }
         if constexpr (FLUCT)
-            raster_batch_body<FLUCT, TOT, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, id_base, seed, nsigma,
-                                                 normal_only, normalize, totals, sc, &sm.queues[wid], qcount, drawn, lane);
+            raster_quad_body<TOT, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, id_base, seed, nsigma,
+                                         normal_only, normalize, totals, sm.warp[wid], qc, sm.inv_k, drawn, lane);
         else
-            raster_batch_body<FLUCT, TOT, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, id_base, seed, nsigma,
-                                                 normal_only, normalize, totals, sc, (DrawQueues<TOT> *)nullptr, qcount, drawn, lane);
+            raster_flat_body(g, clip, sink, t0, x0, st, sx, q, valid, nsigma, normalize, sm.scratch[wid], drawn, lane);
+        if (lane == 0) batch = n_warps_grid + (long long)atomicAdd(&counters->next_batch, 1ull);
+        batch = __shfl_sync(0xffffffffu, batch, 0);
     }
-    if constexpr (FLUCT) {
-#pragma unroll
-        for (int c = 0; c < kNumDrawQueues; ++c) drain_queue(sm.queues[wid], c, qcount[c], true, sink, totals, lane);
-    }
+    if constexpr (FLUCT) drain_all<TOT>(sm.warp[wid], qc, sm.inv_k, sink, totals, lane);
     drawn = warp_sum(drawn);
     skipped = warp_sum(skipped);
     if (lane == 0) {
         if (drawn) atomicAdd(&counters->bins_drawn, drawn);
         if (skipped) atomicAdd(&counters->depos_skipped, skipped);
-        // the last warp to leave re-arms the batch counter for the next launch on this stream
+        // the last warp to leave re-arms the batch counter for the next launch on this stream (every warp has made its
+        // last fetch before it adds itself here)
         const unsigned long long n_warps = (unsigned long long)gridDim.x * kBatchWarps;
-        __threadfence();
         if (atomicAdd(&counters->warps_done, 1ull) == n_warps - 1) {
             counters->next_batch = 0ull;
             counters->warps_done = 0ull;
@@ -648,13 +919,13 @@ constexpr int kTileWarps = 8, kTileSlices = 8, kSliceEntries = 256;
 template <bool FLUCT, bool TOT>
 struct TileSmem {
     unsigned long long acc[kTileW * kTileT];
-    BatchScratch<FLUCT> scratch[kTileWarps];
+    FlatScratch scratch[kTileWarps];
 };
 template <bool TOT>
 struct TileSmem<true, TOT> {
     unsigned long long acc[kTileW * kTileT];
-    BatchScratch<true> scratch[kTileWarps];
-    DrawQueues<TOT> queues[kTileWarps];
+    double inv_k[kQuadInvTab];
+    QuadWarp<TOT> warp[kTileWarps];
 };
 
 template <bool FLUCT, bool TOT>
@@ -680,13 +951,13 @@ __global__ void __launch_bounds__(kTileWarps * 32, 2) tile_accumulate_kernel(Gri
     const int w0 = tw * kTileW, k0 = tt * kTileT;
     const int w1 = min(w0 + kTileW, g.n_wires), k1 = min(k0 + kTileT, g.n_ticks);
     for (int i = threadIdx.x; i < kTileW * kTileT; i += blockDim.x) sm.acc[i] = 0ull;
+    if constexpr (FLUCT) fill_inv_k(sm.inv_k);
     __syncthreads();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const TileSink sink{sm.acc, w0, k0};
     const Clip clip{w0, w1, k0, k1};
-    BatchScratch<FLUCT> &sc = sm.scratch[wid];
     unsigned long long drawn = 0;
-    int qcount[kNumDrawQueues] = {};
+    QuadCounts qc;
     for (unsigned int e0 = beg + (unsigned int)wid * kBatchDepos; e0 < end; e0 += kTileWarps * kBatchDepos) {
         float t0 = 0.f, x0 = 0.f, st = 0.f, sx = 0.f, q = 0.f;
         unsigned int i = 0;
@@ -697,16 +968,12 @@ __global__ void __launch_bounds__(kTileWarps * 32, 2) tile_accumulate_kernel(Gri
             valid = depo_valid(t0, x0, st, sx, q); // listed depos are valid; kept for symmetry with the atomic kernel
         }
         if constexpr (FLUCT)
-            raster_batch_body<FLUCT, TOT, true>(g, clip, sink, t0, x0, st, sx, q, valid, 0ll, i, id_base, seed, nsigma,
-                                                normal_only, normalize, totals, sc, &sm.queues[wid], qcount, drawn, lane);
+            raster_quad_body<TOT, true>(g, clip, sink, t0, x0, st, sx, q, valid, 0ll, i, id_base, seed, nsigma, normal_only,
+                                        normalize, totals, sm.warp[wid], qc, sm.inv_k, drawn, lane);
         else
-            raster_batch_body<FLUCT, TOT, true>(g, clip, sink, t0, x0, st, sx, q, valid, 0ll, i, id_base, seed, nsigma,
-                                                normal_only, normalize, totals, sc, (DrawQueues<TOT> *)nullptr, qcount, drawn, lane);
+            raster_flat_body(g, clip, sink, t0, x0, st, sx, q, valid, nsigma, normalize, sm.scratch[wid], drawn, lane);
     }
-    if constexpr (FLUCT) {
-#pragma unroll
-        for (int c = 0; c < kNumDrawQueues; ++c) drain_queue(sm.queues[wid], c, qcount[c], true, sink, totals, lane);
-    }
+    if constexpr (FLUCT) drain_all<TOT>(sm.warp[wid], qc, sm.inv_k, sink, totals, lane);
     drawn = warp_sum(drawn);
     if (lane == 0 && drawn) atomicAdd(&counters->bins_drawn, drawn);
     __syncthreads();

@@ -96,6 +96,44 @@ __global__ void debug_binomial_kernel(const double *N, const double *p, const un
     k[i] = binomial_draw(N[i], p[i], w[i], normal_only);
 }
 
+// fast path of the rounded-normal draw (rng.cuh): k and whether the fp32 guard accepted it
+__global__ void debug_fast_normal_kernel(const double *N, const double *p, const unsigned int *w, double *k, int *ok,
+                                         long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float kf = 0.f;
+    const bool a = p[i] > 0.0 && p[i] <= 0.5 && fast_normal_draw((float)N[i], p[i], __dmul_rn(N[i], p[i]), w[i], kf);
+    k[i] = (double)kf;
+    ok[i] = a ? 1 : 0;
+}
+
+// z32_from_word against the fp64 AS 241 quantile over the words first .. first + count - 1:
+// out[0] = max |z32 - z64| over the accepted words, out[1] = max |z64| over them, out[2] = number accepted (as a double),
+// out[3] = max |z32 - z64| / max(1, |z64|)
+__global__ void debug_z32_scan_kernel(unsigned long long first, unsigned long long count, unsigned long long *out)
+{
+    double e_abs = 0.0, z_max = 0.0, e_rel = 0.0;
+    unsigned long long accepted = 0;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < count;
+         i += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint32_t w = (uint32_t)(first + i);
+        float z32;
+        if (!z32_from_word(w, z32)) continue;
+        const double z64 = word_is_central(w) ? as241_central(w) : as241_tail(w);
+        const double e = fabs((double)z32 - z64), az = fabs(z64);
+        e_abs = fmax(e_abs, e);
+        z_max = fmax(z_max, az);
+        e_rel = fmax(e_rel, e / fmax(1.0, az));
+        ++accepted;
+    }
+    // non-negative doubles order like their bit patterns
+    atomicMax(out + 0, (unsigned long long)__double_as_longlong(e_abs));
+    atomicMax(out + 1, (unsigned long long)__double_as_longlong(z_max));
+    atomicAdd(out + 2, accepted);
+    atomicMax(out + 3, (unsigned long long)__double_as_longlong(e_rel));
+}
+
 } // namespace
 
 cudaError_t build_response_spectrum(const float *dev_R, int n_rw, int n_rt, int pad_w, int pad_t, int spec_stride,
@@ -133,6 +171,23 @@ cudaError_t launch_debug_binomial(const double *N, const double *p, const unsign
 {
     if (n <= 0) return cudaSuccess;
     debug_binomial_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(N, p, w, k, n, normal_only);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_debug_fast_normal(const double *N, const double *p, const unsigned int *w, double *k, int *ok,
+                                     long long n, cudaStream_t st)
+{
+    if (n <= 0) return cudaSuccess;
+    debug_fast_normal_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(N, p, w, k, ok, n);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_debug_z32_scan(unsigned long long first, unsigned long long count, unsigned long long *out4,
+                                  cudaStream_t st)
+{
+    cudaError_t err = cudaMemsetAsync(out4, 0, 4 * sizeof(unsigned long long), st);
+    if (err != cudaSuccess || count == 0) return err;
+    debug_z32_scan_kernel<<<148 * 8, 256, 0, st>>>(first, count, out4);
     return cudaGetLastError();
 }
 

@@ -159,6 +159,10 @@ __device__ __forceinline__ double exp_neg(double y)
     return __hiloint2double(__double2hiint(e) + (k << 20), __double2loint(e)); // e in [0.7, 1.42), k >= -1010
 }
 
+// log(1 - p) for 2^-5 <= p <= 1/2: rare (N < 512 for mu < 16), kept out of line so that the library routine is
+// instantiated once per kernel
+static __device__ __noinline__ double log1m_large(double p) { return log1p(-p); }
+
 // (1 - p)^N for 0 < p <= 1/2
 __device__ __forceinline__ double pow_one_minus(double N, double p)
 {
@@ -169,7 +173,7 @@ __device__ __forceinline__ double pow_one_minus(double N, double p)
         for (int j = 1; j < 11; ++j) g = fma(g, p, c_log1m[j]);
         L = -p * g;
     } else {
-        L = log1p(-p);
+        L = log1m_large(p);
     }
     return exp_neg(N * L);
 }
@@ -209,8 +213,8 @@ __device__ __forceinline__ double finish_normal(double N, double p, double z)
     return k > N ? N : k;
 }
 
-// AS 241 PPND16, |u - 1/2| <= 0.425
-__device__ __forceinline__ double draw_normal_central(double N, double p, uint32_t w)
+// AS 241 PPND16, |u - 1/2| <= 0.425: the quantile z
+__device__ __forceinline__ double as241_central(uint32_t w)
 {
     const double q = word_to_u01(w) - 0.5;
     const double r = 0.180625 - q * q;
@@ -220,12 +224,16 @@ __device__ __forceinline__ double draw_normal_central(double N, double p, uint32
         num = fma(num, r, c_as241_a[j]);
         den = fma(den, r, c_as241_b[j]);
     }
-    return finish_normal(N, p, fast_div(q * num, den));
+    return fast_div(q * num, den);
+}
+__device__ __forceinline__ double draw_normal_central(double N, double p, uint32_t w)
+{
+    return finish_normal(N, p, as241_central(w));
 }
 
 // AS 241 PPND16, |u - 1/2| > 0.425.  r = sqrt(-log(min(u, 1-u))) <= sqrt(33 log 2) = 4.79 for a 32-bit word, so the
 // routine's third region (r > 5) cannot be reached from a 32-bit word and is not coded.
-__device__ __forceinline__ double draw_normal_tail(double N, double p, uint32_t w)
+__device__ __forceinline__ double as241_tail(uint32_t w)
 {
     const double u = word_to_u01(w);
     const double q = u - 0.5;
@@ -237,7 +245,11 @@ __device__ __forceinline__ double draw_normal_tail(double N, double p, uint32_t 
         den = fma(den, r, c_as241_d[j]);
     }
     const double val = fast_div(num, den);
-    return finish_normal(N, p, q < 0.0 ? -val : val);
+    return q < 0.0 ? -val : val;
+}
+__device__ __forceinline__ double draw_normal_tail(double N, double p, uint32_t w)
+{
+    return finish_normal(N, p, as241_tail(w));
 }
 
 // the draw of an already classified bin (cls >= 0), mirror undone
@@ -247,6 +259,64 @@ __device__ __forceinline__ double draw_classified(int cls, double N, double p, u
                      : cls == kDrawNormalCentral ? draw_normal_central(N, p, w)
                                                  : draw_normal_tail(N, p, w);
     return mirror ? N - k : k;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Guarded fp32 fast path of the rounded-normal branch (mu >= 16, or every mu with the normal-approximation sampler).
+// k = clamp(rint(mu + sd z), 0, N) is an integer decision: if an fp32 estimate x32 of x = mu + sd z is farther from the
+// nearest half-integer than a bound E on |x32 - x|, then rint(x32) = rint(x) and the fp64 evaluation is not needed.
+// Bins that fail the test are drawn again by the fp64 routines above (the raster queues them), so the result is the
+// exact sampler's for every bin; only the cost differs.
+//
+// z32: Phi^-1(u) = x g(wl), x = 2u - 1, wl = -ln(1 - x^2) = -ln(4 t (1 - t)), t = min(u, 1 - u) taken from the integer
+// word so that the tails keep their relative accuracy; g is a degree-8 polynomial in (wl - 2.5) on wl < 5
+// (csrc/z32_fit.py; |u - 1/2| < 0.4983, 99.66 % of the words; the rest are not accepted).  Its error against the fp64
+// AS 241 routine is MEASURED over all 2^32 words by wcsim_debug_z32_scan (tests/test_gpu_fastpath.py): kZ32Err below is
+// asserted there to be at least twice the measured maximum of |z32 - z64|.
+// ------------------------------------------------------------------------------------------------------------------
+static __constant__ float c_z32[9] = {4.035463519e-08f, 4.861039429e-07f, -4.990565230e-06f, -6.217992905e-06f,
+                                      3.091502003e-04f, -1.773010124e-03f, -5.908171181e-03f, 3.488026559e-01f,
+                                      2.123313665e+00f}; // highest power first
+constexpr float kZ32Err = 4.0e-6f; // bound on |z32(w) - z_AS241(w)| for the accepted words (|z| < 2.93)
+
+__device__ __forceinline__ bool z32_from_word(uint32_t w, float &z)
+{
+    const float x = fmaf((float)(int)(w ^ 0x80000000u), 4.656612873077393e-10f, 2.3283064365386963e-10f); // 2u - 1
+    const uint32_t m = min(w, ~w);
+    const float t = fmaf((float)m, 2.3283064365386963e-10f, 1.1641532182693481e-10f); // min(u, 1-u)
+    const float wl = -0.6931471805599453f * __log2f(4.0f * t * (1.0f - t));
+    const float d = wl - 2.5f;
+    float g = c_z32[0];
+#pragma unroll
+    for (int j = 1; j < 9; ++j) g = fmaf(g, d, c_z32[j]);
+    z = x * g;
+    return wl < 5.0f;
+}
+
+// Error budget of x32 = fmaf(sd32, z32, mu32) against x = fma(sd, z, mu) of finish_normal, for 0 < p <= 1/2 (u = 2^-24):
+//   mu32 = fp32(mu):                      |d mu| <= u mu
+//   q32 = fp32(1 - fp32(p)):              relative 2u (1 - p >= 1/2)
+//   v32 = fp32(mu32 q32):                 relative 4u;   sd32 = sqrt.approx(v32): relative 2u + 2^-22 = 6u
+//   z32:                                  |d z| <= kZ32Err, |z| < 2.93
+//   fmaf rounding:                        u (mu + 2.93 sd)
+//   => |x32 - x| <= 2u mu + (7u 2.93 + kZ32Err) sd + second order  <  1.2e-7 mu + 5.3e-6 sd.
+// The guard uses 2.5e-7 mu + 8e-6 sd + 1e-6 (the constant also covers x64's own rounding and the bound's evaluation).
+constexpr float kGuardMu = 2.5e-7f, kGuardSd = 8.0e-6f, kGuardAbs = 1.0e-6f;
+
+// true: k is the exact sampler's rounded-normal draw for (N, p; w), p <= 1/2, mu = N p (fp64).  false: not decided.
+__device__ __forceinline__ bool fast_normal_draw(float N, double p, double mu, uint32_t w, float &k)
+{
+    float z;
+    bool ok = z32_from_word(w, z);
+    const float muf = (float)mu, pf = (float)p;
+    float sd;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(sd) : "f"(muf * (1.0f - pf))); // MUFU.SQRT: relative error <= 2^-22
+    const float x = fmaf(sd, z, muf);
+    const float kf = rintf(x);
+    const float E = fmaf(kGuardMu, muf, fmaf(kGuardSd, sd, kGuardAbs));
+    ok = ok && (fabsf(x - kf) < 0.5f - E); // false for NaN, and for every x once E >= 1/2 (mu > 2e6)
+    k = fminf(fmaxf(kf, 0.0f), N);
+    return ok;
 }
 
 // the whole sampler for one bin (debug hook, big-patch and tiled paths)

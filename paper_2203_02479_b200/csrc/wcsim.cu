@@ -712,6 +712,22 @@ int wcsim_debug_normal_draw(const double *dev_N, const double *dev_p, const unsi
     return WCSIM_OK;
 }
 
+int wcsim_debug_fast_normal(const double *dev_N, const double *dev_p, const unsigned int *dev_w, double *dev_k,
+                            int *dev_ok, long long n, void *cuda_stream)
+{
+    if (n < 0 || (n > 0 && (!dev_N || !dev_p || !dev_w || !dev_k || !dev_ok))) return WCSIM_EINVAL;
+    CU_TRY(launch_debug_fast_normal(dev_N, dev_p, dev_w, dev_k, dev_ok, n, (cudaStream_t)cuda_stream));
+    return WCSIM_OK;
+}
+
+int wcsim_debug_z32_scan(unsigned long long first_word, unsigned long long n_words, double *dev_out4, void *cuda_stream)
+{
+    if (!dev_out4 || first_word + n_words > (1ull << 32)) return WCSIM_EINVAL;
+    CU_TRY(launch_debug_z32_scan(first_word, n_words, reinterpret_cast<unsigned long long *>(dev_out4),
+                                 (cudaStream_t)cuda_stream));
+    return WCSIM_OK;
+}
+
 int wcsim_debug_response_spectrum(wcsim_plan *plan, float *host_out)
 {
     if (!plan || !host_out) return WCSIM_EINVAL;
