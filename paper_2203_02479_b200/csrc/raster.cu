@@ -271,7 +271,7 @@ struct FlatScratch {
 template <typename Sink>
 __device__ __forceinline__ void raster_flat_body(GridDims g, Clip clip, const Sink &sink, float t0, float x0, float st,
                                                  float sx, float q, bool valid, double nsigma, bool normalize,
-                                                 FlatScratch &sc, unsigned long long &drawn, int lane)
+                                                 FlatScratch &sc, unsigned int &drawn, int lane)
 {
     const double T0 = t0, X0 = x0, ST = st, SX = sx;
     Extent et{0, 0}, ex{0, 0};
@@ -295,7 +295,7 @@ __device__ __forceinline__ void raster_flat_body(GridDims g, Clip clip, const Si
         sc.boff[32] = bincl;
     }
     __syncwarp();
-    drawn += (unsigned long long)nb;
+    drawn += (unsigned int)nb;
 
     // patches too big for the scratch: the whole warp walks them one at a time
     unsigned int big_mask = __ballot_sync(0xffffffffu, live && big);
@@ -366,20 +366,21 @@ __device__ __forceinline__ void raster_flat_body(GridDims g, Clip clip, const Si
 }
 
 // ---- fluctuation on: quads ------------------------------------------------------------------------------------------
-// One Philox call gives the words of four consecutive absolute grid bins (reading A8), so the unit of work of a lane is
-// a QUAD: (depo, wire row of its patch, aligned group of four bins g>>2 of that row).  A lane finds its depo once, calls
-// Philox once, loads the five tick-edge values and the wire weight once and then decides its (up to) four bins:
-//   * k known without a draw (p <= 0, p >= 1, N = 0, or u <= 1 - mu, which implies u <= (1-p)^N);
-//   * mu >= 16 (or the normal-approximation sampler): the guarded fp32 estimate of rng.cuh; accepted for ~99 % of such bins;
-//   * everything else goes to one of two per-warp shared-memory queues and is drawn by the fp64 routines of rng.cuh:
-//     the inversion queue (mu < 16), worked off by a loop whose lanes pick up the next queued bin as soon as their
-//     own inversion ends (a lane's trip count is k+1; without that the warp waits for its slowest lane), and the exact
-//     queue (bins the fp32 guard did not accept), drawn 32 at a time.
-// The edges of a batch are laid out per depo as [3 pad][nt+1 tick edges][3 pad][nx+1 wire edges], so that the five
-// loads of a quad never need a bounds check (pad values only ever reach bins that are masked off).
-constexpr int kQuadEdgeCap = 256, kEdgePad = 3;
-constexpr int kInvCap = 96, kInvDrainAt = 64, kExactCap = 64;
-constexpr int kQuadInvTab = 64;
+// One Philox call gives the words of four consecutive absolute grid bins (reading A8), so the unit of work of the front
+// end is a QUAD: (depo, wire row of its patch, aligned group of four bins g>>2 of that row).  A lane finds its depo once,
+// calls Philox once, loads the wire weight once and then classifies its (up to) four bins:
+//   * k known without a draw (p <= 0, p >= 1, N = 0, or u <= 1 - mu, which implies u <= (1-p)^N): added at once;
+//   * everything else is pushed to one of five per-warp shared-memory queues and drawn from there 32 bins at a time by
+//     straight-line code, all lanes busy:
+//     NORMAL  (mu >= 16, or the normal-approximation sampler): the guarded fp32 estimate of rng.cuh;
+//     INV_A/B/C (mu < 2 / < 6 / < 16): the guarded fp32 inversion of rng.cuh with 8 / 16 / 32 terms;
+//     EXACT   whatever the fp32 guards do not accept (~1 %), and bins not eligible for them: the fp64 routines.
+// The edges of a batch are laid out per depo as [3 pad][nt+1 tick edges][3 pad][nx+1 wire edges], so that the loads of a
+// quad never need a bounds check (pad values only ever reach bins that are masked off).
+constexpr int kQuadEdgeCap = 192, kEdgePad = 3;
+constexpr int kQueueCap = 64; // entries per queue: at most 31 left over + 32 pushed
+enum QuadQueue : int { kQNorm = 0, kQInvA = 1, kQInvB = 2, kQInvC = 3, kQExact = 4, kNumQuadQueues = 5 };
+constexpr int kQTotal = kNumQuadQueues * kQueueCap;
 
 struct alignas(16) DepoRec {
     int lo_t, lo_x;  // first tick / wire of the clipped patch
@@ -396,33 +397,25 @@ struct QuadScratch {
     double inv_norm[kBatchDepos];
     int eoff[33], qoff[33];
 };
-// queue entry: 20 bytes (24 with per-depo totals).  [0, kInvCap): inversion queue; [kInvCap, kInvCap + kExactCap): exact queue
+// queue entry: 20 bytes (24 with per-depo totals); queue c holds entries c kQueueCap .. c kQueueCap + fill - 1
 template <bool TOT>
 struct QuadQueues {
-    double p[kInvCap + kExactCap];   // after the mirror: 0 < p <= 1/2
-    float N[kInvCap + kExactCap];
-    uint32_t w[kInvCap + kExactCap]; // after the mirror
-    uint32_t bin[kInvCap + kExactCap]; // sink index | kBinMirror | kBinNegative
-    uint32_t depo[TOT ? kInvCap + kExactCap : 1];
-};
-// inversions in flight between two calls of drain_inversion (one per lane)
-template <bool TOT>
-struct InvState {
-    double f[32], c[32], u[32], r[32], rN1[32];
-    float N[32], kd[32];
-    uint32_t fb[32];
-    uint32_t depo[TOT ? 32 : 1];
+    double p[kQTotal];     // after the mirror: 0 < p <= 1/2 (normal-approximation sampler: 0 < p < 1)
+    float N[kQTotal];      // exact queue: -N marks a bin of the inversion class (mu < 16)
+    uint32_t w[kQTotal];   // after the mirror
+    uint32_t bin[kQTotal]; // sink index | kBinMirror | kBinNegative
+    uint32_t depo[TOT ? kQTotal : 1];
 };
 template <bool TOT>
 struct QuadWarp {
     QuadScratch sc;
     QuadQueues<TOT> q;
-    InvState<TOT> st;
 };
-// per-warp registers that live across batches
+// per-warp registers that live across batches: the fills of the four fp32 queues, 8 bits each (kQNorm lowest), and of the
+// exact queue
 struct QuadCounts {
-    int inv = 0, exact = 0;
-    uint32_t inflight = 0; // lanes whose InvState slot holds an unfinished inversion
+    uint32_t fast = 0;
+    int exact = 0;
 };
 
 template <bool TOT, typename Sink>
@@ -437,113 +430,98 @@ __device__ __forceinline__ void commit_draw(const Sink &sink, int *__restrict__ 
     }
 }
 
-// the exact queue: bins whose fp32 estimate was too close to a rounding boundary; the fp64 AS 241 routines
+// the exact queue: the fp64 routines of rng.cuh, 32 bins at a time (out of line: it is rare).  Returns the new fill.
 template <bool TOT, typename Sink>
-__device__ __noinline__ void drain_exact(QuadQueues<TOT> &Q, int &count, bool everything, const Sink &sink,
-                                            int *__restrict__ totals, int lane)
+__device__ __noinline__ int drain_exact(QuadQueues<TOT> *Qp, int count, bool everything, Sink sink, int *__restrict__ totals,
+                                        int lane)
 {
+    QuadQueues<TOT> &Q = *Qp;
     while (count >= 32 || (everything && count > 0)) {
         const int take = min(32, count);
         count -= take;
         if (lane < take) {
-            const int e = kInvCap + count + lane;
-            const double N = (double)Q.N[e], p = Q.p[e];
+            const int e = kQExact * kQueueCap + count + lane;
+            const float Nq = Q.N[e];
+            const double N = (double)fabsf(Nq), p = Q.p[e];
             const uint32_t w = Q.w[e];
-            const double k = word_is_central(w) ? draw_normal_central(N, p, w) : draw_normal_tail(N, p, w);
-            commit_draw<TOT>(sink, totals, Q.bin[e], Q.N[e], (float)k, TOT ? Q.depo[e] : 0u);
+            const double k = Nq < 0.0f               ? draw_inversion(N, p, w)
+                             : word_is_central(w) ? draw_normal_central(N, p, w)
+                                                  : draw_normal_tail(N, p, w);
+            commit_draw<TOT>(sink, totals, Q.bin[e], fabsf(Nq), (float)k, TOT ? Q.depo[e] : 0u);
         }
         __syncwarp();
     }
+    return count;
 }
 
-// The inversion queue (reading A6, mu < 16): k = the number of CDF values F(0), F(1), ... below u, summed term by term
-// in fp64 exactly as draw_inversion does.  Every lane runs its own inversion; a lane whose inversion has ended commits it
-// and takes the next queued bin, so the loop's lanes stay busy whatever the individual trip counts are.  With
-// `finish` false the call returns as soon as the queue is empty and parks the unfinished inversions in `st`
-// (`inflight` says which lanes); the next call picks them up.  With `finish` true it runs until nothing is left.
-template <bool TOT, typename Sink>
-__device__ __noinline__ void drain_inversion(QuadQueues<TOT> &Q, InvState<TOT> &st, int &count, uint32_t &inflight,
-                                                bool finish, const double *__restrict__ inv_k, const Sink &sink,
-                                                int *__restrict__ totals, int lane)
+// one group of up to 32 bins from the top of fp32 queue QI; bins the guard does not accept move to the exact queue
+template <int QI, bool TOT, typename Sink>
+__device__ __forceinline__ void drain_fast_group(QuadQueues<TOT> &Q, QuadCounts &qc, const Sink &sink, int *__restrict__ totals,
+                                                 int lane)
 {
-    const uint32_t bit = 1u << lane;
-    bool active = (inflight & bit) != 0;
-    double f = 0.0, c = 0.0, u = 0.0, r = 0.0, rN1 = 0.0;
-    float N = 0.f, kd = 0.f;
-    uint32_t fb = 0u, depo = 0u;
-    if (active) {
-        f = st.f[lane], c = st.c[lane], u = st.u[lane], r = st.r[lane], rN1 = st.rN1[lane];
-        N = st.N[lane], kd = st.kd[lane], fb = st.fb[lane];
-        if constexpr (TOT) depo = st.depo[lane];
+    const int fill = (int)((qc.fast >> (8 * QI)) & 0xffu);
+    const int take = min(32, fill);
+    qc.fast -= (uint32_t)take << (8 * QI);
+    const int e = QI * kQueueCap + fill - take + lane;
+    bool rej = false;
+    if (lane < take) {
+        const double p = Q.p[e];
+        const float N = Q.N[e];
+        const uint32_t w = Q.w[e];
+        float kv;
+        bool ok;
+        if constexpr (QI == kQNorm) ok = p <= 0.5 && fast_normal_draw(N, p, __dmul_rn((double)N, p), w, kv);
+        else if constexpr (QI == kQInvA) ok = inv_fast_draw<8>(N, p, w, kv);
+        else if constexpr (QI == kQInvB) ok = inv_fast_draw<16>(N, p, w, kv);
+        else ok = inv_fast_draw<32>(N, p, w, kv);
+        if (ok) commit_draw<TOT>(sink, totals, Q.bin[e], N, kv, TOT ? Q.depo[e] : 0u);
+        rej = !ok;
     }
-    for (;;) {
-        const uint32_t idle = __ballot_sync(0xffffffffu, !active);
-        if (idle) {
-            if (count > 0) {
-                const int take = min(__popc(idle), count);
-                const int rank = __popc(idle & (bit - 1u));
-                if (!active && rank < take) {
-                    const int e = count - 1 - rank;
-                    const double p = Q.p[e];
-                    N = Q.N[e];
-                    fb = Q.bin[e];
-                    if constexpr (TOT) depo = Q.depo[e];
-                    u = word_to_u01(Q.w[e]);
-                    f = pow_one_minus((double)N, p);
-                    c = f;
-                    r = fast_div(p, 1.0 - p);
-                    rN1 = r * ((double)N + 1.0);
-                    kd = 0.f;
-                    active = true;
-                }
-                count -= take;
-            } else if (!finish || idle == 0xffffffffu) {
-                break;
-            }
+    const unsigned int mr = __ballot_sync(0xffffffffu, rej);
+    if (mr) { // the exact queue holds < 32 entries here
+        if (rej) {
+            const int x = kQExact * kQueueCap + qc.exact + __popc(mr & ((1u << lane) - 1u));
+            Q.p[x] = Q.p[e], Q.w[x] = Q.w[e], Q.bin[x] = Q.bin[e];
+            Q.N[x] = QI == kQNorm ? Q.N[e] : -Q.N[e]; // -N: inversion class
+            if constexpr (TOT) Q.depo[x] = Q.depo[e];
         }
-        // f_k = f_{k-1} r (N - k + 1) / k, written as f_{k-1} (r (N+1) / k - r)
-#pragma unroll
-        for (int s = 0; s < 4; ++s) {
-            if (active && u > c && kd < N) {
-                kd += 1.0f;
-                const double rk = kd < (float)kQuadInvTab ? inv_k[(int)kd] : fast_rcp((double)kd);
-                f *= fma(rN1, rk, -r);
-                c += f;
-            }
-        }
-        if (active && !(u > c && kd < N)) {
-            commit_draw<TOT>(sink, totals, fb, N, kd, depo);
-            active = false;
-        }
+        qc.exact += __popc(mr);
+        __syncwarp();
+        if (qc.exact >= 32) qc.exact = drain_exact<TOT>(&Q, qc.exact, false, sink, totals, lane);
     }
-    inflight = __ballot_sync(0xffffffffu, active);
-    if (active) {
-        st.f[lane] = f, st.c[lane] = c, st.u[lane] = u, st.r[lane] = r, st.rN1[lane] = rN1;
-        st.N[lane] = N, st.kd[lane] = kd, st.fb[lane] = fb;
-        if constexpr (TOT) st.depo[lane] = depo;
-    }
+}
+
+// The queues.  Called (from one place) when one of them holds a warp's worth of work: every queue with 32 or more entries
+// is worked off in groups of 32; with `finish`, everything.
+template <bool TOT, typename Sink>
+__device__ __forceinline__ void drain_queues(QuadWarp<TOT> &ws, QuadCounts &qc, bool finish, const Sink &sink,
+                                             int *__restrict__ totals, int lane)
+{
+    QuadQueues<TOT> &Q = ws.q;
     __syncwarp();
-}
-
-// everything still queued or in flight (end of a kernel's work)
-template <bool TOT, typename Sink>
-__device__ __forceinline__ void drain_all(QuadWarp<TOT> &ws, QuadCounts &qc, const double *__restrict__ inv_k,
-                                          const Sink &sink, int *__restrict__ totals, int lane)
-{
-    drain_inversion<TOT>(ws.q, ws.st, qc.inv, qc.inflight, true, inv_k, sink, totals, lane);
-    drain_exact<TOT>(ws.q, qc.exact, true, sink, totals, lane);
+    // the exact queue first if it is what is full: the groups below may each add up to 32 rejected bins to it
+    if (qc.exact >= 32) qc.exact = drain_exact<TOT>(&Q, qc.exact, false, sink, totals, lane);
+    const uint32_t thresh = finish ? 0xffffffffu : 0xe0e0e0e0u; // a queue is due when its fill is >= 32 (finish: > 0)
+    while (qc.fast & (0xffu << (8 * kQNorm)) & thresh) drain_fast_group<kQNorm, TOT>(Q, qc, sink, totals, lane);
+    while (qc.fast & (0xffu << (8 * kQInvA)) & thresh) drain_fast_group<kQInvA, TOT>(Q, qc, sink, totals, lane);
+    while (qc.fast & (0xffu << (8 * kQInvB)) & thresh) drain_fast_group<kQInvB, TOT>(Q, qc, sink, totals, lane);
+    while (qc.fast & (0xffu << (8 * kQInvC)) & thresh) drain_fast_group<kQInvC, TOT>(Q, qc, sink, totals, lane);
+    if (qc.exact >= 32 || (finish && qc.exact > 0)) qc.exact = drain_exact<TOT>(&Q, qc.exact, finish, sink, totals, lane);
+    __syncwarp();
 }
 
 // One batch of up to kBatchDepos depos, one per lane (lanes >= kBatchDepos own none), fluctuation on.  The call-wide index
 // of the depo of lane l is dbase + l, or dbase + dl (of lane l) when the batch comes from an index list (INDIRECT).
-template <bool TOT, bool INDIRECT, typename Sink>
+// `flush`: the caller has no more batches (the lanes then carry no depo): every queue is emptied before the call returns.
+// NORMAL_ONLY: the normal-approximation sampler of reading A21 (no inversion branch, no mirror).
+template <bool NORMAL_ONLY, bool TOT, bool INDIRECT, typename Sink>
 __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Sink &sink, float t0, float x0, float st,
                                                  float sx, float q, bool valid, long long dbase, uint32_t dl,
-                                                 uint64_t id_base, uint64_t seed, double nsigma, bool normal_only,
-                                                 bool normalize, int *__restrict__ totals, QuadWarp<TOT> &ws,
-                                                 QuadCounts &qc, const double *__restrict__ inv_k,
-                                                 unsigned long long &drawn, int lane)
+                                                 uint64_t id_base, uint64_t seed, double nsigma, bool normalize,
+                                                 int *__restrict__ totals, QuadWarp<TOT> &ws, QuadCounts &qc, bool flush,
+                                                 unsigned int &drawn, int lane)
 {
+    constexpr bool normal_only = NORMAL_ONLY;
     QuadScratch &sc = ws.sc;
     QuadQueues<TOT> &Q = ws.q;
     const double T0 = t0, X0 = x0, ST = st, SX = sx;
@@ -561,7 +539,6 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
     const int nq = aligned ? ((((et.lo & 3) + nt - 1) >> 2) + 1) : (((nt + 2) >> 2) + 1);
     const int ne = flat ? nt + nx + 2 : 0, nqs = flat ? nx * nq : 0;
     const int eincl = warp_incl_scan(ne, lane), qincl = warp_incl_scan(nqs, lane);
-    const float Ntr = (float)floor(fabs((double)q) + 0.5);
     const uint32_t didx = INDIRECT ? dl : (uint32_t)lane;
     __syncwarp();
     sc.eoff[lane] = eincl - ne;
@@ -575,7 +552,7 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
         rc.lo_t = et.lo, rc.lo_x = ex.lo;
         rc.shape = (uint32_t)nt | ((uint32_t)nx << 8) | ((uint32_t)nq << 16) | (q < 0.0f ? 0x80000000u : 0u);
         rc.ebase = 0;
-        rc.t0 = t0, rc.x0 = x0, rc.N = Ntr, rc.idx = didx;
+        rc.t0 = t0, rc.x0 = x0, rc.N = (float)floor(fabs((double)q) + 0.5), rc.idx = didx;
         rc.inv_t = ST < 1e-6 ? 0.0 : fast_rcp(1.4142135623730951 * ST);
         rc.inv_x = SX < 1e-6 ? 0.0 : fast_rcp(1.4142135623730951 * SX);
         sc.rec[lane] = rc;
@@ -584,7 +561,7 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
             sc.inv_norm[lane] = flat ? __ddiv_rn(1.0, axis_norm(T0, ST, nsigma) * axis_norm(X0, SX, nsigma)) : 1.0;
     }
     __syncwarp();
-    if (flat) drawn += (unsigned long long)(nt * nx);
+    if (flat) drawn += (unsigned int)(nt * nx);
 
     // patches too big for the scratch: the whole warp walks them one at a time (fp64 sampler per bin)
     unsigned int big_mask = __ballot_sync(0xffffffffu, live && big);
@@ -612,8 +589,8 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
     int d0 = 0;
     while (d0 < 32) {
         const int ebase = sc.eoff[d0];
-        const unsigned int fits =
-            __ballot_sync(0xffffffffu, lane >= d0 && eincl - ebase + 2 * kEdgePad * (min(lane, kBatchDepos - 1) - d0 + 1) <= kQuadEdgeCap);
+        const unsigned int fits = __ballot_sync(
+            0xffffffffu, lane >= d0 && eincl - ebase + 2 * kEdgePad * (min(lane, kBatchDepos - 1) - d0 + 1) <= kQuadEdgeCap);
         const int d1 = d0 + __popc(fits); // monotone: the fitting lanes are d0 .. d1-1, at least one
         const int etot = sc.eoff[d1] - ebase, qbase = sc.qoff[d0], qtot = sc.qoff[d1] - qbase;
         if (lane >= d0 && lane < d1 && lane < kBatchDepos) sc.rec[lane].ebase = eincl - ne - ebase + 2 * kEdgePad * (lane - d0);
@@ -641,8 +618,9 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
             if (act) sc.edge[a.w + kEdgePad + le + (on_t ? 0 : kEdgePad)] = E;
         }
         __syncwarp();
-        // ---- quads ----------------------------------------------------------------------------------------------------
-        for (int s0 = 0; s0 < qtot; s0 += 32) {
+        // ---- quads (one more, empty pass when flushing, so that the queues are drained from this one place) -----------
+        const bool flush_here = flush && d1 >= 32;
+        for (int s0 = 0; s0 < qtot || (flush_here && s0 == 0); s0 += 32) {
             const int s = s0 + lane;
             const bool act = s < qtot;
             const int own = owner_of(sc.qoff, qbase + (act ? s : 0));
@@ -651,9 +629,7 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
             const int4 a = *reinterpret_cast<const int4 *>(&rc.lo_t);
             const float4 bq = *reinterpret_cast<const float4 *>(&rc.t0);
             const float Nf = bq.z;
-            const uint32_t didx_o = __float_as_uint(bq.w);
             const int nto = a.z & 255, nqo = (a.z >> 16) & 255;
-            const bool neg = a.z < 0;
             // wire row of the quad, l / nq: (l + 1/2) / nq is at least 1/(2 nq) away from an integer, far more than the
             // rounding of the product for l < 2^16
             const int j = __float2int_rz(((float)l + 0.5f) * __frcp_rn((float)max(nqo, 1)));
@@ -662,64 +638,65 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
             const uint32_t g0 = (uint32_t)wire * (uint32_t)g.n_ticks + (uint32_t)a.x; // absolute bin of the row's first tick
             const uint32_t gq = (g0 >> 2) + (uint32_t)qi;
             const int ii0 = (int)(4u * gq - g0); // patch tick index of the quad's first bin: -3 .. nt-1
-            const double *E = sc.edge + a.w + kEdgePad;
-            const double wxq = 0.25 * (E[nto + 1 + kEdgePad + j + 1] - E[nto + 1 + kEdgePad + j]); // wx / 2
+            const double *E = sc.edge + a.w + kEdgePad + ii0;
+            const double *Ex = sc.edge + a.w + 2 * kEdgePad + nto + 1 + j;
+            const double wxq = 0.25 * (Ex[1] - Ex[0]); // wx / 2: p = (wx / 2) (E_t[i+1] - E_t[i])
             const double inv_n = normalize ? sc.inv_norm[own] : 1.0;
-            const long long dio = dbase + (long long)didx_o;
-            const uint4 words = fluct_words(seed, id_base + (uint64_t)dio, (uint64_t)gq);
-            const uint32_t idx0 = sink.index(wire, a.x);
-            const double Nd = (double)Nf;
-
-            // the four bins of the quad, one after the other (a loop, not unrolled: the code of the kernel has to stay
-            // inside the instruction cache)
+            const uint32_t dio = (uint32_t)dbase + __float_as_uint(bq.w); // index of the depo in the call (< 2^32: totals)
+            const uint4 words = fluct_words(seed, id_base + (uint64_t)(dbase + (long long)__float_as_uint(bq.w)), (uint64_t)gq);
+            const uint32_t idx0 = sink.index(wire, a.x) + (uint32_t)ii0; // sink index of the quad's first bin (mod 2^32)
+            const uint32_t neg = a.z < 0 ? kBinNegative : 0u;
+            const bool live_q = act && Nf > 0.0f; // N = 0 draws nothing
+            uint32_t w0 = words.x, w1 = words.y, w2 = words.z, w3 = words.w;
 #pragma unroll 1
             for (int k = 0; k < 4; ++k) {
-                uint32_t w = k == 0 ? words.x : k == 1 ? words.y : k == 2 ? words.z : words.w;
-                const double ea = E[ii0 + k], eb = E[ii0 + k + 1];
-                const int ii = ii0 + k;
-                const bool v = act && (unsigned)ii < (unsigned)nto;
-                double p = __dmul_rn(__dsub_rn(eb, ea), wxq); // = wt wx: the two factors 1/2 are exact scalings
+                uint32_t w = w0; // the word of this bin; the others move up
+                w0 = w1, w1 = w2, w2 = w3;
+                const bool v = live_q && (unsigned)(ii0 + k) < (unsigned)nto;
+                double p = __dmul_rn(__dsub_rn(E[k + 1], E[k]), wxq); // = wt wx: the two factors 1/2 are exact scalings
                 if (normalize) p *= inv_n;
-                const bool nontrivial = v && p > 0.0 && p < 1.0 && Nf > 0.0f;
-                float kv = (p >= 1.0) ? Nf : 0.0f; // p <= 0 or N = 0: k = 0; p >= 1: k = N
-                bool mirror = false;
-                if (!normal_only && p > 0.5 && p < 1.0) {
-                    mirror = true;
+                const bool all = p >= 1.0; // every electron lands here
+                const bool mirror = !normal_only && p > 0.5 && !all;
+                if (mirror) {
                     p = __dsub_rn(1.0, p);
                     w = ~w;
                 }
-                const double mu = __dmul_rn(Nd, p);
-                const bool small = !normal_only && mu < 16.0;
-                bool decided = !nontrivial;
-                if (nontrivial) {
-                    if (small) {
-                        // u <= 1 - mu implies u <= (1-p)^N = F(0), i.e. k = 0 (Bernoulli); in fp32 with a margin that
-                        // covers the roundings of u, mu and their sum (3 x 2^-24)
-                        const float uf = fmaf((float)w, 2.3283064365386963e-10f, 1.1641532182693481e-10f);
-                        decided = uf + (float)mu <= 0.9999996f;
-                    } else if (p <= 0.5) {
-                        decided = fast_normal_draw(Nf, p, mu, w, kv);
-                    }
+                const float muf = (float)__dmul_rn((double)Nf, p); // class boundaries below: see the note on `cls`
+                const bool small = !normal_only && __dmul_rn((double)Nf, p) < 16.0;
+                // u <= 1 - mu implies u <= (1-p)^N = F(0), i.e. k = 0 (Bernoulli); in fp32 with a margin that covers the
+                // roundings of u, mu and their sum (3 x 2^-24)
+                const bool quick = small && fmaf((float)w, 2.3283064365386963e-10f, 1.1641532182693481e-10f) + muf <= 0.9999996f;
+                const bool draw = v && p > 0.0 && !all && !quick;
+                // k = N without a draw: p >= 1, or k = 0 of the mirrored draw
+                if (v && (all || (quick && mirror))) {
+                    sink.add_at(idx0 + k, neg ? -Nf : Nf);
+                    if constexpr (TOT) atomicAdd(totals + dio, (int)(neg ? -Nf : Nf));
                 }
-                const uint32_t fb = (idx0 + (uint32_t)ii) | (mirror ? kBinMirror : 0u) | (neg ? kBinNegative : 0u);
-                if (v && decided) commit_draw<TOT>(sink, totals, fb, Nf, kv, (uint32_t)dio);
-                const bool to_inv = nontrivial && !decided && small, to_exact = nontrivial && !decided && !small;
-                const unsigned int mi = __ballot_sync(0xffffffffu, to_inv), me = __ballot_sync(0xffffffffu, to_exact);
-                if (to_inv || to_exact) {
-                    const int pos = to_inv ? qc.inv + __popc(mi & ((1u << lane) - 1u))
-                                           : kInvCap + qc.exact + __popc(me & ((1u << lane) - 1u));
+                // The queue.  mu < 16 against mu >= 16 is the sampler's own branch and is decided in fp64 (`small`); the
+                // bands of the inversion only choose how many terms the fp32 routine sums, so fp32 mu is good enough
+                // (a bin next to a band edge that needs more terms than its band has fails the guard and is redone).
+                int cls = !small ? kQNorm : !inv_fast_eligible(Nf, p) ? kQExact : muf < 2.0f ? kQInvA : muf < 6.0f ? kQInvB : kQInvC;
+                if (!draw) cls = -1;
+                const unsigned int peers = __match_any_sync(0xffffffffu, cls); // the lanes that push to the same queue
+                const int rank = __popc(peers & ((1u << lane) - 1u));
+                // new fills: the first lane of every group adds its group's size to the queue's byte
+                const bool lead = rank == 0 && cls >= 0 && cls < kQExact;
+                const uint32_t add = __reduce_add_sync(0xffffffffu, lead ? (uint32_t)__popc(peers) << (8 * cls) : 0u);
+                const int add_x = __popc(__ballot_sync(0xffffffffu, cls == kQExact));
+                if (cls >= 0) {
+                    const int fill = cls == kQExact ? qc.exact : (int)((qc.fast >> (8 * cls)) & 0xffu);
+                    const int pos = cls * kQueueCap + fill + rank;
                     Q.p[pos] = p;
-                    Q.N[pos] = Nf;
+                    Q.N[pos] = (cls == kQExact && small) ? -Nf : Nf;
                     Q.w[pos] = w;
-                    Q.bin[pos] = fb;
-                    if constexpr (TOT) Q.depo[pos] = (uint32_t)dio;
+                    Q.bin[pos] = (idx0 + k) | neg | (mirror ? kBinMirror : 0u);
+                    if constexpr (TOT) Q.depo[pos] = dio;
                 }
-                qc.inv += __popc(mi);
-                qc.exact += __popc(me);
-                __syncwarp();
-                if (qc.inv >= kInvDrainAt)
-                    drain_inversion<TOT>(Q, ws.st, qc.inv, qc.inflight, false, inv_k, sink, totals, lane);
-                if (qc.exact >= 32) drain_exact<TOT>(Q, qc.exact, false, sink, totals, lane);
+                qc.fast += add;
+                qc.exact += add_x;
+                const bool last = flush_here && k == 3 && s0 + 32 >= qtot;
+                if ((qc.fast & 0xe0e0e0e0u) | (uint32_t)(qc.exact >> 5) | (uint32_t)last)
+                    drain_queues<TOT>(ws, qc, last, sink, totals, lane);
             }
         }
         __syncwarp();
@@ -734,28 +711,22 @@ struct BatchSmem {
 };
 template <bool TOT>
 struct BatchSmem<true, TOT> {
-    double inv_k[kQuadInvTab]; // 1/k of the inversion recurrence
     QuadWarp<TOT> warp[kBatchWarps];
 };
-
-__device__ __forceinline__ void fill_inv_k(double *inv_k)
-{
-    for (int k = threadIdx.x; k < kQuadInvTab; k += blockDim.x) inv_k[k] = k ? 1.0 / (double)k : 0.0;
-    __syncthreads();
-}
 
 // ------------------------------------------------------------------------------------------------------------------
 // atomic mode: persistent warps; a warp's first batch is its own index in the grid, further ones come from a device
 // counter (guided: kBatchDepos depos at a time, kTailDepos at a time near the end)
 // ------------------------------------------------------------------------------------------------------------------
-template <bool FLUCT, bool TOT, bool FIX>
+// FLUCT: 0 off, 1 binomial (reading A6), 2 normal approximation (reading A21)
+template <int FLUCT, bool TOT, bool FIX>
 __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
                                                                         uint64_t id_base, uint64_t seed, double nsigma,
                                                                         float *__restrict__ S, int *__restrict__ totals,
-                                                                        Counters *counters, bool normal_only, bool normalize)
+                                                                        Counters *counters, bool normalize)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    BatchSmem<FLUCT, TOT> &sm = *reinterpret_cast<BatchSmem<FLUCT, TOT> *>(smem_raw);
+    BatchSmem<FLUCT != 0, TOT> &sm = *reinterpret_cast<BatchSmem<FLUCT != 0, TOT> *>(smem_raw);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     // FIX: S points at the 64-bit fixed-point grid (deterministic mode without tiles)
     using Sink = typename std::conditional<FIX, FixSink, GlobalSink>::type;
@@ -769,9 +740,8 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
     const long long big_batches = (n - tail_depos) >> kBatchShift;
     const long long big_depos = big_batches << kBatchShift;
     const long long n_batches = big_batches + (n - big_depos + kTailDepos - 1) / kTailDepos;
-    unsigned long long drawn = 0, skipped = 0;
+    unsigned int drawn = 0, skipped = 0; // per lane
     QuadCounts qc;
-    if constexpr (FLUCT) fill_inv_k(sm.inv_k);
     // the grid is one wave, so the next kernel's CTAs may take the slots this one frees as it drains.  As a
     // programmatic dependent itself it only overlaps a preceding KERNEL's tail: copies and memsets ahead of it in the
     // stream are still fully ordered (checked with 300 host-buffer plane-events of changing depos, 0 mismatches)
@@ -785,31 +755,32 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
     // (Fetching the NEXT batch's index early to hide the round trip was tried: a warp then sits on a batch while it
     // works on another, and the load balance suffers more than the latency costs.)
     long long batch = (long long)blockIdx.x * kBatchWarps + wid;
-    while (batch < n_batches) {
+    for (;;) {
+        const bool more = batch < n_batches;
         const long long first = batch < big_batches ? batch << kBatchShift : big_depos + (batch - big_batches) * kTailDepos;
         const int count = batch < big_batches ? kBatchDepos : kTailDepos;
         const long long i = first + lane;
         float t0 = 0.f, x0 = 0.f, st = 0.f, sx = 0.f, q = 0.f;
         bool valid = false;
-        if (lane < count && i < n) {
+        if (more && lane < count && i < n) {
             t0 = d.t0[i], x0 = d.x0[i], st = d.sigma_t[i], sx = d.sigma_x[i], q = d.q[i]; // plain loads: pdl.cuh
             valid = depo_valid(t0, x0, st, sx, q);
             skipped += !valid;
         }
+        // fluctuated: one more call without depos after the last batch empties the warp's draw queues
         if constexpr (FLUCT)
-            raster_quad_body<TOT, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, id_base, seed, nsigma,
-                                         normal_only, normalize, totals, sm.warp[wid], qc, sm.inv_k, drawn, lane);
-        else
+            raster_quad_body<FLUCT == 2, TOT, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, id_base, seed, nsigma,
+                                                     normalize, totals, sm.warp[wid], qc, !more, drawn, lane);
+        else if (more)
             raster_flat_body(g, clip, sink, t0, x0, st, sx, q, valid, nsigma, normalize, sm.scratch[wid], drawn, lane);
+        if (!more) break;
         if (lane == 0) batch = n_warps_grid + (long long)atomicAdd(&counters->next_batch, 1ull);
         batch = __shfl_sync(0xffffffffu, batch, 0);
     }
-    if constexpr (FLUCT) drain_all<TOT>(sm.warp[wid], qc, sm.inv_k, sink, totals, lane);
-    drawn = warp_sum(drawn);
-    skipped = warp_sum(skipped);
+    const unsigned long long drawn_w = warp_sum((unsigned long long)drawn), skipped_w = warp_sum((unsigned long long)skipped);
     if (lane == 0) {
-        if (drawn) atomicAdd(&counters->bins_drawn, drawn);
-        if (skipped) atomicAdd(&counters->depos_skipped, skipped);
+        if (drawn_w) atomicAdd(&counters->bins_drawn, drawn_w);
+        if (skipped_w) atomicAdd(&counters->depos_skipped, skipped_w);
         // the last warp to leave re-arms the batch counter for the next launch on this stream (every warp has made its
         // last fetch before it adds itself here)
         const unsigned long long n_warps = (unsigned long long)gridDim.x * kBatchWarps;
@@ -924,18 +895,17 @@ struct TileSmem {
 template <bool TOT>
 struct TileSmem<true, TOT> {
     unsigned long long acc[kTileW * kTileT];
-    double inv_k[kQuadInvTab];
     QuadWarp<TOT> warp[kTileWarps];
 };
 
-template <bool FLUCT, bool TOT>
+template <int FLUCT, bool TOT>
 __global__ void __launch_bounds__(kTileWarps * 32, 2) tile_accumulate_kernel(GridDims g, DepoArrays d, uint64_t id_base,
                                                                           uint64_t seed, double nsigma, TileScratch ts,
                                                                           float *__restrict__ S, int *__restrict__ totals,
-                                                                          Counters *counters, bool normal_only, bool normalize)
+                                                                          Counters *counters, bool normalize)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    TileSmem<FLUCT, TOT> &sm = *reinterpret_cast<TileSmem<FLUCT, TOT> *>(smem_raw);
+    TileSmem<FLUCT != 0, TOT> &sm = *reinterpret_cast<TileSmem<FLUCT != 0, TOT> *>(smem_raw);
     const int tile = blockIdx.x / kTileSlices, slice = blockIdx.x % kTileSlices;
     const unsigned int tile_beg = ts.tile_count[tile], tile_end = ts.tile_count[tile + 1];
     const unsigned int listed = tile_end - tile_beg;
@@ -951,31 +921,31 @@ __global__ void __launch_bounds__(kTileWarps * 32, 2) tile_accumulate_kernel(Gri
     const int w0 = tw * kTileW, k0 = tt * kTileT;
     const int w1 = min(w0 + kTileW, g.n_wires), k1 = min(k0 + kTileT, g.n_ticks);
     for (int i = threadIdx.x; i < kTileW * kTileT; i += blockDim.x) sm.acc[i] = 0ull;
-    if constexpr (FLUCT) fill_inv_k(sm.inv_k);
     __syncthreads();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const TileSink sink{sm.acc, w0, k0};
     const Clip clip{w0, w1, k0, k1};
-    unsigned long long drawn = 0;
+    unsigned int drawn = 0; // per lane
     QuadCounts qc;
-    for (unsigned int e0 = beg + (unsigned int)wid * kBatchDepos; e0 < end; e0 += kTileWarps * kBatchDepos) {
+    for (unsigned int e0 = beg + (unsigned int)wid * kBatchDepos;; e0 += kTileWarps * kBatchDepos) {
+        const bool more = e0 < end;
         float t0 = 0.f, x0 = 0.f, st = 0.f, sx = 0.f, q = 0.f;
         unsigned int i = 0;
         bool valid = false;
-        if (lane < kBatchDepos && e0 + lane < end) {
+        if (more && lane < kBatchDepos && e0 + lane < end) {
             i = ts.entries[e0 + lane];
             t0 = __ldg(d.t0 + i), x0 = __ldg(d.x0 + i), st = __ldg(d.sigma_t + i), sx = __ldg(d.sigma_x + i), q = __ldg(d.q + i);
             valid = depo_valid(t0, x0, st, sx, q); // listed depos are valid; kept for symmetry with the atomic kernel
         }
         if constexpr (FLUCT)
-            raster_quad_body<TOT, true>(g, clip, sink, t0, x0, st, sx, q, valid, 0ll, i, id_base, seed, nsigma, normal_only,
-                                        normalize, totals, sm.warp[wid], qc, sm.inv_k, drawn, lane);
-        else
+            raster_quad_body<FLUCT == 2, TOT, true>(g, clip, sink, t0, x0, st, sx, q, valid, 0ll, i, id_base, seed, nsigma,
+                                                    normalize, totals, sm.warp[wid], qc, !more, drawn, lane);
+        else if (more)
             raster_flat_body(g, clip, sink, t0, x0, st, sx, q, valid, nsigma, normalize, sm.scratch[wid], drawn, lane);
+        if (!more) break;
     }
-    if constexpr (FLUCT) drain_all<TOT>(sm.warp[wid], qc, sm.inv_k, sink, totals, lane);
-    drawn = warp_sum(drawn);
-    if (lane == 0 && drawn) atomicAdd(&counters->bins_drawn, drawn);
+    const unsigned long long drawn_w = warp_sum((unsigned long long)drawn);
+    if (lane == 0 && drawn_w) atomicAdd(&counters->bins_drawn, drawn_w);
     __syncthreads();
     for (int i = threadIdx.x; i < kTileW * kTileT; i += blockDim.x) {
         const int w = w0 + i / kTileT, k = k0 + i % kTileT;
@@ -1029,40 +999,47 @@ cudaError_t raster_configure(cudaStream_t st)
     if (err != cudaSuccess) return err;
 #define WCSIM_RASTER_SMEM(F, T, X)                                                                                     \
     err = cudaFuncSetAttribute(raster_batch_kernel<F, T, X>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
-                               (int)sizeof(BatchSmem<F, T>));                                                          \
+                               (int)sizeof(BatchSmem<F != 0, T>));                                                     \
     if (err != cudaSuccess) return err;
-    WCSIM_RASTER_SMEM(true, true, false)
-    WCSIM_RASTER_SMEM(true, false, false)
-    WCSIM_RASTER_SMEM(false, false, false)
-    WCSIM_RASTER_SMEM(true, true, true)
-    WCSIM_RASTER_SMEM(true, false, true)
-    WCSIM_RASTER_SMEM(false, false, true)
+    WCSIM_RASTER_SMEM(1, true, false)
+    WCSIM_RASTER_SMEM(1, false, false)
+    WCSIM_RASTER_SMEM(2, true, false)
+    WCSIM_RASTER_SMEM(2, false, false)
+    WCSIM_RASTER_SMEM(0, false, false)
+    WCSIM_RASTER_SMEM(1, true, true)
+    WCSIM_RASTER_SMEM(1, false, true)
+    WCSIM_RASTER_SMEM(2, true, true)
+    WCSIM_RASTER_SMEM(2, false, true)
+    WCSIM_RASTER_SMEM(0, false, true)
 #undef WCSIM_RASTER_SMEM
-    err = cudaFuncSetAttribute(tile_accumulate_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               (int)sizeof(TileSmem<true, true>));
+#define WCSIM_TILE_SMEM(F, T)                                                                                          \
+    err = cudaFuncSetAttribute(tile_accumulate_kernel<F, T>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
+                               (int)sizeof(TileSmem<F != 0, T>));                                                      \
     if (err != cudaSuccess) return err;
-    err = cudaFuncSetAttribute(tile_accumulate_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               (int)sizeof(TileSmem<true, false>));
-    if (err != cudaSuccess) return err;
-    return cudaFuncSetAttribute(tile_accumulate_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)sizeof(TileSmem<false, false>));
+    WCSIM_TILE_SMEM(1, true)
+    WCSIM_TILE_SMEM(1, false)
+    WCSIM_TILE_SMEM(2, true)
+    WCSIM_TILE_SMEM(2, false)
+    WCSIM_TILE_SMEM(0, false)
+#undef WCSIM_TILE_SMEM
+    return cudaSuccess;
 }
 
-template <bool FLUCT, bool TOT, bool FIX>
+template <int FLUCT, bool TOT, bool FIX>
 static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, double nsigma,
                                        float *S, int *depo_totals, Counters *counters, int sm_count, cudaStream_t st,
-                                       bool normal_only, bool normalize)
+                                       bool normalize)
 {
     const long long n_batches = (n + kBatchDepos - 1) / kBatchDepos;
-    const size_t smem = sizeof(BatchSmem<FLUCT, TOT>);
+    const size_t smem = sizeof(BatchSmem<FLUCT != 0, TOT>);
     const int fit = (int)((227u * 1024u) / (smem + 1024u)); // 227 KB per SM, 1 KB reserved per CTA
-    const int cap = FLUCT ? 6 : 8; // the kernel's __launch_bounds__ (7 CTAs of 72 registers: configs[1] -2 %, [2] +1.5 %)
+    const int cap = FLUCT ? 6 : 8; // the kernel's __launch_bounds__
     const int ctas_per_sm = fit > cap ? cap : fit;
     long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
     const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
     if (ctas > max_ctas) ctas = max_ctas;
     return launch_pdl(raster_batch_kernel<FLUCT, TOT, FIX>, (unsigned)ctas, kBatchWarps * 32, smem, st, g, d, n, id_base, seed,
-                      nsigma, S, depo_totals, counters, normal_only, normalize);
+                      nsigma, S, depo_totals, counters, normalize);
 }
 
 template <bool FIX>
@@ -1073,14 +1050,11 @@ static cudaError_t launch_raster_grid(GridDims g, DepoArrays d, long long n, uin
     if (n <= 0) return cudaSuccess;
     const bool normalize = (fluctuate & kRasterNormalize) != 0;
     fluctuate &= ~kRasterNormalize;
-    if (!fluctuate) // no draws, no per-depo integer totals
-        return launch_raster_batch<false, false, FIX>(g, d, n, id_base, seed, nsigma, grid, nullptr, counters, sm_count, st,
-                                                      false, normalize);
-    if (depo_totals)
-        return launch_raster_batch<true, true, FIX>(g, d, n, id_base, seed, nsigma, grid, depo_totals, counters, sm_count,
-                                                    st, fluctuate == 2, normalize);
-    return launch_raster_batch<true, false, FIX>(g, d, n, id_base, seed, nsigma, grid, nullptr, counters, sm_count, st,
-                                                 fluctuate == 2, normalize);
+#define WCSIM_BATCH(F, T) launch_raster_batch<F, T, FIX>(g, d, n, id_base, seed, nsigma, grid, T ? depo_totals : nullptr, counters, sm_count, st, normalize)
+    if (!fluctuate) return WCSIM_BATCH(0, false); // no draws, no per-depo integer totals
+    if (fluctuate == 2) return depo_totals ? WCSIM_BATCH(2, true) : WCSIM_BATCH(2, false);
+    return depo_totals ? WCSIM_BATCH(1, true) : WCSIM_BATCH(1, false);
+#undef WCSIM_BATCH
 }
 
 cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
@@ -1118,14 +1092,14 @@ cudaError_t launch_tile_fill(GridDims g, DepoArrays d, long long n, double nsigm
     return cudaGetLastError();
 }
 
-template <bool FLUCT, bool TOT>
+template <int FLUCT, bool TOT>
 static cudaError_t launch_tile_accumulate_t(GridDims g, DepoArrays d, uint64_t id_base, uint64_t seed, double nsigma,
-                                            TileScratch ts, float *S, int *depo_totals, Counters *counters, bool normal_only, bool normalize,
+                                            TileScratch ts, float *S, int *depo_totals, Counters *counters, bool normalize,
                                             cudaStream_t st)
 {
     const int n_tiles = ts.tiles_w * ts.tiles_t;
-    tile_accumulate_kernel<FLUCT, TOT><<<n_tiles * kTileSlices, kTileWarps * 32, sizeof(TileSmem<FLUCT, TOT>), st>>>(
-        g, d, id_base, seed, nsigma, ts, S, depo_totals, counters, normal_only, normalize);
+    tile_accumulate_kernel<FLUCT, TOT><<<n_tiles * kTileSlices, kTileWarps * 32, sizeof(TileSmem<FLUCT != 0, TOT>), st>>>(
+        g, d, id_base, seed, nsigma, ts, S, depo_totals, counters, normalize);
     return cudaGetLastError();
 }
 
@@ -1135,14 +1109,11 @@ cudaError_t launch_tile_accumulate(GridDims g, DepoArrays d, uint64_t id_base, u
 {
     const bool normalize = (fluctuate & kRasterNormalize) != 0;
     fluctuate &= ~kRasterNormalize;
-    if (!fluctuate)
-        return launch_tile_accumulate_t<false, false>(g, d, id_base, seed, nsigma, ts, S, nullptr, counters, false, normalize,
-                                                      st);
-    if (depo_totals)
-        return launch_tile_accumulate_t<true, true>(g, d, id_base, seed, nsigma, ts, S, depo_totals, counters,
-                                                    fluctuate == 2, normalize, st);
-    return launch_tile_accumulate_t<true, false>(g, d, id_base, seed, nsigma, ts, S, nullptr, counters, fluctuate == 2,
-                                                 normalize, st);
+#define WCSIM_TILE(F, T) launch_tile_accumulate_t<F, T>(g, d, id_base, seed, nsigma, ts, S, T ? depo_totals : nullptr, counters, normalize, st)
+    if (!fluctuate) return WCSIM_TILE(0, false);
+    if (fluctuate == 2) return depo_totals ? WCSIM_TILE(2, true) : WCSIM_TILE(2, false);
+    return depo_totals ? WCSIM_TILE(1, true) : WCSIM_TILE(1, false);
+#undef WCSIM_TILE
 }
 
 cudaError_t launch_tile_finalize(GridDims g, TileScratch ts, float *S, cudaStream_t st)

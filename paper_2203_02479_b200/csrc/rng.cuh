@@ -319,6 +319,58 @@ __device__ __forceinline__ bool fast_normal_draw(float N, double p, double mu, u
     return ok;
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Guarded fp32 inversion (mu < 16).  k is the number of CDF values F(0), F(1), ... below u.  The fp32 routine sums a FIXED
+// number T of terms of the same recurrence (straight-line code, every lane busy; the raster queues bins by mu so that
+// T = 8, 16 or 32 is enough: P(k >= T) < 1.2e-3 at the top of each band) and counts the F(j) below u.  The count is the
+// fp64 routine's whenever u is farther from every F(j), j < T, than a bound on their fp32 error, and u <= F(T-1).
+// Taken for N >= 128 and p < 2^-5 (every bin of BASELINE.json's workloads with mu < 16); bins that fail the guard are drawn
+// again by draw_inversion in fp64.
+// Error budget (u = 2^-24; quantities marked ' are the fp32 ones):
+//   p' = fp32(p): relative u.   s' = p' (1 + p'/2 + ... + p'^5/6) = -log(1 - p): truncation p^6/7 < 2^-32, Horner
+//   roundings 4u, the rounding of p another 1.04u;  L' = N s': relative 6.1u, L < 16.3, so |dL| < 5.9e-6;
+//   f0' = ex2(-L' log2 e): the product adds 1.5e-6, ex2.approx is accurate to 2^-22 relative  =>  f0 relative 7.7e-6.
+//   r' = p' rcp(1 - p'): relative 5u;  a' = r' (N + 1): relative 6u.
+//   term j: f_j = f_{j-1} (a'/j - r'), one fma with the constant fp32(1/j): relative to the true factor r (N+1-j)/j the
+//   error is u + 7u (N+1)/(N+1-j) + 5u j/(N+1-j) <= 14.3u for N >= 128, j < 32; with the product and the running sum
+//   c_j = c_{j-1} + f_j: at most 17u = 1.0e-6 per term.
+//   u' = fma(fp32(w), 2^-32, 2^-33): |u' - u| <= 2u = 1.2e-7.
+//   =>  |c_j' - c_j| <= (7.7e-6 + 1.0e-6 j) c_j, c_j <= 1.  Guard G(T) = 8.2e-6 + 1.3e-6 T (absolute, for every j < T).
+// ------------------------------------------------------------------------------------------------------------------
+constexpr float kInvFastMinN = 128.0f, kInvFastMaxP = 0.03125f;
+constexpr float kInvGuard0 = 8.2e-6f, kInvGuardK = 1.3e-6f;
+
+__device__ __forceinline__ bool inv_fast_eligible(float N, double p) { return N >= kInvFastMinN && p < (double)kInvFastMaxP; }
+
+// true: k is the fp64 inversion's draw for (N, p; w); false: not decided
+template <int T>
+__device__ __forceinline__ bool inv_fast_draw(float N, double p, uint32_t w, float &k)
+{
+    const float pf = (float)p;
+    float g = 1.0f / 6.0f;
+    g = fmaf(g, pf, 0.2f);
+    g = fmaf(g, pf, 0.25f);
+    g = fmaf(g, pf, 1.0f / 3.0f);
+    g = fmaf(g, pf, 0.5f);
+    g = fmaf(g, pf, 1.0f);
+    const float L = N * (pf * g); // -N log(1 - p)
+    float f, rc;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(f) : "f"(L * -1.4426950408889634f));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rc) : "f"(1.0f - pf));
+    const float r = pf * rc, a = r * (N + 1.0f);
+    const float u = fmaf((float)w, 2.3283064365386963e-10f, 1.1641532182693481e-10f);
+    float c = f, dmin = fabsf(u - c);
+    k = u > c ? 1.0f : 0.0f;
+#pragma unroll
+    for (int j = 1; j < T; ++j) {
+        f *= fmaf(a, 1.0f / (float)j, -r);
+        c += f;
+        dmin = fminf(dmin, fabsf(u - c));
+        k += u > c ? 1.0f : 0.0f;
+    }
+    return dmin >= kInvGuard0 + kInvGuardK * (float)T && !(u > c);
+}
+
 // the whole sampler for one bin (debug hook, big-patch and tiled paths)
 __device__ __forceinline__ double binomial_draw(double N, double p, uint32_t w, bool normal_only = false)
 {
