@@ -32,6 +32,8 @@
 #include "pdl.cuh"
 #include "rng.cuh"
 #include <type_traits>
+#include <cstdio>
+#include <cstdlib>
 
 namespace wcsim {
 
@@ -231,9 +233,15 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v)
 // batches: a warp takes kBatchDepos depos at a time, one per lane
 // ------------------------------------------------------------------------------------------------------------------
 constexpr int kBatchWarps = 4;          // warps per CTA
-constexpr int kBatchShift = 3;          // log2 of the depos a warp fetches at a time (lanes beyond that own no depo):
+#ifndef WCSIM_BATCH_SHIFT
+#define WCSIM_BATCH_SHIFT 4
+#endif
+#ifndef WCSIM_FLUCT_CTAS
+#define WCSIM_FLUCT_CTAS 5
+#endif
+constexpr int kBatchShift = WCSIM_BATCH_SHIFT;          // log2 of the depos a warp fetches at a time (lanes beyond that own no depo):
 constexpr int kBatchDepos = 1 << kBatchShift; // small batches keep the per-warp serial path short and the load balanced
-constexpr int kTailDepos = 2, kTailPerWarp = 4; // guided scheduling of the last batches (raster_batch_kernel)
+constexpr int kTailDepos = 4, kTailPerWarp = 2; // guided scheduling of the last batches (raster_batch_kernel)
 constexpr uint32_t kBinMirror = 1u << 30, kBinNegative = 1u << 31, kBinMask = kBinMirror - 1u; // grid < 2^30 bins
 
 // largest d in [0, kBatchDepos) with off[d] <= x (off is an exclusive prefix over the depos of a batch; entries from
@@ -720,10 +728,10 @@ struct BatchSmem<true, TOT> {
 // ------------------------------------------------------------------------------------------------------------------
 // FLUCT: 0 off, 1 binomial (reading A6), 2 normal approximation (reading A21)
 template <int FLUCT, bool TOT, bool FIX>
-__global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
+__global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
                                                                         uint64_t id_base, uint64_t seed, double nsigma,
                                                                         float *__restrict__ S, int *__restrict__ totals,
-                                                                        Counters *counters, bool normalize)
+                                                                        Counters *counters, bool normalize, int3 sched)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     BatchSmem<FLUCT != 0, TOT> &sm = *reinterpret_cast<BatchSmem<FLUCT != 0, TOT> *>(smem_raw);
@@ -736,10 +744,11 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
     // grid, so that the warps run out of work within a short batch of one another (on configs[1] a warp gets only
     // 3-4 batches of 8)
     const long long n_warps_grid = (long long)gridDim.x * kBatchWarps;
-    const long long tail_depos = n_warps_grid * kTailPerWarp < n ? n_warps_grid * kTailPerWarp : n;
+    const int tail_size = sched.x, n_static = sched.z;
+    const long long tail_depos = n_warps_grid * sched.y < n ? n_warps_grid * sched.y : n;
     const long long big_batches = (n - tail_depos) >> kBatchShift;
     const long long big_depos = big_batches << kBatchShift;
-    const long long n_batches = big_batches + (n - big_depos + kTailDepos - 1) / kTailDepos;
+    const long long n_batches = big_batches + (n - big_depos + tail_size - 1) / tail_size;
     unsigned int drawn = 0, skipped = 0; // per lane
     QuadCounts qc;
     // the grid is one wave, so the next kernel's CTAs may take the slots this one frees as it drains.  As a
@@ -755,10 +764,11 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
     // (Fetching the NEXT batch's index early to hide the round trip was tried: a warp then sits on a batch while it
     // works on another, and the load balance suffers more than the latency costs.)
     long long batch = (long long)blockIdx.x * kBatchWarps + wid;
+    int round = 0;
     for (;;) {
         const bool more = batch < n_batches;
-        const long long first = batch < big_batches ? batch << kBatchShift : big_depos + (batch - big_batches) * kTailDepos;
-        const int count = batch < big_batches ? kBatchDepos : kTailDepos;
+        const long long first = batch < big_batches ? batch << kBatchShift : big_depos + (batch - big_batches) * tail_size;
+        const int count = batch < big_batches ? kBatchDepos : tail_size;
         const long long i = first + lane;
         float t0 = 0.f, x0 = 0.f, st = 0.f, sx = 0.f, q = 0.f;
         bool valid = false;
@@ -774,8 +784,12 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? 6 : 8) raster_batch_
         else if (more)
             raster_flat_body(g, clip, sink, t0, x0, st, sx, q, valid, nsigma, normalize, sm.scratch[wid], drawn, lane);
         if (!more) break;
-        if (lane == 0) batch = n_warps_grid + (long long)atomicAdd(&counters->next_batch, 1ull);
-        batch = __shfl_sync(0xffffffffu, batch, 0);
+        if (++round < n_static) {
+            batch += n_warps_grid;
+        } else {
+            if (lane == 0) batch = n_static * n_warps_grid + (long long)atomicAdd(&counters->next_batch, 1ull);
+            batch = __shfl_sync(0xffffffffu, batch, 0);
+        }
     }
     const unsigned long long drawn_w = warp_sum((unsigned long long)drawn), skipped_w = warp_sum((unsigned long long)skipped);
     if (lane == 0) {
@@ -1033,13 +1047,19 @@ static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, ui
     const long long n_batches = (n + kBatchDepos - 1) / kBatchDepos;
     const size_t smem = sizeof(BatchSmem<FLUCT != 0, TOT>);
     const int fit = (int)((227u * 1024u) / (smem + 1024u)); // 227 KB per SM, 1 KB reserved per CTA
-    const int cap = FLUCT ? 6 : 8; // the kernel's __launch_bounds__
+    const int cap = FLUCT ? WCSIM_FLUCT_CTAS : 8; // the kernel's __launch_bounds__
     const int ctas_per_sm = fit > cap ? cap : fit;
     long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
     const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
     if (ctas > max_ctas) ctas = max_ctas;
+    int3 sched = make_int3(kTailDepos, kTailPerWarp, 2);
+    int max_per_sm = 0;
+    if (const char *e = getenv("WCSIM_SCHED")) sscanf(e, "%d,%d,%d,%d", &sched.x, &sched.y, &sched.z, &max_per_sm);
+    if (max_per_sm > 0 && ctas > (long long)sm_count * max_per_sm) ctas = (long long)sm_count * max_per_sm;
+    if (sched.x < 1 || sched.x > kBatchDepos) sched.x = kTailDepos;
+    if (sched.z < 1) sched.z = 1;
     return launch_pdl(raster_batch_kernel<FLUCT, TOT, FIX>, (unsigned)ctas, kBatchWarps * 32, smem, st, g, d, n, id_base, seed,
-                      nsigma, S, depo_totals, counters, normalize);
+                      nsigma, S, depo_totals, counters, normalize, sched);
 }
 
 template <bool FIX>
