@@ -12,6 +12,28 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
 
 
+# Measured parity figures (rel-L2, max-abs, flipped bins ...) of the -m gpu tests: record(name, key=value, ...) from a
+# test; written to gpurun_out/parity_measured.json when the session ends (quoted under profiles/).
+_MEASURED = {}
+
+
+def record(name, **values):
+    _MEASURED.setdefault(name, {}).update({k: (float(v) if isinstance(v, float) else v) for k, v in values.items()})
+
+
+def pytest_sessionfinish(session, exitstatus):
+    if not _MEASURED:
+        return
+    import json
+    out = os.path.join(ROOT, "gpurun_out")
+    try:
+        os.makedirs(out, exist_ok=True)
+        with open(os.path.join(out, "parity_measured.json"), "w") as f:
+            json.dump(_MEASURED, f, indent=1, sort_keys=True, default=lambda o: o.item() if hasattr(o, "item") else str(o))
+    except OSError:
+        pass
+
+
 def golden(name):
     """Rows of a whitespace-separated golden text file under tests/golden/ ('#' starts a comment)."""
     rows = []

@@ -46,6 +46,8 @@ def assert_close(got, ref, what, rel=REL_L2, mabs=MAX_ABS):
     r = rel_l2(got, ref)
     m = float(np.max(np.abs(got - ref)))
     scale = float(np.max(np.abs(ref)))
+    from conftest import record
+    record(what, rel_l2=r, max_abs_over_scale=m / max(scale, 1e-300), bound_rel_l2=rel, bound_max_abs=mabs)
     assert r <= rel, "%s: rel-L2 %.3e > %.1e" % (what, r, rel)
     assert m <= mabs * scale, "%s: max-abs %.3e > %.1e * %.3e" % (what, m, mabs, scale)
     return r, m / max(scale, 1e-300)
@@ -92,7 +94,7 @@ def test_binomial_sampler_matches_oracle(B, O):
     got = dk.cpu().numpy()
     ref = np.array([O.binomial(N[i], p[i], int(w[i])) for i in range(n)])
     bad = np.flatnonzero(got != ref)
-    assert bad.size <= max(1, int(1e-6 * n)), "sampler differs in %d of %d draws, first %s" % (
+    assert bad.size <= int(1e-6 * n), "sampler differs in %d of %d draws, first %s" % (
         bad.size, n, [(N[i], p[i], w[i], got[i], ref[i]) for i in bad[:5]])
     assert np.all(got >= 0) and np.all(got <= N)
 
@@ -311,13 +313,13 @@ def test_noise_alone_and_fused(B, O):
         p.add_noise(seed=1)
         p.sync()
         N1 = p.output().cpu().numpy()
-        assert_close(N1, ref, "noise standalone", rel=2e-5)
+        assert_close(N1, ref, "noise standalone")
         # fused into the inverse transform of a convolution of S = 0
         p.arm_noise(seed=1)
         p.convolve()
         p.sync()
         N2 = p.output().cpu().numpy()
-        assert_close(N2, ref, "noise fused", rel=2e-5)
+        assert_close(N2, ref, "noise fused")
         # a second convolve is noise free again (the arm is cleared)
         p.convolve()
         p.sync()
@@ -328,7 +330,7 @@ def test_noise_alone_and_fused(B, O):
         p.clear_output()
         p.add_noise(amp=amp, seed=99)
         p.sync()
-        assert_close(p.output().cpu().numpy(), ref2, "noise custom amp", rel=2e-5)
+        assert_close(p.output().cpu().numpy(), ref2, "noise custom amp")
     rms = float(np.sqrt(np.mean(N1.astype(np.float64) ** 2)))
     assert abs(rms - 0.4743) < 0.02
 
@@ -463,7 +465,7 @@ def test_normal_draw_sampler_matches_oracle(B, O):
     got = dk.cpu().numpy()
     ref = np.array([O.normal_draw(N[i], p[i], int(w[i])) for i in range(n)])
     bad = np.flatnonzero(got != ref)
-    assert bad.size <= max(1, int(1e-6 * n)), [(N[i], p[i], w[i], got[i], ref[i]) for i in bad[:5]]
+    assert bad.size <= int(1e-6 * n), [(N[i], p[i], w[i], got[i], ref[i]) for i in bad[:5]]
 
 
 @pytest.mark.parametrize("mode", [0, 1])
@@ -518,6 +520,8 @@ def test_drift_three_planes_matches_oracle_and_feeds_the_raster(B, O):
             assert np.all(np.isnan(got[behind])) and np.all(np.isnan(ref[k][behind]))
             same = got[~behind] == ref[k][~behind]
             # exp differs by <= 1 ulp of fp64 between the two libraries: after rounding to fp32 all but a stray value agree
+            from conftest import record
+            record("drift plane %d %s" % (p, k), values=int(same.size), not_bit_equal=int(same.size - same.sum()))
             assert same.mean() >= (0.999999 if k != "q" else 0.9999), (p, k, same.mean())
             assert np.allclose(got[~behind], ref[k][~behind], rtol=2e-7, atol=0)
     # the drifted depos of plane 2 go straight into the raster; groups behind the plane are skipped and counted
@@ -532,7 +536,7 @@ def test_drift_three_planes_matches_oracle_and_feeds_the_raster(B, O):
     refd = O.drift(g["x"], g["y"], g["z"], g["t"], g["q"], **params, **planes[2])
     S_ref, _, ost = O.raster_scatter(800, 6000, refd, seed=4, fluctuate=True)
     assert st["depos_skipped"] == ost["skipped"] == int((g["x"].astype(np.float64) < planes[2]["x_plane"]).sum())
-    assert np.count_nonzero(S != S_ref) <= max(2, 1e-6 * ost["drawn"])
+    assert np.count_nonzero(S != S_ref) <= int(1e-6 * ost["drawn"])
     with pytest.raises(B.WcsimError):
         B.wcsim_drift(dev, dict(params, v_drift=0.0), planes, out)
 
@@ -681,11 +685,11 @@ def test_noise_every_row_kernel(B, O, nt, pad_t):
         p.arm_noise(None, seed=21)
         p.convolve()  # S = 0: M = N, fused into the inverse rows
         p.sync()
-        assert_close(p.output().cpu().numpy(), ref, "fused noise pad_t %d" % pad_t, rel=2e-5)
+        assert_close(p.output().cpu().numpy(), ref, "fused noise pad_t %d" % pad_t)
         p.clear_output()
         p.add_noise(seed=21)  # standalone pass
         p.sync()
-        assert_close(p.output().cpu().numpy(), ref, "standalone noise pad_t %d" % pad_t, rel=2e-5)
+        assert_close(p.output().cpu().numpy(), ref, "standalone noise pad_t %d" % pad_t)
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -712,7 +716,7 @@ def test_normalized_patches_match_oracle(B, O, mode):
             S = p.charge().cpu().numpy().astype(np.float64)
             if fluct:
                 flipped = int(np.count_nonzero(S != S_ref))
-                assert flipped <= max(1, 1e-6 * st["drawn"]), (mode, fluct, flipped)
+                assert flipped <= int(1e-6 * st["drawn"]), (mode, fluct, flipped)
                 assert int(np.count_nonzero(totals.cpu().numpy() != tot_ref)) <= flipped
             else:
                 assert_close(S, S_ref, "normalised S, mode %d" % mode)
