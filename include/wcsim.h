@@ -161,8 +161,15 @@ int wcsim_reset_stats(wcsim_plan *plan);
 #define WCSIM_STAGE_COLS 2         /* a4 wire axis + a5 multiply + a6 wire axis */
 #define WCSIM_STAGE_ROWS_INVERSE 3 /* a6 tick axis (+ armed noise) */
 #define WCSIM_STAGE_NOISE 4        /* a7 as its own pass (wcsim_add_noise) */
-#define WCSIM_N_STAGES 5
-int wcsim_set_profiling(wcsim_plan *plan, int enable);
+#define WCSIM_STAGE_CONVOLVE 5     /* the whole wcsim_convolve call as ONE span (level WCSIM_PROFILE_CALLS only) */
+#define WCSIM_N_STAGES 6
+/* level: 0 off; WCSIM_PROFILE_KERNELS: an event pair around every kernel of wcsim_convolve (the records sit between the
+ * kernels, which are programmatic dependents of one another, and cost a few microseconds per plane-event);
+ * WCSIM_PROFILE_CALLS: one pair around the whole wcsim_convolve call, nothing between its kernels (stage CONVOLVE).
+ * wcsim_raster_scatter and wcsim_add_noise are one span each at either level. */
+#define WCSIM_PROFILE_KERNELS 1
+#define WCSIM_PROFILE_CALLS 2
+int wcsim_set_profiling(wcsim_plan *plan, int level);
 int wcsim_get_stage_times(wcsim_plan *plan, double *ms, unsigned long long *calls, int reset);
 /* number of kernels of this library enqueued through `plan` so far (memsets and copies are not counted) */
 int wcsim_get_launch_count(const wcsim_plan *plan, unsigned long long *out);

@@ -293,11 +293,13 @@ def wcsim_simulate_host_async(plan, host_depos, host_M, **kw):
     wcsim_simulate_host(plan, host_depos, host_M, _fn="wcsim_simulate_host_async", **kw)
 
 
-STAGES = ("raster", "rows_forward", "cols", "rows_inverse", "noise")
+STAGES = ("raster", "rows_forward", "cols", "rows_inverse", "noise", "convolve")
+WCSIM_PROFILE_KERNELS, WCSIM_PROFILE_CALLS = 1, 2
 
 
-def wcsim_set_profiling(plan, enable):
-    _check(lib().wcsim_set_profiling(plan, int(bool(enable))), "wcsim_set_profiling")
+def wcsim_set_profiling(plan, level):
+    """0 / False off; True or WCSIM_PROFILE_KERNELS: a span per kernel; WCSIM_PROFILE_CALLS: one span per call."""
+    _check(lib().wcsim_set_profiling(plan, int(level)), "wcsim_set_profiling")
 
 
 def wcsim_get_stage_times(plan, reset=True):

@@ -39,11 +39,11 @@ struct wcsim_plan {
         cudaEvent_t beg, end;
         int stage;
     };
-    bool profiling = false;
+    int profiling = 0; // 0 off, WCSIM_PROFILE_KERNELS, WCSIM_PROFILE_CALLS
     std::vector<Span> pending;
     std::vector<cudaEvent_t> free_events;
-    double stage_ms[WCSIM_N_STAGES] = {0, 0, 0, 0, 0};
-    unsigned long long stage_calls[WCSIM_N_STAGES] = {0, 0, 0, 0, 0};
+    double stage_ms[WCSIM_N_STAGES] = {};
+    unsigned long long stage_calls[WCSIM_N_STAGES] = {};
     unsigned long long launches = 0; // kernels of this library enqueued so far
 };
 
@@ -117,9 +117,9 @@ struct StageSpan {
     wcsim_plan *p;
     cudaEvent_t beg = nullptr, end = nullptr;
     int stage;
-    StageSpan(wcsim_plan *plan, int st) : p(plan), stage(st)
+    StageSpan(wcsim_plan *plan, int st, bool enabled = true) : p(plan), stage(st)
     {
-        if (!p->profiling) return;
+        if (!p->profiling || !enabled) return;
         if (p->pending.size() >= 8192) harvest_spans(p);
         beg = take_event(p);
         end = take_event(p);
@@ -449,19 +449,21 @@ int wcsim_convolve(wcsim_plan *plan)
         nz.seed = plan->armed_seed;
         plan->noise_armed = false;
     }
+    const bool per_kernel = plan->profiling == WCSIM_PROFILE_KERNELS;
+    StageSpan whole(plan, WCSIM_STAGE_CONVOLVE, !per_kernel);
     {
-        StageSpan span(plan, WCSIM_STAGE_ROWS_FORWARD);
+        StageSpan span(plan, WCSIM_STAGE_ROWS_FORWARD, per_kernel);
         CU_TRY(launch_rows_forward(g, plan->pad_t, b, plan->stream));
     }
     {
-        StageSpan span(plan, WCSIM_STAGE_COLS);
+        StageSpan span(plan, WCSIM_STAGE_COLS, per_kernel);
         if (wires_direct(plan))
             CU_TRY(launch_wires(g, plan->pad_t, b, plan->stream));
         else
             CU_TRY(launch_cols(g, plan->pad_w, plan->pad_t, b, plan->stream));
     }
     {
-        StageSpan span(plan, WCSIM_STAGE_ROWS_INVERSE);
+        StageSpan span(plan, WCSIM_STAGE_ROWS_INVERSE, per_kernel);
         CU_TRY(launch_rows_inverse(g, plan->pad_t, b, nz, true, false, plan->stream));
     }
     plan->launches += 3;
@@ -739,10 +741,10 @@ int wcsim_debug_response_spectrum(wcsim_plan *plan, float *host_out)
     return WCSIM_OK;
 }
 
-int wcsim_set_profiling(wcsim_plan *plan, int enable)
+int wcsim_set_profiling(wcsim_plan *plan, int level)
 {
-    if (!plan) return WCSIM_EINVAL;
-    plan->profiling = enable != 0;
+    if (!plan || level < 0 || level > WCSIM_PROFILE_CALLS) return WCSIM_EINVAL;
+    plan->profiling = level;
     return WCSIM_OK;
 }
 
