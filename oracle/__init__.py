@@ -63,6 +63,8 @@ def lib():
         L.wco_raster_scatter.restype = C.c_int
         L.wco_convolve_direct.argtypes = [C.c_int, C.c_int, f64p, f64p, C.c_int, C.c_int, f64p]
         L.wco_convolve_direct.restype = C.c_int
+        L.wco_convolve_impact.argtypes = [C.c_int, C.c_int, C.c_int, f64p, f64p, C.c_int, C.c_int, f64p]
+        L.wco_convolve_impact.restype = C.c_int
         L.wco_convolve_points.argtypes = [C.c_int, C.c_int, f64p, f64p, C.c_int, C.c_int, C.c_int64, i32p, i32p, f64p]
         L.wco_convolve_points.restype = C.c_int
         L.wco_convolve_fft.argtypes = [C.c_int, C.c_int, f64p, f64p, C.c_int, C.c_int, C.c_int, C.c_int, f64p]
@@ -235,6 +237,22 @@ def convolve_direct(S, R):
                                    _p(M, C.c_double))
     if rc != 0:
         raise ValueError("wco_convolve_direct rc=%d" % rc)
+    return M
+
+
+def convolve_impact(Sf, R, K):
+    """Reading A25: Sf [n_wires*K][n_ticks] (fine row x*K + k = impact position k of wire x), R [K][n_rw][n_rt];
+    returns M [n_wires][n_ticks]."""
+    Sf, R = _f64(Sf), _f64(R)
+    K = int(K)
+    if R.ndim != 3 or R.shape[0] != K or Sf.shape[0] % K:
+        raise ValueError("R must be [K][n_rw][n_rt] and Sf must have a multiple of K rows")
+    n_wires = Sf.shape[0] // K
+    M = np.zeros((n_wires, Sf.shape[1]))
+    rc = lib().wco_convolve_impact(n_wires, Sf.shape[1], K, _p(Sf, C.c_double), _p(R, C.c_double), R.shape[1],
+                                   R.shape[2], _p(M, C.c_double))
+    if rc != 0:
+        raise ValueError("wco_convolve_impact rc=%d" % rc)
     return M
 
 

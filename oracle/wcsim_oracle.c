@@ -29,13 +29,15 @@
  *   normal_draw ........... its formula restated with scipy's ndtri, moments, the paper's
  *                           0.01 % agreement with the binomial waveforms
  *   noise ................. Parseval closed form, spectrum round trip, direct vs FFT
+ *   convolve_impact ....... K = 1 is convolve_direct; a delta at impact position k reproduces R_k;
+ *                           linearity; pure-python brute force; sum over the K sub-grids of convolve_direct
  * PARITY UNPINNED (conventions of this build that nothing in the paper fixes;
  * DESIGN.md readings A3, A6, A8, A15): no patch renormalisation; the mu<16
  * inversion / mu>=16 rounded-normal split of the binomial sampler and its use of
  * AS 241; the Philox counter layout; the orthonormal noise scaling; and, of the
- * steps around the hot path, the conventions of readings A21-A24 (clamp and
+ * steps around the hot path, the conventions of readings A21-A25 (clamp and
  * rounding of the normal draw, drift coordinates and units, the ideal ADC, the
- * patch renormalisation).
+ * patch renormalisation, the layout of the impact-position grid and response).
  *
  * Build: gcc -O2 -std=c11 -fopenmp -ffp-contract=off -shared -fPIC
  *        (-ffp-contract=off: every product and sum is rounded separately, so the
@@ -418,6 +420,46 @@ int wco_convolve_direct(int n_wires, int n_ticks, const double *S, const double 
                 if (s == 0.0) continue;
                 int lim = n_ticks - ts < n_rt ? n_ticks - ts : n_rt;
                 for (int dt = 0; dt < lim; ++dt) Mx[ts + dt] += Rd[dt] * s;
+            }
+        }
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------- */
+/* Sub-wire ("impact position") response binning (reading A25 of DESIGN.md;    */
+/* patches are "typically O(20x20) elements", which a raster on    */
+/* whole wires does not give -- SURVEY 8(f)-4).  The charge grid is K times     */
+/* finer along the wire axis: fine row xf = x*K + k holds the charge that       */
+/* arrives at impact position k (0..K-1) of wire x, i.e. at pitch coordinate    */
+/* [xf/K, (xf+1)/K).  The response is given per impact position, R[k][dx+c][dt],*/
+/* and the measured waveform of wire x sums over the impact positions:          */
+/*   M[x][t] = sum_{k=0..K-1} sum_{dx=-c..c} sum_{dt=0..n_rt-1}                 */
+/*                 R[k][dx+c][dt] Sf[(x-dx)*K + k][t-dt],   Sf = 0 outside.     */
+/* K = 1 is wco_convolve_direct.  Plain loops in the order written; output rows */
+/* are independent.                                                            */
+/* ------------------------------------------------------------------------- */
+int wco_convolve_impact(int n_wires, int n_ticks, int K, const double *Sf, const double *R, int n_rw, int n_rt,
+                        double *M)
+{
+    if (n_wires <= 0 || n_ticks <= 0 || K <= 0 || n_rw <= 0 || n_rt <= 0 || (n_rw % 2) == 0) return -1;
+    const int c = (n_rw - 1) / 2;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int x = 0; x < n_wires; ++x) {
+        double *Mx = M + (size_t)x * n_ticks;
+        for (int t = 0; t < n_ticks; ++t) Mx[t] = 0.0;
+        for (int k = 0; k < K; ++k) {
+            for (int dx = -c; dx <= c; ++dx) {
+                int xs = x - dx;
+                if (xs < 0 || xs >= n_wires) continue;
+                const double *Sx = Sf + ((size_t)xs * K + k) * n_ticks;
+                const double *Rd = R + ((size_t)k * n_rw + (size_t)(dx + c)) * n_rt;
+                for (int ts = 0; ts < n_ticks; ++ts) {
+                    double s = Sx[ts];
+                    if (s == 0.0) continue;
+                    int lim = n_ticks - ts < n_rt ? n_ticks - ts : n_rt;
+                    for (int dt = 0; dt < lim; ++dt) Mx[ts + dt] += Rd[dt] * s;
+                }
             }
         }
     }
