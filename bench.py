@@ -226,7 +226,12 @@ def run_ours(args):
     # plans on three streams are used in turn through wcsim_simulate_host_async, so the 19 MB device->host copy of
     # one plane-event runs under the next event's copies and kernels; a step's M is on the host when its plan is
     # synchronised, which happens before that plan is reused and, for the last steps, before the clock stops.
-    host = {k: torch.from_numpy(v).pin_memory() for k, v in pl["depos"].items()}
+    # the five depo arrays in ONE pinned block: wcsim_simulate_host*_async then sends them in a single copy
+    host_block = torch.empty(5 * n_depos, dtype=torch.float32).pin_memory()
+    host = {}
+    for a_, k_ in enumerate(("t0", "x0", "sigma_t", "sigma_x", "q")):
+        host[k_] = host_block[a_ * n_depos:(a_ + 1) * n_depos]
+        host[k_].copy_(torch.from_numpy(pl["depos"][k_]))
     n_e2e_plans = 3  # two leave the device->host engine idle part of the time (436 us); four gain nothing over three
     e2e_streams = [torch.cuda.Stream(device=dev) for _ in range(n_e2e_plans)]
     e2e_plans = [B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]),
@@ -258,11 +263,8 @@ def run_ours(args):
     for _ in range(min(e2e_steps, 20)):
         plan.simulate_host(host, host_M[0], seed=cfg["fluct_seed"], fluctuate=fluct)
     e2e_sync_ms = (time.perf_counter() - t0) * 1e3 / min(e2e_steps, 20)
-    # extra: the same round trip returning 12-bit ADC codes (wcsim_digitize, reading A23) instead of the fp32 M: half the
-    # device->host bytes.  Copies are torch's, on each plan's stream; every step's codes are on the host when its plan
-    # is synchronised.
-    dev_in = [{k: torch.empty_like(v, device=dev) for k, v in host.items()} for _ in range(n_e2e_plans)]
-    dev_adc = [torch.empty((pl["n_wires"], pl["n_ticks"]), dtype=torch.int16, device=dev) for _ in range(n_e2e_plans)]
+    # extra: the same round trip returning 12-bit ADC codes (wcsim_simulate_host_adc_async, reading A23) instead of the
+    # fp32 M: half the device->host bytes; every step's codes are on the host when its plan is synchronised
     host_adc = [torch.empty((pl["n_wires"], pl["n_ticks"]), dtype=torch.int16).pin_memory() for _ in range(n_e2e_plans)]
 
     def run_e2e_adc(k):
@@ -270,14 +272,7 @@ def run_ours(args):
             j = i % n_e2e_plans
             p = e2e_plans[j]
             p.sync()
-            with torch.cuda.stream(e2e_streams[j]):
-                for kk in host:
-                    dev_in[j][kk].copy_(host[kk], non_blocking=True)
-                p.clear()
-                p.raster_scatter(dev_in[j], seed=cfg["fluct_seed"], fluctuate=fluct)
-                p.convolve()
-                p.digitize(ADC_GAIN, ADC_BASELINE, 12, out=dev_adc[j])
-                host_adc[j].copy_(dev_adc[j], non_blocking=True)
+            p.simulate_host_adc_async(host, host_adc[j], ADC_GAIN, ADC_BASELINE, 12, seed=cfg["fluct_seed"], fluctuate=fluct)
         for p in e2e_plans:
             p.sync()
 
@@ -292,9 +287,16 @@ def run_ours(args):
 
     # ---- several independent plane-events in flight (the paper's section 3.3 runs several processes
     # per GPU for the same reason: one event does not fill the device).  Extra figure, not the headline.
-    concurrent = None
+    concurrent = batched = graphed = None
     if args.streams > 1 and world == 1:
         concurrent = concurrent_planes(args, B, cfg, pl, d, fluct, mode, dev, n_depos)
+        if len(cfg["planes"]) == 1:
+            # the same number of independent plane-events through ONE launch sequence of a multi-plane plan
+            batched = batched_events(args, B, cfg, [pl] * args.streams, [d] * args.streams, fluct, mode, dev)
+            batched["ms_per_plane_event"] = batched["ms_per_event"] / args.streams
+            batched["ms_per_plane_event_cuda_graph"] = batched["ms_per_event_cuda_graph"] / args.streams
+    if world == 1:
+        graphed = graph_plane_event(args, B, cfg, pl, d, fluct, mode, dev, flush)
 
     # configs[3] is an APA event: three planes with their own responses, noise on every one.  Extra figure: whole events,
     # the three planes of an event on three plans/streams (planes are independent)
@@ -385,7 +387,7 @@ def run_ours(args):
                 "ms_per_step_synchronous_call": e2e_sync_ms,
                 "adc_variant": {"ms_per_step": e2e_adc_ms, "value": n_depos / (e2e_adc_ms * 1e-3),
                                 "d2h_bytes_per_step": d2h // 2,
-                                "what": "same round trip with wcsim_digitize: 12-bit ADC codes (int16) come back instead of fp32 M"}},
+                                "what": "wcsim_simulate_host_adc_async: 12-bit ADC codes (int16) come back instead of fp32 M"}},
         "gpu_launches": launches,
         "roofline": roofline,
         "ms_per_step_median": statistics.median(per_step),
@@ -395,6 +397,10 @@ def run_ours(args):
     }
     if concurrent:
         out["concurrent"] = concurrent
+    if batched:
+        out["batched"] = batched
+    if graphed:
+        out["cuda_graph"] = graphed
     if apa:
         out["apa_event"] = apa
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -459,7 +465,9 @@ def concurrent_planes(args, B, cfg, pl, d, fluct, mode, dev, n_depos):
 
 
 def apa_events(args, B, cfg, fluct, mode, dev):
-    """K whole events of a multi-plane config: plane p of every event on plan/stream p; one CUDA-event pair around all."""
+    """K whole events of a multi-plane config, two ways: plane p of every event on its own plan/stream (round 1's way),
+    and all planes through ONE launch sequence of a multi-plane plan (wcsim_plan_create_planes: one raster launch, row
+    transforms over the stacked rows, one wire pass), issued call by call and replayed from a CUDA graph."""
     import torch
     planes = cfg["planes"]
     streams = [torch.cuda.Stream(device=dev) for _ in planes]
@@ -492,9 +500,100 @@ def apa_events(args, B, cfg, fluct, mode, dev):
     ms = run(args.steps)
     for p in plans:
         p.destroy()
-    return {"planes": len(planes), "depos_per_event": n_depos, "events": args.steps, "ms_per_event": ms / args.steps,
-            "value": n_depos * args.steps / (ms * 1e-3), "unit": UNIT,
-            "what": "whole events, plane p on plan/stream p (raster + fused noise + convolve per plane)"}
+    out = {"planes": len(planes), "depos_per_event": n_depos, "events": args.steps, "ms_per_event": ms / args.steps,
+           "value": n_depos * args.steps / (ms * 1e-3), "unit": UNIT,
+           "what": "whole events, plane p on plan/stream p (raster + fused noise + convolve per plane)"}
+    out["batched"] = batched_events(args, B, cfg, planes, depos, fluct, mode, dev)
+    return out
+
+
+def batched_events(args, B, cfg, planes, depos, fluct, mode, dev):
+    """K events, all planes of an event through one launch sequence of a multi-plane plan; call by call and as a CUDA graph."""
+    import torch
+    n_depos = sum(int(d["t0"].numel()) for d in depos)
+    st = torch.cuda.Stream(device=dev)
+    bmode = mode if mode != B.WCSIM_SCATTER_TILED else B.WCSIM_SCATTER_FIXED  # the tiled mode is per plane
+    plan = B.PlanesPlan([pl["n_wires"] for pl in planes], planes[0]["n_ticks"], [pl["response"] for pl in planes],
+                        pad_ticks=planes[0]["pad_t"], nsigma=cfg["nsigma"], scatter_mode=bmode, stream=st)
+
+    def event():
+        plan.clear()
+        plan.raster_scatter_planes(depos, seed=cfg["fluct_seed"], fluctuate=fluct)
+        if cfg.get("noise"):
+            plan.arm_noise(None, seed=cfg["noise_seed"])
+        plan.convolve()
+
+    def run(fn, k):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record(st)
+        for _ in range(k):
+            fn()
+        b.record(st)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b)
+
+    run(event, 3)
+    l0 = plan.launch_count()
+    ms_calls = run(event, args.steps)
+    launches = (plan.launch_count() - l0) / args.steps
+    plan.graph_begin()
+    event()
+    graph = plan.graph_end()
+    run(graph.launch, 3)
+    ms_graph = run(graph.launch, args.steps)
+    graph.destroy()
+    plan.destroy()
+    return {"planes": len(planes), "depos_per_event": n_depos, "events": args.steps, "kernel_launches_per_event": launches,
+            "ms_per_event": ms_calls / args.steps, "value": n_depos * args.steps / (ms_calls * 1e-3),
+            "ms_per_event_cuda_graph": ms_graph / args.steps, "value_cuda_graph": n_depos * args.steps / (ms_graph * 1e-3),
+            "unit": UNIT, "what": "all planes of an event through one launch sequence of a multi-plane plan "
+                                  "(wcsim_plan_create_planes), events back to back, no L2 flush"}
+
+
+def graph_plane_event(args, B, cfg, pl, d, fluct, mode, dev, flush):
+    """The headline plane-event replayed from a CUDA graph on its own stream (clear, raster, convolve recorded once):
+    per-step CUDA-event pairs, L2 flushed before each step as in the headline."""
+    import torch
+    st = torch.cuda.Stream(device=dev)
+    if mode == B.WCSIM_SCATTER_TILED:
+        return None
+    plan = B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]), nsigma=cfg["nsigma"],
+                  scatter_mode=mode, stream=st)
+
+    def event():
+        plan.clear()
+        plan.raster_scatter(d, seed=cfg["fluct_seed"], fluctuate=fluct)
+        if cfg.get("noise"):
+            plan.arm_noise(None, seed=cfg["noise_seed"])
+        plan.convolve()
+
+    event()  # first use allocates what the mode needs
+    plan.sync()
+    plan.graph_begin()
+    event()
+    graph = plan.graph_end()
+
+    def timed(fn, k):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            for a, b in ev:
+                flush.fill_(1.0)
+                a.record(st)
+                fn()
+                b.record(st)
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in ev]
+
+    timed(graph.launch, 3)
+    per_graph = timed(graph.launch, args.steps)
+    per_calls = timed(event, args.steps)
+    graph.destroy()
+    plan.destroy()
+    return {"ms_per_step": sum(per_graph) / len(per_graph), "ms_per_step_median": statistics.median(per_graph),
+            "ms_per_step_same_stream_call_by_call": sum(per_calls) / len(per_calls),
+            "what": "the same plane-event replayed from a CUDA graph (wcsim_graph_*), L2 flushed between steps"}
 
 
 def cufft_comparator(pl, dev, flush):

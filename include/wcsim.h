@@ -197,6 +197,57 @@ int wcsim_simulate_host_async(wcsim_plan *plan, const float *host_t0, const floa
                         const float *host_sigma_x, const float *host_q, long long n, unsigned long long seed,
                         int fluctuate, int noise, unsigned long long noise_seed, float *host_M);
 
+/* The same round trip returning ADC codes instead of the fp32 M (wcsim_digitize below, reading A23): half the device->host
+ * bytes.  host_adc: HOST, n_wires*n_ticks int16, written; valid after wcsim_sync(plan).  The codes are staged in a device
+ * buffer the plan owns.  If the five host depo arrays follow one another in memory (one block of 5 n floats, as here), they
+ * go over in one copy.  Errors: as wcsim_simulate_host_async; bits outside 1..15: WCSIM_EINVAL. */
+int wcsim_simulate_host_adc_async(wcsim_plan *plan, const float *host_t0, const float *host_x0, const float *host_sigma_t,
+                                  const float *host_sigma_x, const float *host_q, long long n, unsigned long long seed,
+                                  int fluctuate, int noise, unsigned long long noise_seed, float gain, float baseline,
+                                  int bits, short *host_adc);
+
+/*
+ * Several planes through ONE launch sequence (Section 3.3 and Fig. 4: "with one process
+ * per GPU the GPU is under-utilized"; the planes of an anode are independent).  A multi-plane plan stacks
+ * 1..8 planes of the same n_ticks, tick padding and response footprint (n_rwires x n_rticks) along the wire axis:
+ * plane p owns rows first_row(p) .. first_row(p) + n_wires[p] - 1 of S and M (wcsim_get_plane_rows).  One raster launch
+ * takes the depos of all planes, the row transforms run over all stacked rows, one direct wire pass applies every plane's
+ * own response (planes never mix: each has its own zero halo rows), noise is keyed by the plane's own wire index.  Every
+ * plane's S and M equal what a plan of that plane alone gives (same seeds; depo ids start at 0 in every plane).
+ *   n_wires   : HOST, n_planes ints;  responses : HOST, n_planes pointers to n_rwires x n_rticks floats each.
+ *   pad_ticks : 0 = automatic.  The wire axis is always done directly (WCSIM_WIRES_DIRECT), so there is no wire padding.
+ *   scatter_mode : WCSIM_SCATTER_ATOMIC or WCSIM_SCATTER_FIXED (the tiled mode is per plane: WCSIM_EINVAL).
+ * wcsim_clear, wcsim_convolve, wcsim_arm_noise / wcsim_add_noise (the same spectrum and seed for every plane),
+ * wcsim_digitize, wcsim_charge_ptr / wcsim_output_ptr (the stacked grids) work on such a plan as on any other;
+ * wcsim_raster_scatter and the *_host calls return WCSIM_ESTATE.
+ */
+int wcsim_plan_create_planes(wcsim_plan **out, int n_planes, const int *n_wires, int n_ticks,
+                             const float *const *responses, int n_rwires, int n_rticks, int pad_ticks, float nsigma,
+                             int scatter_mode, void *cuda_stream);
+/* a1-a3 for all planes of the plan in one launch.  depos: HOST array of n_planes structs of DEVICE pointers; n: HOST,
+ * n_planes counts (0 allowed).  Depo d of plane p has id d; the Philox bin is the plane's own wire * n_ticks + tick (A8).
+ * Works on single-plane plans too (n_planes = 1).  No per-depo totals.  Errors: WCSIM_ESTATE in tiled scatter mode. */
+int wcsim_raster_scatter_planes(wcsim_plan *plan, const wcsim_depos *depos, const long long *n, unsigned long long seed,
+                                int fluctuate);
+int wcsim_get_plane_rows(const wcsim_plan *plan, int plane, int *first_row, int *n_rows);
+
+/*
+ * CUDA graphs (a small plane-event is bound by launch latency).  Between wcsim_graph_begin and
+ * wcsim_graph_end the plan's stream is in capture mode: wcsim_clear, wcsim_raster_scatter(_planes), wcsim_arm_noise
+ * (built-in spectrum), wcsim_convolve, wcsim_add_noise (built-in), wcsim_digitize only RECORD their work (the kernels keep
+ * their programmatic-dependent-launch edges); the graph replays that sequence on the plan's stream at every
+ * wcsim_graph_launch, with the pointers and sizes recorded (the depo arrays must still be valid and may hold new values).
+ * Not capturable (WCSIM_ESTATE while capturing): the tiled scatter mode (it reads a size back), a first use of the
+ * fixed-point mode on the plan, custom noise spectra, anything that synchronises (wcsim_sync, wcsim_get_stats, the
+ * *_host calls must not be called).  The plan's stream must not be the legacy default stream (WCSIM_ESTATE).
+ * Stage timing is off inside a capture.  Destroy graphs before their plan.
+ */
+typedef struct wcsim_graph wcsim_graph;
+int wcsim_graph_begin(wcsim_plan *plan);
+int wcsim_graph_end(wcsim_plan *plan, wcsim_graph **out); /* *out = NULL on failure */
+int wcsim_graph_launch(wcsim_graph *graph);
+int wcsim_graph_destroy(wcsim_graph *graph);
+
 /*
  * Drift: the step upstream of the Raster ("After simulating the diffusion process along the drifting, each
  * ionization electron group is diffused into a 2D distribution along the drifting and wire pitch directions"; reading

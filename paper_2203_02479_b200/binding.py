@@ -25,6 +25,8 @@ SYMBOLS = [
     "wcsim_simulate_host", "wcsim_set_profiling", "wcsim_get_stage_times", "wcsim_get_launch_count",
     "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf", "wcsim_simulate_host_async", "wcsim_debug_normal_draw", "wcsim_drift", "wcsim_digitize", "wcsim_set_normalize",
     "wcsim_debug_fast_normal", "wcsim_debug_z32_scan",
+    "wcsim_plan_create_planes", "wcsim_raster_scatter_planes", "wcsim_get_plane_rows", "wcsim_simulate_host_adc_async",
+    "wcsim_graph_begin", "wcsim_graph_end", "wcsim_graph_launch", "wcsim_graph_destroy",
     "wcsim_strerror", "wcsim_last_cuda_error", "wcsim_version",
 ]
 
@@ -100,6 +102,14 @@ def lib():
         L.wcsim_digitize.argtypes = [vp, C.c_float, C.c_float, i, vp]
         L.wcsim_drift.argtypes = [vp, vp, vp, vp, vp, ll, C.POINTER(wcsim_drift_params), C.POINTER(wcsim_plane_geom), i,
                                   C.POINTER(wcsim_depos), vp]
+        L.wcsim_plan_create_planes.argtypes = [C.POINTER(vp), i, C.POINTER(i), i, C.POINTER(vp), i, i, i, C.c_float, i, vp]
+        L.wcsim_raster_scatter_planes.argtypes = [vp, C.POINTER(wcsim_depos), C.POINTER(ll), ull, i]
+        L.wcsim_get_plane_rows.argtypes = [vp, i, C.POINTER(i), C.POINTER(i)]
+        L.wcsim_simulate_host_adc_async.argtypes = [vp, vp, vp, vp, vp, vp, ll, ull, i, i, ull, C.c_float, C.c_float, i, vp]
+        L.wcsim_graph_begin.argtypes = [vp]
+        L.wcsim_graph_end.argtypes = [vp, C.POINTER(vp)]
+        L.wcsim_graph_launch.argtypes = [vp]
+        L.wcsim_graph_destroy.argtypes = [vp]
         L.wcsim_strerror.argtypes = [i]
         L.wcsim_strerror.restype = C.c_char_p
         L.wcsim_last_cuda_error.argtypes = []
@@ -269,28 +279,111 @@ def wcsim_reset_stats(plan):
     _check(lib().wcsim_reset_stats(plan), "wcsim_reset_stats")
 
 
+def _host_ptr(a, itemsize=4):
+    """(pointer, element count) of a contiguous HOST array of `itemsize`-byte elements (numpy, or a torch CPU tensor)."""
+    if hasattr(a, "data_ptr"):
+        if a.is_cuda or not a.is_contiguous() or a.element_size() != itemsize:
+            raise ValueError("expected a contiguous host tensor of %d-byte elements" % itemsize)
+        return C.c_void_p(a.data_ptr()), a.numel()
+    if a.dtype.itemsize != itemsize or not a.flags.c_contiguous:
+        raise ValueError("expected a C-contiguous host array of %d-byte elements" % itemsize)
+    return a.ctypes.data_as(C.c_void_p), a.size
+
+
+def _host_depo_ptrs(host_depos, n):
+    ptrs = [_host_ptr(host_depos[k]) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")]
+    for k in ("t0", "x0", "sigma_t", "sigma_x", "q"):
+        if not str(host_depos[k].dtype).endswith("float32"):
+            raise ValueError("host depo array %s must be float32" % k)
+    if n is None:
+        n = ptrs[0][1]
+    if any(cnt < n for _, cnt in ptrs):
+        raise ValueError("host depo array shorter than n")
+    return [p for p, _ in ptrs], int(n)
+
+
 def wcsim_simulate_host(plan, host_depos, host_M, n=None, seed=0, fluctuate=False, noise=False, noise_seed=0,
                         _fn="wcsim_simulate_host"):
     """host_depos: dict of HOST float32 arrays (numpy, or torch CPU tensors -- pinned makes the copies asynchronous);
     host_M: HOST float32 [n_wires][n_ticks], written."""
-    def hp(a):
-        if hasattr(a, "data_ptr"):
-            assert (not a.is_cuda) and a.is_contiguous() and a.element_size() == 4
-            return C.c_void_p(a.data_ptr()), a.numel()
-        assert a.dtype == np.float32 and a.flags.c_contiguous
-        return a.ctypes.data_as(C.c_void_p), a.size
-    ptrs = [hp(host_depos[k]) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")]
-    if n is None:
-        n = ptrs[0][1]
-    pm, _ = hp(host_M)
-    st = getattr(lib(), _fn)(plan, *[p for p, _ in ptrs], int(n), int(seed), _fluct(fluctuate),
-                             int(bool(noise)), int(noise_seed), pm)
+    ptrs, n = _host_depo_ptrs(host_depos, n)
+    pm, cnt = _host_ptr(host_M)
+    n_wires, n_ticks, _, _ = wcsim_get_dims(plan)
+    if cnt != n_wires * n_ticks:
+        raise ValueError("host_M must hold n_wires * n_ticks = %d floats, got %d" % (n_wires * n_ticks, cnt))
+    st = getattr(lib(), _fn)(plan, *ptrs, n, int(seed), _fluct(fluctuate), int(bool(noise)), int(noise_seed), pm)
     _check(st, _fn)
 
 
 def wcsim_simulate_host_async(plan, host_depos, host_M, **kw):
     """As wcsim_simulate_host without the final synchronisation: host_M is valid after wcsim_sync(plan)."""
     wcsim_simulate_host(plan, host_depos, host_M, _fn="wcsim_simulate_host_async", **kw)
+
+
+def wcsim_simulate_host_adc_async(plan, host_depos, host_adc, gain, baseline, bits=12, n=None, seed=0, fluctuate=False,
+                                  noise=False, noise_seed=0):
+    """host_adc: HOST int16 [n_wires][n_ticks], written; valid after wcsim_sync(plan)."""
+    ptrs, n = _host_depo_ptrs(host_depos, n)
+    pa, cnt = _host_ptr(host_adc, 2)
+    n_wires, n_ticks, _, _ = wcsim_get_dims(plan)
+    if cnt != n_wires * n_ticks:
+        raise ValueError("host_adc must hold n_wires * n_ticks = %d int16, got %d" % (n_wires * n_ticks, cnt))
+    st = lib().wcsim_simulate_host_adc_async(plan, *ptrs, n, int(seed), _fluct(fluctuate), int(bool(noise)),
+                                             int(noise_seed), float(gain), float(baseline), int(bits), pa)
+    _check(st, "wcsim_simulate_host_adc_async")
+
+
+def wcsim_plan_create_planes(n_wires, n_ticks, responses, pad_ticks=0, nsigma=3.0, scatter_mode=WCSIM_SCATTER_ATOMIC,
+                             stream=None):
+    """n_wires: one int per plane; responses: one host array [n_rwires][n_rticks] per plane (same shape)."""
+    rs = [np.ascontiguousarray(r, dtype=np.float32) for r in responses]
+    if len(rs) != len(n_wires) or not rs or any(r.ndim != 2 or r.shape != rs[0].shape for r in rs):
+        raise ValueError("one 2-D response of the same shape per plane")
+    nw = (C.c_int * len(rs))(*[int(w) for w in n_wires])
+    rp = (C.c_void_p * len(rs))(*[r.ctypes.data_as(C.c_void_p) for r in rs])
+    h = C.c_void_p()
+    st = lib().wcsim_plan_create_planes(C.byref(h), len(rs), nw, int(n_ticks), rp, rs[0].shape[0], rs[0].shape[1],
+                                        int(pad_ticks), float(nsigma), int(scatter_mode), _stream_ptr(stream))
+    _check(st, "wcsim_plan_create_planes")
+    return h
+
+
+def wcsim_raster_scatter_planes(plan, depos, n=None, seed=0, fluctuate=False):
+    """depos: one dict of torch CUDA float32 tensors t0, x0, sigma_t, sigma_x, q per plane."""
+    import torch
+    keys = ("t0", "x0", "sigma_t", "sigma_x", "q")
+    if n is None:
+        n = [d["t0"].numel() for d in depos]
+    for d, cnt in zip(depos, n):
+        if any(d[k].numel() < cnt for k in keys):
+            raise ValueError("depo array shorter than n")
+    ds = (wcsim_depos * len(depos))(*[wcsim_depos(*[_dev_ptr(d[k], torch.float32) for k in keys]) for d in depos])
+    ns = (C.c_longlong * len(depos))(*[int(c) for c in n])
+    _check(lib().wcsim_raster_scatter_planes(plan, ds, ns, int(seed), _fluct(fluctuate)), "wcsim_raster_scatter_planes")
+
+
+def wcsim_get_plane_rows(plan, plane):
+    a, b = C.c_int(), C.c_int()
+    _check(lib().wcsim_get_plane_rows(plan, int(plane), C.byref(a), C.byref(b)), "wcsim_get_plane_rows")
+    return a.value, b.value
+
+
+def wcsim_graph_begin(plan):
+    _check(lib().wcsim_graph_begin(plan), "wcsim_graph_begin")
+
+
+def wcsim_graph_end(plan):
+    g = C.c_void_p()
+    _check(lib().wcsim_graph_end(plan, C.byref(g)), "wcsim_graph_end")
+    return g
+
+
+def wcsim_graph_launch(graph):
+    _check(lib().wcsim_graph_launch(graph), "wcsim_graph_launch")
+
+
+def wcsim_graph_destroy(graph):
+    _check(lib().wcsim_graph_destroy(graph), "wcsim_graph_destroy")
 
 
 STAGES = ("raster", "rows_forward", "cols", "rows_inverse", "noise", "convolve")
@@ -329,6 +422,9 @@ def wcsim_debug_binomial(dev_N, dev_p, dev_w, dev_k, n, stream=None):
 def wcsim_digitize(plan, gain, baseline, bits, dev_adc):
     """dev_adc: DEVICE int16 tensor of n_wires*n_ticks elements, written (ideal ADC of reading A23)."""
     import torch
+    n_wires, n_ticks, _, _ = wcsim_get_dims(plan)
+    if dev_adc is None or dev_adc.numel() < n_wires * n_ticks:
+        raise ValueError("dev_adc must hold n_wires * n_ticks int16")
     _check(lib().wcsim_digitize(plan, float(gain), float(baseline), int(bits), _dev_ptr(dev_adc, torch.int16)),
            "wcsim_digitize")
 
@@ -337,13 +433,18 @@ def wcsim_drift(groups, params, planes, out, n=None, stream=None):
     """groups: dict x, y, z, t, q of DEVICE float32 tensors; params: dict of wcsim_drift_params fields; planes: list of
     dicts of wcsim_plane_geom fields; out: list (one per plane) of dicts t0, x0, sigma_t, sigma_x, q of DEVICE float32
     tensors, written."""
-    ptrs = [_dev_ptr(groups[k]) for k in ("x", "y", "z", "t", "q")]
+    import torch
+    ptrs = [_dev_ptr(groups[k], torch.float32) for k in ("x", "y", "z", "t", "q")]
     if n is None:
         n = groups["x"].numel()
+    if any(groups[k].numel() < n for k in ("x", "y", "z", "t", "q")):
+        raise ValueError("group array shorter than n")
+    if len(out) != len(planes) or any(o[k].numel() < n for o in out for k in ("t0", "x0", "sigma_t", "sigma_x", "q")):
+        raise ValueError("one set of output arrays of at least n floats per plane")
     prm = wcsim_drift_params(**{k: float(params.get(k, 0.0)) for k, _ in wcsim_drift_params._fields_})
     geo = (wcsim_plane_geom * len(planes))(*[wcsim_plane_geom(**{k: float(p[k]) for k, _ in wcsim_plane_geom._fields_})
                                             for p in planes])
-    outs = (wcsim_depos * len(planes))(*[wcsim_depos(*[_dev_ptr(o[k]) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")])
+    outs = (wcsim_depos * len(planes))(*[wcsim_depos(*[_dev_ptr(o[k], torch.float32) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")])
                                          for o in out])
     _check(lib().wcsim_drift(*ptrs, int(n), C.byref(prm), geo, len(planes), outs, _stream_ptr(stream)), "wcsim_drift")
 
@@ -473,5 +574,51 @@ class Plan:
     def simulate_host_async(self, host_depos, host_M, **kw):
         wcsim_simulate_host_async(self.handle, host_depos, host_M, **kw)
 
+    def simulate_host_adc_async(self, host_depos, host_adc, gain, baseline, bits=12, **kw):
+        wcsim_simulate_host_adc_async(self.handle, host_depos, host_adc, gain, baseline, bits, **kw)
+
     def response_spectrum(self):
         return wcsim_debug_response_spectrum(self.handle)
+
+    def raster_scatter_planes(self, depos, **kw):
+        wcsim_raster_scatter_planes(self.handle, depos, **kw)
+
+    def plane_rows(self, plane):
+        return wcsim_get_plane_rows(self.handle, plane)
+
+    def graph_begin(self):
+        wcsim_graph_begin(self.handle)
+
+    def graph_end(self):
+        return Graph(wcsim_graph_end(self.handle), self)
+
+
+class PlanesPlan(Plan):
+    """A multi-plane plan (wcsim_plan_create_planes): the planes of one event through one launch sequence."""
+
+    def __init__(self, n_wires, n_ticks, responses, pad_ticks=0, nsigma=3.0, scatter_mode=WCSIM_SCATTER_ATOMIC, stream=None):
+        self.handle = wcsim_plan_create_planes(n_wires, n_ticks, responses, pad_ticks, nsigma, scatter_mode, stream)
+        self.n_wires, self.n_ticks, self.pad_w, self.pad_t = wcsim_get_dims(self.handle)
+        self.n_planes = len(n_wires)
+
+
+class Graph:
+    """A captured launch sequence of a plan (wcsim_graph_*); keeps the plan alive."""
+
+    def __init__(self, handle, plan):
+        self.handle, self.plan = handle, plan
+
+    def launch(self):
+        wcsim_graph_launch(self.handle)
+
+    def destroy(self):
+        if self.handle is not None:
+            h, self.handle = self.handle, None
+            wcsim_graph_destroy(h)
+
+    def __del__(self):
+        try:
+            if self.plan.handle is not None:
+                self.destroy()
+        except Exception:
+            pass

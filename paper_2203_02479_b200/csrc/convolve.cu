@@ -73,7 +73,8 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
 #pragma unroll
     for (int e = 0; e < E; ++e) smem[smem_index<1>(i + e * NT, 0)] = v[e];
     __syncthreads();
-    float2 *dst = b.spec + (size_t)row * b.spec_stride;
+    const int pl = plane_of_row(b.planes, row);
+    float2 *dst = b.spec + (size_t)(b.planes.srow0[pl] + row - b.planes.row0[pl]) * b.spec_stride;
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const int k = i + e * NT;
@@ -169,16 +170,19 @@ __global__ void __launch_bounds__(32 * kWiresRG, 3) wires_kernel(GridDims g, Con
     if ((int)(blockIdx.y * gridDim.x + blockIdx.x) >= tail_from) pdl_trigger();
     pdl_wait(); // the row spectra are rows_forward's
     const int k = blockIdx.x * 32 + threadIdx.x;
-    const int x0 = (blockIdx.y * kWiresRG + threadIdx.y) * O;
-    if (k >= nk || x0 >= g.n_wires) return;
+    int pl = 0; // the plane of this row group (uniform over the CTA)
+    while (pl + 1 < b.planes.n && (int)blockIdx.y >= b.planes.grp0[pl + 1]) ++pl;
+    const int x0 = ((blockIdx.y - b.planes.grp0[pl]) * kWiresRG + threadIdx.y) * O; // first output wire, in the plane
+    const int n_wires = b.planes.row0[pl + 1] - b.planes.row0[pl];
+    if (k >= nk || x0 >= n_wires) return;
     const ptrdiff_t stride = STRIDE ? (ptrdiff_t)STRIDE : (ptrdiff_t)b.spec_stride;
     const int c = (b.n_rw - 1) / 2;
     float2 acc[O];
 #pragma unroll
     for (int o = 0; o < O; ++o) acc[o] = make_float2(0.f, 0.f);
     // chunk d0 uses wire rows x0 + c - d0 - (D-1) .. x0 + c - d0 + O - 1 (halo rows included) and Rt rows d0 .. d0+D-1
-    const float2 *in = b.spec + k + ((ptrdiff_t)x0 + c - (D - 1)) * stride; // plain loads: see pdl.cuh
-    const float2 *__restrict__ rt = b.Rt + k;
+    const float2 *in = b.spec + k + ((ptrdiff_t)(b.planes.srow0[pl] + x0) + c - (D - 1)) * stride; // plain loads: see pdl.cuh
+    const float2 *__restrict__ rt = b.Rt + k + (ptrdiff_t)pl * b.rt_rows * stride;
     const int n_chunks = NCH ? NCH : b.rt_rows / D;
 #pragma unroll
     for (int ch = 0; ch < n_chunks; ++ch) {
@@ -200,10 +204,10 @@ __global__ void __launch_bounds__(32 * kWiresRG, 3) wires_kernel(GridDims g, Con
         in -= D * stride;
         rt += D * stride;
     }
-    float2 *__restrict__ out = b.spec2 + k + (ptrdiff_t)x0 * stride;
+    float2 *__restrict__ out = b.spec2 + k + (ptrdiff_t)(b.planes.row0[pl] + x0) * stride;
 #pragma unroll
     for (int o = 0; o < O; ++o)
-        if (x0 + o < g.n_wires) out[o * stride] = acc[o];
+        if (x0 + o < n_wires) out[o * stride] = acc[o];
 }
 
 // ------------------------------------------------------------------------------------------------------------------
@@ -234,6 +238,7 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
     pdl_wait(); // a no-op unless launched as a programmatic dependent
     const float2 *src = b.spec_inv + (size_t)row * b.spec_stride;
     const bool noisy = nz.amp != nullptr;
+    const uint32_t wire = (uint32_t)(row - b.planes.row0[plane_of_row(b.planes, row)]); // the noise is keyed by the plane's own wire
     float2 v[E];
     if (use_spec && !noisy) {
         // plain convolution: the partner bin X_{N-k} is read straight from the spectrum row (descending, still
@@ -256,11 +261,11 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
         for (int e = 0; e < E; ++e) {
             const int k = i + e * NT;
             float2 x = use_spec ? src[k] : make_float2(0.f, 0.f);
-            if (noisy) x = cadd(x, noise_bin(nz, (uint32_t)row, (uint32_t)k));
+            if (noisy) x = cadd(x, noise_bin(nz, wire, (uint32_t)k));
             if (k == 0) {
                 x.y = 0.f; // the imaginary parts of the DC and Nyquist bins do not reach a real output
                 float2 xn = use_spec ? src[N] : make_float2(0.f, 0.f);
-                if (noisy) xn = cadd(xn, noise_bin(nz, (uint32_t)row, (uint32_t)N));
+                if (noisy) xn = cadd(xn, noise_bin(nz, wire, (uint32_t)N));
                 xn.y = 0.f;
                 smem[smem_index<1>(N, 0)] = xn;
             }
@@ -327,9 +332,10 @@ __global__ void __launch_bounds__(RowTma<N>::threads, RowTma<N>::min_ctas) rows_
         mbar_wait(bar, parity);
         parity ^= 1u;
         if (noisy) {
+            const uint32_t wire = (uint32_t)(row - b.planes.row0[plane_of_row(b.planes, row)]); // the plane's own wire
             // one Philox call gives the phases of four consecutive frequency bins (A17): a thread takes whole calls
             for (int q = i; q < N / 4; q += NT) {
-                const uint4 words = noise_words(nz.seed, (uint32_t)row, (uint32_t)q);
+                const uint4 words = noise_words(nz.seed, wire, (uint32_t)q);
                 const float4 a = __ldg(reinterpret_cast<const float4 *>(nz.amp) + q);
                 float4 *x = reinterpret_cast<float4 *>(stage + 4 * q);
                 float4 lo = x[0], hi = x[1];
@@ -340,7 +346,7 @@ __global__ void __launch_bounds__(RowTma<N>::threads, RowTma<N>::min_ctas) rows_
                 sincospif(noise_phase(words.w), &sn, &cs), hi.z = fmaf(a.w, cs, hi.z), hi.w = fmaf(a.w, sn, hi.w);
                 x[0] = lo, x[1] = hi;
             }
-            if (i == 0) stage[N] = cadd(stage[N], noise_bin(nz, (uint32_t)row, (uint32_t)N));
+            if (i == 0) stage[N] = cadd(stage[N], noise_bin(nz, wire, (uint32_t)N));
             __syncthreads();
         }
         // Z_k = (X_k + conj X_{N-k}) + i exp(+2 pi i k / 2N) (X_k - conj X_{N-k});  inverse FFT of Z = even + i odd
@@ -501,6 +507,7 @@ cudaError_t launch_cols(GridDims g, int pad_w, int pad_t, ConvBuffers b, cudaStr
 }
 
 int wires_chunk() { return kWiresD; }
+int wires_rows_per_group() { return kWiresO * kWiresRG; }
 
 // zero rows the direct wire kernel may read below wire 0 / above wire n_wires-1 of the row spectra
 void wires_halo(int n_rw, int *below, int *above)
@@ -515,7 +522,7 @@ cudaError_t launch_wires(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st)
 {
     constexpr int O = kWiresO;
     const int nk = pad_t / 2 + 1;
-    const dim3 block(32, kWiresRG), grid((nk + 31) / 32, (g.n_wires + O * kWiresRG - 1) / (O * kWiresRG));
+    const dim3 block(32, kWiresRG), grid((nk + 31) / 32, b.planes.grp0[b.planes.n]); // row groups of all planes
     // BASELINE.json's paddings and response widths (21 wires -> 3 chunks, 41 -> 6) get immediate-offset loads and an
     // unrolled chunk loop; anything else takes the generic instance
     const int key = b.rt_rows / kWiresD * 100000 + b.spec_stride;

@@ -13,6 +13,23 @@ struct GridDims {
     int n_wires, n_ticks;
 };
 
+// The planes of a plan, stacked along the wire axis (wcsim_plan_create_planes: the planes of one APA event go through one
+// launch sequence; an ordinary plan has n = 1).  Plane p owns rows row0[p] .. row0[p+1]-1 of S, M and the
+// product spectra; in the row-spectrum buffer its rows start at srow0[p], with the wire pass's zero halo rows in between.
+constexpr int kMaxPlanes = 8;
+struct PlaneTable {
+    int n;
+    int row0[kMaxPlanes + 1];
+    int srow0[kMaxPlanes];
+    int grp0[kMaxPlanes + 1]; // first row group (blockIdx.y of the direct wire pass) of plane p
+};
+__host__ __device__ inline int plane_of_row(const PlaneTable &t, int row)
+{
+    int p = 0;
+    while (p + 1 < t.n && row >= t.row0[p + 1]) ++p;
+    return p;
+}
+
 // device counters (wcsim_stats)
 struct Counters {
     unsigned long long depos_skipped;
@@ -38,6 +55,21 @@ cudaError_t launch_raster_fixed(GridDims g, DepoArrays d, long long n, uint64_t 
                                 double nsigma, unsigned long long *fix, int *depo_totals, Counters *counters, int sm_count,
                                 cudaStream_t st);
 
+// a1-a3 for the planes of a multi-plane plan in ONE launch (atomic or fixed-point sink): plane p's depos are cut into
+// batches batch0[p] .. batch0[p+1]-1, a warp's batch index says which plane (depo arrays, wire count, row offset in the
+// stacked grid) it works on; depo ids and Philox bins are the plane's own, as if each plane were rastered by its own plan
+struct RasterPlanes {
+    int n;
+    DepoArrays d[kMaxPlanes];
+    long long count[kMaxPlanes];
+    long long batch0[kMaxPlanes + 1];
+    int n_wires[kMaxPlanes];
+    int row0[kMaxPlanes];
+};
+int raster_batch_depos(); // depos per batch (for batch0)
+cudaError_t launch_raster_planes(int n_ticks, const RasterPlanes &planes, uint64_t seed, int fluctuate, double nsigma,
+                                 void *grid, bool fixed, Counters *counters, int sm_count, cudaStream_t st);
+
 // a1-a3, tiled mode (deterministic): scratch buffers are owned by the plan and grown by the caller
 struct TileScratch {
     int tile_w, tile_t;           // tile shape in bins
@@ -46,7 +78,8 @@ struct TileScratch {
     unsigned int *tile_cursor;    // [n_tiles] fill cursors
     unsigned int *entries;        // [capacity] depo indices grouped by tile
     unsigned long long capacity;  // entries allocated
-    unsigned int *total;          // [1] total number of (depo, tile) pairs
+    unsigned long long *total;    // [1] total number of (depo, tile) pairs, summed in 64 bits by tile_count (the per-tile
+                                  // offsets are 32-bit: the caller rejects totals >= 2^32)
     unsigned int slice_entries;   // listed depos per slice of a hot tile (set per call from the mean tile load)
     unsigned long long *fix;      // [n_wires * n_ticks] 2^-24 fixed-point grid the tile CTAs add into; zero between calls
 };
@@ -77,6 +110,8 @@ struct ConvBuffers {
     const float2 *tw_col; // per-pass twiddle tables of a pad_w-point FFT
     int spec_stride;      // pad_t/2 + 8
     int sm_count;         // SMs of the plan's device (grid size of the persistent row kernels)
+    PlaneTable planes;    // GridDims::n_wires of the convolution launchers is the stacked row count planes.row0[planes.n];
+                          // Rt holds planes.n blocks of rt_rows rows, plane p's response at Rt + p rt_rows spec_stride
 };
 struct NoiseArgs {
     const float *amp; // DEVICE [pad_t/2 + 1], already scaled by pad_t^-1/2; NULL = no noise
@@ -88,6 +123,7 @@ cudaError_t launch_rows_forward(GridDims g, int pad_t, ConvBuffers b, cudaStream
 cudaError_t launch_cols(GridDims g, int pad_w, int pad_t, ConvBuffers b, cudaStream_t st);
 int wires_chunk(); // response offsets per register chunk of the direct wire-axis kernel
 void wires_halo(int n_rw, int *below, int *above); // zero rows of `spec` that kernel reads outside [0, n_wires)
+int wires_rows_per_group();                        // output wires per CTA of that kernel (PlaneTable::grp0)
 cudaError_t launch_wires(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st);
 // M = (accumulate ? M : 0) + c2r(use_spec ? spec : 0  +  noise)
 cudaError_t launch_rows_inverse(GridDims g, int pad_t, ConvBuffers b, NoiseArgs noise, bool use_spec, bool accumulate,

@@ -32,6 +32,7 @@
 #include "pdl.cuh"
 #include "rng.cuh"
 #include <type_traits>
+#include <mutex>
 #include <cstdio>
 #include <cstdlib>
 
@@ -118,6 +119,7 @@ struct GlobalSink {
         atomicAdd(S + idx, v); // result unused -> RED.E.ADD.F32
     }
     __device__ __forceinline__ void add(int wire, int tick, float v) const { add_at(index(wire, tick), v); }
+    __device__ __forceinline__ GlobalSink shifted(int rows) const { return GlobalSink{S + (size_t)rows * n_ticks, n_ticks}; }
 };
 
 // the same adds in 2^-24 fixed point into a 64-bit grid (RED.ADD.64: order independent); tile_finalize_kernel folds it into S
@@ -133,6 +135,7 @@ struct FixSink {
         atomicAdd(fix + idx, (unsigned long long)__double2ll_rn((double)v * kFixScale));
     }
     __device__ __forceinline__ void add(int wire, int tick, float v) const { add_at(index(wire, tick), v); }
+    __device__ __forceinline__ FixSink shifted(int rows) const { return FixSink{fix + (size_t)rows * n_ticks, n_ticks}; }
 };
 
 template <bool FIX>
@@ -161,11 +164,14 @@ struct TileSink {
         if (h) atomicAdd(a + 1, h);
     }
     __device__ __forceinline__ void add(int wire, int tick, float v) const { add_at(index(wire, tick), v); }
+    __device__ __forceinline__ TileSink shifted(int) const { return *this; } // tiles belong to one plane
 };
 
-// the clip window of a batch: the grid, or one tile of it
+// the clip window of a batch: the plane, or one tile of it.  row_off: the plane's first row in a stacked multi-plane grid
+// (wire indices, Philox bins and the window are the plane's own; only the sink index carries the offset)
 struct Clip {
     int w_lo, w_hi, k_lo, k_hi;
+    int row_off = 0;
 };
 
 // Rasters depo (t0, x0, st, sx, q) into the clip window [w_lo, w_hi) x [k_lo, k_hi) (already inside the grid).
@@ -586,7 +592,8 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
         drawn += raster_depo<true>(__shfl_sync(0xffffffffu, t0, src), __shfl_sync(0xffffffffu, x0, src),
                                    __shfl_sync(0xffffffffu, st, src), __shfl_sync(0xffffffffu, sx, src),
                                    __shfl_sync(0xffffffffu, q, src), id_base + (uint64_t)dio, seed, nsigma, g.n_ticks,
-                                   clip.w_lo, clip.w_hi, clip.k_lo, clip.k_hi, sink, lane, &tot, normal_only, inv_norm);
+                                   clip.w_lo, clip.w_hi, clip.k_lo, clip.k_hi, sink.shifted(clip.row_off), lane, &tot,
+                                   normal_only, inv_norm);
         if (totals != nullptr) {
             tot = warp_sum(tot);
             if (lane == 0 && tot != 0) atomicAdd(totals + dio, tot);
@@ -652,7 +659,7 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
             const double inv_n = normalize ? sc.inv_norm[own] : 1.0;
             const uint32_t dio = (uint32_t)dbase + __float_as_uint(bq.w); // index of the depo in the call (< 2^32: totals)
             const uint4 words = fluct_words(seed, id_base + (uint64_t)(dbase + (long long)__float_as_uint(bq.w)), (uint64_t)gq);
-            const uint32_t idx0 = sink.index(wire, a.x) + (uint32_t)ii0; // sink index of the quad's first bin (mod 2^32)
+            const uint32_t idx0 = sink.index(wire + clip.row_off, a.x) + (uint32_t)ii0; // sink index of the quad's first bin (mod 2^32)
             const uint32_t neg = a.z < 0 ? kBinNegative : 0u;
             const bool live_q = act && Nf > 0.0f; // N = 0 draws nothing
             uint32_t w0 = words.x, w1 = words.y, w2 = words.z, w3 = words.w;
@@ -806,6 +813,73 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8
 }
 
 // ------------------------------------------------------------------------------------------------------------------
+// The planes of a multi-plane plan in ONE launch (one plane-event does not fill the
+// device).  The batch list is the concatenation of the planes' batch lists; a warp looks its batch's plane up (uniform
+// over the warp) and runs the same batch body with that plane's depo arrays, wire count and row offset in the stacked
+// grid.  Depo ids and Philox bins are the plane's own, so the result equals the planes rastered one by one.
+// ------------------------------------------------------------------------------------------------------------------
+template <int FLUCT, bool FIX>
+__global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8)
+    raster_planes_kernel(int n_ticks, const __grid_constant__ RasterPlanes P, uint64_t seed, double nsigma,
+                         float *__restrict__ S, Counters *counters, bool normalize, int n_static)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    BatchSmem<FLUCT != 0, false> &sm = *reinterpret_cast<BatchSmem<FLUCT != 0, false> *>(smem_raw);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    using Sink = typename std::conditional<FIX, FixSink, GlobalSink>::type;
+    const Sink sink = make_grid_sink<FIX>(S, n_ticks);
+    const long long n_warps_grid = (long long)gridDim.x * kBatchWarps;
+    const long long n_batches = P.batch0[P.n];
+    unsigned int drawn = 0, skipped = 0; // per lane
+    QuadCounts qc;
+    pdl_trigger();
+    pdl_wait();
+    long long batch = (long long)blockIdx.x * kBatchWarps + wid;
+    int round = 0;
+    for (;;) {
+        const bool more = batch < n_batches;
+        int pl = 0;
+        if (more)
+            while (pl + 1 < P.n && batch >= P.batch0[pl + 1]) ++pl;
+        const long long first = more ? (batch - P.batch0[pl]) << kBatchShift : 0;
+        const long long i = first + lane;
+        float t0 = 0.f, x0 = 0.f, st = 0.f, sx = 0.f, q = 0.f;
+        bool valid = false;
+        if (more && lane < kBatchDepos && i < P.count[pl]) {
+            const DepoArrays &d = P.d[pl];
+            t0 = d.t0[i], x0 = d.x0[i], st = d.sigma_t[i], sx = d.sigma_x[i], q = d.q[i]; // plain loads: pdl.cuh
+            valid = depo_valid(t0, x0, st, sx, q);
+            skipped += !valid;
+        }
+        const GridDims g{P.n_wires[pl], n_ticks};
+        const Clip clip{0, g.n_wires, 0, n_ticks, P.row0[pl]};
+        if constexpr (FLUCT)
+            raster_quad_body<FLUCT == 2, false, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, 0ull, seed, nsigma,
+                                                       normalize, nullptr, sm.warp[wid], qc, !more, drawn, lane);
+        else if (more)
+            raster_flat_body(g, clip, sink.shifted(clip.row_off), t0, x0, st, sx, q, valid, nsigma, normalize,
+                             sm.scratch[wid], drawn, lane);
+        if (!more) break;
+        if (++round < n_static) {
+            batch += n_warps_grid;
+        } else {
+            if (lane == 0) batch = n_static * n_warps_grid + (long long)atomicAdd(&counters->next_batch, 1ull);
+            batch = __shfl_sync(0xffffffffu, batch, 0);
+        }
+    }
+    const unsigned long long drawn_w = warp_sum((unsigned long long)drawn), skipped_w = warp_sum((unsigned long long)skipped);
+    if (lane == 0) {
+        if (drawn_w) atomicAdd(&counters->bins_drawn, drawn_w);
+        if (skipped_w) atomicAdd(&counters->depos_skipped, skipped_w);
+        const unsigned long long n_warps = (unsigned long long)gridDim.x * kBatchWarps;
+        if (atomicAdd(&counters->warps_done, 1ull) == n_warps - 1) { // the last warp re-arms the batch counter
+            counters->next_batch = 0ull;
+            counters->warps_done = 0ull;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
 // tiled mode
 // ------------------------------------------------------------------------------------------------------------------
 struct TileRange {
@@ -831,10 +905,15 @@ __device__ __forceinline__ TileRange depo_tiles(GridDims g, DepoArrays d, long l
 __global__ void tile_count_kernel(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const TileRange r = depo_tiles(g, d, i, nsigma);
-    for (int tw = r.w0; tw <= r.w1; ++tw)
-        for (int tt = r.t0; tt <= r.t1; ++tt) atomicAdd(ts.tile_count + (size_t)tw * ts.tiles_t + tt, 1u);
+    unsigned long long pairs = 0;
+    if (i < n) {
+        const TileRange r = depo_tiles(g, d, i, nsigma);
+        for (int tw = r.w0; tw <= r.w1; ++tw)
+            for (int tt = r.t0; tt <= r.t1; ++tt) atomicAdd(ts.tile_count + (size_t)tw * ts.tiles_t + tt, 1u);
+        if (r.w0 <= r.w1 && r.t0 <= r.t1) pairs = (unsigned long long)(r.w1 - r.w0 + 1) * (unsigned long long)(r.t1 - r.t0 + 1);
+    }
+    pairs = warp_sum(pairs); // blockDim.x is a multiple of 32: whole warps reach this point
+    if ((threadIdx.x & 31) == 0 && pairs) atomicAdd(ts.total, pairs);
 }
 
 // exclusive scan of tile_count[0..n_tiles) in place, tile_count[n_tiles] = total, cursors = offsets; one CTA
@@ -876,10 +955,7 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(TileScratch ts)
         if (threadIdx.x == 0) carry += warp_tot[31];
         __syncthreads();
     }
-    if (threadIdx.x == 0) {
-        ts.tile_count[n_tiles] = carry;
-        *ts.total = carry;
-    }
+    if (threadIdx.x == 0) ts.tile_count[n_tiles] = carry;
 }
 
 __global__ void tile_fill_kernel(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts)
@@ -992,24 +1068,34 @@ __global__ void count_invalid_kernel(DepoArrays d, long long n, Counters *counte
 
 } // namespace
 
-void erf_table_host(const double *z, double *out, long long n)
+static const double *erf_table_once()
 {
     static double tab[(kErfDegree + 1) * kErfIntervals];
-    static bool built = false;
-    if (!built) {
-        build_erf_table(tab);
-        built = true;
-    }
+    static std::once_flag once;
+    std::call_once(once, [] { build_erf_table(tab); });
+    return tab;
+}
+
+void erf_table_host(const double *z, double *out, long long n)
+{
+    const double *tab = erf_table_once();
     for (long long i = 0; i < n; ++i) out[i] = erf_from_table(tab, z[i]);
 }
 
+// Once per device (under a mutex): later plans must not rewrite the table while other plans' kernels read it.
 cudaError_t raster_configure(cudaStream_t st)
 {
-    double tab[(kErfDegree + 1) * kErfIntervals];
-    build_erf_table(tab);
-    cudaError_t err = cudaMemcpyToSymbolAsync(g_erf_tab, tab, sizeof(tab), 0, cudaMemcpyHostToDevice, st);
+    static std::mutex mu;
+    static bool done[64] = {};
+    int dev = 0;
+    cudaError_t err = cudaGetDevice(&dev);
     if (err != cudaSuccess) return err;
-    err = cudaStreamSynchronize(st); // `tab` is on this stack
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;
+    err = cudaMemcpyToSymbolAsync(g_erf_tab, erf_table_once(), sizeof(double) * (kErfDegree + 1) * kErfIntervals, 0,
+                                  cudaMemcpyHostToDevice, st);
+    if (err != cudaSuccess) return err;
+    err = cudaStreamSynchronize(st);
     if (err != cudaSuccess) return err;
 #define WCSIM_RASTER_SMEM(F, T, X)                                                                                     \
     err = cudaFuncSetAttribute(raster_batch_kernel<F, T, X>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
@@ -1026,6 +1112,17 @@ cudaError_t raster_configure(cudaStream_t st)
     WCSIM_RASTER_SMEM(2, false, true)
     WCSIM_RASTER_SMEM(0, false, true)
 #undef WCSIM_RASTER_SMEM
+#define WCSIM_PLANES_SMEM(F, X)                                                                                        \
+    err = cudaFuncSetAttribute(raster_planes_kernel<F, X>, cudaFuncAttributeMaxDynamicSharedMemorySize,                \
+                               (int)sizeof(BatchSmem<F != 0, false>));                                                 \
+    if (err != cudaSuccess) return err;
+    WCSIM_PLANES_SMEM(0, false)
+    WCSIM_PLANES_SMEM(1, false)
+    WCSIM_PLANES_SMEM(2, false)
+    WCSIM_PLANES_SMEM(0, true)
+    WCSIM_PLANES_SMEM(1, true)
+    WCSIM_PLANES_SMEM(2, true)
+#undef WCSIM_PLANES_SMEM
 #define WCSIM_TILE_SMEM(F, T)                                                                                          \
     err = cudaFuncSetAttribute(tile_accumulate_kernel<F, T>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
                                (int)sizeof(TileSmem<F != 0, T>));                                                      \
@@ -1036,6 +1133,7 @@ cudaError_t raster_configure(cudaStream_t st)
     WCSIM_TILE_SMEM(2, false)
     WCSIM_TILE_SMEM(0, false)
 #undef WCSIM_TILE_SMEM
+    if (dev >= 0 && dev < 64) done[dev] = true;
     return cudaSuccess;
 }
 
@@ -1044,15 +1142,24 @@ static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, ui
                                        float *S, int *depo_totals, Counters *counters, int sm_count, cudaStream_t st,
                                        bool normalize)
 {
-    const long long n_batches = (n + kBatchDepos - 1) / kBatchDepos;
     const size_t smem = sizeof(BatchSmem<FLUCT != 0, TOT>);
     const int fit = (int)((227u * 1024u) / (smem + 1024u)); // 227 KB per SM, 1 KB reserved per CTA
     const int cap = FLUCT ? WCSIM_FLUCT_CTAS : 8; // the kernel's __launch_bounds__
     const int ctas_per_sm = fit > cap ? cap : fit;
-    long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
     const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
-    if (ctas > max_ctas) ctas = max_ctas;
     int3 sched = make_int3(kTailDepos, kTailPerWarp, 2);
+    // A small call (fewer depos than kBatchDepos per resident warp) is latency bound: a warp works its batch off serially,
+    // so the depos are spread over as many warps as there are, in batches of `per` < kBatchDepos depos each (the kernel's
+    // "tail" batches, here for every depo).  configs[0]: 100 depos -> 100 one-depo batches instead of 7 batches of 16.
+    long long n_batches = (n + kBatchDepos - 1) / kBatchDepos;
+    const long long warp_slots = max_ctas * kBatchWarps;
+    const long long per = (n + warp_slots - 1) / warp_slots;
+    if (per < kBatchDepos) {
+        sched = make_int3((int)(per > 0 ? per : 1), 1 << 24, 1); // every depo in a `per`-depo batch
+        n_batches = (n + sched.x - 1) / sched.x;
+    }
+    long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
+    if (ctas > max_ctas) ctas = max_ctas;
     int max_per_sm = 0;
     if (const char *e = getenv("WCSIM_SCHED")) sscanf(e, "%d,%d,%d,%d", &sched.x, &sched.y, &sched.z, &max_per_sm);
     if (max_per_sm > 0 && ctas > (long long)sm_count * max_per_sm) ctas = (long long)sm_count * max_per_sm;
@@ -1090,6 +1197,39 @@ cudaError_t launch_raster_fixed(GridDims g, DepoArrays d, long long n, uint64_t 
 {
     return launch_raster_grid<true>(g, d, n, id_base, seed, fluctuate, nsigma, reinterpret_cast<float *>(fix), depo_totals,
                                     counters, sm_count, st);
+}
+
+int raster_batch_depos() { return kBatchDepos; }
+
+template <int FLUCT, bool FIX>
+static cudaError_t launch_raster_planes_t(int n_ticks, const RasterPlanes &planes, uint64_t seed, double nsigma, float *grid,
+                                          Counters *counters, int sm_count, cudaStream_t st, bool normalize)
+{
+    const long long n_batches = planes.batch0[planes.n];
+    if (n_batches <= 0) return cudaSuccess;
+    const size_t smem = sizeof(BatchSmem<FLUCT != 0, false>);
+    const int fit = (int)((227u * 1024u) / (smem + 1024u));
+    const int cap = FLUCT ? WCSIM_FLUCT_CTAS : 8;
+    const int ctas_per_sm = fit > cap ? cap : fit;
+    long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
+    const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
+    if (ctas > max_ctas) ctas = max_ctas;
+    return launch_pdl(raster_planes_kernel<FLUCT, FIX>, (unsigned)ctas, kBatchWarps * 32, smem, st, n_ticks, planes, seed, nsigma,
+                      grid, counters, normalize, 2);
+}
+
+cudaError_t launch_raster_planes(int n_ticks, const RasterPlanes &planes, uint64_t seed, int fluctuate, double nsigma,
+                                 void *grid, bool fixed, Counters *counters, int sm_count, cudaStream_t st)
+{
+    const bool normalize = (fluctuate & kRasterNormalize) != 0;
+    fluctuate &= ~kRasterNormalize;
+    float *gp = reinterpret_cast<float *>(grid);
+#define WCSIM_PLANES(F) (fixed ? launch_raster_planes_t<F, true>(n_ticks, planes, seed, nsigma, gp, counters, sm_count, st, normalize) \
+                               : launch_raster_planes_t<F, false>(n_ticks, planes, seed, nsigma, gp, counters, sm_count, st, normalize))
+    if (!fluctuate) return WCSIM_PLANES(0);
+    if (fluctuate == 2) return WCSIM_PLANES(2);
+    return WCSIM_PLANES(1);
+#undef WCSIM_PLANES
 }
 
 cudaError_t launch_tile_count(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts, cudaStream_t st)

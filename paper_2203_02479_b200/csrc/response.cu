@@ -143,7 +143,7 @@ cudaError_t build_response_spectrum(const float *dev_R, int n_rw, int n_rt, int 
     dim3 g1((pad_t / 2 + 1 + threads - 1) / threads, n_rw);
     response_ticks_kernel<<<g1, threads, 0, st>>>(dev_R, n_rw, n_rt, pad_t, dev_tmp);
     cudaError_t err = cudaGetLastError();
-    if (err != cudaSuccess) return err;
+    if (err != cudaSuccess || dev_Rhat == nullptr) return err; // no Rhat: only the tick-axis spectra are wanted
     dim3 g2((spec_stride + threads - 1) / threads, pad_w);
     response_wires_kernel<<<g2, threads, 0, st>>>(dev_tmp, n_rw, pad_w, pad_t, spec_stride, dev_Rhat);
     return cudaGetLastError();

@@ -25,14 +25,20 @@ struct wcsim_plan {
     int rt_rows = 0;
     int wire_mode = WCSIM_WIRES_AUTO;
     bool normalize = false; // renormalised patches (reading A24)
+    bool multi = false;     // created by wcsim_plan_create_planes
+    bool capturing = false; // between wcsim_graph_begin and wcsim_graph_end
+    unsigned long long captured_launches = 0;
+    short *dev_adc = nullptr; // ADC codes of wcsim_simulate_host_adc_async (allocated on first use)
+    PlaneTable pt{};        // n = 1 for an ordinary plan
     Counters *counters = nullptr;
     float *amp_builtin = nullptr, *amp_custom = nullptr; // device, pad_t/2+1, scaled by pad_t^-1/2
+    float *amp_armed = nullptr; // the armed custom spectrum's own copy (a later wcsim_add_noise must not change it)
     bool noise_armed = false;
     const float *armed_amp = nullptr;
     uint64_t armed_seed = 0;
     TileScratch ts{};
-    unsigned int *host_total = nullptr; // pinned
-    float *stage[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    unsigned long long *host_total = nullptr; // pinned
+    float *stage_block = nullptr; // device staging of the five host depo arrays, 5 * stage_cap floats
     long long stage_cap = 0;
     // profiling: CUDA events recorded around each stage on the plan's stream while enabled
     struct Span {
@@ -119,7 +125,7 @@ struct StageSpan {
     int stage;
     StageSpan(wcsim_plan *plan, int st, bool enabled = true) : p(plan), stage(st)
     {
-        if (!p->profiling || !enabled) return;
+        if (!p->profiling || !enabled || p->capturing) return;
         if (p->pending.size() >= 8192) harvest_spans(p);
         beg = take_event(p);
         end = take_event(p);
@@ -168,6 +174,7 @@ ConvBuffers conv_buffers(const wcsim_plan *p)
     b.tw_col = p->tw_col;
     b.spec_stride = p->spec_stride;
     b.sm_count = p->sm_count;
+    b.planes = p->pt;
     return b;
 }
 
@@ -215,13 +222,11 @@ int ensure_stage(wcsim_plan *p, long long n)
 {
     if (n <= p->stage_cap) return WCSIM_OK;
     CU_TRY(cudaStreamSynchronize(p->stream));
-    for (float *&s : p->stage) {
-        if (s) cudaFree(s);
-        s = nullptr;
-    }
+    if (p->stage_block) cudaFree(p->stage_block);
+    p->stage_block = nullptr;
     p->stage_cap = 0;
     const long long cap = n + n / 4 + 1024;
-    for (float *&s : p->stage) CU_TRY(cudaMalloc((void **)&s, sizeof(float) * (size_t)cap));
+    CU_TRY(cudaMalloc((void **)&p->stage_block, sizeof(float) * 5 * (size_t)cap));
     p->stage_cap = cap;
     return WCSIM_OK;
 }
@@ -233,11 +238,13 @@ int raster_tiled(wcsim_plan *p, GridDims g, DepoArrays d, long long n, uint64_t 
     const int n_tiles = ts.tiles_w * ts.tiles_t;
     if (n > 0xFFFFFFFFll) return WCSIM_EINVAL; // entries hold 32-bit depo indices
     CU_TRY(cudaMemsetAsync(ts.tile_count, 0, sizeof(unsigned int) * (size_t)(n_tiles + 1), p->stream));
+    CU_TRY(cudaMemsetAsync(ts.total, 0, sizeof(unsigned long long), p->stream));
     CU_TRY(launch_tile_count(g, d, n, p->nsigma, ts, p->stream));
     CU_TRY(launch_tile_scan(ts, p->stream));
-    CU_TRY(cudaMemcpyAsync(p->host_total, ts.total, sizeof(unsigned int), cudaMemcpyDeviceToHost, p->stream));
+    CU_TRY(cudaMemcpyAsync(p->host_total, ts.total, sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
     CU_TRY(cudaStreamSynchronize(p->stream));
     const unsigned long long need = *p->host_total;
+    if (need > 0xFFFFFFFFull) return WCSIM_EINVAL; // the per-tile offsets are 32-bit: raster fewer depos per call
     if (need > ts.capacity) {
         if (ts.entries) cudaFree(ts.entries);
         ts.entries = nullptr;
@@ -270,8 +277,8 @@ int destroy_impl(wcsim_plan *p)
     void *bufs[] = {p->spec2,    p->Rt,
                     p->S,        p->M,           p->spec_alloc,  p->Rhat,           p->tw_row,        p->tw_real,
                     p->tw_col,   p->counters,    p->amp_builtin, p->amp_custom,     p->ts.tile_count, p->ts.tile_cursor,
-                    p->ts.entries, p->ts.total, p->ts.fix,  p->stage[0],    p->stage[1],       p->stage[2],      p->stage[3],
-                    p->stage[4]};
+                    p->amp_armed, p->dev_adc,
+                    p->ts.entries, p->ts.total, p->ts.fix,  p->stage_block};
     for (void *b : bufs)
         if (b) cudaFree(b);
     if (p->host_total) cudaFreeHost(p->host_total);
@@ -286,28 +293,40 @@ int destroy_impl(wcsim_plan *p)
 
 } // namespace
 
-extern "C" {
+namespace {
 
-int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *response, int n_rwires, int n_rticks,
-                      wcsim_pad pad, float nsigma, int scatter_mode, void *cuda_stream)
+// plan creation for 1..kMaxPlanes planes stacked along the wire axis (same n_ticks, padding and response footprint).
+// `multi`: created by wcsim_plan_create_planes (direct wire pass only, no Rhat)
+int create_impl(wcsim_plan **out, int n_planes, const int *plane_wires, int n_ticks, const float *const *responses,
+                int n_rwires, int n_rticks, wcsim_pad pad, float nsigma, int scatter_mode, void *cuda_stream, bool multi)
 {
     if (!out) return WCSIM_EINVAL;
     *out = nullptr;
-    if (!response || n_wires <= 0 || n_ticks <= 0 || n_rwires <= 0 || n_rticks <= 0 || (n_rwires % 2) == 0)
+    if (!plane_wires || !responses || n_planes < 1 || n_planes > kMaxPlanes || n_ticks <= 0 || n_rwires <= 0 ||
+        n_rticks <= 0 || (n_rwires % 2) == 0)
         return WCSIM_EINVAL;
+    long long total_wires = 0;
+    int max_wires = 0;
+    for (int p = 0; p < n_planes; ++p) {
+        if (plane_wires[p] <= 0 || !responses[p]) return WCSIM_EINVAL;
+        total_wires += plane_wires[p];
+        max_wires = plane_wires[p] > max_wires ? plane_wires[p] : max_wires;
+    }
     if (!(nsigma > 0.0f) || !std::isfinite(nsigma)) return WCSIM_EINVAL;
     if (scatter_mode < WCSIM_SCATTER_ATOMIC || scatter_mode > WCSIM_SCATTER_FIXED) return WCSIM_EINVAL;
+    if (multi && scatter_mode == WCSIM_SCATTER_TILED) return WCSIM_EINVAL; // tiles belong to one plane
     if (pad.wires < 0 || pad.ticks < 0) return WCSIM_EINVAL;
     const int c = (n_rwires - 1) / 2;
-    const long long need_t = (long long)n_ticks + n_rticks - 1, need_w = (long long)n_wires + c;
+    const long long need_t = (long long)n_ticks + n_rticks - 1, need_w = (long long)max_wires + c;
     const int pad_t = pad.ticks ? pad.ticks : next_pow2(need_t, 32);
     // automatic wire padding also keeps the wrapped response from overlapping itself (pad_w >= n_rwires)
-    const int pad_w = pad.wires ? pad.wires : next_pow2(need_w > n_rwires ? need_w : (long long)n_rwires, 16);
+    const int pad_w = (pad.wires && !multi) ? pad.wires : next_pow2(need_w > n_rwires ? need_w : (long long)n_rwires, 16);
     if (!is_pow2(pad_t) || !is_pow2(pad_w) || pad_t < need_t || pad_w < need_w || pad_t < 32 || pad_w < 16)
         return WCSIM_EINVAL;
     if (pad_w < n_rwires) return WCSIM_EINVAL; // the wrapped response must not overlap itself
     if (!conv_sizes_supported(pad_w, pad_t)) return WCSIM_EINVAL;
-    if ((long long)n_wires * n_ticks >= (1ll << 30)) return WCSIM_EINVAL; // bin index + 2 flag bits in 32 (draw queues)
+    if (total_wires * n_ticks >= (1ll << 30)) return WCSIM_EINVAL; // bin index + 2 flag bits in 32 (draw queues)
+    const int n_wires = (int)total_wires;
 
     int dev = 0;
     CU_TRY(cudaGetDevice(&dev));
@@ -324,6 +343,26 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
     p->scatter_mode = scatter_mode;
     p->stream = (cudaStream_t)cuda_stream;
     p->device = dev;
+    p->multi = multi;
+    if (multi) p->wire_mode = WCSIM_WIRES_DIRECT;
+
+    // the plane table: stacked rows, halo rows of the row spectra between the planes, row groups of the wire pass
+    int halo_lo = 0, halo_hi = 0;
+    wires_halo(n_rwires, &halo_lo, &halo_hi);
+    const int per_group = wires_rows_per_group();
+    PlaneTable &pt = p->pt;
+    pt.n = n_planes;
+    int row = 0, srow = 0, grp = 0;
+    for (int q = 0; q < n_planes; ++q) {
+        pt.row0[q] = row;
+        pt.srow0[q] = srow + q * (halo_lo + halo_hi); // relative to `spec`, which starts after the first low halo
+        pt.grp0[q] = grp;
+        row += plane_wires[q];
+        srow += plane_wires[q];
+        grp += (plane_wires[q] + per_group - 1) / per_group;
+    }
+    for (int q = n_planes; q <= kMaxPlanes; ++q) pt.row0[q] = row, pt.grp0[q] = grp;
+    for (int q = n_planes; q < kMaxPlanes; ++q) pt.srow0[q] = 0;
 
     float *dev_R = nullptr;
     double2 *dev_tmp = nullptr;
@@ -332,18 +371,17 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
         const size_t grid = (size_t)n_wires * n_ticks;
         CU_TRY(cudaMalloc((void **)&p->S, sizeof(float) * grid));
         CU_TRY(cudaMalloc((void **)&p->M, sizeof(float) * grid));
-        int halo_lo = 0, halo_hi = 0;
-        wires_halo(n_rwires, &halo_lo, &halo_hi);
-        const size_t spec_rows = (size_t)halo_lo + n_wires + halo_hi;
+        const size_t spec_rows = (size_t)n_wires + (size_t)n_planes * (halo_lo + halo_hi);
         CU_TRY(cudaMalloc((void **)&p->spec_alloc, sizeof(float2) * spec_rows * p->spec_stride));
         p->spec = p->spec_alloc + (size_t)halo_lo * p->spec_stride;
         CU_TRY(cudaMalloc((void **)&p->spec2, sizeof(float2) * (size_t)n_wires * p->spec_stride));
-        CU_TRY(cudaMalloc((void **)&p->Rhat, sizeof(float2) * (size_t)pad_w * p->spec_stride));
+        if (!multi) CU_TRY(cudaMalloc((void **)&p->Rhat, sizeof(float2) * (size_t)pad_w * p->spec_stride));
         p->rt_rows = (n_rwires + wires_chunk() - 1) / wires_chunk() * wires_chunk();
-        CU_TRY(cudaMalloc((void **)&p->Rt, sizeof(float2) * (size_t)p->rt_rows * p->spec_stride));
+        CU_TRY(cudaMalloc((void **)&p->Rt, sizeof(float2) * (size_t)n_planes * p->rt_rows * p->spec_stride));
         CU_TRY(cudaMalloc((void **)&p->counters, sizeof(Counters)));
         CU_TRY(cudaMalloc((void **)&p->amp_builtin, sizeof(float) * (size_t)(pad_t / 2 + 1)));
         CU_TRY(cudaMalloc((void **)&p->amp_custom, sizeof(float) * (size_t)(pad_t / 2 + 1)));
+        CU_TRY(cudaMalloc((void **)&p->amp_armed, sizeof(float) * (size_t)(pad_t / 2 + 1)));
         CU_TRY(cudaMemsetAsync(p->S, 0, sizeof(float) * grid, p->stream));
         CU_TRY(cudaMemsetAsync(p->M, 0, sizeof(float) * grid, p->stream));
         CU_TRY(cudaMemsetAsync(p->spec_alloc, 0, sizeof(float2) * spec_rows * p->spec_stride, p->stream));
@@ -364,16 +402,20 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
         const size_t n_tiles = (size_t)p->ts.tiles_w * p->ts.tiles_t;
         CU_TRY(cudaMalloc((void **)&p->ts.tile_count, sizeof(unsigned int) * (n_tiles + 1)));
         CU_TRY(cudaMalloc((void **)&p->ts.tile_cursor, sizeof(unsigned int) * n_tiles));
-        CU_TRY(cudaMalloc((void **)&p->ts.total, sizeof(unsigned int)));
-        CU_TRY(cudaMallocHost((void **)&p->host_total, sizeof(unsigned int)));
-        // response spectrum
+        CU_TRY(cudaMalloc((void **)&p->ts.total, sizeof(unsigned long long)));
+        CU_TRY(cudaMallocHost((void **)&p->host_total, sizeof(unsigned long long)));
+        // response spectra: Rt of every plane (direct wire pass), Rhat of a single-plane plan (FFT wire pass)
         const size_t nr = (size_t)n_rwires * n_rticks;
         CU_TRY(cudaMalloc((void **)&dev_R, sizeof(float) * nr));
         CU_TRY(cudaMalloc((void **)&dev_tmp, sizeof(double2) * (size_t)n_rwires * (pad_t / 2 + 1)));
-        CU_TRY(cudaMemcpyAsync(dev_R, response, sizeof(float) * nr, cudaMemcpyHostToDevice, p->stream));
-        CU_TRY(build_response_spectrum(dev_R, n_rwires, n_rticks, pad_w, pad_t, p->spec_stride, dev_tmp, p->Rhat,
-                                       p->stream));
-        CU_TRY(build_response_rows(dev_tmp, n_rwires, p->rt_rows, pad_t, p->spec_stride, p->Rt, p->stream));
+        for (int q = 0; q < n_planes; ++q) {
+            CU_TRY(cudaMemcpyAsync(dev_R, responses[q], sizeof(float) * nr, cudaMemcpyHostToDevice, p->stream));
+            CU_TRY(build_response_spectrum(dev_R, n_rwires, n_rticks, pad_w, pad_t, p->spec_stride, dev_tmp, p->Rhat,
+                                           p->stream));
+            CU_TRY(build_response_rows(dev_tmp, n_rwires, p->rt_rows, pad_t, p->spec_stride,
+                                       p->Rt + (size_t)q * p->rt_rows * p->spec_stride, p->stream));
+            CU_TRY(cudaStreamSynchronize(p->stream)); // responses[q] may be pageable; dev_R is reused
+        }
         CU_TRY(conv_configure(pad_w, pad_t));
         CU_TRY(raster_configure(p->stream));
         CU_TRY(cudaStreamSynchronize(p->stream));
@@ -391,10 +433,35 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
     return WCSIM_OK;
 }
 
+} // namespace
+
+extern "C" {
+
+int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *response, int n_rwires, int n_rticks,
+                      wcsim_pad pad, float nsigma, int scatter_mode, void *cuda_stream)
+{
+    if (out) *out = nullptr;
+    return create_impl(out, 1, &n_wires, n_ticks, &response, n_rwires, n_rticks, pad, nsigma, scatter_mode, cuda_stream,
+                       false);
+}
+
+int wcsim_plan_create_planes(wcsim_plan **out, int n_planes, const int *n_wires, int n_ticks,
+                             const float *const *responses, int n_rwires, int n_rticks, int pad_ticks, float nsigma,
+                             int scatter_mode, void *cuda_stream)
+{
+    if (out) *out = nullptr;
+    wcsim_pad pad;
+    pad.wires = 0;
+    pad.ticks = pad_ticks;
+    return create_impl(out, n_planes, n_wires, n_ticks, responses, n_rwires, n_rticks, pad, nsigma, scatter_mode,
+                       cuda_stream, true);
+}
+
 int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n, unsigned long long depo_id_base,
                          unsigned long long seed, int fluctuate, int *dev_depo_totals)
 {
     if (!plan || n < 0 || fluctuate < 0 || fluctuate > 2) return WCSIM_EINVAL;
+    if (plan->multi) return WCSIM_ESTATE; // a multi-plane plan is rastered by wcsim_raster_scatter_planes
     if (n == 0) return WCSIM_OK;
     if (!depos || !depos->t0 || !depos->x0 || !depos->sigma_t || !depos->sigma_x || !depos->q) return WCSIM_EINVAL;
     DeviceGuard guard(plan->device);
@@ -404,12 +471,14 @@ int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n
     if (plan->normalize) fluctuate |= kRasterNormalize; // internal.h: flag bit of the launchers' `fluctuate`
     StageSpan span(plan, WCSIM_STAGE_RASTER);
     if (plan->scatter_mode == WCSIM_SCATTER_TILED) {
+        if (plan->capturing) return WCSIM_ESTATE; // the tiled mode reads a size back: it cannot be captured
         plan->launches += 6;
         return raster_tiled(plan, g, d, n, depo_id_base, seed, fluctuate, dev_depo_totals);
     }
     if (dev_depo_totals) CU_TRY(cudaMemsetAsync(dev_depo_totals, 0, sizeof(int) * (size_t)n, plan->stream));
     const bool fixed = plan->scatter_mode == WCSIM_SCATTER_FIXED;
     if (fixed && !plan->ts.fix) { // first use of the fixed-point grid on this plan
+        if (plan->capturing) return WCSIM_ESTATE; // allocate before capturing: run the call once outside the capture
         const size_t bytes = sizeof(unsigned long long) * (size_t)g.n_wires * g.n_ticks;
         CU_TRY(cudaMalloc((void **)&plan->ts.fix, bytes));
         CU_TRY(cudaMemsetAsync(plan->ts.fix, 0, bytes, plan->stream));
@@ -433,6 +502,58 @@ int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n
         plan->launches += 1;
         CU_TRY(launch_tile_finalize(g, plan->ts, plan->S, plan->stream));
     }
+    return WCSIM_OK;
+}
+
+int wcsim_raster_scatter_planes(wcsim_plan *plan, const wcsim_depos *depos, const long long *n, unsigned long long seed,
+                                int fluctuate)
+{
+    if (!plan || !depos || !n || fluctuate < 0 || fluctuate > 2) return WCSIM_EINVAL;
+    if (plan->scatter_mode == WCSIM_SCATTER_TILED) return WCSIM_ESTATE;
+    DeviceGuard guard(plan->device);
+    if (!guard.ok) return fail_cuda(cudaGetLastError());
+    RasterPlanes rp{};
+    rp.n = plan->pt.n;
+    const int per_batch = raster_batch_depos();
+    long long batches = 0;
+    for (int p = 0; p < rp.n; ++p) {
+        if (n[p] < 0) return WCSIM_EINVAL;
+        if (n[p] > 0 && (!depos[p].t0 || !depos[p].x0 || !depos[p].sigma_t || !depos[p].sigma_x || !depos[p].q))
+            return WCSIM_EINVAL;
+        rp.d[p] = DepoArrays{depos[p].t0, depos[p].x0, depos[p].sigma_t, depos[p].sigma_x, depos[p].q};
+        rp.count[p] = n[p];
+        rp.batch0[p] = batches;
+        batches += (n[p] + per_batch - 1) / per_batch;
+        rp.n_wires[p] = plan->pt.row0[p + 1] - plan->pt.row0[p];
+        rp.row0[p] = plan->pt.row0[p];
+    }
+    for (int p = rp.n; p <= kMaxPlanes; ++p) rp.batch0[p] = batches;
+    if (batches == 0) return WCSIM_OK;
+    if (plan->normalize) fluctuate |= kRasterNormalize;
+    StageSpan span(plan, WCSIM_STAGE_RASTER);
+    const bool fixed = plan->scatter_mode == WCSIM_SCATTER_FIXED;
+    if (fixed && !plan->ts.fix) { // first use of the fixed-point grid on this plan
+        if (plan->capturing) return WCSIM_ESTATE;
+        const size_t bytes = sizeof(unsigned long long) * (size_t)plan->n_wires * plan->n_ticks;
+        CU_TRY(cudaMalloc((void **)&plan->ts.fix, bytes));
+        CU_TRY(cudaMemsetAsync(plan->ts.fix, 0, bytes, plan->stream));
+    }
+    plan->launches += 1;
+    CU_TRY(launch_raster_planes(plan->n_ticks, rp, seed, fluctuate, plan->nsigma,
+                                fixed ? (void *)plan->ts.fix : (void *)plan->S, fixed, plan->counters, plan->sm_count,
+                                plan->stream));
+    if (fixed) {
+        plan->launches += 1;
+        CU_TRY(launch_tile_finalize(GridDims{plan->n_wires, plan->n_ticks}, plan->ts, plan->S, plan->stream));
+    }
+    return WCSIM_OK;
+}
+
+int wcsim_get_plane_rows(const wcsim_plan *plan, int plane, int *first_row, int *n_rows)
+{
+    if (!plan || plane < 0 || plane >= plan->pt.n) return WCSIM_EINVAL;
+    if (first_row) *first_row = plan->pt.row0[plane];
+    if (n_rows) *n_rows = plan->pt.row0[plane + 1] - plan->pt.row0[plane];
     return WCSIM_OK;
 }
 
@@ -486,6 +607,7 @@ int wcsim_add_noise(wcsim_plan *plan, const float *amp, unsigned long long seed)
     if (!plan) return WCSIM_EINVAL;
     DeviceGuard guard(plan->device);
     if (!guard.ok) return fail_cuda(cudaGetLastError());
+    if (amp && plan->capturing) return WCSIM_ESTATE; // the upload synchronises
     NoiseArgs nz{nullptr, seed};
     const int rc = noise_amp_ptr(plan, amp, &nz.amp);
     if (rc) return rc;
@@ -501,9 +623,13 @@ int wcsim_arm_noise(wcsim_plan *plan, const float *amp, unsigned long long seed)
     if (!plan) return WCSIM_EINVAL;
     DeviceGuard guard(plan->device);
     if (!guard.ok) return fail_cuda(cudaGetLastError());
-    const float *dev = nullptr;
-    const int rc = noise_amp_ptr(plan, amp, &dev);
-    if (rc) return rc;
+    if (amp && plan->capturing) return WCSIM_ESTATE; // the upload synchronises
+    const float *dev = plan->amp_builtin;
+    if (amp) { // the armed spectrum gets its own device copy: a later wcsim_add_noise(amp') must not change it
+        const int rc = upload_amp(plan, amp, plan->amp_armed);
+        if (rc) return rc;
+        dev = plan->amp_armed;
+    }
     plan->armed_amp = dev;
     plan->armed_seed = seed;
     plan->noise_armed = true;
@@ -558,6 +684,8 @@ int wcsim_set_normalize(wcsim_plan *plan, int on)
 int wcsim_set_wire_mode(wcsim_plan *plan, int wire_mode)
 {
     if (!plan || wire_mode < WCSIM_WIRES_AUTO || wire_mode > WCSIM_WIRES_DIRECT) return WCSIM_EINVAL;
+    if (plan->multi && wire_mode == WCSIM_WIRES_FFT) return WCSIM_ESTATE; // stacked planes: direct wire pass only
+    if (plan->multi) wire_mode = WCSIM_WIRES_DIRECT;
     plan->wire_mode = wire_mode;
     return WCSIM_OK;
 }
@@ -606,22 +734,36 @@ int wcsim_reset_stats(wcsim_plan *plan)
     return WCSIM_OK;
 }
 
-int wcsim_simulate_host_async(wcsim_plan *plan, const float *host_t0, const float *host_x0, const float *host_sigma_t,
-                        const float *host_sigma_x, const float *host_q, long long n, unsigned long long seed,
-                        int fluctuate, int noise, unsigned long long noise_seed, float *host_M)
+namespace {
+
+// copies the depos in, runs the plane-event, copies M (host_M) or its ADC codes (host_adc) out; everything enqueued
+int simulate_host_impl(wcsim_plan *plan, const float *const host[5], long long n, unsigned long long seed, int fluctuate,
+                       int noise, unsigned long long noise_seed, float *host_M, short *host_adc, float gain, float baseline,
+                       int bits)
 {
-    if (!plan || n < 0 || !host_M) return WCSIM_EINVAL;
-    if (n > 0 && (!host_t0 || !host_x0 || !host_sigma_t || !host_sigma_x || !host_q)) return WCSIM_EINVAL;
+    if (!plan || n < 0 || (!host_M && !host_adc) || plan->multi) return plan && plan->multi ? WCSIM_ESTATE : WCSIM_EINVAL;
+    if (n > 0 && (!host[0] || !host[1] || !host[2] || !host[3] || !host[4])) return WCSIM_EINVAL;
+    if (host_adc && (bits < 1 || bits > 15)) return WCSIM_EINVAL;
     DeviceGuard guard(plan->device);
     if (!guard.ok) return fail_cuda(cudaGetLastError());
     int rc = ensure_stage(plan, n);
     if (rc) return rc;
-    const float *src[5] = {host_t0, host_x0, host_sigma_t, host_sigma_x, host_q};
-    for (int a = 0; a < 5 && n > 0; ++a)
-        CU_TRY(cudaMemcpyAsync(plan->stage[a], src[a], sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, plan->stream));
+    const size_t grid = (size_t)plan->n_wires * plan->n_ticks;
+    if (host_adc && !plan->dev_adc) CU_TRY(cudaMalloc((void **)&plan->dev_adc, sizeof(short) * ((grid + 3) / 4 * 4)));
+    float *dev[5];
+    for (int a = 0; a < 5; ++a) dev[a] = plan->stage_block + (size_t)a * (size_t)n;
+    // five arrays that follow one another in host memory (one pinned block) go over in one copy
+    bool contiguous = n > 0;
+    for (int a = 1; a < 5 && contiguous; ++a) contiguous = host[a] == host[a - 1] + n;
+    if (contiguous) {
+        CU_TRY(cudaMemcpyAsync(dev[0], host[0], sizeof(float) * 5 * (size_t)n, cudaMemcpyHostToDevice, plan->stream));
+    } else {
+        for (int a = 0; a < 5 && n > 0; ++a)
+            CU_TRY(cudaMemcpyAsync(dev[a], host[a], sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, plan->stream));
+    }
     rc = wcsim_clear(plan);
     if (rc) return rc;
-    const wcsim_depos d{plan->stage[0], plan->stage[1], plan->stage[2], plan->stage[3], plan->stage[4]};
+    const wcsim_depos d{dev[0], dev[1], dev[2], dev[3], dev[4]};
     rc = wcsim_raster_scatter(plan, &d, n, 0ull, seed, fluctuate, nullptr);
     if (rc) return rc;
     if (noise) {
@@ -630,9 +772,34 @@ int wcsim_simulate_host_async(wcsim_plan *plan, const float *host_t0, const floa
     }
     rc = wcsim_convolve(plan);
     if (rc) return rc;
-    CU_TRY(cudaMemcpyAsync(host_M, plan->M, sizeof(float) * (size_t)plan->n_wires * plan->n_ticks,
-                           cudaMemcpyDeviceToHost, plan->stream));
+    if (host_adc) {
+        rc = wcsim_digitize(plan, gain, baseline, bits, plan->dev_adc);
+        if (rc) return rc;
+        CU_TRY(cudaMemcpyAsync(host_adc, plan->dev_adc, sizeof(short) * grid, cudaMemcpyDeviceToHost, plan->stream));
+    }
+    if (host_M) CU_TRY(cudaMemcpyAsync(host_M, plan->M, sizeof(float) * grid, cudaMemcpyDeviceToHost, plan->stream));
     return WCSIM_OK;
+}
+
+} // namespace
+
+int wcsim_simulate_host_async(wcsim_plan *plan, const float *host_t0, const float *host_x0, const float *host_sigma_t,
+                        const float *host_sigma_x, const float *host_q, long long n, unsigned long long seed,
+                        int fluctuate, int noise, unsigned long long noise_seed, float *host_M)
+{
+    if (!host_M) return WCSIM_EINVAL;
+    const float *const host[5] = {host_t0, host_x0, host_sigma_t, host_sigma_x, host_q};
+    return simulate_host_impl(plan, host, n, seed, fluctuate, noise, noise_seed, host_M, nullptr, 0.f, 0.f, 0);
+}
+
+int wcsim_simulate_host_adc_async(wcsim_plan *plan, const float *host_t0, const float *host_x0, const float *host_sigma_t,
+                                  const float *host_sigma_x, const float *host_q, long long n, unsigned long long seed,
+                                  int fluctuate, int noise, unsigned long long noise_seed, float gain, float baseline,
+                                  int bits, short *host_adc)
+{
+    if (!host_adc) return WCSIM_EINVAL;
+    const float *const host[5] = {host_t0, host_x0, host_sigma_t, host_sigma_x, host_q};
+    return simulate_host_impl(plan, host, n, seed, fluctuate, noise, noise_seed, nullptr, host_adc, gain, baseline, bits);
 }
 
 int wcsim_simulate_host(wcsim_plan *plan, const float *host_t0, const float *host_x0, const float *host_sigma_t,
@@ -645,6 +812,78 @@ int wcsim_simulate_host(wcsim_plan *plan, const float *host_t0, const float *hos
     DeviceGuard guard(plan->device);
     if (!guard.ok) return fail_cuda(cudaGetLastError());
     CU_TRY(cudaStreamSynchronize(plan->stream));
+    return WCSIM_OK;
+}
+
+// ---- CUDA graphs: a launch sequence captured once and replayed ----
+struct wcsim_graph {
+    wcsim_plan *plan;
+    cudaGraph_t graph;
+    cudaGraphExec_t exec;
+    unsigned long long launches; // kernels of this library inside one replay
+};
+
+int wcsim_graph_begin(wcsim_plan *plan)
+{
+    if (!plan) return WCSIM_EINVAL;
+    if (plan->capturing || plan->stream == nullptr) return WCSIM_ESTATE; // the legacy default stream cannot be captured
+    DeviceGuard guard(plan->device);
+    if (!guard.ok) return fail_cuda(cudaGetLastError());
+    const int rc = harvest_spans(plan);
+    if (rc) return rc;
+    CU_TRY(cudaStreamBeginCapture(plan->stream, cudaStreamCaptureModeRelaxed));
+    plan->capturing = true;
+    plan->captured_launches = plan->launches;
+    return WCSIM_OK;
+}
+
+int wcsim_graph_end(wcsim_plan *plan, wcsim_graph **out)
+{
+    if (out) *out = nullptr;
+    if (!plan || !out) return WCSIM_EINVAL;
+    if (!plan->capturing) return WCSIM_ESTATE;
+    DeviceGuard guard(plan->device);
+    plan->capturing = false;
+    const unsigned long long inside = plan->launches - plan->captured_launches;
+    plan->launches = plan->captured_launches; // nothing ran yet
+    cudaGraph_t g = nullptr;
+    CU_TRY(cudaStreamEndCapture(plan->stream, &g));
+    if (!g) return WCSIM_ECUDA;
+    cudaGraphExec_t exec = nullptr;
+    const cudaError_t e = cudaGraphInstantiate(&exec, g, 0);
+    if (e != cudaSuccess) {
+        cudaGraphDestroy(g);
+        return fail_cuda(e);
+    }
+    wcsim_graph *gr = new (std::nothrow) wcsim_graph{plan, g, exec, inside};
+    if (!gr) {
+        cudaGraphExecDestroy(exec);
+        cudaGraphDestroy(g);
+        return WCSIM_ENOMEM;
+    }
+    *out = gr;
+    return WCSIM_OK;
+}
+
+int wcsim_graph_launch(wcsim_graph *graph)
+{
+    if (!graph) return WCSIM_EINVAL;
+    if (graph->plan->capturing) return WCSIM_ESTATE;
+    DeviceGuard guard(graph->plan->device);
+    if (!guard.ok) return fail_cuda(cudaGetLastError());
+    CU_TRY(cudaGraphLaunch(graph->exec, graph->plan->stream));
+    graph->plan->launches += graph->launches;
+    return WCSIM_OK;
+}
+
+int wcsim_graph_destroy(wcsim_graph *graph)
+{
+    if (!graph) return WCSIM_OK;
+    DeviceGuard guard(graph->plan->device);
+    cudaStreamSynchronize(graph->plan->stream);
+    cudaGraphExecDestroy(graph->exec);
+    cudaGraphDestroy(graph->graph);
+    delete graph;
     return WCSIM_OK;
 }
 
@@ -733,6 +972,7 @@ int wcsim_debug_z32_scan(unsigned long long first_word, unsigned long long n_wor
 int wcsim_debug_response_spectrum(wcsim_plan *plan, float *host_out)
 {
     if (!plan || !host_out) return WCSIM_EINVAL;
+    if (!plan->Rhat) return WCSIM_ESTATE; // multi-plane plans keep no Rhat
     DeviceGuard guard(plan->device);
     const int nk = plan->pad_t / 2 + 1;
     CU_TRY(cudaMemcpy2DAsync(host_out, sizeof(float2) * (size_t)nk, plan->Rhat, sizeof(float2) * (size_t)plan->spec_stride,
