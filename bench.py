@@ -43,13 +43,15 @@ def load_peaks():
         return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)", "sm_max_mhz": 1965.0}
 
 
-def stage_bytes(pl, direct):
-    """Algorithmic HBM bytes of each convolution kernel for one plane-event."""
+def stage_bytes(pl, direct, K=1):
+    """Algorithmic HBM bytes of each convolution kernel for one plane-event; K impact positions
+    per wire make the charge grid and the row spectra K times taller (reading A25)."""
     nw, nt, pw, pt = pl["n_wires"], pl["n_ticks"], pl["pad_w"], pl["pad_t"]
     nk = pt // 2 + 1
     grid, spec = nw * nt * 4, nw * nk * 8
-    resp = pl["response"].shape[0] * nk * 8 if direct else pw * nk * 8  # Rt rows (direct) or Rhat (FFT wire mode)
-    return {"rows_forward": grid + spec, "cols": 2 * spec + resp, "rows_inverse": spec + grid}
+    n_rw = pl["response"].shape[-2]
+    resp = K * n_rw * nk * 8 if direct else pw * nk * 8  # Rt rows (direct) or Rhat (FFT wire mode)
+    return {"rows_forward": K * (grid + spec), "cols": (K + 1) * spec + resp, "rows_inverse": spec + grid}
 
 
 class ClockSampler:
@@ -136,9 +138,21 @@ def run_ours(args):
         fluct = 2
     mode = {"atomic": B.WCSIM_SCATTER_ATOMIC, "tiled": B.WCSIM_SCATTER_TILED, "fixed": B.WCSIM_SCATTER_FIXED}[args.scatter]
     stream = torch.cuda.current_stream()
-    plan = B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]), nsigma=cfg["nsigma"],
-                  scatter_mode=mode, stream=stream)
-    plan.set_wire_mode({"auto": B.WCSIM_WIRES_AUTO, "fft": B.WCSIM_WIRES_FFT, "direct": B.WCSIM_WIRES_DIRECT}[args.wires])
+    if args.impact > 1:
+        # labelled variant (reading A25): K impact positions per wire, depos in units of pitch / K
+        pl = dict(pl, depos=synth.to_impact_units(pl["depos"], args.impact),
+                  response=synth.response_impact(args.impact, *pl["response"].shape))
+
+    def make_plan(st):
+        if args.impact > 1:
+            return B.ImpactPlan(pl["n_wires"], pl["n_ticks"], pl["response"], pad_ticks=pl["pad_t"], nsigma=cfg["nsigma"],
+                                scatter_mode=mode, stream=st)
+        p_ = B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]), nsigma=cfg["nsigma"],
+                    scatter_mode=mode, stream=st)
+        p_.set_wire_mode({"auto": B.WCSIM_WIRES_AUTO, "fft": B.WCSIM_WIRES_FFT, "direct": B.WCSIM_WIRES_DIRECT}[args.wires])
+        return p_
+
+    plan = make_plan(stream)
     d = {k: torch.from_numpy(v).to(dev) for k, v in pl["depos"].items()}
     flush = torch.empty(FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
 
@@ -234,8 +248,7 @@ def run_ours(args):
         host[k_].copy_(torch.from_numpy(pl["depos"][k_]))
     n_e2e_plans = 3  # two leave the device->host engine idle part of the time (436 us); four gain nothing over three
     e2e_streams = [torch.cuda.Stream(device=dev) for _ in range(n_e2e_plans)]
-    e2e_plans = [B.Plan(pl["n_wires"], pl["n_ticks"], pl["response"], pad=(pl["pad_w"], pl["pad_t"]),
-                        nsigma=cfg["nsigma"], scatter_mode=mode, stream=st) for st in e2e_streams]
+    e2e_plans = [make_plan(st) for st in e2e_streams]
     host_M = [torch.empty((pl["n_wires"], pl["n_ticks"]), dtype=torch.float32).pin_memory() for _ in range(n_e2e_plans)]
 
     def run_e2e(k):
@@ -288,26 +301,26 @@ def run_ours(args):
     # ---- several independent plane-events in flight (the paper's section 3.3 runs several processes
     # per GPU for the same reason: one event does not fill the device).  Extra figure, not the headline.
     concurrent = batched = graphed = None
-    if args.streams > 1 and world == 1:
+    if args.streams > 1 and world == 1 and args.impact == 1:
         concurrent = concurrent_planes(args, B, cfg, pl, d, fluct, mode, dev, n_depos)
         if len(cfg["planes"]) == 1:
             # the same number of independent plane-events through ONE launch sequence of a multi-plane plan
             batched = batched_events(args, B, cfg, [pl] * args.streams, [d] * args.streams, fluct, mode, dev)
             batched["ms_per_plane_event"] = batched["ms_per_event"] / args.streams
             batched["ms_per_plane_event_cuda_graph"] = batched["ms_per_event_cuda_graph"] / args.streams
-    if world == 1:
+    if world == 1 and args.impact == 1:
         graphed = graph_plane_event(args, B, cfg, pl, d, fluct, mode, dev, flush)
 
     # configs[3] is an APA event: three planes with their own responses, noise on every one.  Extra figure: whole events,
     # the three planes of an event on three plans/streams (planes are independent)
     apa = None
-    if len(cfg["planes"]) > 1 and world == 1:
+    if len(cfg["planes"]) > 1 and world == 1 and args.impact == 1:
         apa = apa_events(args, B, cfg, fluct, mode, dev)
 
     # ---- roofline of the dominant kernel --------------------------------------------------------------------------
     peaks = load_peaks()
-    direct = args.wires == "direct" or (args.wires == "auto" and pl["response"].shape[0] <= 64)
-    sb = stage_bytes(pl, direct)
+    direct = args.impact > 1 or args.wires == "direct" or (args.wires == "auto" and pl["response"].shape[-2] <= 64)
+    sb = stage_bytes(pl, direct, args.impact)
     stage_rows = []
     for name in ("raster", "rows_forward", "cols", "rows_inverse"):
         ms, calls = stages[name]
@@ -375,7 +388,9 @@ def run_ours(args):
                                              else ", fluctuation on") +
                                (", noise fused (plane 0 timed)" if noisy else "") +
                                (", LARGE-PATCH VARIANT sigma x %g (not one of the five configs)" % args.sigma_scale
-                                if args.sigma_scale != 1.0 else ""),
+                                if args.sigma_scale != 1.0 else "") +
+                               (", IMPACT-POSITION VARIANT: %d impact positions per wire, reading A25 (not one of the five "
+                                "configs)" % args.impact if args.impact > 1 else ""),
                    "grid": [pl["n_wires"], pl["n_ticks"]], "pad": [pl["pad_w"], pl["pad_t"]],
                    "response": list(pl["response"].shape), "depos": n_depos, "scatter": args.scatter,
                    "wire_axis": "direct" if direct else "fft",
@@ -403,7 +418,7 @@ def run_ours(args):
         out["cuda_graph"] = graphed
     if apa:
         out["apa_event"] = apa
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and args.impact == 1:
         out["cpu_baseline"] = cpu_baseline(cfg, budget_s=args.cpu_budget)
     if rank == 0 and world == 1 and args.cufft:
         out["cufft_comparator"] = cufft_comparator(pl, dev, flush)
@@ -701,6 +716,8 @@ def main():
                     help="sampler of the fluctuated raster: reading A6 (headline) or the Kokkos port's normal approximation (A21)")
     ap.add_argument("--sigma-scale", type=float, default=1.0,
                     help="labelled large-patch variant of configs[1]/[2] (reading A19): widths multiplied by this factor")
+    ap.add_argument("--impact", type=int, default=1,
+                    help="labelled variant (reading A25): impact positions per wire; depos and response are re-expressed on the finer grid")
     ap.add_argument("--streams", type=int, default=3, help="plane-events in flight for the extra `concurrent` figure")
     ap.add_argument("--e2e-steps", type=int, default=200)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")

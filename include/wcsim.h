@@ -40,7 +40,8 @@ typedef enum wcsim_status {
 #define WCSIM_SCATTER_ATOMIC 0 /* fp32 red.global adds straight into S; order of equal-address adds is not fixed */
 #define WCSIM_SCATTER_TILED 1  /* depos are binned by grid tile, each tile is accumulated in shared memory in
                                   integer / fixed-point arithmetic (order independent => bitwise reproducible)
-                                  and stored once; "deterministic sort-by-tile mode" of BASELINE.json north_star */
+                                  and stored once; "deterministic sort-by-tile mode" of BASELINE.json north_star.
+                                  WCSIM_SCATTER_FIXED gives the same bits faster */
 #define WCSIM_SCATTER_FIXED 2  /* the atomic mode's kernel adding in 2^-24 fixed point into a 64-bit grid (integer
                                   red.global adds: order independent => bitwise reproducible), folded into S by one
                                   pass; deterministic without sorting, 8 bytes per bin of extra device memory */
@@ -105,8 +106,10 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
  * Bins outside the grid are dropped and not drawn (A5).  S accumulates across calls; wcsim_clear zeroes it.
  *   depos           : struct of DEVICE pointers (the struct itself is read on the host during the call).
  *   dev_depo_totals : DEVICE, n int32, or NULL.  With fluctuate = 1 or 2 receives the signed sum of each depo's draws.
- * n = 0 is valid and does nothing.  In WCSIM_SCATTER_TILED mode the call synchronises the stream once (the size of the
- * per-tile depo lists is read back before they are filled) and n must be < 2^32; the other modes only enqueue.
+ * n = 0 is valid and does nothing.  Every mode only enqueues.  WCSIM_SCATTER_TILED lists a depo in the at most 4 tiles
+ * its patch touches (so 4 n list entries always suffice and nothing is read back; the lists are grown, with one stream
+ * synchronisation, when a call brings more depos than any before) and sends a patch that touches more tiles through the
+ * fixed-point grid of WCSIM_SCATTER_FIXED instead; 4 n + 16 must be < 2^32.
  */
 int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n, unsigned long long depo_id_base,
                          unsigned long long seed, int fluctuate, int *dev_depo_totals);
@@ -232,13 +235,33 @@ int wcsim_raster_scatter_planes(wcsim_plan *plan, const wcsim_depos *depos, cons
 int wcsim_get_plane_rows(const wcsim_plan *plan, int plane, int *first_row, int *n_rows);
 
 /*
+ * Sub-wire "impact position" response binning (reading A25 of DESIGN.md; the patches are
+ * "typically O(20x20) elements", which whole-wire bins do not give).  The charge grid is n_impact times finer along the
+ * wire axis: fine row x * n_impact + k holds the charge arriving at impact position k of wire x, i.e. at pitch coordinate
+ * [(x n_impact + k) / n_impact, +1/n_impact).  Depos given to such a plan carry x0 and sigma_x in units of
+ * pitch / n_impact (wcsim_drift with pitch / n_impact as its pitch produces them); the raster, the fluctuation and the
+ * Philox bin (fine row * n_ticks + tick) are those of a plane with n_wires * n_impact rows.  The response is given per
+ * impact position and the measured waveform of a wire sums over its impact positions:
+ *     M[x][t] = sum_k sum_dx sum_dt R_k[dx + c][dt] S[(x - dx) n_impact + k][t - dt]
+ * (n_impact = 1: Eq. (1) as wcsim_plan_create computes it).  wcsim_convolve transforms the n_wires * n_impact fine rows
+ * along ticks, applies the n_impact * n_rwires taps directly along wires, and inverts n_wires rows.
+ *   responses : HOST, n_impact pointers to n_rwires x n_rticks floats (position k's response, layout as in wcsim_plan_create).
+ * wcsim_charge_ptr gives the fine grid (wcsim_get_charge_dims: its rows), wcsim_output_ptr the n_wires x n_ticks M.
+ * Errors: WCSIM_EINVAL (n_impact outside 1..64, n_wires * n_impact * n_ticks >= 2^30, ...).
+ */
+int wcsim_plan_create_impact(wcsim_plan **out, int n_wires, int n_ticks, int n_impact, const float *const *responses,
+                             int n_rwires, int n_rticks, int pad_ticks, float nsigma, int scatter_mode, void *cuda_stream);
+/* rows and ticks of the charge grid S (rows = n_wires * n_impact; the stacked rows of a multi-plane plan) */
+int wcsim_get_charge_dims(const wcsim_plan *plan, int *rows, int *n_ticks, int *n_impact);
+
+/*
  * CUDA graphs (a small plane-event is bound by launch latency).  Between wcsim_graph_begin and
  * wcsim_graph_end the plan's stream is in capture mode: wcsim_clear, wcsim_raster_scatter(_planes), wcsim_arm_noise
  * (built-in spectrum), wcsim_convolve, wcsim_add_noise (built-in), wcsim_digitize only RECORD their work (the kernels keep
  * their programmatic-dependent-launch edges); the graph replays that sequence on the plan's stream at every
  * wcsim_graph_launch, with the pointers and sizes recorded (the depo arrays must still be valid and may hold new values).
- * Not capturable (WCSIM_ESTATE while capturing): the tiled scatter mode (it reads a size back), a first use of the
- * fixed-point mode on the plan, custom noise spectra, anything that synchronises (wcsim_sync, wcsim_get_stats, the
+ * Not capturable (WCSIM_ESTATE while capturing): a first use of the fixed-point or tiled mode on the plan, or a tiled
+ * call with more depos than any before (they allocate: run the call once outside the capture), custom noise spectra, anything that synchronises (wcsim_sync, wcsim_get_stats, the
  * *_host calls must not be called).  The plan's stream must not be the legacy default stream (WCSIM_ESTATE).
  * Stage timing is off inside a capture.  Destroy graphs before their plan.
  */

@@ -26,6 +26,7 @@ SYMBOLS = [
     "wcsim_debug_philox", "wcsim_debug_binomial", "wcsim_debug_response_spectrum", "wcsim_debug_erf", "wcsim_simulate_host_async", "wcsim_debug_normal_draw", "wcsim_drift", "wcsim_digitize", "wcsim_set_normalize",
     "wcsim_debug_fast_normal", "wcsim_debug_z32_scan",
     "wcsim_plan_create_planes", "wcsim_raster_scatter_planes", "wcsim_get_plane_rows", "wcsim_simulate_host_adc_async",
+    "wcsim_plan_create_impact", "wcsim_get_charge_dims",
     "wcsim_graph_begin", "wcsim_graph_end", "wcsim_graph_launch", "wcsim_graph_destroy",
     "wcsim_strerror", "wcsim_last_cuda_error", "wcsim_version",
 ]
@@ -106,6 +107,8 @@ def lib():
         L.wcsim_raster_scatter_planes.argtypes = [vp, C.POINTER(wcsim_depos), C.POINTER(ll), ull, i]
         L.wcsim_get_plane_rows.argtypes = [vp, i, C.POINTER(i), C.POINTER(i)]
         L.wcsim_simulate_host_adc_async.argtypes = [vp, vp, vp, vp, vp, vp, ll, ull, i, i, ull, C.c_float, C.c_float, i, vp]
+        L.wcsim_plan_create_impact.argtypes = [C.POINTER(vp), i, i, i, C.POINTER(vp), i, i, i, C.c_float, i, vp]
+        L.wcsim_get_charge_dims.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(i)]
         L.wcsim_graph_begin.argtypes = [vp]
         L.wcsim_graph_end.argtypes = [vp, C.POINTER(vp)]
         L.wcsim_graph_launch.argtypes = [vp]
@@ -251,17 +254,24 @@ def wcsim_get_dims(plan):
     return tuple(x.value for x in v)
 
 
-def _borrow(plan, fn, name):
+def _borrow(plan, fn, name, rows=None):
     import torch
     p = C.c_void_p()
     _check(fn(plan, C.byref(p)), name)
     n_wires, n_ticks, _, _ = wcsim_get_dims(plan)
-    return torch.as_tensor(_Borrowed(p.value, (n_wires, n_ticks), plan), device="cuda")
+    return torch.as_tensor(_Borrowed(p.value, (rows or n_wires, n_ticks), plan), device="cuda")
+
+
+def wcsim_get_charge_dims(plan):
+    """(rows, ticks, impact positions per wire) of the charge grid S."""
+    v = [C.c_int() for _ in range(3)]
+    _check(lib().wcsim_get_charge_dims(plan, *[C.byref(x) for x in v]), "wcsim_get_charge_dims")
+    return tuple(x.value for x in v)
 
 
 def wcsim_charge_ptr(plan):
-    """S as a torch view [n_wires][n_ticks] of the plan's buffer (borrowed: valid until wcsim_plan_destroy)."""
-    return _borrow(plan, lib().wcsim_charge_ptr, "wcsim_charge_ptr")
+    """S as a torch view [rows][n_ticks] of the plan's buffer (borrowed: valid until wcsim_plan_destroy)."""
+    return _borrow(plan, lib().wcsim_charge_ptr, "wcsim_charge_ptr", rows=wcsim_get_charge_dims(plan)[0])
 
 
 def wcsim_output_ptr(plan):
@@ -345,6 +355,20 @@ def wcsim_plan_create_planes(n_wires, n_ticks, responses, pad_ticks=0, nsigma=3.
     st = lib().wcsim_plan_create_planes(C.byref(h), len(rs), nw, int(n_ticks), rp, rs[0].shape[0], rs[0].shape[1],
                                         int(pad_ticks), float(nsigma), int(scatter_mode), _stream_ptr(stream))
     _check(st, "wcsim_plan_create_planes")
+    return h
+
+
+def wcsim_plan_create_impact(n_wires, n_ticks, responses, pad_ticks=0, nsigma=3.0, scatter_mode=WCSIM_SCATTER_ATOMIC,
+                             stream=None):
+    """responses: host array [n_impact][n_rwires][n_rticks] (reading A25)."""
+    r = np.ascontiguousarray(responses, dtype=np.float32)
+    if r.ndim != 3:
+        raise ValueError("responses must be 3-D [n_impact][n_rwires][n_rticks]")
+    rp = (C.c_void_p * r.shape[0])(*[r[k].ctypes.data_as(C.c_void_p) for k in range(r.shape[0])])
+    h = C.c_void_p()
+    st = lib().wcsim_plan_create_impact(C.byref(h), int(n_wires), int(n_ticks), r.shape[0], rp, r.shape[1], r.shape[2],
+                                        int(pad_ticks), float(nsigma), int(scatter_mode), _stream_ptr(stream))
+    _check(st, "wcsim_plan_create_impact")
     return h
 
 
@@ -600,6 +624,15 @@ class PlanesPlan(Plan):
         self.handle = wcsim_plan_create_planes(n_wires, n_ticks, responses, pad_ticks, nsigma, scatter_mode, stream)
         self.n_wires, self.n_ticks, self.pad_w, self.pad_t = wcsim_get_dims(self.handle)
         self.n_planes = len(n_wires)
+
+
+class ImpactPlan(Plan):
+    """A plan with sub-wire impact positions (wcsim_plan_create_impact, reading A25): depos in units of pitch / n_impact."""
+
+    def __init__(self, n_wires, n_ticks, responses, pad_ticks=0, nsigma=3.0, scatter_mode=WCSIM_SCATTER_ATOMIC, stream=None):
+        self.handle = wcsim_plan_create_impact(n_wires, n_ticks, responses, pad_ticks, nsigma, scatter_mode, stream)
+        self.n_wires, self.n_ticks, self.pad_w, self.pad_t = wcsim_get_dims(self.handle)
+        self.n_impact = wcsim_get_charge_dims(self.handle)[2]
 
 
 class Graph:

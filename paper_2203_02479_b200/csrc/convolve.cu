@@ -176,33 +176,40 @@ __global__ void __launch_bounds__(32 * kWiresRG, 3) wires_kernel(GridDims g, Con
     const int n_wires = b.planes.row0[pl + 1] - b.planes.row0[pl];
     if (k >= nk || x0 >= n_wires) return;
     const ptrdiff_t stride = STRIDE ? (ptrdiff_t)STRIDE : (ptrdiff_t)b.spec_stride;
+    // impact positions (reading A25): position kk of wire x is fine row x K + kk of the row spectra, so the inputs of one
+    // position are K rows apart and the taps of every position accumulate into the same outputs.  The instances with a
+    // compile-time stride are only launched for K = 1.
+    const int K = STRIDE ? 1 : b.impact_K;
+    const ptrdiff_t rstep = STRIDE ? (ptrdiff_t)STRIDE : stride * K;
     const int c = (b.n_rw - 1) / 2;
     float2 acc[O];
 #pragma unroll
     for (int o = 0; o < O; ++o) acc[o] = make_float2(0.f, 0.f);
-    // chunk d0 uses wire rows x0 + c - d0 - (D-1) .. x0 + c - d0 + O - 1 (halo rows included) and Rt rows d0 .. d0+D-1
-    const float2 *in = b.spec + k + ((ptrdiff_t)(b.planes.srow0[pl] + x0) + c - (D - 1)) * stride; // plain loads: see pdl.cuh
-    const float2 *__restrict__ rt = b.Rt + k + (ptrdiff_t)pl * b.rt_rows * stride;
     const int n_chunks = NCH ? NCH : b.rt_rows / D;
+    for (int kk = 0; kk < K; ++kk) {
+        // chunk d0 uses wire rows x0 + c - d0 - (D-1) .. x0 + c - d0 + O - 1 (halo rows included) and Rt rows d0 .. d0+D-1
+        const float2 *in = b.spec + k + ((ptrdiff_t)b.planes.srow0[pl] + ((ptrdiff_t)x0 + c - (D - 1)) * K + kk) * stride; // plain loads: see pdl.cuh
+        const float2 *__restrict__ rt = b.Rt + k + ((ptrdiff_t)pl * K + kk) * b.rt_rows * stride;
 #pragma unroll
-    for (int ch = 0; ch < n_chunks; ++ch) {
-        float2 coef[D], s[O + D - 1];
+        for (int ch = 0; ch < n_chunks; ++ch) {
+            float2 coef[D], s[O + D - 1];
 #pragma unroll
-        for (int j = 0; j < D; ++j) coef[j] = __ldg(rt + j * stride);
+            for (int j = 0; j < D; ++j) coef[j] = __ldg(rt + j * stride);
 #pragma unroll
-        for (int q = 0; q < O + D - 1; ++q) s[q] = in[q * stride];
+            for (int q = 0; q < O + D - 1; ++q) s[q] = in[q * rstep];
 #pragma unroll
-        for (int o = 0; o < O; ++o)
+            for (int o = 0; o < O; ++o)
 #pragma unroll
-            for (int j = 0; j < D; ++j) {
-                const float2 v = s[o - j + D - 1], w = coef[j];
-                acc[o].x = fmaf(w.x, v.x, acc[o].x);
-                acc[o].x = fmaf(-w.y, v.y, acc[o].x);
-                acc[o].y = fmaf(w.x, v.y, acc[o].y);
-                acc[o].y = fmaf(w.y, v.x, acc[o].y);
-            }
-        in -= D * stride;
-        rt += D * stride;
+                for (int j = 0; j < D; ++j) {
+                    const float2 v = s[o - j + D - 1], w = coef[j];
+                    acc[o].x = fmaf(w.x, v.x, acc[o].x);
+                    acc[o].x = fmaf(-w.y, v.y, acc[o].x);
+                    acc[o].y = fmaf(w.x, v.y, acc[o].y);
+                    acc[o].y = fmaf(w.y, v.x, acc[o].y);
+                }
+            in -= D * rstep;
+            rt += D * stride;
+        }
     }
     float2 *__restrict__ out = b.spec2 + k + (ptrdiff_t)(b.planes.row0[pl] + x0) * stride;
 #pragma unroll
@@ -525,7 +532,7 @@ cudaError_t launch_wires(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st)
     const dim3 block(32, kWiresRG), grid((nk + 31) / 32, b.planes.grp0[b.planes.n]); // row groups of all planes
     // BASELINE.json's paddings and response widths (21 wires -> 3 chunks, 41 -> 6) get immediate-offset loads and an
     // unrolled chunk loop; anything else takes the generic instance
-    const int key = b.rt_rows / kWiresD * 100000 + b.spec_stride;
+    const int key = b.impact_K == 1 ? b.rt_rows / kWiresD * 100000 + b.spec_stride : -1;
     const int tail = pdl_tail_from((long long)grid.x * grid.y, (long long)b.sm_count * 3); // 80 registers x 256 threads
     cudaError_t err = cudaSuccess;
     switch (key) {

@@ -51,9 +51,10 @@ cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t
 
 // the same kernel adding in 2^-24 fixed point into a 64-bit grid (RED.ADD.64: order independent, so reproducible bit for
 // bit whatever the order of the adds); launch_tile_finalize folds the grid into S afterwards
+// big_only: raster only the depos whose patch touches more than tile_max_listed() tiles (the rest of the tiled mode's work)
 cudaError_t launch_raster_fixed(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
                                 double nsigma, unsigned long long *fix, int *depo_totals, Counters *counters, int sm_count,
-                                cudaStream_t st);
+                                cudaStream_t st, bool big_only = false);
 
 // a1-a3 for the planes of a multi-plane plan in ONE launch (atomic or fixed-point sink): plane p's depos are cut into
 // batches batch0[p] .. batch0[p+1]-1, a warp's batch index says which plane (depo arrays, wire count, row offset in the
@@ -77,10 +78,9 @@ struct TileScratch {
     unsigned int *tile_count;     // [n_tiles + 1] counts, then exclusive offsets
     unsigned int *tile_cursor;    // [n_tiles] fill cursors
     unsigned int *entries;        // [capacity] depo indices grouped by tile
-    unsigned long long capacity;  // entries allocated
-    unsigned long long *total;    // [1] total number of (depo, tile) pairs, summed in 64 bits by tile_count (the per-tile
-                                  // offsets are 32-bit: the caller rejects totals >= 2^32)
-    unsigned int slice_entries;   // listed depos per slice of a hot tile (set per call from the mean tile load)
+    unsigned long long capacity;  // entries allocated: >= kMaxListedTiles * n of the call (a depo is listed in at most that
+                                  // many tiles; one that touches more is rastered straight into `fix` by the atomic kernel)
+    unsigned int *slice_dev;      // [1] DEVICE: listed depos per slice of a hot tile, set by tile_scan from the mean tile load
     unsigned long long *fix;      // [n_wires * n_ticks] 2^-24 fixed-point grid the tile CTAs add into; zero between calls
 };
 cudaError_t launch_tile_count(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts, cudaStream_t st);
@@ -88,6 +88,7 @@ cudaError_t launch_tile_scan(TileScratch ts, cudaStream_t st);
 cudaError_t launch_tile_fill(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts, cudaStream_t st);
 cudaError_t launch_count_invalid(DepoArrays d, long long n, Counters *counters, cudaStream_t st);
 void tile_shape(int *tile_w, int *tile_t);
+int tile_max_listed(); // kMaxListedTiles
 cudaError_t launch_tile_accumulate(GridDims g, DepoArrays d, uint64_t id_base, uint64_t seed, int fluctuate,
                                    double nsigma, TileScratch ts, float *S, int *depo_totals, Counters *counters,
                                    cudaStream_t st);
@@ -110,6 +111,8 @@ struct ConvBuffers {
     const float2 *tw_col; // per-pass twiddle tables of a pad_w-point FFT
     int spec_stride;      // pad_t/2 + 8
     int sm_count;         // SMs of the plan's device (grid size of the persistent row kernels)
+    int impact_K;         // impact positions per wire (reading A25): the row spectra hold n_wires * impact_K fine rows, fine
+                          // row x K + k = position k of wire x; Rt holds impact_K blocks of rt_rows rows.  1: whole wires
     PlaneTable planes;    // GridDims::n_wires of the convolution launchers is the stacked row count planes.row0[planes.n];
                           // Rt holds planes.n blocks of rt_rows rows, plane p's response at Rt + p rt_rows spec_stride
 };

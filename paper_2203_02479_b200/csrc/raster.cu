@@ -222,6 +222,35 @@ __device__ __noinline__ unsigned int raster_depo(float t0f, float x0f, float stf
     return drawn;
 }
 
+// ---- tiles of the deterministic sort-by-tile mode (the kernels are further down) ----
+constexpr int kSliceEntries = 256;  // listed depos per slice of a hot tile, at least
+constexpr int kMaxListedTiles = 4; // a depo is listed in at most this many tiles; bigger patches go through the fixed-point grid
+struct TileRange {
+    int w0, w1, t0, t1; // tile index ranges [w0, w1] x [t0, t1]; empty if w0 > w1
+    __device__ __forceinline__ int count() const { return w0 > w1 || t0 > t1 ? 0 : (w1 - w0 + 1) * (t1 - t0 + 1); }
+};
+__device__ __forceinline__ TileRange depo_tile_range(GridDims g, float t0, float x0, float st, float sx, float q, double nsigma)
+{
+    TileRange r{0, -1, 0, -1};
+    if (!depo_valid(t0, x0, st, sx, q)) return r;
+    const Extent et = axis_extent(t0, st, nsigma, 0, g.n_ticks);
+    const Extent ex = axis_extent(x0, sx, nsigma, 0, g.n_wires);
+    if (et.lo >= et.hi || ex.lo >= ex.hi) return r;
+    r.w0 = ex.lo / kTileW;
+    r.w1 = (ex.hi - 1) / kTileW;
+    r.t0 = et.lo / kTileT;
+    r.t1 = (et.hi - 1) / kTileT;
+    return r;
+}
+// the tiles a depo is LISTED in: none if it touches more than kMaxListedTiles
+__device__ __forceinline__ TileRange depo_tiles(GridDims g, DepoArrays d, long long i, double nsigma)
+{
+    TileRange r = depo_tile_range(g, __ldg(d.t0 + i), __ldg(d.x0 + i), __ldg(d.sigma_t + i), __ldg(d.sigma_x + i),
+                                  __ldg(d.q + i), nsigma);
+    if (r.count() > kMaxListedTiles) r = TileRange{0, -1, 0, -1};
+    return r;
+}
+
 __device__ __forceinline__ int warp_sum(int v)
 {
 #pragma unroll
@@ -738,7 +767,7 @@ template <int FLUCT, bool TOT, bool FIX>
 __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8) raster_batch_kernel(GridDims g, DepoArrays d, long long n,
                                                                         uint64_t id_base, uint64_t seed, double nsigma,
                                                                         float *__restrict__ S, int *__restrict__ totals,
-                                                                        Counters *counters, bool normalize, int3 sched)
+                                                                        Counters *counters, bool normalize, int4 sched)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     BatchSmem<FLUCT != 0, TOT> &sm = *reinterpret_cast<BatchSmem<FLUCT != 0, TOT> *>(smem_raw);
@@ -752,6 +781,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8
     // 3-4 batches of 8)
     const long long n_warps_grid = (long long)gridDim.x * kBatchWarps;
     const int tail_size = sched.x, n_static = sched.z;
+    const bool big_only = sched.w != 0; // the tiled mode's pass over the depos that are too big to be listed by tile
     const long long tail_depos = n_warps_grid * sched.y < n ? n_warps_grid * sched.y : n;
     const long long big_batches = (n - tail_depos) >> kBatchShift;
     const long long big_depos = big_batches << kBatchShift;
@@ -782,7 +812,8 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8
         if (more && lane < count && i < n) {
             t0 = d.t0[i], x0 = d.x0[i], st = d.sigma_t[i], sx = d.sigma_x[i], q = d.q[i]; // plain loads: pdl.cuh
             valid = depo_valid(t0, x0, st, sx, q);
-            skipped += !valid;
+            if (big_only) valid = valid && depo_tile_range(g, t0, x0, st, sx, q, nsigma).count() > kMaxListedTiles;
+            else skipped += !valid; // (the tiled mode counts invalid depos in its own pass)
         }
         // fluctuated: one more call without depos after the last batch empties the warp's draw queues
         if constexpr (FLUCT)
@@ -882,38 +913,13 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8
 // ------------------------------------------------------------------------------------------------------------------
 // tiled mode
 // ------------------------------------------------------------------------------------------------------------------
-struct TileRange {
-    int w0, w1, t0, t1; // tile index ranges [w0, w1] x [t0, t1]; empty if w0 > w1
-};
-
-__device__ __forceinline__ TileRange depo_tiles(GridDims g, DepoArrays d, long long i, double nsigma)
-{
-    TileRange r{0, -1, 0, -1};
-    const float t0 = __ldg(d.t0 + i), x0 = __ldg(d.x0 + i), st = __ldg(d.sigma_t + i), sx = __ldg(d.sigma_x + i),
-                q = __ldg(d.q + i);
-    if (!depo_valid(t0, x0, st, sx, q)) return r;
-    const Extent et = axis_extent(t0, st, nsigma, 0, g.n_ticks);
-    const Extent ex = axis_extent(x0, sx, nsigma, 0, g.n_wires);
-    if (et.lo >= et.hi || ex.lo >= ex.hi) return r;
-    r.w0 = ex.lo / kTileW;
-    r.w1 = (ex.hi - 1) / kTileW;
-    r.t0 = et.lo / kTileT;
-    r.t1 = (et.hi - 1) / kTileT;
-    return r;
-}
-
 __global__ void tile_count_kernel(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    unsigned long long pairs = 0;
-    if (i < n) {
-        const TileRange r = depo_tiles(g, d, i, nsigma);
-        for (int tw = r.w0; tw <= r.w1; ++tw)
-            for (int tt = r.t0; tt <= r.t1; ++tt) atomicAdd(ts.tile_count + (size_t)tw * ts.tiles_t + tt, 1u);
-        if (r.w0 <= r.w1 && r.t0 <= r.t1) pairs = (unsigned long long)(r.w1 - r.w0 + 1) * (unsigned long long)(r.t1 - r.t0 + 1);
-    }
-    pairs = warp_sum(pairs); // blockDim.x is a multiple of 32: whole warps reach this point
-    if ((threadIdx.x & 31) == 0 && pairs) atomicAdd(ts.total, pairs);
+    if (i >= n) return;
+    const TileRange r = depo_tiles(g, d, i, nsigma);
+    for (int tw = r.w0; tw <= r.w1; ++tw)
+        for (int tt = r.t0; tt <= r.t1; ++tt) atomicAdd(ts.tile_count + (size_t)tw * ts.tiles_t + tt, 1u);
 }
 
 // exclusive scan of tile_count[0..n_tiles) in place, tile_count[n_tiles] = total, cursors = offsets; one CTA
@@ -955,7 +961,12 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(TileScratch ts)
         if (threadIdx.x == 0) carry += warp_tot[31];
         __syncthreads();
     }
-    if (threadIdx.x == 0) ts.tile_count[n_tiles] = carry;
+    if (threadIdx.x == 0) {
+        ts.tile_count[n_tiles] = carry;
+        // a tile is split over several CTAs only when it lists well over the average: twice the mean, at least kSliceEntries
+        const unsigned int twice_mean = (unsigned int)(2ull * carry / (unsigned int)(n_tiles > 0 ? n_tiles : 1));
+        *ts.slice_dev = twice_mean > (unsigned int)kSliceEntries ? twice_mean : (unsigned int)kSliceEntries;
+    }
 }
 
 __global__ void tile_fill_kernel(GridDims g, DepoArrays d, long long n, double nsigma, TileScratch ts)
@@ -976,7 +987,7 @@ __global__ void tile_fill_kernel(GridDims g, DepoArrays d, long long n, double n
 // accumulating into fixed-point shared-memory accumulators; at the end the CTA adds its non-zero accumulators into the
 // global fixed-point grid `fix` (64-bit integer atomics: order independent), and tile_finalize_kernel folds `fix`
 // into S with one float add per bin.
-constexpr int kTileWarps = 8, kTileSlices = 8, kSliceEntries = 256;
+constexpr int kTileWarps = 8, kTileSlices = 8;
 template <bool FLUCT, bool TOT>
 struct TileSmem {
     unsigned long long acc[kTileW * kTileT];
@@ -999,9 +1010,10 @@ __global__ void __launch_bounds__(kTileWarps * 32, 2) tile_accumulate_kernel(Gri
     const int tile = blockIdx.x / kTileSlices, slice = blockIdx.x % kTileSlices;
     const unsigned int tile_beg = ts.tile_count[tile], tile_end = ts.tile_count[tile + 1];
     const unsigned int listed = tile_end - tile_beg;
-    // a tile is split only when it lists well over the average (ts.slice_entries = max(kSliceEntries, 2 x mean)): on an
+    // a tile is split only when it lists well over the average (*ts.slice_dev = max(kSliceEntries, 2 x mean)): on an
     // evenly busy plane (configs[4]) slicing only adds clears, flushes and partial queue drains
-    const unsigned int n_slices = min((unsigned int)kTileSlices, (listed + ts.slice_entries - 1) / ts.slice_entries);
+    const unsigned int slice_entries = *ts.slice_dev;
+    const unsigned int n_slices = min((unsigned int)kTileSlices, (listed + slice_entries - 1) / slice_entries);
     if ((unsigned int)slice >= n_slices) return; // uniform over the CTA (also: nothing listed)
     // equal slices in whole batches
     const unsigned int per = ((listed + n_slices - 1) / n_slices + kBatchDepos - 1) / kBatchDepos * kBatchDepos;
@@ -1140,14 +1152,14 @@ cudaError_t raster_configure(cudaStream_t st)
 template <int FLUCT, bool TOT, bool FIX>
 static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, double nsigma,
                                        float *S, int *depo_totals, Counters *counters, int sm_count, cudaStream_t st,
-                                       bool normalize)
+                                       bool normalize, bool big_only)
 {
     const size_t smem = sizeof(BatchSmem<FLUCT != 0, TOT>);
     const int fit = (int)((227u * 1024u) / (smem + 1024u)); // 227 KB per SM, 1 KB reserved per CTA
     const int cap = FLUCT ? WCSIM_FLUCT_CTAS : 8; // the kernel's __launch_bounds__
     const int ctas_per_sm = fit > cap ? cap : fit;
     const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
-    int3 sched = make_int3(kTailDepos, kTailPerWarp, 2);
+    int4 sched = make_int4(kTailDepos, kTailPerWarp, 2, big_only ? 1 : 0);
     // A small call (fewer depos than kBatchDepos per resident warp) is latency bound: a warp works its batch off serially,
     // so the depos are spread over as many warps as there are, in batches of `per` < kBatchDepos depos each (the kernel's
     // "tail" batches, here for every depo).  configs[0]: 100 depos -> 100 one-depo batches instead of 7 batches of 16.
@@ -1155,7 +1167,7 @@ static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, ui
     const long long warp_slots = max_ctas * kBatchWarps;
     const long long per = (n + warp_slots - 1) / warp_slots;
     if (per < kBatchDepos) {
-        sched = make_int3((int)(per > 0 ? per : 1), 1 << 24, 1); // every depo in a `per`-depo batch
+        sched = make_int4((int)(per > 0 ? per : 1), 1 << 24, 1, big_only ? 1 : 0); // every depo in a `per`-depo batch
         n_batches = (n + sched.x - 1) / sched.x;
     }
     long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
@@ -1172,12 +1184,12 @@ static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, ui
 template <bool FIX>
 static cudaError_t launch_raster_grid(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
                                       double nsigma, float *grid, int *depo_totals, Counters *counters, int sm_count,
-                                      cudaStream_t st)
+                                      cudaStream_t st, bool big_only = false)
 {
     if (n <= 0) return cudaSuccess;
     const bool normalize = (fluctuate & kRasterNormalize) != 0;
     fluctuate &= ~kRasterNormalize;
-#define WCSIM_BATCH(F, T) launch_raster_batch<F, T, FIX>(g, d, n, id_base, seed, nsigma, grid, T ? depo_totals : nullptr, counters, sm_count, st, normalize)
+#define WCSIM_BATCH(F, T) launch_raster_batch<F, T, FIX>(g, d, n, id_base, seed, nsigma, grid, T ? depo_totals : nullptr, counters, sm_count, st, normalize, big_only)
     if (!fluctuate) return WCSIM_BATCH(0, false); // no draws, no per-depo integer totals
     if (fluctuate == 2) return depo_totals ? WCSIM_BATCH(2, true) : WCSIM_BATCH(2, false);
     return depo_totals ? WCSIM_BATCH(1, true) : WCSIM_BATCH(1, false);
@@ -1193,10 +1205,10 @@ cudaError_t launch_raster_atomic(GridDims g, DepoArrays d, long long n, uint64_t
 
 cudaError_t launch_raster_fixed(GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
                                 double nsigma, unsigned long long *fix, int *depo_totals, Counters *counters, int sm_count,
-                                cudaStream_t st)
+                                cudaStream_t st, bool big_only)
 {
     return launch_raster_grid<true>(g, d, n, id_base, seed, fluctuate, nsigma, reinterpret_cast<float *>(fix), depo_totals,
-                                    counters, sm_count, st);
+                                    counters, sm_count, st, big_only);
 }
 
 int raster_batch_depos() { return kBatchDepos; }
@@ -1289,6 +1301,8 @@ cudaError_t launch_count_invalid(DepoArrays d, long long n, Counters *counters, 
     count_invalid_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d, n, counters);
     return cudaGetLastError();
 }
+
+int tile_max_listed() { return kMaxListedTiles; }
 
 void tile_shape(int *tile_w, int *tile_t)
 {

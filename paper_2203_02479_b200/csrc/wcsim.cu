@@ -25,6 +25,8 @@ struct wcsim_plan {
     int rt_rows = 0;
     int wire_mode = WCSIM_WIRES_AUTO;
     bool normalize = false; // renormalised patches (reading A24)
+    int impact_K = 1;       // impact positions per wire (reading A25); S has s_wires = n_wires * impact_K fine rows
+    int s_wires = 0;
     bool multi = false;     // created by wcsim_plan_create_planes
     bool capturing = false; // between wcsim_graph_begin and wcsim_graph_end
     unsigned long long captured_launches = 0;
@@ -37,7 +39,6 @@ struct wcsim_plan {
     const float *armed_amp = nullptr;
     uint64_t armed_seed = 0;
     TileScratch ts{};
-    unsigned long long *host_total = nullptr; // pinned
     float *stage_block = nullptr; // device staging of the five host depo arrays, 5 * stage_cap floats
     long long stage_cap = 0;
     // profiling: CUDA events recorded around each stage on the plan's stream while enabled
@@ -175,6 +176,7 @@ ConvBuffers conv_buffers(const wcsim_plan *p)
     b.spec_stride = p->spec_stride;
     b.sm_count = p->sm_count;
     b.planes = p->pt;
+    b.impact_K = p->impact_K;
     return b;
 }
 
@@ -231,41 +233,42 @@ int ensure_stage(wcsim_plan *p, long long n)
     return WCSIM_OK;
 }
 
+// Deterministic sort-by-tile mode, all on the stream (no read-back): a depo is listed in the at most tile_max_listed()
+// tiles its patch touches, so tile_max_listed() * n entries always suffice; a depo whose patch touches more tiles is not
+// listed and goes through the atomic kernel into the same fixed-point grid (integer adds: the sum does not depend on the
+// order), which tile_finalize folds into S.
 int raster_tiled(wcsim_plan *p, GridDims g, DepoArrays d, long long n, uint64_t id_base, uint64_t seed, int fluctuate,
                  int *totals)
 {
     TileScratch &ts = p->ts;
     const int n_tiles = ts.tiles_w * ts.tiles_t;
-    if (n > 0xFFFFFFFFll) return WCSIM_EINVAL; // entries hold 32-bit depo indices
-    CU_TRY(cudaMemsetAsync(ts.tile_count, 0, sizeof(unsigned int) * (size_t)(n_tiles + 1), p->stream));
-    CU_TRY(cudaMemsetAsync(ts.total, 0, sizeof(unsigned long long), p->stream));
-    CU_TRY(launch_tile_count(g, d, n, p->nsigma, ts, p->stream));
-    CU_TRY(launch_tile_scan(ts, p->stream));
-    CU_TRY(cudaMemcpyAsync(p->host_total, ts.total, sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
-    CU_TRY(cudaStreamSynchronize(p->stream));
-    const unsigned long long need = *p->host_total;
-    if (need > 0xFFFFFFFFull) return WCSIM_EINVAL; // the per-tile offsets are 32-bit: raster fewer depos per call
+    const unsigned long long need = (unsigned long long)tile_max_listed() * (unsigned long long)n + 16ull;
+    if (need > 0xFFFFFFFFull) return WCSIM_EINVAL; // 32-bit list offsets and depo indices: raster fewer depos per call
     if (need > ts.capacity) {
+        if (p->capturing) return WCSIM_ESTATE; // grow the lists outside a capture: run the call once before
+        CU_TRY(cudaStreamSynchronize(p->stream));
         if (ts.entries) cudaFree(ts.entries);
         ts.entries = nullptr;
         ts.capacity = 0;
-        const unsigned long long cap = need + need / 4 + 4096;
+        const unsigned long long cap = need + need / 4;
         CU_TRY(cudaMalloc((void **)&ts.entries, sizeof(unsigned int) * cap));
         ts.capacity = cap;
     }
-    {
-        const unsigned long long twice_mean = 2ull * need / (unsigned long long)(n_tiles > 0 ? n_tiles : 1);
-        ts.slice_entries = (unsigned int)(twice_mean > 256ull ? (twice_mean < 0x7fffffffull ? twice_mean : 0x7fffffffull) : 256ull);
-    }
-    if (!ts.fix) { // first use of the tiled mode on this plan
+    if (!ts.fix) { // first use of the fixed-point grid on this plan
+        if (p->capturing) return WCSIM_ESTATE;
         const size_t bytes = sizeof(unsigned long long) * (size_t)g.n_wires * g.n_ticks;
         CU_TRY(cudaMalloc((void **)&ts.fix, bytes));
         CU_TRY(cudaMemsetAsync(ts.fix, 0, bytes, p->stream));
     }
+    CU_TRY(cudaMemsetAsync(ts.tile_count, 0, sizeof(unsigned int) * (size_t)(n_tiles + 1), p->stream));
+    CU_TRY(launch_tile_count(g, d, n, p->nsigma, ts, p->stream));
+    CU_TRY(launch_tile_scan(ts, p->stream));
     CU_TRY(launch_tile_fill(g, d, n, p->nsigma, ts, p->stream));
     if (totals) CU_TRY(cudaMemsetAsync(totals, 0, sizeof(int) * (size_t)n, p->stream));
     CU_TRY(launch_count_invalid(d, n, p->counters, p->stream));
     CU_TRY(launch_tile_accumulate(g, d, id_base, seed, fluctuate, p->nsigma, ts, p->S, totals, p->counters, p->stream));
+    CU_TRY(launch_raster_fixed(g, d, n, id_base, seed, fluctuate, p->nsigma, ts.fix, totals, p->counters, p->sm_count,
+                               p->stream, true));
     CU_TRY(launch_tile_finalize(g, ts, p->S, p->stream));
     return WCSIM_OK;
 }
@@ -278,10 +281,9 @@ int destroy_impl(wcsim_plan *p)
                     p->S,        p->M,           p->spec_alloc,  p->Rhat,           p->tw_row,        p->tw_real,
                     p->tw_col,   p->counters,    p->amp_builtin, p->amp_custom,     p->ts.tile_count, p->ts.tile_cursor,
                     p->amp_armed, p->dev_adc,
-                    p->ts.entries, p->ts.total, p->ts.fix,  p->stage_block};
+                    p->ts.entries, p->ts.slice_dev, p->ts.fix,  p->stage_block};
     for (void *b : bufs)
         if (b) cudaFree(b);
-    if (p->host_total) cudaFreeHost(p->host_total);
     for (auto &sp : p->pending) {
         cudaEventDestroy(sp.beg);
         cudaEventDestroy(sp.end);
@@ -298,10 +300,12 @@ namespace {
 // plan creation for 1..kMaxPlanes planes stacked along the wire axis (same n_ticks, padding and response footprint).
 // `multi`: created by wcsim_plan_create_planes (direct wire pass only, no Rhat)
 int create_impl(wcsim_plan **out, int n_planes, const int *plane_wires, int n_ticks, const float *const *responses,
-                int n_rwires, int n_rticks, wcsim_pad pad, float nsigma, int scatter_mode, void *cuda_stream, bool multi)
+                int n_rwires, int n_rticks, wcsim_pad pad, float nsigma, int scatter_mode, void *cuda_stream, bool multi,
+                int K = 1)
 {
     if (!out) return WCSIM_EINVAL;
     *out = nullptr;
+    if (K < 1 || K > 64 || (K > 1 && (multi || n_planes != 1))) return WCSIM_EINVAL;
     if (!plane_wires || !responses || n_planes < 1 || n_planes > kMaxPlanes || n_ticks <= 0 || n_rwires <= 0 ||
         n_rticks <= 0 || (n_rwires % 2) == 0)
         return WCSIM_EINVAL;
@@ -312,6 +316,8 @@ int create_impl(wcsim_plan **out, int n_planes, const int *plane_wires, int n_ti
         total_wires += plane_wires[p];
         max_wires = plane_wires[p] > max_wires ? plane_wires[p] : max_wires;
     }
+    for (int k = 1; k < K; ++k)
+        if (!responses[k]) return WCSIM_EINVAL; // K > 1: responses[k] is the response of impact position k
     if (!(nsigma > 0.0f) || !std::isfinite(nsigma)) return WCSIM_EINVAL;
     if (scatter_mode < WCSIM_SCATTER_ATOMIC || scatter_mode > WCSIM_SCATTER_FIXED) return WCSIM_EINVAL;
     if (multi && scatter_mode == WCSIM_SCATTER_TILED) return WCSIM_EINVAL; // tiles belong to one plane
@@ -325,8 +331,9 @@ int create_impl(wcsim_plan **out, int n_planes, const int *plane_wires, int n_ti
         return WCSIM_EINVAL;
     if (pad_w < n_rwires) return WCSIM_EINVAL; // the wrapped response must not overlap itself
     if (!conv_sizes_supported(pad_w, pad_t)) return WCSIM_EINVAL;
-    if (total_wires * n_ticks >= (1ll << 30)) return WCSIM_EINVAL; // bin index + 2 flag bits in 32 (draw queues)
+    if (total_wires * K * n_ticks >= (1ll << 30)) return WCSIM_EINVAL; // bin index + 2 flag bits in 32 (draw queues)
     const int n_wires = (int)total_wires;
+    const int s_wires = n_wires * K; // rows of S and of the row spectra
 
     int dev = 0;
     CU_TRY(cudaGetDevice(&dev));
@@ -344,11 +351,15 @@ int create_impl(wcsim_plan **out, int n_planes, const int *plane_wires, int n_ti
     p->stream = (cudaStream_t)cuda_stream;
     p->device = dev;
     p->multi = multi;
-    if (multi) p->wire_mode = WCSIM_WIRES_DIRECT;
+    p->impact_K = K;
+    p->s_wires = s_wires;
+    if (multi || K > 1) p->wire_mode = WCSIM_WIRES_DIRECT;
 
     // the plane table: stacked rows, halo rows of the row spectra between the planes, row groups of the wire pass
     int halo_lo = 0, halo_hi = 0;
     wires_halo(n_rwires, &halo_lo, &halo_hi);
+    halo_lo *= K; // fine rows
+    halo_hi = halo_hi * K + (K - 1);
     const int per_group = wires_rows_per_group();
     PlaneTable &pt = p->pt;
     pt.n = n_planes;
@@ -368,21 +379,23 @@ int create_impl(wcsim_plan **out, int n_planes, const int *plane_wires, int n_ti
     double2 *dev_tmp = nullptr;
     int rc = [&]() -> int {
         CU_TRY(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev));
-        const size_t grid = (size_t)n_wires * n_ticks;
-        CU_TRY(cudaMalloc((void **)&p->S, sizeof(float) * grid));
+        const size_t grid = (size_t)n_wires * n_ticks, sgrid = (size_t)s_wires * n_ticks;
+        CU_TRY(cudaMalloc((void **)&p->S, sizeof(float) * sgrid));
         CU_TRY(cudaMalloc((void **)&p->M, sizeof(float) * grid));
-        const size_t spec_rows = (size_t)n_wires + (size_t)n_planes * (halo_lo + halo_hi);
+        const size_t spec_rows = (size_t)s_wires + (size_t)n_planes * (halo_lo + halo_hi);
         CU_TRY(cudaMalloc((void **)&p->spec_alloc, sizeof(float2) * spec_rows * p->spec_stride));
         p->spec = p->spec_alloc + (size_t)halo_lo * p->spec_stride;
         CU_TRY(cudaMalloc((void **)&p->spec2, sizeof(float2) * (size_t)n_wires * p->spec_stride));
-        if (!multi) CU_TRY(cudaMalloc((void **)&p->Rhat, sizeof(float2) * (size_t)pad_w * p->spec_stride));
+        const bool want_rhat = !multi && K == 1;
+        if (want_rhat) CU_TRY(cudaMalloc((void **)&p->Rhat, sizeof(float2) * (size_t)pad_w * p->spec_stride));
         p->rt_rows = (n_rwires + wires_chunk() - 1) / wires_chunk() * wires_chunk();
-        CU_TRY(cudaMalloc((void **)&p->Rt, sizeof(float2) * (size_t)n_planes * p->rt_rows * p->spec_stride));
+        const int n_resp = n_planes * K; // response blocks: one per plane, or one per impact position
+        CU_TRY(cudaMalloc((void **)&p->Rt, sizeof(float2) * (size_t)n_resp * p->rt_rows * p->spec_stride));
         CU_TRY(cudaMalloc((void **)&p->counters, sizeof(Counters)));
         CU_TRY(cudaMalloc((void **)&p->amp_builtin, sizeof(float) * (size_t)(pad_t / 2 + 1)));
         CU_TRY(cudaMalloc((void **)&p->amp_custom, sizeof(float) * (size_t)(pad_t / 2 + 1)));
         CU_TRY(cudaMalloc((void **)&p->amp_armed, sizeof(float) * (size_t)(pad_t / 2 + 1)));
-        CU_TRY(cudaMemsetAsync(p->S, 0, sizeof(float) * grid, p->stream));
+        CU_TRY(cudaMemsetAsync(p->S, 0, sizeof(float) * sgrid, p->stream));
         CU_TRY(cudaMemsetAsync(p->M, 0, sizeof(float) * grid, p->stream));
         CU_TRY(cudaMemsetAsync(p->spec_alloc, 0, sizeof(float2) * spec_rows * p->spec_stride, p->stream));
         CU_TRY(cudaMemsetAsync(p->spec2, 0, sizeof(float2) * (size_t)n_wires * p->spec_stride, p->stream));
@@ -397,18 +410,17 @@ int create_impl(wcsim_plan **out, int n_planes, const int *plane_wires, int n_ti
         if (r) return r;
         // tile lists of the deterministic scatter mode
         tile_shape(&p->ts.tile_w, &p->ts.tile_t);
-        p->ts.tiles_w = (n_wires + p->ts.tile_w - 1) / p->ts.tile_w;
+        p->ts.tiles_w = (s_wires + p->ts.tile_w - 1) / p->ts.tile_w;
         p->ts.tiles_t = (n_ticks + p->ts.tile_t - 1) / p->ts.tile_t;
         const size_t n_tiles = (size_t)p->ts.tiles_w * p->ts.tiles_t;
         CU_TRY(cudaMalloc((void **)&p->ts.tile_count, sizeof(unsigned int) * (n_tiles + 1)));
         CU_TRY(cudaMalloc((void **)&p->ts.tile_cursor, sizeof(unsigned int) * n_tiles));
-        CU_TRY(cudaMalloc((void **)&p->ts.total, sizeof(unsigned long long)));
-        CU_TRY(cudaMallocHost((void **)&p->host_total, sizeof(unsigned long long)));
+        CU_TRY(cudaMalloc((void **)&p->ts.slice_dev, sizeof(unsigned int)));
         // response spectra: Rt of every plane (direct wire pass), Rhat of a single-plane plan (FFT wire pass)
         const size_t nr = (size_t)n_rwires * n_rticks;
         CU_TRY(cudaMalloc((void **)&dev_R, sizeof(float) * nr));
         CU_TRY(cudaMalloc((void **)&dev_tmp, sizeof(double2) * (size_t)n_rwires * (pad_t / 2 + 1)));
-        for (int q = 0; q < n_planes; ++q) {
+        for (int q = 0; q < n_resp; ++q) {
             CU_TRY(cudaMemcpyAsync(dev_R, responses[q], sizeof(float) * nr, cudaMemcpyHostToDevice, p->stream));
             CU_TRY(build_response_spectrum(dev_R, n_rwires, n_rticks, pad_w, pad_t, p->spec_stride, dev_tmp, p->Rhat,
                                            p->stream));
@@ -445,6 +457,26 @@ int wcsim_plan_create(wcsim_plan **out, int n_wires, int n_ticks, const float *r
                        false);
 }
 
+int wcsim_plan_create_impact(wcsim_plan **out, int n_wires, int n_ticks, int n_impact, const float *const *responses,
+                             int n_rwires, int n_rticks, int pad_ticks, float nsigma, int scatter_mode, void *cuda_stream)
+{
+    if (out) *out = nullptr;
+    wcsim_pad pad;
+    pad.wires = 0;
+    pad.ticks = pad_ticks;
+    return create_impl(out, 1, &n_wires, n_ticks, responses, n_rwires, n_rticks, pad, nsigma, scatter_mode, cuda_stream,
+                       false, n_impact);
+}
+
+int wcsim_get_charge_dims(const wcsim_plan *plan, int *rows, int *n_ticks, int *n_impact)
+{
+    if (!plan) return WCSIM_EINVAL;
+    if (rows) *rows = plan->s_wires;
+    if (n_ticks) *n_ticks = plan->n_ticks;
+    if (n_impact) *n_impact = plan->impact_K;
+    return WCSIM_OK;
+}
+
 int wcsim_plan_create_planes(wcsim_plan **out, int n_planes, const int *n_wires, int n_ticks,
                              const float *const *responses, int n_rwires, int n_rticks, int pad_ticks, float nsigma,
                              int scatter_mode, void *cuda_stream)
@@ -466,13 +498,12 @@ int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n
     if (!depos || !depos->t0 || !depos->x0 || !depos->sigma_t || !depos->sigma_x || !depos->q) return WCSIM_EINVAL;
     DeviceGuard guard(plan->device);
     if (!guard.ok) return fail_cuda(cudaGetLastError());
-    const GridDims g{plan->n_wires, plan->n_ticks};
+    const GridDims g{plan->s_wires, plan->n_ticks}; // the charge grid: n_wires * impact_K rows
     const DepoArrays d{depos->t0, depos->x0, depos->sigma_t, depos->sigma_x, depos->q};
     if (plan->normalize) fluctuate |= kRasterNormalize; // internal.h: flag bit of the launchers' `fluctuate`
     StageSpan span(plan, WCSIM_STAGE_RASTER);
     if (plan->scatter_mode == WCSIM_SCATTER_TILED) {
-        if (plan->capturing) return WCSIM_ESTATE; // the tiled mode reads a size back: it cannot be captured
-        plan->launches += 6;
+        plan->launches += 7;
         return raster_tiled(plan, g, d, n, depo_id_base, seed, fluctuate, dev_depo_totals);
     }
     if (dev_depo_totals) CU_TRY(cudaMemsetAsync(dev_depo_totals, 0, sizeof(int) * (size_t)n, plan->stream));
@@ -524,7 +555,7 @@ int wcsim_raster_scatter_planes(wcsim_plan *plan, const wcsim_depos *depos, cons
         rp.count[p] = n[p];
         rp.batch0[p] = batches;
         batches += (n[p] + per_batch - 1) / per_batch;
-        rp.n_wires[p] = plan->pt.row0[p + 1] - plan->pt.row0[p];
+        rp.n_wires[p] = plan->impact_K > 1 ? plan->s_wires : plan->pt.row0[p + 1] - plan->pt.row0[p];
         rp.row0[p] = plan->pt.row0[p];
     }
     for (int p = rp.n; p <= kMaxPlanes; ++p) rp.batch0[p] = batches;
@@ -534,7 +565,7 @@ int wcsim_raster_scatter_planes(wcsim_plan *plan, const wcsim_depos *depos, cons
     const bool fixed = plan->scatter_mode == WCSIM_SCATTER_FIXED;
     if (fixed && !plan->ts.fix) { // first use of the fixed-point grid on this plan
         if (plan->capturing) return WCSIM_ESTATE;
-        const size_t bytes = sizeof(unsigned long long) * (size_t)plan->n_wires * plan->n_ticks;
+        const size_t bytes = sizeof(unsigned long long) * (size_t)plan->s_wires * plan->n_ticks;
         CU_TRY(cudaMalloc((void **)&plan->ts.fix, bytes));
         CU_TRY(cudaMemsetAsync(plan->ts.fix, 0, bytes, plan->stream));
     }
@@ -544,7 +575,7 @@ int wcsim_raster_scatter_planes(wcsim_plan *plan, const wcsim_depos *depos, cons
                                 plan->stream));
     if (fixed) {
         plan->launches += 1;
-        CU_TRY(launch_tile_finalize(GridDims{plan->n_wires, plan->n_ticks}, plan->ts, plan->S, plan->stream));
+        CU_TRY(launch_tile_finalize(GridDims{plan->s_wires, plan->n_ticks}, plan->ts, plan->S, plan->stream));
     }
     return WCSIM_OK;
 }
@@ -574,7 +605,7 @@ int wcsim_convolve(wcsim_plan *plan)
     StageSpan whole(plan, WCSIM_STAGE_CONVOLVE, !per_kernel);
     {
         StageSpan span(plan, WCSIM_STAGE_ROWS_FORWARD, per_kernel);
-        CU_TRY(launch_rows_forward(g, plan->pad_t, b, plan->stream));
+        CU_TRY(launch_rows_forward(GridDims{plan->s_wires, plan->n_ticks}, plan->pad_t, b, plan->stream));
     }
     {
         StageSpan span(plan, WCSIM_STAGE_COLS, per_kernel);
@@ -647,7 +678,7 @@ int wcsim_clear(wcsim_plan *plan)
 {
     if (!plan) return WCSIM_EINVAL;
     DeviceGuard guard(plan->device);
-    CU_TRY(cudaMemsetAsync(plan->S, 0, sizeof(float) * (size_t)plan->n_wires * plan->n_ticks, plan->stream));
+    CU_TRY(cudaMemsetAsync(plan->S, 0, sizeof(float) * (size_t)plan->s_wires * plan->n_ticks, plan->stream));
     return WCSIM_OK;
 }
 
@@ -684,8 +715,9 @@ int wcsim_set_normalize(wcsim_plan *plan, int on)
 int wcsim_set_wire_mode(wcsim_plan *plan, int wire_mode)
 {
     if (!plan || wire_mode < WCSIM_WIRES_AUTO || wire_mode > WCSIM_WIRES_DIRECT) return WCSIM_EINVAL;
-    if (plan->multi && wire_mode == WCSIM_WIRES_FFT) return WCSIM_ESTATE; // stacked planes: direct wire pass only
-    if (plan->multi) wire_mode = WCSIM_WIRES_DIRECT;
+    const bool direct_only = plan->multi || plan->impact_K > 1; // stacked planes, impact positions: direct wire pass only
+    if (direct_only && wire_mode == WCSIM_WIRES_FFT) return WCSIM_ESTATE;
+    if (direct_only) wire_mode = WCSIM_WIRES_DIRECT;
     plan->wire_mode = wire_mode;
     return WCSIM_OK;
 }

@@ -27,6 +27,28 @@ def response(n_rwires: int = 21, n_rticks: int = 200, unipolar: bool = False) ->
     return np.ascontiguousarray(r.astype(np.float32))
 
 
+def response_impact(n_impact: int, n_rwires: int = 21, n_rticks: int = 200, unipolar: bool = False) -> np.ndarray:
+    """R[k][dx + c][dt] for n_impact impact positions per wire (reading A25): the analytic form of configs[0] evaluated at
+    the distance between the target wire and the source position, x = dx - delta_k, delta_k = (k + 1/2)/n_impact - 1/2
+    (position k of a wire sits delta_k pitches from that wire's centre)."""
+    c = (n_rwires - 1) // 2
+    k = np.arange(n_impact, dtype=np.float64)[:, None, None]
+    x = np.arange(-c, c + 1, dtype=np.float64)[None, :, None] - ((k + 0.5) / n_impact - 0.5)
+    t = np.arange(n_rticks, dtype=np.float64)[None, None, :]
+    r = np.exp(-x * x / 4.5) * (t / 8.0) ** 4 * np.exp(-t / 8.0)
+    if not unipolar:
+        r = r * (1.0 - t / 40.0)
+    return np.ascontiguousarray(r.astype(np.float32))
+
+
+def to_impact_units(depos: dict, n_impact: int) -> dict:
+    """The same depos with x0 and sigma_x in units of pitch / n_impact (what a plan with impact positions takes)."""
+    out = dict(depos)
+    for key in ("x0", "sigma_x"):
+        out[key] = np.ascontiguousarray((depos[key].astype(np.float64) * n_impact).astype(np.float32))
+    return out
+
+
 def _rng(gen_seed: int, plane: int) -> np.random.Generator:
     return np.random.Generator(np.random.Philox(key=np.array([gen_seed, 0x47454E00 + plane], dtype=np.uint64)))
 

@@ -188,7 +188,7 @@ def test_graph_replays_a_plane_event(B, O):
         M_ref = O.convolve_direct(S_ref, R) + O.noise_add(np.zeros((nw, nt)), pl["pad_t"], 4)
         check_close(plan.output().cpu().numpy(), M_ref, "graph replay M + N")
         assert np.array_equal(adc.cpu().numpy(), O.digitize(plan.output().cpu().numpy(), 0.01, 900.0, 12))
-        # what cannot be captured says so instead of breaking the capture
+        # what cannot be captured says so instead of breaking the capture: the tiled mode's first call allocates its lists
         plan.graph_begin()
         plan.set_scatter_mode(B.WCSIM_SCATTER_TILED)
         with pytest.raises(B.WcsimError):
@@ -199,6 +199,22 @@ def test_graph_replays_a_plane_event(B, O):
         g2 = plan.graph_end()
         g2.destroy()
         graph.destroy()
+        # once its lists exist the tiled (sort-by-tile) mode is stream-ordered like the others and can be captured
+        plan.set_scatter_mode(B.WCSIM_SCATTER_TILED)
+        plan.clear()
+        plan.raster_scatter(dev, seed=3, fluctuate=True)
+        plan.sync()
+        S_tiled = plan.charge().cpu().numpy().copy()
+        assert np.array_equal(S_tiled.astype(np.float64), S_ref)
+        plan.graph_begin()
+        plan.clear()
+        plan.raster_scatter(dev, seed=3, fluctuate=True)
+        g3 = plan.graph_end()
+        plan.clear()
+        g3.launch()
+        plan.sync()
+        assert np.array_equal(plan.charge().cpu().numpy(), S_tiled)
+        g3.destroy()
     finally:
         plan.destroy()
     # the legacy default stream cannot be captured
