@@ -54,6 +54,15 @@ def stage_bytes(pl, direct, K=1):
     return {"rows_forward": K * (grid + spec), "cols": (K + 1) * spec + resp, "rows_inverse": spec + grid}
 
 
+def nvml_index(local_rank):
+    """NVML index of the rank's GPU: CUDA_VISIBLE_DEVICES may renumber devices; UUID / MIG entries or a list shorter than
+    the rank fall back to the local rank (the sampler then reports what that device does, or 'unsampled')."""
+    try:
+        return int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank])
+    except (KeyError, IndexError, ValueError):
+        return local_rank
+
+
 class ClockSampler:
     """Samples SM clock and throttle reasons of one GPU while the timed region runs (NVML, in a thread)."""
 
@@ -196,8 +205,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     plan.reset_stats()
     launches0 = plan.launch_count()
-    sampler = ClockSampler(local_rank if "CUDA_VISIBLE_DEVICES" not in os.environ else
-                           int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank]))
+    sampler = ClockSampler(nvml_index(local_rank))
     per_step = timed(step, args.steps, sampler)
     launches = plan.launch_count() - launches0
     local_s = sum(per_step) * 1e-3
@@ -319,7 +327,7 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel --------------------------------------------------------------------------
     peaks = load_peaks()
-    direct = args.impact > 1 or args.wires == "direct" or (args.wires == "auto" and pl["response"].shape[-2] <= 64)
+    direct = args.impact > 1 or args.wires == "direct" or (args.wires == "auto" and pl["response"].shape[-2] <= (32 if pl["pad_w"] <= 512 else 52 if pl["pad_w"] <= 2048 else 112))
     sb = stage_bytes(pl, direct, args.impact)
     stage_rows = []
     for name in ("raster", "rows_forward", "cols", "rows_inverse"):

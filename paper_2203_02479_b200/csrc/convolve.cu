@@ -5,7 +5,7 @@
 //   rows_forward : one CTA per populated wire row.  The real row of pad_t samples is packed as pad_t/2 complex
 //                  points (even + i odd), transformed in shared memory, and split into the half spectrum
 //                  k = 0 .. pad_t/2.  Samples beyond n_ticks are zeros made in registers.
-//   wires        : (default when the response spans <= 64 wires) the wire-axis transform / multiply / inverse done
+//   wires        : (default up to the measured crossover width, wcsim.cu wires_direct) the wire-axis transform / multiply / inverse done
 //                  directly as an n_rw-tap convolution over wires for every tick frequency; see wires_kernel.
 //   cols         : (otherwise, or on request) one CTA per tile of C adjacent tick-frequencies.  Forward transform over
 //                  the wire axis (rows beyond n_wires are zeros made in registers), multiply by the response spectrum
@@ -160,12 +160,19 @@ __global__ void __launch_bounds__(ColCfg<N>::threads) cols_kernel(GridDims g, Co
 // argument every load of a chunk is one instruction off a single pointer (immediate offsets): the inner loop is
 // 4 O D FFMAs against O + 2 D - 1 loads.  Neighbouring row groups of a CTA share their halo rows through L1.
 // ------------------------------------------------------------------------------------------------------------------
-constexpr int kWiresD = 7, kWiresRG = 8, kWiresO = 8;
+#ifndef WCSIM_WIRES_CTAS
+#define WCSIM_WIRES_CTAS 3
+#endif
+#ifndef WCSIM_WIRES_RG
+#define WCSIM_WIRES_RG 8
+#endif
+constexpr int kWiresD = 7, kWiresRG = WCSIM_WIRES_RG, kWiresO = 8;
+constexpr int kWiresCtas = WCSIM_WIRES_CTAS; // resident CTAs per SM the register budget is set for
 
 // STRIDE = 0: row stride read from the buffers (any pad_t); NCH = 0: chunk count read from the buffers (any n_rw),
 // else the chunk loop is unrolled so that the loads of the next chunk are in flight under the FFMAs of this one
 template <int O, int D, int NCH, int STRIDE>
-__global__ void __launch_bounds__(32 * kWiresRG, 3) wires_kernel(GridDims g, ConvBuffers b, int nk, int tail_from)
+__global__ void __launch_bounds__(32 * kWiresRG, kWiresCtas) wires_kernel(GridDims g, ConvBuffers b, int nk, int tail_from)
 {
     if ((int)(blockIdx.y * gridDim.x + blockIdx.x) >= tail_from) pdl_trigger();
     pdl_wait(); // the row spectra are rows_forward's
@@ -533,7 +540,7 @@ cudaError_t launch_wires(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st)
     // BASELINE.json's paddings and response widths (21 wires -> 3 chunks, 41 -> 6) get immediate-offset loads and an
     // unrolled chunk loop; anything else takes the generic instance
     const int key = b.impact_K == 1 ? b.rt_rows / kWiresD * 100000 + b.spec_stride : -1;
-    const int tail = pdl_tail_from((long long)grid.x * grid.y, (long long)b.sm_count * 3); // 80 registers x 256 threads
+    const int tail = pdl_tail_from((long long)grid.x * grid.y, (long long)b.sm_count * kWiresCtas);
     cudaError_t err = cudaSuccess;
     switch (key) {
     case 3 * 100000 + 1024 / 2 + 8: err = launch_pdl(wires_kernel<O, kWiresD, 3, 1024 / 2 + 8>, grid, block, 0, st, g, b, nk, tail); break;

@@ -420,7 +420,14 @@ __device__ __forceinline__ void raster_flat_body(GridDims g, Clip clip, const Si
 //     EXACT   whatever the fp32 guards do not accept (~1 %), and bins not eligible for them: the fp64 routines.
 // The edges of a batch are laid out per depo as [3 pad][nt+1 tick edges][3 pad][nx+1 wire edges], so that the loads of a
 // quad never need a bounds check (pad values only ever reach bins that are masked off).
-constexpr int kQuadEdgeCap = 192, kEdgePad = 3;
+#ifndef WCSIM_KUNROLL
+#define WCSIM_KUNROLL 1
+#endif
+constexpr int kQuadUnroll = WCSIM_KUNROLL; // unroll factor of the loop over the four bins of a quad
+#ifndef WCSIM_EDGE_CAP
+#define WCSIM_EDGE_CAP 192
+#endif
+constexpr int kQuadEdgeCap = WCSIM_EDGE_CAP, kEdgePad = 3;
 constexpr int kQueueCap = 64; // entries per queue: at most 31 left over + 32 pushed
 enum QuadQueue : int { kQNorm = 0, kQInvA = 1, kQInvB = 2, kQInvC = 3, kQExact = 4, kNumQuadQueues = 5 };
 constexpr int kQTotal = kNumQuadQueues * kQueueCap;
@@ -448,18 +455,25 @@ struct QuadQueues {
     uint32_t w[kQTotal];   // after the mirror
     uint32_t bin[kQTotal]; // sink index | kBinMirror | kBinNegative
     uint32_t depo[TOT ? kQTotal : 1];
+    alignas(16) int fill[8]; // entries in each of the five queues (kQNorm .. kQExact); pushed to with shared-memory atomics
 };
 template <bool TOT>
 struct QuadWarp {
     QuadScratch sc;
     QuadQueues<TOT> q;
 };
-// per-warp registers that live across batches: the fills of the four fp32 queues, 8 bits each (kQNorm lowest), and of the
-// exact queue
+// the fills while the queues are drained (registers, uniform over the warp): the four fp32 queues, 8 bits each (kQNorm
+// lowest), and the exact queue.  Between drains the fills live in QuadQueues::fill.
 struct QuadCounts {
     uint32_t fast = 0;
     int exact = 0;
 };
+template <bool TOT>
+__device__ __forceinline__ void queues_init(QuadWarp<TOT> &ws, int lane)
+{
+    if (lane < 8) ws.q.fill[lane] = 0;
+    __syncwarp();
+}
 
 template <bool TOT, typename Sink>
 __device__ __forceinline__ void commit_draw(const Sink &sink, int *__restrict__ totals, uint32_t fb, float N, float k,
@@ -537,11 +551,17 @@ __device__ __forceinline__ void drain_fast_group(QuadQueues<TOT> &Q, QuadCounts 
 // The queues.  Called (from one place) when one of them holds a warp's worth of work: every queue with 32 or more entries
 // is worked off in groups of 32; with `finish`, everything.
 template <bool TOT, typename Sink>
-__device__ __forceinline__ void drain_queues(QuadWarp<TOT> &ws, QuadCounts &qc, bool finish, const Sink &sink,
-                                             int *__restrict__ totals, int lane)
+__device__ __forceinline__ void drain_queues(QuadWarp<TOT> &ws, bool finish, const Sink &sink, int *__restrict__ totals,
+                                             int lane)
 {
     QuadQueues<TOT> &Q = ws.q;
     __syncwarp();
+    QuadCounts qc;
+    {
+        const int4 f = *reinterpret_cast<const int4 *>(Q.fill);
+        qc.fast = (uint32_t)f.x | ((uint32_t)f.y << 8) | ((uint32_t)f.z << 16) | ((uint32_t)f.w << 24);
+        qc.exact = Q.fill[kQExact];
+    }
     // the exact queue first if it is what is full: the groups below may each add up to 32 rejected bins to it
     if (qc.exact >= 32) qc.exact = drain_exact<TOT>(&Q, qc.exact, false, sink, totals, lane);
     const uint32_t thresh = finish ? 0xffffffffu : 0xe0e0e0e0u; // a queue is due when its fill is >= 32 (finish: > 0)
@@ -550,6 +570,12 @@ __device__ __forceinline__ void drain_queues(QuadWarp<TOT> &ws, QuadCounts &qc, 
     while (qc.fast & (0xffu << (8 * kQInvB)) & thresh) drain_fast_group<kQInvB, TOT>(Q, qc, sink, totals, lane);
     while (qc.fast & (0xffu << (8 * kQInvC)) & thresh) drain_fast_group<kQInvC, TOT>(Q, qc, sink, totals, lane);
     if (qc.exact >= 32 || (finish && qc.exact > 0)) qc.exact = drain_exact<TOT>(&Q, qc.exact, finish, sink, totals, lane);
+    __syncwarp();
+    if (lane == 0) {
+        *reinterpret_cast<int4 *>(Q.fill) = make_int4((int)(qc.fast & 0xffu), (int)((qc.fast >> 8) & 0xffu),
+                                                       (int)((qc.fast >> 16) & 0xffu), (int)(qc.fast >> 24));
+        Q.fill[kQExact] = qc.exact;
+    }
     __syncwarp();
 }
 
@@ -561,7 +587,7 @@ template <bool NORMAL_ONLY, bool TOT, bool INDIRECT, typename Sink>
 __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Sink &sink, float t0, float x0, float st,
                                                  float sx, float q, bool valid, long long dbase, uint32_t dl,
                                                  uint64_t id_base, uint64_t seed, double nsigma, bool normalize,
-                                                 int *__restrict__ totals, QuadWarp<TOT> &ws, QuadCounts &qc, bool flush,
+                                                 int *__restrict__ totals, QuadWarp<TOT> &ws, bool flush,
                                                  unsigned int &drawn, int lane)
 {
     constexpr bool normal_only = NORMAL_ONLY;
@@ -692,7 +718,7 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
             const uint32_t neg = a.z < 0 ? kBinNegative : 0u;
             const bool live_q = act && Nf > 0.0f; // N = 0 draws nothing
             uint32_t w0 = words.x, w1 = words.y, w2 = words.z, w3 = words.w;
-#pragma unroll 1
+#pragma unroll kQuadUnroll
             for (int k = 0; k < 4; ++k) {
                 uint32_t w = w0; // the word of this bin; the others move up
                 w0 = w1, w1 = w2, w2 = w3;
@@ -721,26 +747,20 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
                 // (a bin next to a band edge that needs more terms than its band has fails the guard and is redone).
                 int cls = !small ? kQNorm : !inv_fast_eligible(Nf, p) ? kQExact : muf < 2.0f ? kQInvA : muf < 6.0f ? kQInvB : kQInvC;
                 if (!draw) cls = -1;
-                const unsigned int peers = __match_any_sync(0xffffffffu, cls); // the lanes that push to the same queue
-                const int rank = __popc(peers & ((1u << lane) - 1u));
-                // new fills: the first lane of every group adds its group's size to the queue's byte
-                const bool lead = rank == 0 && cls >= 0 && cls < kQExact;
-                const uint32_t add = __reduce_add_sync(0xffffffffu, lead ? (uint32_t)__popc(peers) << (8 * cls) : 0u);
-                const int add_x = __popc(__ballot_sync(0xffffffffu, cls == kQExact));
+                // push: a shared-memory atomic on the queue's fill hands every lane its slot (the order of the entries in a
+                // queue does not matter: each carries all it needs, and the adds into S are order independent or exact)
                 if (cls >= 0) {
-                    const int fill = cls == kQExact ? qc.exact : (int)((qc.fast >> (8 * cls)) & 0xffu);
-                    const int pos = cls * kQueueCap + fill + rank;
+                    const int pos = cls * kQueueCap + atomicAdd(&Q.fill[cls], 1);
                     Q.p[pos] = p;
                     Q.N[pos] = (cls == kQExact && small) ? -Nf : Nf;
                     Q.w[pos] = w;
                     Q.bin[pos] = (idx0 + k) | neg | (mirror ? kBinMirror : 0u);
                     if constexpr (TOT) Q.depo[pos] = dio;
                 }
-                qc.fast += add;
-                qc.exact += add_x;
+                __syncwarp();
+                const int4 f = *reinterpret_cast<const int4 *>(Q.fill); // every fill is < 64: bit 5 says "a warp's worth"
                 const bool last = flush_here && k == 3 && s0 + 32 >= qtot;
-                if ((qc.fast & 0xe0e0e0e0u) | (uint32_t)(qc.exact >> 5) | (uint32_t)last)
-                    drain_queues<TOT>(ws, qc, last, sink, totals, lane);
+                if ((((f.x | f.y) | (f.z | f.w) | Q.fill[kQExact]) & 32) | (int)last) drain_queues<TOT>(ws, last, sink, totals, lane);
             }
         }
         __syncwarp();
@@ -787,7 +807,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8
     const long long big_depos = big_batches << kBatchShift;
     const long long n_batches = big_batches + (n - big_depos + tail_size - 1) / tail_size;
     unsigned int drawn = 0, skipped = 0; // per lane
-    QuadCounts qc;
+    if constexpr (FLUCT != 0) queues_init(sm.warp[wid], lane);
     // the grid is one wave, so the next kernel's CTAs may take the slots this one frees as it drains.  As a
     // programmatic dependent itself it only overlaps a preceding KERNEL's tail: copies and memsets ahead of it in the
     // stream are still fully ordered (checked with 300 host-buffer plane-events of changing depos, 0 mismatches)
@@ -818,7 +838,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8
         // fluctuated: one more call without depos after the last batch empties the warp's draw queues
         if constexpr (FLUCT)
             raster_quad_body<FLUCT == 2, TOT, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, id_base, seed, nsigma,
-                                                     normalize, totals, sm.warp[wid], qc, !more, drawn, lane);
+                                                     normalize, totals, sm.warp[wid], !more, drawn, lane);
         else if (more)
             raster_flat_body(g, clip, sink, t0, x0, st, sx, q, valid, nsigma, normalize, sm.scratch[wid], drawn, lane);
         if (!more) break;
@@ -862,7 +882,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8
     const long long n_warps_grid = (long long)gridDim.x * kBatchWarps;
     const long long n_batches = P.batch0[P.n];
     unsigned int drawn = 0, skipped = 0; // per lane
-    QuadCounts qc;
+    if constexpr (FLUCT != 0) queues_init(sm.warp[wid], lane);
     pdl_trigger();
     pdl_wait();
     long long batch = (long long)blockIdx.x * kBatchWarps + wid;
@@ -886,7 +906,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8
         const Clip clip{0, g.n_wires, 0, n_ticks, P.row0[pl]};
         if constexpr (FLUCT)
             raster_quad_body<FLUCT == 2, false, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, 0ull, seed, nsigma,
-                                                       normalize, nullptr, sm.warp[wid], qc, !more, drawn, lane);
+                                                       normalize, nullptr, sm.warp[wid], !more, drawn, lane);
         else if (more)
             raster_flat_body(g, clip, sink.shifted(clip.row_off), t0, x0, st, sx, q, valid, nsigma, normalize,
                              sm.scratch[wid], drawn, lane);
@@ -1028,7 +1048,7 @@ __global__ void __launch_bounds__(kTileWarps * 32, 2) tile_accumulate_kernel(Gri
     const TileSink sink{sm.acc, w0, k0};
     const Clip clip{w0, w1, k0, k1};
     unsigned int drawn = 0; // per lane
-    QuadCounts qc;
+    if constexpr (FLUCT != 0) queues_init(sm.warp[wid], lane);
     for (unsigned int e0 = beg + (unsigned int)wid * kBatchDepos;; e0 += kTileWarps * kBatchDepos) {
         const bool more = e0 < end;
         float t0 = 0.f, x0 = 0.f, st = 0.f, sx = 0.f, q = 0.f;
@@ -1041,7 +1061,7 @@ __global__ void __launch_bounds__(kTileWarps * 32, 2) tile_accumulate_kernel(Gri
         }
         if constexpr (FLUCT)
             raster_quad_body<FLUCT == 2, TOT, true>(g, clip, sink, t0, x0, st, sx, q, valid, 0ll, i, id_base, seed, nsigma,
-                                                    normalize, totals, sm.warp[wid], qc, !more, drawn, lane);
+                                                    normalize, totals, sm.warp[wid], !more, drawn, lane);
         else if (more)
             raster_flat_body(g, clip, sink, t0, x0, st, sx, q, valid, nsigma, normalize, sm.scratch[wid], drawn, lane);
         if (!more) break;
