@@ -425,9 +425,13 @@ __device__ __forceinline__ void raster_flat_body(GridDims g, Clip clip, const Si
 #endif
 constexpr int kQuadUnroll = WCSIM_KUNROLL; // unroll factor of the loop over the four bins of a quad
 #ifndef WCSIM_EDGE_CAP
-#define WCSIM_EDGE_CAP 192
+#define WCSIM_EDGE_CAP 400
 #endif
-constexpr int kQuadEdgeCap = WCSIM_EDGE_CAP, kEdgePad = 3;
+// Edge values a warp's scratch holds.  The atomic kernels take 400: a whole 16-depo batch of BASELINE.json's patches
+// (<= 16 + 5 + 2 edges and 6 pad slots each) then fits at once -- with 192 every batch was cut into two or three
+// sub-batches whose edge and quad passes ran with a quarter of their lanes empty (configs[1] 66.2 -> 64.6 us, configs[4]
+// 6.48 -> 6.23 ms).  The tile kernel keeps 192: with 8 warps and the tile's accumulators two of its CTAs must fit an SM.
+constexpr int kQuadEdgeCap = WCSIM_EDGE_CAP, kTileEdgeCap = 192, kEdgePad = 3;
 constexpr int kQueueCap = 64; // entries per queue: at most 31 left over + 32 pushed
 enum QuadQueue : int { kQNorm = 0, kQInvA = 1, kQInvB = 2, kQInvC = 3, kQExact = 4, kNumQuadQueues = 5 };
 constexpr int kQTotal = kNumQuadQueues * kQueueCap;
@@ -441,8 +445,9 @@ struct alignas(16) DepoRec {
     double inv_t, inv_x; // 1 / (sqrt2 sigma); 0: sigma < 1e-6 (A4)
 };
 
+template <int CAP>
 struct QuadScratch {
-    double edge[kQuadEdgeCap + 8]; // + slack: a quad past the end of a row may read up to 3 slots beyond the last pad
+    double edge[CAP + 8]; // + slack: a quad past the end of a row may read up to 3 slots beyond the last pad
     DepoRec rec[kBatchDepos];
     double inv_norm[kBatchDepos];
     int eoff[33], qoff[33];
@@ -457,9 +462,9 @@ struct QuadQueues {
     uint32_t depo[TOT ? kQTotal : 1];
     alignas(16) int fill[8]; // entries in each of the five queues (kQNorm .. kQExact); pushed to with shared-memory atomics
 };
-template <bool TOT>
+template <bool TOT, int CAP>
 struct QuadWarp {
-    QuadScratch sc;
+    QuadScratch<CAP> sc;
     QuadQueues<TOT> q;
 };
 // the fills while the queues are drained (registers, uniform over the warp): the four fp32 queues, 8 bits each (kQNorm
@@ -468,8 +473,8 @@ struct QuadCounts {
     uint32_t fast = 0;
     int exact = 0;
 };
-template <bool TOT>
-__device__ __forceinline__ void queues_init(QuadWarp<TOT> &ws, int lane)
+template <bool TOT, int CAP>
+__device__ __forceinline__ void queues_init(QuadWarp<TOT, CAP> &ws, int lane)
 {
     if (lane < 8) ws.q.fill[lane] = 0;
     __syncwarp();
@@ -550,8 +555,8 @@ __device__ __forceinline__ void drain_fast_group(QuadQueues<TOT> &Q, QuadCounts 
 
 // The queues.  Called (from one place) when one of them holds a warp's worth of work: every queue with 32 or more entries
 // is worked off in groups of 32; with `finish`, everything.
-template <bool TOT, typename Sink>
-__device__ __forceinline__ void drain_queues(QuadWarp<TOT> &ws, bool finish, const Sink &sink, int *__restrict__ totals,
+template <bool TOT, int CAP, typename Sink>
+__device__ __forceinline__ void drain_queues(QuadWarp<TOT, CAP> &ws, bool finish, const Sink &sink, int *__restrict__ totals,
                                              int lane)
 {
     QuadQueues<TOT> &Q = ws.q;
@@ -583,15 +588,15 @@ __device__ __forceinline__ void drain_queues(QuadWarp<TOT> &ws, bool finish, con
 // of the depo of lane l is dbase + l, or dbase + dl (of lane l) when the batch comes from an index list (INDIRECT).
 // `flush`: the caller has no more batches (the lanes then carry no depo): every queue is emptied before the call returns.
 // NORMAL_ONLY: the normal-approximation sampler of reading A21 (no inversion branch, no mirror).
-template <bool NORMAL_ONLY, bool TOT, bool INDIRECT, typename Sink>
+template <bool NORMAL_ONLY, bool TOT, bool INDIRECT, int CAP, typename Sink>
 __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Sink &sink, float t0, float x0, float st,
                                                  float sx, float q, bool valid, long long dbase, uint32_t dl,
                                                  uint64_t id_base, uint64_t seed, double nsigma, bool normalize,
-                                                 int *__restrict__ totals, QuadWarp<TOT> &ws, bool flush,
+                                                 int *__restrict__ totals, QuadWarp<TOT, CAP> &ws, bool flush,
                                                  unsigned int &drawn, int lane)
 {
     constexpr bool normal_only = NORMAL_ONLY;
-    QuadScratch &sc = ws.sc;
+    QuadScratch<CAP> &sc = ws.sc;
     QuadQueues<TOT> &Q = ws.q;
     const double T0 = t0, X0 = x0, ST = st, SX = sx;
     Extent et{0, 0}, ex{0, 0};
@@ -601,7 +606,7 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
     }
     const bool live = et.lo < et.hi && ex.lo < ex.hi;
     const int nt = live ? et.hi - et.lo : 0, nx = live ? ex.hi - ex.lo : 0;
-    const bool big = nt + nx + 2 + 2 * kEdgePad > kQuadEdgeCap || nt > 255 || nx > 255;
+    const bool big = nt + nx + 2 + 2 * kEdgePad > CAP || nt > 255 || nx > 255;
     const bool flat = live && !big;
     // quads per wire row: with n_ticks a multiple of 4 every row of a patch starts at the same offset in its quad
     const bool aligned = (g.n_ticks & 3) == 0;
@@ -660,7 +665,7 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
     while (d0 < 32) {
         const int ebase = sc.eoff[d0];
         const unsigned int fits = __ballot_sync(
-            0xffffffffu, lane >= d0 && eincl - ebase + 2 * kEdgePad * (min(lane, kBatchDepos - 1) - d0 + 1) <= kQuadEdgeCap);
+            0xffffffffu, lane >= d0 && eincl - ebase + 2 * kEdgePad * (min(lane, kBatchDepos - 1) - d0 + 1) <= CAP);
         const int d1 = d0 + __popc(fits); // monotone: the fitting lanes are d0 .. d1-1, at least one
         const int etot = sc.eoff[d1] - ebase, qbase = sc.qoff[d0], qtot = sc.qoff[d1] - qbase;
         if (lane >= d0 && lane < d1 && lane < kBatchDepos) sc.rec[lane].ebase = eincl - ne - ebase + 2 * kEdgePad * (lane - d0);
@@ -760,7 +765,7 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
                 __syncwarp();
                 const int4 f = *reinterpret_cast<const int4 *>(Q.fill); // every fill is < 64: bit 5 says "a warp's worth"
                 const bool last = flush_here && k == 3 && s0 + 32 >= qtot;
-                if ((((f.x | f.y) | (f.z | f.w) | Q.fill[kQExact]) & 32) | (int)last) drain_queues<TOT>(ws, last, sink, totals, lane);
+                if ((((f.x | f.y) | (f.z | f.w) | Q.fill[kQExact]) & 32) | (int)last) drain_queues(ws, last, sink, totals, lane);
             }
         }
         __syncwarp();
@@ -775,7 +780,7 @@ struct BatchSmem {
 };
 template <bool TOT>
 struct BatchSmem<true, TOT> {
-    QuadWarp<TOT> warp[kBatchWarps];
+    QuadWarp<TOT, kQuadEdgeCap> warp[kBatchWarps];
 };
 
 // ------------------------------------------------------------------------------------------------------------------
@@ -1016,7 +1021,7 @@ struct TileSmem {
 template <bool TOT>
 struct TileSmem<true, TOT> {
     unsigned long long acc[kTileW * kTileT];
-    QuadWarp<TOT> warp[kTileWarps];
+    QuadWarp<TOT, kTileEdgeCap> warp[kTileWarps];
 };
 
 template <int FLUCT, bool TOT>
