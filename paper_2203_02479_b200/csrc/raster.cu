@@ -467,11 +467,11 @@ struct QuadWarp {
     QuadScratch<CAP> sc;
     QuadQueues<TOT> q;
 };
-// the fills while the queues are drained (registers, uniform over the warp): the four fp32 queues, 8 bits each (kQNorm
-// lowest), and the exact queue.  Between drains the fills live in QuadQueues::fill.
+// the fills while the queues are drained (registers, uniform over the warp): the four fp32 queues (kQNorm .. kQInvC) and
+// the exact queue.  Between drains the fills live in QuadQueues::fill.
 struct QuadCounts {
-    uint32_t fast = 0;
-    int exact = 0;
+    int fast[4];
+    int exact;
 };
 template <bool TOT, int CAP>
 __device__ __forceinline__ void queues_init(QuadWarp<TOT, CAP> &ws, int lane)
@@ -521,9 +521,9 @@ template <int QI, bool TOT, typename Sink>
 __device__ __forceinline__ void drain_fast_group(QuadQueues<TOT> &Q, QuadCounts &qc, const Sink &sink, int *__restrict__ totals,
                                                  int lane)
 {
-    const int fill = (int)((qc.fast >> (8 * QI)) & 0xffu);
+    const int fill = qc.fast[QI];
     const int take = min(32, fill);
-    qc.fast -= (uint32_t)take << (8 * QI);
+    qc.fast[QI] = fill - take;
     const int e = QI * kQueueCap + fill - take + lane;
     bool rej = false;
     if (lane < take) {
@@ -556,29 +556,22 @@ __device__ __forceinline__ void drain_fast_group(QuadQueues<TOT> &Q, QuadCounts 
 // The queues.  Called (from one place) when one of them holds a warp's worth of work: every queue with 32 or more entries
 // is worked off in groups of 32; with `finish`, everything.
 template <bool TOT, int CAP, typename Sink>
-__device__ __forceinline__ void drain_queues(QuadWarp<TOT, CAP> &ws, bool finish, const Sink &sink, int *__restrict__ totals,
-                                             int lane)
+__device__ __forceinline__ void drain_queues(QuadWarp<TOT, CAP> &ws, int4 fills, int fill_exact, bool finish, const Sink &sink,
+                                             int *__restrict__ totals, int lane)
 {
     QuadQueues<TOT> &Q = ws.q;
-    __syncwarp();
-    QuadCounts qc;
-    {
-        const int4 f = *reinterpret_cast<const int4 *>(Q.fill);
-        qc.fast = (uint32_t)f.x | ((uint32_t)f.y << 8) | ((uint32_t)f.z << 16) | ((uint32_t)f.w << 24);
-        qc.exact = Q.fill[kQExact];
-    }
+    QuadCounts qc{{fills.x, fills.y, fills.z, fills.w}, fill_exact}; // what the caller has just read from Q.fill
+    const int due = finish ? 1 : 32; // a queue is due when it holds a warp's worth (finish: anything)
     // the exact queue first if it is what is full: the groups below may each add up to 32 rejected bins to it
     if (qc.exact >= 32) qc.exact = drain_exact<TOT>(&Q, qc.exact, false, sink, totals, lane);
-    const uint32_t thresh = finish ? 0xffffffffu : 0xe0e0e0e0u; // a queue is due when its fill is >= 32 (finish: > 0)
-    while (qc.fast & (0xffu << (8 * kQNorm)) & thresh) drain_fast_group<kQNorm, TOT>(Q, qc, sink, totals, lane);
-    while (qc.fast & (0xffu << (8 * kQInvA)) & thresh) drain_fast_group<kQInvA, TOT>(Q, qc, sink, totals, lane);
-    while (qc.fast & (0xffu << (8 * kQInvB)) & thresh) drain_fast_group<kQInvB, TOT>(Q, qc, sink, totals, lane);
-    while (qc.fast & (0xffu << (8 * kQInvC)) & thresh) drain_fast_group<kQInvC, TOT>(Q, qc, sink, totals, lane);
+    while (qc.fast[kQNorm] >= due) drain_fast_group<kQNorm, TOT>(Q, qc, sink, totals, lane);
+    while (qc.fast[kQInvA] >= due) drain_fast_group<kQInvA, TOT>(Q, qc, sink, totals, lane);
+    while (qc.fast[kQInvB] >= due) drain_fast_group<kQInvB, TOT>(Q, qc, sink, totals, lane);
+    while (qc.fast[kQInvC] >= due) drain_fast_group<kQInvC, TOT>(Q, qc, sink, totals, lane);
     if (qc.exact >= 32 || (finish && qc.exact > 0)) qc.exact = drain_exact<TOT>(&Q, qc.exact, finish, sink, totals, lane);
-    __syncwarp();
+    __syncwarp(); // every lane has read its entries
     if (lane == 0) {
-        *reinterpret_cast<int4 *>(Q.fill) = make_int4((int)(qc.fast & 0xffu), (int)((qc.fast >> 8) & 0xffu),
-                                                       (int)((qc.fast >> 16) & 0xffu), (int)(qc.fast >> 24));
+        *reinterpret_cast<int4 *>(Q.fill) = make_int4(qc.fast[0], qc.fast[1], qc.fast[2], qc.fast[3]);
         Q.fill[kQExact] = qc.exact;
     }
     __syncwarp();
@@ -729,7 +722,7 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
                 w0 = w1, w1 = w2, w2 = w3;
                 const bool v = live_q && (unsigned)(ii0 + k) < (unsigned)nto;
                 double p = __dmul_rn(__dsub_rn(E[k + 1], E[k]), wxq); // = wt wx: the two factors 1/2 are exact scalings
-                if (normalize) p *= inv_n;
+                p = __dmul_rn(p, inv_n); // inv_n = 1 unless patches are renormalised (A24): an exact no-op then
                 const bool all = p >= 1.0; // every electron lands here
                 const bool mirror = !normal_only && p > 0.5 && !all;
                 if (mirror) {
@@ -764,8 +757,9 @@ __device__ __forceinline__ void raster_quad_body(GridDims g, Clip clip, const Si
                 }
                 __syncwarp();
                 const int4 f = *reinterpret_cast<const int4 *>(Q.fill); // every fill is < 64: bit 5 says "a warp's worth"
+                const int fx = Q.fill[kQExact];
                 const bool last = flush_here && k == 3 && s0 + 32 >= qtot;
-                if ((((f.x | f.y) | (f.z | f.w) | Q.fill[kQExact]) & 32) | (int)last) drain_queues(ws, last, sink, totals, lane);
+                if ((((f.x | f.y) | (f.z | f.w) | fx) & 32) | (int)last) drain_queues(ws, f, fx, last, sink, totals, lane);
             }
         }
         __syncwarp();
@@ -849,6 +843,8 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8
         if (!more) break;
         if (++round < n_static) {
             batch += n_warps_grid;
+        } else if (n_static * n_warps_grid >= n_batches) {
+            batch = n_batches; // the static rounds cover every batch: no fetch (one more pass empties the draw queues)
         } else {
             if (lane == 0) batch = n_static * n_warps_grid + (long long)atomicAdd(&counters->next_batch, 1ull);
             batch = __shfl_sync(0xffffffffu, batch, 0);
@@ -918,6 +914,8 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8
         if (!more) break;
         if (++round < n_static) {
             batch += n_warps_grid;
+        } else if (n_static * n_warps_grid >= n_batches) {
+            batch = n_batches; // every batch was assigned statically
         } else {
             if (lane == 0) batch = n_static * n_warps_grid + (long long)atomicAdd(&counters->next_batch, 1ull);
             batch = __shfl_sync(0xffffffffu, batch, 0);
