@@ -374,10 +374,19 @@ def run_ours(args):
         peak = 148 * 64 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
         roofline = {"kernel": "raster_batch_kernel<fluct>", "bound": "alu", "achieved": tflops, "peak": peak,
                     "unit": "TFLOP/s", "frac": tflops / peak, "traffic": TRAFFIC.get("raster") if args.config == 1 else None,
-                    "peak_source": "derived: 148 SMs x 64 fp64 FMA/clk x 2 x %.0f MHz (DESIGN.md); DFMA microbenchmark "
-                                   "reached 56.4 of 64 per clk per SM" % peaks["sm_max_mhz"],
+                    "peak_source": "derived, not measured in this run: 148 SMs x 64 fp64 FMA/clk x 2 x %.0f MHz (DESIGN.md); a DFMA "
+                                   "microbenchmark reached 56.4 of 64 per clk per SM in round 1" % peaks["sm_max_mhz"],
                     "algorithmic": {"bins_per_launch": bins, "fp64_flop_per_bin": FP64_FLOP_PER_BIN,
                                     "bins_per_s": bins / (dom["ms"] * 1e-3)}}
+        # the informative roof (the kernel is issue bound, not fp64 bound): warp-instructions per drawn bin as ncu counted
+        # them on this workload (smsp__inst_executed.sum / bins; profiles/r02_ncu_full.md: 35.77 M / 2,127,063) against 4 per clock per SM
+        issue_peak = 148 * 4 * peaks["sm_max_mhz"] * 1e6
+        issued = bins * WARP_INST_PER_BIN / (dom["ms"] * 1e-3)
+        roofline["issue"] = {"warp_instructions_per_bin": WARP_INST_PER_BIN if args.config == 1 else None,
+                             "achieved_warp_inst_per_s": issued if args.config == 1 else None, "peak_warp_inst_per_s": issue_peak,
+                             "frac": issued / issue_peak if args.config == 1 else None,
+                             "source": "instruction count from the committed ncu capture of configs[1] (a constant here, not "
+                                       "re-measured in this run); peak derived: 148 SMs x 4 schedulers x %.0f MHz" % peaks["sm_max_mhz"]}
     else:
         if dom["stage"] not in sb:
             dom = max((r for r in stage_rows if r["stage"] in sb), key=lambda r: r["ms"])
@@ -437,8 +446,10 @@ def run_ours(args):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1], from the committed `ncu --set full` capture
-# (profiles/r01i_ncu_full.md; cold-cache replays, so reads are compulsory misses and writes mostly stay in L2)
-TRAFFIC = {"raster": 6.03e6, "rows_forward": 19.29e6, "cols": 27.68e6, "rows_inverse": 26.36e6}
+# (profiles/r02_ncu_full.md; cold-cache replays, so reads are compulsory misses and writes mostly stay in L2)
+TRAFFIC = {"raster": 5.96e6, "rows_forward": 19.29e6, "cols": 27.70e6, "rows_inverse": 26.36e6}
+# warp-instructions per drawn bin of the fluctuated raster on configs[1] (ncu: smsp__inst_executed.sum / 2,127,063 bins)
+WARP_INST_PER_BIN = 16.8
 # algorithmic fp64 work per drawn bin of the fluctuated raster (DESIGN.md section 6 derives it from the oracle's steps)
 FP64_FLOP_PER_BIN = 70.0
 # the e2e ADC variant's ideal converter (reading A23): codes per unit of M, and pedestal
