@@ -75,6 +75,8 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
     __syncthreads();
     const int pl = plane_of_row(b.planes, row);
     float2 *dst = b.spec + (size_t)(b.planes.srow0[pl] + row - b.planes.row0[pl]) * b.spec_stride;
+    float2 tws[E];
+    split_twiddles<E>(tws, load_tw(b.tw_real, i)); // exp(-2 pi i k / 2N) at k = i + e NT: one load, 15 constant rotations
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const int k = i + e * NT;
@@ -82,7 +84,7 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
         const float2 zn = smem[smem_index<1>((N - k) & (N - 1), 0)];
         const float2 A = make_float2(0.5f * (zk.x + zn.x), 0.5f * (zk.y - zn.y));
         const float2 B = make_float2(0.5f * (zk.y + zn.y), -0.5f * (zk.x - zn.x));
-        const float2 w = load_tw(b.tw_real, k);
+        const float2 w = tws[e];
         dst[k] = cadd(A, cmul(w, B));
         if (k == 0) dst[N] = make_float2(zk.x - zk.y, 0.f);
     }
@@ -254,6 +256,8 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
     const bool noisy = nz.amp != nullptr;
     const uint32_t wire = (uint32_t)(row - b.planes.row0[plane_of_row(b.planes, row)]); // the noise is keyed by the plane's own wire
     float2 v[E];
+    float2 tws[E];
+    split_twiddles<E>(tws, load_tw(b.tw_real, i)); // exp(-2 pi i k / 2N) at k = i + e NT: one load, 15 constant rotations
     if (use_spec && !noisy) {
         // plain convolution: the partner bin X_{N-k} is read straight from the spectrum row (descending, still
         // coalesced; L1 / L2 hits), which saves the staging stores and a barrier
@@ -264,7 +268,7 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
             if (k == 0) xk.y = 0.f, xn.y = 0.f; // imaginary parts of the DC and Nyquist bins do not reach a real output
             const float2 s = make_float2(xk.x + xn.x, xk.y - xn.y);
             const float2 d = make_float2(xk.x - xn.x, xk.y + xn.y);
-            const float2 w = load_tw(b.tw_real, k); // (cos, -sin)
+            const float2 w = tws[e]; // (cos, -sin)
             const float2 t = make_float2(w.x * d.x + w.y * d.y, w.x * d.y - w.y * d.x);
             v[e] = make_float2(s.x - t.y, s.y + t.x);
         }
@@ -294,7 +298,7 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
             const float2 xn = smem[smem_index<1>(N - k, 0)];
             const float2 s = make_float2(xk.x + xn.x, xk.y - xn.y);
             const float2 d = make_float2(xk.x - xn.x, xk.y + xn.y);
-            const float2 w = load_tw(b.tw_real, k); // (cos, -sin)
+            const float2 w = tws[e]; // (cos, -sin)
             const float2 t = make_float2(w.x * d.x + w.y * d.y, w.x * d.y - w.y * d.x);
             v[e] = make_float2(s.x - t.y, s.y + t.x);
         }
@@ -342,6 +346,8 @@ __global__ void __launch_bounds__(RowTma<N>::threads, RowTma<N>::min_ctas) rows_
     pdl_wait();
     __syncthreads();
     uint32_t parity = 0;
+    float2 tws[E];
+    split_twiddles<E>(tws, load_tw(b.tw_real, i)); // the same for every row this thread works on
     for (; row < g.n_wires; row += gridDim.x) {
         mbar_wait(bar, parity);
         parity ^= 1u;
@@ -372,7 +378,7 @@ __global__ void __launch_bounds__(RowTma<N>::threads, RowTma<N>::min_ctas) rows_
             if (k == 0) xk.y = 0.f, xn.y = 0.f; // imaginary parts of the DC and Nyquist bins do not reach a real output
             const float2 s = make_float2(xk.x + xn.x, xk.y - xn.y);
             const float2 d = make_float2(xk.x - xn.x, xk.y + xn.y);
-            const float2 w = load_tw(b.tw_real, k); // (cos, -sin)
+            const float2 w = tws[e]; // (cos, -sin)
             const float2 t = make_float2(w.x * d.x + w.y * d.y, w.x * d.y - w.y * d.x);
             v[e] = make_float2(s.x - t.y, s.y + t.x);
         }

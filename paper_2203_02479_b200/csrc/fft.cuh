@@ -130,6 +130,34 @@ struct Butterfly<16, DIR> {
     }
 };
 
+// w * exp(-2 pi i e / 32) for a compile-time e in 0..15: the real-row split needs exp(-2 pi i (i + e N/16) / (2N)) =
+// exp(-2 pi i i / (2N)) exp(-2 pi i e / 32) at a thread's 16 points, i.e. one table load and 15 constant rotations instead
+// of 16 loads (the row kernels are bound by the load/store path)
+template <int EIDX>
+WCSIM_HD float2 rot32(float2 w)
+{
+    constexpr float C[16] = {1.0f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
+                             0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f, 0.19509032201612826785f,
+                             0.0f, -0.19509032201612826785f, -0.38268343236508977173f, -0.55557023301960222474f,
+                             -0.70710678118654752440f, -0.83146961230254523708f, -0.92387953251128675613f, -0.98078528040323044913f};
+    constexpr float S[16] = {0.0f, 0.19509032201612826785f, 0.38268343236508977173f, 0.55557023301960222474f,
+                             0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f, 0.98078528040323044913f,
+                             1.0f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
+                             0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f, 0.19509032201612826785f};
+    if constexpr (EIDX == 0) return w;
+    else return make_float2(w.x * C[EIDX] + w.y * S[EIDX], w.y * C[EIDX] - w.x * S[EIDX]); // (a + ib)(c - is)
+}
+// the 16 split twiddles of thread i (E = 16 points per thread): tw[e] = exp(-2 pi i (i + e N/16) / (2N))
+template <int E>
+WCSIM_HD void split_twiddles(float2 (&tw)[E], float2 w0)
+{
+    static_assert(E == 16, "the row kernels keep 16 points per thread");
+    tw[0] = w0;
+    tw[1] = rot32<1>(w0), tw[2] = rot32<2>(w0), tw[3] = rot32<3>(w0), tw[4] = rot32<4>(w0), tw[5] = rot32<5>(w0);
+    tw[6] = rot32<6>(w0), tw[7] = rot32<7>(w0), tw[8] = rot32<8>(w0), tw[9] = rot32<9>(w0), tw[10] = rot32<10>(w0);
+    tw[11] = rot32<11>(w0), tw[12] = rot32<12>(w0), tw[13] = rot32<13>(w0), tw[14] = rot32<14>(w0), tw[15] = rot32<15>(w0);
+}
+
 constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n >> 1); }
 
 // radix of the pass that starts with P points already combined: the first pass takes the odd bits, the rest are 16
@@ -204,12 +232,32 @@ WCSIM_HD void fft_pass(float2 (&v)[E], int i, const float2 *__restrict__ tw)
             const int b = i + u * (N / E);
             const int k = b & (P - 1);
             constexpr int off = tw_offset(N, P);
+#ifdef WCSIM_TW_ALL_LOADS
 #pragma unroll
             for (int r = 1; r < R; ++r) {
                 float2 w = load_tw(tw, off + (r - 1) * P + k);
                 if (DIR > 0) w.y = -w.y;
                 x[r] = cmul(x[r], w);
             }
+#else
+            // The row kernels are bound by the load/store path (L1/TEX 74 % busy in `ncu`), not by arithmetic: only
+            // w^1, w^2, w^4, w^8 are loaded and the other eleven powers are products of them (at most three
+            // multiplications deep: ~2e-7 relative, the size of the transform's own fp32 rounding).
+            float2 w[R];
+#pragma unroll
+            for (int r = 1; r < R; r <<= 1) {
+                w[r] = load_tw(tw, off + (r - 1) * P + k);
+                if (DIR > 0) w[r].y = -w[r].y;
+            }
+            w[3] = cmul(w[1], w[2]);
+            w[5] = cmul(w[1], w[4]);
+            w[6] = cmul(w[2], w[4]);
+            w[7] = cmul(w[3], w[4]);
+#pragma unroll
+            for (int r = 1; r < 8; ++r) w[8 + r] = cmul(w[r], w[8]);
+#pragma unroll
+            for (int r = 1; r < R; ++r) x[r] = cmul(x[r], w[r]);
+#endif
         }
         Butterfly<R, DIR>::run(x);
 #pragma unroll
