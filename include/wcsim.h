@@ -7,7 +7,7 @@
  * S is built from "ionization electron groups" (depos) by the Raster and Scatter-add tasks of
  * PAPER.md:54-58 (Section 2.2); the convolution follows the FFT route of PAPER.md:46-52 (Eq. 2);
  * N is the optional electronics-noise term of Eq. (1), model from BASELINE.json configs[3].
- * Where the paper is silent the readings A1..A20 of DESIGN.md apply; each call names the ones it uses.
+ * Where the paper is silent the readings A1..A25 of DESIGN.md apply; each call names the ones it uses.
  *
  * Conventions
  *   - Grids are wire-major, tick fastest: S[wire * n_ticks + tick], fp32.  Bin k covers [k, k+1) on both axes (A1).

@@ -3,6 +3,8 @@
     python -m paper_2203_02479_b200.build [--force] [--verbose]
 
 The library links only against the (static) CUDA runtime; torch is not involved.
+WCSIM_NVCC_FLAGS in the environment adds nvcc flags (developer knob for the -DWCSIM_* experiment macros of csrc/: batch size,
+CTAs per SM, edge scratch, wire-pass tiling; the defaults are the measured optima recorded in DESIGN.md section 12).
 """
 from __future__ import annotations
 
