@@ -7,6 +7,7 @@
 // in fp64, rounded once to fp32 (units: cm, us, D in cm^2/s).  A group behind a plane gets NaN fields there, which the
 // raster skips and counts.  HBM bound: 20 B in, 20 B out per group and plane.
 #include "internal.h"
+#include "pdl.cuh"
 
 namespace wcsim {
 
@@ -61,7 +62,30 @@ __global__ void __launch_bounds__(256) digitize_kernel(const float *__restrict__
     }
 }
 
+// S = 0 as a kernel (not a memset node), so that the raster that follows is its programmatic dependent: the raster's CTAs
+// are resident and through their prologue when the last stores of the clear land.  Persistent: a few CTAs per SM stride
+// over the grid with 16-byte stores.
+__global__ void __launch_bounds__(256) clear_kernel(float4 *__restrict__ p, long long n4, float *__restrict__ tail, int n_tail)
+{
+    pdl_trigger();
+    pdl_wait(); // whoever used the grid before (the previous plane-event's forward rows) is done with it
+    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (long long)gridDim.x * blockDim.x) p[i] = z;
+    if (blockIdx.x == 0 && (int)threadIdx.x < n_tail) tail[threadIdx.x] = 0.f;
+}
+
 } // namespace
+
+cudaError_t launch_clear(float *p, long long n, int sm_count, cudaStream_t st)
+{
+    if (n <= 0) return cudaSuccess;
+    const long long n4 = n / 4; // cudaMalloc'ed: 16-byte aligned
+    long long ctas = (n4 + 255) / 256;
+    const long long cap = (long long)sm_count * 8;
+    if (ctas > cap) ctas = cap;
+    if (ctas < 1) ctas = 1;
+    return launch_pdl(clear_kernel, (unsigned)ctas, 256, 0, st, reinterpret_cast<float4 *>(p), n4, p + 4 * n4, (int)(n - 4 * n4));
+}
 
 cudaError_t launch_digitize(const float *M, long long n, float gain, float baseline, int bits, short *adc, cudaStream_t st)
 {

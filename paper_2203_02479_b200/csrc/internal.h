@@ -160,6 +160,8 @@ struct DriftPlanes {
     DriftPlane plane[kMaxDriftPlanes];
 };
 cudaError_t launch_drift(DriftInputs in, long long n, DriftParams prm, DriftPlanes planes, cudaStream_t st);
+// p[0..n) = 0 by a kernel launched as a programmatic dependent (the raster after it overlaps its launch with the clear's tail)
+cudaError_t launch_clear(float *p, long long n, int sm_count, cudaStream_t st);
 // ideal ADC of reading A23: adc[i] = clamp(rint(M[i] gain + baseline), 0, 2^bits - 1); M 16-byte, adc 8-byte aligned
 cudaError_t launch_digitize(const float *M, long long n, float gain, float baseline, int bits, short *adc, cudaStream_t st);
 

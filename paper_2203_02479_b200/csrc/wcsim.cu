@@ -683,7 +683,8 @@ int wcsim_clear(wcsim_plan *plan)
 {
     if (!plan) return WCSIM_EINVAL;
     DeviceGuard guard(plan->device);
-    CU_TRY(cudaMemsetAsync(plan->S, 0, sizeof(float) * (size_t)plan->s_wires * plan->n_ticks, plan->stream));
+    CU_TRY(launch_clear(plan->S, (long long)plan->s_wires * plan->n_ticks, plan->sm_count, plan->stream));
+    plan->launches += 1;
     return WCSIM_OK;
 }
 

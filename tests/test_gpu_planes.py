@@ -124,7 +124,7 @@ def test_config_3_event_through_one_launch_sequence(B, O):
         plan.sync()
         S = plan.charge().cpu().numpy()
         M = plan.output().cpu().numpy()
-        assert plan.launch_count() == 4  # raster, forward rows, wire pass, inverse rows: one launch each for three planes
+        assert plan.launch_count() == 5  # clear, raster, forward rows, wire pass, inverse rows: one launch each for three planes
         for p, pl in enumerate(planes):
             r0, nw = plan.plane_rows(p)
             S_ref, _, st = O.raster_scatter(nw, nt, pl["depos"], seed=cfg["fluct_seed"], fluctuate=True, nsigma=cfg["nsigma"])
@@ -171,7 +171,7 @@ def test_graph_replays_a_plane_event(B, O):
         graph.launch()
         graph.launch()
         plan.sync()
-        assert plan.launch_count() == launches0 + 2 * 5
+        assert plan.launch_count() == launches0 + 2 * 6  # clear, raster, three convolution kernels, digitize
         assert np.array_equal(plan.output().cpu().numpy(), M_direct)
         assert np.array_equal(adc.cpu().numpy(), adc_direct)
         # a new event in the same arrays
