@@ -168,7 +168,11 @@ __global__ void __launch_bounds__(ColCfg<N>::threads) cols_kernel(GridDims g, Co
 #ifndef WCSIM_WIRES_RG
 #define WCSIM_WIRES_RG 8
 #endif
-constexpr int kWiresD = 7, kWiresRG = WCSIM_WIRES_RG, kWiresO = 8;
+#ifndef WCSIM_WIRES_D
+#define WCSIM_WIRES_D 7
+#endif
+constexpr int kWiresD = WCSIM_WIRES_D, kWiresRG = WCSIM_WIRES_RG, kWiresO = 8;
+constexpr int kWiresNch21 = (21 + kWiresD - 1) / kWiresD, kWiresNch41 = (41 + kWiresD - 1) / kWiresD; // chunks of BASELINE.json's widths
 constexpr int kWiresCtas = WCSIM_WIRES_CTAS; // resident CTAs per SM the register budget is set for
 
 // STRIDE = 0: row stride read from the buffers (any pad_t); NCH = 0: chunk count read from the buffers (any n_rw),
@@ -543,15 +547,15 @@ cudaError_t launch_wires(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st)
     constexpr int O = kWiresO;
     const int nk = pad_t / 2 + 1;
     const dim3 block(32, kWiresRG), grid((nk + 31) / 32, b.planes.grp0[b.planes.n]); // row groups of all planes
-    // BASELINE.json's paddings and response widths (21 wires -> 3 chunks, 41 -> 6) get immediate-offset loads and an
+    // BASELINE.json's paddings and response widths (21 wires -> 3 chunks of 7 offsets, 41 -> 6) get immediate-offset loads and an
     // unrolled chunk loop; anything else takes the generic instance
     const int key = b.impact_K == 1 ? b.rt_rows / kWiresD * 100000 + b.spec_stride : -1;
     const int tail = pdl_tail_from((long long)grid.x * grid.y, (long long)b.sm_count * kWiresCtas);
     cudaError_t err = cudaSuccess;
     switch (key) {
-    case 3 * 100000 + 1024 / 2 + 8: err = launch_pdl(wires_kernel<O, kWiresD, 3, 1024 / 2 + 8>, grid, block, 0, st, g, b, nk, tail); break;
-    case 3 * 100000 + 8192 / 2 + 8: err = launch_pdl(wires_kernel<O, kWiresD, 3, 8192 / 2 + 8>, grid, block, 0, st, g, b, nk, tail); break;
-    case 6 * 100000 + 16384 / 2 + 8: err = launch_pdl(wires_kernel<O, kWiresD, 6, 16384 / 2 + 8>, grid, block, 0, st, g, b, nk, tail); break;
+    case kWiresNch21 * 100000 + 1024 / 2 + 8: err = launch_pdl(wires_kernel<O, kWiresD, kWiresNch21, 1024 / 2 + 8>, grid, block, 0, st, g, b, nk, tail); break;
+    case kWiresNch21 * 100000 + 8192 / 2 + 8: err = launch_pdl(wires_kernel<O, kWiresD, kWiresNch21, 8192 / 2 + 8>, grid, block, 0, st, g, b, nk, tail); break;
+    case kWiresNch41 * 100000 + 16384 / 2 + 8: err = launch_pdl(wires_kernel<O, kWiresD, kWiresNch41, 16384 / 2 + 8>, grid, block, 0, st, g, b, nk, tail); break;
     default: err = launch_pdl(wires_kernel<O, kWiresD, 0, 0>, grid, block, 0, st, g, b, nk, tail); break;
     }
     return err != cudaSuccess ? err : cudaGetLastError();
