@@ -327,7 +327,7 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel --------------------------------------------------------------------------
     peaks = load_peaks()
-    direct = args.impact > 1 or args.wires == "direct" or (args.wires == "auto" and pl["response"].shape[-2] <= (32 if pl["pad_w"] <= 512 else 52 if pl["pad_w"] <= 2048 else 112))
+    direct = args.impact > 1 or args.wires == "direct" or (args.wires == "auto" and pl["response"].shape[-2] <= (32 if pl["pad_w"] <= 512 else 45 if pl["pad_w"] <= 2048 else 100))
     sb = stage_bytes(pl, direct, args.impact)
     stage_rows = []
     for name in ("raster", "rows_forward", "cols", "rows_inverse"):

@@ -48,7 +48,7 @@ typedef enum wcsim_status {
 
 /* wire_mode of wcsim_set_wire_mode: how wcsim_convolve treats the wire axis of Eq. (2).  Both give the same M up to
  * fp32 rounding (the cropped result is the linear convolution either way). */
-#define WCSIM_WIRES_AUTO 0   /* direct up to the measured crossover width (32 / 52 / 112 response wires for wire paddings
+#define WCSIM_WIRES_AUTO 0   /* direct up to the measured crossover width (32 / 45 / 100 response wires for wire paddings
                                 <= 512 / <= 2048 / larger), FFT beyond (default) */
 #define WCSIM_WIRES_FFT 1    /* pad_w-point FFT, multiply by Rhat(w_t, w_x), inverse FFT: Eq. (2) literally */
 #define WCSIM_WIRES_DIRECT 2 /* tick axis by FFT, wire axis by direct summation over the n_rwires response offsets:

@@ -216,8 +216,9 @@ inline void build_pass_twiddles(int n, float2 *out)
     }
 }
 
-// One pass: twiddle + butterflies on the registers.
-template <int N, int E, int R, int P, int DIR>
+// One pass: twiddle + butterflies on the registers.  TWP: form eleven of the fifteen twiddles of a butterfly as products of
+// the other four instead of loading all fifteen.
+template <int N, int E, int R, int P, int DIR, bool TWP = true>
 WCSIM_HD void fft_pass(float2 (&v)[E], int i, const float2 *__restrict__ tw)
 {
     constexpr int NB = E / R;
@@ -232,32 +233,32 @@ WCSIM_HD void fft_pass(float2 (&v)[E], int i, const float2 *__restrict__ tw)
             const int b = i + u * (N / E);
             const int k = b & (P - 1);
             constexpr int off = tw_offset(N, P);
-#ifdef WCSIM_TW_ALL_LOADS
+            if constexpr (!TWP) {
 #pragma unroll
-            for (int r = 1; r < R; ++r) {
-                float2 w = load_tw(tw, off + (r - 1) * P + k);
-                if (DIR > 0) w.y = -w.y;
-                x[r] = cmul(x[r], w);
+                for (int r = 1; r < R; ++r) {
+                    float2 w = load_tw(tw, off + (r - 1) * P + k);
+                    if (DIR > 0) w.y = -w.y;
+                    x[r] = cmul(x[r], w);
+                }
+            } else {
+                // The row kernels are bound by the load/store path (L1/TEX 74 % busy in `ncu`), not by arithmetic: only
+                // w^1, w^2, w^4, w^8 are loaded and the other eleven powers are products of them (at most three
+                // multiplications deep: ~2e-7 relative, the size of the transform's own fp32 rounding).
+                float2 w[R];
+#pragma unroll
+                for (int r = 1; r < R; r <<= 1) {
+                    w[r] = load_tw(tw, off + (r - 1) * P + k);
+                    if (DIR > 0) w[r].y = -w[r].y;
+                }
+                w[3] = cmul(w[1], w[2]);
+                w[5] = cmul(w[1], w[4]);
+                w[6] = cmul(w[2], w[4]);
+                w[7] = cmul(w[3], w[4]);
+#pragma unroll
+                for (int r = 1; r < 8; ++r) w[8 + r] = cmul(w[r], w[8]);
+#pragma unroll
+                for (int r = 1; r < R; ++r) x[r] = cmul(x[r], w[r]);
             }
-#else
-            // The row kernels are bound by the load/store path (L1/TEX 74 % busy in `ncu`), not by arithmetic: only
-            // w^1, w^2, w^4, w^8 are loaded and the other eleven powers are products of them (at most three
-            // multiplications deep: ~2e-7 relative, the size of the transform's own fp32 rounding).
-            float2 w[R];
-#pragma unroll
-            for (int r = 1; r < R; r <<= 1) {
-                w[r] = load_tw(tw, off + (r - 1) * P + k);
-                if (DIR > 0) w[r].y = -w[r].y;
-            }
-            w[3] = cmul(w[1], w[2]);
-            w[5] = cmul(w[1], w[4]);
-            w[6] = cmul(w[2], w[4]);
-            w[7] = cmul(w[3], w[4]);
-#pragma unroll
-            for (int r = 1; r < 8; ++r) w[8 + r] = cmul(w[r], w[8]);
-#pragma unroll
-            for (int r = 1; r < R; ++r) x[r] = cmul(x[r], w[r]);
-#endif
         }
         Butterfly<R, DIR>::run(x);
 #pragma unroll
@@ -297,7 +298,10 @@ __device__ __forceinline__ void fft_block(float2 (&v)[E], float2 *smem, int i, i
                                           bool sync_first)
 {
     constexpr int R = PassRadix<N, P>::value;
-    fft_pass<N, E, R, P, DIR>(v, i, tw);
+    // twiddles by products where loads are what binds: the row transforms (a warp's lanes are 32 different k) and the long
+    // column transforms; the short column transforms (few distinct k per warp: cheap loads) keep their 15 loads
+    // (measured: 512-point columns 13.5 us with loads, 17.4 us with products; 1024: 55.6 / 47.5 us; 4096: 598 / 528 us)
+    fft_pass<N, E, R, P, DIR, (C == 1 || N >= 1024)>(v, i, tw);
     if constexpr (P * R < N) {
         if (P > 1 || sync_first) __syncthreads();
         fft_store<N, C, E, R, P>(v, smem, i, c);

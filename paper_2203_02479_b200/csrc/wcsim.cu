@@ -152,12 +152,12 @@ int next_pow2(long long n, int floor_)
 // Wire axis of the convolution: direct summation over the response's wire offsets, or FFT / multiply / inverse FFT.
 // Per output the direct form costs 4 n_rw FMAs, the FFT form a pad_w-point transform pair plus the read of Rhat.  AUTO
 // takes the direct form up to the MEASURED crossover (profiles/r02_wire_crossover.md: both routes timed for response
-// widths 21..193 at three plane sizes): 49 wires at pad_w = 1024 (FFT wins from 57), 97 at pad_w = 4096 (FFT from 129),
-// 21 at pad_w = 512 (FFT from 41).
+// widths 21..129 at three plane sizes): direct wins up to 41 wires at pad_w = 1024 (FFT from 49), up to 97 at pad_w = 4096
+// (FFT from 129), at 21 for pad_w = 512 (FFT from 41).
 bool wires_direct(const wcsim_plan *p)
 {
     if (p->wire_mode == WCSIM_WIRES_AUTO) {
-        const int crossover = p->pad_w <= 512 ? 32 : p->pad_w <= 2048 ? 52 : 112;
+        const int crossover = p->pad_w <= 512 ? 32 : p->pad_w <= 2048 ? 45 : 100;
         return p->multi || p->impact_K > 1 || p->n_rw <= crossover;
     }
     return p->wire_mode == WCSIM_WIRES_DIRECT;
