@@ -125,3 +125,25 @@ def test_configs1_sized_plane_with_ten_impact_positions(B, O):
     assert flipped <= FLIP_BUDGET * st["drawn"] and stats["bins_drawn"] == st["drawn"]
     assert st["drawn"] / d["t0"].shape[0] > 100  # patches of O(20 x 20) / O(26 x 8) bins
     check_close(M, O.convolve_impact(S_ref, R, K), "impact K=10 configs[1]-sized M")
+
+
+def test_impact_plan_with_noise_host_buffers_and_adc(B, O):
+    """the accessories on an impact-position plan: fused noise (keyed by the wire, not the fine row), the host-buffer call
+    and the ADC codes"""
+    from paper_2203_02479_b200 import synth
+    rng = np.random.default_rng(77)
+    K, nw, nt = 3, 50, 640
+    R = synth.response_impact(K, 7, 40)
+    d = fine_depos(rng, 2500, nw, nt, K)
+    host_M = torch.empty((nw, nt), dtype=torch.float32).pin_memory()
+    host_adc = torch.empty((nw, nt), dtype=torch.int16).pin_memory()
+    with B.ImpactPlan(nw, nt, R) as plan:
+        plan.simulate_host({k: torch.from_numpy(v) for k, v in d.items()}, host_M, seed=5, fluctuate=True, noise=True, noise_seed=8)
+        S_ref, _, _ = O.raster_scatter(nw * K, nt, d, seed=5, fluctuate=True)
+        M_ref = O.convolve_impact(S_ref, R, K) + O.noise_add(np.zeros((nw, nt)), plan.pad_t, 8)
+        check_close(host_M.numpy(), M_ref, "impact K=3 host call M + N")
+        plan.simulate_host_adc_async({k: torch.from_numpy(v) for k, v in d.items()}, host_adc, 0.02, 500.0, 12, seed=5,
+                                     fluctuate=True, noise=True, noise_seed=8)
+        plan.sync()
+        assert np.array_equal(host_adc.numpy(), O.digitize(plan.output().cpu().numpy(), 0.02, 500.0, 12))
+        assert np.array_equal(plan.output().cpu().numpy(), host_M.numpy())  # the same plane-event twice: bitwise stable

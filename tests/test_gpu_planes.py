@@ -300,3 +300,47 @@ def test_armed_custom_spectrum_survives_a_later_add_noise(B, O):
         N1 = p.output().cpu().numpy()
     check_close(N2, O.noise_add(np.zeros((nw, nt)), P, seed=7, amp=amp2.astype(np.float64)), "add_noise amp2")
     check_close(N1, O.noise_add(np.zeros((nw, nt)), P, seed=5, amp=amp1.astype(np.float64)), "armed amp1 after add_noise amp2")
+
+
+def test_planes_api_limits_and_single_plane(B, O):
+    """wcsim_raster_scatter_planes on an ordinary (one-plane) plan equals wcsim_raster_scatter bit for bit; 8 planes are the
+    limit, 9 and 0 are refused; a plane may have no depos at all"""
+    from paper_2203_02479_b200 import synth
+    cfg = synth.config(1, n_depos=3000)
+    pl = cfg["planes"][0]
+    nw, nt, R = 120, 900, synth.response(5, 24)
+    d = {k: v.copy() for k, v in pl["depos"].items()}
+    d["x0"] = (d["x0"] * (nw / 800.0)).astype(np.float32)
+    d["t0"] = (d["t0"] * (nt / 6000.0)).astype(np.float32)
+    dev = to_dev(d)
+    with B.Plan(nw, nt, R) as p:
+        p.clear()
+        p.raster_scatter(dev, seed=3, fluctuate=True)
+        p.sync()
+        S1 = p.charge().cpu().numpy().copy()
+        p.clear()
+        p.raster_scatter_planes([dev], seed=3, fluctuate=True)
+        p.sync()
+        assert np.array_equal(p.charge().cpu().numpy(), S1)
+    S_ref, _, st = O.raster_scatter(nw, nt, d, seed=3, fluctuate=True)
+    assert int(np.count_nonzero(S1.astype(np.float64) != S_ref)) <= FLIP_BUDGET * st["drawn"]
+    with B.PlanesPlan([nw] * 8, nt, [R] * 8) as p8:
+        empty = {k: torch.empty(0, dtype=torch.float32, device="cuda") for k in dev}
+        p8.clear()
+        p8.raster_scatter_planes([dev, empty, dev, empty, empty, empty, empty, dev], seed=3, fluctuate=True)
+        p8.convolve()
+        p8.sync()
+        S8 = p8.charge().cpu().numpy()
+        M8 = p8.output().cpu().numpy()
+        M_ref = O.convolve_direct(S_ref, R)
+        for q in range(8):
+            r0, n = p8.plane_rows(q)
+            assert (r0, n) == (q * nw, nw)
+            if q in (0, 2, 7):
+                assert np.array_equal(S8[r0:r0 + n], S1)
+                check_close(M8[r0:r0 + n], M_ref, "8-plane plan, plane %d" % q)
+            else:
+                assert not S8[r0:r0 + n].any() and not M8[r0:r0 + n].any()  # an empty plane stays empty: no leak across the halos
+    for bad in (0, 9):
+        with pytest.raises((B.WcsimError, ValueError)):
+            B.PlanesPlan([nw] * bad, nt, [R] * bad)
