@@ -1,15 +1,17 @@
 // raster.cu -- steps a1-a3 of the hot path: Raster, charge fluctuation, Scatter-add
 // (Section 2.2; Section 3.1 for the binomial fluctuation).
 //
-// Both scatter modes run raster_batch_body: a warp takes a batch of 8 depos, one per lane (the SoA layout of PAPER.md:72
-// makes the depo the unit of parallelism and the loads coalesce; lanes 8..31 own none).  Each owning lane works out its
-// depo's patch extent, clipped to the batch's window (the grid, or a tile of it); a warp scan lays all bin EDGES of the
-// batch's patches end to end and all 32 lanes evaluate erf over that flat list ("erf bin edges once per axis"; own
-// table erf, erf_table.cuh), leaving the values in the warp's shared-memory scratch; then the lanes walk the flat list
-// of all BINS of the batch, 32 at a time, each forming p_ij = wt_i wx_j from four edge values.  All lanes are busy
-// whatever the patch shapes are (patches are 1-5 wires x 1-16 ticks in BASELINE.json's configs).  With fluctuation on,
-// bins are first sorted by the routine that will draw them (inversion in three mu bands / AS 241 central / AS 241
-// tail) into five per-warp queues and drawn 32 at a time from one queue, so the fp64 sampler runs without divergence.
+// Every scatter mode runs the same batch bodies (raster_flat_body with fluctuation off, raster_quad_body with it on): a warp
+// takes a batch of 16 depos, one per lane (the SoA layout of PAPER.md:72 makes the depo the unit of parallelism and the
+// loads coalesce; lanes 16..31 own none).  Each owning lane works out its depo's patch extent, clipped to the batch's
+// window (the plane, or a tile of it); a warp scan lays all bin EDGES of the batch's patches end to end and all 32 lanes
+// evaluate erf over that flat list ("erf bin edges once per axis"; own table erf, erf_table.cuh), leaving the values in
+// the warp's shared-memory scratch; then the lanes walk the flat list of the batch's BINS (fluctuation off) or QUADS
+// (on: aligned groups of four absolute bins, one Philox call each), 32 at a time, forming p_ij = wt_i wx_j from four edge
+// values.  All lanes are busy whatever the patch shapes are (patches are 1-5 wires x 1-16 ticks in BASELINE.json's
+// configs).  With fluctuation on, bins are sorted by the routine that will draw them (rounded normal / inversion in three
+// mu bands / exact) into five per-warp shared-memory queues and drawn 32 at a time from one queue by straight-line code:
+// guarded fp32 estimates first (rng.cuh), the fp64 routines for the ~1 % of bins a guard does not accept.
 // A patch with more edges than the scratch holds falls back to the one-warp-per-depo walk (raster_depo), which chunks
 // it.  Nothing of a patch is ever written to HBM except the final adds into S.
 //
@@ -21,12 +23,16 @@
 //   fluctuate = 1: fp64 weights (erf), p = wt * wx, integer draw B(N, p; Philox word of the absolute bin)
 //   fluctuate = 2: the same with the normal-approximation draw of the paper's Kokkos port (reading A21)
 //
-// Two scatter modes:
-//   atomic: raster_batch_kernel, persistent warps fetching batches from a device counter (guided: 8 depos, then 2 at a
-//           time near the end), red.global.add.f32 straight into S
-//   tiled : depos are grouped by the grid tiles their patch overlaps (count / scan / fill), one CTA per tile runs the
-//           batch body over its depos, clipped to the tile, accumulating in shared memory in 2^-24 fixed point
-//           (integer adds: order independent, so the result is bitwise reproducible) and adds the tile to S once.
+// Scatter modes:
+//   atomic: raster_batch_kernel, persistent warps: two batches by the warp's index in the grid, then batches of 4 depos
+//           from a device counter (guided scheduling); fp32 reductions (REDG.E.ADD.F32) straight into S.
+//           raster_planes_kernel: the same for the stacked planes of a multi-plane plan, one launch for all planes.
+//   fixed : the atomic kernel adding in 2^-24 fixed point into a 64-bit grid (integer reductions: order independent, so the
+//           result is bitwise reproducible), folded into S by tile_finalize_kernel.
+//   tiled : depos are listed under the (at most 4) grid tiles their patch overlaps (count / scan / fill), up to 8 CTAs per
+//           tile run the batch body over its depos, clipped to the tile, accumulating in shared memory in 2^-24 fixed point
+//           and adding the tile into the fixed-point grid once; patches over more than 4 tiles go through the atomic kernel
+//           into the same grid; everything stream-ordered.
 #include "internal.h"
 #include "erf_table.cuh"
 #include "pdl.cuh"
