@@ -26,13 +26,24 @@ namespace wcsim {
 
 namespace {
 
-template <int N>
+template <int N, bool FORWARD = true>
 struct RowCfg {
-    static constexpr int E = 16;
+    // 8192-point FORWARD rows (pad_t = 16384, configs[4]): 32 points per thread and a radix-32 first pass, 32.16.16: two
+    // shared-memory exchanges instead of the three of 2.16.16.16 (the row transforms are bound by the load/store path):
+    // 84.8 -> 74.1 us.  The inverse rows lose with it (92.5 -> 100.6 us: their staging of the partner bins doubles per
+    // thread too) and keep 16 points per thread.
+#ifdef WCSIM_ROWS_NO_R32
+    static constexpr bool r32 = false;
+#else
+    static constexpr bool r32 = FORWARD && N == 8192;
+#endif
+    static constexpr int E = r32 ? 32 : 16;
     static constexpr int threads = N / E;
     static constexpr int smem_bytes = SmemSize<N, 1>::float2s * (int)sizeof(float2);
-    // 64 registers per thread: 1024 threads of row transforms resident per SM whatever the row length
-    static constexpr int min_ctas = threads >= 1024 ? 1 : (1024 / threads > 8 ? 8 : 1024 / threads);
+    // 64 registers per thread (E = 16): 1024 threads of row transforms resident per SM whatever the row length;
+    // 128 registers with 32 points per thread: 512 threads
+    static constexpr int per_sm_threads = r32 ? 512 : 1024;
+    static constexpr int min_ctas = threads >= per_sm_threads ? 1 : (per_sm_threads / threads > 8 ? 8 : per_sm_threads / threads);
 };
 template <int N>
 struct ColCfg {
@@ -66,7 +77,7 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
             v[e].y = (2 * pt + 1 < g.n_ticks) ? src[2 * pt + 1] : 0.f;
         }
     }
-    fft_block<N, 1, E, -1>(v, smem, i, 0, b.tw_row, false);
+    fft_block<N, 1, E, -1, 1, RowCfg<N>::r32>(v, smem, i, 0, b.tw_row, false);
     // split Z = FFT(even + i odd) into the spectrum of the real row:
     //   A = (Z_k + conj Z_{N-k})/2, B = (Z_k - conj Z_{N-k})/(2i), X_k = A + exp(-2 pi i k / 2N) B
     __syncthreads();
@@ -99,9 +110,9 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
 // its row straight into registers, and four 64-register CTAs per SM beat three 80-register ones.)
 template <int N>
 struct RowTma {
-    static constexpr int threads = RowCfg<N>::threads;
+    static constexpr int threads = RowCfg<N, false>::threads;
     static constexpr int min_ctas = threads <= 256 ? 3 : (threads <= 512 ? 2 : 1);
-    static constexpr int work_bytes = (RowCfg<N>::smem_bytes + 127) / 128 * 128;
+    static constexpr int work_bytes = (RowCfg<N, false>::smem_bytes + 127) / 128 * 128;
     static constexpr bool enabled = N <= 4096 && N >= 512;
     static int smem_bytes(int stage_bytes) { return work_bytes + (stage_bytes + 127) / 128 * 128 + 16; }
     static int grid(int rows, int stage_bytes, int sm_count)
@@ -263,10 +274,10 @@ __device__ __forceinline__ float2 noise_bin(const NoiseArgs &nz, uint32_t wire, 
 }
 
 template <int N, bool VEC>
-__global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_inverse_kernel(GridDims g, ConvBuffers b, NoiseArgs nz,
+__global__ void __launch_bounds__(RowCfg<N, false>::threads, RowCfg<N, false>::min_ctas) rows_inverse_kernel(GridDims g, ConvBuffers b, NoiseArgs nz,
                                                                            bool use_spec, bool accumulate)
 {
-    constexpr int E = RowCfg<N>::E, NT = N / E;
+    constexpr int E = RowCfg<N, false>::E, NT = N / E;
     extern __shared__ float2 smem[];
     const int row = blockIdx.x, i = threadIdx.x;
     pdl_wait(); // a no-op unless launched as a programmatic dependent
@@ -290,7 +301,7 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
             const float2 t = make_float2(w.x * d.x + w.y * d.y, w.x * d.y - w.y * d.x);
             v[e] = make_float2(s.x - t.y, s.y + t.x);
         }
-        fft_block<N, 1, E, +1>(v, smem, i, 0, b.tw_row, false);
+        fft_block<N, 1, E, +1, 1, RowCfg<N, false>::r32>(v, smem, i, 0, b.tw_row, false);
     } else {
         // stage X_k (+ noise) in shared memory so that every thread can reach the partner X_{N-k}
 #pragma unroll
@@ -320,7 +331,7 @@ __global__ void __launch_bounds__(RowCfg<N>::threads, RowCfg<N>::min_ctas) rows_
             const float2 t = make_float2(w.x * d.x + w.y * d.y, w.x * d.y - w.y * d.x);
             v[e] = make_float2(s.x - t.y, s.y + t.x);
         }
-        fft_block<N, 1, E, +1>(v, smem, i, 0, b.tw_row, true);
+        fft_block<N, 1, E, +1, 1, RowCfg<N, false>::r32>(v, smem, i, 0, b.tw_row, true);
     }
     float *dst = b.M + (size_t)row * g.n_ticks;
 #pragma unroll
@@ -346,7 +357,7 @@ template <int N>
 __global__ void __launch_bounds__(RowTma<N>::threads, RowTma<N>::min_ctas) rows_inverse_tma_kernel(GridDims g, ConvBuffers b,
                                                                                                    NoiseArgs nz)
 {
-    constexpr int E = RowCfg<N>::E, NT = N / E;
+    constexpr int E = RowCfg<N, false>::E, NT = N / E;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *smem = reinterpret_cast<float2 *>(smem_raw);
     const uint32_t row_bytes = (uint32_t)b.spec_stride * 8u; // whole stride: a multiple of 64
@@ -407,7 +418,7 @@ __global__ void __launch_bounds__(RowTma<N>::threads, RowTma<N>::min_ctas) rows_
             mbar_arrive_expect_tx(bar, row_bytes);
             bulk_copy_g2s(stage, b.spec_inv + (size_t)next * b.spec_stride, row_bytes, bar);
         }
-        fft_block<N, 1, E, +1>(v, smem, i, 0, b.tw_row, false);
+        fft_block<N, 1, E, +1, 1, RowCfg<N, false>::r32>(v, smem, i, 0, b.tw_row, false);
         float2 *dst = reinterpret_cast<float2 *>(b.M + (size_t)row * g.n_ticks);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
@@ -479,8 +490,8 @@ cudaError_t conv_configure(int pad_w, int pad_t)
     case NN:                                                                                                           \
         if (err == cudaSuccess) err = set_smem(rows_forward_kernel<NN, true>, RowCfg<NN>::smem_bytes);                 \
         if (err == cudaSuccess) err = set_smem(rows_forward_kernel<NN, false>, RowCfg<NN>::smem_bytes);                \
-        if (err == cudaSuccess) err = set_smem(rows_inverse_kernel<NN, true>, RowCfg<NN>::smem_bytes);                 \
-        if (err == cudaSuccess) err = set_smem(rows_inverse_kernel<NN, false>, RowCfg<NN>::smem_bytes);                \
+        if (err == cudaSuccess) err = set_smem(rows_inverse_kernel<NN, true>, RowCfg<NN, false>::smem_bytes);                 \
+        if (err == cudaSuccess) err = set_smem(rows_inverse_kernel<NN, false>, RowCfg<NN, false>::smem_bytes);                \
         if (err == cudaSuccess) err = configure_tma<NN>();                                                             \
         break;
         WCSIM_ROW_SIZES(X)
@@ -509,12 +520,11 @@ static bool rows_vectorisable(GridDims g, const void *p)
 cudaError_t launch_rows_forward(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st)
 {
     const bool vec = rows_vectorisable(g, b.S);
-    const int threads = pad_t / 32 > 0 ? pad_t / 32 : 1; // 64 registers: 1024 threads of row transforms per SM
-    const int per_sm = threads >= 1024 ? 1 : (1024 / threads > 8 ? 8 : 1024 / threads);
-    const int tail = pdl_tail_from(g.n_wires, (long long)b.sm_count * per_sm);
+    int tail = 0; // first CTA of the last wave (pdl.cuh): from the resident CTAs per SM of this row length
     switch (pad_t / 2) {
 #define X(NN)                                                                                                          \
     case NN:                                                                                                           \
+        tail = pdl_tail_from(g.n_wires, (long long)b.sm_count * RowCfg<NN>::min_ctas);                                 \
         if (vec)                                                                                                       \
             launch_pdl(rows_forward_kernel<NN, true>, g.n_wires, RowCfg<NN>::threads, RowCfg<NN>::smem_bytes, st, g, b, tail); \
         else                                                                                                           \
@@ -585,10 +595,10 @@ cudaError_t launch_rows_inverse(GridDims g, int pad_t, ConvBuffers b, NoiseArgs 
         if (use_spec && !accumulate && inverse_tma_ok<NN>(g, b))                                                       \
             launch_inverse_tma<NN>(g, b, noise, st);                                                                   \
         else if (vec)                                                                                                  \
-            rows_inverse_kernel<NN, true><<<g.n_wires, RowCfg<NN>::threads, RowCfg<NN>::smem_bytes, st>>>(             \
+            rows_inverse_kernel<NN, true><<<g.n_wires, RowCfg<NN, false>::threads, RowCfg<NN, false>::smem_bytes, st>>>(             \
                 g, b, noise, use_spec, accumulate);                                                                    \
         else                                                                                                           \
-            rows_inverse_kernel<NN, false><<<g.n_wires, RowCfg<NN>::threads, RowCfg<NN>::smem_bytes, st>>>(            \
+            rows_inverse_kernel<NN, false><<<g.n_wires, RowCfg<NN, false>::threads, RowCfg<NN, false>::smem_bytes, st>>>(            \
                 g, b, noise, use_spec, accumulate);                                                                    \
         break;
         WCSIM_ROW_SIZES(X)

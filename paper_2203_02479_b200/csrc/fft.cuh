@@ -133,7 +133,7 @@ struct Butterfly<16, DIR> {
 // w * exp(-2 pi i e / 32) for a compile-time e in 0..15: the real-row split needs exp(-2 pi i (i + e N/16) / (2N)) =
 // exp(-2 pi i i / (2N)) exp(-2 pi i e / 32) at a thread's 16 points, i.e. one table load and 15 constant rotations instead
 // of 16 loads (the row kernels are bound by the load/store path)
-template <int EIDX>
+template <int EIDX, int DIR = -1>
 WCSIM_HD float2 rot32(float2 w)
 {
     constexpr float C[16] = {1.0f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
@@ -145,34 +145,86 @@ WCSIM_HD float2 rot32(float2 w)
                              1.0f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
                              0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f, 0.19509032201612826785f};
     if constexpr (EIDX == 0) return w;
-    else return make_float2(w.x * C[EIDX] + w.y * S[EIDX], w.y * C[EIDX] - w.x * S[EIDX]); // (a + ib)(c - is)
+    else if constexpr (DIR < 0) return make_float2(w.x * C[EIDX] + w.y * S[EIDX], w.y * C[EIDX] - w.x * S[EIDX]); // (a + ib)(c - is)
+    else return make_float2(w.x * C[EIDX] - w.y * S[EIDX], w.y * C[EIDX] + w.x * S[EIDX]);                         // (a + ib)(c + is)
 }
-// the 16 split twiddles of thread i (E = 16 points per thread): tw[e] = exp(-2 pi i (i + e N/16) / (2N))
-template <int E>
+// w * exp(-2 pi i e / 64) for a compile-time e in 0..31 (the split twiddles of a thread that keeps 32 points)
+template <int EIDX>
+WCSIM_HD float2 rot64(float2 w)
+{
+    constexpr float C[32] = {1.0f, 0.99518472667219688624f, 0.98078528040323044913f, 0.95694033573220886494f,
+                             0.92387953251128675613f, 0.88192126434835502971f, 0.83146961230254523708f, 0.77301045336273696081f,
+                             0.70710678118654752440f, 0.63439328416364549822f, 0.55557023301960222474f, 0.47139673682599764856f,
+                             0.38268343236508977173f, 0.29028467725446236764f, 0.19509032201612826785f, 0.09801714032956060199f,
+                             0.0f, -0.09801714032956060199f, -0.19509032201612826785f, -0.29028467725446236764f,
+                             -0.38268343236508977173f, -0.47139673682599764856f, -0.55557023301960222474f, -0.63439328416364549822f,
+                             -0.70710678118654752440f, -0.77301045336273696081f, -0.83146961230254523708f, -0.88192126434835502971f,
+                             -0.92387953251128675613f, -0.95694033573220886494f, -0.98078528040323044913f, -0.99518472667219688624f};
+    constexpr float S[32] = {0.0f, 0.09801714032956060199f, 0.19509032201612826785f, 0.29028467725446236764f,
+                             0.38268343236508977173f, 0.47139673682599764856f, 0.55557023301960222474f, 0.63439328416364549822f,
+                             0.70710678118654752440f, 0.77301045336273696081f, 0.83146961230254523708f, 0.88192126434835502971f,
+                             0.92387953251128675613f, 0.95694033573220886494f, 0.98078528040323044913f, 0.99518472667219688624f,
+                             1.0f, 0.99518472667219688624f, 0.98078528040323044913f, 0.95694033573220886494f,
+                             0.92387953251128675613f, 0.88192126434835502971f, 0.83146961230254523708f, 0.77301045336273696081f,
+                             0.70710678118654752440f, 0.63439328416364549822f, 0.55557023301960222474f, 0.47139673682599764856f,
+                             0.38268343236508977173f, 0.29028467725446236764f, 0.19509032201612826785f, 0.09801714032956060199f};
+    if constexpr (EIDX == 0) return w;
+    else return make_float2(w.x * C[EIDX] + w.y * S[EIDX], w.y * C[EIDX] - w.x * S[EIDX]);
+}
+// the E split twiddles of thread i (E = 16 or 32 points per thread): tw[e] = exp(-2 pi i (i + e N/E) / (2N))
+template <int E, int I = 0>
 WCSIM_HD void split_twiddles(float2 (&tw)[E], float2 w0)
 {
-    static_assert(E == 16, "the row kernels keep 16 points per thread");
-    tw[0] = w0;
-    tw[1] = rot32<1>(w0), tw[2] = rot32<2>(w0), tw[3] = rot32<3>(w0), tw[4] = rot32<4>(w0), tw[5] = rot32<5>(w0);
-    tw[6] = rot32<6>(w0), tw[7] = rot32<7>(w0), tw[8] = rot32<8>(w0), tw[9] = rot32<9>(w0), tw[10] = rot32<10>(w0);
-    tw[11] = rot32<11>(w0), tw[12] = rot32<12>(w0), tw[13] = rot32<13>(w0), tw[14] = rot32<14>(w0), tw[15] = rot32<15>(w0);
+    static_assert(E == 16 || E == 32, "the row kernels keep 16 or 32 points per thread");
+    if constexpr (I < E) {
+        if constexpr (E == 16) tw[I] = rot32<I>(w0);
+        else tw[I] = rot64<I>(w0);
+        split_twiddles<E, I + 1>(tw, w0);
+    }
 }
+
+// radix 32 from two radix-16 transforms of the even and odd inputs: X[q] = E_q + W32^q O_q, X[q+16] = E_q - W32^q O_q
+template <int DIR, int Q = 0>
+WCSIM_HD void combine32(float2 (&x)[32], const float2 (&ev)[16], const float2 (&od)[16])
+{
+    if constexpr (Q < 16) {
+        const float2 t = rot32<Q, DIR>(od[Q]);
+        x[Q] = cadd(ev[Q], t);
+        x[Q + 16] = csub(ev[Q], t);
+        combine32<DIR, Q + 1>(x, ev, od);
+    }
+}
+template <int DIR>
+struct Butterfly<32, DIR> {
+    static WCSIM_HD void run(float2 (&x)[32])
+    {
+        float2 ev[16], od[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) ev[q] = x[2 * q], od[q] = x[2 * q + 1];
+        Butterfly<16, DIR>::run(ev);
+        Butterfly<16, DIR>::run(od);
+        combine32<DIR>(x, ev, od);
+    }
+};
 
 constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n >> 1); }
 
-// radix of the pass that starts with P points already combined: the first pass takes the odd bits, the rest are 16
-template <int N, int P>
+// radix of the pass that starts with P points already combined: the first pass takes the odd bits, the rest are 16.
+// R32 (threads that keep 32 points): a single odd bit is not spent on a radix-2 pass with a shared-memory exchange of its
+// own but folded into a radix-32 first pass (N = 2.16.16.16 becomes 32.16.16: one exchange fewer).
+template <int N, int P, bool R32 = false>
 struct PassRadix {
     static constexpr int rem = ilog2(N) % 4;
-    static constexpr int value = (P == 1 && rem != 0) ? (1 << rem) : 16;
+    static constexpr int value = (P == 1 && rem != 0) ? ((R32 && rem == 1) ? 32 : (1 << rem)) : 16;
 };
 
 // shared-memory index (in float2 units) of point pt of column c: one float2*C of padding after every 16 points,
 // which spreads the radix-strided writes of the first passes over all banks
-template <int C>
+// (SH = 5: one float2 after every 32 points, for the exchange that follows a radix-32 pass)
+template <int C, int SH = 4>
 WCSIM_HD int smem_index(int pt, int c)
 {
-    return (pt + (pt >> 4)) * C + c;
+    return (pt + (pt >> SH)) * C + c;
 }
 template <int N, int C>
 struct SmemSize {
@@ -267,7 +319,7 @@ WCSIM_HD void fft_pass(float2 (&v)[E], int i, const float2 *__restrict__ tw)
 }
 
 // Stockham scatter of a finished pass into shared memory: butterfly b, output r goes to point (b-k)R + k + rP
-template <int N, int C, int E, int R, int P>
+template <int N, int C, int E, int R, int P, int SH = 4>
 WCSIM_HD void fft_store(const float2 (&v)[E], float2 *smem, int i, int c)
 {
     constexpr int NB = E / R;
@@ -277,37 +329,38 @@ WCSIM_HD void fft_store(const float2 (&v)[E], float2 *smem, int i, int c)
         const int k = b & (P - 1);
         const int j = (b - k) * R + k;
 #pragma unroll
-        for (int r = 0; r < R; ++r) smem[smem_index<C>(j + r * P, c)] = v[u + r * NB];
+        for (int r = 0; r < R; ++r) smem[smem_index<C, SH>(j + r * P, c)] = v[u + r * NB];
     }
 }
 
 // gather of the next pass's inputs: points i + e*(N/E)
-template <int N, int C, int E>
+template <int N, int C, int E, int SH = 4>
 WCSIM_HD void fft_load(float2 (&v)[E], const float2 *smem, int i, int c)
 {
 #pragma unroll
-    for (int e = 0; e < E; ++e) v[e] = smem[smem_index<C>(i + e * (N / E), c)];
+    for (int e = 0; e < E; ++e) v[e] = smem[smem_index<C, SH>(i + e * (N / E), c)];
 }
 
 #ifdef __CUDACC__
 // Whole transform from registers to registers (device only: uses __syncthreads).  On entry v holds the input at
 // points i + e*(N/E); on exit it holds the transform at the same points.  `smem` has SmemSize<N,C>::float2s
 // entries.  SYNC_FIRST: set when other threads may still be reading `smem` from earlier work.
-template <int N, int C, int E, int DIR, int P = 1>
+template <int N, int C, int E, int DIR, int P = 1, bool R32 = false>
 __device__ __forceinline__ void fft_block(float2 (&v)[E], float2 *smem, int i, int c, const float2 *__restrict__ tw,
                                           bool sync_first)
 {
-    constexpr int R = PassRadix<N, P>::value;
+    constexpr int R = PassRadix<N, P, R32>::value;
+    constexpr int SH = R32 ? 5 : 4;
     // twiddles by products where loads are what binds: the row transforms (a warp's lanes are 32 different k) and the long
     // column transforms; the short column transforms (few distinct k per warp: cheap loads) keep their 15 loads
     // (measured: 512-point columns 13.5 us with loads, 17.4 us with products; 1024: 55.6 / 47.5 us; 4096: 598 / 528 us)
     fft_pass<N, E, R, P, DIR, (C == 1 || N >= 1024)>(v, i, tw);
     if constexpr (P * R < N) {
         if (P > 1 || sync_first) __syncthreads();
-        fft_store<N, C, E, R, P>(v, smem, i, c);
+        fft_store<N, C, E, R, P, SH>(v, smem, i, c);
         __syncthreads();
-        fft_load<N, C, E>(v, smem, i, c);
-        fft_block<N, C, E, DIR, P * R>(v, smem, i, c, tw, true);
+        fft_load<N, C, E, SH>(v, smem, i, c);
+        fft_block<N, C, E, DIR, P * R, R32>(v, smem, i, c, tw, true);
     }
 }
 #endif

@@ -10,11 +10,12 @@
 
 using namespace wcsim;
 
-template <int N, int C, int E, int DIR, int P>
+template <int N, int C, int E, int DIR, int P, bool R32 = false>
 static void emulate(std::vector<float2> &regs, std::vector<float2> &smem, const float2 *tw)
 {
     constexpr int NT = (N / E) * C;
-    constexpr int R = PassRadix<N, P>::value;
+    constexpr int R = PassRadix<N, P, R32>::value;
+    constexpr int SH = R32 ? 5 : 4;
     for (int t = 0; t < NT; ++t) {
         float2(&v)[E] = *reinterpret_cast<float2(*)[E]>(&regs[(size_t)t * E]);
         fft_pass<N, E, R, P, DIR>(v, t / C, tw);
@@ -23,17 +24,17 @@ static void emulate(std::vector<float2> &regs, std::vector<float2> &smem, const 
         for (auto &s : smem) s = make_float2(NAN, NAN);
         for (int t = 0; t < NT; ++t) {
             float2(&v)[E] = *reinterpret_cast<float2(*)[E]>(&regs[(size_t)t * E]);
-            fft_store<N, C, E, R, P>(v, smem.data(), t / C, t % C);
+            fft_store<N, C, E, R, P, SH>(v, smem.data(), t / C, t % C);
         }
         for (int t = 0; t < NT; ++t) {
             float2(&v)[E] = *reinterpret_cast<float2(*)[E]>(&regs[(size_t)t * E]);
-            fft_load<N, C, E>(v, smem.data(), t / C, t % C);
+            fft_load<N, C, E, SH>(v, smem.data(), t / C, t % C);
         }
-        emulate<N, C, E, DIR, P * R>(regs, smem, tw);
+        emulate<N, C, E, DIR, P * R, R32>(regs, smem, tw);
     }
 }
 
-template <int N, int C, int E, int DIR>
+template <int N, int C, int E, int DIR, bool R32 = false>
 static double check()
 {
     constexpr int NT = (N / E) * C;
@@ -49,7 +50,7 @@ static double check()
             int pt = t / C + e * (N / E), c = t % C;
             regs[(size_t)t * E + e] = make_float2((float)xr[(size_t)pt * C + c], (float)xi[(size_t)pt * C + c]);
         }
-    emulate<N, C, E, DIR, 1>(regs, smem, tw.data());
+    emulate<N, C, E, DIR, 1, R32>(regs, smem, tw.data());
     double err = 0.0, nrm = 0.0;
     for (int c = 0; c < C; ++c)
         for (int t = 0; t < NT; ++t) {
@@ -69,7 +70,7 @@ static double check()
             }
         }
     double rel = sqrt(err / nrm);
-    printf("N=%d C=%d E=%d DIR=%d rel_l2=%.3e\n", N, C, E, DIR, rel);
+    printf("N=%d C=%d E=%d DIR=%d R32=%d rel_l2=%.3e\n", N, C, E, DIR, (int)R32, rel);
     return rel;
 }
 
@@ -92,6 +93,11 @@ int main()
     upd(check<64, 1, 32, -1>());
     upd(check<8192, 1, 16, +1>());
     upd(check<8192, 1, 32, -1>());
+    // the radix-32 first pass of the 8192-point row transforms (32.16.16, padding after every 32 points)
+    upd(check<8192, 1, 32, -1, true>());
+    upd(check<8192, 1, 32, +1, true>());
+    upd(check<32, 1, 32, -1, true>());
+    upd(check<512, 1, 32, +1, true>());
     printf("worst=%.3e\n", worst);
     return worst < 2e-6 ? 0 : 1;
 }
