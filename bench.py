@@ -139,7 +139,12 @@ def run_ours(args):
     replicas.init("nccl")
     B.lib()  # fails loudly here if libwcsim.so cannot be built or loaded
 
-    cfg = synth.config(args.config, sigma_scale=args.sigma_scale) if args.sigma_scale != 1.0 else synth.config(args.config)
+    kw = {}
+    if args.sigma_scale != 1.0:
+        kw["sigma_scale"] = args.sigma_scale
+    if args.shuffle:
+        kw["shuffle"] = True  # the depo order as a sensitivity (generation order is the default)
+    cfg = synth.config(args.config, **kw)
     pl = cfg["planes"][0]
     n_depos = int(pl["depos"]["t0"].shape[0])
     fluct = bool(cfg["fluctuate"]) and not args.no_fluct
@@ -406,6 +411,7 @@ def run_ours(args):
                                (", noise fused (plane 0 timed)" if noisy else "") +
                                (", LARGE-PATCH VARIANT sigma x %g (not one of the five configs)" % args.sigma_scale
                                 if args.sigma_scale != 1.0 else "") +
+                               (", depos in SHUFFLED order (sensitivity run)" if args.shuffle else "") +
                                (", IMPACT-POSITION VARIANT: %d impact positions per wire, reading A25 (not one of the five "
                                 "configs)" % args.impact if args.impact > 1 else ""),
                    "grid": [pl["n_wires"], pl["n_ticks"]], "pad": [pl["pad_w"], pl["pad_t"]],
@@ -735,6 +741,8 @@ def main():
                     help="sampler of the fluctuated raster: reading A6 (headline) or the Kokkos port's normal approximation (A21)")
     ap.add_argument("--sigma-scale", type=float, default=1.0,
                     help="labelled large-patch variant of configs[1]/[2] (reading A19): widths multiplied by this factor")
+    ap.add_argument("--shuffle", action="store_true",
+                    help="sensitivity run (SURVEY 8d): the depos in a random order instead of generation order (tracks consecutive)")
     ap.add_argument("--impact", type=int, default=1,
                     help="labelled variant (reading A25): impact positions per wire; depos and response are re-expressed on the finer grid")
     ap.add_argument("--streams", type=int, default=3, help="plane-events in flight for the extra `concurrent` figure")
