@@ -682,6 +682,15 @@ def cpu_baseline(cfg, budget_s=15.0):
            "ms_per_step": dt * 1e3 / reps,
            "sample": "%d whole plane-events of the same workload (all %d depos, full grid), fp64, "
                      "FFT-route convolution" % (reps, n_depos)}
+    # per stage, all cores (one plane-event): raster + fluctuation + serial scatter, FFT-route convolution
+    pl = cfg["planes"][0]
+    t0 = time.perf_counter()
+    S, _, _ = O.raster_scatter(pl["n_wires"], pl["n_ticks"], pl["depos"], seed=cfg["fluct_seed"],
+                               fluctuate=cfg["fluctuate"], nsigma=cfg["nsigma"])
+    t1 = time.perf_counter()
+    O.convolve_fft(S, pl["response"], pl["pad_w"], pl["pad_t"])
+    t2 = time.perf_counter()
+    out["stages_ms"] = {"raster_scatter": (t1 - t0) * 1e3, "convolve_fft": (t2 - t1) * 1e3}
     # one thread, what the paper's CPU-ref was: one plane-event
     O.set_num_threads(1)
     t0 = time.perf_counter()
