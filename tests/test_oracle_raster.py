@@ -230,3 +230,77 @@ def test_normalized_fluctuation_mean():
     assert abs(tot.mean() - 8000.0) < 4 * np.sqrt(8000.0 / 400)
     S0, tot0, _ = oracle.raster_scatter(64, 256, one, seed=9, fluctuate=True, normalize=False, want_totals=True)
     assert tot0.mean() < tot.mean() - 2  # without it the charge beyond the extent (0.06 % here) is truncated away
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the fluctuated branch of wco_raster_scatter, rebuilt bin by bin from its already-pinned pieces
+# (readings A5, A7, A8)
+# ---------------------------------------------------------------------------------------------------------------
+def _fluct_pin_depos():
+    rng = np.random.default_rng(41)
+    n = 30
+    d = {"t0": rng.uniform(2.0, 45.0, n), "x0": rng.uniform(1.0, 11.0, n), "sigma_t": rng.uniform(0.3, 2.5, n),
+         "sigma_x": rng.uniform(0.2, 1.2, n), "q": rng.lognormal(np.log(5000), 0.5, n)}
+    d["q"][1::4] *= -1.0            # negative charge: the sign is carried, N comes from |q|
+    d["q"][2], d["q"][3], d["q"][4], d["q"][5] = 0.5, 0.2, 1.5, -0.5   # N = 1, 0, 2, 1 (round half up on |q|)
+    d["q"][6] = 2.4999              # N = 2, where floor(|q|) and floor(|q| + 1/2) still agree ...
+    d["q"][7] = 7.5                 # ... and N = 8, where they do not
+    d["sigma_t"][8] = 0.0           # sigma = 0 on one axis, on the other, on both (A4)
+    d["sigma_x"][9] = 0.0
+    d["sigma_t"][10] = d["sigma_x"][10] = 0.0
+    d["t0"][11], d["x0"][11] = 0.4, 0.3       # patch leaves the grid at the low corner (A5)
+    d["t0"][12], d["x0"][12] = 47.7, 11.8     # and at the high corner
+    d["t0"][13] = -20.0                       # wholly outside: nothing drawn
+    d["q"][14] = 2.0e5                        # mu >= 16 in many bins: the rounded-normal branch of B
+    return {k: v.astype(np.float32) for k, v in d.items()}
+
+
+@pytest.mark.parametrize("fluctuate,normalize", [(1, False), (2, False), (1, True), (2, True)])
+@pytest.mark.parametrize("explicit_ids", [False, True])
+def test_fluctuated_scatter_rebuilt_bin_by_bin(fluctuate, normalize, explicit_ids):
+    n_wires, n_ticks, seed = 12, 48, 0x1234567887654321
+    d = _fluct_pin_depos()
+    n = d["t0"].shape[0]
+    if explicit_ids:
+        ids = (np.arange(n, dtype=np.uint64) * np.uint64(1_000_003) + np.uint64((1 << 40) + 17))[::-1].copy()
+        kw = dict(ids=ids)
+    else:
+        ids = np.arange(n, dtype=np.uint64) + np.uint64((1 << 40) + 17)
+        kw = dict(id_base=(1 << 40) + 17)
+    S, tot, st = oracle.raster_scatter(n_wires, n_ticks, d, seed=seed, fluctuate=fluctuate, normalize=normalize,
+                                       want_totals=True, **kw)
+    draw = oracle.binomial if fluctuate == 1 else oracle.normal_draw
+    S_ref = np.zeros((n_wires, n_ticks))
+    tot_ref = np.zeros(n, dtype=np.int64)
+    drawn = 0
+    for k in range(n):
+        t0, x0, s_t, s_x, q = (float(d[key][k]) for key in ("t0", "x0", "sigma_t", "sigma_x", "q"))
+        it0, ix0, wt, wx = oracle.patch_axes(t0, x0, s_t, s_x)
+        N = math.floor(abs(q) + 0.5)
+        sign = -1.0 if q < 0 else 1.0
+        norm = 1.0
+        if normalize:  # A24: the telescoped sum over the whole extent, outside bins included
+            for c, s, i0, w in ((t0, s_t, it0, wt), (x0, s_x, ix0, wx)):
+                if s >= 1e-6:
+                    norm *= 0.5 * (math.erf((i0 + len(w) - c) / (math.sqrt(2.0) * s)) - math.erf((i0 - c) / (math.sqrt(2.0) * s)))
+        for j, wxj in enumerate(wx):
+            wire = ix0 + j
+            if not 0 <= wire < n_wires:
+                continue
+            for i, wti in enumerate(wt):
+                tick = it0 + i
+                if not 0 <= tick < n_ticks:
+                    continue
+                p = wti * wxj
+                if normalize:
+                    p = p / norm
+                c = sign * draw(N, p, oracle.fluct_word(seed, int(ids[k]), wire * n_ticks + tick))
+                S_ref[wire, tick] += c
+                tot_ref[k] += int(c)
+                drawn += 1
+    assert np.array_equal(S, S_ref)
+    assert np.array_equal(tot.astype(np.int64), tot_ref)
+    assert st["drawn"] == drawn and st["skipped"] == 0
+    # the cases are really there: a zero-N depo, a depo off the grid, negative bins, a big bin (the draws of a depo's
+    # bins are independent, reading A6, so a one-electron depo may total more than 1)
+    assert tot_ref[3] == 0 and tot_ref[13] == 0 and (S_ref < 0).any() and S_ref.max() > 1000
