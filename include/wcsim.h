@@ -33,7 +33,8 @@ typedef enum wcsim_status {
                           n_wires * n_ticks >= 2^30 */
     WCSIM_ENOMEM = -2, /* host or device allocation failed */
     WCSIM_ECUDA = -3,  /* a CUDA runtime call or kernel failed; wcsim_last_cuda_error() gives the cudaError_t */
-    WCSIM_ESTATE = -4  /* call not valid in the plan's current state */
+    WCSIM_ESTATE = -4, /* call not valid in the plan's current state */
+    WCSIM_ETOOBIG = -5 /* wcsim_raster_scatter_noalloc only: n_wires * n_ticks exceeds WCSIM_NOALLOC_MAX_BINS */
 } wcsim_status;
 
 /* scatter_mode of wcsim_plan_create */
@@ -254,6 +255,53 @@ int wcsim_plan_create_impact(wcsim_plan **out, int n_wires, int n_ticks, int n_i
                              int n_rwires, int n_rticks, int pad_ticks, float nsigma, int scatter_mode, void *cuda_stream);
 /* rows and ticks of the charge grid S (rows = n_wires * n_impact; the stacked rows of a multi-plane plan) */
 int wcsim_get_charge_dims(const wcsim_plan *plan, int *rows, int *n_ticks, int *n_impact);
+
+/*
+ * Raster + fluctuation + scatter-add WITHOUT any device allocation, and without a plan (creating a plan allocates).
+ *
+ * For callers that cannot call cudaMalloc at the point where they need the charge grid: a plug-in of a host framework
+ * that owns all device memory and forbids driver allocations while its event loop runs (an allocation takes a
+ * device-wide lock and can synchronise every stream in the process, stalling the framework's other work), a
+ * latency-bound acquisition thread that may not block in the driver, or a job so close to the memory limit that a late
+ * allocation could fail.  Such a caller owns S (carved out of its own arena) and passes it in; the one thing the kernel
+ * needs besides its inputs and outputs -- a 64-bit fixed-point accumulation grid of one word per bin plus a 256-byte
+ * counter block -- is built into the library as a fixed device array instead of being allocated.
+ *
+ * The cost and the limit: that array is WCSIM_NOALLOC_MAX_BINS words (4 MiB) + 256 bytes, and every GPU on which the
+ * process uses CUDA with libwcsim.so loaded holds it from then until the process exits, used or not.  A grid with
+ * n_wires * n_ticks > WCSIM_NOALLOC_MAX_BINS is refused with WCSIM_ETOOBIG (nothing is enqueued, nothing is allocated to
+ * make room); use a plan for larger grids.
+ *
+ * What it computes: exactly wcsim_raster_scatter on a plan in WCSIM_SCATTER_FIXED mode -- same kernel, same readings,
+ * same Philox keys, bitwise reproducible -- on the device that is current on the calling thread:
+ *     dev_S[wire * n_ticks + tick] += patch of every depo            (dev_S accumulates; the caller zeroes it when it wants)
+ *   n_wires, n_ticks : the charge grid, n_wires * n_ticks <= WCSIM_NOALLOC_MAX_BINS.
+ *   depos            : HOST struct of five DEVICE pointers, n floats each, caller-owned, read.
+ *   depo_id_base, seed, fluctuate : as wcsim_raster_scatter (0 off, 1 binomial, 2 normal approximation).
+ *   nsigma           : patch half-width in sigmas, > 0 (3 in all BASELINE.json configs).
+ *   dev_S            : DEVICE, n_wires * n_ticks floats, caller-owned, read and written.
+ *   cuda_stream      : the work is enqueued on it (memset of the scratch, raster kernel, fold into S) and the call returns.
+ * Invalid depos (non-finite field, negative sigma) are skipped as everywhere else; their count is not available here
+ * (there is no plan to ask), and there are no per-depo totals.
+ *
+ * First call on each device: it looks up the built-in array's device address, uploads the raster's erf table and sets
+ * kernel attributes, and for that it synchronises cuda_stream once.  Make that first call (n = 1 on a scratch S will do)
+ * during start-up, before the no-allocation phase and before any stream capture is begun on cuda_stream.  Later calls
+ * only enqueue.
+ *
+ * Sharing: all calls on a device use the same built-in array, whatever their stream or thread.  Each call zeroes the
+ * part it uses before its kernel runs, so stale contents of an earlier (even a failed) call never leak into S; but two
+ * calls whose GPU work overlaps -- different streams, or different host threads on different streams -- write the same
+ * words at once and corrupt each other's S.  Keep all calls on one stream, or order them with events.
+ *
+ * Errors: WCSIM_EINVAL (NULL dev_S or depo pointer with n > 0, non-positive dims, n < 0, fluctuate outside 0..2,
+ * nsigma <= 0), WCSIM_ETOOBIG, WCSIM_ECUDA (wcsim_last_cuda_error is not updated by this call).  n = 0 returns WCSIM_OK
+ * without touching the device.  Calls no cudaMalloc, cudaFree, or any library routine that allocates.
+ */
+#define WCSIM_NOALLOC_MAX_BINS 524288 /* e.g. 64 x 8192, 128 x 4096, 256 x 2048; configs[0] (64 x 512) is 1/16 of it */
+int wcsim_raster_scatter_noalloc(int n_wires, int n_ticks, const wcsim_depos *depos, long long n,
+                                 unsigned long long depo_id_base, unsigned long long seed, int fluctuate, float nsigma,
+                                 float *dev_S, void *cuda_stream);
 
 /*
  * CUDA graphs (a small plane-event is bound by launch latency).  Between wcsim_graph_begin and

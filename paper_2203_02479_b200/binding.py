@@ -13,7 +13,8 @@ import numpy as np
 
 from . import build as _build
 
-WCSIM_OK, WCSIM_EINVAL, WCSIM_ENOMEM, WCSIM_ECUDA, WCSIM_ESTATE = 0, -1, -2, -3, -4
+WCSIM_OK, WCSIM_EINVAL, WCSIM_ENOMEM, WCSIM_ECUDA, WCSIM_ESTATE, WCSIM_ETOOBIG = 0, -1, -2, -3, -4, -5
+WCSIM_NOALLOC_MAX_BINS = 524288  # include/wcsim.h
 WCSIM_SCATTER_ATOMIC, WCSIM_SCATTER_TILED, WCSIM_SCATTER_FIXED = 0, 1, 2
 WCSIM_WIRES_AUTO, WCSIM_WIRES_FFT, WCSIM_WIRES_DIRECT = 0, 1, 2
 
@@ -27,6 +28,7 @@ SYMBOLS = [
     "wcsim_debug_fast_normal", "wcsim_debug_z32_scan",
     "wcsim_plan_create_planes", "wcsim_raster_scatter_planes", "wcsim_get_plane_rows", "wcsim_simulate_host_adc_async",
     "wcsim_plan_create_impact", "wcsim_get_charge_dims",
+    "wcsim_raster_scatter_noalloc",
     "wcsim_graph_begin", "wcsim_graph_end", "wcsim_graph_launch", "wcsim_graph_destroy",
     "wcsim_strerror", "wcsim_last_cuda_error", "wcsim_version",
 ]
@@ -109,6 +111,7 @@ def lib():
         L.wcsim_simulate_host_adc_async.argtypes = [vp, vp, vp, vp, vp, vp, ll, ull, i, i, ull, C.c_float, C.c_float, i, vp]
         L.wcsim_plan_create_impact.argtypes = [C.POINTER(vp), i, i, i, C.POINTER(vp), i, i, i, C.c_float, i, vp]
         L.wcsim_get_charge_dims.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(i)]
+        L.wcsim_raster_scatter_noalloc.argtypes = [i, i, C.POINTER(wcsim_depos), ll, ull, ull, i, C.c_float, vp, vp]
         L.wcsim_graph_begin.argtypes = [vp]
         L.wcsim_graph_end.argtypes = [vp, C.POINTER(vp)]
         L.wcsim_graph_launch.argtypes = [vp]
@@ -197,6 +200,30 @@ def wcsim_raster_scatter(plan, depos, n=None, depo_id_base=0, seed=0, fluctuate=
     st = lib().wcsim_raster_scatter(plan, C.byref(d), int(n), int(depo_id_base), int(seed), _fluct(fluctuate),
                                     _dev_ptr(dev_depo_totals, torch.int32))
     _check(st, "wcsim_raster_scatter")
+
+
+def wcsim_raster_scatter_noalloc(n_wires, n_ticks, depos, dev_S, n=None, depo_id_base=0, seed=0, fluctuate=False,
+                                 nsigma=3.0, stream=None):
+    """Raster + scatter-add into the caller's own grid, for code that may not allocate device memory (no plan, no
+    cudaMalloc: the kernel's scratch is a fixed 4 MiB array built into libwcsim.so).  dev_S: torch CUDA float32 tensor of
+    n_wires * n_ticks elements, accumulated into.  Grids above WCSIM_NOALLOC_MAX_BINS bins raise WcsimError
+    (WCSIM_ETOOBIG).  The first call on a device synchronises `stream` once; calls that overlap on the GPU race on the
+    shared scratch (include/wcsim.h has the full contract)."""
+    import torch
+    get = (lambda k: depos[k]) if isinstance(depos, dict) else (lambda k: getattr(depos, k))
+    arrs = [get(k) for k in ("t0", "x0", "sigma_t", "sigma_x", "q")]
+    if n is None:
+        n = arrs[0].numel()
+    for a in arrs:
+        if a.numel() < n:
+            raise ValueError("depo array shorter than n")
+    if dev_S is not None and dev_S.numel() < int(n_wires) * int(n_ticks):
+        raise ValueError("dev_S holds fewer than n_wires * n_ticks floats")
+    d = wcsim_depos(*[_dev_ptr(a, torch.float32) for a in arrs])
+    st = lib().wcsim_raster_scatter_noalloc(int(n_wires), int(n_ticks), C.byref(d), int(n), int(depo_id_base), int(seed),
+                                            _fluct(fluctuate), float(nsigma), _dev_ptr(dev_S, torch.float32),
+                                            _stream_ptr(stream))
+    _check(st, "wcsim_raster_scatter_noalloc")
 
 
 def wcsim_convolve(plan):

@@ -19,7 +19,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 OBJ_DIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libwcsim.so")
-SOURCES = ["wcsim.cu", "raster.cu", "convolve.cu", "response.cu", "drift.cu"]
+SOURCES = ["wcsim.cu", "raster.cu", "convolve.cu", "response.cu", "drift.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
               "--expt-relaxed-constexpr", "-Wno-deprecated-gpu-targets"]
 

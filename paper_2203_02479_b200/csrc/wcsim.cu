@@ -1058,6 +1058,9 @@ const char *wcsim_strerror(int status)
     case WCSIM_ENOMEM: return "out of host or device memory";
     case WCSIM_ECUDA: return "CUDA runtime or kernel failure (see wcsim_last_cuda_error)";
     case WCSIM_ESTATE: return "call not valid in the plan's current state";
+    case WCSIM_ETOOBIG:
+        return "grid larger than the built-in scratch of wcsim_raster_scatter_noalloc (n_wires * n_ticks > "
+               "WCSIM_NOALLOC_MAX_BINS = 524288); nothing was allocated or enqueued -- use a plan for this size";
     default: return "unknown wcsim status";
     }
 }

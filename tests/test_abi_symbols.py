@@ -44,6 +44,10 @@ def test_argument_errors_need_no_device():
                              3.0, 0, None)
     assert st == binding.WCSIM_EINVAL and h.value is None
     assert b"sm_100a" in L.wcsim_version()
+    # the no-allocation entry point refuses a grid beyond its built-in scratch before it touches the device
+    st = L.wcsim_raster_scatter_noalloc(1024, 1024, None, 1, 0, 0, 0, 3.0, ctypes.c_void_p(256), None)
+    assert st == binding.WCSIM_ETOOBIG and b"WCSIM_NOALLOC_MAX_BINS" in L.wcsim_strerror(st)
+    assert L.wcsim_raster_scatter_noalloc(64, 512, None, 1, 0, 0, 0, 3.0, None, None) == binding.WCSIM_EINVAL
 
 
 def test_binding_imports_nothing_from_the_oracle():
