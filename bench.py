@@ -332,7 +332,7 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel --------------------------------------------------------------------------
     peaks = load_peaks()
-    direct = args.impact > 1 or args.wires == "direct" or (args.wires == "auto" and pl["response"].shape[-2] <= (32 if pl["pad_w"] <= 512 else 45 if pl["pad_w"] <= 2048 else 100))
+    direct = plan.wire_mode() == B.WCSIM_WIRES_DIRECT  # the route the library resolved (wcsim_get_wire_mode), not a copy of its rule
     sb = stage_bytes(pl, direct, args.impact)
     stage_rows = []
     for name in ("raster", "rows_forward", "cols", "rows_inverse"):
@@ -524,11 +524,11 @@ def apa_events(args, B, cfg, fluct, mode, dev):
         for st in streams:
             st.wait_event(a)
         for _ in range(k):
-            for p, d in zip(plans, depos):
+            for p, d, pl in zip(plans, depos, planes):  # every plane with its own seeds (reading A26)
                 p.clear()
-                p.raster_scatter(d, seed=cfg["fluct_seed"], fluctuate=fluct)
+                p.raster_scatter(d, seed=pl["fluct_seed"], fluctuate=fluct)
                 if cfg.get("noise"):
-                    p.arm_noise(None, seed=cfg["noise_seed"])
+                    p.arm_noise(None, seed=pl["noise_seed"])
                 p.convolve()
         for st in streams:
             main.wait_stream(st)
@@ -556,11 +556,15 @@ def batched_events(args, B, cfg, planes, depos, fluct, mode, dev):
     plan = B.PlanesPlan([pl["n_wires"] for pl in planes], planes[0]["n_ticks"], [pl["response"] for pl in planes],
                         pad_ticks=planes[0]["pad_t"], nsigma=cfg["nsigma"], scatter_mode=bmode, stream=st)
 
+    # a seed per plane (reading A26); copies of one plane (--streams) get distinct seeds too
+    fluct_seeds = [pl["fluct_seed"] + 0x100000 * i for i, pl in enumerate(planes)]
+    noise_seeds = [pl["noise_seed"] + 0x100000 * i for i, pl in enumerate(planes)]
+
     def event():
         plan.clear()
-        plan.raster_scatter_planes(depos, seed=cfg["fluct_seed"], fluctuate=fluct)
+        plan.raster_scatter_planes(depos, seeds=fluct_seeds, fluctuate=fluct)
         if cfg.get("noise"):
-            plan.arm_noise(None, seed=cfg["noise_seed"])
+            plan.arm_noise_planes(None, seeds=noise_seeds)
         plan.convolve()
 
     def run(fn, k):

@@ -7,7 +7,7 @@
  * S is built from "ionization electron groups" (depos) by the Raster and Scatter-add tasks of
  * PAPER.md:54-58 (Section 2.2); the convolution follows the FFT route of PAPER.md:46-52 (Eq. 2);
  * N is the optional electronics-noise term of Eq. (1), model from BASELINE.json configs[3].
- * Where the paper is silent the readings A1..A25 of DESIGN.md apply; each call names the ones it uses.
+ * Where the paper is silent the readings A1..A26 of DESIGN.md apply; each call names the ones it uses.
  *
  * Conventions
  *   - Grids are wire-major, tick fastest: S[wire * n_ticks + tick], fp32.  Bin k covers [k, k+1) on both axes (A1).
@@ -140,7 +140,8 @@ int wcsim_convolve(wcsim_plan *plan);
 int wcsim_add_noise(wcsim_plan *plan, const float *amp, unsigned long long seed);
 int wcsim_arm_noise(wcsim_plan *plan, const float *amp, unsigned long long seed);
 
-/* Waits for the plan's stream, frees everything the plan owns.  NULL is accepted. */
+/* Waits for the plan's stream, frees everything the plan owns.  NULL is accepted.  WCSIM_ESTATE (nothing freed) while a
+ * wcsim_graph made from the plan has not been destroyed. */
 int wcsim_plan_destroy(wcsim_plan *plan);
 
 /* ---- accessories ---- */
@@ -149,6 +150,8 @@ int wcsim_clear_output(wcsim_plan *plan); /* M = 0 (enqueued) */
 int wcsim_sync(wcsim_plan *plan);        /* waits for the plan's stream; returns the first deferred CUDA fault */
 int wcsim_set_scatter_mode(wcsim_plan *plan, int scatter_mode);
 int wcsim_set_wire_mode(wcsim_plan *plan, int wire_mode);
+/* the route wcsim_convolve takes on this plan now: WCSIM_WIRES_DIRECT or WCSIM_WIRES_FFT (WCSIM_WIRES_AUTO resolved) */
+int wcsim_get_wire_mode(const wcsim_plan *plan, int *resolved);
 /* borrowed DEVICE pointers to n_wires*n_ticks floats, valid until wcsim_plan_destroy */
 int wcsim_charge_ptr(wcsim_plan *plan, float **dev);
 int wcsim_output_ptr(wcsim_plan *plan, float **dev);
@@ -222,7 +225,8 @@ int wcsim_simulate_host_adc_async(wcsim_plan *plan, const float *host_t0, const 
  *   n_wires   : HOST, n_planes ints;  responses : HOST, n_planes pointers to n_rwires x n_rticks floats each.
  *   pad_ticks : 0 = automatic.  The wire axis is always done directly (WCSIM_WIRES_DIRECT), so there is no wire padding.
  *   scatter_mode : WCSIM_SCATTER_ATOMIC or WCSIM_SCATTER_FIXED (the tiled mode is per plane: WCSIM_EINVAL).
- * wcsim_clear, wcsim_convolve, wcsim_arm_noise / wcsim_add_noise (the same spectrum and seed for every plane),
+ * wcsim_clear, wcsim_convolve, wcsim_arm_noise / wcsim_add_noise (the same spectrum and seed for every plane; see the
+ * *_planes variants below for a seed per plane),
  * wcsim_digitize, wcsim_charge_ptr / wcsim_output_ptr (the stacked grids) work on such a plan as on any other;
  * wcsim_raster_scatter and the *_host calls return WCSIM_ESTATE.
  */
@@ -234,6 +238,16 @@ int wcsim_plan_create_planes(wcsim_plan **out, int n_planes, const int *n_wires,
  * Works on single-plane plans too (n_planes = 1).  No per-depo totals.  Errors: WCSIM_ESTATE in tiled scatter mode. */
 int wcsim_raster_scatter_planes(wcsim_plan *plan, const wcsim_depos *depos, const long long *n, unsigned long long seed,
                                 int fluctuate);
+/* Independent planes (reading A26 of DESIGN.md; the simulation "treats each plane independently", PAPER.md:40
+ * for N(t,x)): with ONE seed, equal (depo id, bin) pairs of different planes draw from the same Philox word and wire x of
+ * every plane carries the same noise waveform -- fine for a test, wrong for physics.  These variants take one seed per
+ * plane, seeds: HOST, n_planes values; plane p is then exactly what a single-plane plan gives with seeds[p] (Philox key =
+ * seeds[p]; counters unchanged: depo id and the plane's own bin for the fluctuation, the plane's own wire for the noise).
+ * Everything else as wcsim_raster_scatter_planes / wcsim_arm_noise / wcsim_add_noise.  NULL seeds: WCSIM_EINVAL. */
+int wcsim_raster_scatter_planes_seeded(wcsim_plan *plan, const wcsim_depos *depos, const long long *n,
+                                       const unsigned long long *seeds, int fluctuate);
+int wcsim_arm_noise_planes(wcsim_plan *plan, const float *amp, const unsigned long long *seeds);
+int wcsim_add_noise_planes(wcsim_plan *plan, const float *amp, const unsigned long long *seeds);
 int wcsim_get_plane_rows(const wcsim_plan *plan, int plane, int *first_row, int *n_rows);
 
 /*
@@ -312,11 +326,26 @@ int wcsim_raster_scatter_noalloc(int n_wires, int n_ticks, const wcsim_depos *de
  * Not capturable (WCSIM_ESTATE while capturing): a first use of the fixed-point or tiled mode on the plan, or a tiled
  * call with more depos than any before (they allocate: run the call once outside the capture), custom noise spectra, anything that synchronises (wcsim_sync, wcsim_get_stats, the
  * *_host calls must not be called).  The plan's stream must not be the legacy default stream (WCSIM_ESTATE).
- * Stage timing is off inside a capture.  Destroy graphs before their plan.
+ * Stage timing is off inside a capture.  Destroy graphs before their plan: wcsim_plan_destroy returns WCSIM_ESTATE (and
+ * frees nothing) while a graph made from the plan is alive.
+ *
+ * What a replay repeats.  Everything passed BY VALUE to the recorded calls is frozen in the graph: the fluctuation seed,
+ * depo_id_base and the depo count n of wcsim_raster_scatter(_planes), the noise seed of wcsim_arm_noise / wcsim_add_noise,
+ * gain / baseline / bits of wcsim_digitize.  Only the CONTENTS of the recorded device arrays are read afresh.  So plain
+ * replays over new depos reuse the same Philox stream and the same noise realisation (Eq. (1)'s N(t,x),
+ * PAPER.md:40): consecutive events would be statistically correlated.  For independent events give every event its own
+ * seeds through wcsim_graph_update: wcsim_graph_begin, the same calls in the same order with the new seeds / counts /
+ * pointers, then wcsim_graph_update(plan, graph) instead of wcsim_graph_end.  It ends the capture and rewrites the
+ * parameters of the existing executable graph in place (no re-instantiation; launches of the old parameters that are
+ * already enqueued are not affected).  If the recorded sequence is not the one the graph was made from (another call
+ * order, another scatter mode, a tiled call, a different number of kernels) it returns WCSIM_ESTATE; the graph should then
+ * be destroyed and made anew.  With NULL arguments (WCSIM_EINVAL), or a graph of another plan or no capture in progress
+ * (WCSIM_ESTATE), the capture state is left as it was.
  */
 typedef struct wcsim_graph wcsim_graph;
 int wcsim_graph_begin(wcsim_plan *plan);
 int wcsim_graph_end(wcsim_plan *plan, wcsim_graph **out); /* *out = NULL on failure */
+int wcsim_graph_update(wcsim_plan *plan, wcsim_graph *graph);
 int wcsim_graph_launch(wcsim_graph *graph);
 int wcsim_graph_destroy(wcsim_graph *graph);
 

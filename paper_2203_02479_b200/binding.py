@@ -8,6 +8,7 @@ from __future__ import annotations
 
 import ctypes as C
 import os
+import weakref
 
 import numpy as np
 
@@ -29,6 +30,8 @@ SYMBOLS = [
     "wcsim_plan_create_planes", "wcsim_raster_scatter_planes", "wcsim_get_plane_rows", "wcsim_simulate_host_adc_async",
     "wcsim_plan_create_impact", "wcsim_get_charge_dims",
     "wcsim_raster_scatter_noalloc",
+    "wcsim_graph_update", "wcsim_get_wire_mode",
+    "wcsim_raster_scatter_planes_seeded", "wcsim_arm_noise_planes", "wcsim_add_noise_planes",
     "wcsim_graph_begin", "wcsim_graph_end", "wcsim_graph_launch", "wcsim_graph_destroy",
     "wcsim_strerror", "wcsim_last_cuda_error", "wcsim_version",
 ]
@@ -85,6 +88,7 @@ def lib():
         L.wcsim_set_scatter_mode.argtypes = [vp, i]
         L.wcsim_set_wire_mode.argtypes = [vp, i]
         L.wcsim_set_normalize.argtypes = [vp, i]
+        L.wcsim_get_wire_mode.argtypes = [vp, C.POINTER(i)]
         L.wcsim_charge_ptr.argtypes = [vp, C.POINTER(vp)]
         L.wcsim_output_ptr.argtypes = [vp, C.POINTER(vp)]
         L.wcsim_get_dims.argtypes = [vp] + [C.POINTER(i)] * 4
@@ -107,6 +111,9 @@ def lib():
                                   C.POINTER(wcsim_depos), vp]
         L.wcsim_plan_create_planes.argtypes = [C.POINTER(vp), i, C.POINTER(i), i, C.POINTER(vp), i, i, i, C.c_float, i, vp]
         L.wcsim_raster_scatter_planes.argtypes = [vp, C.POINTER(wcsim_depos), C.POINTER(ll), ull, i]
+        L.wcsim_raster_scatter_planes_seeded.argtypes = [vp, C.POINTER(wcsim_depos), C.POINTER(ll), C.POINTER(ull), i]
+        L.wcsim_arm_noise_planes.argtypes = [vp, vp, C.POINTER(ull)]
+        L.wcsim_add_noise_planes.argtypes = [vp, vp, C.POINTER(ull)]
         L.wcsim_get_plane_rows.argtypes = [vp, i, C.POINTER(i), C.POINTER(i)]
         L.wcsim_simulate_host_adc_async.argtypes = [vp, vp, vp, vp, vp, vp, ll, ull, i, i, ull, C.c_float, C.c_float, i, vp]
         L.wcsim_plan_create_impact.argtypes = [C.POINTER(vp), i, i, i, C.POINTER(vp), i, i, i, C.c_float, i, vp]
@@ -115,6 +122,7 @@ def lib():
         L.wcsim_graph_begin.argtypes = [vp]
         L.wcsim_graph_end.argtypes = [vp, C.POINTER(vp)]
         L.wcsim_graph_launch.argtypes = [vp]
+        L.wcsim_graph_update.argtypes = [vp, vp]
         L.wcsim_graph_destroy.argtypes = [vp]
         L.wcsim_strerror.argtypes = [i]
         L.wcsim_strerror.restype = C.c_char_p
@@ -275,6 +283,13 @@ def wcsim_set_wire_mode(plan, wire_mode):
     _check(lib().wcsim_set_wire_mode(plan, int(wire_mode)), "wcsim_set_wire_mode")
 
 
+def wcsim_get_wire_mode(plan):
+    """The wire-axis route wcsim_convolve takes on this plan now (WCSIM_WIRES_DIRECT or WCSIM_WIRES_FFT)."""
+    m = C.c_int()
+    _check(lib().wcsim_get_wire_mode(plan, C.byref(m)), "wcsim_get_wire_mode")
+    return m.value
+
+
 def wcsim_get_dims(plan):
     v = [C.c_int() for _ in range(4)]
     _check(lib().wcsim_get_dims(plan, *[C.byref(x) for x in v]), "wcsim_get_dims")
@@ -413,6 +428,47 @@ def wcsim_raster_scatter_planes(plan, depos, n=None, seed=0, fluctuate=False):
     _check(lib().wcsim_raster_scatter_planes(plan, ds, ns, int(seed), _fluct(fluctuate)), "wcsim_raster_scatter_planes")
 
 
+def wcsim_raster_scatter_planes_seeded(plan, depos, seeds, n=None, fluctuate=False):
+    """The same with one fluctuation seed per plane (reading A26): seeds[p] keys plane p's Philox draws."""
+    import torch
+    keys = ("t0", "x0", "sigma_t", "sigma_x", "q")
+    if len(seeds) != len(depos) or len(depos) != _n_planes(plan):
+        raise ValueError("one depo dict and one seed per plane of the plan")
+    if n is None:
+        n = [d["t0"].numel() for d in depos]
+    for d, cnt in zip(depos, n):
+        if any(d[k].numel() < cnt for k in keys):
+            raise ValueError("depo array shorter than n")
+    ds = (wcsim_depos * len(depos))(*[wcsim_depos(*[_dev_ptr(d[k], torch.float32) for k in keys]) for d in depos])
+    ns = (C.c_longlong * len(depos))(*[int(c) for c in n])
+    sd = (C.c_ulonglong * len(seeds))(*[int(x) for x in seeds])
+    _check(lib().wcsim_raster_scatter_planes_seeded(plan, ds, ns, sd, _fluct(fluctuate)), "wcsim_raster_scatter_planes_seeded")
+
+
+def _n_planes(plan) -> int:
+    a, b, n = C.c_int(), C.c_int(), 0
+    while lib().wcsim_get_plane_rows(plan, n, C.byref(a), C.byref(b)) == WCSIM_OK:
+        n += 1
+    return n
+
+
+def _plane_seeds(plan, seeds):
+    if len(seeds) != _n_planes(plan):
+        raise ValueError("one seed per plane of the plan")
+    return (C.c_ulonglong * len(seeds))(*[int(x) for x in seeds])
+
+
+def wcsim_arm_noise_planes(plan, amp=None, seeds=()):
+    """wcsim_arm_noise with one noise seed per plane of a multi-plane plan (reading A26)."""
+    keep, p = _amp_ptr(amp)
+    _check(lib().wcsim_arm_noise_planes(plan, p, _plane_seeds(plan, seeds)), "wcsim_arm_noise_planes")
+
+
+def wcsim_add_noise_planes(plan, amp=None, seeds=()):
+    keep, p = _amp_ptr(amp)
+    _check(lib().wcsim_add_noise_planes(plan, p, _plane_seeds(plan, seeds)), "wcsim_add_noise_planes")
+
+
 def wcsim_get_plane_rows(plan, plane):
     a, b = C.c_int(), C.c_int()
     _check(lib().wcsim_get_plane_rows(plan, int(plane), C.byref(a), C.byref(b)), "wcsim_get_plane_rows")
@@ -427,6 +483,10 @@ def wcsim_graph_end(plan):
     g = C.c_void_p()
     _check(lib().wcsim_graph_end(plan, C.byref(g)), "wcsim_graph_end")
     return g
+
+
+def wcsim_graph_update(plan, graph):
+    _check(lib().wcsim_graph_update(plan, graph), "wcsim_graph_update")
 
 
 def wcsim_graph_launch(graph):
@@ -552,6 +612,10 @@ class Plan:
 
     def destroy(self):
         if self.handle is not None:
+            for r in getattr(self, "_graphs", []):  # the library refuses to free a plan its graphs still point at
+                g = r()
+                if g is not None:
+                    g.destroy()
             h, self.handle = self.handle, None
             wcsim_plan_destroy(h)
 
@@ -587,6 +651,9 @@ class Plan:
 
     def set_normalize(self, on):
         wcsim_set_normalize(self.handle, on)
+
+    def wire_mode(self):
+        return wcsim_get_wire_mode(self.handle)
 
     def set_wire_mode(self, mode):
         wcsim_set_wire_mode(self.handle, mode)
@@ -631,8 +698,16 @@ class Plan:
     def response_spectrum(self):
         return wcsim_debug_response_spectrum(self.handle)
 
-    def raster_scatter_planes(self, depos, **kw):
+    def raster_scatter_planes(self, depos, seeds=None, **kw):
+        if seeds is not None:
+            return wcsim_raster_scatter_planes_seeded(self.handle, depos, seeds, **kw)
         wcsim_raster_scatter_planes(self.handle, depos, **kw)
+
+    def arm_noise_planes(self, amp=None, seeds=()):
+        wcsim_arm_noise_planes(self.handle, amp, seeds)
+
+    def add_noise_planes(self, amp=None, seeds=()):
+        wcsim_add_noise_planes(self.handle, amp, seeds)
 
     def plane_rows(self, plane):
         return wcsim_get_plane_rows(self.handle, plane)
@@ -641,7 +716,9 @@ class Plan:
         wcsim_graph_begin(self.handle)
 
     def graph_end(self):
-        return Graph(wcsim_graph_end(self.handle), self)
+        g = Graph(wcsim_graph_end(self.handle), self)
+        self._graphs = [r for r in getattr(self, "_graphs", []) if r() is not None] + [weakref.ref(g)]
+        return g
 
 
 class PlanesPlan(Plan):
@@ -670,6 +747,11 @@ class Graph:
 
     def launch(self):
         wcsim_graph_launch(self.handle)
+
+    def update(self):
+        """Ends a capture begun with plan.graph_begin() and rewrites this graph's parameters with the sequence just
+        recorded (new seeds, depo counts, pointers): see wcsim_graph_update in include/wcsim.h."""
+        wcsim_graph_update(self.plan.handle, self.handle)
 
     def destroy(self):
         if self.handle is not None:

@@ -263,9 +263,9 @@ __device__ __forceinline__ void noise_sincos(float x, float *s, float *c)
     *c = -__cosf(a);
 #endif
 }
-__device__ __forceinline__ float2 noise_bin(const NoiseArgs &nz, uint32_t wire, uint32_t k)
+__device__ __forceinline__ float2 noise_bin(const NoiseArgs &nz, uint64_t seed, uint32_t wire, uint32_t k)
 {
-    const uint4 words = noise_words(nz.seed, wire, k >> 2);
+    const uint4 words = noise_words(seed, wire, k >> 2);
     const uint32_t w = pick_word(words, k & 3u);
     float s, c;
     noise_sincos(noise_phase(w), &s, &c);
@@ -283,7 +283,9 @@ __global__ void __launch_bounds__(RowCfg<N, false>::threads, RowCfg<N, false>::m
     pdl_wait(); // a no-op unless launched as a programmatic dependent
     const float2 *src = b.spec_inv + (size_t)row * b.spec_stride;
     const bool noisy = nz.amp != nullptr;
-    const uint32_t wire = (uint32_t)(row - b.planes.row0[plane_of_row(b.planes, row)]); // the noise is keyed by the plane's own wire
+    const int noise_plane = plane_of_row(b.planes, row);
+    const uint32_t wire = (uint32_t)(row - b.planes.row0[noise_plane]); // the noise is keyed by the plane's own wire ...
+    const uint64_t noise_seed = nz.seed[noise_plane];                  // ... and the plane's own seed (A26)
     float2 v[E];
     float2 tws[E];
     split_twiddles<E>(tws, load_tw(b.tw_real, i)); // exp(-2 pi i k / 2N) at k = i + e NT: one load, 15 constant rotations
@@ -308,11 +310,11 @@ __global__ void __launch_bounds__(RowCfg<N, false>::threads, RowCfg<N, false>::m
         for (int e = 0; e < E; ++e) {
             const int k = i + e * NT;
             float2 x = use_spec ? src[k] : make_float2(0.f, 0.f);
-            if (noisy) x = cadd(x, noise_bin(nz, wire, (uint32_t)k));
+            if (noisy) x = cadd(x, noise_bin(nz, noise_seed, wire, (uint32_t)k));
             if (k == 0) {
                 x.y = 0.f; // the imaginary parts of the DC and Nyquist bins do not reach a real output
                 float2 xn = use_spec ? src[N] : make_float2(0.f, 0.f);
-                if (noisy) xn = cadd(xn, noise_bin(nz, wire, (uint32_t)N));
+                if (noisy) xn = cadd(xn, noise_bin(nz, noise_seed, wire, (uint32_t)N));
                 xn.y = 0.f;
                 smem[smem_index<1>(N, 0)] = xn;
             }
@@ -381,10 +383,12 @@ __global__ void __launch_bounds__(RowTma<N>::threads, RowTma<N>::min_ctas) rows_
         mbar_wait(bar, parity);
         parity ^= 1u;
         if (noisy) {
-            const uint32_t wire = (uint32_t)(row - b.planes.row0[plane_of_row(b.planes, row)]); // the plane's own wire
+            const int noise_plane = plane_of_row(b.planes, row);
+            const uint32_t wire = (uint32_t)(row - b.planes.row0[noise_plane]); // the plane's own wire and seed (A26)
+            const uint64_t noise_seed = nz.seed[noise_plane];
             // one Philox call gives the phases of four consecutive frequency bins (A17): a thread takes whole calls
             for (int q = i; q < N / 4; q += NT) {
-                const uint4 words = noise_words(nz.seed, wire, (uint32_t)q);
+                const uint4 words = noise_words(noise_seed, wire, (uint32_t)q);
                 const float4 a = __ldg(reinterpret_cast<const float4 *>(nz.amp) + q);
                 float4 *x = reinterpret_cast<float4 *>(stage + 4 * q);
                 float4 lo = x[0], hi = x[1];
@@ -395,7 +399,7 @@ __global__ void __launch_bounds__(RowTma<N>::threads, RowTma<N>::min_ctas) rows_
                 noise_sincos(noise_phase(words.w), &sn, &cs), hi.z = fmaf(a.w, cs, hi.z), hi.w = fmaf(a.w, sn, hi.w);
                 x[0] = lo, x[1] = hi;
             }
-            if (i == 0) stage[N] = cadd(stage[N], noise_bin(nz, wire, (uint32_t)N));
+            if (i == 0) stage[N] = cadd(stage[N], noise_bin(nz, noise_seed, wire, (uint32_t)N));
             __syncthreads();
         }
         // Z_k = (X_k + conj X_{N-k}) + i exp(+2 pi i k / 2N) (X_k - conj X_{N-k});  inverse FFT of Z = even + i odd

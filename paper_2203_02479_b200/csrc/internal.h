@@ -63,12 +63,13 @@ struct RasterPlanes {
     int n;
     DepoArrays d[kMaxPlanes];
     long long count[kMaxPlanes];
+    uint64_t seed[kMaxPlanes]; // Philox key of plane p's fluctuation draws (reading A26)
     long long batch0[kMaxPlanes + 1];
     int n_wires[kMaxPlanes];
     int row0[kMaxPlanes];
 };
 int raster_batch_depos(); // depos per batch (for batch0)
-cudaError_t launch_raster_planes(int n_ticks, const RasterPlanes &planes, uint64_t seed, int fluctuate, double nsigma,
+cudaError_t launch_raster_planes(int n_ticks, const RasterPlanes &planes, int fluctuate, double nsigma,
                                  void *grid, bool fixed, Counters *counters, int sm_count, cudaStream_t st);
 
 // a1-a3, tiled mode (deterministic): scratch buffers are owned by the plan and grown by the caller
@@ -118,8 +119,15 @@ struct ConvBuffers {
 };
 struct NoiseArgs {
     const float *amp; // DEVICE [pad_t/2 + 1], already scaled by pad_t^-1/2; NULL = no noise
-    uint64_t seed;
+    uint64_t seed[kMaxPlanes]; // Philox key of plane p's noise (reading A26); a single-seed call fills every entry alike
 };
+inline NoiseArgs noise_args(const float *amp, const uint64_t *seeds, int n_seeds)
+{
+    NoiseArgs nz{};
+    nz.amp = amp;
+    for (int p = 0; p < kMaxPlanes; ++p) nz.seed[p] = seeds[p < n_seeds ? p : n_seeds - 1];
+    return nz;
+}
 bool conv_sizes_supported(int pad_w, int pad_t);
 cudaError_t conv_configure(int pad_w, int pad_t); // sets the kernels' shared-memory attributes (once per plan)
 cudaError_t launch_rows_forward(GridDims g, int pad_t, ConvBuffers b, cudaStream_t st);

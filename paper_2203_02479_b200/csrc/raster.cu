@@ -878,7 +878,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8
 // ------------------------------------------------------------------------------------------------------------------
 template <int FLUCT, bool FIX>
 __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8)
-    raster_planes_kernel(int n_ticks, const __grid_constant__ RasterPlanes P, uint64_t seed, double nsigma,
+    raster_planes_kernel(int n_ticks, const __grid_constant__ RasterPlanes P, double nsigma,
                          float *__restrict__ S, Counters *counters, bool normalize, int n_static)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -912,7 +912,7 @@ __global__ void __launch_bounds__(kBatchWarps * 32, FLUCT ? WCSIM_FLUCT_CTAS : 8
         const GridDims g{P.n_wires[pl], n_ticks};
         const Clip clip{0, g.n_wires, 0, n_ticks, P.row0[pl]};
         if constexpr (FLUCT)
-            raster_quad_body<FLUCT == 2, false, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, 0ull, seed, nsigma,
+            raster_quad_body<FLUCT == 2, false, false>(g, clip, sink, t0, x0, st, sx, q, valid, first, 0u, 0ull, P.seed[pl], nsigma,
                                                        normalize, nullptr, sm.warp[wid], !more, drawn, lane);
         else if (more)
             raster_flat_body(g, clip, sink.shifted(clip.row_off), t0, x0, st, sx, q, valid, nsigma, normalize,
@@ -1201,11 +1201,18 @@ static cudaError_t launch_raster_batch(GridDims g, DepoArrays d, long long n, ui
     }
     long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
     if (ctas > max_ctas) ctas = max_ctas;
-    int max_per_sm = 0;
-    if (const char *e = getenv("WCSIM_SCHED")) sscanf(e, "%d,%d,%d,%d", &sched.x, &sched.y, &sched.z, &max_per_sm);
-    if (max_per_sm > 0 && ctas > (long long)sm_count * max_per_sm) ctas = (long long)sm_count * max_per_sm;
-    if (sched.x < 1 || sched.x > kBatchDepos) sched.x = kTailDepos;
-    if (sched.z < 1) sched.z = 1;
+#ifdef WCSIM_SCHED_ENV // experiment knob, off in the shipped library: WCSIM_SCHED="tail depos,tail batches per warp,chunk,CTAs per SM"
+    {
+        int4 e4 = sched;
+        int max_per_sm = 0;
+        const char *e = getenv("WCSIM_SCHED");
+        if (e && sscanf(e, "%d,%d,%d,%d", &e4.x, &e4.y, &e4.z, &max_per_sm) >= 3 && e4.x >= 1 && e4.x <= kBatchDepos &&
+            e4.y >= 0 && e4.z >= 1) {
+            sched = make_int4(e4.x, e4.y, e4.z, sched.w);
+            if (max_per_sm > 0 && ctas > (long long)sm_count * max_per_sm) ctas = (long long)sm_count * max_per_sm;
+        }
+    }
+#endif
     return launch_pdl(raster_batch_kernel<FLUCT, TOT, FIX>, (unsigned)ctas, kBatchWarps * 32, smem, st, g, d, n, id_base, seed,
                       nsigma, S, depo_totals, counters, normalize, sched);
 }
@@ -1243,7 +1250,7 @@ cudaError_t launch_raster_fixed(GridDims g, DepoArrays d, long long n, uint64_t 
 int raster_batch_depos() { return kBatchDepos; }
 
 template <int FLUCT, bool FIX>
-static cudaError_t launch_raster_planes_t(int n_ticks, const RasterPlanes &planes, uint64_t seed, double nsigma, float *grid,
+static cudaError_t launch_raster_planes_t(int n_ticks, const RasterPlanes &planes, double nsigma, float *grid,
                                           Counters *counters, int sm_count, cudaStream_t st, bool normalize)
 {
     const long long n_batches = planes.batch0[planes.n];
@@ -1255,18 +1262,18 @@ static cudaError_t launch_raster_planes_t(int n_ticks, const RasterPlanes &plane
     long long ctas = (n_batches + kBatchWarps - 1) / kBatchWarps;
     const long long max_ctas = (long long)sm_count * (ctas_per_sm > 0 ? ctas_per_sm : 1);
     if (ctas > max_ctas) ctas = max_ctas;
-    return launch_pdl(raster_planes_kernel<FLUCT, FIX>, (unsigned)ctas, kBatchWarps * 32, smem, st, n_ticks, planes, seed, nsigma,
+    return launch_pdl(raster_planes_kernel<FLUCT, FIX>, (unsigned)ctas, kBatchWarps * 32, smem, st, n_ticks, planes, nsigma,
                       grid, counters, normalize, 2);
 }
 
-cudaError_t launch_raster_planes(int n_ticks, const RasterPlanes &planes, uint64_t seed, int fluctuate, double nsigma,
+cudaError_t launch_raster_planes(int n_ticks, const RasterPlanes &planes, int fluctuate, double nsigma,
                                  void *grid, bool fixed, Counters *counters, int sm_count, cudaStream_t st)
 {
     const bool normalize = (fluctuate & kRasterNormalize) != 0;
     fluctuate &= ~kRasterNormalize;
     float *gp = reinterpret_cast<float *>(grid);
-#define WCSIM_PLANES(F) (fixed ? launch_raster_planes_t<F, true>(n_ticks, planes, seed, nsigma, gp, counters, sm_count, st, normalize) \
-                               : launch_raster_planes_t<F, false>(n_ticks, planes, seed, nsigma, gp, counters, sm_count, st, normalize))
+#define WCSIM_PLANES(F) (fixed ? launch_raster_planes_t<F, true>(n_ticks, planes, nsigma, gp, counters, sm_count, st, normalize) \
+                               : launch_raster_planes_t<F, false>(n_ticks, planes, nsigma, gp, counters, sm_count, st, normalize))
     if (!fluctuate) return WCSIM_PLANES(0);
     if (fluctuate == 2) return WCSIM_PLANES(2);
     return WCSIM_PLANES(1);

@@ -30,6 +30,7 @@ struct wcsim_plan {
     bool multi = false;     // created by wcsim_plan_create_planes
     bool capturing = false; // between wcsim_graph_begin and wcsim_graph_end
     unsigned long long captured_launches = 0;
+    int live_graphs = 0;    // wcsim_graph objects that point at this plan (wcsim_plan_destroy refuses while > 0)
     short *dev_adc = nullptr; // ADC codes of wcsim_simulate_host_adc_async (allocated on first use)
     PlaneTable pt{};        // n = 1 for an ordinary plan
     Counters *counters = nullptr;
@@ -37,7 +38,7 @@ struct wcsim_plan {
     float *amp_armed = nullptr; // the armed custom spectrum's own copy (a later wcsim_add_noise must not change it)
     bool noise_armed = false;
     const float *armed_amp = nullptr;
-    uint64_t armed_seed = 0;
+    uint64_t armed_seed[kMaxPlanes] = {}; // plane p's noise seed (A26); a single-seed arm fills every entry alike
     TileScratch ts{};
     float *stage_block = nullptr; // device staging of the five host depo arrays, 5 * stage_cap floats
     long long stage_cap = 0;
@@ -508,8 +509,9 @@ int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n
     if (plan->normalize) fluctuate |= kRasterNormalize; // internal.h: flag bit of the launchers' `fluctuate`
     StageSpan span(plan, WCSIM_STAGE_RASTER);
     if (plan->scatter_mode == WCSIM_SCATTER_TILED) {
-        plan->launches += 7;
-        return raster_tiled(plan, g, d, n, depo_id_base, seed, fluctuate, dev_depo_totals);
+        const int rc = raster_tiled(plan, g, d, n, depo_id_base, seed, fluctuate, dev_depo_totals);
+        if (rc == WCSIM_OK) plan->launches += 7;
+        return rc;
     }
     if (dev_depo_totals) CU_TRY(cudaMemsetAsync(dev_depo_totals, 0, sizeof(int) * (size_t)n, plan->stream));
     const bool fixed = plan->scatter_mode == WCSIM_SCATTER_FIXED;
@@ -541,8 +543,27 @@ int wcsim_raster_scatter(wcsim_plan *plan, const wcsim_depos *depos, long long n
     return WCSIM_OK;
 }
 
+namespace {
+int raster_scatter_planes_impl(wcsim_plan *plan, const wcsim_depos *depos, const long long *n,
+                               const unsigned long long *seeds, int n_seeds, int fluctuate);
+}
+
 int wcsim_raster_scatter_planes(wcsim_plan *plan, const wcsim_depos *depos, const long long *n, unsigned long long seed,
                                 int fluctuate)
+{
+    return raster_scatter_planes_impl(plan, depos, n, &seed, 1, fluctuate);
+}
+
+int wcsim_raster_scatter_planes_seeded(wcsim_plan *plan, const wcsim_depos *depos, const long long *n,
+                                       const unsigned long long *seeds, int fluctuate)
+{
+    if (!plan || !seeds) return WCSIM_EINVAL;
+    return raster_scatter_planes_impl(plan, depos, n, seeds, plan->pt.n, fluctuate);
+}
+
+namespace {
+int raster_scatter_planes_impl(wcsim_plan *plan, const wcsim_depos *depos, const long long *n,
+                               const unsigned long long *seeds, int n_seeds, int fluctuate)
 {
     if (!plan || !depos || !n || fluctuate < 0 || fluctuate > 2) return WCSIM_EINVAL;
     if (plan->scatter_mode == WCSIM_SCATTER_TILED) return WCSIM_ESTATE;
@@ -558,6 +579,7 @@ int wcsim_raster_scatter_planes(wcsim_plan *plan, const wcsim_depos *depos, cons
             return WCSIM_EINVAL;
         rp.d[p] = DepoArrays{depos[p].t0, depos[p].x0, depos[p].sigma_t, depos[p].sigma_x, depos[p].q};
         rp.count[p] = n[p];
+        rp.seed[p] = seeds[p < n_seeds ? p : n_seeds - 1];
         rp.batch0[p] = batches;
         batches += (n[p] + per_batch - 1) / per_batch;
         rp.n_wires[p] = plan->impact_K > 1 ? plan->s_wires : plan->pt.row0[p + 1] - plan->pt.row0[p];
@@ -575,7 +597,7 @@ int wcsim_raster_scatter_planes(wcsim_plan *plan, const wcsim_depos *depos, cons
         CU_TRY(cudaMemsetAsync(plan->ts.fix, 0, bytes, plan->stream));
     }
     plan->launches += 1;
-    CU_TRY(launch_raster_planes(plan->n_ticks, rp, seed, fluctuate, plan->nsigma,
+    CU_TRY(launch_raster_planes(plan->n_ticks, rp, fluctuate, plan->nsigma,
                                 fixed ? (void *)plan->ts.fix : (void *)plan->S, fixed, plan->counters, plan->sm_count,
                                 plan->stream));
     if (fixed) {
@@ -584,6 +606,7 @@ int wcsim_raster_scatter_planes(wcsim_plan *plan, const wcsim_depos *depos, cons
     }
     return WCSIM_OK;
 }
+} // namespace
 
 int wcsim_get_plane_rows(const wcsim_plan *plan, int plane, int *first_row, int *n_rows)
 {
@@ -600,10 +623,9 @@ int wcsim_convolve(wcsim_plan *plan)
     if (!guard.ok) return fail_cuda(cudaGetLastError());
     const GridDims g{plan->n_wires, plan->n_ticks};
     const ConvBuffers b = conv_buffers(plan);
-    NoiseArgs nz{nullptr, 0};
+    NoiseArgs nz{};
     if (plan->noise_armed) {
-        nz.amp = plan->armed_amp;
-        nz.seed = plan->armed_seed;
+        nz = noise_args(plan->armed_amp, plan->armed_seed, kMaxPlanes);
         plan->noise_armed = false;
     }
     const bool per_kernel = plan->profiling == WCSIM_PROFILE_KERNELS;
@@ -638,15 +660,18 @@ static int noise_amp_ptr(wcsim_plan *plan, const float *amp, const float **dev)
     return rc;
 }
 
-int wcsim_add_noise(wcsim_plan *plan, const float *amp, unsigned long long seed)
+namespace {
+int add_noise_impl(wcsim_plan *plan, const float *amp, const unsigned long long *seeds, int n_seeds)
 {
     if (!plan) return WCSIM_EINVAL;
     DeviceGuard guard(plan->device);
     if (!guard.ok) return fail_cuda(cudaGetLastError());
     if (amp && plan->capturing) return WCSIM_ESTATE; // the upload synchronises
-    NoiseArgs nz{nullptr, seed};
-    const int rc = noise_amp_ptr(plan, amp, &nz.amp);
+    const float *dev_amp = nullptr;
+    const int rc = noise_amp_ptr(plan, amp, &dev_amp);
     if (rc) return rc;
+    static_assert(sizeof(unsigned long long) == sizeof(uint64_t), "seed width");
+    const NoiseArgs nz = noise_args(dev_amp, reinterpret_cast<const uint64_t *>(seeds), n_seeds);
     const GridDims g{plan->n_wires, plan->n_ticks};
     StageSpan span(plan, WCSIM_STAGE_NOISE);
     CU_TRY(launch_rows_inverse(g, plan->pad_t, conv_buffers(plan), nz, false, true, plan->stream));
@@ -654,7 +679,7 @@ int wcsim_add_noise(wcsim_plan *plan, const float *amp, unsigned long long seed)
     return WCSIM_OK;
 }
 
-int wcsim_arm_noise(wcsim_plan *plan, const float *amp, unsigned long long seed)
+int arm_noise_impl(wcsim_plan *plan, const float *amp, const unsigned long long *seeds, int n_seeds)
 {
     if (!plan) return WCSIM_EINVAL;
     DeviceGuard guard(plan->device);
@@ -667,14 +692,29 @@ int wcsim_arm_noise(wcsim_plan *plan, const float *amp, unsigned long long seed)
         dev = plan->amp_armed;
     }
     plan->armed_amp = dev;
-    plan->armed_seed = seed;
+    for (int p = 0; p < kMaxPlanes; ++p) plan->armed_seed[p] = seeds[p < n_seeds ? p : n_seeds - 1];
     plan->noise_armed = true;
     return WCSIM_OK;
+}
+} // namespace
+
+int wcsim_add_noise(wcsim_plan *plan, const float *amp, unsigned long long seed) { return add_noise_impl(plan, amp, &seed, 1); }
+int wcsim_arm_noise(wcsim_plan *plan, const float *amp, unsigned long long seed) { return arm_noise_impl(plan, amp, &seed, 1); }
+int wcsim_add_noise_planes(wcsim_plan *plan, const float *amp, const unsigned long long *seeds)
+{
+    if (!plan || !seeds) return WCSIM_EINVAL;
+    return add_noise_impl(plan, amp, seeds, plan->pt.n);
+}
+int wcsim_arm_noise_planes(wcsim_plan *plan, const float *amp, const unsigned long long *seeds)
+{
+    if (!plan || !seeds) return WCSIM_EINVAL;
+    return arm_noise_impl(plan, amp, seeds, plan->pt.n);
 }
 
 int wcsim_plan_destroy(wcsim_plan *plan)
 {
     if (!plan) return WCSIM_OK;
+    if (plan->live_graphs > 0) return WCSIM_ESTATE; // its graphs hold a pointer to it: destroy them first
     DeviceGuard guard(plan->device);
     return destroy_impl(plan);
 }
@@ -708,6 +748,13 @@ int wcsim_set_scatter_mode(wcsim_plan *plan, int scatter_mode)
 {
     if (!plan || scatter_mode < WCSIM_SCATTER_ATOMIC || scatter_mode > WCSIM_SCATTER_FIXED) return WCSIM_EINVAL;
     plan->scatter_mode = scatter_mode;
+    return WCSIM_OK;
+}
+
+int wcsim_get_wire_mode(const wcsim_plan *plan, int *resolved)
+{
+    if (!plan || !resolved) return WCSIM_EINVAL;
+    *resolved = wires_direct(plan) ? WCSIM_WIRES_DIRECT : WCSIM_WIRES_FFT;
     return WCSIM_OK;
 }
 
@@ -899,7 +946,35 @@ int wcsim_graph_end(wcsim_plan *plan, wcsim_graph **out)
         cudaGraphDestroy(g);
         return WCSIM_ENOMEM;
     }
+    plan->live_graphs += 1;
     *out = gr;
+    return WCSIM_OK;
+}
+
+int wcsim_graph_update(wcsim_plan *plan, wcsim_graph *graph)
+{
+    if (!plan || !graph) return WCSIM_EINVAL;
+    if (!plan->capturing || graph->plan != plan) return WCSIM_ESTATE;
+    DeviceGuard guard(plan->device);
+    plan->capturing = false;
+    const unsigned long long inside = plan->launches - plan->captured_launches;
+    plan->launches = plan->captured_launches; // nothing ran yet
+    cudaGraph_t g = nullptr;
+    CU_TRY(cudaStreamEndCapture(plan->stream, &g));
+    if (!g) return WCSIM_ECUDA;
+    cudaGraphExecUpdateResultInfo info{};
+    const cudaError_t e = cudaGraphExecUpdate(graph->exec, g, &info);
+    if (e != cudaSuccess) {
+        cudaGraphDestroy(g);
+        if (e == cudaErrorGraphExecUpdateFailure) { // not the same sequence of calls as the one the graph was made from
+            cudaGetLastError();
+            return WCSIM_ESTATE;
+        }
+        return fail_cuda(e);
+    }
+    cudaGraphDestroy(graph->graph);
+    graph->graph = g;
+    graph->launches = inside;
     return WCSIM_OK;
 }
 
@@ -921,6 +996,7 @@ int wcsim_graph_destroy(wcsim_graph *graph)
     cudaStreamSynchronize(graph->plan->stream);
     cudaGraphExecDestroy(graph->exec);
     cudaGraphDestroy(graph->graph);
+    graph->plan->live_graphs -= 1;
     delete graph;
     return WCSIM_OK;
 }

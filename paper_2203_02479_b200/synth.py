@@ -99,6 +99,14 @@ def depos_tracks(n, n_wires, n_ticks, line_frac, n_seg, td_max_ms, gen_seed=1, p
     return _pack(t0, x0, st, sx, q)
 
 
+def _with_plane_seeds(cfg: dict) -> dict:
+    """Every plane dict carries fluct_seed and noise_seed (the event's own where the plane names none)."""
+    for pl in cfg["planes"]:
+        pl.setdefault("fluct_seed", cfg["fluct_seed"])
+        pl.setdefault("noise_seed", cfg["noise_seed"])
+    return cfg
+
+
 def config(i: int, *, n_depos: int | None = None, shuffle: bool = False, sigma_scale: float = 1.0) -> dict:
     """The workload of BASELINE.json configs[i] as a dict:
     planes: list of dict(n_wires, n_ticks, pad_w, pad_t, response, depos); fluctuate, noise, seeds, nsigma.
@@ -108,27 +116,30 @@ def config(i: int, *, n_depos: int | None = None, shuffle: bool = False, sigma_s
         n = n_depos or 100
         planes = [dict(n_wires=64, n_ticks=512, pad_w=128, pad_t=1024, response=response(),
                        depos=depos_uniform_box(n))]
-        return {**base, "name": "configs[0] tiny 64x512, 100 depos", "fluctuate": False, "planes": planes}
+        return _with_plane_seeds({**base, "name": "configs[0] tiny 64x512, 100 depos", "fluctuate": False, "planes": planes})
     if i in (1, 2):
         n = n_depos or (100_000 if i == 1 else 1_000_000)
         frac, nseg, td = (0.9, 50, 2.25) if i == 1 else (0.8, 500, 4.5)
         nseg = max(1, min(nseg, n // 200))
         planes = [dict(n_wires=800, n_ticks=6000, pad_w=1024, pad_t=8192, response=response(),
                        depos=depos_tracks(n, 800, 6000, frac, nseg, td, shuffle=shuffle, sigma_scale=sigma_scale))]
-        return {**base, "name": "configs[%d] 800x6000, %d depos" % (i, n), "fluctuate": True, "planes": planes}
+        return _with_plane_seeds({**base, "name": "configs[%d] 800x6000, %d depos" % (i, n), "fluctuate": True, "planes": planes})
     if i == 3:
         n = n_depos or 200_000
         planes = []
         for p, nw in enumerate((800, 800, 960)):
             nseg = max(1, min(100, n // 200))
+            # every plane has its own fluctuation and noise seed (reading A26: the planes of an anode are independent,
+            # PAPER.md:30, so wire x of U, V and W must not carry the same noise waveform); plane 0 keeps the event's
             planes.append(dict(n_wires=nw, n_ticks=6000, pad_w=1024, pad_t=8192, response=response(unipolar=(p == 2)),
-                               depos=depos_tracks(n, nw, 6000, 0.9, nseg, 2.25, plane=p, shuffle=shuffle)))
-        return {**base, "name": "configs[3] APA 3 planes x %d depos + noise" % n, "fluctuate": True, "noise": True,
-                "planes": planes}
+                               depos=depos_tracks(n, nw, 6000, 0.9, nseg, 2.25, plane=p, shuffle=shuffle),
+                               fluct_seed=base["fluct_seed"] + 0x1000 * p, noise_seed=base["noise_seed"] + 0x1000 * p))
+        return _with_plane_seeds({**base, "name": "configs[3] APA 3 planes x %d depos + noise" % n, "fluctuate": True,
+                                  "noise": True, "planes": planes})
     if i == 4:
         n = n_depos or 10_000_000
         nseg = max(1, min(5000, n // 200))
         planes = [dict(n_wires=2560, n_ticks=9600, pad_w=4096, pad_t=16384, response=response(41, 400),
                        depos=depos_tracks(n, 2560, 9600, 0.7, nseg, 4.5, shuffle=shuffle))]
-        return {**base, "name": "configs[4] 2560x9600, %d depos" % n, "fluctuate": True, "planes": planes}
+        return _with_plane_seeds({**base, "name": "configs[4] 2560x9600, %d depos" % n, "fluctuate": True, "planes": planes})
     raise ValueError("config index must be 0..4")

@@ -105,9 +105,9 @@ def run_plane(B, pl, cfg, *, fluctuate, mode=0, want_totals=False, noise=False, 
     n = pl["depos"]["t0"].shape[0]
     totals = torch.zeros(n, dtype=torch.int32, device="cuda") if want_totals else None
     plan.clear()
-    plan.raster_scatter(d, seed=cfg["fluct_seed"], fluctuate=fluctuate, dev_depo_totals=totals)
+    plan.raster_scatter(d, seed=pl["fluct_seed"], fluctuate=fluctuate, dev_depo_totals=totals)
     if noise:
-        plan.arm_noise(None, seed=cfg["noise_seed"])
+        plan.arm_noise(None, seed=pl["noise_seed"])
     if convolve:
         plan.convolve()
     plan.sync()
@@ -127,7 +127,7 @@ def test_config_1_2_full(B, O, idx):
     cfg = synth.config(idx)
     pl = cfg["planes"][0]
     nw, nt, R = pl["n_wires"], pl["n_ticks"], pl["response"]
-    S_ref, tot_ref, st = O.raster_scatter(nw, nt, pl["depos"], seed=cfg["fluct_seed"], fluctuate=True,
+    S_ref, tot_ref, st = O.raster_scatter(nw, nt, pl["depos"], seed=pl["fluct_seed"], fluctuate=True,
                                           nsigma=cfg["nsigma"], want_totals=True)
     assert float(np.max(np.abs(S_ref))) < 2 ** 24  # fp32 adds of integers stay exact (reading A9)
     S, M, tot, stats = run_plane(B, pl, cfg, fluctuate=True, want_totals=True)
@@ -156,7 +156,7 @@ def test_config_3_full(B, O):
     assert cfg["noise"] and len(cfg["planes"]) == 3
     for p, pl in enumerate(cfg["planes"]):
         nw, nt, R = pl["n_wires"], pl["n_ticks"], pl["response"]
-        S_ref, _, st = O.raster_scatter(nw, nt, pl["depos"], seed=cfg["fluct_seed"], fluctuate=True, nsigma=cfg["nsigma"])
+        S_ref, _, st = O.raster_scatter(nw, nt, pl["depos"], seed=pl["fluct_seed"], fluctuate=True, nsigma=cfg["nsigma"])
         S, M, _, _ = run_plane(B, pl, cfg, fluctuate=True)
         flipped = int(np.count_nonzero(S.astype(np.float64) != S_ref))
         record("configs[3] plane %d S" % p, flipped_bins=flipped, drawn_bins=int(st["drawn"]))
@@ -166,12 +166,12 @@ def test_config_3_full(B, O):
         check_points(O, S_ref, R, M, np.random.default_rng(30 + p), 2000, "configs[3] plane %d points" % p)
         # signal + noise in one pass (noise rides the inverse row transform): M' = M + N within M's tolerance
         _, Mn, _, _ = run_plane(B, pl, cfg, fluctuate=True, noise=True)
-        N_ref = O.noise_add(np.zeros((nw, nt)), pl["pad_t"], cfg["noise_seed"])
+        N_ref = O.noise_add(np.zeros((nw, nt)), pl["pad_t"], pl["noise_seed"])
         check_M(Mn, M_ref + N_ref, "configs[3] plane %d M + N" % p)
         # noise on its own (S = 0 => M = N): it is invisible against 1e-4 max|M| otherwise
         plan = B.Plan(nw, nt, R, pad=(pl["pad_w"], pl["pad_t"]))
         plan.clear()
-        plan.arm_noise(None, seed=cfg["noise_seed"])
+        plan.arm_noise(None, seed=pl["noise_seed"])
         plan.convolve()
         plan.sync()
         N = plan.output().cpu().numpy().astype(np.float64)
@@ -217,7 +217,7 @@ def test_config_4_windows_both_modes(B, O):
         w1, k1 = w0 + WW, k0 + WT
         idx = _reach(pl["depos"], cfg["nsigma"], w0, w1, k0, k1)
         sub = {k: v[idx] for k, v in pl["depos"].items()}
-        S_ref, _, st = O.raster_scatter(nw, nt, sub, seed=cfg["fluct_seed"], fluctuate=True, nsigma=cfg["nsigma"],
+        S_ref, _, st = O.raster_scatter(nw, nt, sub, seed=pl["fluct_seed"], fluctuate=True, nsigma=cfg["nsigma"],
                                         ids=idx.astype(np.uint64), window=(w0, w1, k0, k1))
         drawn += st["drawn"]
         flipped += int(np.count_nonzero(S64[w0:w1, k0:k1] != S_ref))
@@ -245,7 +245,7 @@ def test_config_4_whole_plane(B, O):
     cfg = synth.config(4)
     pl = cfg["planes"][0]
     nw, nt, R = pl["n_wires"], pl["n_ticks"], pl["response"]
-    S_ref, tot_ref, st = O.raster_scatter(nw, nt, pl["depos"], seed=cfg["fluct_seed"], fluctuate=True,
+    S_ref, tot_ref, st = O.raster_scatter(nw, nt, pl["depos"], seed=pl["fluct_seed"], fluctuate=True,
                                           nsigma=cfg["nsigma"], want_totals=True)
     assert float(np.max(np.abs(S_ref))) < 2 ** 24  # fp32 adds of integers stay exact (reading A9)
     M = None

@@ -118,8 +118,10 @@ def test_config_3_event_through_one_launch_sequence(B, O):
                       pad_ticks=planes[0]["pad_t"], nsigma=cfg["nsigma"]) as plan:
         dev = [to_dev(pl["depos"]) for pl in planes]
         plan.clear()
-        plan.raster_scatter_planes(dev, seed=cfg["fluct_seed"], fluctuate=True)
-        plan.arm_noise(None, seed=cfg["noise_seed"])
+        fluct_seeds, noise_seeds = [pl["fluct_seed"] for pl in planes], [pl["noise_seed"] for pl in planes]
+        assert len(set(noise_seeds)) == 3 and len(set(fluct_seeds)) == 3  # reading A26: a seed per plane
+        plan.raster_scatter_planes(dev, seeds=fluct_seeds, fluctuate=True)
+        plan.arm_noise_planes(None, seeds=noise_seeds)
         plan.convolve()
         plan.sync()
         S = plan.charge().cpu().numpy()
@@ -127,13 +129,40 @@ def test_config_3_event_through_one_launch_sequence(B, O):
         assert plan.launch_count() == 5  # clear, raster, forward rows, wire pass, inverse rows: one launch each for three planes
         for p, pl in enumerate(planes):
             r0, nw = plan.plane_rows(p)
-            S_ref, _, st = O.raster_scatter(nw, nt, pl["depos"], seed=cfg["fluct_seed"], fluctuate=True, nsigma=cfg["nsigma"])
+            S_ref, _, st = O.raster_scatter(nw, nt, pl["depos"], seed=pl["fluct_seed"], fluctuate=True, nsigma=cfg["nsigma"])
             flipped = int(np.count_nonzero(S[r0:r0 + nw].astype(np.float64) != S_ref))
             record("configs[3] batched plane %d S" % p, flipped_bins=flipped, drawn_bins=int(st["drawn"]))
             assert flipped <= FLIP_BUDGET * st["drawn"]
             M_ref = O.convolve_fft(S_ref, pl["response"], pl["pad_w"], pl["pad_t"])
-            M_ref += O.noise_add(np.zeros((nw, nt)), pl["pad_t"], cfg["noise_seed"])
+            M_ref += O.noise_add(np.zeros((nw, nt)), pl["pad_t"], pl["noise_seed"])
             check_close(M[r0:r0 + nw], M_ref, "configs[3] batched plane %d M + N" % p)
+        # noise alone through the same plan (S = 0 => M = N): plane p equals a single-plane run with plane p's seed, and
+        # wire 5 of plane 0 and wire 5 of plane 1 carry different waveforms
+        plan.clear()
+        plan.arm_noise_planes(None, seeds=noise_seeds)
+        plan.convolve()
+        plan.sync()
+        N = plan.output().cpu().numpy().astype(np.float64)
+        rows = [plan.plane_rows(p) for p in range(3)]
+        for p, pl in enumerate(planes):
+            r0, nw = rows[p]
+            check_close(N[r0:r0 + nw], O.noise_add(np.zeros((nw, nt)), pl["pad_t"], pl["noise_seed"]),
+                        "configs[3] batched plane %d noise alone" % p)
+        assert not np.allclose(N[rows[0][0] + 5], N[rows[1][0] + 5], atol=1e-3)
+        # one seed for all planes (wcsim_arm_noise on a multi-plane plan) still means what it says: identical waveforms
+        plan.clear()
+        plan.arm_noise(None, seed=noise_seeds[1])
+        plan.convolve()
+        plan.sync()
+        N1 = plan.output().cpu().numpy().astype(np.float64)
+        assert np.array_equal(N1[rows[0][0] + 5], N1[rows[1][0] + 5])
+        assert np.array_equal(N1[rows[1][0]:rows[1][0] + rows[1][1]], N[rows[1][0]:rows[1][0] + rows[1][1]])
+        # the stand-alone pass takes per-plane seeds too: M += N on top of the armed result gives 2 N for plane 1
+        plan.add_noise_planes(None, seeds=noise_seeds)
+        plan.sync()
+        N2 = plan.output().cpu().numpy().astype(np.float64)
+        r0, nw = rows[1]
+        check_close(N2[r0:r0 + nw], 2.0 * N[r0:r0 + nw], "configs[3] batched add_noise_planes")
 
 
 def test_graph_replays_a_plane_event(B, O):
@@ -221,6 +250,74 @@ def test_graph_replays_a_plane_event(B, O):
     with B.Plan(nw, nt, R, stream=0) as p0:
         with pytest.raises(B.WcsimError):
             p0.graph_begin()
+
+
+def test_graph_update_gives_each_event_its_own_seeds(B, O):
+    """A plain replay repeats the recorded seeds, depo count and id base (they are kernel arguments frozen in the graph), so
+    consecutive events would share one Philox stream and one noise realisation.  wcsim_graph_update re-records the sequence
+    with the new event's values into the existing executable graph; each replay then equals the oracle with ITS seeds."""
+    from paper_2203_02479_b200 import synth
+    cfg = synth.config(0)
+    pl = cfg["planes"][0]
+    nw, nt, R = pl["n_wires"], pl["n_ticks"], pl["response"]
+    events = [dict(depos=synth.depos_uniform_box(100, gen_seed=21), n=100, seed=3, noise_seed=4, id_base=0),
+              dict(depos=synth.depos_uniform_box(100, gen_seed=22), n=100, seed=0xABCDEF0123, noise_seed=99, id_base=1 << 33),
+              dict(depos=synth.depos_uniform_box(100, gen_seed=23), n=61, seed=5, noise_seed=6, id_base=7)]  # fewer depos too
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        dev = to_dev(events[0]["depos"])
+    stream.synchronize()
+    plan = B.Plan(nw, nt, R, pad=(pl["pad_w"], pl["pad_t"]), stream=stream)
+    try:
+        def sequence(ev):
+            plan.clear()
+            plan.raster_scatter(dev, n=ev["n"], seed=ev["seed"], depo_id_base=ev["id_base"], fluctuate=True)
+            plan.arm_noise(None, seed=ev["noise_seed"])
+            plan.convolve()
+
+        graph = None
+        noise_of_wire5 = []
+        for ev in events:
+            with torch.cuda.stream(stream):
+                for k in dev:
+                    dev[k].copy_(torch.from_numpy(ev["depos"][k]))
+            plan.graph_begin()
+            sequence(ev)
+            if graph is None:
+                graph = plan.graph_end()
+            else:
+                graph.update()
+            plan.clear_output()
+            graph.launch()
+            plan.sync()
+            d = {k: v[: ev["n"]] for k, v in ev["depos"].items()}
+            S_ref, _, st = O.raster_scatter(nw, nt, d, seed=ev["seed"], id_base=ev["id_base"], fluctuate=True)
+            S = plan.charge().cpu().numpy().astype(np.float64)
+            assert int(np.count_nonzero(S != S_ref)) <= FLIP_BUDGET * st["drawn"]
+            N_ref = O.noise_add(np.zeros((nw, nt)), pl["pad_t"], ev["noise_seed"])
+            check_close(plan.output().cpu().numpy(), O.convolve_direct(S_ref, R) + N_ref, "graph update M + N")
+            noise_of_wire5.append(N_ref[5].copy())
+        assert not np.allclose(noise_of_wire5[0], noise_of_wire5[1])
+        # without the update the old values come back: a replay over event 0's depos still uses event 2's seed, count and ids
+        with torch.cuda.stream(stream):
+            for k in dev:
+                dev[k].copy_(torch.from_numpy(events[0]["depos"][k]))
+        graph.launch()
+        plan.sync()
+        ev = events[2]
+        d = {k: v[: ev["n"]] for k, v in events[0]["depos"].items()}
+        S_ref, _, st = O.raster_scatter(nw, nt, d, seed=ev["seed"], id_base=ev["id_base"], fluctuate=True)
+        assert int(np.count_nonzero(plan.charge().cpu().numpy().astype(np.float64) != S_ref)) <= FLIP_BUDGET * st["drawn"]
+        # a different sequence is refused and the capture is closed; a plan with a live graph is not freed from under it
+        plan.graph_begin()
+        plan.clear()
+        with pytest.raises(B.WcsimError) as e:
+            graph.update()
+        assert e.value.status == B.WCSIM_ESTATE
+        assert B.lib().wcsim_plan_destroy(plan.handle) == B.WCSIM_ESTATE
+        graph.destroy()
+    finally:
+        plan.destroy()
 
 
 def test_planes_plan_graph(B, O):
