@@ -362,6 +362,11 @@ def run_ours(args):
     # wire-axis pass never reads) is the labelled secondary figure.
     c_ms, c_calls = stages_calls["convolve"]
     convolve = hbm_fracs(c_ms / max(c_calls, 1))
+    # compulsory floor: S read once, Rhat read once, M written once -- no intermediate spectrum traffic
+    floor_bytes = 2 * pl["n_wires"] * pl["n_ticks"] * 4 + pl["pad_w"] * (pl["pad_t"] // 2 + 1) * 8
+    floor_ms = floor_bytes / (peaks["hbm_gbs"] * 1e9) * 1e3
+    convolve.update({"compulsory_floor": {"bytes": floor_bytes, "ms_at_peak": floor_ms, "frac": floor_ms / convolve["ms"],
+                                          "what": "read S + read Rhat + write M at the measured copy bandwidth, over the measured time"}})
     convolve.update({"bytes": conv_bytes, "survey_pass_model_bytes": pass_model,
                      "how": "one CUDA-event pair around wcsim_convolve in the back-to-back plane-event",
                      "frac_of_8TBs_nominal": convolve["achieved"] / 8000.0,
@@ -427,6 +432,7 @@ def run_ours(args):
                                 "d2h_bytes_per_step": d2h // 2,
                                 "what": "wcsim_simulate_host_adc_async: 12-bit ADC codes (int16) come back instead of fp32 M"}},
         "gpu_launches": launches,
+        "build": build_identity(B),
         "roofline": roofline,
         "ms_per_step_median": statistics.median(per_step),
         "ms_per_step_min": min(per_step),
@@ -443,7 +449,7 @@ def run_ours(args):
         out["apa_event"] = apa
     if rank == 0 and world == 1 and not args.no_cpu_baseline and args.impact == 1:
         out["cpu_baseline"] = cpu_baseline(cfg, budget_s=args.cpu_budget)
-    if rank == 0 and world == 1 and args.cufft:
+    if rank == 0 and world == 1 and not args.no_cufft:
         out["cufft_comparator"] = cufft_comparator(pl, dev, flush)
     plan.destroy()
     replicas.shutdown()
@@ -460,6 +466,17 @@ WARP_INST_PER_BIN = 16.8
 FP64_FLOP_PER_BIN = 70.0
 # the e2e ADC variant's ideal converter (reading A23): codes per unit of M, and pedestal
 ADC_GAIN, ADC_BASELINE = 0.01, 900.0
+
+
+def build_identity(B):
+    """Which libwcsim.so was timed: its version string and a hash of the file, so that the constants typed in above from one
+    ncu capture (TRAFFIC, WARP_INST_PER_BIN) can be matched against the build named in the header of profiles/r03_*.md."""
+    import hashlib
+    from paper_2203_02479_b200 import build as _b
+    with open(_b.LIB, "rb") as f:
+        digest = hashlib.sha256(f.read()).hexdigest()
+    return {"version": B.wcsim_version(), "libwcsim_sha256_16": digest[:16],
+            "ncu_constants_from": "profiles/r02_ncu_full.md (round-2 build; the raster kernels are unchanged since)"}
 
 
 def survey_pass_model_bytes(pl):
@@ -762,7 +779,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=200)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cufft", action="store_true", help="also time the cuFFT comparator")
+    ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT comparator (8 iterations of torch.fft on the padded sizes)")
+    ap.add_argument("--cufft", action="store_true", help=argparse.SUPPRESS)  # old spelling: the comparator now runs by default
     ap.add_argument("--ref-max-steps", type=int, default=20)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
